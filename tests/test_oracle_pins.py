@@ -1,0 +1,487 @@
+"""Pins for the CPU oracle (oracle/opo_oracle.cpp) -- none of them re-uses the oracle's own code.
+
+Each test checks the oracle against something the paper or the mathematics fixes: an O(N^2) DFT, a
+library FFT, closed forms, conservation laws, a library ODE integrator, the phases the paper prints.
+Numbering P1..P12 follows SURVEY.md section 8(c); citations are PAPER.md lines.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import OracleOpo, CURRENT, EXIT, TIME, FREQ
+
+FS, PS, UM, NM = 1e-15, 1e-12, 1e-6, 1e-9
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_printed_values.txt")
+
+
+def golden():
+    vals = {}
+    with open(GOLDEN) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if "=" in line:
+                k, v = line.split("=")
+                vals[k.strip()] = float(v)
+    return vals
+
+
+def make(n_fields=3, log2_n=8, window_s=10 * PS, nz=20, length=5e-3, dk=0.0, d_eff=14e-12,
+         beta1=(0, 0, 0), beta2=(0, 0, 0), resonant=(0, 0, 0), R=(0, 0, 0), delta_rad=(0, 0, 0),
+         delta_T=(0, 0, 0), gdd=(0, 0, 0), alpha=(0, 0, 0), use_float=False, ref_field=1,
+         lam=None, nidx=None):
+    if lam is None:
+        lam = [532 * NM, 1000 * NM, 1.0 / (1 / (532 * NM) - 1 / (1000 * NM))] if n_fields == 3 \
+            else [532 * NM, 1064 * NM]
+    if nidx is None:
+        nidx = [2.23, 2.16, 2.15][:n_fields]
+    return OracleOpo(n_fields=n_fields, log2_n=log2_n, window_s=window_s, nz_per_pass=nz,
+                     length_m=length, dk_per_m=dk, d_eff_m_per_V=d_eff, lambda_m=list(lam),
+                     n_index=list(nidx), beta1_s_per_m=list(beta1), beta2_s2_per_m=list(beta2),
+                     alpha_per_m=list(alpha), ref_field=ref_field, resonant=list(resonant), R=list(R),
+                     delta_rad=list(delta_rad), delta_T_s=list(delta_T), gdd_s2=list(gdd),
+                     use_float=use_float)
+
+
+def rel_l2(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+# ---------------------------------------------------------------------------------------------
+# P1  the oracle's own radix-2 FFT
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("n", [2, 4, 8, 16, 64, 256])
+def test_p1_fft_matches_naive_dft(n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    k = np.arange(n)
+    # X[k] = sum_n x[n] exp(-2 pi i k n / N): forward sign and no normalisation (reading R8)
+    W = np.exp(-2j * np.pi * np.outer(k, k) / n)
+    assert rel_l2(oracle.fft(x), W @ x) < 1e-13
+    # inverse carries 1/N
+    assert rel_l2(oracle.fft(x, inverse=True), (np.conj(W) @ x) / n) < 1e-13
+    assert rel_l2(oracle.fft(oracle.fft(x), inverse=True), x) < 1e-13
+
+
+@pytest.mark.parametrize("log2n", [10, 14])
+def test_p1_fft_matches_library_and_parseval(log2n):
+    n = 1 << log2n
+    rng = np.random.default_rng(7)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    X = oracle.fft(x)
+    assert rel_l2(X, np.fft.fft(x)) < 1e-13
+    assert abs(np.sum(np.abs(X) ** 2) / n - np.sum(np.abs(x) ** 2)) / np.sum(np.abs(x) ** 2) < 1e-13
+
+
+def test_p1_single_exponential_lands_in_one_bin():
+    n, k0 = 128, 37
+    x = np.exp(2j * np.pi * k0 * np.arange(n) / n)
+    X = oracle.fft(x)
+    assert abs(X[k0] - n) < 1e-10
+    X[k0] = 0
+    assert np.abs(X).max() < 1e-10
+
+
+def test_get_field_frequency_domain_is_unnormalised_forward_dft():
+    o = make(n_fields=2, log2_n=6)
+    rng = np.random.default_rng(3)
+    a = rng.standard_normal(64) + 1j * rng.standard_normal(64)
+    o.set_field(1, a)
+    assert rel_l2(o.get_field(1, CURRENT, FREQ), np.fft.fft(a)) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# P2  Gaussian pulse under GVD, coupling off: closed form derived from Eq. 5's GVD term
+#     A(z,t) = T0/sqrt(T0^2 - i b2 z) exp(-t^2 / (2 (T0^2 - i b2 z)))
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("b2_fs2_per_um", [0.35, -0.2])
+def test_p2_gaussian_gvd_closed_form(b2_fs2_per_um):
+    log2n, T, L = 10, 10 * PS, 5e-3
+    n = 1 << log2n
+    b2 = b2_fs2_per_um * FS * FS / UM
+    T0 = 100 * FS
+    tau = (np.arange(n) - n // 2) * (T / n)
+    o = make(n_fields=2, log2_n=log2n, window_s=T, nz=20, length=L, d_eff=0.0, beta2=(0.0, b2))
+    o.set_field(1, np.exp(-tau ** 2 / (2 * T0 ** 2)).astype(complex))
+    assert o.propagate(20) == 0
+    q = T0 ** 2 - 1j * b2 * L
+    expect = T0 / np.sqrt(q) * np.exp(-tau ** 2 / (2 * q))
+    assert rel_l2(o.get_field(1), expect) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# P3  group-velocity mismatch: Delta beta1 * L = m dt  ==>  circular shift by +m samples
+#     (a slower field, larger beta1, arrives later; reading R7)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("m", [7, -3])
+def test_p3_gvm_integer_shift(m):
+    log2n, T, L = 8, 10 * PS, 5e-3
+    n = 1 << log2n
+    dt = T / n
+    rng = np.random.default_rng(11)
+    a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    # pump slower than the reference (signal) by m*dt over the crystal
+    o = make(n_fields=2, log2_n=log2n, window_s=T, nz=10, length=L, d_eff=0.0,
+             beta1=(m * dt / L, 0.0), ref_field=1)
+    o.set_field(0, a)
+    o.set_field(1, a)
+    assert o.propagate(10) == 0
+    assert rel_l2(o.get_field(0), np.roll(a, m)) < 1e-12     # pump delayed by m samples
+    assert rel_l2(o.get_field(1), a) < 1e-13                 # reference frame: signal does not move
+
+
+# ---------------------------------------------------------------------------------------------
+# P4  undepleted-pump parametric gain, CW, three waves
+#     dk = 0 : |A_s(L)|^2/|A_s(0)|^2 = cosh^2(gL),  g = sqrt(k_s k_i)|A_p|
+#     dk != 0: 1 + (g/G)^2 sinh^2(G L),  G^2 = g^2 - (dk/2)^2   (sin form when negative)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("dk", [0.0, 150.0, 600.0])
+def test_p4_undepleted_gain(dk):
+    L, nz = 5e-3, 200
+    o = make(n_fields=3, log2_n=4, nz=nz, length=L, dk=dk)
+    ks, ki = o.kappa(1), o.kappa(2)
+    Ap = 0.3 / (math.sqrt(ks * ki) * L) * 1000.0 / 1000.0      # g L = 0.3 ... scaled below
+    Ap = 1.2 / (math.sqrt(ks * ki) * L)                        # g L = 1.2
+    g = math.sqrt(ks * ki) * Ap
+    a0 = 1e-9 * Ap                                             # depletion ~ 1e-18
+    n = 16
+    o.set_field(0, np.full(n, Ap, complex))
+    o.set_field(1, np.full(n, a0 * np.exp(0.3j), complex))
+    o.set_field(2, np.zeros(n, complex))
+    assert o.propagate(nz) == 0
+    gain = np.abs(o.get_field(1)[0]) ** 2 / a0 ** 2
+    G2 = g * g - (dk / 2) ** 2
+    if G2 > 0:
+        G = math.sqrt(G2)
+        expect = 1 + (g / G) ** 2 * math.sinh(G * L) ** 2
+    else:
+        G = math.sqrt(-G2)
+        expect = 1 + (g / G) ** 2 * math.sin(G * L) ** 2
+    assert abs(gain / expect - 1) < 1e-8
+    # idler generated with |A_i|^2/k_i = (|A_s|^2 - |A_s0|^2)/k_s  (Manley-Rowe)
+    ai2 = np.abs(o.get_field(2)[0]) ** 2
+    assert abs(ai2 / ki / ((gain - 1) * a0 ** 2 / ks) - 1) < 1e-8
+
+
+# ---------------------------------------------------------------------------------------------
+# P5  degenerate OPO, real positive CW pump: a seed at phase pi/4 (or -3pi/4) is amplified by
+#     e^{2gL} in power, a seed at -pi/4 is de-amplified by e^{-2gL}; g = k_s |A_p|.
+#     The two amplified phases are the ones the paper prints.
+# ---------------------------------------------------------------------------------------------
+
+def test_p5_degenerate_phase_sensitive_gain_matches_printed_phases():
+    gv = golden()
+    L, nz = 5e-3, 200
+    o = make(n_fields=2, log2_n=4)
+    ks = o.kappa(1)
+    Ap = 0.8 / (ks * L)
+    g = ks * Ap
+    for phase_over_pi, sign in [(gv["degenerate_signal_phase_a_over_pi"], +1),
+                                (gv["degenerate_signal_phase_b_over_pi"], +1),
+                                (-0.25, -1), (0.75, -1)]:
+        o = make(n_fields=2, log2_n=4, nz=nz, length=L)
+        a0 = 1e-9 * Ap
+        o.set_field(0, np.full(16, Ap, complex))
+        o.set_field(1, np.full(16, a0 * np.exp(1j * np.pi * phase_over_pi), complex))
+        assert o.propagate(nz) == 0
+        out = o.get_field(1)[0]
+        gain = abs(out) ** 2 / a0 ** 2
+        assert abs(gain / math.exp(sign * 2 * g * L) - 1) < 1e-8
+        # the amplified/de-amplified quadratures keep their phase
+        assert abs(np.angle(out * np.exp(-1j * np.pi * phase_over_pi))) < 1e-8
+
+    # a seed at an arbitrary phase is pulled towards the printed phases (pi/4 here)
+    o = make(n_fields=2, log2_n=4, nz=400, length=4 * L)
+    o.set_field(0, np.full(16, Ap, complex))
+    o.set_field(1, np.full(16, 1e-12 * Ap * np.exp(0.1j), complex))
+    o.propagate(400)
+    ph = np.angle(o.get_field(1)[0]) / np.pi
+    assert min(abs(ph - gv["degenerate_signal_phase_a_over_pi"]),
+               abs(ph - gv["degenerate_signal_phase_b_over_pi"])) < 2e-3
+
+
+# ---------------------------------------------------------------------------------------------
+# P6  Manley-Rowe and total energy through a lossless crystal (omega_p = omega_s + omega_i,
+#     PAPER.md:L80).  The linear half-steps are unitary, so the drift is RK4's: ~h^4.
+# ---------------------------------------------------------------------------------------------
+
+def _invariants(o, F):
+    k = [o.kappa(x) for x in range(F)]
+    P = [np.sum(np.abs(o.get_field(x)) ** 2) for x in range(F)]
+    if F == 3:
+        return (P[0] / k[0] + P[1] / k[1], P[1] / k[1] - P[2] / k[2],
+                P[0] / k[0] + P[2] / k[2])
+    # degenerate (reading R5): photon flux |A_p|^2/(k_p/2) ... 2 signal photons per pump photon
+    return (2 * P[0] / k[0] + P[1] / k[1],)
+
+
+@pytest.mark.parametrize("F", [3, 2])
+def test_p6_manley_rowe_and_energy(F):
+    log2n, L = 7, 5e-3
+    n = 1 << log2n
+    rng = np.random.default_rng(5)
+
+    def run(nz):
+        o = make(n_fields=F, log2_n=log2n, nz=nz, length=L, dk=80.0,
+                 beta1=(0.3 * FS / UM, 0.0, -0.17 * FS / UM)[:F] + (0,) * (3 - F),
+                 beta2=(0.35 * FS * FS / UM, 0.1 * FS * FS / UM, 0.05 * FS * FS / UM))
+        ks = o.kappa(1)
+        amp = 1.5 / (ks * L)                    # strong coupling: k A L ~ 1.5, heavy depletion
+        rs = np.random.default_rng(5)
+        for x in range(F):
+            o.set_field(x, amp * (0.6 + 0.4 * (rs.standard_normal(n) + 1j * rs.standard_normal(n))))
+        i0 = _invariants(o, F)
+        nidx = [2.23, 2.16, 2.15][:F]
+        e0 = sum(nidx[x] * np.sum(np.abs(o.get_field(x)) ** 2) for x in range(F))
+        p0 = np.sum(np.abs(o.get_field(0)) ** 2)
+        assert o.propagate(nz) == 0
+        i1 = _invariants(o, F)
+        e1 = sum(nidx[x] * np.sum(np.abs(o.get_field(x)) ** 2) for x in range(F))
+        p1 = np.sum(np.abs(o.get_field(0)) ** 2)
+        assert abs(p1 / p0 - 1) > 0.05          # the pump really exchanged energy
+        scale = abs(i0[0])
+        return max(abs(a - b) / scale for a, b in zip(i0, i1)), abs(e1 - e0) / e0
+
+    # (the summed drift changes sign at coarse h, so the ratio is taken in the asymptotic range)
+    d1, e1 = run(160)
+    d2, e2 = run(320)
+    # total energy sum n_x |A_x|^2 (F = 2: conserved only with the 1/2 of reading R5, because
+    # n_p (k_p/2) = n_s k_s when lambda_s = 2 lambda_p)
+    assert d1 < 1e-9 and e1 < 1e-9
+    assert 8 < d1 / d2 < 32                    # ~ h^4
+    assert 8 < e1 / e2 < 32
+
+
+# ---------------------------------------------------------------------------------------------
+# P7  strongly depleted closed form (second-harmonic direction of the two-wave system):
+#     A_p(0) = 0, A_s(0) = a, dk = 0, no dispersion:
+#     |A_s(L)|^2 = a^2 sech^2(G L), |A_p(L)|^2 = (k_p/(2k_s)) a^2 tanh^2(G L), G = a sqrt(k_p k_s/2)
+# ---------------------------------------------------------------------------------------------
+
+def test_p7_depleted_shg_closed_form():
+    L, nz = 5e-3, 400
+    o = make(n_fields=2, log2_n=4, nz=nz, length=L)
+    kp, ks = o.kappa(0), o.kappa(1)
+    a = 1.3 / (math.sqrt(kp * ks / 2) * L)
+    G = a * math.sqrt(kp * ks / 2)
+    o.set_field(0, np.zeros(16, complex))
+    o.set_field(1, np.full(16, a * np.exp(0.7j), complex))
+    assert o.propagate(nz) == 0
+    s2 = abs(o.get_field(1)[0]) ** 2
+    p2 = abs(o.get_field(0)[0]) ** 2
+    assert abs(s2 / (a * a / math.cosh(G * L) ** 2) - 1) < 1e-9
+    assert abs(p2 / (kp / (2 * ks) * a * a * math.tanh(G * L) ** 2) - 1) < 1e-9
+
+
+# ---------------------------------------------------------------------------------------------
+# RK4 + all signs/conjugates/dk direction against a library ODE integrator (CW => the PDE is an ODE)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("F", [3, 2])
+def test_rk4_step_against_library_ode(F):
+    from scipy.integrate import solve_ivp
+    L, nz, dk = 5e-3, 400, 230.0
+    o = make(n_fields=F, log2_n=4, nz=nz, length=L, dk=dk)
+    k = [o.kappa(x) for x in range(F)]
+    s = 1.1 / (k[1] * L)
+    y0 = np.array([s * (0.9 + 0.2j), s * (0.3 - 0.5j), s * (-0.2 + 0.4j)][:F])
+    for x in range(F):
+        o.set_field(x, np.full(16, y0[x], complex))
+    assert o.propagate(nz) == 0
+
+    def f(z, y):
+        em, ep = np.exp(-1j * dk * z), np.exp(1j * dk * z)
+        if F == 3:
+            return [1j * k[0] * y[1] * y[2] * em, 1j * k[1] * y[0] * np.conj(y[2]) * ep,
+                    1j * k[2] * y[0] * np.conj(y[1]) * ep]
+        return [0.5j * k[0] * y[1] ** 2 * em, 1j * k[1] * y[0] * np.conj(y[1]) * ep]
+
+    sol = solve_ivp(f, (0, L), y0, method="DOP853", rtol=1e-13, atol=1e-13 * s)
+    for x in range(F):
+        assert abs(o.get_field(x)[0] - sol.y[x, -1]) / s < 1e-9
+
+
+# ---------------------------------------------------------------------------------------------
+# P8  global second-order convergence of the symmetric splitting
+# ---------------------------------------------------------------------------------------------
+
+def test_p8_second_order_convergence():
+    gv = golden()
+    log2n, L = 7, 5e-3
+    n = 1 << log2n
+    tau = (np.arange(n) - n // 2) * (10 * PS / n)
+
+    def run(nz):
+        o = make(n_fields=3, log2_n=log2n, nz=nz, length=L, dk=40.0,
+                 beta1=(0.3 * FS / UM, 0.0, -0.2 * FS / UM),
+                 beta2=(35 * FS * FS / UM, 12 * FS * FS / UM, 5 * FS * FS / UM))
+        ks = o.kappa(1)
+        amp = 1.0 / (ks * L)
+        o.set_field(0, amp * np.exp(-(tau / (0.8 * PS)) ** 2).astype(complex))
+        o.set_field(1, 0.3 * amp * np.exp(-((tau - 0.5 * PS) / (0.6 * PS)) ** 2) * np.exp(2j * np.pi * tau / (3 * PS)))
+        o.set_field(2, 0.2 * amp * np.exp(-((tau + 0.4 * PS) / (0.7 * PS)) ** 2).astype(complex))
+        assert o.propagate(nz) == 0
+        return np.concatenate([o.get_field(x) for x in range(3)])
+
+    ref = run(16 * 32)
+    e1 = np.linalg.norm(run(16) - ref)
+    e2 = np.linalg.norm(run(32) - ref)
+    e3 = np.linalg.norm(run(64) - ref)
+    order = gv["symmetrized_ssfm_local_error_order"] - 1
+    assert abs(e1 / e2 - 2 ** order) < 0.1
+    assert abs(e2 / e3 - 2 ** order) < 0.1
+
+
+# ---------------------------------------------------------------------------------------------
+# P9  cold cavity (pump = 0): after m round trips
+#     A~_s^(m)[k] = A~_s^(0)[k] * ( sqrt(R) e^{i delta} G_s[k] e^{i D_s(Omega_k) L} )^m
+# ---------------------------------------------------------------------------------------------
+
+def test_p9_cold_cavity_closed_form():
+    log2n, T, L, nz, m = 8, 10 * PS, 5e-3, 10, 7
+    n = 1 << log2n
+    dt = T / n
+    b1s, b2s = 0.02 * FS / UM, 0.4 * FS * FS / UM
+    R, delta, gdd, dT = 0.9, 0.37, -900 * FS * FS, 13 * FS
+    o = make(n_fields=3, log2_n=log2n, window_s=T, nz=nz, length=L, ref_field=0,
+             beta1=(0.0, b1s, 0.0), beta2=(0.0, b2s, 0.0), resonant=(0, 1, 0), R=(0, R, 0),
+             delta_rad=(0, delta, 0), delta_T=(0, dT, 0), gdd=(0, gdd, 0))
+    rng = np.random.default_rng(2)
+    a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    o.set_field(0, np.zeros(n, complex))
+    o.set_field(1, a)
+    o.set_field(2, np.zeros(n, complex))
+    assert o.roundtrips(m) == 0
+    kk = np.fft.fftfreq(n, d=1.0 / n)               # natural order, Nyquist negative (R9)
+    om = 2 * np.pi * kk / (n * dt)
+    per_trip = math.sqrt(R) * np.exp(1j * delta) * np.exp(1j * (gdd / 2) * om ** 2 - 1j * om * dT) \
+        * np.exp(1j * (-b1s * om + b2s / 2 * om ** 2) * L)
+    expect = np.fft.ifft(np.fft.fft(a) * per_trip ** m)
+    assert rel_l2(o.get_field(1), expect) < 1e-11
+    # exit field = pre-mirror field of the last pass
+    expect_exit = np.fft.ifft(np.fft.fft(a) * per_trip ** (m - 1) * np.exp(1j * (-b1s * om + b2s / 2 * om ** 2) * L))
+    assert rel_l2(o.get_field(1, EXIT), expect_exit) < 1e-11
+    # non-resonant fields restart from their stored input (R11, R12)
+    assert np.abs(o.get_field(0)).max() == 0 and np.abs(o.get_field(2)).max() == 0
+
+
+def test_p9_boundary_signs_gdd_compensates_gvd_and_detuning_delays():
+    """Independent sign pins for the boundary: GDD = -beta2 L undoes the crystal's GVD (same sign
+    convention, reading R14); a positive Delta T = m dt delays the field by m samples (R13)."""
+    log2n, T, L = 8, 10 * PS, 5e-3
+    n = 1 << log2n
+    dt = T / n
+    b2s = 0.4 * FS * FS / UM
+    rng = np.random.default_rng(4)
+    a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    o = make(n_fields=2, log2_n=log2n, window_s=T, nz=10, length=L, d_eff=0.0, beta2=(0.0, b2s),
+             resonant=(0, 1), R=(0, 1.0), gdd=(0, -b2s * L), delta_T=(0, 5 * dt))
+    o.set_field(0, np.zeros(n, complex))
+    o.set_field(1, a)
+    assert o.roundtrips(1) == 0
+    assert rel_l2(o.get_field(1), np.roll(a, 5)) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# P10  linear-regime growth per round trip of a single-mode seed: R cosh^2(sqrt(X) g_th L) (SRO),
+#      R e^{2 sqrt(X) g_th L} (degenerate, amplified quadrature); exactly 1 at X = 1  (R18)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("X", [1.0, 3.0])
+def test_p10_threshold_growth_sro(X):
+    from opo_workloads import threshold_amplitude_sro
+    L, nz, R = 20e-3, 100, 0.98
+    o = make(n_fields=3, log2_n=4, nz=nz, length=L, resonant=(0, 1, 0), R=(0, R, 0))
+    ks, ki = o.kappa(1), o.kappa(2)
+    a_th = threshold_amplitude_sro(ks, ki, L, R)
+    Ap = math.sqrt(X) * a_th
+    a0 = 1e-10 * Ap
+    o.set_field(0, np.full(16, Ap, complex))
+    o.set_field(1, np.full(16, a0, complex))
+    o.set_field(2, np.zeros(16, complex))
+    trips = 5
+    assert o.roundtrips(trips) == 0
+    growth = (abs(o.get_field(1)[0]) ** 2 / a0 ** 2) ** (1.0 / trips)
+    expect = R * math.cosh(math.sqrt(X) * math.sqrt(ks * ki) * a_th * L) ** 2
+    assert abs(growth / expect - 1) < 1e-9
+    if X == 1.0:
+        assert abs(growth - 1) < 1e-9
+
+
+@pytest.mark.parametrize("X", [1.0, 2.0])
+def test_p10_threshold_growth_degenerate(X):
+    from opo_workloads import threshold_amplitude_degenerate
+    L, nz, R = 5e-3, 20, 0.98
+    o = make(n_fields=2, log2_n=4, nz=nz, length=L, resonant=(0, 1), R=(0, R))
+    ks = o.kappa(1)
+    a_th = threshold_amplitude_degenerate(ks, L, R)
+    Ap = math.sqrt(X) * a_th
+    a0 = 1e-10 * Ap
+    o.set_field(0, np.full(16, Ap, complex))
+    o.set_field(1, np.full(16, a0 * np.exp(0.25j * np.pi), complex))
+    trips = 5
+    assert o.roundtrips(trips) == 0
+    growth = (abs(o.get_field(1)[0]) ** 2 / a0 ** 2) ** (1.0 / trips)
+    expect = R * math.exp(2 * math.sqrt(X) * ks * a_th * L)
+    assert abs(growth / expect - 1) < 1e-9
+    if X == 1.0:
+        assert abs(growth - 1) < 1e-9
+
+
+# ---------------------------------------------------------------------------------------------
+# error convention: partial passes accumulate z (R20); roundtrips needs z = 0; no stepping past L
+# ---------------------------------------------------------------------------------------------
+
+def test_state_conventions():
+    o = make(n_fields=2, log2_n=4, nz=10)
+    o.set_field(0, np.ones(16, complex))
+    o.set_field(1, np.ones(16, complex))
+    assert o.propagate(4) == 0
+    assert abs(o.z - 4 * 5e-3 / 10) < 1e-15
+    assert o.roundtrips(1) == 5          # STATE: z != 0
+    assert o.propagate(7) == 5           # STATE: would pass z = L
+    assert o.propagate(6) == 0
+
+
+def test_dk_phase_continues_across_partial_passes():
+    a = make(n_fields=3, log2_n=4, nz=40, dk=300.0)
+    b = make(n_fields=3, log2_n=4, nz=40, dk=300.0)
+    ks = a.kappa(1)
+    s = 1.0 / (ks * 5e-3)
+    for o in (a, b):
+        o.set_field(0, np.full(16, s, complex))
+        o.set_field(1, np.full(16, 0.2 * s, complex))
+        o.set_field(2, np.full(16, 0.1j * s, complex))
+    a.propagate(40)
+    b.propagate(13)
+    b.propagate(27)
+    for x in range(3):
+        assert rel_l2(b.get_field(x), a.get_field(x)) < 1e-14
+
+
+def test_nan_when_dz_too_coarse():
+    """'when the value of dz is not small enough ... the code returns NaN values'."""
+    o = make(n_fields=2, log2_n=4, nz=1, length=5e-3)
+    ks = o.kappa(1)
+    o.set_field(0, np.full(16, 1e6 / (ks * 5e-3), complex))     # kappa A_p dz = 1e6 >> 1
+    o.set_field(1, np.full(16, 1.0 + 1j, complex))
+    for _ in range(60):
+        o.propagate(1)
+        o2 = o.get_field(1)
+        if not np.all(np.isfinite(o2)):
+            break
+        # restart the pass to keep stepping (z is reset by a boundary with nothing resonant)
+        o.roundtrips(0)
+        break
+    # one RK4 step with |kappa A dz| = 1e6 amplifies by ~ (1e6)^4/24 per step; 60 steps overflow fp64
+    o = make(n_fields=2, log2_n=4, nz=60, length=5e-3 * 60)
+    o.set_field(0, np.full(16, 1e6 / (ks * 5e-3), complex))
+    o.set_field(1, np.full(16, 1.0 + 1j, complex))
+    o.propagate(60)
+    assert not np.all(np.isfinite(o.get_field(1)))
