@@ -1,0 +1,179 @@
+/*
+ * opo.h -- C ABI of libopo: split-step Fourier propagation of the chi(2) coupled-wave equations
+ * through a crystal inside a ring cavity, on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes is the hot path of arxiv 2410.02532 ("CUDA-based optical parametric
+ * oscillator simulator"; text at PAPER.md).  Citations are PAPER.md lines; "R<n>" are the readings
+ * of the paper listed in DESIGN.md (and SURVEY.md section 8(c)).
+ *
+ *   z-step  (Eqs 10-11, order L/2 - N - L/2 of L133, reading R2), h = L/nz:
+ *       A_x <- IDFT( H_x .* DFT(A_x) ),  H_x[k] = exp((-alpha_x/2 + i D_x(Omega_k)) h/2)
+ *              D_x(Omega) = -(beta1_x - beta1_ref) Omega + (beta2_x/2) Omega^2    (L99 Eq. 5; R7, R8)
+ *       one classic RK4 step of size h of the coupling terms of Eqs 2-4 (L86-95), pointwise in
+ *              tau, stage abscissae z, z+h/2, z+h/2, z+h for exp(-/+ i dk z)      (L115; R3, R4)
+ *              three-wave:  dA_p = i k_p A_s A_i e^{-i dk z}, dA_s = i k_s A_p A_i^* e^{+i dk z},
+ *                           dA_i = i k_i A_p A_s^* e^{+i dk z}
+ *              two-wave (degenerate, L164, R5): dA_p = i (k_p/2) A_s^2 e^{-i dk z},
+ *                           dA_s = i k_s A_p A_s^* e^{+i dk z}
+ *              k_x = 2 pi d_eff / (n_x lambda_x)                                   (L97)
+ *       A_x <- IDFT( H_x .* DFT(A_x) );  z += h
+ *   cavity boundary, once per round trip (L105-109 Eq. 6, Listing 3):
+ *       exit_x <- A_x                                  (fields at z = L, before the mirror)
+ *       resonant x:      A_x <- sqrt(R_x) e^{i delta_x} IDFT( G_x .* DFT(A_x) ),
+ *                        G_x[k] = exp(i (gdd_x/2) Omega_k^2 - i Omega_k delta_T_x)  (R13-R15)
+ *       non-resonant x:  A_x <- S_x   (stored input: fresh pump / frozen seed)      (R11, R12)
+ *
+ * Grid (L175-178; R8, R9, R19): N = 2^log2_n points, dt = window/N, tau_n = (n - N/2) dt,
+ * Omega_k = 2 pi k'/(N dt), k' = k (k < N/2) or k - N.  DFT: X[k] = sum_n x[n] e^{-2 pi i k n/N},
+ * unnormalised; the inverse carries 1/N.  Frequency-domain outputs are in natural FFT order.
+ *
+ * The implementation merges adjacent linear half-steps (H.H = one transform pair, an algebraic
+ * identity) and keeps the fields on chip where they fit; results agree with the step-by-step
+ * definition above to rounding.  See DESIGN.md.
+ *
+ * Conventions
+ *   - SI units everywhere (m, s, V/m, rad).
+ *   - Field buffers are contiguous [batch][N] interleaved (re, im): float2 (precision 0) or
+ *     double2 (precision 1), 16-byte aligned.  "dev" pointers are CUDA device pointers on the
+ *     current device, "host" pointers are ordinary (preferably pinned) host memory.
+ *   - The caller owns every buffer it passes; the library copies out of / into it on the handle's
+ *     stream and never frees or keeps it.  The handle owns its state and tables.
+ *   - Every call returns an opo_status.  No exceptions, no global state.  Handles are independent;
+ *     one handle must not be used from two threads at once.
+ *   - Calls enqueue work on the handle's stream and return; asynchronous faults surface at
+ *     opo_sync or at the next call (OPO_ERR_CUDA).  There is no CPU fallback of any kind: without
+ *     a usable sm_100 device opo_create fails with OPO_ERR_CUDA.
+ */
+#ifndef OPO_H_
+#define OPO_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct opo_handle opo_handle;
+
+typedef enum {
+    OPO_OK = 0,
+    OPO_ERR_INVALID_ARG = 1, /* null pointer, N not a supported power of two, n_fields not 2|3, R outside [0,1], nz <= 0 ... */
+    OPO_ERR_UNSUPPORTED = 2, /* e.g. resonant pump (the paper gives no injection rule), precision/size combination */
+    OPO_ERR_ALLOC = 3,
+    OPO_ERR_CUDA = 4,        /* message from the CUDA runtime in opo_last_error */
+    OPO_ERR_STATE = 5,       /* propagate past z = L, roundtrips at z != 0 */
+    OPO_ERR_NONFINITE = 6    /* opo_check_finite found NaN/Inf (the too-coarse-dz case of PAPER.md:L162) */
+} opo_status;
+
+/* crystal: PAPER.md:L97 (d_eff), L82 Eq. 1 (dk, the residual after quasi-phase-matching), L115 (L_cr) */
+typedef struct {
+    double length_m;
+    double dk_per_m;      /* default for all batch instances; per-instance via opo_set_batch_param */
+    double d_eff_m_per_V;
+} opo_crystal;
+
+/* fields: index 0 = pump, 1 = signal, 2 = idler (three-wave only).  PAPER.md:L99 Eq. 5, L105-109 Eq. 6,
+ * L145 (GDD), L316-320 (resonance flags). */
+typedef struct {
+    int n_fields;              /* 2 (degenerate, signal = idler) or 3 */
+    double lambda_m[3];
+    double n[3];               /* refractive indices n_x */
+    double beta1_s_per_m[3];   /* 1/v_x, any common origin; only differences to ref_field are used */
+    double beta2_s2_per_m[3];  /* k''_x */
+    double alpha_per_m[3];     /* power attenuation alpha_x */
+    int ref_field;             /* co-moving frame (paper: the signal, L101) */
+    int resonant[3];           /* pump must be 0 */
+    double R[3];               /* power reflectivity 1 - theta_x, resonant fields */
+    double delta_rad[3];       /* carrier detuning phase delta_x of Eq. 6 */
+    double delta_T_s[3];       /* group-delay detuning: A(tau) -> A(tau - delta_T), circular (R13) */
+    double gdd_s2[3];          /* gamma_x of L145: spectral phase (gamma/2) Omega^2 (R14) */
+} opo_fields;
+
+#define OPO_PRECISION_C64 0
+#define OPO_PRECISION_C128 1
+
+/* grid: PAPER.md:L175-178 (dt = t_rt/n), L162 (nz), L193 (precision) */
+typedef struct {
+    int log2_n;        /* 6 .. 18 (c64), 6 .. 13 (c128) */
+    double window_s;   /* N dt, the round-trip window t_rt */
+    int nz_per_pass;   /* z-steps per crystal pass; h = length_m / nz_per_pass */
+    int precision;     /* OPO_PRECISION_C64 | OPO_PRECISION_C128 */
+    int batch;         /* independent OPO instances sharing crystal, fields and grid */
+} opo_grid;
+
+/* Create a handle: validates, builds the fp64 host tables, allocates device state (zeroed) and
+ * uploads the tables on the default stream.  *out is untouched on failure. */
+int opo_create(const opo_crystal* crystal, const opo_fields* fields, const opo_grid* grid, opo_handle** out);
+int opo_destroy(opo_handle* h);
+
+/* All later work is enqueued on this stream (a cudaStream_t cast to void*; NULL = default stream).
+ * The caller owns the stream and keeps it alive while the handle uses it. */
+int opo_set_stream(opo_handle* h, void* cuda_stream);
+
+/* Per-instance sweep parameters (BASELINE.json configs[2] detuning sweep, configs[4] dk sweep).
+ * host_vals has `count` doubles and count must equal batch.  `field` is ignored for OPO_PARAM_DK. */
+#define OPO_PARAM_DK 0
+#define OPO_PARAM_DELTA_T 1
+#define OPO_PARAM_DELTA_RAD 2
+#define OPO_PARAM_GDD 3
+int opo_set_batch_param(opo_handle* h, int param, int field, const double* host_vals, int count);
+
+/* Pump input S_p (PAPER.md:L268 ReadPump): time-domain complex [N] (per_instance = 0, broadcast to
+ * all instances) or [batch][N].  Copied into the handle; re-injected at every round-trip boundary;
+ * also becomes the current pump field when z = 0. */
+int opo_set_pump(opo_handle* h, const void* dev_pump, int per_instance);
+int opo_set_pump_host(opo_handle* h, const void* host_pump, int per_instance);
+
+/* Signal / idler (or pump) seed, [batch][N]: sets the current field and the stored input S_x
+ * (noise seed).  Resets nothing else; allowed at any z. */
+int opo_set_field(opo_handle* h, int field, const void* dev_data);
+int opo_set_field_host(opo_handle* h, int field, const void* host_data);
+
+/* nz fixed z-steps from the current z; no boundary operator.  OPO_ERR_STATE if it would pass z = L. */
+int opo_propagate(opo_handle* h, int nz);
+
+/* n x (full crystal pass + cavity boundary).  Requires z = 0.  Afterwards the current fields are
+ * those at z = 0 of the next round trip and the exit buffer holds the fields at z = L of the last
+ * pass (before the mirror). */
+int opo_roundtrips(opo_handle* h, int n);
+
+#define OPO_WHICH_CURRENT 0
+#define OPO_WHICH_EXIT 1
+#define OPO_DOMAIN_TIME 0
+#define OPO_DOMAIN_FREQ 1
+/* Copy field `field` of every instance, [batch][N], into the caller's buffer.  FREQ = unnormalised
+ * forward DFT, natural order, no fftshift. */
+int opo_get_fields(opo_handle* h, int field, int which, int domain, void* dev_out);
+int opo_get_fields_host(opo_handle* h, int field, int which, int domain, void* host_out);
+
+/* Wait for the stream; reports asynchronous faults. */
+int opo_sync(opo_handle* h);
+/* Synchronises, then scans the current fields: OPO_ERR_NONFINITE if any NaN/Inf. */
+int opo_check_finite(opo_handle* h);
+/* Position inside the crystal in z-steps taken since the entrance (0 .. nz_per_pass). */
+int opo_get_z_steps(const opo_handle* h, int* out_steps);
+
+/* Execution engine.  AUTO picks RESIDENT where one field fits one SM's shared memory (N <= 2^14 c64,
+ * N <= 2^13 c128), else STREAMING.
+ *   RESIDENT : one thread-block cluster per instance, one CTA per field, fields stay in shared
+ *              memory across z-steps and round trips; one launch per opo_propagate/opo_roundtrips.
+ *   STREAMING: fields live in HBM/L2; one fused FFT-multiply-IFFT kernel and one RK4 kernel per z-step
+ *              (N <= 2^14), or the four-step decomposition (N >= 2^15). */
+#define OPO_ENGINE_AUTO 0
+#define OPO_ENGINE_RESIDENT 1
+#define OPO_ENGINE_STREAMING 2
+#define OPO_OPT_ENGINE 0
+int opo_set_option(opo_handle* h, int option, int value);
+
+#define OPO_INFO_ENGINE 0        /* engine the next propagate/roundtrips call will use */
+#define OPO_INFO_LAUNCHES 1      /* kernels launched by this handle so far */
+#define OPO_INFO_N 2
+#define OPO_INFO_BATCH 3
+#define OPO_INFO_SM_COUNT 4
+int opo_get_info(const opo_handle* h, int what, long long* out);
+
+/* Last error text of this handle (or of the failed opo_create when h is NULL).  Never NULL. */
+const char* opo_last_error(const opo_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OPO_H_ */

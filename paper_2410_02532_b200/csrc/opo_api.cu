@@ -1,0 +1,651 @@
+// opo_api.cu -- the C ABI of include/opo.h: handle, fp64 host tables, engine selection, launches.
+//
+// Everything numerical on the path runs in the kernels of opo_kernels.cuh / opo_resident.cuh /
+// opo_large.cuh; the host only builds constant tables in fp64 (dispersion multipliers, boundary
+// multipliers, FFT twiddles, dk phases) and sequences launches.  There is no CPU fallback.
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/opo.h"
+#include "opo_internal.h"
+
+namespace {
+
+using cd = std::complex<double>;
+constexpr double kPi = 3.14159265358979323846264338327950288;
+
+thread_local std::string g_create_error;
+
+// ---- radix plan on the host (mirror of opo::plan<L> in opo_fft.cuh) ------------------------------------
+struct HostPlan {
+    int L = 0, P = 0;
+    int rbits[8] = {0}, sbits[8] = {0}, tw_offset[9] = {0};
+    int tw_total = 0;
+    explicit HostPlan(int L_) : L(L_) {
+        const int rem = L % 4;
+        const int n16 = (rem == 1) ? (L / 4 - 1) : (L / 4);
+        P = n16 + (rem == 0 ? 0 : (rem == 1 ? 2 : 1));
+        int used = 0, off = 0;
+        for (int p = 0; p < P; ++p) {
+            int rb;
+            if (p < n16) rb = 4;
+            else if (rem == 1) rb = (p == n16) ? 3 : 2;
+            else if (rem == 2) rb = 2;
+            else rb = 3;
+            rbits[p] = rb;
+            used += rb;
+            sbits[p] = L - used;
+            tw_offset[p] = off;
+            off += ((1 << rb) - 1) << sbits[p];
+        }
+        tw_offset[P] = off;
+        tw_total = off;
+    }
+    // position after all forward passes -> frequency index:  pos = sum_p k_p S_p,  k = sum_p k_p R_1..R_{p-1}
+    int freq_of_pos(int pos) const {
+        int k = 0, mult = 1;
+        for (int p = 0; p < P; ++p) {
+            const int kp = (pos >> sbits[p]) & ((1 << rbits[p]) - 1);
+            k += kp * mult;
+            mult <<= rbits[p];
+        }
+        return k;
+    }
+};
+
+// (c, s) on the unit circle -> floats bracketing the exact values, chosen so that c^2 + s^2 is
+// closest to 1: twiddle *magnitude* error is what accumulates over z-steps (see opo_fft.cuh).
+void round_unit(double c, double s, float* cf, float* sf) {
+    float cc[2] = {(float)c, (float)c}, ss[2] = {(float)s, (float)s};
+    if ((double)cc[0] != c) cc[1] = std::nextafterf(cc[0], (double)cc[0] < c ? INFINITY : -INFINITY);
+    if ((double)ss[0] != s) ss[1] = std::nextafterf(ss[0], (double)ss[0] < s ? INFINITY : -INFINITY);
+    double best = 1e300;
+    for (int i = 0; i < 2; ++i)
+        for (int j = 0; j < 2; ++j) {
+            double e = std::fabs((double)cc[i] * cc[i] + (double)ss[j] * ss[j] - 1.0);
+            if (e < best) { best = e; *cf = cc[i]; *sf = ss[j]; }
+        }
+}
+
+}  // namespace
+
+struct opo_handle {
+    opo_crystal crystal{};
+    opo_fields fields{};
+    opo_grid grid{};
+    int N = 0, L = 0, F = 0, B = 0, nz = 0;
+    bool dbl = false;
+    size_t esz = 8;            // bytes per complex element
+    double h = 0.0;
+    double kappa[3] = {0, 0, 0};
+    cudaStream_t stream = nullptr;
+    int sm_count = 0;
+
+    // per-instance parameters
+    std::vector<double> dk;                 // [B]
+    std::vector<double> dT[3], drad[3], gdd[3];
+    bool per_inst_boundary[3] = {false, false, false};
+    bool tables_dirty = true, phase_dirty = true;
+
+    // device state
+    void* cur[3] = {nullptr, nullptr, nullptr};
+    void* S[3] = {nullptr, nullptr, nullptr};
+    void* exitb[3] = {nullptr, nullptr, nullptr};
+    void* SH[3] = {nullptr, nullptr, nullptr};
+    void* scratch = nullptr;
+    // device tables
+    void* tw = nullptr;
+    int* perm = nullptr;
+    void* tabH[3] = {nullptr, nullptr, nullptr};
+    void* tabH2[3] = {nullptr, nullptr, nullptr};
+    void* tabGM[3] = {nullptr, nullptr, nullptr};
+    void* tabHB[3] = {nullptr, nullptr, nullptr};
+    size_t tabB_count[3] = {0, 0, 0};      // instances allocated for GM / HB (1 or B)
+    void* mirror[3] = {nullptr, nullptr, nullptr};
+    bool boundary_fft[3] = {false, false, false};
+    void* phase = nullptr;
+    int* flag = nullptr;
+
+    int z_steps = 0;
+    int engine_opt = OPO_ENGINE_AUTO;
+    bool resident_ok = false;
+    opo::ResidentInfo rinfo{};
+    long long launches = 0;
+    std::string err;
+    std::vector<int> host_perm;
+
+    size_t field_bytes() const { return (size_t)B * N * esz; }
+};
+
+namespace {
+
+int fail(opo_handle* h, int code, const std::string& msg) {
+    if (h) h->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define OPO_CUDA(h, call)                                                                  \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess)                                                             \
+            return fail((h), OPO_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+// upload complex<double> values as float2 / double2
+int upload_complex(opo_handle* h, void* dst, const cd* src, size_t count, bool unit_twiddles = false) {
+    if (h->dbl) {
+        OPO_CUDA(h, cudaMemcpyAsync(dst, src, count * sizeof(cd), cudaMemcpyHostToDevice, h->stream));
+        OPO_CUDA(h, cudaStreamSynchronize(h->stream));
+    } else {
+        std::vector<float> tmp(2 * count);
+        for (size_t i = 0; i < count; ++i) {
+            if (unit_twiddles) round_unit(src[i].real(), src[i].imag(), &tmp[2 * i], &tmp[2 * i + 1]);
+            else { tmp[2 * i] = (float)src[i].real(); tmp[2 * i + 1] = (float)src[i].imag(); }
+        }
+        OPO_CUDA(h, cudaMemcpyAsync(dst, tmp.data(), tmp.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        OPO_CUDA(h, cudaStreamSynchronize(h->stream));
+    }
+    return OPO_OK;
+}
+
+// Omega_k = 2 pi k' / (N dt), natural FFT order, Nyquist bin negative (R9)
+double omega_of(const opo_handle* h, int k) {
+    const int kp = (k < h->N / 2) ? k : k - h->N;
+    return 2.0 * kPi * (double)kp / h->grid.window_s;
+}
+
+// natural-order frequency multiplier -> register layout of mid_pass_smem: tab[kk * NBF + u] = M[freq(u R + kk)]
+void to_mid_layout(const opo_handle* h, const HostPlan& pl, const cd* M, cd* out) {
+    const int R = 1 << pl.rbits[pl.P - 1];
+    const int NBF = h->N / R;
+    for (int u = 0; u < NBF; ++u)
+        for (int kk = 0; kk < R; ++kk) out[(size_t)kk * NBF + u] = M[h->host_perm[u * R + kk]];
+}
+
+}  // namespace
+
+namespace {
+
+// ---- tables ----------------------------------------------------------------------------------------------
+// H_x[k]  = exp((-alpha_x/2 + i D_x(Omega_k)) h/2),  D_x = -(beta1_x - beta1_ref) Omega + (beta2_x/2) Omega^2
+//           (Eq. 5 with readings R7, R8, R10)
+// G_x[k]  = exp(i (gdd_x/2) Omega_k^2 - i Omega_k delta_T_x)     (R13, R14)
+// m_x     = sqrt(R_x) exp(i delta_x)                              (Eq. 6)
+// Device tables carry the 1/N of the inverse transform and are stored in mid-pass layout:
+//   tabH = H/N, tabH2 = H^2/N, tabGM = G m/N, tabHB = H^2 G m/N (half-steps merged across the boundary).
+int build_tables(opo_handle* h) {
+    const int N = h->N, F = h->F, B = h->B;
+    HostPlan pl(h->L);
+    const double invN = 1.0 / (double)N;
+    std::vector<cd> Hh(N), M(N), lay(N);
+    for (int x = 0; x < F; ++x) {
+        const double db1 = h->fields.beta1_s_per_m[x] - h->fields.beta1_s_per_m[h->fields.ref_field];
+        const double b2 = h->fields.beta2_s2_per_m[x], al = h->fields.alpha_per_m[x];
+        for (int k = 0; k < N; ++k) {
+            const double om = omega_of(h, k);
+            const double D = -db1 * om + 0.5 * b2 * om * om;
+            Hh[k] = std::exp(cd(-0.5 * al, D) * (0.5 * h->h));
+        }
+        for (int k = 0; k < N; ++k) M[k] = Hh[k] * invN;
+        to_mid_layout(h, pl, M.data(), lay.data());
+        if (int rc = upload_complex(h, h->tabH[x], lay.data(), N)) return rc;
+        for (int k = 0; k < N; ++k) {
+            const double om = omega_of(h, k);
+            const double D = -db1 * om + 0.5 * b2 * om * om;
+            M[k] = std::exp(cd(-0.5 * al, D) * h->h) * invN;     // H^2 evaluated directly in fp64
+        }
+        to_mid_layout(h, pl, M.data(), lay.data());
+        if (int rc = upload_complex(h, h->tabH2[x], lay.data(), N)) return rc;
+
+        if (!h->fields.resonant[x]) continue;
+        // boundary tables, shared or per instance
+        const size_t need = h->per_inst_boundary[x] ? (size_t)B : 1;
+        if (h->tabB_count[x] != need) {
+            if (h->tabGM[x]) cudaFree(h->tabGM[x]);
+            if (h->tabHB[x]) cudaFree(h->tabHB[x]);
+            h->tabGM[x] = h->tabHB[x] = nullptr;
+            if (cudaMalloc(&h->tabGM[x], need * N * h->esz) != cudaSuccess ||
+                cudaMalloc(&h->tabHB[x], need * N * h->esz) != cudaSuccess)
+                return fail(h, OPO_ERR_ALLOC, "cudaMalloc of boundary tables failed");
+            h->tabB_count[x] = need;
+        }
+        bool any_fft = false;
+        std::vector<cd> mir(B);
+        for (int b = 0; b < B; ++b) {
+            if (h->gdd[x][b] != 0.0 || h->dT[x][b] != 0.0) any_fft = true;
+            mir[b] = std::sqrt(h->fields.R[x]) * cd(std::cos(h->drad[x][b]), std::sin(h->drad[x][b]));
+        }
+        h->boundary_fft[x] = any_fft;
+        if (int rc = upload_complex(h, h->mirror[x], mir.data(), B)) return rc;
+        for (size_t b = 0; b < need; ++b) {
+            for (int k = 0; k < N; ++k) {
+                const double om = omega_of(h, k);
+                const double ph = 0.5 * h->gdd[x][b] * om * om - om * h->dT[x][b];
+                const cd gm = cd(std::cos(ph), std::sin(ph)) * mir[b];
+                const double D = -db1 * om + 0.5 * b2 * om * om;
+                M[k] = gm * invN;
+                Hh[k] = std::exp(cd(-0.5 * al, D) * h->h) * gm * invN;
+            }
+            to_mid_layout(h, pl, M.data(), lay.data());
+            if (int rc = upload_complex(h, (char*)h->tabGM[x] + b * N * h->esz, lay.data(), N)) return rc;
+            to_mid_layout(h, pl, Hh.data(), lay.data());
+            if (int rc = upload_complex(h, (char*)h->tabHB[x] + b * N * h->esz, lay.data(), N)) return rc;
+        }
+    }
+    h->tables_dirty = false;
+    return OPO_OK;
+}
+
+// phase[b][j] = exp(i dk_b j h/2), j = 0 .. 2 nz   (R4: z from the crystal entrance)
+int build_phase(opo_handle* h) {
+    const int stride = 2 * h->nz + 1;
+    std::vector<cd> ph((size_t)h->B * stride);
+    for (int b = 0; b < h->B; ++b)
+        for (int j = 0; j < stride; ++j) {
+            const double a = h->dk[b] * (0.5 * h->h) * (double)j;
+            ph[(size_t)b * stride + j] = cd(std::cos(a), std::sin(a));
+        }
+    if (int rc = upload_complex(h, h->phase, ph.data(), ph.size())) return rc;
+    h->phase_dirty = false;
+    return OPO_OK;
+}
+
+int build_fft_tables(opo_handle* h) {
+    HostPlan pl(h->L);
+    std::vector<cd> tw((size_t)std::max(pl.tw_total, 1));
+    for (int p = 0; p < pl.P; ++p) {
+        const int R = 1 << pl.rbits[p], S = 1 << pl.sbits[p];
+        const double M = (double)R * (double)S;
+        for (int k = 1; k < R; ++k)
+            for (int t = 0; t < S; ++t) {
+                const double a = -2.0 * kPi * (double)k * (double)t / M;
+                tw[(size_t)pl.tw_offset[p] + (size_t)(k - 1) * S + t] = cd(std::cos(a), std::sin(a));
+            }
+    }
+    if (cudaMalloc(&h->tw, tw.size() * h->esz) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc(tw)");
+    if (int rc = upload_complex(h, h->tw, tw.data(), tw.size(), /*unit_twiddles=*/true)) return rc;
+    h->host_perm.resize(h->N);
+    for (int pos = 0; pos < h->N; ++pos) h->host_perm[pos] = pl.freq_of_pos(pos);
+    if (cudaMalloc(&h->perm, (size_t)h->N * sizeof(int)) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc(perm)");
+    OPO_CUDA(h, cudaMemcpy(h->perm, h->host_perm.data(), (size_t)h->N * sizeof(int), cudaMemcpyHostToDevice));
+    return OPO_OK;
+}
+
+int ensure_tables(opo_handle* h) {
+    if (h->tables_dirty) if (int rc = build_tables(h)) return rc;
+    if (h->phase_dirty) if (int rc = build_phase(h)) return rc;
+    return OPO_OK;
+}
+
+void free_all(opo_handle* h) {
+    for (int x = 0; x < 3; ++x) {
+        void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->mirror[x]};
+        for (void* p : ptrs) if (p) cudaFree(p);
+    }
+    void* more[] = {h->scratch, h->tw, h->perm, h->phase, h->flag};
+    for (void* p : more) if (p) cudaFree(p);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* opo_last_error(const opo_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo_handle** out) {
+    if (!c || !f || !g || !out) return fail(nullptr, OPO_ERR_INVALID_ARG, "null argument");
+    if (f->n_fields != 2 && f->n_fields != 3) return fail(nullptr, OPO_ERR_INVALID_ARG, "n_fields must be 2 or 3");
+    if (g->precision != OPO_PRECISION_C64 && g->precision != OPO_PRECISION_C128)
+        return fail(nullptr, OPO_ERR_INVALID_ARG, "precision must be 0 (c64) or 1 (c128)");
+    if (g->log2_n < 4 || g->log2_n > 18) return fail(nullptr, OPO_ERR_INVALID_ARG, "log2_n outside [4, 18]");
+    if (g->nz_per_pass <= 0 || g->batch <= 0 || !(g->window_s > 0.0) || !(c->length_m > 0.0))
+        return fail(nullptr, OPO_ERR_INVALID_ARG, "nz_per_pass, batch, window_s and length_m must be positive");
+    if (f->ref_field < 0 || f->ref_field >= f->n_fields) return fail(nullptr, OPO_ERR_INVALID_ARG, "ref_field out of range");
+    for (int x = 0; x < f->n_fields; ++x) {
+        if (!(f->lambda_m[x] > 0.0) || !(f->n[x] > 0.0)) return fail(nullptr, OPO_ERR_INVALID_ARG, "lambda and n must be positive");
+        if (f->resonant[x] && !(f->R[x] >= 0.0 && f->R[x] <= 1.0)) return fail(nullptr, OPO_ERR_INVALID_ARG, "R outside [0, 1]");
+    }
+    if (f->resonant[0]) return fail(nullptr, OPO_ERR_UNSUPPORTED, "resonant pump: the paper gives no input-coupling rule");
+    const int maxL = (g->precision == OPO_PRECISION_C64) ? opo::kMaxLog2Smem : opo::kMaxLog2Smem - 1;
+    if (g->log2_n < opo::kMinLog2 || g->log2_n > maxL)
+        return fail(nullptr, OPO_ERR_UNSUPPORTED, "grid size not supported for this precision (c64: 2^6..2^14, c128: 2^6..2^13)");
+
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+        return fail(nullptr, OPO_ERR_CUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(cudaGetLastError()));
+    if (prop.major != 10)
+        return fail(nullptr, OPO_ERR_CUDA, "libopo is built for sm_100a only; device is sm_" + std::to_string(prop.major) + std::to_string(prop.minor));
+
+    opo_handle* h = new opo_handle();
+    h->crystal = *c; h->fields = *f; h->grid = *g;
+    h->L = g->log2_n; h->N = 1 << g->log2_n; h->F = f->n_fields; h->B = g->batch; h->nz = g->nz_per_pass;
+    h->dbl = (g->precision == OPO_PRECISION_C128);
+    h->esz = h->dbl ? 16 : 8;
+    h->h = c->length_m / (double)g->nz_per_pass;
+    h->sm_count = prop.multiProcessorCount;
+    for (int x = 0; x < h->F; ++x) h->kappa[x] = 2.0 * kPi * c->d_eff_m_per_V / (f->n[x] * f->lambda_m[x]);
+    if (h->F == 2) h->kappa[0] *= 0.5;                                                                         // reading R5
+    h->dk.assign(h->B, c->dk_per_m);
+    for (int x = 0; x < 3; ++x) {
+        h->dT[x].assign(h->B, x < h->F ? f->delta_T_s[x] : 0.0);
+        h->drad[x].assign(h->B, x < h->F ? f->delta_rad[x] : 0.0);
+        h->gdd[x].assign(h->B, x < h->F ? f->gdd_s2[x] : 0.0);
+    }
+    auto bail = [&](int code, const std::string& msg) { free_all(h); delete h; return fail(nullptr, code, msg); };
+    const size_t fb = h->field_bytes();
+    for (int x = 0; x < h->F; ++x) {
+        void** arrs[] = {&h->cur[x], &h->S[x], &h->exitb[x], &h->SH[x]};
+        for (void** p : arrs) {
+            if (cudaMalloc(p, fb) != cudaSuccess) return bail(OPO_ERR_ALLOC, "cudaMalloc of field state failed");
+            cudaMemset(*p, 0, fb);
+        }
+        if (cudaMalloc(&h->tabH[x], (size_t)h->N * h->esz) != cudaSuccess || cudaMalloc(&h->tabH2[x], (size_t)h->N * h->esz) != cudaSuccess ||
+            cudaMalloc(&h->mirror[x], (size_t)h->B * h->esz) != cudaSuccess)
+            return bail(OPO_ERR_ALLOC, "cudaMalloc of tables failed");
+    }
+    if (cudaMalloc(&h->scratch, fb) != cudaSuccess || cudaMalloc(&h->phase, (size_t)h->B * (2 * h->nz + 1) * h->esz) != cudaSuccess ||
+        cudaMalloc((void**)&h->flag, sizeof(int)) != cudaSuccess)
+        return bail(OPO_ERR_ALLOC, "cudaMalloc of scratch failed");
+    if (int rc = build_fft_tables(h)) { std::string m = h->err; return bail(rc, m); }
+    if (int rc = ensure_tables(h)) { std::string m = h->err; return bail(rc, m); }
+    // resident engine availability
+    cudaError_t e = h->dbl ? opo::resident_info_f64(h->L, h->F, &h->rinfo) : opo::resident_info_f32(h->L, h->F, &h->rinfo);
+    h->resident_ok = (e == cudaSuccess && h->rinfo.max_clusters > 0);
+    if (e != cudaSuccess) cudaGetLastError();
+    if (cudaDeviceSynchronize() != cudaSuccess) return bail(OPO_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
+    *out = h;
+    return OPO_OK;
+}
+
+int opo_destroy(opo_handle* h) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    cudaStreamSynchronize(h->stream);
+    free_all(h);
+    delete h;
+    return OPO_OK;
+}
+
+int opo_set_stream(opo_handle* h, void* s) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    h->stream = (cudaStream_t)s;
+    return OPO_OK;
+}
+
+int opo_set_batch_param(opo_handle* h, int param, int field, const double* v, int count) {
+    if (!h || !v) return fail(h, OPO_ERR_INVALID_ARG, "null argument");
+    if (count != h->B) return fail(h, OPO_ERR_INVALID_ARG, "count must equal batch");
+    if (param == OPO_PARAM_DK) {
+        h->dk.assign(v, v + count);
+        h->phase_dirty = true;
+        return OPO_OK;
+    }
+    if (field < 0 || field >= h->F) return fail(h, OPO_ERR_INVALID_ARG, "field out of range");
+    std::vector<double>* dst = nullptr;
+    if (param == OPO_PARAM_DELTA_T) dst = &h->dT[field];
+    else if (param == OPO_PARAM_DELTA_RAD) dst = &h->drad[field];
+    else if (param == OPO_PARAM_GDD) dst = &h->gdd[field];
+    else return fail(h, OPO_ERR_INVALID_ARG, "unknown param");
+    dst->assign(v, v + count);
+    bool uniform = true;
+    for (int x = 0; x < h->F; ++x) {
+        bool u = true;
+        for (int b = 1; b < h->B; ++b)
+            if (h->dT[x][b] != h->dT[x][0] || h->gdd[x][b] != h->gdd[x][0] || h->drad[x][b] != h->drad[x][0]) u = false;
+        h->per_inst_boundary[x] = !u;
+        uniform = uniform && u;
+    }
+    (void)uniform;
+    h->tables_dirty = true;
+    return OPO_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+#define OPO_LAUNCH(h, call)                                                                \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess)                                                             \
+            return fail((h), OPO_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+        ++(h)->launches;                                                                   \
+    } while (0)
+
+// surface a sticky asynchronous fault from earlier work without synchronising
+int check_async(opo_handle* h) {
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) return fail(h, OPO_ERR_CUDA, std::string("earlier asynchronous fault: ") + cudaGetErrorString(e));
+    return OPO_OK;
+}
+
+int engine_in_use(const opo_handle* h) {
+    if (h->engine_opt == OPO_ENGINE_STREAMING) return OPO_ENGINE_STREAMING;
+    return h->resident_ok ? OPO_ENGINE_RESIDENT : OPO_ENGINE_STREAMING;
+}
+
+// ---- streaming engine ------------------------------------------------------------------------------------------
+enum TableKind { TAB_H, TAB_H2 };
+
+int stream_linear_all(opo_handle* h, TableKind kind, bool to_exit) {
+    opo::LinArgs a{};
+    a.n_slots = h->F; a.batch = h->B; a.tw = h->tw;
+    for (int x = 0; x < h->F; ++x) {
+        a.slot[x].src = h->cur[x]; a.slot[x].dst = h->cur[x];
+        a.slot[x].dst2 = to_exit ? h->exitb[x] : nullptr;
+        a.slot[x].tab = (kind == TAB_H) ? h->tabH[x] : h->tabH2[x];
+        a.slot[x].tab_stride = 0;
+    }
+    OPO_LAUNCH(h, h->dbl ? opo::launch_linear_f64(h->L, a, h->stream) : opo::launch_linear_f32(h->L, a, h->stream));
+    return OPO_OK;
+}
+
+int stream_rk4(opo_handle* h, int step) {
+    opo::Rk4Args a{};
+    for (int x = 0; x < h->F; ++x) { a.A[x] = h->cur[x]; a.kappa[x] = h->kappa[x]; }
+    a.n_fields = h->F; a.batch = h->B; a.n = h->N; a.h = h->h;
+    a.phase = h->phase; a.phase_stride = 2 * h->nz + 1; a.step = step;
+    OPO_LAUNCH(h, h->dbl ? opo::launch_rk4_f64(a, h->stream) : opo::launch_rk4_f32(a, h->stream));
+    return OPO_OK;
+}
+
+// nsteps z-steps from step index z0, half-steps merged:  H, N, H^2, N, ..., N, H
+int stream_steps(opo_handle* h, int z0, int nsteps, bool to_exit) {
+    if (nsteps <= 0) return OPO_OK;
+    if (int rc = stream_linear_all(h, TAB_H, false)) return rc;
+    for (int s = 0; s < nsteps; ++s) {
+        if (int rc = stream_rk4(h, z0 + s)) return rc;
+        if (s + 1 < nsteps) if (int rc = stream_linear_all(h, TAB_H2, false)) return rc;
+    }
+    return stream_linear_all(h, TAB_H, to_exit);
+}
+
+// cavity boundary on the fields at z = L (readings R11-R15)
+int stream_boundary(opo_handle* h) {
+    opo::LinArgs a{};
+    a.batch = h->B; a.tw = h->tw;
+    for (int x = 0; x < h->F; ++x) {
+        if (!h->fields.resonant[x]) {
+            OPO_CUDA(h, cudaMemcpyAsync(h->cur[x], h->S[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+        } else if (h->boundary_fft[x]) {
+            opo::LinSlot& sl = a.slot[a.n_slots++];
+            sl.src = h->cur[x]; sl.dst = h->cur[x]; sl.dst2 = nullptr;
+            sl.tab = h->tabGM[x]; sl.tab_stride = h->per_inst_boundary[x] ? h->N : 0;
+        } else {
+            opo::ScaleArgs sc{h->cur[x], h->mirror[x], h->B, h->N};
+            OPO_LAUNCH(h, h->dbl ? opo::launch_scale_f64(sc, h->stream) : opo::launch_scale_f32(sc, h->stream));
+        }
+    }
+    if (a.n_slots > 0)
+        OPO_LAUNCH(h, h->dbl ? opo::launch_linear_f64(h->L, a, h->stream) : opo::launch_linear_f32(h->L, a, h->stream));
+    return OPO_OK;
+}
+
+// ---- resident engine ---------------------------------------------------------------------------------------------
+int resident_run(opo_handle* h, int mode, int z0, int steps) {
+    opo::ResidentArgs a{};
+    for (int x = 0; x < h->F; ++x) {
+        a.cur[x] = h->cur[x]; a.S[x] = h->S[x]; a.exitb[x] = h->exitb[x]; a.SH[x] = h->SH[x];
+        a.tabH[x] = h->tabH[x]; a.tabH2[x] = h->tabH2[x]; a.tabHB[x] = h->tabHB[x]; a.tabGM[x] = h->tabGM[x];
+        a.tab_stride[x] = h->per_inst_boundary[x] ? h->N : 0;
+        a.mirror[x] = h->mirror[x];
+        a.boundary_fft[x] = h->boundary_fft[x] ? 1 : 0;
+        a.resonant[x] = h->fields.resonant[x] ? 1 : 0;
+        a.kappa[x] = h->kappa[x];
+    }
+    a.tw = h->tw; a.phase = h->phase; a.phase_stride = 2 * h->nz + 1;
+    a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
+    a.mode = mode; a.z0 = z0; a.steps = steps;
+    const int n_clusters = std::min(h->B, h->rinfo.max_clusters);
+    OPO_LAUNCH(h, h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream)
+                         : opo::launch_resident_f32(h->L, a, n_clusters, h->stream));
+    return OPO_OK;
+}
+
+int copy_in(opo_handle* h, void* dst_field, const void* src, bool per_instance, cudaMemcpyKind kind) {
+    const size_t one = (size_t)h->N * h->esz;
+    if (per_instance) {
+        OPO_CUDA(h, cudaMemcpyAsync(dst_field, src, one * h->B, kind, h->stream));
+    } else {
+        OPO_CUDA(h, cudaMemcpyAsync(dst_field, src, one, kind, h->stream));
+        for (int b = 1; b < h->B; ++b)
+            OPO_CUDA(h, cudaMemcpyAsync((char*)dst_field + b * one, dst_field, one, cudaMemcpyDeviceToDevice, h->stream));
+    }
+    return OPO_OK;
+}
+
+int set_pump_impl(opo_handle* h, const void* p, int per_instance, cudaMemcpyKind kind) {
+    if (!h || !p) return fail(h, OPO_ERR_INVALID_ARG, "null argument");
+    if (int rc = check_async(h)) return rc;
+    if (int rc = copy_in(h, h->S[0], p, per_instance != 0, kind)) return rc;
+    if (h->z_steps == 0)
+        OPO_CUDA(h, cudaMemcpyAsync(h->cur[0], h->S[0], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+    return OPO_OK;
+}
+
+int set_field_impl(opo_handle* h, int field, const void* p, cudaMemcpyKind kind) {
+    if (!h || !p) return fail(h, OPO_ERR_INVALID_ARG, "null argument");
+    if (field < 0 || field >= h->F) return fail(h, OPO_ERR_INVALID_ARG, "field out of range");
+    if (int rc = check_async(h)) return rc;
+    if (int rc = copy_in(h, h->S[field], p, true, kind)) return rc;
+    OPO_CUDA(h, cudaMemcpyAsync(h->cur[field], h->S[field], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+    return OPO_OK;
+}
+
+int get_fields_impl(opo_handle* h, int field, int which, int domain, void* out, bool host) {
+    if (!h || !out) return fail(h, OPO_ERR_INVALID_ARG, "null argument");
+    if (field < 0 || field >= h->F) return fail(h, OPO_ERR_INVALID_ARG, "field out of range");
+    if (which != OPO_WHICH_CURRENT && which != OPO_WHICH_EXIT) return fail(h, OPO_ERR_INVALID_ARG, "which must be CURRENT or EXIT");
+    if (domain != OPO_DOMAIN_TIME && domain != OPO_DOMAIN_FREQ) return fail(h, OPO_ERR_INVALID_ARG, "domain must be TIME or FREQ");
+    if (int rc = check_async(h)) return rc;
+    const void* src = (which == OPO_WHICH_CURRENT) ? h->cur[field] : h->exitb[field];
+    if (domain == OPO_DOMAIN_FREQ) {
+        opo::FreqArgs a{src, host ? h->scratch : out, h->perm, h->tw, h->B};
+        OPO_LAUNCH(h, h->dbl ? opo::launch_freq_f64(h->L, a, h->stream) : opo::launch_freq_f32(h->L, a, h->stream));
+        if (!host) return OPO_OK;
+        src = h->scratch;
+    }
+    OPO_CUDA(h, cudaMemcpyAsync(out, src, h->field_bytes(), host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, h->stream));
+    if (host) OPO_CUDA(h, cudaStreamSynchronize(h->stream));
+    return OPO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int opo_set_pump(opo_handle* h, const void* dev_pump, int per_instance) { return set_pump_impl(h, dev_pump, per_instance, cudaMemcpyDeviceToDevice); }
+int opo_set_pump_host(opo_handle* h, const void* host_pump, int per_instance) { return set_pump_impl(h, host_pump, per_instance, cudaMemcpyHostToDevice); }
+int opo_set_field(opo_handle* h, int field, const void* dev_data) { return set_field_impl(h, field, dev_data, cudaMemcpyDeviceToDevice); }
+int opo_set_field_host(opo_handle* h, int field, const void* host_data) { return set_field_impl(h, field, host_data, cudaMemcpyHostToDevice); }
+int opo_get_fields(opo_handle* h, int field, int which, int domain, void* dev_out) { return get_fields_impl(h, field, which, domain, dev_out, false); }
+int opo_get_fields_host(opo_handle* h, int field, int which, int domain, void* host_out) { return get_fields_impl(h, field, which, domain, host_out, true); }
+
+int opo_propagate(opo_handle* h, int nz) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    if (nz < 0) return fail(h, OPO_ERR_INVALID_ARG, "nz must be >= 0");
+    if (h->z_steps + nz > h->nz) return fail(h, OPO_ERR_STATE, "propagate would pass z = L");
+    if (nz == 0) return OPO_OK;
+    if (int rc = check_async(h)) return rc;
+    if (int rc = ensure_tables(h)) return rc;
+    int rc;
+    if (engine_in_use(h) == OPO_ENGINE_RESIDENT) rc = resident_run(h, 0, h->z_steps, nz);
+    else rc = stream_steps(h, h->z_steps, nz, false);
+    if (rc) return rc;
+    h->z_steps += nz;
+    return OPO_OK;
+}
+
+int opo_roundtrips(opo_handle* h, int n) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    if (n < 0) return fail(h, OPO_ERR_INVALID_ARG, "n must be >= 0");
+    if (h->z_steps != 0) return fail(h, OPO_ERR_STATE, "roundtrips requires z = 0");
+    if (n == 0) return OPO_OK;
+    if (int rc = check_async(h)) return rc;
+    if (int rc = ensure_tables(h)) return rc;
+    if (engine_in_use(h) == OPO_ENGINE_RESIDENT) return resident_run(h, 1, 0, n);
+    for (int m = 0; m < n; ++m) {
+        if (int rc = stream_steps(h, 0, h->nz, true)) return rc;
+        if (int rc = stream_boundary(h)) return rc;
+    }
+    return OPO_OK;
+}
+
+int opo_sync(opo_handle* h) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    OPO_CUDA(h, cudaStreamSynchronize(h->stream));
+    return check_async(h);
+}
+
+int opo_check_finite(opo_handle* h) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    OPO_CUDA(h, cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
+    for (int x = 0; x < h->F; ++x) {
+        const long long count = 2LL * h->B * h->N;
+        OPO_LAUNCH(h, h->dbl ? opo::launch_finite_f64(h->cur[x], count, h->flag, h->stream)
+                             : opo::launch_finite_f32(h->cur[x], count, h->flag, h->stream));
+    }
+    int flag = 0;
+    OPO_CUDA(h, cudaMemcpyAsync(&flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    OPO_CUDA(h, cudaStreamSynchronize(h->stream));
+    if (flag) return fail(h, OPO_ERR_NONFINITE, "non-finite field values (dz too coarse? PAPER.md:L162)");
+    return OPO_OK;
+}
+
+int opo_get_z_steps(const opo_handle* h, int* out) {
+    if (!h || !out) return OPO_ERR_INVALID_ARG;
+    *out = h->z_steps;
+    return OPO_OK;
+}
+
+int opo_set_option(opo_handle* h, int option, int value) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    if (option != OPO_OPT_ENGINE) return fail(h, OPO_ERR_INVALID_ARG, "unknown option");
+    if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING)
+        return fail(h, OPO_ERR_INVALID_ARG, "unknown engine");
+    if (value == OPO_ENGINE_RESIDENT && !h->resident_ok)
+        return fail(h, OPO_ERR_UNSUPPORTED, "resident engine unavailable for this size/precision on this device");
+    h->engine_opt = value;
+    return OPO_OK;
+}
+
+int opo_get_info(const opo_handle* h, int what, long long* out) {
+    if (!h || !out) return OPO_ERR_INVALID_ARG;
+    switch (what) {
+        case OPO_INFO_ENGINE: *out = engine_in_use(h); return OPO_OK;
+        case OPO_INFO_LAUNCHES: *out = h->launches; return OPO_OK;
+        case OPO_INFO_N: *out = h->N; return OPO_OK;
+        case OPO_INFO_BATCH: *out = h->B; return OPO_OK;
+        case OPO_INFO_SM_COUNT: *out = h->sm_count; return OPO_OK;
+        default: return OPO_ERR_INVALID_ARG;
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,303 @@
+// opo_fft.cuh -- in-place shared-memory complex FFT building blocks for sm_100a.
+//
+// The linear half-step of the split-step method (Eq. 11) is
+//     A <- IDFT( H .* DFT(A) ).
+// This file provides it as ONE pass structure over a field held in shared memory:
+//
+//   forward  : decimation-in-frequency passes p = 1..P (radix R_p, N = R_1 ... R_P); natural order
+//              in, digit-reversed order out, so no reordering pass is ever executed;
+//   multiply : in registers, against a table that the host stored in the digit-reversed order;
+//   inverse  : the exact adjoint factorisation (decimation-in-time, passes P..1, conjugate
+//              twiddles), digit-reversed in, natural order out.
+//
+// The last forward pass, the table multiply and the first inverse pass run on registers without
+// touching shared memory.  Because the inverse is the adjoint of the forward factorisation using
+// the *same* rounded twiddles, twiddle phase rounding cancels between the two transforms and
+// does not accumulate over thousands of z-steps; only twiddle magnitude rounding can, and the
+// host picks table roundings that minimise | |w| - 1 | ("fp32 error budget").
+//
+// Shared-memory layout: element i lives at i + (i >> PADSH) (one pad element per 16 float2 / per
+// 8 double2), which makes every pass -- including the stride-R last one -- bank-conflict free.
+#pragma once
+#include <cuda_runtime.h>
+#include <utility>
+
+namespace opo {
+
+template <class T>
+struct alignas(2 * sizeof(T)) cplx {
+    T re, im;
+};
+
+template <class T> __device__ __forceinline__ cplx<T> operator+(cplx<T> a, cplx<T> b) { return {a.re + b.re, a.im + b.im}; }
+template <class T> __device__ __forceinline__ cplx<T> operator-(cplx<T> a, cplx<T> b) { return {a.re - b.re, a.im - b.im}; }
+// a * b
+template <class T> __device__ __forceinline__ cplx<T> cmul(cplx<T> a, cplx<T> b) {
+    return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re};
+}
+// a * conj(b)
+template <class T> __device__ __forceinline__ cplx<T> cmulc(cplx<T> a, cplx<T> b) {
+    return {a.re * b.re + a.im * b.im, a.im * b.re - a.re * b.im};
+}
+
+// read-only (non-coherent) global load of one complex value
+__device__ __forceinline__ cplx<float> ldg(const cplx<float>* p) {
+    float2 v = __ldg(reinterpret_cast<const float2*>(p));
+    return {v.x, v.y};
+}
+__device__ __forceinline__ cplx<double> ldg(const cplx<double>* p) {
+    double2 v = __ldg(reinterpret_cast<const double2*>(p));
+    return {v.x, v.y};
+}
+
+template <class T> struct pad_shift;
+template <> struct pad_shift<float> { static constexpr int value = 4; };
+template <> struct pad_shift<double> { static constexpr int value = 3; };
+
+template <class T> __host__ __device__ __forceinline__ constexpr int phys(int i) { return i + (i >> pad_shift<T>::value); }
+template <class T> __host__ __device__ constexpr int padded_len(int n) { return n + (n >> pad_shift<T>::value); }
+
+// ---- compile-time roots of unity for the register butterflies -----------------------------------
+// cos(2 pi m / 32), m = 0..8
+__host__ __device__ constexpr double cos32(int m) {
+    constexpr double c[9] = {1.0,
+                             0.98078528040323044912618223613424,
+                             0.92387953251128675612818318939679,
+                             0.83146961230254523707878837761791,
+                             0.70710678118654752440084436210485,
+                             0.55557023301960222474283081394853,
+                             0.38268343236508977172845998403040,
+                             0.19509032201612826784828486847702,
+                             0.0};
+    return c[m];
+}
+// w_R^J = exp(-2 pi i J / R) for 0 <= J < R/2, R <= 32: (wr, wi) with wi <= 0
+template <int R, int J> struct root {
+    static constexpr int m = J * (32 / R);   // angle 2 pi m / 32, m in [0, 16)
+    static constexpr double c = (m <= 8) ? cos32(m) : -cos32(16 - m);
+    static constexpr double s = (m <= 8) ? cos32(8 - m) : cos32(m - 8);   // sin >= 0
+};
+
+// a * w_R^J (forward) or a * conj(w_R^J) (INV)
+template <class T, int R, int J, bool INV>
+__device__ __forceinline__ cplx<T> mul_root(cplx<T> a) {
+    if constexpr (J == 0) {
+        return a;
+    } else if constexpr (4 * J == R) {            // w = -i
+        if constexpr (INV) return {-a.im, a.re};
+        else return {a.im, -a.re};
+    } else if constexpr (8 * J == R) {            // w = (1 - i)/sqrt2
+        constexpr T h = (T)0.70710678118654752440084436210485;
+        if constexpr (INV) return {(a.re - a.im) * h, (a.re + a.im) * h};
+        else return {(a.re + a.im) * h, (a.im - a.re) * h};
+    } else if constexpr (8 * J == 3 * R) {        // w = (-1 - i)/sqrt2
+        constexpr T h = (T)0.70710678118654752440084436210485;
+        if constexpr (INV) return {(-a.re - a.im) * h, (a.re - a.im) * h};
+        else return {(a.im - a.re) * h, (-a.re - a.im) * h};
+    } else {
+        constexpr T c = (T)root<R, J>::c;
+        constexpr T s = (T)root<R, J>::s;
+        // forward: w = c - i s ; inverse: conj(w) = c + i s
+        if constexpr (INV) return {a.re * c - a.im * s, a.im * c + a.re * s};
+        else return {a.re * c + a.im * s, a.im * c - a.re * s};
+    }
+}
+
+// ---- register DFT of size R, natural order in and out ---------------------------------------------
+// Forward: decimation in frequency.  v[j] -> sum_j v[j] w_R^{jk}.
+template <class T, int R> struct dif {
+    template <int J>
+    static __device__ __forceinline__ void bf(cplx<T>* v) {
+        cplx<T> a = v[J], b = v[J + R / 2];
+        v[J] = a + b;
+        v[J + R / 2] = mul_root<T, R, J, false>(a - b);
+    }
+    template <int... J>
+    static __device__ __forceinline__ void stage(cplx<T>* v, std::integer_sequence<int, J...>) {
+        (bf<J>(v), ...);
+    }
+    static __device__ __forceinline__ void run(cplx<T>* v) {
+        stage(v, std::make_integer_sequence<int, R / 2>{});
+        dif<T, R / 2>::run(v);
+        dif<T, R / 2>::run(v + R / 2);
+        // X[2m] = first half [m], X[2m+1] = second half [m]
+        cplx<T> t[R];
+#pragma unroll
+        for (int m = 0; m < R / 2; ++m) { t[2 * m] = v[m]; t[2 * m + 1] = v[m + R / 2]; }
+#pragma unroll
+        for (int m = 0; m < R; ++m) v[m] = t[m];
+    }
+};
+template <class T> struct dif<T, 1> { static __device__ __forceinline__ void run(cplx<T>*) {} };
+
+// Inverse (unnormalised): decimation in time with conjugate roots -- the adjoint of dif<T,R>.
+template <class T, int R> struct dit_inv {
+    template <int J>
+    static __device__ __forceinline__ void bf(cplx<T>* v) {
+        cplx<T> a = v[J], b = mul_root<T, R, J, true>(v[J + R / 2]);
+        v[J] = a + b;
+        v[J + R / 2] = a - b;
+    }
+    template <int... J>
+    static __device__ __forceinline__ void stage(cplx<T>* v, std::integer_sequence<int, J...>) {
+        (bf<J>(v), ...);
+    }
+    static __device__ __forceinline__ void run(cplx<T>* v) {
+        cplx<T> t[R];
+#pragma unroll
+        for (int m = 0; m < R / 2; ++m) { t[m] = v[2 * m]; t[m + R / 2] = v[2 * m + 1]; }
+#pragma unroll
+        for (int m = 0; m < R; ++m) v[m] = t[m];
+        dit_inv<T, R / 2>::run(v);
+        dit_inv<T, R / 2>::run(v + R / 2);
+        stage(v, std::make_integer_sequence<int, R / 2>{});
+    }
+};
+template <class T> struct dit_inv<T, 1> { static __device__ __forceinline__ void run(cplx<T>*) {} };
+
+// ---- radix plan ------------------------------------------------------------------------------------
+// N = 2^L split into passes of radix 16 (as many as possible) then 8 / 4; never a radix-2 pass
+// for L >= 6:   L%4 == 0: 16..16 | 1: 16..16,8,4 | 2: 16..16,4 | 3: 16..16,8
+template <int L> struct plan {
+    static_assert(L >= 6 && L <= 14, "shared-memory FFT supports 2^6 .. 2^14");
+    static constexpr int rem = L % 4;
+    static constexpr int n16 = (rem == 1) ? (L / 4 - 1) : (L / 4);
+    static constexpr int P = n16 + (rem == 0 ? 0 : (rem == 1 ? 2 : 1));
+    __host__ __device__ static constexpr int rbits(int p) {   // p = 0 .. P-1
+        if (p < n16) return 4;
+        if (rem == 1) return (p == n16) ? 3 : 2;
+        if (rem == 2) return 2;
+        return 3;   // rem == 3
+    }
+    // log2 of S_p = M_p / R_p (stride between the R_p inputs of a butterfly)
+    __host__ __device__ static constexpr int sbits(int p) {
+        int used = 0;
+        for (int q = 0; q <= p; ++q) used += rbits(q);
+        return L - used;
+    }
+    // offset (in complex elements) of pass p's twiddle block W_p[k-1][t'] inside the twiddle table
+    __host__ __device__ static constexpr int tw_offset(int p) {
+        int off = 0;
+        for (int q = 0; q < p; ++q) off += ((1 << rbits(q)) - 1) << sbits(q);
+        return off;
+    }
+    static constexpr int tw_total = tw_offset(P);
+};
+
+// ---- one forward (DIF) pass over shared memory -------------------------------------------------------
+// butterflies u = tid, tid + NT, ...;  b = u >> sbits, t = u & (S-1); element j at b*M + j*S + t.
+template <class T, int L, int PASS, int NT>
+__device__ __forceinline__ void fwd_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid) {
+    using PL = plan<L>;
+    constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
+    constexpr int NBF = (1 << L) / R;
+    const cplx<T>* __restrict__ w = tw + PL::tw_offset(PASS);
+#pragma unroll 1
+    for (int u = tid; u < NBF; u += NT) {
+        const int b = u >> SB, t = u & (S - 1);
+        const int base = (b << (SB + RB)) + t;
+        cplx<T> v[R];
+#pragma unroll
+        for (int j = 0; j < R; ++j) v[j] = sm[phys<T>(base + (j << SB))];
+        dif<T, R>::run(v);
+        if constexpr (SB > 0) {
+#pragma unroll
+            for (int k = 1; k < R; ++k) v[k] = cmul(v[k], ldg(&w[((k - 1) << SB) + t]));
+        }
+#pragma unroll
+        for (int k = 0; k < R; ++k) sm[phys<T>(base + (k << SB))] = v[k];
+    }
+}
+
+// ---- one inverse (DIT) pass over shared memory ---------------------------------------------------------
+template <class T, int L, int PASS, int NT>
+__device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid) {
+    using PL = plan<L>;
+    constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
+    constexpr int NBF = (1 << L) / R;
+    const cplx<T>* __restrict__ w = tw + PL::tw_offset(PASS);
+#pragma unroll 1
+    for (int u = tid; u < NBF; u += NT) {
+        const int b = u >> SB, t = u & (S - 1);
+        const int base = (b << (SB + RB)) + t;
+        cplx<T> v[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = sm[phys<T>(base + (k << SB))];
+        if constexpr (SB > 0) {
+#pragma unroll
+            for (int k = 1; k < R; ++k) v[k] = cmulc(v[k], ldg(&w[((k - 1) << SB) + t]));
+        }
+        dit_inv<T, R>::run(v);
+#pragma unroll
+        for (int j = 0; j < R; ++j) sm[phys<T>(base + (j << SB))] = v[j];
+    }
+}
+
+// ---- the fused middle: last forward pass, table multiply, first inverse pass, all in registers ----------
+// The last pass has S = 1: butterfly u owns positions u*R .. u*R + R-1.  The table is stored as
+// tab[k * (N/R) + u] so that consecutive threads read consecutive addresses.
+template <class T, int L, int NT>
+__device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab, int tid) {
+    using PL = plan<L>;
+    constexpr int PASS = PL::P - 1;
+    constexpr int RB = PL::rbits(PASS), R = 1 << RB;
+    static_assert(PL::sbits(PASS) == 0, "last pass must have unit stride");
+    constexpr int NBF = (1 << L) / R;
+#pragma unroll 1
+    for (int u = tid; u < NBF; u += NT) {
+        const int base = u << RB;
+        cplx<T> v[R];
+#pragma unroll
+        for (int j = 0; j < R; ++j) v[j] = sm[phys<T>(base + j)];
+        dif<T, R>::run(v);
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[k] = cmul(v[k], ldg(&tab[k * NBF + u]));
+        dit_inv<T, R>::run(v);
+#pragma unroll
+        for (int j = 0; j < R; ++j) sm[phys<T>(base + j)] = v[j];
+    }
+}
+
+// forward passes 0 .. P-2 (everything before the fused middle), with the barriers between them
+template <class T, int L, int NT, int PASS = 0>
+__device__ __forceinline__ void fwd_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
+    if constexpr (PASS < plan<L>::P - 1) {
+        fwd_pass_smem<T, L, PASS, NT>(sm, tw, tid);
+        __syncthreads();
+        fwd_passes<T, L, NT, PASS + 1>(sm, tw, tid);
+    }
+}
+// inverse passes P-2 .. 0
+template <class T, int L, int NT, int PASS = plan<L>::P - 2>
+__device__ __forceinline__ void inv_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
+    if constexpr (PASS >= 0) {
+        __syncthreads();
+        inv_pass_smem<T, L, PASS, NT>(sm, tw, tid);
+        inv_passes<T, L, NT, PASS - 1>(sm, tw, tid);
+    }
+}
+
+// A <- IDFT( tab .* DFT(A) ) on a field in (padded) shared memory.  Caller guarantees the field is
+// visible to all threads on entry (barrier) and must barrier before reading the result.
+template <class T, int L, int NT>
+__device__ __forceinline__ void linear_op_smem(cplx<T>* sm, const cplx<T>* tw, const cplx<T>* tab, int tid) {
+    fwd_passes<T, L, NT>(sm, tw, tid);
+    mid_pass_smem<T, L, NT>(sm, tab, tid);
+    inv_passes<T, L, NT>(sm, tw, tid);
+}
+
+// forward transform only (for frequency-domain output): result in digit-reversed order in smem
+template <class T, int L, int NT>
+__device__ __forceinline__ void forward_only_smem(cplx<T>* sm, const cplx<T>* tw, int tid) {
+    fwd_passes<T, L, NT>(sm, tw, tid);
+    fwd_pass_smem<T, L, plan<L>::P - 1, NT>(sm, tw, tid);
+}
+
+// threads per CTA for a 2^L-point field: 32 points per thread for fp32, 16 for fp64
+template <class T, int L> struct cta_threads {
+    static constexpr int per = (sizeof(T) == 4) ? 32 : 16;
+    static constexpr int raw = (1 << L) / per;
+    static constexpr int value = raw < 32 ? 32 : raw;
+};
+
+}  // namespace opo

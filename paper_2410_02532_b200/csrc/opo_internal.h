@@ -1,0 +1,99 @@
+// opo_internal.h -- plain-C++ interface between the host library (opo_api.cu) and the templated
+// kernel launchers (opo_inst_f32.cu / opo_inst_f64.cu).  No CUDA templates leak through here.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace opo {
+
+constexpr int kMinLog2 = 6;
+constexpr int kMaxLog2Smem = 14;   // one field in one SM's shared memory (fp32); fp64: 13
+
+// ---- streaming engine ------------------------------------------------------------------------------
+// One CTA per (slot, instance): dst[b] = IDFT( tab[b?] .* DFT(src[b]) ), optionally also to dst2.
+struct LinSlot {
+    const void* src;       // [B][N]
+    void* dst;             // [B][N]
+    void* dst2;            // optional second destination (exit buffer), may be null
+    const void* tab;       // mid-pass table, [N] or [B][N] in the layout of mid_pass_smem
+    long long tab_stride;  // elements between instances (0 = shared)
+};
+struct LinArgs {
+    LinSlot slot[3];
+    int n_slots;
+    int batch;
+    const void* tw;        // pass twiddles
+};
+
+struct Rk4Args {
+    void* A[3];            // current fields, [B][N]
+    int n_fields;          // 2 | 3
+    int batch;
+    int n;                 // N
+    double kappa[3];       // coupling of each equation (two-wave: kappa[0] already halved, reading R5)
+    double h;
+    const void* phase;     // [B][2 nz + 1] complex: exp(i dk_b * j * h/2)
+    int phase_stride;      // 2 nz + 1
+    int step;              // z-step index s: stage phases at 2s, 2s+1, 2s+2
+};
+
+// A[b][n] *= m[b]  (mirror sqrt(R) e^{i delta}, Eq. 6)
+struct ScaleArgs {
+    void* A;
+    const void* m;         // [B] complex
+    int batch, n;
+};
+
+// out[b][perm[pos]] = DFT(src[b])[pos]  (frequency-domain read-out, natural order)
+struct FreqArgs {
+    const void* src;
+    void* dst;
+    const int* perm;       // digit-reversed position -> frequency index
+    const void* tw;
+    int batch;
+};
+
+// ---- resident engine ---------------------------------------------------------------------------------
+// One thread-block cluster per instance, CTA rank = field.  See opo_resident.cuh.
+struct ResidentArgs {
+    void* cur[3];          // [B][N] current fields (read at start, written at end)
+    const void* S[3];      // stored inputs (non-resonant fields restart from these)
+    void* exitb[3];        // exit fields (z = L of the last pass), written when write_exit
+    void* SH[3];           // scratch [B][N]: IDFT(H DFT(S_x)) of non-resonant fields
+    const void* tabH[3];   // half step            (shared)
+    const void* tabH2[3];  // merged full step     (shared)
+    const void* tabHB[3];  // H G m H merged across the boundary (resonant; maybe per instance)
+    const void* tabGM[3];  // G m / N, un-merged boundary       (resonant; maybe per instance)
+    long long tab_stride[3];   // instance stride of HB / GM (0 = shared)
+    const void* mirror[3]; // [B] complex sqrt(R) e^{i delta} (used when the boundary has no G)
+    int boundary_fft[3];   // resonant field needs the transform pair at the boundary
+    int resonant[3];
+    const void* tw;
+    const void* phase;     // as Rk4Args
+    int phase_stride;
+    double kappa[3];
+    double h;
+    int n_fields, batch, nz;   // nz = steps per pass
+    int mode;              // 0 = propagate `steps` z-steps from step index z0; 1 = `steps` round trips
+    int z0;
+    int steps;
+};
+
+struct ResidentInfo {
+    int threads;
+    size_t smem_bytes;
+    int max_clusters;      // co-resident clusters (0 = cannot launch)
+};
+
+#define OPO_DECLARE_LAUNCHERS(SUFFIX)                                                   \
+    cudaError_t launch_linear_##SUFFIX(int log2n, const LinArgs& a, cudaStream_t s);    \
+    cudaError_t launch_rk4_##SUFFIX(const Rk4Args& a, cudaStream_t s);                  \
+    cudaError_t launch_scale_##SUFFIX(const ScaleArgs& a, cudaStream_t s);              \
+    cudaError_t launch_freq_##SUFFIX(int log2n, const FreqArgs& a, cudaStream_t s);     \
+    cudaError_t launch_finite_##SUFFIX(const void* A, long long count, int* flag, cudaStream_t s); \
+    cudaError_t resident_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);     \
+    cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s);
+
+OPO_DECLARE_LAUNCHERS(f32)
+OPO_DECLARE_LAUNCHERS(f64)
+
+}  // namespace opo

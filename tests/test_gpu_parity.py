@@ -1,0 +1,313 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances are those of BASELINE.json:north_star: complex128 rel. L2 <= 1e-10,
+complex64 rel. L2 <= 1e-4 (single pass and <= 20 round trips).  Run with -m gpu on a B200."""
+import math
+
+import numpy as np
+import pytest
+
+import opo_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"c128": 1e-10, "c64": 1e-4}
+
+
+def _gpu():
+    import torch
+    import paper_2410_02532_b200 as P
+    return torch, P
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def small_workload(log2_n, n_fields, precision, nz=6, batch=1, dk=0.0, seed=7, gdd_dt2=0.0, drad=0.0,
+                   strong=True, alpha=0.0):
+    """A short synthetic OPO with all effects switched on and every field O(1) populated, so that a
+    wrong sign / index / table anywhere shows up at O(1)."""
+    base = W.config1() if n_fields == 3 else W.config0()
+    w = W.Workload(
+        name=f"small{n_fields}w_2^{log2_n}_{precision}", length_m=base.length_m, d_eff_m_per_V=base.d_eff_m_per_V,
+        n_fields=n_fields, lambda_m=list(base.lambda_m), n_index=list(base.n_index),
+        beta1_s_per_m=list(base.beta1_s_per_m), beta2_s2_per_m=list(base.beta2_s2_per_m),
+        alpha_per_m=[alpha * (x + 1) for x in range(n_fields)], ref_field=1,
+        resonant=[0, 1, 1][:n_fields] if n_fields == 3 else [0, 1], R=[0.0, 0.9, 0.7][:n_fields],
+        delta_rad=[0.0, drad, -0.5 * drad][:n_fields], delta_T_s=[0.0, 0.0, 0.0][:n_fields],
+        gdd_s2=[0.0, 0.0, 0.0][:n_fields], log2_n=log2_n, window_s=base.window_s * (1 << log2_n) / base.n,
+        nz_per_pass=nz, precision=precision, batch=batch, n_roundtrips=2,
+        dk_per_m=np.full(batch, dk) + (np.arange(batch) * 7.0 if batch > 1 else 0.0))
+    n = w.n
+    k = w.kappa()
+    # GDD in units of dt^2: spectral phase (gdd/2) Omega^2 reaches gdd_dt2 * pi^2 / 2 at the band edge
+    w.gdd_s2 = [0.0, gdd_dt2 * w.dt ** 2, 0.5 * gdd_dt2 * w.dt ** 2][:n_fields]
+    # pump strong enough for visible gain and depletion within one pass
+    g_target = 1.5 if strong else 0.3
+    a_p = g_target / (math.sqrt(k[1] * k[-1]) * w.length_m)
+    rng = np.random.default_rng(seed)
+    tau = w.tau / (w.window_s / 8)
+    pump = a_p * (0.6 + 0.4 * np.exp(-tau ** 2)) * np.exp(1j * 0.3 * np.sin(2 * np.pi * np.arange(n) / n))
+    pumps = np.stack([pump * (1.0 + 0.1 * b) for b in range(batch)])
+    w.pump = W._round_to_precision(pumps, precision)
+    seeds = [None]
+    for x in range(1, n_fields):
+        s = np.stack([W.complex_gaussian_noise(seed * 100 + 10 * x + b, n, 0.2 * a_p) for b in range(batch)])
+        # band-limit the seed a little so the spectrum is not flat white (closer to a real field)
+        sf = np.fft.fft(s, axis=1) * np.exp(-(np.fft.fftfreq(n) * 6) ** 2)[None, :]
+        seeds.append(W._round_to_precision(np.fft.ifft(sf, axis=1), precision))
+    w.seeds = seeds
+    return w
+
+
+def run_gpu(w, engine, n_roundtrips=None, propagate=None, calls=1):
+    torch, P = _gpu()
+    o = P.from_workload(w, engine=engine)
+    if propagate is not None:
+        for nzp in propagate:
+            o.propagate(nzp)
+    else:
+        nrt = w.n_roundtrips if n_roundtrips is None else n_roundtrips
+        per = nrt // calls
+        for c in range(calls):
+            o.roundtrips(per if c < calls - 1 else nrt - per * (calls - 1))
+    o.sync()
+    cur = np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    ex = np.stack([o.get_fields(x, P.WHICH_EXIT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    eng = o.engine
+    o.close()
+    return cur, ex, eng
+
+
+def run_oracle(w, n_roundtrips=None, propagate=None):
+    import oracle
+    cur, ex = [], []
+    for b in range(w.batch):
+        o = oracle.from_workload(w, b)
+        if propagate is not None:
+            for nzp in propagate:
+                assert o.propagate(nzp) == 0
+        else:
+            assert o.roundtrips(w.n_roundtrips if n_roundtrips is None else n_roundtrips) == 0
+        cur.append(np.stack([o.get_field(x, oracle.CURRENT) for x in range(w.n_fields)]))
+        ex.append(np.stack([o.get_field(x, oracle.EXIT) for x in range(w.n_fields)]))
+    return np.stack(cur), np.stack(ex)
+
+
+def engines():
+    import paper_2410_02532_b200 as P
+    return [P.ENGINE_STREAMING, P.ENGINE_RESIDENT]
+
+
+def _engine_or_skip(w, engine):
+    torch, P = _gpu()
+    if engine == P.ENGINE_RESIDENT:
+        o = P.from_workload(w, engine=P.ENGINE_AUTO)
+        ok = o.engine == P.ENGINE_RESIDENT
+        o.close()
+        if not ok:
+            pytest.skip("resident engine not available for this size on this device")
+
+
+def assert_close(got, ref, tol, what):
+    worst = 0.0
+    for b in range(ref.shape[0]):
+        for x in range(ref.shape[1]):
+            if np.linalg.norm(ref[b, x]) == 0.0:
+                assert np.linalg.norm(got[b, x]) == 0.0
+                continue
+            worst = max(worst, rel_l2(got[b, x], ref[b, x]))
+    assert worst <= tol, f"{what}: worst rel L2 {worst:.3e} > {tol:.1e}"
+    return worst
+
+
+# ---------------------------------------------------------------------------------------------------------
+# FFT read-out: opo_get_fields(FREQ) against the oracle's own transform, every supported size
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision,log2_n", [("c64", l) for l in range(6, 15)] + [("c128", l) for l in range(6, 14)])
+def test_frequency_readout_matches_oracle_fft(precision, log2_n):
+    import oracle
+    torch, P = _gpu()
+    w = small_workload(log2_n, 2, precision, batch=2)
+    o = P.from_workload(w)
+    got = o.get_fields(1, P.WHICH_CURRENT, P.DOMAIN_FREQ).cpu().numpy().astype(np.complex128)
+    o.close()
+    for b in range(2):
+        ref = oracle.fft(w.seeds[1][b])
+        assert rel_l2(got[b], ref) <= (1e-13 if precision == "c128" else 2e-6)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# single crystal pass, every size (several tiles, ragged radix plans), both engines, dk != 0
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("engine_idx", [0, 1])
+@pytest.mark.parametrize("precision,log2_n,n_fields", [
+    ("c128", 6, 2), ("c128", 7, 3), ("c128", 9, 3), ("c128", 10, 2), ("c128", 11, 3), ("c128", 13, 3),
+    ("c64", 6, 3), ("c64", 8, 2), ("c64", 9, 3), ("c64", 10, 3), ("c64", 11, 2), ("c64", 12, 3), ("c64", 13, 3),
+    ("c64", 14, 3), ("c64", 14, 2)])
+def test_single_pass_matches_oracle(precision, log2_n, n_fields, engine_idx):
+    engine = engines()[engine_idx]
+    w = small_workload(log2_n, n_fields, precision, nz=5, dk=35.0, alpha=3.0)
+    _engine_or_skip(w, engine)
+    cur, _, eng = run_gpu(w, engine, propagate=[5])
+    assert eng == engine
+    ref, _ = run_oracle(w, propagate=[5])
+    assert_close(cur, ref, TOL[precision] if precision == "c128" else 2e-5, w.name)
+
+
+@pytest.mark.parametrize("engine_idx", [0, 1])
+def test_partial_passes_continue_dk_phase(engine_idx):
+    engine = engines()[engine_idx]
+    w = small_workload(9, 3, "c128", nz=7, dk=120.0)
+    _engine_or_skip(w, engine)
+    cur, _, _ = run_gpu(w, engine, propagate=[2, 1, 4])
+    ref, _ = run_oracle(w, propagate=[7])
+    assert_close(cur, ref, 1e-10, "partial passes")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# round trips with the full boundary operator: mirror, carrier phase, GDD, group-delay detuning,
+# per-instance sweeps; one call (half-steps merged across the boundary) and call-by-call
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("engine_idx", [0, 1])
+@pytest.mark.parametrize("precision,log2_n,n_fields,calls", [
+    ("c128", 8, 3, 1), ("c128", 8, 3, 3), ("c128", 10, 2, 1), ("c64", 11, 3, 1), ("c64", 12, 2, 3)])
+def test_roundtrips_with_boundary(precision, log2_n, n_fields, calls, engine_idx):
+    engine = engines()[engine_idx]
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=4, batch=3, dk=-20.0, gdd_dt2=-1.7, drad=0.4, strong=False)
+    # per-instance group-delay detuning of the signal in units of the grid step
+    w.delta_T_signal_s = np.array([-2.5, 0.0, 1.25]) * w.dt
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine, n_roundtrips=3, calls=calls)
+    rcur, rex = run_oracle(w, n_roundtrips=3)
+    tol = TOL[precision] if precision == "c128" else 3e-5
+    assert_close(cur, rcur, tol, "current")
+    assert_close(ex, rex, tol, "exit")
+
+
+@pytest.mark.parametrize("engine_idx", [0, 1])
+def test_boundary_without_transform_and_nonresonant_restart(engine_idx):
+    engine = engines()[engine_idx]
+    w = small_workload(9, 3, "c128", nz=3, batch=2, dk=10.0, drad=-0.7, strong=False)
+    w.resonant = [0, 1, 0]          # idler restarts from its seed every round trip (R12)
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine, n_roundtrips=4)
+    rcur, rex = run_oracle(w, n_roundtrips=4)
+    assert_close(cur, rcur, 1e-10, "current")
+    assert_close(ex, rex, 1e-10, "exit")
+    assert np.array_equal(cur[:, 0], w.pump) and np.array_equal(cur[:, 2], w.seeds[2])
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the five configurations of BASELINE.json (truncated to <= 20 round trips where they are longer)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("engine_idx", [0, 1])
+def test_config0_full_c128(engine_idx):
+    engine = engines()[engine_idx]
+    w = W.config0()
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine)
+    rcur, rex = run_oracle(w)
+    e1 = assert_close(cur, rcur, 1e-10, "C0 current")
+    e2 = assert_close(ex, rex, 1e-10, "C0 exit")
+    print(f"C0 engine {engine}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+@pytest.mark.parametrize("engine_idx", [0, 1])
+@pytest.mark.parametrize("nrt", [1, 20])
+def test_config1_c64(nrt, engine_idx):
+    engine = engines()[engine_idx]
+    w = W.config1().truncated(nrt)
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine)
+    rcur, rex = run_oracle(w)
+    e1 = assert_close(cur, rcur, 1e-4, "C1 current")
+    e2 = assert_close(ex, rex, 1e-4, "C1 exit")
+    print(f"C1 {nrt} RT engine {engine}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+@pytest.mark.parametrize("engine_idx", [0, 1])
+def test_config2_subset_c64(engine_idx):
+    engine = engines()[engine_idx]
+    w = W.config2().truncated(5).subset([0, 5, 10])
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine)
+    rcur, rex = run_oracle(w)
+    e1 = assert_close(cur, rcur, 1e-4, "C2 current")
+    e2 = assert_close(ex, rex, 1e-4, "C2 exit")
+    print(f"C2 5 RT engine {engine}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+@pytest.mark.parametrize("engine_idx", [0, 1])
+def test_config4_corners_c64(engine_idx):
+    engine = engines()[engine_idx]
+    w = W.config4(batch_side=16).truncated(5).subset([0, 15, 240, 255, 100])
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine)
+    rcur, rex = run_oracle(w)
+    e1 = assert_close(cur, rcur, 1e-4, "C4 current")
+    e2 = assert_close(ex, rex, 1e-4, "C4 exit")
+    print(f"C4 5 RT engine {engine}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# boundary behaviour of the ABI itself
+# ---------------------------------------------------------------------------------------------------------
+def test_abi_errors_and_state():
+    torch, P = _gpu()
+    w = small_workload(8, 2, "c64", nz=4)
+    o = P.from_workload(w)
+    o.propagate(3)
+    assert o.z_steps == 3
+    with pytest.raises(P.OpoError) as e:
+        o.propagate(2)                       # would pass z = L
+    assert e.value.status == P.ERR_STATE
+    with pytest.raises(P.OpoError) as e:
+        o.roundtrips(1)                      # z != 0
+    assert e.value.status == P.ERR_STATE
+    with pytest.raises(P.OpoError) as e:
+        o.set_batch_param(P.PARAM_DK, 0, [1.0, 2.0])     # count != batch
+    assert e.value.status == P.ERR_INVALID_ARG
+    o.check_finite()
+    o.close()
+    with pytest.raises(P.OpoError) as e:
+        bad = small_workload(8, 2, "c64")
+        bad.resonant = [1, 1]
+        P.from_workload(bad)
+    assert e.value.status == P.ERR_UNSUPPORTED
+    with pytest.raises(P.OpoError) as e:
+        bad = small_workload(8, 2, "c64")
+        bad.R = [0.0, 1.5]
+        P.from_workload(bad)
+    assert e.value.status == P.ERR_INVALID_ARG
+
+
+def test_nonfinite_is_reported_when_dz_too_coarse():
+    """too coarse a dz makes the fields blow up to NaN; the ABI reports it."""
+    torch, P = _gpu()
+    w = small_workload(8, 2, "c64", nz=1)
+    w.pump = w.pump * 1e4
+    w.length_m *= 50
+    o = P.from_workload(w)
+    o.roundtrips(30)
+    with pytest.raises(P.OpoError) as e:
+        o.check_finite()
+    assert e.value.status == P.ERR_NONFINITE
+    o.close()
+
+
+def test_host_buffer_calls_match_device_calls():
+    torch, P = _gpu()
+    w = small_workload(10, 3, "c64", nz=4, batch=2)
+    a = P.from_workload(w)
+    b = P.from_workload(w, host_inputs=True)
+    a.roundtrips(2)
+    b.roundtrips(2)
+    for x in range(3):
+        da = a.get_fields(x).cpu()
+        hb = torch.empty((2, w.n), dtype=torch.complex64).pin_memory()
+        b.get_fields(x, out=hb)
+        assert torch.equal(da, hb)
+    a.close()
+    b.close()
