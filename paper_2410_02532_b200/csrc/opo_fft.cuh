@@ -78,28 +78,59 @@ template <int R, int J> struct root {
     static constexpr double s = (m <= 8) ? cos32(8 - m) : cos32(m - 8);   // sin >= 0
 };
 
+// x * c for a compile-time constant c.  fp32: c is carried as hi + lo so that the product has no
+// systematic (constant-rounding) bias -- a biased |w| != 1 inside every butterfly would change the
+// field amplitude by ~1e-8 per transform, coherently, and thousands of z-steps add up.
+template <class T> struct kconst;
+template <> struct kconst<double> {
+    template <class C> static __device__ __forceinline__ double mul(double x, C) { return x * C::value; }
+    // x * C1 + y * C2
+    template <class C1, class C2> static __device__ __forceinline__ double dot(double x, C1, double y, C2) {
+        return x * C1::value + y * C2::value;
+    }
+};
+template <> struct kconst<float> {
+    template <class C> static __device__ __forceinline__ float mul(float x, C) {
+        constexpr float hi = (float)C::value;
+        constexpr float lo = (float)(C::value - (double)hi);
+        return __fmaf_rn(x, hi, x * lo);
+    }
+    template <class C1, class C2> static __device__ __forceinline__ float dot(float x, C1, float y, C2) {
+        constexpr float h1 = (float)C1::value, l1 = (float)(C1::value - (double)h1);
+        constexpr float h2 = (float)C2::value, l2 = (float)(C2::value - (double)h2);
+        float t = x * l1;
+        t = __fmaf_rn(y, l2, t);
+        t = __fmaf_rn(x, h1, t);
+        return __fmaf_rn(y, h2, t);
+    }
+};
+struct c_sqrt_half { static constexpr double value = 0.70710678118654752440084436210485; };
+template <int R, int J, bool NEG> struct c_cos { static constexpr double value = NEG ? -root<R, J>::c : root<R, J>::c; };
+template <int R, int J, bool NEG> struct c_sin { static constexpr double value = NEG ? -root<R, J>::s : root<R, J>::s; };
+
 // a * w_R^J (forward) or a * conj(w_R^J) (INV)
 template <class T, int R, int J, bool INV>
 __device__ __forceinline__ cplx<T> mul_root(cplx<T> a) {
+    using K = kconst<T>;
     if constexpr (J == 0) {
         return a;
     } else if constexpr (4 * J == R) {            // w = -i
         if constexpr (INV) return {-a.im, a.re};
         else return {a.im, -a.re};
     } else if constexpr (8 * J == R) {            // w = (1 - i)/sqrt2
-        constexpr T h = (T)0.70710678118654752440084436210485;
-        if constexpr (INV) return {(a.re - a.im) * h, (a.re + a.im) * h};
-        else return {(a.re + a.im) * h, (a.im - a.re) * h};
+        if constexpr (INV) return {K::mul(a.re - a.im, c_sqrt_half{}), K::mul(a.re + a.im, c_sqrt_half{})};
+        else return {K::mul(a.re + a.im, c_sqrt_half{}), K::mul(a.im - a.re, c_sqrt_half{})};
     } else if constexpr (8 * J == 3 * R) {        // w = (-1 - i)/sqrt2
-        constexpr T h = (T)0.70710678118654752440084436210485;
-        if constexpr (INV) return {(-a.re - a.im) * h, (a.re - a.im) * h};
-        else return {(a.im - a.re) * h, (-a.re - a.im) * h};
+        if constexpr (INV) return {K::mul(-a.re - a.im, c_sqrt_half{}), K::mul(a.re - a.im, c_sqrt_half{})};
+        else return {K::mul(a.im - a.re, c_sqrt_half{}), K::mul(-a.re - a.im, c_sqrt_half{})};
     } else {
-        constexpr T c = (T)root<R, J>::c;
-        constexpr T s = (T)root<R, J>::s;
         // forward: w = c - i s ; inverse: conj(w) = c + i s
-        if constexpr (INV) return {a.re * c - a.im * s, a.im * c + a.re * s};
-        else return {a.re * c + a.im * s, a.im * c - a.re * s};
+        if constexpr (INV)
+            return {K::dot(a.re, c_cos<R, J, false>{}, a.im, c_sin<R, J, true>{}),
+                    K::dot(a.im, c_cos<R, J, false>{}, a.re, c_sin<R, J, false>{})};
+        else
+            return {K::dot(a.re, c_cos<R, J, false>{}, a.im, c_sin<R, J, false>{}),
+                    K::dot(a.im, c_cos<R, J, false>{}, a.re, c_sin<R, J, true>{})};
     }
 }
 
@@ -293,9 +324,10 @@ __device__ __forceinline__ void forward_only_smem(cplx<T>* sm, const cplx<T>* tw
     fwd_pass_smem<T, L, plan<L>::P - 1, NT>(sm, tw, tid);
 }
 
-// threads per CTA for a 2^L-point field: 32 points per thread for fp32, 16 for fp64
+// threads per CTA for a 2^L-point field: 32 points per thread for large fields (keeps the register
+// budget at 128+/thread for the radix-16 butterflies), 16 for small ones
 template <class T, int L> struct cta_threads {
-    static constexpr int per = (sizeof(T) == 4) ? 32 : 16;
+    static constexpr int per = (L >= 11) ? 32 : 16;
     static constexpr int raw = (1 << L) / per;
     static constexpr int value = raw < 32 ? 32 : raw;
 };
