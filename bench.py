@@ -1,0 +1,295 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the SSFM/OPO hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4|C1]
+
+One "step" = the whole hot path over one batch: `rt_per_step` cavity round trips (each = nz z-steps
+of FFT . dispersion . IFFT + RK4, then the boundary operator) of every instance of the workload.
+Default workload: BASELINE.json configs[4] (256 independent N = 2^14 three-wave OPOs, 100 z-steps,
+300 round trips -- the batched N = 2^14 case the roofline target is quoted on); `--workload C1` runs
+configs[1] (the same OPO, a single instance: latency-bound, 3 of 148 SMs).
+
+Prints ONE JSON line (rank 0).  `value` = grid-point z-steps/s with inputs resident in HBM;
+`e2e` = the same through the host-buffer ABI calls (H2D of pump and seeds, D2H of the exit signal
+inside the timed region); `roofline` = the resident kernel against the FP32-pipe peak;
+`cpu_baseline` = the fp64 oracle on this host's cores on a bounded sample.
+`--impl reference` times the oracle instead (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import opo_workloads as W
+
+METRIC = "ssfm_grid_point_z_steps_per_s"
+UNIT = "grid-point z-steps/s"
+# flops per field-point z-step of the scheme actually executed (half-steps merged): 2 transforms
+# x 5 log2(N) + table multiply 6 + RK4 76
+def flops_per_grid_point_zstep(log2_n: int, n_fields: int) -> float:
+    return n_fields * (2 * 5 * log2_n + 6 + 76)
+
+
+def make_workload(name: str, rank: int):
+    if name == "C4":
+        w = W.config4()
+    elif name == "C1":
+        w = W.config1()
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    if rank:   # other ranks run their own sweep with their own seeds (weak scaling, no collective)
+        rng = np.random.default_rng(1000 + rank)
+        for x in range(1, w.n_fields):
+            w.seeds[x] = W._round_to_precision(np.roll(w.seeds[x], 17 * rank, axis=1) * np.exp(2j * np.pi * rng.random()), w.precision)
+    return w
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.t = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        for ln in self.lines:
+            p = [s.strip() for s in ln.split(",")]
+            if len(p) < 9:
+                continue
+            try:
+                sm.append(float(p[1])); mx.append(float(p[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def run_reference(args, rank, world):
+    """The oracle as it stands, on this host's cores, on a bounded sample of the same workload."""
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    w = make_workload(args.workload, 0)
+    cores = os.cpu_count() or 1
+    inst = list(range(min(w.batch, cores)))
+    # ~0.6 s per round trip per core at N = 2^14, nz = 100: one round trip per instance per step
+    rt = 1
+    sample = f"{len(inst)} instance(s) x {rt} round trip(s) of {w.name}, one thread per instance"
+
+    def step():
+        oracle.run_workload(w, n_roundtrips=rt, instances=inst, threads=len(inst))
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    val = len(inst) * w.n * w.nz_per_pass * rt / dt
+    line = {"metric": METRIC, "value": val, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name} (BASELINE.json configs[{4 if args.workload == 'C4' else 1}])", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": len(inst), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "round_trips_per_s": len(inst) * rt / dt, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(w, budget_s=15.0):
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    inst = list(range(min(w.batch, cores)))
+    t0 = time.perf_counter()
+    oracle.run_workload(w, n_roundtrips=1, instances=inst[:1], threads=1)
+    t1 = time.perf_counter() - t0                    # one round trip, one core
+    rt = max(1, int(budget_s / max(t1, 1e-3)))
+    rt = min(rt, 25)
+    t0 = time.perf_counter()
+    oracle.run_workload(w, n_roundtrips=rt, instances=inst, threads=len(inst))
+    dt = time.perf_counter() - t0
+    return {"value": len(inst) * w.n * w.nz_per_pass * rt / dt, "unit": UNIT, "cores": len(inst), "kind": "oracle",
+            "sample": f"{len(inst)} instance(s) x {rt} round trip(s) of {w.name}, one thread per instance, {dt:.1f} s",
+            "round_trips_per_s": len(inst) * rt / dt}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4", choices=["C4", "C1"])
+    ap.add_argument("--rt-per-step", type=int, default=0, help="round trips per step (default: the config's full length for C4, 100 for C1)")
+    ap.add_argument("--engine", default="auto", choices=["auto", "resident", "streaming"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    import torch.distributed as dist
+    import paper_2410_02532_b200 as P
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload(args.workload, rank)
+    rt_per_step = args.rt_per_step or (w.n_roundtrips if args.workload == "C4" else 100)
+    engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "streaming": P.ENGINE_STREAMING}[args.engine]
+    o = P.from_workload(w, engine=engine)
+    units_per_step = w.batch * w.n * w.nz_per_pass * rt_per_step          # grid-point z-steps, this rank
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
+
+    # pinned host copies of the step's inputs / output for the e2e leg
+    dt_t = o.dtype
+    h_pump = torch.from_numpy(np.ascontiguousarray(w.pump)).to(dt_t).contiguous().pin_memory()
+    h_seeds = [None] + [torch.from_numpy(np.ascontiguousarray(w.seeds[x])).to(dt_t).contiguous().pin_memory() for x in range(1, w.n_fields)]
+    h_out = torch.empty((w.batch, w.n), dtype=dt_t).pin_memory()
+    d_pump = h_pump.cuda()
+    d_seeds = [None] + [h_seeds[x].cuda() for x in range(1, w.n_fields)]
+
+    def reset_device_inputs():
+        o.set_pump(d_pump if d_pump.shape[0] > 1 else d_pump[0].contiguous())
+        for x in range(1, w.n_fields):
+            o.set_field(x, d_seeds[x])
+
+    def step_resident_inputs():
+        o.roundtrips(rt_per_step)
+
+    def step_e2e():
+        o.set_pump(h_pump if h_pump.shape[0] > 1 else h_pump[0])
+        for x in range(1, w.n_fields):
+            o.set_field(x, h_seeds[x])
+        o.roundtrips(rt_per_step)
+        o.get_fields(1, P.WHICH_EXIT, P.DOMAIN_TIME, out=h_out)          # D2H + stream sync inside
+
+    # ---- device-resident timing -------------------------------------------------------------------------
+    for _ in range(args.warmup):
+        reset_device_inputs(); step_resident_inputs()
+    barrier()
+    launches0 = o.launches
+    sampler = ClockSampler(local_rank); sampler.start()
+    evs = []
+    t_wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        reset_device_inputs()                      # untimed: state back to the seeds (same work every step)
+        flush.fill_(1)                             # untimed: evict L2 between timed iterations
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); step_resident_inputs(); e1.record()
+        evs.append((e0, e1))
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    launches = o.launches - launches0
+    per_step_ms = [a.elapsed_time(b) for a, b in evs]
+    t_local = sum(per_step_ms) * 1e-3
+    tt = torch.tensor([t_local], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_total = float(tt.item())
+    value = world * units_per_step * args.steps / t_total
+    o.check_finite()
+
+    # ---- end-to-end timing (host buffers through the ABI) ---------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        step_e2e()
+        barrier()
+        t0 = time.perf_counter()
+        e2e_steps = max(1, min(args.steps, 3))
+        for _ in range(e2e_steps):
+            step_e2e()
+        barrier()
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        esz = 16 if w.precision == "c128" else 8
+        h2d = (h_pump.numel() + sum(h_seeds[x].numel() for x in range(1, w.n_fields))) * esz
+        e2e = {"value": world * units_per_step * e2e_steps / float(te.item()), "unit": UNIT,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(h_out.numel() * esz), "steps": e2e_steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (resident engine: FP32 pipe) ----------------------------------
+    fl = flops_per_grid_point_zstep(w.log2_n, w.n_fields) * units_per_step          # per launch (= per step)
+    avg_s = statistics.mean(per_step_ms) * 1e-3
+    peak_tflops = 148 * 128 * 2 * 1.965e9 / 1e12
+    roofline = {"bound": "alu", "kernel": "k_resident" if o.engine == P.ENGINE_RESIDENT else "k_linear+k_rk4",
+                "achieved": fl / avg_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s", "frac": fl / avg_s / 1e12 / peak_tflops,
+                "traffic": None,
+                "note": "FP32 FMA-pipe peak = 148 SM x 128 lanes x 2 x 1.965 GHz (guide unit counts, max clock); algorithmic flops = "
+                        f"{flops_per_grid_point_zstep(w.log2_n, w.n_fields):.0f}/grid-point z-step (merged half-steps, 5 N log2 N per transform)"}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if w.precision == "c64" else "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name}: BASELINE.json configs[{4 if args.workload == 'C4' else 1}], batch {w.batch} x N=2^{w.log2_n} x "
+                                   f"{w.n_fields} fields, nz={w.nz_per_pass}, {rt_per_step} round trips per step",
+                       "engine": "resident" if o.engine == P.ENGINE_RESIDENT else "streaming",
+                       "l2": "512 MiB flush write between timed steps", "sharding": "independent instances per rank, no collective"},
+            "round_trips_per_s": world * w.batch * rt_per_step * args.steps / t_total,
+            "field_point_z_steps_per_s": value * w.n_fields,
+            "clocks": clocks, "gpu_launches": int(launches), "wall_s_timed_region": t_wall,
+            "roofline": roofline}
+    if e2e:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(w)
+    print(json.dumps(line), flush=True)
+    o.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
