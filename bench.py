@@ -55,6 +55,21 @@ def make_workload(name: str, rank: int):
     return w
 
 
+def max_over_ranks(t_local: float, world: int, device="cuda") -> float:
+    """Job time = the slowest rank's device time (no other collective exists on this path)."""
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([t_local], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def job_throughput(units_per_step_per_rank: int, steps: int, world: int, t_total: float) -> float:
+    """Whole-job aggregate: every rank processes the same number of units (weak scaling)."""
+    return world * units_per_step_per_rank * steps / t_total
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -231,11 +246,8 @@ def main():
     launches = o.launches - launches0
     per_step_ms = [a.elapsed_time(b) for a, b in evs]
     t_local = sum(per_step_ms) * 1e-3
-    tt = torch.tensor([t_local], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_total = float(tt.item())
-    value = world * units_per_step * args.steps / t_total
+    t_total = max_over_ranks(t_local, world)
+    value = job_throughput(units_per_step, args.steps, world, t_total)
     o.check_finite()
 
     # ---- end-to-end timing (host buffers through the ABI) ---------------------------------------------------
@@ -248,12 +260,10 @@ def main():
         for _ in range(e2e_steps):
             step_e2e()
         barrier()
-        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        te = max_over_ranks(time.perf_counter() - t0, world)
         esz = 16 if w.precision == "c128" else 8
         h2d = (h_pump.numel() + sum(h_seeds[x].numel() for x in range(1, w.n_fields))) * esz
-        e2e = {"value": world * units_per_step * e2e_steps / float(te.item()), "unit": UNIT,
+        e2e = {"value": job_throughput(units_per_step, e2e_steps, world, te), "unit": UNIT,
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(h_out.numel() * esz), "steps": e2e_steps}
 
     if rank != 0:
