@@ -16,7 +16,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libopo.so")
-SOURCES = ["opo_api.cu", "opo_inst_f32.cu", "opo_inst_f64.cu"]
+PLAIN_SOURCES = ["opo_api.cu", "opo_dispatch.cu", "opo_pointwise.cu"]
+# (type, suffix, log2 N): one object per size-specialised instance of opo_inst.cu
+INSTANCES = [("float", "f32", l) for l in range(6, 15)] + [("double", "f64", l) for l in range(6, 14)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -34,26 +36,44 @@ def _newest_source_mtime() -> float:
     return max(os.path.getmtime(p) for p in paths)
 
 
+def _jobs(only=None):
+    jobs = [(src, src.replace(".cu", ".o"), []) for src in PLAIN_SOURCES]
+    for typ, suf, l in INSTANCES:
+        if only and f"{suf}:{l}" not in only:
+            continue
+        jobs.append(("opo_inst.cu", f"opo_inst_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
+    return jobs
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source_mtime():
+    """Compile every CUDA source for sm_100a and link libopo.so.  OPO_BUILD_ONLY="f32:14,f64:10"
+    (development only) restricts the size-specialised instances; sizes left out report
+    OPO_ERR_UNSUPPORTED at opo_create."""
+    only = os.environ.get("OPO_BUILD_ONLY")
+    only = set(only.split(",")) if only else None
+    if not force and not only and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source_mtime():
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
+    newest = _newest_source_mtime()
 
-    def compile_one(src: str) -> str:
-        obj = os.path.join(OBJ, src.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+    def compile_one(job) -> str:
+        src, objname, defs = job
+        obj = os.path.join(OBJ, objname)
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) >= newest:
+            return obj
+        cmd = [nvcc, *NVCC_FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", obj]
         res = subprocess.run(cmd, capture_output=True, text=True)
         with open(obj + ".log", "w") as f:
             f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
         if res.returncode != 0:
-            raise RuntimeError(f"nvcc failed on {src}:\n{res.stdout}\n{res.stderr}")
+            raise RuntimeError(f"nvcc failed on {src} {defs}:\n{res.stdout}\n{res.stderr}")
         if verbose:
             print(res.stderr)
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(compile_one, SOURCES))
+    with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
+        objs = list(ex.map(compile_one, _jobs(only)))
     cmd = [nvcc, "-shared", "-o", LIB, *objs, "-cudart", "static"]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:

@@ -29,14 +29,18 @@ struct HostPlan {
     int rbits[8] = {0}, sbits[8] = {0}, tw_offset[9] = {0};
     int tw_total = 0;
     explicit HostPlan(int L_) : L(L_) {
-        const int rem = L % 4;
-        const int n16 = (rem == 1) ? (L / 4 - 1) : (L / 4);
-        P = n16 + (rem == 0 ? 0 : (rem == 1 ? 2 : 1));
+        // pass 0: radix 4; the remaining L - 2 bits: radix 16 as often as possible, then 8 / 4
+        const int L1 = L - 2;
+        const int rem = L1 % 4;
+        const int n16 = (rem == 1) ? (L1 / 4 - 1) : (L1 / 4);
+        P = 1 + n16 + (rem == 0 ? 0 : (rem == 1 ? 2 : 1));
         int used = 0, off = 0;
         for (int p = 0; p < P; ++p) {
             int rb;
-            if (p < n16) rb = 4;
-            else if (rem == 1) rb = (p == n16) ? 3 : 2;
+            const int q = p - 1;
+            if (p == 0) rb = 2;
+            else if (q < n16) rb = 4;
+            else if (rem == 1) rb = (q == n16) ? 3 : 2;
             else if (rem == 2) rb = 2;
             else rb = 3;
             rbits[p] = rb;

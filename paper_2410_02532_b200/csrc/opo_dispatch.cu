@@ -1,0 +1,43 @@
+// opo_dispatch.cu -- routes the size-templated launchers to the per-(precision, log2 N) translation
+// units (opo_inst.cu).  The instances are declared weak: a size that was not built simply reports
+// cudaErrorNotSupported (opo_create turns that into OPO_ERR_UNSUPPORTED).
+#include "opo_internal.h"
+
+namespace opo {
+
+#define OPO_DECL(SUF, LL)                                                                                     \
+    cudaError_t launch_linear_##SUF##_L##LL(const LinArgs&, cudaStream_t) __attribute__((weak));              \
+    cudaError_t launch_freq_##SUF##_L##LL(const FreqArgs&, cudaStream_t) __attribute__((weak));               \
+    cudaError_t resident_info_##SUF##_L##LL(int, ResidentInfo*) __attribute__((weak));                        \
+    cudaError_t launch_resident_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
+
+#define OPO_DECL_ALL(SUF) \
+    OPO_DECL(SUF, 6) OPO_DECL(SUF, 7) OPO_DECL(SUF, 8) OPO_DECL(SUF, 9) OPO_DECL(SUF, 10) OPO_DECL(SUF, 11) \
+    OPO_DECL(SUF, 12) OPO_DECL(SUF, 13) OPO_DECL(SUF, 14)
+
+OPO_DECL_ALL(f32)
+OPO_DECL_ALL(f64)
+
+#define OPO_CASE(FN, SUF, LL, ...) \
+    case LL: return FN##SUF##_L##LL ? FN##SUF##_L##LL(__VA_ARGS__) : cudaErrorNotSupported;
+
+#define OPO_SWITCH(FN, SUF, log2n, ...)                                                            \
+    switch (log2n) {                                                                               \
+        OPO_CASE(FN, SUF, 6, __VA_ARGS__) OPO_CASE(FN, SUF, 7, __VA_ARGS__) OPO_CASE(FN, SUF, 8, __VA_ARGS__)    \
+        OPO_CASE(FN, SUF, 9, __VA_ARGS__) OPO_CASE(FN, SUF, 10, __VA_ARGS__) OPO_CASE(FN, SUF, 11, __VA_ARGS__)  \
+        OPO_CASE(FN, SUF, 12, __VA_ARGS__) OPO_CASE(FN, SUF, 13, __VA_ARGS__) OPO_CASE(FN, SUF, 14, __VA_ARGS__) \
+        default: return cudaErrorNotSupported;                                                     \
+    }
+
+#define OPO_DISPATCHERS(SUF)                                                                                      \
+    cudaError_t launch_linear_##SUF(int log2n, const LinArgs& a, cudaStream_t s) { OPO_SWITCH(launch_linear_, SUF, log2n, a, s) } \
+    cudaError_t launch_freq_##SUF(int log2n, const FreqArgs& a, cudaStream_t s) { OPO_SWITCH(launch_freq_, SUF, log2n, a, s) }   \
+    cudaError_t resident_info_##SUF(int log2n, int n_fields, ResidentInfo* out) { OPO_SWITCH(resident_info_, SUF, log2n, n_fields, out) } \
+    cudaError_t launch_resident_##SUF(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s) {        \
+        OPO_SWITCH(launch_resident_, SUF, log2n, a, n_clusters, s)                                                \
+    }
+
+OPO_DISPATCHERS(f32)
+OPO_DISPATCHERS(f64)
+
+}  // namespace opo

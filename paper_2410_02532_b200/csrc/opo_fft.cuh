@@ -4,20 +4,28 @@
 //     A <- IDFT( H .* DFT(A) ).
 // This file provides it as ONE pass structure over a field held in shared memory:
 //
-//   forward  : decimation-in-frequency passes p = 1..P (radix R_p, N = R_1 ... R_P); natural order
-//              in, digit-reversed order out, so no reordering pass is ever executed;
+//   forward  : decimation-in-frequency passes p = 0..P-1 (radix R_p, N = R_0 ... R_{P-1}); natural
+//              order in, digit-reversed order out, so no reordering pass is ever executed;
 //   multiply : in registers, against a table that the host stored in the digit-reversed order;
-//   inverse  : the exact adjoint factorisation (decimation-in-time, passes P..1, conjugate
+//   inverse  : the exact adjoint factorisation (decimation-in-time, passes P-1..0, conjugate
 //              twiddles), digit-reversed in, natural order out.
 //
-// The last forward pass, the table multiply and the first inverse pass run on registers without
-// touching shared memory.  Because the inverse is the adjoint of the forward factorisation using
-// the *same* rounded twiddles, twiddle phase rounding cancels between the two transforms and
-// does not accumulate over thousands of z-steps; only twiddle magnitude rounding can, and the
-// host picks table roundings that minimise | |w| - 1 | ("fp32 error budget").
+// Pass 0 has radix 4 and is special: its butterflies touch x[t + j N/4], j = 0..3, and nothing else,
+// in both directions.  The resident engine (opo_resident.cuh) therefore runs "inverse pass 0 -> RK4
+// on those four grid points -> forward pass 0" on registers, for all coupled fields at once -- the
+// nonlinear step costs no shared-memory pass of its own.  Passes 1..P-2 are radix-16 (8/4 for the
+// remainder) shared-memory passes; the last forward pass, the table multiply and the first inverse
+// pass ("mid") also run on registers without touching shared memory in between.
+//
+// Because the inverse is the adjoint of the forward factorisation using the *same* rounded
+// twiddles, twiddle phase rounding cancels between the two transforms and does not accumulate
+// over thousands of z-steps; only twiddle magnitude rounding can, and the host picks table
+// roundings that minimise | |w| - 1 | ("fp32 error budget").
 //
 // Shared-memory layout: element i lives at i + (i >> PADSH) (one pad element per 16 float2 / per
-// 8 double2), which makes every pass -- including the stride-R last one -- bank-conflict free.
+// 8 double2, i.e. per 128 bytes), which makes every pass -- including the unit-stride last one --
+// bank-conflict free.  All element addresses of a butterfly are one runtime base plus
+// compile-time offsets (elem_addr below).
 #pragma once
 #include <cuda_runtime.h>
 #include <utility>
@@ -48,6 +56,11 @@ __device__ __forceinline__ cplx<float> ldg(const cplx<float>* p) {
 __device__ __forceinline__ cplx<double> ldg(const cplx<double>* p) {
     double2 v = __ldg(reinterpret_cast<const double2*>(p));
     return {v.x, v.y};
+}
+// twiddle fetch: SMEM = plain load from a shared-memory copy, otherwise read-only global load
+template <bool SMEM, class T> __device__ __forceinline__ cplx<T> ldtw(const cplx<T>* p) {
+    if constexpr (SMEM) return *p;
+    else return ldg(p);
 }
 
 template <class T> struct pad_shift;
@@ -187,16 +200,20 @@ template <class T, int R> struct dit_inv {
 template <class T> struct dit_inv<T, 1> { static __device__ __forceinline__ void run(cplx<T>*) {} };
 
 // ---- radix plan ------------------------------------------------------------------------------------
-// N = 2^L split into passes of radix 16 (as many as possible) then 8 / 4; never a radix-2 pass
-// for L >= 6:   L%4 == 0: 16..16 | 1: 16..16,8,4 | 2: 16..16,4 | 3: 16..16,8
+// N = 2^L: pass 0 has radix 4 (the RK4-fused exchange pass); the remaining L - 2 bits are split into
+// radix-16 passes (as many as possible) then 8 / 4, never radix 2:
+//   (L-2)%4 == 0: 16..16 | 1: 16..16,8,4 | 2: 16..16,4 | 3: 16..16,8
 template <int L> struct plan {
     static_assert(L >= 6 && L <= 14, "shared-memory FFT supports 2^6 .. 2^14");
-    static constexpr int rem = L % 4;
-    static constexpr int n16 = (rem == 1) ? (L / 4 - 1) : (L / 4);
-    static constexpr int P = n16 + (rem == 0 ? 0 : (rem == 1 ? 2 : 1));
+    static constexpr int L1 = L - 2;
+    static constexpr int rem = L1 % 4;
+    static constexpr int n16 = (rem == 1) ? (L1 / 4 - 1) : (L1 / 4);
+    static constexpr int P = 1 + n16 + (rem == 0 ? 0 : (rem == 1 ? 2 : 1));
     __host__ __device__ static constexpr int rbits(int p) {   // p = 0 .. P-1
-        if (p < n16) return 4;
-        if (rem == 1) return (p == n16) ? 3 : 2;
+        if (p == 0) return 2;
+        const int q = p - 1;
+        if (q < n16) return 4;
+        if (rem == 1) return (q == n16) ? 3 : 2;
         if (rem == 2) return 2;
         return 3;   // rem == 3
     }
@@ -206,18 +223,40 @@ template <int L> struct plan {
         for (int q = 0; q <= p; ++q) used += rbits(q);
         return L - used;
     }
-    // offset (in complex elements) of pass p's twiddle block W_p[k-1][t'] inside the twiddle table
+    // offset (in complex elements) of pass p's twiddle block W_p[k-1][t] inside the twiddle table
     __host__ __device__ static constexpr int tw_offset(int p) {
         int off = 0;
         for (int q = 0; q < p; ++q) off += ((1 << rbits(q)) - 1) << sbits(q);
         return off;
     }
     static constexpr int tw_total = tw_offset(P);
+    // twiddles of the shared-memory passes 1 .. P-2 (the last pass has none): one contiguous block
+    static constexpr int tw_local_begin = tw_offset(1);
+    static constexpr int tw_local_count = tw_offset(P - 1) - tw_offset(1);
 };
+
+// Address (in elements of the padded array) of butterfly input j, j = 0..R-1, of the butterfly
+// (b, t) of a pass with R = 2^RB, S = 2^SB: logical index (b << (SB+RB)) + (j << SB) + t.
+// Returns the runtime part; elem_off<..>(j) is the compile-time part.
+template <class T, int RB, int SB>
+__device__ __forceinline__ int elem_base(int b, int t) {
+    constexpr int PS = pad_shift<T>::value;
+    const int base = (b << (SB + RB)) + t;
+    if constexpr (SB >= PS) return base + (base >> PS);
+    else if constexpr (SB + RB >= PS) return base + (b << (SB + RB - PS));
+    else return base + (b >> (PS - SB - RB));
+}
+template <class T, int RB, int SB>
+__device__ __forceinline__ constexpr int elem_off(int j) {
+    constexpr int PS = pad_shift<T>::value;
+    if constexpr (SB >= PS) return j * ((1 << SB) + (1 << (SB - PS)));
+    else if constexpr (SB + RB >= PS) return (j << SB) + (j >> (PS - SB));
+    else return j << SB;
+}
 
 // ---- one forward (DIF) pass over shared memory -------------------------------------------------------
 // butterflies u = tid, tid + NT, ...;  b = u >> sbits, t = u & (S-1); element j at b*M + j*S + t.
-template <class T, int L, int PASS, int NT>
+template <class T, int L, int PASS, int NT, bool TWS>
 __device__ __forceinline__ void fwd_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid) {
     using PL = plan<L>;
     constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
@@ -226,22 +265,22 @@ __device__ __forceinline__ void fwd_pass_smem(cplx<T>* __restrict__ sm, const cp
 #pragma unroll 1
     for (int u = tid; u < NBF; u += NT) {
         const int b = u >> SB, t = u & (S - 1);
-        const int base = (b << (SB + RB)) + t;
+        cplx<T>* __restrict__ p = sm + elem_base<T, RB, SB>(b, t);
         cplx<T> v[R];
 #pragma unroll
-        for (int j = 0; j < R; ++j) v[j] = sm[phys<T>(base + (j << SB))];
+        for (int j = 0; j < R; ++j) v[j] = p[elem_off<T, RB, SB>(j)];
         dif<T, R>::run(v);
         if constexpr (SB > 0) {
 #pragma unroll
-            for (int k = 1; k < R; ++k) v[k] = cmul(v[k], ldg(&w[((k - 1) << SB) + t]));
+            for (int k = 1; k < R; ++k) v[k] = cmul(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
         }
 #pragma unroll
-        for (int k = 0; k < R; ++k) sm[phys<T>(base + (k << SB))] = v[k];
+        for (int k = 0; k < R; ++k) p[elem_off<T, RB, SB>(k)] = v[k];
     }
 }
 
 // ---- one inverse (DIT) pass over shared memory ---------------------------------------------------------
-template <class T, int L, int PASS, int NT>
+template <class T, int L, int PASS, int NT, bool TWS>
 __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid) {
     using PL = plan<L>;
     constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
@@ -250,23 +289,24 @@ __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cp
 #pragma unroll 1
     for (int u = tid; u < NBF; u += NT) {
         const int b = u >> SB, t = u & (S - 1);
-        const int base = (b << (SB + RB)) + t;
+        cplx<T>* __restrict__ p = sm + elem_base<T, RB, SB>(b, t);
         cplx<T> v[R];
 #pragma unroll
-        for (int k = 0; k < R; ++k) v[k] = sm[phys<T>(base + (k << SB))];
+        for (int k = 0; k < R; ++k) v[k] = p[elem_off<T, RB, SB>(k)];
         if constexpr (SB > 0) {
 #pragma unroll
-            for (int k = 1; k < R; ++k) v[k] = cmulc(v[k], ldg(&w[((k - 1) << SB) + t]));
+            for (int k = 1; k < R; ++k) v[k] = cmulc(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
         }
         dit_inv<T, R>::run(v);
 #pragma unroll
-        for (int j = 0; j < R; ++j) sm[phys<T>(base + (j << SB))] = v[j];
+        for (int j = 0; j < R; ++j) p[elem_off<T, RB, SB>(j)] = v[j];
     }
 }
 
 // ---- the fused middle: last forward pass, table multiply, first inverse pass, all in registers ----------
 // The last pass has S = 1: butterfly u owns positions u*R .. u*R + R-1.  The table is stored as
-// tab[k * (N/R) + u] so that consecutive threads read consecutive addresses.
+// tab[k * (N/R) + u] so that consecutive threads read consecutive addresses; it streams from L2 and
+// its loads are issued before the shared-memory loads of the same butterfly.
 template <class T, int L, int NT>
 __device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab, int tid) {
     using PL = plan<L>;
@@ -276,52 +316,80 @@ __device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const cp
     constexpr int NBF = (1 << L) / R;
 #pragma unroll 1
     for (int u = tid; u < NBF; u += NT) {
-        const int base = u << RB;
+        cplx<T> h[R];
+#pragma unroll
+        for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
+        cplx<T>* __restrict__ p = sm + elem_base<T, RB, 0>(u, 0);
         cplx<T> v[R];
 #pragma unroll
-        for (int j = 0; j < R; ++j) v[j] = sm[phys<T>(base + j)];
+        for (int j = 0; j < R; ++j) v[j] = p[elem_off<T, RB, 0>(j)];
         dif<T, R>::run(v);
 #pragma unroll
-        for (int k = 0; k < R; ++k) v[k] = cmul(v[k], ldg(&tab[k * NBF + u]));
+        for (int k = 0; k < R; ++k) v[k] = cmul(v[k], h[k]);
         dit_inv<T, R>::run(v);
 #pragma unroll
-        for (int j = 0; j < R; ++j) sm[phys<T>(base + j)] = v[j];
+        for (int j = 0; j < R; ++j) p[elem_off<T, RB, 0>(j)] = v[j];
     }
 }
 
-// forward passes 0 .. P-2 (everything before the fused middle), with the barriers between them
-template <class T, int L, int NT, int PASS = 0>
+// forward passes FIRST .. P-2 (everything before the fused middle), with the barriers between them
+template <class T, int L, int NT, bool TWS, int PASS>
 __device__ __forceinline__ void fwd_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
     if constexpr (PASS < plan<L>::P - 1) {
-        fwd_pass_smem<T, L, PASS, NT>(sm, tw, tid);
+        fwd_pass_smem<T, L, PASS, NT, TWS>(sm, tw, tid);
         __syncthreads();
-        fwd_passes<T, L, NT, PASS + 1>(sm, tw, tid);
+        fwd_passes<T, L, NT, TWS, PASS + 1>(sm, tw, tid);
     }
 }
-// inverse passes P-2 .. 0
-template <class T, int L, int NT, int PASS = plan<L>::P - 2>
+// inverse passes P-2 .. LAST
+template <class T, int L, int NT, bool TWS, int LAST, int PASS = plan<L>::P - 2>
 __device__ __forceinline__ void inv_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
-    if constexpr (PASS >= 0) {
+    if constexpr (PASS >= LAST) {
         __syncthreads();
-        inv_pass_smem<T, L, PASS, NT>(sm, tw, tid);
-        inv_passes<T, L, NT, PASS - 1>(sm, tw, tid);
+        inv_pass_smem<T, L, PASS, NT, TWS>(sm, tw, tid);
+        inv_passes<T, L, NT, TWS, LAST, PASS - 1>(sm, tw, tid);
     }
 }
 
-// A <- IDFT( tab .* DFT(A) ) on a field in (padded) shared memory.  Caller guarantees the field is
-// visible to all threads on entry (barrier) and must barrier before reading the result.
+// A <- IDFT( tab .* DFT(A) ) on a field in (padded) shared memory, twiddles from global memory.
+// Caller guarantees the field is visible to all threads on entry (barrier) and must barrier before
+// reading the result.
 template <class T, int L, int NT>
 __device__ __forceinline__ void linear_op_smem(cplx<T>* sm, const cplx<T>* tw, const cplx<T>* tab, int tid) {
-    fwd_passes<T, L, NT>(sm, tw, tid);
+    fwd_passes<T, L, NT, false, 0>(sm, tw, tid);
     mid_pass_smem<T, L, NT>(sm, tab, tid);
-    inv_passes<T, L, NT>(sm, tw, tid);
+    inv_passes<T, L, NT, false, 0>(sm, tw, tid);
+}
+
+// Shared-memory layout of the resident engine: the padded field, then a copy of the twiddles of the
+// local passes 1..P-2.
+template <class T, int L> struct smem_layout {
+    static constexpr size_t field_bytes = (size_t)padded_len<T>(1 << L) * sizeof(cplx<T>);
+    static constexpr size_t tw_bytes = (size_t)plan<L>::tw_local_count * sizeof(cplx<T>);
+    static constexpr size_t total = field_bytes + (tw_bytes ? tw_bytes : 16);
+};
+
+// The part of the linear operator between the two pass-0 halves: forward passes 1..P-2, middle,
+// inverse passes P-2..1, on the field at the start of dynamic shared memory with the twiddles of
+// the local passes behind it (smem_layout).  Input: the field after forward pass 0; output: the
+// field before inverse pass 0.  Barriers as for linear_op_smem.  Not inlined: one copy serves every
+// call site of a kernel (and both the two- and three-wave kernels).
+template <class T, int L, int NT>
+__device__ __noinline__ void linear_core_smem(const cplx<T>* tab, int tid) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+    // addressed as the global table is: twl[tw_offset(p) + ...]
+    const cplx<T>* twl = reinterpret_cast<const cplx<T>*>(smem_raw + smem_layout<T, L>::field_bytes) - plan<L>::tw_local_begin;
+    fwd_passes<T, L, NT, true, 1>(sm, twl, tid);
+    mid_pass_smem<T, L, NT>(sm, tab, tid);
+    inv_passes<T, L, NT, true, 1>(sm, twl, tid);
 }
 
 // forward transform only (for frequency-domain output): result in digit-reversed order in smem
 template <class T, int L, int NT>
 __device__ __forceinline__ void forward_only_smem(cplx<T>* sm, const cplx<T>* tw, int tid) {
-    fwd_passes<T, L, NT>(sm, tw, tid);
-    fwd_pass_smem<T, L, plan<L>::P - 1, NT>(sm, tw, tid);
+    fwd_passes<T, L, NT, false, 0>(sm, tw, tid);
+    fwd_pass_smem<T, L, plan<L>::P - 1, NT, false>(sm, tw, tid);
 }
 
 // threads per CTA for a 2^L-point field: 32 points per thread for large fields (keeps the register

@@ -2,15 +2,24 @@
 //
 // Each CTA keeps its field in (padded) shared memory for the whole call -- every z-step of every
 // round trip -- so HBM is touched only at the ends of the call and, per round trip, for the
-// re-injected non-resonant inputs and the constant tables (L2-resident).
+// re-injected non-resonant inputs; the constant tables stream from L2.
 //
-//   linear step  : CTA-local FFT . table . IFFT on its own field (opo_fft.cuh); adjacent half-steps
-//                  are merged (H.H = H2) and, between round trips, merged across the cavity
-//                  boundary (H . G m . H = HB), so a z-step costs one transform pair per field.
-//   nonlinear    : RK4 needs all F fields at the same tau.  The grid points are dealt to the F
-//                  CTAs in tiles of 32; a CTA reads the two foreign fields of its tiles through
-//                  distributed shared memory, integrates, and writes all F results back.
-//   two cluster barriers per z-step order the two phases.
+// A z-step (order L/2 - N - L/2, adjacent half-steps merged) is two phases:
+//
+//   core   : CTA-local.  Forward passes 1..P-2, [last forward pass . table . first inverse pass] in
+//            registers, inverse passes P-2..1 (opo_fft.cuh), twiddles from a shared-memory copy.
+//   fused  : inverse pass 0 -> RK4 -> forward pass 0, in registers.  Pass 0 is a radix-4 butterfly
+//            over x[t + j N/4], j = 0..3; the RK4 step of the coupling terms
+//            needs all F fields at those four grid points.  The butterflies t are dealt to the F
+//            CTAs in tiles of 32; a CTA reads its own field locally and the foreign fields through
+//            distributed shared memory, transforms, integrates, transforms back and writes all F
+//            fields back.  The DSMEM traffic (2/3 of the state in each direction) overlaps the
+//            butterfly and RK4 arithmetic of the same phase.
+//   one cluster barrier before and after the fused phase.
+//
+// Merged tables: H.H = H2 between RK4 steps; H . G m . H = HB across the cavity boundary for a
+// resonant field; a non-resonant field restarts every round trip
+// from IDFT(H DFT(S_x)) (kept, up to its inverse pass 0, in the scratch buffer SH).
 //
 // A cluster loops over instances b = cluster_id, cluster_id + n_clusters, ... (batched mode,
 // BASELINE.json configs[4]); instances are independent, there is no inter-cluster communication.
@@ -23,32 +32,70 @@ namespace opo {
 
 namespace cg = cooperative_groups;
 
+// inverse pass 0 -> RK4 -> forward pass 0 on this CTA's share of the radix-4 butterflies
 template <class T, int L, int F, int NT>
-__device__ __forceinline__ void resident_rk4(cplx<T>* const* fld, int rank, int tid, cplx<T> e0, cplx<T> e1, cplx<T> e2,
-                                             const T* kap, T h) {
-    constexpr int N = 1 << L, NTILES = N / 32, NW = NT / 32;
+__device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int rank, int tid, const cplx<T>* __restrict__ tw0,
+                                                cplx<T> e0, cplx<T> e1, cplx<T> e2, const T* kap, T h) {
+    static_assert(plan<L>::rbits(0) == 2, "pass 0 must be radix 4");
+    constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
+    constexpr int NTILES = (S + 31) / 32, NW = NT / 32;
     const int warp = tid >> 5, lane = tid & 31;
-    // tiles tau = rank + F * j, j = warp, warp + NW, ...   two tiles in flight per iteration
-    for (int j = warp; rank + F * j < NTILES; j += 2 * NW) {
-        const int t0 = rank + F * j, t1 = rank + F * (j + NW);
-        const bool has1 = t1 < NTILES;
-        const int i0 = phys<T>(t0 * 32 + lane), i1 = phys<T>((has1 ? t1 : t0) * 32 + lane);
-        cplx<T> y0[F], y1[F];
+#pragma unroll 1
+    for (int tile = rank + F * warp; tile < NTILES; tile += F * NW) {
+        const int t = tile * 32 + lane;
+        if (S >= 32 || t < S) {
+            cplx<T> w[R - 1];
 #pragma unroll
-        for (int x = 0; x < F; ++x) { y0[x] = fld[x][i0]; y1[x] = fld[x][i1]; }
-        Rk4<T, F>::step(y0, e0, e1, e2, kap, h);
-        Rk4<T, F>::step(y1, e0, e1, e2, kap, h);
+            for (int k = 0; k < R - 1; ++k) w[k] = ldg(&tw0[k * S + t]);
+            const int p0 = elem_base<T, RB, SB>(0, t);
+            cplx<T> v[F][R];
 #pragma unroll
-        for (int x = 0; x < F; ++x) {
-            fld[x][i0] = y0[x];
-            if (has1) fld[x][i1] = y1[x];
+            for (int x = 0; x < F; ++x)
+#pragma unroll
+                for (int k = 0; k < R; ++k) v[x][k] = fld[x][p0 + elem_off<T, RB, SB>(k)];
+#pragma unroll
+            for (int x = 0; x < F; ++x) {
+#pragma unroll
+                for (int k = 1; k < R; ++k) v[x][k] = cmulc(v[x][k], w[k - 1]);
+                dit_inv<T, R>::run(v[x]);
+            }
+#pragma unroll
+            for (int j = 0; j < R; ++j) {
+                cplx<T> y[F];
+#pragma unroll
+                for (int x = 0; x < F; ++x) y[x] = v[x][j];
+                Rk4<T, F>::step(y, e0, e1, e2, kap, h);
+#pragma unroll
+                for (int x = 0; x < F; ++x) v[x][j] = y[x];
+            }
+#pragma unroll
+            for (int x = 0; x < F; ++x) {
+                dif<T, R>::run(v[x]);
+#pragma unroll
+                for (int k = 1; k < R; ++k) v[x][k] = cmul(v[x][k], w[k - 1]);
+            }
+#pragma unroll
+            for (int x = 0; x < F; ++x)
+#pragma unroll
+                for (int k = 0; k < R; ++k) fld[x][p0 + elem_off<T, RB, SB>(k)] = v[x][k];
         }
     }
+}
+
+// stand-alone pass 0 on the CTA's own field (the first and last linear operator of a call)
+template <class T, int L, int NT>
+__device__ __noinline__ void pass0_local(const cplx<T>* tw, int tid, bool inverse) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+    if (inverse) inv_pass_smem<T, L, 0, NT, false>(sm, tw, tid);
+    else fwd_pass_smem<T, L, 0, NT, false>(sm, tw, tid);
 }
 
 template <class T, int L, int F>
 __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(ResidentArgs a) {
     constexpr int N = 1 << L, NT = cta_threads<T, L>::value;
+    using PL = plan<L>;
+    using SL = smem_layout<T, L>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
     cg::cluster_group cluster = cg::this_cluster();
@@ -61,15 +108,24 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
     for (int f = 0; f < F; ++f) fld[f] = cluster.map_shared_rank(sm, f);
 
     const cplx<T>* tw = reinterpret_cast<const cplx<T>*>(a.tw);
+    {   // shared-memory copy of the twiddles of the local passes
+        cplx<T>* twl = reinterpret_cast<cplx<T>*>(smem_raw + SL::field_bytes);
+        for (int i = tid; i < PL::tw_local_count; i += NT) twl[i] = ldg(&tw[PL::tw_local_begin + i]);
+    }
     const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
     const cplx<T>* tabH2 = reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
     const bool resonant = a.resonant[x] != 0;
     T kap[3] = {(T)a.kappa[0], (T)a.kappa[1], (T)a.kappa[2]};
     const T h = (T)a.h;
+    const int nz = a.nz;
+    const bool rt_mode = a.mode != 0;
+    const int total = rt_mode ? a.steps * nz : a.steps;     // RK4 steps in this call
 
     for (int b = cid; b < a.batch; b += n_clusters) {
         cplx<T>* cur = reinterpret_cast<cplx<T>*>(a.cur[x]) + (size_t)b * N;
         const cplx<T>* ph = reinterpret_cast<const cplx<T>*>(a.phase) + (size_t)b * a.phase_stride;
+        const cplx<T>* tabHB = reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x];
+        cplx<T>* SH = reinterpret_cast<cplx<T>*>(a.SH[x]) + (size_t)b * N;
 
         auto load = [&](const cplx<T>* __restrict__ g) {
 #pragma unroll 4
@@ -79,79 +135,74 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
 #pragma unroll 4
             for (int i = tid; i < N; i += NT) g[i] = sm[phys<T>(i)];
         };
-        auto nonlinear = [&](int s) {
-            cluster.sync();     // every field has finished its linear step
-            const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
-            resident_rk4<T, L, F, NT>(fld, x, tid, e0, e1, e2, kap, h);
-            cluster.sync();     // every RK4 result has landed in its owner's shared memory
-        };
 
         load(cur);
         __syncthreads();
+        pass0_local<T, L, NT>(tw, tid, false);
+        __syncthreads();
 
-        if (a.mode == 0) {
-            // `steps` z-steps from step index z0:  H, N, H2, N, ..., N, H
-            linear_op_smem<T, L, NT>(sm, tw, tabH, tid);
-            for (int s = 0; s < a.steps; ++s) {
-                nonlinear(a.z0 + s);
-                if (s + 1 < a.steps) linear_op_smem<T, L, NT>(sm, tw, tabH2, tid);
+        // q counts linear operators: q = 0 first half-step, q = total last half-step, between them the
+        // merged full steps; in round-trip mode q = m nz + s and s = 0 (m > 0) crosses the boundary
+#pragma unroll 1
+        for (int q = 0; q <= total; ++q) {
+            const int s = rt_mode ? q % nz : a.z0 + q;          // index of the RK4 step that follows
+            const bool crossing = rt_mode && q > 0 && q < total && s == 0;
+            if (crossing && !resonant) {
+                load(SH);                                        // fresh pump / frozen seed, already half-stepped
+            } else {
+                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
+                linear_core_smem<T, L, NT>(tab, tid);
             }
-            linear_op_smem<T, L, NT>(sm, tw, tabH, tid);
-            __syncthreads();
+            if (rt_mode && q == 0 && !resonant && a.steps > 1) {   // keep it for the later round trips
+                __syncthreads();
+                store(SH);
+            }
+            if (q == total) break;
+            const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
+            cluster.sync();     // every field is ready for its inverse pass 0
+            fused_pass0_rk4<T, L, F, NT>(fld, x, tid, tw, e0, e1, e2, kap, h);
+            cluster.sync();     // every result has landed in its owner's shared memory
+        }
+        __syncthreads();
+        pass0_local<T, L, NT>(tw, tid, true);
+        __syncthreads();
+
+        if (!rt_mode) {
             store(cur);
         } else {
-            const cplx<T>* tabHB = reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x];
-            const cplx<T>* tabGM = reinterpret_cast<const cplx<T>*>(a.tabGM[x]) + (size_t)b * a.tab_stride[x];
-            cplx<T>* SH = reinterpret_cast<cplx<T>*>(a.SH[x]) + (size_t)b * N;
-            for (int m = 0; m < a.steps; ++m) {
-                const bool first = (m == 0), last = (m == a.steps - 1);
-                if (first) {
-                    linear_op_smem<T, L, NT>(sm, tw, tabH, tid);
-                    if (!resonant && a.steps > 1) {       // keep IDFT(H DFT(S_x)) for the later round trips
-                        __syncthreads();
-                        store(SH);
-                    }
-                } else if (resonant) {
-                    linear_op_smem<T, L, NT>(sm, tw, tabHB, tid);   // H . G m . H across the boundary
-                } else {
-                    load(SH);                                        // fresh pump / frozen seed, already half-stepped
-                }
-                for (int s = 0; s < a.nz; ++s) {
-                    nonlinear(s);
-                    if (s + 1 < a.nz) linear_op_smem<T, L, NT>(sm, tw, tabH2, tid);
-                }
-                if (last) {
-                    linear_op_smem<T, L, NT>(sm, tw, tabH, tid);
+            store(reinterpret_cast<cplx<T>*>(a.exitb[x]) + (size_t)b * N);     // fields at z = L of the last pass
+            if (resonant) {
+                if (a.boundary_fft[x]) {
+                    const cplx<T>* tabGM = reinterpret_cast<const cplx<T>*>(a.tabGM[x]) + (size_t)b * a.tab_stride[x];
                     __syncthreads();
-                    store(reinterpret_cast<cplx<T>*>(a.exitb[x]) + (size_t)b * N);     // fields at z = L
-                    if (resonant) {
-                        if (a.boundary_fft[x]) {
-                            linear_op_smem<T, L, NT>(sm, tw, tabGM, tid);
-                            __syncthreads();
-                            store(cur);
-                        } else {
-                            const cplx<T> mf = ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b);
+                    pass0_local<T, L, NT>(tw, tid, false);
+                    __syncthreads();
+                    linear_core_smem<T, L, NT>(tabGM, tid);
+                    __syncthreads();
+                    pass0_local<T, L, NT>(tw, tid, true);
+                    __syncthreads();
+                    store(cur);
+                } else {
+                    const cplx<T> mf = ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b);
 #pragma unroll 4
-                            for (int i = tid; i < N; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
-                        }
-                    } else {
-                        const cplx<T>* __restrict__ S = reinterpret_cast<const cplx<T>*>(a.S[x]) + (size_t)b * N;
-#pragma unroll 4
-                        for (int i = tid; i < N; i += NT) cur[i] = S[i];
-                    }
+                    for (int i = tid; i < N; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
                 }
+            } else {
+                const cplx<T>* __restrict__ S = reinterpret_cast<const cplx<T>*>(a.S[x]) + (size_t)b * N;
+#pragma unroll 4
+                for (int i = tid; i < N; i += NT) cur[i] = S[i];
             }
         }
-        // all foreign reads/writes of this instance are fenced by the last nonlinear(); make sure
-        // nobody reloads its shared memory for the next instance while a peer still stores from it
+        // nobody reloads its shared memory for the next instance while it still stores from it; all
+        // foreign accesses of this instance ended at the last cluster barrier
         __syncthreads();
     }
-    cluster.sync();     // keep shared memory alive until every peer has left its last RK4
+    cluster.sync();     // keep shared memory alive until every peer has left its last fused phase
 }
 
 template <class T, int L, int F> cudaError_t resident_cfg(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, int n_clusters, cudaStream_t s) {
     constexpr int NT = cta_threads<T, L>::value;
-    const size_t smem = (size_t)padded_len<T>(1 << L) * sizeof(cplx<T>);
+    const size_t smem = smem_layout<T, L>::total;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(k_resident<T, L, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
