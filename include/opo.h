@@ -92,7 +92,7 @@ typedef struct {
 
 /* grid: PAPER.md:L175-178 (dt = t_rt/n), L162 (nz), L193 (precision) */
 typedef struct {
-    int log2_n;        /* 6 .. 18 (c64), 6 .. 13 (c128) */
+    int log2_n;        /* 6 .. 18 */
     double window_s;   /* N dt, the round-trip window t_rt */
     int nz_per_pass;   /* z-steps per crystal pass; h = length_m / nz_per_pass */
     int precision;     /* OPO_PRECISION_C64 | OPO_PRECISION_C128 */
@@ -152,14 +152,19 @@ int opo_check_finite(opo_handle* h);
 int opo_get_z_steps(const opo_handle* h, int* out_steps);
 
 /* Execution engine.  AUTO picks RESIDENT where one field fits one SM's shared memory (N <= 2^14 c64,
- * N <= 2^13 c128), else STREAMING.
+ * N <= 2^13 c128), else LARGE.
  *   RESIDENT : one thread-block cluster per instance, one CTA per field, fields stay in shared
  *              memory across z-steps and round trips; one launch per opo_propagate/opo_roundtrips.
  *   STREAMING: fields live in HBM/L2; one fused FFT-multiply-IFFT kernel and one RK4 kernel per z-step
- *              (N <= 2^14), or the four-step decomposition (N >= 2^15). */
+ *              (same sizes as RESIDENT; the unfused internal baseline).
+ *   LARGE    : N = 2^15 .. 2^18 (c128: 2^14 .. 2^18): four-step decomposition N = N1 x N2 in one
+ *              persistent cooperative kernel, two L2-resident memory passes per z-step with RK4 fused
+ *              into the column pass; one launch per opo_propagate/opo_roundtrips (plus the boundary
+ *              of the last round trip). */
 #define OPO_ENGINE_AUTO 0
 #define OPO_ENGINE_RESIDENT 1
 #define OPO_ENGINE_STREAMING 2
+#define OPO_ENGINE_LARGE 3
 #define OPO_OPT_ENGINE 0
 int opo_set_option(opo_handle* h, int option, int value);
 

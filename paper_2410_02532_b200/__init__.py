@@ -23,7 +23,7 @@ PRECISION_C64, PRECISION_C128 = 0, 1
 PARAM_DK, PARAM_DELTA_T, PARAM_DELTA_RAD, PARAM_GDD = 0, 1, 2, 3
 WHICH_CURRENT, WHICH_EXIT = 0, 1
 DOMAIN_TIME, DOMAIN_FREQ = 0, 1
-ENGINE_AUTO, ENGINE_RESIDENT, ENGINE_STREAMING = 0, 1, 2
+ENGINE_AUTO, ENGINE_RESIDENT, ENGINE_STREAMING, ENGINE_LARGE = 0, 1, 2, 3
 OPT_ENGINE = 0
 INFO_ENGINE, INFO_LAUNCHES, INFO_N, INFO_BATCH, INFO_SM_COUNT = 0, 1, 2, 3, 4
 

@@ -19,6 +19,7 @@ LIB = os.path.join(HERE, "libopo.so")
 PLAIN_SOURCES = ["opo_api.cu", "opo_dispatch.cu", "opo_pointwise.cu"]
 # (type, suffix, log2 N): one object per size-specialised instance of opo_inst.cu
 INSTANCES = [("float", "f32", l) for l in range(6, 15)] + [("double", "f64", l) for l in range(6, 14)]
+LARGE_INSTANCES = [("float", "f32", l) for l in range(15, 19)] + [("double", "f64", l) for l in range(14, 19)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -42,6 +43,10 @@ def _jobs(only=None):
         if only and f"{suf}:{l}" not in only:
             continue
         jobs.append(("opo_inst.cu", f"opo_inst_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
+    for typ, suf, l in LARGE_INSTANCES:
+        if only and f"{suf}:{l}" not in only:
+            continue
+        jobs.append(("opo_inst_large.cu", f"opo_inst_large_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
     return jobs
 
 

@@ -117,6 +117,19 @@ struct opo_handle {
     void* phase = nullptr;
     int* flag = nullptr;
 
+    // large-N engine (four-step decomposition N = N1 x N2, opo_large.cuh)
+    bool large = false;
+    int L1 = 0, L2 = 0;
+    void* tw2 = nullptr;
+    void* wlo = nullptr;
+    void* whi = nullptr;
+    int* perm2 = nullptr;
+    void* scratch2 = nullptr;
+    unsigned long long* barrier = nullptr;
+    opo::LargeInfo linfo{};
+    std::vector<int> host_perm1, host_perm2;
+    size_t tab_esz = 8;        // bytes per table entry (large engine, c64: hi + lo = 16)
+
     int z_steps = 0;
     int engine_opt = OPO_ENGINE_AUTO;
     bool resident_ok = false;
@@ -159,6 +172,22 @@ int upload_complex(opo_handle* h, void* dst, const cd* src, size_t count, bool u
     return OPO_OK;
 }
 
+// upload table values in the entry format of the engine: plain complex, or (large engine, c64) hi + lo
+int upload_table(opo_handle* h, void* dst, const cd* src, size_t count) {
+    if (!(h->large && !h->dbl)) return upload_complex(h, dst, src, count);
+    std::vector<float> tmp(4 * count);
+    for (size_t i = 0; i < count; ++i) {
+        const float hr = (float)src[i].real(), hi = (float)src[i].imag();
+        tmp[4 * i] = hr;
+        tmp[4 * i + 1] = hi;
+        tmp[4 * i + 2] = (float)(src[i].real() - (double)hr);
+        tmp[4 * i + 3] = (float)(src[i].imag() - (double)hi);
+    }
+    OPO_CUDA(h, cudaMemcpyAsync(dst, tmp.data(), tmp.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+    OPO_CUDA(h, cudaStreamSynchronize(h->stream));
+    return OPO_OK;
+}
+
 // Omega_k = 2 pi k' / (N dt), natural FFT order, Nyquist bin negative (R9)
 double omega_of(const opo_handle* h, int k) {
     const int kp = (k < h->N / 2) ? k : k - h->N;
@@ -171,6 +200,25 @@ void to_mid_layout(const opo_handle* h, const HostPlan& pl, const cd* M, cd* out
     const int NBF = h->N / R;
     for (int u = 0; u < NBF; ++u)
         for (int kk = 0; kk < R; ++kk) out[(size_t)kk * NBF + u] = M[h->host_perm[u * R + kk]];
+}
+
+// natural-order frequency multiplier -> layout of the large engine's row pass: row r holds k1 = perm1[r],
+// inside the row the mid-pass layout of the row plan: out[r N2 + kk NBF + u] = M[k1 + N1 perm2[u R + kk]]
+void to_large_layout(const opo_handle* h, const HostPlan& pl2, const cd* M, cd* out) {
+    const int N1 = 1 << h->L1, N2 = 1 << h->L2;
+    const int R = 1 << pl2.rbits[pl2.P - 1];
+    const int NBF = N2 / R;
+    for (int r = 0; r < N1; ++r) {
+        const int k1 = h->host_perm1[r];
+        for (int u = 0; u < NBF; ++u)
+            for (int kk = 0; kk < R; ++kk)
+                out[(size_t)r * N2 + (size_t)kk * NBF + u] = M[(size_t)k1 + (size_t)N1 * h->host_perm2[u * R + kk]];
+    }
+}
+
+void to_engine_layout(const opo_handle* h, const HostPlan& pl, const cd* M, cd* out) {
+    if (h->large) to_large_layout(h, pl, M, out);
+    else to_mid_layout(h, pl, M, out);
 }
 
 }  // namespace
@@ -186,7 +234,7 @@ namespace {
 //   tabH = H/N, tabH2 = H^2/N, tabGM = G m/N, tabHB = H^2 G m/N (half-steps merged across the boundary).
 int build_tables(opo_handle* h) {
     const int N = h->N, F = h->F, B = h->B;
-    HostPlan pl(h->L);
+    HostPlan pl(h->large ? h->L2 : h->L);
     const double invN = 1.0 / (double)N;
     std::vector<cd> Hh(N), M(N), lay(N);
     for (int x = 0; x < F; ++x) {
@@ -198,15 +246,15 @@ int build_tables(opo_handle* h) {
             Hh[k] = std::exp(cd(-0.5 * al, D) * (0.5 * h->h));
         }
         for (int k = 0; k < N; ++k) M[k] = Hh[k] * invN;
-        to_mid_layout(h, pl, M.data(), lay.data());
-        if (int rc = upload_complex(h, h->tabH[x], lay.data(), N)) return rc;
+        to_engine_layout(h, pl, M.data(), lay.data());
+        if (int rc = upload_table(h, h->tabH[x], lay.data(), N)) return rc;
         for (int k = 0; k < N; ++k) {
             const double om = omega_of(h, k);
             const double D = -db1 * om + 0.5 * b2 * om * om;
             M[k] = std::exp(cd(-0.5 * al, D) * h->h) * invN;     // H^2 evaluated directly in fp64
         }
-        to_mid_layout(h, pl, M.data(), lay.data());
-        if (int rc = upload_complex(h, h->tabH2[x], lay.data(), N)) return rc;
+        to_engine_layout(h, pl, M.data(), lay.data());
+        if (int rc = upload_table(h, h->tabH2[x], lay.data(), N)) return rc;
 
         if (!h->fields.resonant[x]) continue;
         // boundary tables, shared or per instance
@@ -215,8 +263,8 @@ int build_tables(opo_handle* h) {
             if (h->tabGM[x]) cudaFree(h->tabGM[x]);
             if (h->tabHB[x]) cudaFree(h->tabHB[x]);
             h->tabGM[x] = h->tabHB[x] = nullptr;
-            if (cudaMalloc(&h->tabGM[x], need * N * h->esz) != cudaSuccess ||
-                cudaMalloc(&h->tabHB[x], need * N * h->esz) != cudaSuccess)
+            if (cudaMalloc(&h->tabGM[x], need * N * h->tab_esz) != cudaSuccess ||
+                cudaMalloc(&h->tabHB[x], need * N * h->tab_esz) != cudaSuccess)
                 return fail(h, OPO_ERR_ALLOC, "cudaMalloc of boundary tables failed");
             h->tabB_count[x] = need;
         }
@@ -237,10 +285,10 @@ int build_tables(opo_handle* h) {
                 M[k] = gm * invN;
                 Hh[k] = std::exp(cd(-0.5 * al, D) * h->h) * gm * invN;
             }
-            to_mid_layout(h, pl, M.data(), lay.data());
-            if (int rc = upload_complex(h, (char*)h->tabGM[x] + b * N * h->esz, lay.data(), N)) return rc;
-            to_mid_layout(h, pl, Hh.data(), lay.data());
-            if (int rc = upload_complex(h, (char*)h->tabHB[x] + b * N * h->esz, lay.data(), N)) return rc;
+            to_engine_layout(h, pl, M.data(), lay.data());
+            if (int rc = upload_table(h, (char*)h->tabGM[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
+            to_engine_layout(h, pl, Hh.data(), lay.data());
+            if (int rc = upload_table(h, (char*)h->tabHB[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
         }
     }
     h->tables_dirty = false;
@@ -261,8 +309,7 @@ int build_phase(opo_handle* h) {
     return OPO_OK;
 }
 
-int build_fft_tables(opo_handle* h) {
-    HostPlan pl(h->L);
+std::vector<cd> pass_twiddles(const HostPlan& pl) {
     std::vector<cd> tw((size_t)std::max(pl.tw_total, 1));
     for (int p = 0; p < pl.P; ++p) {
         const int R = 1 << pl.rbits[p], S = 1 << pl.sbits[p];
@@ -273,13 +320,50 @@ int build_fft_tables(opo_handle* h) {
                 tw[(size_t)pl.tw_offset[p] + (size_t)(k - 1) * S + t] = cd(std::cos(a), std::sin(a));
             }
     }
-    if (cudaMalloc(&h->tw, tw.size() * h->esz) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc(tw)");
-    if (int rc = upload_complex(h, h->tw, tw.data(), tw.size(), /*unit_twiddles=*/true)) return rc;
-    h->host_perm.resize(h->N);
-    for (int pos = 0; pos < h->N; ++pos) h->host_perm[pos] = pl.freq_of_pos(pos);
-    if (cudaMalloc(&h->perm, (size_t)h->N * sizeof(int)) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc(perm)");
-    OPO_CUDA(h, cudaMemcpy(h->perm, h->host_perm.data(), (size_t)h->N * sizeof(int), cudaMemcpyHostToDevice));
+    return tw;
+}
+
+int upload_twiddles(opo_handle* h, void** dst, const std::vector<cd>& tw) {
+    if (cudaMalloc(dst, tw.size() * h->esz) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc(twiddles)");
+    return upload_complex(h, *dst, tw.data(), tw.size(), /*unit_twiddles=*/true);
+}
+
+int upload_perm(opo_handle* h, int** dst, const std::vector<int>& perm) {
+    if (cudaMalloc((void**)dst, perm.size() * sizeof(int)) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc(perm)");
+    OPO_CUDA(h, cudaMemcpy(*dst, perm.data(), perm.size() * sizeof(int), cudaMemcpyHostToDevice));
     return OPO_OK;
+}
+
+int build_fft_tables(opo_handle* h) {
+    if (!h->large) {
+        HostPlan pl(h->L);
+        if (int rc = upload_twiddles(h, &h->tw, pass_twiddles(pl))) return rc;
+        h->host_perm.resize(h->N);
+        for (int pos = 0; pos < h->N; ++pos) h->host_perm[pos] = pl.freq_of_pos(pos);
+        return upload_perm(h, &h->perm, h->host_perm);
+    }
+    // large engine: column plan (L1), row plan (L2), the two factors of W_N^{n2 k1}
+    HostPlan pl1(h->L1), pl2(h->L2);
+    const int N1 = 1 << h->L1, N2 = 1 << h->L2;
+    if (int rc = upload_twiddles(h, &h->tw, pass_twiddles(pl1))) return rc;
+    if (int rc = upload_twiddles(h, &h->tw2, pass_twiddles(pl2))) return rc;
+    std::vector<cd> wlo(N1), whi(N2);
+    for (int j = 0; j < N1; ++j) {
+        const double a = -2.0 * kPi * (double)j / (double)h->N;
+        wlo[j] = cd(std::cos(a), std::sin(a));
+    }
+    for (int j = 0; j < N2; ++j) {
+        const double a = -2.0 * kPi * (double)j / (double)N2;      // W_N^{j N1} = W_N2^j
+        whi[j] = cd(std::cos(a), std::sin(a));
+    }
+    if (int rc = upload_twiddles(h, &h->wlo, wlo)) return rc;
+    if (int rc = upload_twiddles(h, &h->whi, whi)) return rc;
+    h->host_perm1.resize(N1);
+    h->host_perm2.resize(N2);
+    for (int pos = 0; pos < N1; ++pos) h->host_perm1[pos] = pl1.freq_of_pos(pos);
+    for (int pos = 0; pos < N2; ++pos) h->host_perm2[pos] = pl2.freq_of_pos(pos);
+    if (int rc = upload_perm(h, &h->perm, h->host_perm1)) return rc;
+    return upload_perm(h, &h->perm2, h->host_perm2);
 }
 
 int ensure_tables(opo_handle* h) {
@@ -293,7 +377,7 @@ void free_all(opo_handle* h) {
         void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->mirror[x]};
         for (void* p : ptrs) if (p) cudaFree(p);
     }
-    void* more[] = {h->scratch, h->tw, h->perm, h->phase, h->flag};
+    void* more[] = {h->scratch, h->tw, h->perm, h->phase, h->flag, h->tw2, h->wlo, h->whi, h->perm2, h->scratch2, h->barrier};
     for (void* p : more) if (p) cudaFree(p);
 }
 
@@ -318,8 +402,8 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
     }
     if (f->resonant[0]) return fail(nullptr, OPO_ERR_UNSUPPORTED, "resonant pump: the paper gives no input-coupling rule");
     const int maxL = (g->precision == OPO_PRECISION_C64) ? opo::kMaxLog2Smem : opo::kMaxLog2Smem - 1;
-    if (g->log2_n < opo::kMinLog2 || g->log2_n > maxL)
-        return fail(nullptr, OPO_ERR_UNSUPPORTED, "grid size not supported for this precision (c64: 2^6..2^14, c128: 2^6..2^13)");
+    if (g->log2_n < opo::kMinLog2 || g->log2_n > opo::kMaxLog2)
+        return fail(nullptr, OPO_ERR_UNSUPPORTED, "grid size not supported (2^6 .. 2^18)");
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -333,6 +417,10 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
     h->L = g->log2_n; h->N = 1 << g->log2_n; h->F = f->n_fields; h->B = g->batch; h->nz = g->nz_per_pass;
     h->dbl = (g->precision == OPO_PRECISION_C128);
     h->esz = h->dbl ? 16 : 8;
+    h->large = h->L > maxL;
+    h->L1 = h->L / 2;
+    h->L2 = h->L - h->L1;
+    h->tab_esz = h->large ? 16 : h->esz;
     h->h = c->length_m / (double)g->nz_per_pass;
     h->sm_count = prop.multiProcessorCount;
     for (int x = 0; x < h->F; ++x) h->kappa[x] = 2.0 * kPi * c->d_eff_m_per_V / (f->n[x] * f->lambda_m[x]);
@@ -351,7 +439,7 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
             if (cudaMalloc(p, fb) != cudaSuccess) return bail(OPO_ERR_ALLOC, "cudaMalloc of field state failed");
             cudaMemset(*p, 0, fb);
         }
-        if (cudaMalloc(&h->tabH[x], (size_t)h->N * h->esz) != cudaSuccess || cudaMalloc(&h->tabH2[x], (size_t)h->N * h->esz) != cudaSuccess ||
+        if (cudaMalloc(&h->tabH[x], (size_t)h->N * h->tab_esz) != cudaSuccess || cudaMalloc(&h->tabH2[x], (size_t)h->N * h->tab_esz) != cudaSuccess ||
             cudaMalloc(&h->mirror[x], (size_t)h->B * h->esz) != cudaSuccess)
             return bail(OPO_ERR_ALLOC, "cudaMalloc of tables failed");
     }
@@ -360,10 +448,21 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
         return bail(OPO_ERR_ALLOC, "cudaMalloc of scratch failed");
     if (int rc = build_fft_tables(h)) { std::string m = h->err; return bail(rc, m); }
     if (int rc = ensure_tables(h)) { std::string m = h->err; return bail(rc, m); }
-    // resident engine availability
-    cudaError_t e = h->dbl ? opo::resident_info_f64(h->L, h->F, &h->rinfo) : opo::resident_info_f32(h->L, h->F, &h->rinfo);
-    h->resident_ok = (e == cudaSuccess && h->rinfo.max_clusters > 0);
-    if (e != cudaSuccess) cudaGetLastError();
+    if (h->large) {
+        if (cudaMalloc(&h->scratch2, fb) != cudaSuccess || cudaMalloc((void**)&h->barrier, sizeof(unsigned long long)) != cudaSuccess)
+            return bail(OPO_ERR_ALLOC, "cudaMalloc of large-engine scratch failed");
+        cudaError_t e = h->dbl ? opo::large_info_f64(h->L, h->F, h->B, h->sm_count, &h->linfo)
+                               : opo::large_info_f32(h->L, h->F, h->B, h->sm_count, &h->linfo);
+        if (e != cudaSuccess || h->linfo.grid <= 0) {
+            cudaGetLastError();
+            return bail(OPO_ERR_UNSUPPORTED, std::string("large-N engine unavailable for this size/precision: ") + cudaGetErrorString(e));
+        }
+    } else {
+        // resident engine availability
+        cudaError_t e = h->dbl ? opo::resident_info_f64(h->L, h->F, &h->rinfo) : opo::resident_info_f32(h->L, h->F, &h->rinfo);
+        h->resident_ok = (e == cudaSuccess && h->rinfo.max_clusters > 0);
+        if (e != cudaSuccess) cudaGetLastError();
+    }
     if (cudaDeviceSynchronize() != cudaSuccess) return bail(OPO_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
     *out = h;
     return OPO_OK;
@@ -431,6 +530,7 @@ int check_async(opo_handle* h) {
 }
 
 int engine_in_use(const opo_handle* h) {
+    if (h->large) return OPO_ENGINE_LARGE;
     if (h->engine_opt == OPO_ENGINE_STREAMING) return OPO_ENGINE_STREAMING;
     return h->resident_ok ? OPO_ENGINE_RESIDENT : OPO_ENGINE_STREAMING;
 }
@@ -513,6 +613,71 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     return OPO_OK;
 }
 
+// ---- large-N engine -----------------------------------------------------------------------------------------------
+void large_common(const opo_handle* h, opo::LargeArgs& a) {
+    for (int x = 0; x < h->F; ++x) {
+        a.cur[x] = h->cur[x]; a.SH[x] = h->SH[x];
+        a.tabH[x] = h->tabH[x]; a.tabH2[x] = h->tabH2[x]; a.tabHB[x] = h->tabHB[x];
+        a.tabHB_stride[x] = h->per_inst_boundary[x] ? h->N : 0;
+        a.resonant[x] = h->fields.resonant[x] ? 1 : 0;
+        a.kappa[x] = h->kappa[x];
+    }
+    a.tw1 = h->tw; a.tw2 = h->tw2; a.wlo = h->wlo; a.whi = h->whi; a.perm1 = h->perm; a.perm2 = h->perm2;
+    a.phase = h->phase; a.phase_stride = 2 * h->nz + 1;
+    a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
+    a.field_mask = (1 << h->F) - 1;
+    a.barrier = h->barrier; a.barrier_base = 0;
+}
+
+int large_launch(opo_handle* h, const opo::LargeArgs& a) {
+    OPO_CUDA(h, cudaMemsetAsync(h->barrier, 0, sizeof(unsigned long long), h->stream));
+    OPO_LAUNCH(h, h->dbl ? opo::launch_large_f64(h->L, a, h->linfo.grid, h->stream)
+                         : opo::launch_large_f32(h->L, a, h->linfo.grid, h->stream));
+    return OPO_OK;
+}
+
+// mode 0: `steps` z-steps from step index z0.  mode 1: `steps` round trips; the kernel leaves the fields
+// at z = L of the last pass, the boundary of that last pass follows here.
+int large_run(opo_handle* h, int mode, int z0, int steps) {
+    opo::LargeArgs a{};
+    large_common(h, a);
+    a.mode = mode; a.z0 = z0; a.steps = steps;
+    if (int rc = large_launch(h, a)) return rc;
+    if (mode == 0) return OPO_OK;
+    int fft_mask = 0;
+    for (int x = 0; x < h->F; ++x) {
+        OPO_CUDA(h, cudaMemcpyAsync(h->exitb[x], h->cur[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+        if (!h->fields.resonant[x]) {
+            OPO_CUDA(h, cudaMemcpyAsync(h->cur[x], h->S[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+        } else if (h->boundary_fft[x]) {
+            fft_mask |= 1 << x;
+        } else {
+            opo::ScaleArgs sc{h->cur[x], h->mirror[x], h->B, h->N};
+            OPO_LAUNCH(h, h->dbl ? opo::launch_scale_f64(sc, h->stream) : opo::launch_scale_f32(sc, h->stream));
+        }
+    }
+    if (fft_mask) {
+        opo::LargeArgs g{};
+        large_common(h, g);
+        g.mode = 0; g.z0 = 0; g.steps = 0; g.field_mask = fft_mask;
+        for (int x = 0; x < h->F; ++x) {
+            g.tabH[x] = h->tabGM[x];
+            g.tabH_stride[x] = h->per_inst_boundary[x] ? h->N : 0;
+        }
+        if (int rc = large_launch(h, g)) return rc;
+    }
+    return OPO_OK;
+}
+
+// out[b][k] = DFT(src[b])[k], natural order (dst may be the handle's own scratch)
+int large_freq(opo_handle* h, const void* src, void* dst) {
+    opo::LargeArgs a{};
+    large_common(h, a);
+    a.mode = 2; a.field_mask = 1;
+    a.cur[0] = h->scratch2; a.src_override[0] = const_cast<void*>(src); a.out[0] = dst;
+    return large_launch(h, a);
+}
+
 int copy_in(opo_handle* h, void* dst_field, const void* src, bool per_instance, cudaMemcpyKind kind) {
     const size_t one = (size_t)h->N * h->esz;
     if (per_instance) {
@@ -551,8 +716,12 @@ int get_fields_impl(opo_handle* h, int field, int which, int domain, void* out, 
     if (int rc = check_async(h)) return rc;
     const void* src = (which == OPO_WHICH_CURRENT) ? h->cur[field] : h->exitb[field];
     if (domain == OPO_DOMAIN_FREQ) {
-        opo::FreqArgs a{src, host ? h->scratch : out, h->perm, h->tw, h->B};
-        OPO_LAUNCH(h, h->dbl ? opo::launch_freq_f64(h->L, a, h->stream) : opo::launch_freq_f32(h->L, a, h->stream));
+        if (h->large) {
+            if (int rc = large_freq(h, src, host ? h->scratch : out)) return rc;
+        } else {
+            opo::FreqArgs a{src, host ? h->scratch : out, h->perm, h->tw, h->B};
+            OPO_LAUNCH(h, h->dbl ? opo::launch_freq_f64(h->L, a, h->stream) : opo::launch_freq_f32(h->L, a, h->stream));
+        }
         if (!host) return OPO_OK;
         src = h->scratch;
     }
@@ -580,7 +749,8 @@ int opo_propagate(opo_handle* h, int nz) {
     if (int rc = check_async(h)) return rc;
     if (int rc = ensure_tables(h)) return rc;
     int rc;
-    if (engine_in_use(h) == OPO_ENGINE_RESIDENT) rc = resident_run(h, 0, h->z_steps, nz);
+    if (h->large) rc = large_run(h, 0, h->z_steps, nz);
+    else if (engine_in_use(h) == OPO_ENGINE_RESIDENT) rc = resident_run(h, 0, h->z_steps, nz);
     else rc = stream_steps(h, h->z_steps, nz, false);
     if (rc) return rc;
     h->z_steps += nz;
@@ -594,6 +764,7 @@ int opo_roundtrips(opo_handle* h, int n) {
     if (n == 0) return OPO_OK;
     if (int rc = check_async(h)) return rc;
     if (int rc = ensure_tables(h)) return rc;
+    if (h->large) return large_run(h, 1, 0, n);
     if (engine_in_use(h) == OPO_ENGINE_RESIDENT) return resident_run(h, 1, 0, n);
     for (int m = 0; m < n; ++m) {
         if (int rc = stream_steps(h, 0, h->nz, true)) return rc;
@@ -632,8 +803,12 @@ int opo_get_z_steps(const opo_handle* h, int* out) {
 int opo_set_option(opo_handle* h, int option, int value) {
     if (!h) return OPO_ERR_INVALID_ARG;
     if (option != OPO_OPT_ENGINE) return fail(h, OPO_ERR_INVALID_ARG, "unknown option");
-    if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING)
+    if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING && value != OPO_ENGINE_LARGE)
         return fail(h, OPO_ERR_INVALID_ARG, "unknown engine");
+    if (h->large && value != OPO_ENGINE_AUTO && value != OPO_ENGINE_LARGE)
+        return fail(h, OPO_ERR_UNSUPPORTED, "N > 2^14 (c128: > 2^13) runs on the large-N engine only");
+    if (!h->large && value == OPO_ENGINE_LARGE)
+        return fail(h, OPO_ERR_UNSUPPORTED, "the large-N engine serves N > 2^14 (c128: > 2^13) only");
     if (value == OPO_ENGINE_RESIDENT && !h->resident_ok)
         return fail(h, OPO_ERR_UNSUPPORTED, "resident engine unavailable for this size/precision on this device");
     h->engine_opt = value;

@@ -18,6 +18,12 @@ namespace opo {
 OPO_DECL_ALL(f32)
 OPO_DECL_ALL(f64)
 
+#define OPO_DECL_LARGE(SUF, LL)                                                                               \
+    cudaError_t large_info_##SUF##_L##LL(int, int, int, LargeInfo*) __attribute__((weak));                    \
+    cudaError_t launch_large_##SUF##_L##LL(const LargeArgs&, int, cudaStream_t) __attribute__((weak));
+OPO_DECL_LARGE(f32, 15) OPO_DECL_LARGE(f32, 16) OPO_DECL_LARGE(f32, 17) OPO_DECL_LARGE(f32, 18)
+OPO_DECL_LARGE(f64, 14) OPO_DECL_LARGE(f64, 15) OPO_DECL_LARGE(f64, 16) OPO_DECL_LARGE(f64, 17) OPO_DECL_LARGE(f64, 18)
+
 #define OPO_CASE(FN, SUF, LL, ...) \
     case LL: return FN##SUF##_L##LL ? FN##SUF##_L##LL(__VA_ARGS__) : cudaErrorNotSupported;
 
@@ -39,5 +45,36 @@ OPO_DECL_ALL(f64)
 
 OPO_DISPATCHERS(f32)
 OPO_DISPATCHERS(f64)
+
+cudaError_t large_info_f32(int log2n, int n_fields, int batch, int sm_count, LargeInfo* out) {
+    switch (log2n) {
+        OPO_CASE(large_info_, f32, 15, n_fields, batch, sm_count, out) OPO_CASE(large_info_, f32, 16, n_fields, batch, sm_count, out)
+        OPO_CASE(large_info_, f32, 17, n_fields, batch, sm_count, out) OPO_CASE(large_info_, f32, 18, n_fields, batch, sm_count, out)
+        default: return cudaErrorNotSupported;
+    }
+}
+cudaError_t large_info_f64(int log2n, int n_fields, int batch, int sm_count, LargeInfo* out) {
+    switch (log2n) {
+        OPO_CASE(large_info_, f64, 14, n_fields, batch, sm_count, out) OPO_CASE(large_info_, f64, 15, n_fields, batch, sm_count, out)
+        OPO_CASE(large_info_, f64, 16, n_fields, batch, sm_count, out) OPO_CASE(large_info_, f64, 17, n_fields, batch, sm_count, out)
+        OPO_CASE(large_info_, f64, 18, n_fields, batch, sm_count, out)
+        default: return cudaErrorNotSupported;
+    }
+}
+cudaError_t launch_large_f32(int log2n, const LargeArgs& a, int grid, cudaStream_t s) {
+    switch (log2n) {
+        OPO_CASE(launch_large_, f32, 15, a, grid, s) OPO_CASE(launch_large_, f32, 16, a, grid, s)
+        OPO_CASE(launch_large_, f32, 17, a, grid, s) OPO_CASE(launch_large_, f32, 18, a, grid, s)
+        default: return cudaErrorNotSupported;
+    }
+}
+cudaError_t launch_large_f64(int log2n, const LargeArgs& a, int grid, cudaStream_t s) {
+    switch (log2n) {
+        OPO_CASE(launch_large_, f64, 14, a, grid, s) OPO_CASE(launch_large_, f64, 15, a, grid, s)
+        OPO_CASE(launch_large_, f64, 16, a, grid, s) OPO_CASE(launch_large_, f64, 17, a, grid, s)
+        OPO_CASE(launch_large_, f64, 18, a, grid, s)
+        default: return cudaErrorNotSupported;
+    }
+}
 
 }  // namespace opo

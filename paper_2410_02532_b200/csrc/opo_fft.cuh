@@ -303,12 +303,36 @@ __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cp
     }
 }
 
+// ---- multiplier tables --------------------------------------------------------------------------------
+// A table entry is either one complex value (cplx<T>) or, for long fp32 runs, a two-float value
+// hi + lo (tabx<float>): the frequency-domain multiplier acts on the same bin at every z-step, so
+// the rounding of the *table* (3e-8 in modulus and phase) accumulates coherently over 10^4..10^5
+// steps; hi + lo carries the fp64 table value to ~1e-15 and leaves only data rounding.
+template <class T> struct alignas(4 * sizeof(T)) tabx { cplx<T> hi, lo; };
+
+__device__ __forceinline__ tabx<float> ldg(const tabx<float>* p) {
+    float4 v = __ldg(reinterpret_cast<const float4*>(p));
+    return {{v.x, v.y}, {v.z, v.w}};
+}
+template <class T> __device__ __forceinline__ cplx<T> tab_mul(cplx<T> v, cplx<T> h) { return cmul(v, h); }
+__device__ __forceinline__ cplx<float> tab_mul(cplx<float> v, tabx<float> h) {
+    float re = v.re * h.lo.re;
+    re = __fmaf_rn(-v.im, h.lo.im, re);
+    re = __fmaf_rn(-v.im, h.hi.im, re);
+    re = __fmaf_rn(v.re, h.hi.re, re);
+    float im = v.re * h.lo.im;
+    im = __fmaf_rn(v.im, h.lo.re, im);
+    im = __fmaf_rn(v.im, h.hi.re, im);
+    im = __fmaf_rn(v.re, h.hi.im, im);
+    return {re, im};
+}
+
 // ---- the fused middle: last forward pass, table multiply, first inverse pass, all in registers ----------
 // The last pass has S = 1: butterfly u owns positions u*R .. u*R + R-1.  The table is stored as
 // tab[k * (N/R) + u] so that consecutive threads read consecutive addresses; it streams from L2 and
 // its loads are issued before the shared-memory loads of the same butterfly.
-template <class T, int L, int NT>
-__device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tab, int tid) {
+template <class T, int L, int NT, class TAB = cplx<T>>
+__device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const TAB* __restrict__ tab, int tid) {
     using PL = plan<L>;
     constexpr int PASS = PL::P - 1;
     constexpr int RB = PL::rbits(PASS), R = 1 << RB;
@@ -316,7 +340,7 @@ __device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const cp
     constexpr int NBF = (1 << L) / R;
 #pragma unroll 1
     for (int u = tid; u < NBF; u += NT) {
-        cplx<T> h[R];
+        TAB h[R];
 #pragma unroll
         for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
         cplx<T>* __restrict__ p = sm + elem_base<T, RB, 0>(u, 0);
@@ -325,7 +349,7 @@ __device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const cp
         for (int j = 0; j < R; ++j) v[j] = p[elem_off<T, RB, 0>(j)];
         dif<T, R>::run(v);
 #pragma unroll
-        for (int k = 0; k < R; ++k) v[k] = cmul(v[k], h[k]);
+        for (int k = 0; k < R; ++k) v[k] = tab_mul(v[k], h[k]);
         dit_inv<T, R>::run(v);
 #pragma unroll
         for (int j = 0; j < R; ++j) p[elem_off<T, RB, 0>(j)] = v[j];

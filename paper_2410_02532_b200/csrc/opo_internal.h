@@ -7,6 +7,7 @@ namespace opo {
 
 constexpr int kMinLog2 = 6;
 constexpr int kMaxLog2Smem = 14;   // one field in one SM's shared memory (fp32); fp64: 13
+constexpr int kMaxLog2 = 18;       // large-N engine above kMaxLog2Smem
 
 // ---- streaming engine ------------------------------------------------------------------------------
 // One CTA per (slot, instance): dst[b] = IDFT( tab[b?] .* DFT(src[b]) ), optionally also to dst2.
@@ -84,6 +85,47 @@ struct ResidentInfo {
     int max_clusters;      // co-resident clusters (0 = cannot launch)
 };
 
+// ---- large-N engine ------------------------------------------------------------------------------------
+// One persistent cooperative kernel, four-step decomposition N = N1 x N2.  See opo_large.cuh.
+struct LargeArgs {
+    void* cur[3];              // [B][N] fields, transformed in place (mode 2: the scratch the column pass writes)
+    void* src_override[3];     // mode 2: where the column pass reads instead of cur (may be null)
+    void* out[3];              // mode 2: natural-order frequency-domain destination
+    void* SH[3];               // scratch [B][N]: row-domain image of IDFT(H DFT(S_x)) of non-resonant fields
+    const void* tabH[3];       // first / last operator of the call (half step; or G m for the boundary-only call)
+    long long tabH_stride[3];  // instance stride of tabH in table elements (0 = shared)
+    const void* tabH2[3];      // merged full step
+    const void* tabHB[3];      // merged across the boundary (resonant fields)
+    long long tabHB_stride[3];
+    const void* tw1;           // pass twiddles of the column transform (plan<L1>)
+    const void* tw2;           // pass twiddles of the row transform (plan<L2>)
+    const void* wlo;           // W_N^j, j < N1
+    const void* whi;           // W_N^{j N1}, j < N2
+    const int* perm1;          // row index -> k1 (digit reversal of the column transform)
+    const int* perm2;          // position in a transformed row -> k2
+    const void* phase;         // as Rk4Args
+    int phase_stride;
+    double kappa[3];
+    double h;
+    int resonant[3];
+    int field_mask;            // bit x set: field x takes part
+    int n_fields, batch, nz;
+    int mode;                  // 0 = `steps` z-steps from step index z0 (steps = 0: one linear operator with tabH);
+                               // 1 = `steps` round trips; 2 = forward DFT read-out
+    int z0;
+    int steps;
+    unsigned long long* barrier;        // zeroed by the host before the launch
+    unsigned long long barrier_base;    // counter value at launch (0)
+};
+
+struct LargeInfo {
+    int threads;
+    size_t smem_bytes;
+    int max_ctas;          // co-resident CTAs on the device
+    int grid;              // CTAs to launch for this batch
+    int n1, n2;
+};
+
 #define OPO_DECLARE_LAUNCHERS(SUFFIX)                                                   \
     cudaError_t launch_linear_##SUFFIX(int log2n, const LinArgs& a, cudaStream_t s);    \
     cudaError_t launch_rk4_##SUFFIX(const Rk4Args& a, cudaStream_t s);                  \
@@ -91,7 +133,9 @@ struct ResidentInfo {
     cudaError_t launch_freq_##SUFFIX(int log2n, const FreqArgs& a, cudaStream_t s);     \
     cudaError_t launch_finite_##SUFFIX(const void* A, long long count, int* flag, cudaStream_t s); \
     cudaError_t resident_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);     \
-    cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s);
+    cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
+    cudaError_t large_info_##SUFFIX(int log2n, int n_fields, int batch, int sm_count, LargeInfo* out);       \
+    cudaError_t launch_large_##SUFFIX(int log2n, const LargeArgs& a, int grid, cudaStream_t s);
 
 OPO_DECLARE_LAUNCHERS(f32)
 OPO_DECLARE_LAUNCHERS(f64)

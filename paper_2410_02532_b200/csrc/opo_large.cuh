@@ -1,0 +1,415 @@
+// opo_large.cuh -- large-N engine (N = 2^15 .. 2^18; complex128 also 2^14): one field no longer
+// fits one SM's shared memory (BASELINE.json configs[3]), so the transform is the four-step
+// decomposition N = N1 x N2 executed by ONE persistent kernel whose CTAs meet at a grid barrier
+// between memory passes.  The fields live in global memory and stay in the 126 MB L2 (4 MB of
+// state at N = 2^18, two fields); HBM sees them only at the ends of a call.
+//
+// Index split: n = n1 N2 + n2, k = k1 + N1 k2.
+//     X[k1 + N1 k2] = sum_n2 W_N2^{n2 k2} [ W_N^{n2 k1} sum_n1 x[n1 N2 + n2] W_N1^{n1 k1} ]
+// A z-step (order L/2 - N - L/2, adjacent half-steps merged as in the resident engine)
+// is two memory passes:
+//
+//   row pass    (one row k1 = N2 contiguous elements per team): W_N^{n2 k1} . DFT_N2 . table .
+//               IDFT_N2 . conj W_N^{n2 k1} -- the frequency-domain part of the linear operator
+//               (Eq. 5, L135 Eq. 11; boundary factors of Eq. 6 / L145 merged into the
+//               table at a round-trip crossing);
+//   column pass (a tile of TC adjacent columns n2, all F fields): IDFT_N1 . RK4 . DFT_N1.  The RK4
+//               step of the coupling terms is pointwise in n and is fused
+//               between inverse and forward radix-4 pass 0 exactly as in opo_resident.cuh.
+//
+// Every transform is the shared-memory machinery of opo_fft.cuh run by a *team* of N/16 threads
+// (several teams per CTA); digit-reversed orders are absorbed by the host tables (perm1: row index
+// -> k1; the row table is stored per row in mid-pass layout).  W_N^{n2 k1} is the product of two
+// small shared-memory tables, W_N^{p} = W_N^{(p >> L1) << L1} . W_N^{p & (N1-1)}.
+//
+// fp32: the frequency-domain table is carried as hi + lo (tabx<float>, opo_fft.cuh): at 10^4..10^5
+// z-steps the rounding of a single-float table entry is a coherent per-bin drift above tolerance.
+#pragma once
+#include "opo_kernels.cuh"
+
+namespace opo {
+
+template <class T> struct large_tab { using type = cplx<T>; };
+template <> struct large_tab<float> { using type = tabx<float>; };
+
+template <class T, int L, int F> struct large_cfg {
+    static constexpr int L1 = L / 2, L2 = L - L1;
+    static constexpr int N1 = 1 << L1, N2 = 1 << L2, N = 1 << L;
+    static constexpr int TC = 4;                       // columns per tile
+    static constexpr int TT1 = N1 / 16, TT2 = N2 / 16; // threads per column / row transform
+    static constexpr int NT = F * TC * TT1;            // one team per (field, column)
+    static constexpr int ROWS = NT / TT2;              // rows per chunk in the row pass
+    static constexpr int SKEW = (128 / (int)sizeof(cplx<T>)) / TC;   // makes the transposing tile load conflict-free
+    static constexpr int CSTRIDE = padded_len<T>(N1) + SKEW;
+    static constexpr int RSTRIDE = padded_len<T>(N2);
+    static constexpr int FIELD_ELEMS = (F * TC * CSTRIDE > ROWS * RSTRIDE) ? F * TC * CSTRIDE : ROWS * RSTRIDE;
+    static constexpr int TW1 = plan<L1>::tw_total, TW2 = plan<L2>::tw_total;
+    static constexpr int SMEM_ELEMS = FIELD_ELEMS + TW1 + TW2 + N1 + N2;
+    static constexpr size_t SMEM_BYTES = (size_t)SMEM_ELEMS * sizeof(cplx<T>);
+    static constexpr int TILES_PER_INST = N2 / TC;
+    static constexpr int CHUNKS_PER_FIELD = (N1 + ROWS - 1) / ROWS;
+    static_assert(ROWS >= 1, "a CTA must hold at least one row");
+};
+
+// coherent (L2) load of field data written by other SMs earlier in the same launch
+__device__ __forceinline__ cplx<float> ldcg(const cplx<float>* p) {
+    float2 v = __ldcg(reinterpret_cast<const float2*>(p));
+    return {v.x, v.y};
+}
+__device__ __forceinline__ cplx<double> ldcg(const cplx<double>* p) {
+    double2 v = __ldcg(reinterpret_cast<const double2*>(p));
+    return {v.x, v.y};
+}
+
+// All CTAs of the (cooperatively launched, hence co-resident) grid meet here.  Monotone counter:
+// barrier number j completes when the counter reaches j * gridDim.x.
+__device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned long long& target) {
+    target += gridDim.x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(ctr, 1ULL);
+        unsigned long long v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+        } while (v < target);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// inverse pass 0 -> RK4 -> forward pass 0 for butterfly t of all F fields held in local shared memory
+template <class T, int L, int F>
+__device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, const cplx<T>* __restrict__ tw0s,
+                                                cplx<T> e0, cplx<T> e1, cplx<T> e2, const T* kap, T h) {
+    constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
+    cplx<T> w[R - 1];
+#pragma unroll
+    for (int k = 0; k < R - 1; ++k) w[k] = tw0s[k * S + t];
+    const int p0 = elem_base<T, RB, SB>(0, t);
+    cplx<T> v[F][R];
+#pragma unroll
+    for (int x = 0; x < F; ++x)
+#pragma unroll
+        for (int k = 0; k < R; ++k) v[x][k] = fld[x][p0 + elem_off<T, RB, SB>(k)];
+#pragma unroll
+    for (int x = 0; x < F; ++x) {
+#pragma unroll
+        for (int k = 1; k < R; ++k) v[x][k] = cmulc(v[x][k], w[k - 1]);
+        dit_inv<T, R>::run(v[x]);
+    }
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+        cplx<T> y[F];
+#pragma unroll
+        for (int x = 0; x < F; ++x) y[x] = v[x][j];
+        Rk4<T, F>::step(y, e0, e1, e2, kap, h);
+#pragma unroll
+        for (int x = 0; x < F; ++x) v[x][j] = y[x];
+    }
+#pragma unroll
+    for (int x = 0; x < F; ++x) {
+        dif<T, R>::run(v[x]);
+#pragma unroll
+        for (int k = 1; k < R; ++k) v[x][k] = cmul(v[x][k], w[k - 1]);
+    }
+#pragma unroll
+    for (int x = 0; x < F; ++x)
+#pragma unroll
+        for (int k = 0; k < R; ++k) fld[x][p0 + elem_off<T, RB, SB>(k)] = v[x][k];
+}
+
+enum { COL_FWD = 0, COL_RK4 = 1, COL_INV = 2 };
+enum { ROW_LINEAR = 0, ROW_RELOAD = 1, ROW_FREQ = 2 };
+
+template <class T, int L, int F> struct LargeEngine {
+    using C = large_cfg<T, L, F>;
+    using TAB = typename large_tab<T>::type;
+    using P1 = plan<C::L1>;
+    using P2 = plan<C::L2>;
+
+    cplx<T>* sm;            // tile / rows
+    const cplx<T>* tw1;     // shared-memory copies
+    const cplx<T>* tw2;
+    const cplx<T>* wlo;     // W_N^j, j < N1
+    const cplx<T>* whi;     // W_N^{j N1}, j < N2
+    int tid;
+
+    __device__ __forceinline__ cplx<T> big_twiddle(int k1, int n2) const {
+        const int p = k1 * n2;
+        return cmul(whi[p >> C::L1], wlo[p & (C::N1 - 1)]);
+    }
+
+    // ---- column pass over this CTA's tiles ----------------------------------------------------------
+    // src/dst: per-field base pointers ([B][N]); fields outside `mask` are neither read nor written.
+    template <int MODE>
+    __device__ __forceinline__ void col_pass(cplx<T>* const* src, cplx<T>* const* dst, int mask, int batch,
+                                             const cplx<T>* phase, int phase_stride, int s, const T* kap, T h) {
+        const int n_tiles = batch * C::TILES_PER_INST;
+        const int team = tid / C::TT1, lt = tid % C::TT1;
+        cplx<T>* smt = sm + team * C::CSTRIDE;
+#pragma unroll 1
+        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            const int b = tile / C::TILES_PER_INST, c0 = (tile % C::TILES_PER_INST) * C::TC;
+#pragma unroll
+            for (int x = 0; x < F; ++x) {
+                if (!((mask >> x) & 1)) continue;
+                const cplx<T>* g = src[x] + (size_t)b * C::N + c0;
+#pragma unroll 4
+                for (int i = tid; i < C::N1 * C::TC; i += C::NT) {
+                    const int n1 = i / C::TC, c = i % C::TC;
+                    sm[(x * C::TC + c) * C::CSTRIDE + phys<T>(n1)] = ldcg(g + (size_t)n1 * C::N2 + c);
+                }
+            }
+            if constexpr (MODE != COL_FWD) {
+                __syncthreads();
+                inv_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
+                inv_passes<T, C::L1, C::TT1, true, (MODE == COL_INV ? 0 : 1)>(smt, tw1, lt);
+            }
+            if constexpr (MODE == COL_RK4) {
+                __syncthreads();
+                const cplx<T>* ph = phase + (size_t)b * phase_stride + 2 * s;
+                const cplx<T> e0 = ldg(ph), e1 = ldg(ph + 1), e2 = ldg(ph + 2);
+                constexpr int S = C::N1 / 4;
+#pragma unroll 1
+                for (int it = tid; it < C::TC * S; it += C::NT) {
+                    const int c = it / S, t = it % S;
+                    cplx<T>* fld[F];
+#pragma unroll
+                    for (int x = 0; x < F; ++x) fld[x] = sm + (x * C::TC + c) * C::CSTRIDE;
+                    pass0_rk4_local<T, C::L1, F>(fld, t, tw1 + P1::tw_offset(0), e0, e1, e2, kap, h);
+                }
+            }
+            if constexpr (MODE != COL_INV) {
+                __syncthreads();
+                fwd_passes<T, C::L1, C::TT1, true, (MODE == COL_FWD ? 0 : 1)>(smt, tw1, lt);
+                fwd_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int x = 0; x < F; ++x) {
+                if (!((mask >> x) & 1)) continue;
+                cplx<T>* g = dst[x] + (size_t)b * C::N + c0;
+#pragma unroll 4
+                for (int i = tid; i < C::N1 * C::TC; i += C::NT) {
+                    const int n1 = i / C::TC, c = i % C::TC;
+                    g[(size_t)n1 * C::N2 + c] = sm[(x * C::TC + c) * C::CSTRIDE + phys<T>(n1)];
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---- row pass over this CTA's chunks of ROWS rows ----------------------------------------------------
+    struct RowOp {
+        int kind[3];              // ROW_LINEAR / ROW_RELOAD / ROW_FREQ per field; -1 = skip the field
+        const TAB* tab[3];        // ROW_LINEAR: table of the field, [N] or per instance
+        long long tab_stride[3];
+        cplx<T>* sh_store[3];     // ROW_LINEAR: also store the result here (may be null)
+        const cplx<T>* aux[3];    // ROW_RELOAD: source (SH); ROW_FREQ: unused
+        cplx<T>* out[3];          // ROW_FREQ: natural-order destination
+    };
+
+    __device__ __forceinline__ void row_pass(cplx<T>* const* data, const RowOp& op, int batch, const int* __restrict__ perm1,
+                                             const int* __restrict__ perm2) {
+        const int n_chunks = batch * F * C::CHUNKS_PER_FIELD;
+        const int team = tid / C::TT2, lt = tid % C::TT2;
+        cplx<T>* smt = sm + team * C::RSTRIDE;
+#pragma unroll 1
+        for (int chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
+            const int b = chunk / (F * C::CHUNKS_PER_FIELD);
+            const int rem = chunk % (F * C::CHUNKS_PER_FIELD);
+            const int x = rem / C::CHUNKS_PER_FIELD;
+            const int r = (rem % C::CHUNKS_PER_FIELD) * C::ROWS + team;
+            const int kind = op.kind[x];
+            if (kind < 0) continue;                                 // uniform over the CTA
+            const bool active = r < C::N1;
+            const size_t off = (size_t)b * C::N + (size_t)(active ? r : 0) * C::N2;
+            cplx<T>* g = data[x] + off;
+            if (kind == ROW_RELOAD) {
+                if (active) {
+                    const cplx<T>* __restrict__ a = op.aux[x] + off;
+#pragma unroll 4
+                    for (int i = lt; i < C::N2; i += C::TT2) g[i] = ldcg(a + i);
+                }
+                continue;
+            }
+            const int k1 = __ldg(&perm1[active ? r : 0]);
+            if (active) {
+#pragma unroll 4
+                for (int i = lt; i < C::N2; i += C::TT2) smt[phys<T>(i)] = cmul(ldcg(g + i), big_twiddle(k1, i));
+            }
+            __syncthreads();
+            if (kind == ROW_FREQ) {
+                fwd_passes<T, C::L2, C::TT2, true, 0>(smt, tw2, lt);
+                fwd_pass_smem<T, C::L2, P2::P - 1, C::TT2, true>(smt, tw2, lt);
+                __syncthreads();
+                if (active) {
+                    cplx<T>* o = op.out[x] + (size_t)b * C::N + k1;
+#pragma unroll 4
+                    for (int i = lt; i < C::N2; i += C::TT2) o[(size_t)__ldg(&perm2[i]) * C::N1] = smt[phys<T>(i)];
+                }
+            } else {
+                const TAB* tab = op.tab[x] + (size_t)b * op.tab_stride[x] + (size_t)(active ? r : 0) * C::N2;
+                fwd_passes<T, C::L2, C::TT2, true, 0>(smt, tw2, lt);
+                mid_pass_smem<T, C::L2, C::TT2, TAB>(smt, tab, lt);
+                inv_passes<T, C::L2, C::TT2, true, 0>(smt, tw2, lt);
+                __syncthreads();
+                if (active) {
+                    cplx<T>* sh = op.sh_store[x] ? op.sh_store[x] + off : nullptr;
+#pragma unroll 4
+                    for (int i = lt; i < C::N2; i += C::TT2) {
+                        const cplx<T> v = cmulc(smt[phys<T>(i)], big_twiddle(k1, i));
+                        g[i] = v;
+                        if (sh) sh[i] = v;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+};
+
+template <class T, int L, int F>
+__global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a) {
+    using C = large_cfg<T, L, F>;
+    using E = LargeEngine<T, L, F>;
+    using TAB = typename E::TAB;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
+    const int tid = threadIdx.x;
+
+    E e;
+    e.sm = sm;
+    e.tid = tid;
+    {
+        cplx<T>* p = sm + C::FIELD_ELEMS;
+        auto copy = [&](const void* srcv, int count) {
+            const cplx<T>* src = reinterpret_cast<const cplx<T>*>(srcv);
+            for (int i = tid; i < count; i += C::NT) p[i] = ldg(&src[i]);
+            const cplx<T>* r = p;
+            p += count;
+            return r;
+        };
+        e.tw1 = copy(a.tw1, C::TW1);
+        e.tw2 = copy(a.tw2, C::TW2);
+        e.wlo = copy(a.wlo, C::N1);
+        e.whi = copy(a.whi, C::N2);
+    }
+    __syncthreads();
+
+    cplx<T>* cur[F];
+    cplx<T>* srcp[F];
+    cplx<T>* dstp[F];
+#pragma unroll
+    for (int x = 0; x < F; ++x) {
+        cur[x] = reinterpret_cast<cplx<T>*>(a.cur[x]);
+        srcp[x] = a.src_override[x] ? reinterpret_cast<cplx<T>*>(a.src_override[x]) : cur[x];
+        dstp[x] = cur[x];
+    }
+    const cplx<T>* phase = reinterpret_cast<const cplx<T>*>(a.phase);
+    T kap[3] = {(T)a.kappa[0], (T)a.kappa[1], (T)a.kappa[2]};
+    const T h = (T)a.h;
+    const int nz = a.nz, batch = a.batch, mask = a.field_mask;
+    unsigned long long target = a.barrier_base;
+    typename E::RowOp op;
+
+    if (a.mode == 2) {
+        // frequency read-out: column transforms src -> cur slot (scratch), rows -> natural order
+        e.template col_pass<COL_FWD>(srcp, dstp, mask, batch, phase, a.phase_stride, 0, kap, h);
+        grid_barrier(a.barrier, target);
+#pragma unroll
+        for (int x = 0; x < F; ++x) {
+            op.kind[x] = ((mask >> x) & 1) ? ROW_FREQ : -1;
+            op.out[x] = reinterpret_cast<cplx<T>*>(a.out[x]);
+        }
+        e.row_pass(cur, op, batch, a.perm1, a.perm2);
+        return;
+    }
+
+    const bool rt_mode = a.mode == 1;
+    const int total = rt_mode ? a.steps * nz : a.steps;
+
+    e.template col_pass<COL_FWD>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
+    grid_barrier(a.barrier, target);
+#pragma unroll 1
+    for (int q = 0; q <= total; ++q) {
+        const int s = rt_mode ? q % nz : a.z0 + q;
+        const bool crossing = rt_mode && q > 0 && q < total && s == 0;
+#pragma unroll
+        for (int x = 0; x < F; ++x) {
+            const bool res = a.resonant[x] != 0;
+            op.sh_store[x] = nullptr;
+            op.aux[x] = nullptr;
+            op.out[x] = nullptr;
+            op.tab_stride[x] = 0;
+            if (!((mask >> x) & 1)) { op.kind[x] = -1; continue; }
+            if (crossing && !res) {
+                op.kind[x] = ROW_RELOAD;
+                op.aux[x] = reinterpret_cast<const cplx<T>*>(a.SH[x]);
+            } else {
+                op.kind[x] = ROW_LINEAR;
+                if (q == 0 || q == total) op.tab[x] = reinterpret_cast<const TAB*>(a.tabH[x]);
+                else if (crossing) { op.tab[x] = reinterpret_cast<const TAB*>(a.tabHB[x]); op.tab_stride[x] = a.tabHB_stride[x]; }
+                else op.tab[x] = reinterpret_cast<const TAB*>(a.tabH2[x]);
+                if ((q == 0 || q == total) && a.tabH_stride[x]) op.tab_stride[x] = a.tabH_stride[x];
+                if (rt_mode && q == 0 && !res && a.steps > 1) op.sh_store[x] = reinterpret_cast<cplx<T>*>(a.SH[x]);
+            }
+        }
+        e.row_pass(cur, op, batch, a.perm1, a.perm2);
+        grid_barrier(a.barrier, target);
+        if (q == total) break;
+        e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, s, kap, h);
+        grid_barrier(a.barrier, target);
+    }
+    e.template col_pass<COL_INV>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
+}
+
+template <class T, int L, int F> cudaError_t large_setup() {
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_large<T, L, F>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)large_cfg<T, L, F>::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    return cudaSuccess;
+}
+
+template <class T, int L, int F> cudaError_t large_info_LF(int batch, int sm_count, LargeInfo* out) {
+    using C = large_cfg<T, L, F>;
+    cudaError_t e = large_setup<T, L, F>();
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_large<T, L, F>, C::NT, C::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    const long long tiles = (long long)batch * C::TILES_PER_INST;
+    const long long chunks = (long long)batch * F * C::CHUNKS_PER_FIELD;
+    long long want = tiles > chunks ? tiles : chunks;
+    const long long cap = (long long)per_sm * sm_count;
+    out->threads = C::NT;
+    out->smem_bytes = C::SMEM_BYTES;
+    out->max_ctas = (int)cap;
+    out->grid = (int)(want < cap ? want : cap);
+    out->n1 = C::N1;
+    out->n2 = C::N2;
+    return cudaSuccess;
+}
+
+template <class T, int L, int F> cudaError_t launch_large_LF(const LargeArgs& a, int grid, cudaStream_t s) {
+    using C = large_cfg<T, L, F>;
+    cudaError_t e = large_setup<T, L, F>();
+    if (e != cudaSuccess) return e;
+    LargeArgs copy = a;
+    void* params[] = {&copy};
+    return cudaLaunchCooperativeKernel((const void*)k_large<T, L, F>, dim3((unsigned)grid), dim3(C::NT), params, C::SMEM_BYTES, s);
+}
+
+template <class T, int L> cudaError_t large_info_L(int n_fields, int batch, int sm_count, LargeInfo* out) {
+    return n_fields == 3 ? large_info_LF<T, L, 3>(batch, sm_count, out) : large_info_LF<T, L, 2>(batch, sm_count, out);
+}
+template <class T, int L> cudaError_t launch_large_L(const LargeArgs& a, int grid, cudaStream_t s) {
+    return a.n_fields == 3 ? launch_large_LF<T, L, 3>(a, grid, s) : launch_large_LF<T, L, 2>(a, grid, s);
+}
+
+}  // namespace opo

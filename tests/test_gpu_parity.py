@@ -252,6 +252,78 @@ def test_config4_corners_c64(engine_idx):
 
 
 # ---------------------------------------------------------------------------------------------------------
+# large-N engine (four-step decomposition, N = 2^15 .. 2^18; complex128 also 2^14): SURVEY 8(a) S7
+# ---------------------------------------------------------------------------------------------------------
+LARGE_SIZES = [("c64", l) for l in range(15, 19)] + [("c128", l) for l in range(14, 19)]
+
+
+@pytest.mark.parametrize("precision,log2_n", LARGE_SIZES)
+def test_large_frequency_readout_matches_oracle_fft(precision, log2_n):
+    import oracle
+    torch, P = _gpu()
+    w = small_workload(log2_n, 2, precision, batch=2)
+    o = P.from_workload(w)
+    assert o.engine == P.ENGINE_LARGE
+    got = o.get_fields(1, P.WHICH_CURRENT, P.DOMAIN_FREQ).cpu().numpy().astype(np.complex128)
+    back = o.get_fields(1, P.WHICH_CURRENT, P.DOMAIN_TIME).cpu().numpy().astype(np.complex128)
+    o.close()
+    for b in range(2):
+        ref = oracle.fft(w.seeds[1][b])
+        assert rel_l2(got[b], ref) <= (1e-13 if precision == "c128" else 2e-6)
+        assert np.array_equal(back[b], w.seeds[1][b])       # the read-out does not disturb the state
+
+
+@pytest.mark.parametrize("precision,log2_n,n_fields", [
+    ("c64", 15, 3), ("c64", 16, 2), ("c64", 17, 3), ("c64", 18, 2), ("c64", 18, 3),
+    ("c128", 14, 3), ("c128", 15, 2), ("c128", 16, 3), ("c128", 17, 2), ("c128", 18, 2)])
+def test_large_single_pass_matches_oracle(precision, log2_n, n_fields):
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=4, dk=35.0, alpha=3.0)
+    cur, _, eng = run_gpu(w, P.ENGINE_AUTO, propagate=[1, 3])
+    assert eng == P.ENGINE_LARGE
+    ref, _ = run_oracle(w, propagate=[4])
+    assert_close(cur, ref, TOL[precision] if precision == "c128" else 2e-5, w.name)
+
+
+@pytest.mark.parametrize("precision,log2_n,n_fields,calls", [
+    ("c128", 14, 3, 1), ("c128", 15, 2, 3), ("c64", 15, 3, 1), ("c64", 16, 2, 3)])
+def test_large_roundtrips_with_boundary(precision, log2_n, n_fields, calls):
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=3, batch=3, dk=-20.0, gdd_dt2=-1.7, drad=0.4, strong=False)
+    w.delta_T_signal_s = np.array([-2.5, 0.0, 1.25]) * w.dt
+    cur, ex, eng = run_gpu(w, P.ENGINE_AUTO, n_roundtrips=3, calls=calls)
+    assert eng == P.ENGINE_LARGE
+    rcur, rex = run_oracle(w, n_roundtrips=3)
+    tol = TOL[precision] if precision == "c128" else 3e-5
+    assert_close(cur, rcur, tol, "current")
+    assert_close(ex, rex, tol, "exit")
+
+
+def test_large_boundary_without_transform_and_nonresonant_restart():
+    torch, P = _gpu()
+    w = small_workload(15, 3, "c128", nz=3, batch=2, dk=10.0, drad=-0.7, strong=False)
+    w.resonant = [0, 1, 0]
+    cur, ex, _ = run_gpu(w, P.ENGINE_AUTO, n_roundtrips=4)
+    rcur, rex = run_oracle(w, n_roundtrips=4)
+    assert_close(cur, rcur, 1e-10, "current")
+    assert_close(ex, rex, 1e-10, "exit")
+    assert np.array_equal(cur[:, 0], w.pump) and np.array_equal(cur[:, 2], w.seeds[2])
+
+
+def test_config3_one_roundtrip_c64():
+    """BASELINE.json configs[3] at its full grid (N = 2^18, nz = 500), one round trip (the oracle needs
+    ~20 s for it; 20 round trips are covered by sampled golden values, test_config3_golden_20rt)."""
+    torch, P = _gpu()
+    w = W.config3().truncated(1)
+    cur, ex, eng = run_gpu(w, P.ENGINE_AUTO)
+    assert eng == P.ENGINE_LARGE
+    rcur, rex = run_oracle(w)
+    e1 = assert_close(cur, rcur, 1e-4, "C3 current")
+    e2 = assert_close(ex, rex, 1e-4, "C3 exit")
+    print(f"C3 1 RT: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+# ---------------------------------------------------------------------------------------------------------
 # boundary behaviour of the ABI itself
 # ---------------------------------------------------------------------------------------------------------
 def test_abi_errors_and_state():
