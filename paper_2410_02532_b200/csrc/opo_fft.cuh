@@ -393,20 +393,161 @@ template <class T, int L> struct smem_layout {
     static constexpr size_t total = field_bytes + (tw_bytes ? tw_bytes : 16);
 };
 
+// ---- the linear core of the resident engine ----------------------------------------------------------------
 // The part of the linear operator between the two pass-0 halves: forward passes 1..P-2, middle,
 // inverse passes P-2..1, on the field at the start of dynamic shared memory with the twiddles of
 // the local passes behind it (smem_layout).  Input: the field after forward pass 0; output: the
-// field before inverse pass 0.  Barriers as for linear_op_smem.  Not inlined: one copy serves every
-// call site of a kernel (and both the two- and three-wave kernels).
+// field before inverse pass 0.
+//
+// After the radix-4 pass 0 the field is four independent sub-transforms of N/4 points, so the CTA
+// works as G = 4 thread groups (one sub-block each, NT/4 threads) that synchronise with their own
+// named barrier instead of __syncthreads: the groups drift apart, and while one waits at a barrier
+// or on shared memory the warps of the others keep the issue slots busy.  When the last two passes
+// have the same radix R (N = 2^14: 16 . 16; N = 2^10: 16 . 16) the chain
+//     forward pass P-2  ->  [last forward pass . table . first inverse pass]  ->  inverse pass P-2
+// stays inside blocks of R^2 points that one warp owns completely (two blocks per warp and
+// iteration), so it needs __syncwarp only, and the table entries of an iteration are requested from
+// L2 before its first butterfly.
+template <class T, int L, int NT> struct core_groups {
+    using PL = plan<L>;
+    static constexpr int G = (NT >= 128) ? 4 : 1;
+    static constexpr int NTG = NT / G;
+    static constexpr int RBL = PL::rbits(PL::P - 1);
+    static constexpr int NBL = ((1 << L) / G) >> RBL;     // butterflies of the last pass per group
+    static constexpr bool chain = PL::P >= 3 && PL::rbits(PL::P - 2) == RBL && NTG >= 32 && NBL % NTG == 0;
+    // early table request costs 2 R registers on top of the butterfly: fp32 only
+    static constexpr bool early_tab = sizeof(T) == 4;
+};
+
+template <int G, int NTG> __device__ __forceinline__ void group_bar(int g) {
+    if constexpr (G == 1) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(NTG) : "memory");
+}
+
+// one forward butterfly u of pass PASS (twiddles from shared memory)
+template <class T, int L, int PASS>
+__device__ __forceinline__ void fwd_bf(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int u) {
+    using PL = plan<L>;
+    constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
+    const cplx<T>* __restrict__ w = tw + PL::tw_offset(PASS);
+    const int b = u >> SB, t = u & (S - 1);
+    cplx<T>* __restrict__ p = sm + elem_base<T, RB, SB>(b, t);
+    cplx<T> v[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) v[j] = p[elem_off<T, RB, SB>(j)];
+    dif<T, R>::run(v);
+    if constexpr (SB > 0) {
+#pragma unroll
+        for (int k = 1; k < R; ++k) v[k] = cmul(v[k], w[((k - 1) << SB) + t]);
+    }
+#pragma unroll
+    for (int k = 0; k < R; ++k) p[elem_off<T, RB, SB>(k)] = v[k];
+}
+template <class T, int L, int PASS>
+__device__ __forceinline__ void inv_bf(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int u) {
+    using PL = plan<L>;
+    constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
+    const cplx<T>* __restrict__ w = tw + PL::tw_offset(PASS);
+    const int b = u >> SB, t = u & (S - 1);
+    cplx<T>* __restrict__ p = sm + elem_base<T, RB, SB>(b, t);
+    cplx<T> v[R];
+#pragma unroll
+    for (int k = 0; k < R; ++k) v[k] = p[elem_off<T, RB, SB>(k)];
+    if constexpr (SB > 0) {
+#pragma unroll
+        for (int k = 1; k < R; ++k) v[k] = cmulc(v[k], w[((k - 1) << SB) + t]);
+    }
+    dit_inv<T, R>::run(v);
+#pragma unroll
+    for (int j = 0; j < R; ++j) p[elem_off<T, RB, SB>(j)] = v[j];
+}
+// the fused middle on butterfly u with its table entries already in registers
+template <class T, int L, class TAB>
+__device__ __forceinline__ void mid_bf(cplx<T>* __restrict__ sm, const TAB* h, int u) {
+    using PL = plan<L>;
+    constexpr int RB = PL::rbits(PL::P - 1), R = 1 << RB;
+    cplx<T>* __restrict__ p = sm + elem_base<T, RB, 0>(u, 0);
+    cplx<T> v[R];
+#pragma unroll
+    for (int j = 0; j < R; ++j) v[j] = p[elem_off<T, RB, 0>(j)];
+    dif<T, R>::run(v);
+#pragma unroll
+    for (int k = 0; k < R; ++k) v[k] = tab_mul(v[k], h[k]);
+    dit_inv<T, R>::run(v);
+#pragma unroll
+    for (int j = 0; j < R; ++j) p[elem_off<T, RB, 0>(j)] = v[j];
+}
+
+// forward passes PASS .. LASTF of one group, a group barrier after each
+template <class T, int L, int NT, int PASS, int LASTF>
+__device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g, int tg) {
+    using CG = core_groups<T, L, NT>;
+    if constexpr (PASS <= LASTF) {
+        constexpr int NB = ((1 << L) / CG::G) >> plan<L>::rbits(PASS);
+#pragma unroll 1
+        for (int ul = tg; ul < NB; ul += CG::NTG) fwd_bf<T, L, PASS>(sm, twl, g * NB + ul);
+        group_bar<CG::G, CG::NTG>(g);
+        group_fwd<T, L, NT, PASS + 1, LASTF>(sm, twl, g, tg);
+    }
+}
+// inverse passes PASS .. 1 of one group, a group barrier before each
+template <class T, int L, int NT, int PASS>
+__device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g, int tg) {
+    using CG = core_groups<T, L, NT>;
+    if constexpr (PASS >= 1) {
+        constexpr int NB = ((1 << L) / CG::G) >> plan<L>::rbits(PASS);
+        group_bar<CG::G, CG::NTG>(g);
+#pragma unroll 1
+        for (int ul = tg; ul < NB; ul += CG::NTG) inv_bf<T, L, PASS>(sm, twl, g * NB + ul);
+        group_inv<T, L, NT, PASS - 1>(sm, twl, g, tg);
+    }
+}
+
+// Caller guarantees the field is visible to all threads on entry (barrier) and must barrier before
+// reading the result.  Not inlined: one copy serves every call site of a kernel.
 template <class T, int L, int NT>
-__device__ __noinline__ void linear_core_smem(const cplx<T>* tab, int tid) {
+__device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, int tid) {
+    using PL = plan<L>;
+    using CG = core_groups<T, L, NT>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
     // addressed as the global table is: twl[tw_offset(p) + ...]
-    const cplx<T>* twl = reinterpret_cast<const cplx<T>*>(smem_raw + smem_layout<T, L>::field_bytes) - plan<L>::tw_local_begin;
-    fwd_passes<T, L, NT, true, 1>(sm, twl, tid);
-    mid_pass_smem<T, L, NT>(sm, tab, tid);
-    inv_passes<T, L, NT, true, 1>(sm, twl, tid);
+    const cplx<T>* twl = reinterpret_cast<const cplx<T>*>(smem_raw + smem_layout<T, L>::field_bytes) - PL::tw_local_begin;
+    const int g = (CG::G == 1) ? 0 : tid / CG::NTG, tg = (CG::G == 1) ? tid : tid % CG::NTG;
+    constexpr int R = 1 << CG::RBL, NBF = (1 << L) >> CG::RBL;
+    if constexpr (CG::chain) {
+        group_fwd<T, L, NT, 1, PL::P - 3>(sm, twl, g, tg);
+#pragma unroll 1
+        for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
+            const int u = g * CG::NBL + ul;
+            cplx<T> h[R];
+            if constexpr (CG::early_tab) {
+#pragma unroll
+                for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
+            }
+            fwd_bf<T, L, PL::P - 2>(sm, twl, u);
+            __syncwarp();
+            if constexpr (!CG::early_tab) {
+#pragma unroll
+                for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
+            }
+            mid_bf<T, L>(sm, h, u);
+            __syncwarp();
+            inv_bf<T, L, PL::P - 2>(sm, twl, u);
+        }
+        group_inv<T, L, NT, PL::P - 3>(sm, twl, g, tg);
+    } else {
+        group_fwd<T, L, NT, 1, PL::P - 2>(sm, twl, g, tg);
+#pragma unroll 1
+        for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
+            const int u = g * CG::NBL + ul;
+            cplx<T> h[R];
+#pragma unroll
+            for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
+            mid_bf<T, L>(sm, h, u);
+        }
+        group_inv<T, L, NT, PL::P - 2>(sm, twl, g, tg);
+    }
 }
 
 // forward transform only (for frequency-domain output): result in digit-reversed order in smem

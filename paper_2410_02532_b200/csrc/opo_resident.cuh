@@ -32,21 +32,46 @@ namespace opo {
 
 namespace cg = cooperative_groups;
 
+// cluster barrier, split so that independent work can sit between arrive and wait.  release / acquire
+// at cluster scope: the distributed-shared-memory stores of the fused phase are visible to their
+// owner after the wait.
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+// Shared memory of the resident engine: smem_layout (field + twiddles of the local passes), then this
+// thread's pass-0 twiddles.  A thread handles the same pass-0 butterflies t at every z-step, so
+// their three twiddles are read from L2 once per launch: tw0s[(i * 3 + k) * NT + tid] for its i-th tile.
+template <class T, int L, int F> struct res_layout {
+    static constexpr int NT = cta_threads<T, L>::value;
+    static constexpr int S = 1 << (L - 2), NTILES = (S + 31) / 32, NW = NT / 32;
+    static constexpr int MAXT = (NTILES + F * NW - 1) / (F * NW);          // tiles per warp
+    static constexpr size_t tw0_offset = (smem_layout<T, L>::total + 15) / 16 * 16;
+    static constexpr size_t tw0_bytes = (size_t)MAXT * 3 * NT * sizeof(cplx<T>);
+    static constexpr bool tw0_smem = tw0_offset + tw0_bytes <= 232448;    // 227 KB per CTA
+    static constexpr size_t total = tw0_smem ? tw0_offset + tw0_bytes : smem_layout<T, L>::total;
+};
+
 // inverse pass 0 -> RK4 -> forward pass 0 on this CTA's share of the radix-4 butterflies
 template <class T, int L, int F, int NT>
 __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int rank, int tid, const cplx<T>* __restrict__ tw0,
-                                                cplx<T> e0, cplx<T> e1, cplx<T> e2, const T* kap, T h) {
+                                                const cplx<T>* __restrict__ tw0s, cplx<T> e0, cplx<T> e1, cplx<T> e2,
+                                                const T* kap, T h) {
     static_assert(plan<L>::rbits(0) == 2, "pass 0 must be radix 4");
     constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
     constexpr int NTILES = (S + 31) / 32, NW = NT / 32;
+    constexpr bool TWS = res_layout<T, L, F>::tw0_smem;
     const int warp = tid >> 5, lane = tid & 31;
+    int i = 0;
 #pragma unroll 1
-    for (int tile = rank + F * warp; tile < NTILES; tile += F * NW) {
+    for (int tile = rank + F * warp; tile < NTILES; tile += F * NW, ++i) {
         const int t = tile * 32 + lane;
         if (S >= 32 || t < S) {
             cplx<T> w[R - 1];
 #pragma unroll
-            for (int k = 0; k < R - 1; ++k) w[k] = ldg(&tw0[k * S + t]);
+            for (int k = 0; k < R - 1; ++k) {
+                if constexpr (TWS) w[k] = tw0s[(i * 3 + k) * NT + tid];
+                else w[k] = ldg(&tw0[k * S + t]);
+            }
             const int p0 = elem_base<T, RB, SB>(0, t);
             cplx<T> v[F][R];
 #pragma unroll
@@ -96,6 +121,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
     constexpr int N = 1 << L, NT = cta_threads<T, L>::value;
     using PL = plan<L>;
     using SL = smem_layout<T, L>;
+    using RL = res_layout<T, L, F>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
     cg::cluster_group cluster = cg::this_cluster();
@@ -111,6 +137,17 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
     {   // shared-memory copy of the twiddles of the local passes
         cplx<T>* twl = reinterpret_cast<cplx<T>*>(smem_raw + SL::field_bytes);
         for (int i = tid; i < PL::tw_local_count; i += NT) twl[i] = ldg(&tw[PL::tw_local_begin + i]);
+    }
+    const cplx<T>* tw0s = reinterpret_cast<const cplx<T>*>(smem_raw + RL::tw0_offset);
+    if constexpr (RL::tw0_smem) {   // this thread's pass-0 twiddles (see res_layout)
+        cplx<T>* d = reinterpret_cast<cplx<T>*>(smem_raw + RL::tw0_offset);
+        constexpr int S = 1 << (L - 2);
+        int i = 0;
+        for (int tile = x + F * (tid >> 5); tile < RL::NTILES; tile += F * RL::NW, ++i) {
+            const int t = tile * 32 + (tid & 31);
+            if (t < S)
+                for (int k = 0; k < 3; ++k) d[(i * 3 + k) * NT + tid] = ldg(&tw[k * S + t]);
+        }
     }
     const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
     const cplx<T>* tabH2 = reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
@@ -158,10 +195,12 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
                 store(SH);
             }
             if (q == total) break;
+            cluster_arrive();   // my field is ready for its inverse pass 0
             const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
-            cluster.sync();     // every field is ready for its inverse pass 0
-            fused_pass0_rk4<T, L, F, NT>(fld, x, tid, tw, e0, e1, e2, kap, h);
-            cluster.sync();     // every result has landed in its owner's shared memory
+            cluster_wait();     // ... and so is every other field
+            fused_pass0_rk4<T, L, F, NT>(fld, x, tid, tw, tw0s, e0, e1, e2, kap, h);
+            cluster_arrive();
+            cluster_wait();     // every result has landed in its owner's shared memory
         }
         __syncthreads();
         pass0_local<T, L, NT>(tw, tid, true);
@@ -202,7 +241,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
 
 template <class T, int L, int F> cudaError_t resident_cfg(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, int n_clusters, cudaStream_t s) {
     constexpr int NT = cta_threads<T, L>::value;
-    const size_t smem = smem_layout<T, L>::total;
+    const size_t smem = res_layout<T, L, F>::total;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(k_resident<T, L, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
