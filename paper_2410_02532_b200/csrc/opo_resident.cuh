@@ -51,9 +51,13 @@ template <class T, int L, int F> struct res_layout {
     static constexpr size_t total = tw0_smem ? tw0_offset + tw0_bytes : smem_layout<T, L>::total;
 };
 
-// inverse pass 0 -> RK4 -> forward pass 0 on this CTA's share of the radix-4 butterflies
-template <class T, int L, int F, int NT>
-__device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int rank, int tid, const cplx<T>* __restrict__ tw0,
+// inverse pass 0 -> RK4 -> forward pass 0 on this CTA's share of the radix-4 butterflies.
+// Software-pipelined over the warp's tiles: the distributed-shared-memory loads of the next tile's
+// foreign fields are issued before the arithmetic of the current one (the link moves ~16 B/clk per
+// SM, so the exchange takes about as long as the arithmetic and has to run under it).  RANK is a
+// template parameter so that "foreign" is a compile-time property of the field index.
+template <class T, int L, int F, int NT, int RANK>
+__device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, const cplx<T>* __restrict__ tw0,
                                                 const cplx<T>* __restrict__ tw0s, cplx<T> e0, cplx<T> e1, cplx<T> e2,
                                                 const T* kap, T h) {
     static_assert(plan<L>::rbits(0) == 2, "pass 0 must be radix 4");
@@ -61,23 +65,45 @@ __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int rank, i
     constexpr int NTILES = (S + 31) / 32, NW = NT / 32;
     constexpr bool TWS = res_layout<T, L, F>::tw0_smem;
     const int warp = tid >> 5, lane = tid & 31;
-    int i = 0;
-#pragma unroll 1
-    for (int tile = rank + F * warp; tile < NTILES; tile += F * NW, ++i) {
+    cplx<T> nv[F][R];                       // foreign fields of the next tile (slot RANK unused)
+    auto prefetch = [&](int tile) {
         const int t = tile * 32 + lane;
         if (S >= 32 || t < S) {
-            cplx<T> w[R - 1];
+            const int p0 = elem_base<T, RB, SB>(0, t);
+#pragma unroll
+            for (int x = 0; x < F; ++x)
+                if (x != RANK) {
+#pragma unroll
+                    for (int k = 0; k < R; ++k) nv[x][k] = fld[x][p0 + elem_off<T, RB, SB>(k)];
+                }
+        }
+    };
+    int tile = RANK + F * warp, i = 0;
+    if (tile < NTILES) prefetch(tile);
+#pragma unroll 1
+    for (; tile < NTILES; tile += F * NW, ++i) {
+        const int t = tile * 32 + lane;
+        const bool active = S >= 32 || t < S;
+        const int p0 = elem_base<T, RB, SB>(0, t);
+        cplx<T> w[R - 1];
+        cplx<T> v[F][R];
+        if (active) {
 #pragma unroll
             for (int k = 0; k < R - 1; ++k) {
                 if constexpr (TWS) w[k] = tw0s[(i * 3 + k) * NT + tid];
                 else w[k] = ldg(&tw0[k * S + t]);
             }
-            const int p0 = elem_base<T, RB, SB>(0, t);
-            cplx<T> v[F][R];
+#pragma unroll
+            for (int k = 0; k < R; ++k) v[RANK][k] = fld[RANK][p0 + elem_off<T, RB, SB>(k)];
 #pragma unroll
             for (int x = 0; x < F; ++x)
+                if (x != RANK) {
 #pragma unroll
-                for (int k = 0; k < R; ++k) v[x][k] = fld[x][p0 + elem_off<T, RB, SB>(k)];
+                    for (int k = 0; k < R; ++k) v[x][k] = nv[x][k];
+                }
+        }
+        if (tile + F * NW < NTILES) prefetch(tile + F * NW);
+        if (active) {
 #pragma unroll
             for (int x = 0; x < F; ++x) {
 #pragma unroll
@@ -198,7 +224,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
             cluster_arrive();   // my field is ready for its inverse pass 0
             const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
             cluster_wait();     // ... and so is every other field
-            fused_pass0_rk4<T, L, F, NT>(fld, x, tid, tw, tw0s, e0, e1, e2, kap, h);
+            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0>(fld, tid, tw, tw0s, e0, e1, e2, kap, h);
+            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h);
+            else fused_pass0_rk4<T, L, F, NT, F - 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h);
             cluster_arrive();
             cluster_wait();     // every result has landed in its owner's shared memory
         }
