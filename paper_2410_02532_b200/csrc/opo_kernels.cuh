@@ -14,53 +14,46 @@ namespace opo {
 // ---- RK4 of the nonlinear operator at one grid point ---------------------------------------------------
 // e0, e1, e2 = exp(i dk z) at z, z + h/2, z + h.  kap[x] real couplings.  Readings R3, R4, R5.
 template <class T, int F> struct Rk4 {
-    // f = N(y) at phase e
-    static __device__ __forceinline__ void rhs(const cplx<T>* y, cplx<T> e, const T* kap, cplx<T>* f) {
+    // g = N(y) / (i kappa) at phase e: the complex products of Eqs 2-4 without the factor i kappa_x,
+    // which step() folds into its update constants (y + c i kappa g costs one FMA per component)
+    static __device__ __forceinline__ void rhs(const cplx<T>* y, cplx<T> e, cplx<T>* g) {
         if constexpr (F == 3) {
             // dA_p = i k_p A_s A_i e^{-i dk z}
-            cplx<T> si = cmul(y[1], y[2]);
-            cplx<T> a = cmulc(si, e);
-            f[0] = {-kap[0] * a.im, kap[0] * a.re};
+            g[0] = cmulc(cmul(y[1], y[2]), e);
             // dA_s = i k_s A_p A_i^* e^{+i dk z},  dA_i = i k_i A_p A_s^* e^{+i dk z}
-            cplx<T> pe = cmul(y[0], e);
-            cplx<T> b = cmulc(pe, y[2]);
-            cplx<T> c = cmulc(pe, y[1]);
-            f[1] = {-kap[1] * b.im, kap[1] * b.re};
-            f[2] = {-kap[2] * c.im, kap[2] * c.re};
+            const cplx<T> pe = cmul(y[0], e);
+            g[1] = cmulc(pe, y[2]);
+            g[2] = cmulc(pe, y[1]);
         } else {
             // dA_p = i (k_p/2) A_s^2 e^{-i dk z}   (kap[0] holds k_p/2),  dA_s = i k_s A_p A_s^* e^{+i dk z}
-            cplx<T> ss = cmul(y[1], y[1]);
-            cplx<T> a = cmulc(ss, e);
-            f[0] = {-kap[0] * a.im, kap[0] * a.re};
-            cplx<T> pe = cmul(y[0], e);
-            cplx<T> b = cmulc(pe, y[1]);
-            f[1] = {-kap[1] * b.im, kap[1] * b.re};
+            g[0] = cmulc(cmul(y[1], y[1]), e);
+            g[1] = cmulc(cmul(y[0], e), y[1]);
         }
     }
+    // a + c * (i g)
+    static __device__ __forceinline__ cplx<T> axpy_i(cplx<T> a, T c, cplx<T> g) { return {a.re - c * g.im, a.im + c * g.re}; }
     static __device__ __forceinline__ void step(cplx<T>* y, cplx<T> e0, cplx<T> e1, cplx<T> e2, const T* kap, T h) {
-        cplx<T> k[F], t[F], acc[F];
-        const T h2 = (T)0.5 * h, h6 = h / (T)6, h3 = h / (T)3;
-        rhs(y, e0, kap, k);
+        cplx<T> g[F], t[F], acc[F];
+        T c2[F], c3[F], c6[F], c1[F];
 #pragma unroll
         for (int x = 0; x < F; ++x) {
-            acc[x] = {y[x].re + h6 * k[x].re, y[x].im + h6 * k[x].im};
-            t[x] = {y[x].re + h2 * k[x].re, y[x].im + h2 * k[x].im};
+            c1[x] = h * kap[x];
+            c2[x] = (T)0.5 * c1[x];
+            c3[x] = c1[x] / (T)3;
+            c6[x] = c1[x] / (T)6;
         }
-        rhs(t, e1, kap, k);
+        rhs(y, e0, g);
 #pragma unroll
-        for (int x = 0; x < F; ++x) {
-            acc[x] = {acc[x].re + h3 * k[x].re, acc[x].im + h3 * k[x].im};
-            t[x] = {y[x].re + h2 * k[x].re, y[x].im + h2 * k[x].im};
-        }
-        rhs(t, e1, kap, k);
+        for (int x = 0; x < F; ++x) { acc[x] = axpy_i(y[x], c6[x], g[x]); t[x] = axpy_i(y[x], c2[x], g[x]); }
+        rhs(t, e1, g);
 #pragma unroll
-        for (int x = 0; x < F; ++x) {
-            acc[x] = {acc[x].re + h3 * k[x].re, acc[x].im + h3 * k[x].im};
-            t[x] = {y[x].re + h * k[x].re, y[x].im + h * k[x].im};
-        }
-        rhs(t, e2, kap, k);
+        for (int x = 0; x < F; ++x) { acc[x] = axpy_i(acc[x], c3[x], g[x]); t[x] = axpy_i(y[x], c2[x], g[x]); }
+        rhs(t, e1, g);
 #pragma unroll
-        for (int x = 0; x < F; ++x) y[x] = {acc[x].re + h6 * k[x].re, acc[x].im + h6 * k[x].im};
+        for (int x = 0; x < F; ++x) { acc[x] = axpy_i(acc[x], c3[x], g[x]); t[x] = axpy_i(y[x], c1[x], g[x]); }
+        rhs(t, e2, g);
+#pragma unroll
+        for (int x = 0; x < F; ++x) y[x] = axpy_i(acc[x], c6[x], g[x]);
     }
 };
 
