@@ -41,13 +41,23 @@ def flops_per_grid_point_zstep(log2_n: int, n_fields: int) -> float:
     return n_fields * (2 * 5 * log2_n + 6 + 76)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu captures
+# of exactly this launch configuration (profiles/r01e_*.md); None where no capture of that configuration exists.
+NCU_DRAM_BYTES_PER_LAUNCH = {
+    # (workload, engine, round trips per step): bytes
+    ("C4", "resident", 300): 185325824 + 242958080,     # profiles/r01e_dram_c4_default.csv (one 3.16 s launch)
+}
+
+
+def ncu_traffic_bytes(workload: str, engine: str, rt_per_step: int):
+    return NCU_DRAM_BYTES_PER_LAUNCH.get((workload, engine, rt_per_step))
+
+
 def make_workload(name: str, rank: int):
-    if name == "C4":
-        w = W.config4()
-    elif name == "C1":
-        w = W.config1()
-    else:
+    makers = {"C0": W.config0, "C1": W.config1, "C2": W.config2, "C3": W.config3, "C4": W.config4}
+    if name not in makers:
         raise SystemExit(f"unknown workload {name}")
+    w = makers[name]()
     if rank:   # other ranks run their own sweep with their own seeds (weak scaling, no collective)
         rng = np.random.default_rng(1000 + rank)
         for x in range(1, w.n_fields):
@@ -134,7 +144,7 @@ def run_reference(args, rank, world):
     line = {"metric": METRIC, "value": val, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{w.name} (BASELINE.json configs[{4 if args.workload == 'C4' else 1}])", "sample": sample},
+            "config": {"workload": f"{w.name} (BASELINE.json configs[{args.workload[1]}])", "sample": sample},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": len(inst), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "round_trips_per_s": len(inst) * rt / dt, "gpu_launches": 0}
@@ -165,8 +175,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C4", choices=["C4", "C1"])
-    ap.add_argument("--rt-per-step", type=int, default=0, help="round trips per step (default: the config's full length for C4, 100 for C1)")
+    ap.add_argument("--workload", default="C4", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--rt-per-step", type=int, default=0, help="round trips per step (default: the config's full length for C4 and C0, 100 for C1, 20 for C2, 2 for C3)")
     ap.add_argument("--engine", default="auto", choices=["auto", "resident", "streaming"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -197,7 +207,7 @@ def main():
         torch.cuda.synchronize()
 
     w = make_workload(args.workload, rank)
-    rt_per_step = args.rt_per_step or (w.n_roundtrips if args.workload == "C4" else 100)
+    rt_per_step = args.rt_per_step or {"C0": w.n_roundtrips, "C1": 100, "C2": 20, "C3": 2, "C4": w.n_roundtrips}[args.workload]
     engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "streaming": P.ENGINE_STREAMING}[args.engine]
     o = P.from_workload(w, engine=engine)
     units_per_step = w.batch * w.n * w.nz_per_pass * rt_per_step          # grid-point z-steps, this rank
@@ -271,21 +281,41 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (resident engine: FP32 pipe) ----------------------------------
-    fl = flops_per_grid_point_zstep(w.log2_n, w.n_fields) * units_per_step          # per launch (= per step)
+    # ---- roofline of the dominant kernel ----------------------------------------------------
     avg_s = statistics.mean(per_step_ms) * 1e-3
-    peak_tflops = 148 * 128 * 2 * 1.965e9 / 1e12
-    roofline = {"bound": "alu", "kernel": "k_resident" if o.engine == P.ENGINE_RESIDENT else "k_linear+k_rk4",
-                "achieved": fl / avg_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s", "frac": fl / avg_s / 1e12 / peak_tflops,
-                "traffic": None,
-                "note": "FP32 FMA-pipe peak = 148 SM x 128 lanes x 2 x 1.965 GHz (guide unit counts, max clock); algorithmic flops = "
-                        f"{flops_per_grid_point_zstep(w.log2_n, w.n_fields):.0f}/grid-point z-step (merged half-steps, 5 N log2 N per transform)"}
+    eng = o.engine
+    eng_name = {P.ENGINE_RESIDENT: "resident", P.ENGINE_STREAMING: "streaming", P.ENGINE_LARGE: "large"}.get(eng, str(eng))
+    traffic = ncu_traffic_bytes(args.workload, eng_name, rt_per_step)
+    if eng == P.ENGINE_RESIDENT:
+        # fields stay in shared memory: bound by FP32 instruction issue
+        fl = flops_per_grid_point_zstep(w.log2_n, w.n_fields) * units_per_step          # per launch (= per step)
+        dbl = w.precision == "c128"
+        peak_tflops = 148 * (64 if dbl else 128) * 2 * 1.965e9 / 1e12
+        roofline = {"bound": "alu", "kernel": "k_resident", "achieved": fl / avg_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
+                    "frac": fl / avg_s / 1e12 / peak_tflops, "traffic": traffic,
+                    "note": f"{'FP64' if dbl else 'FP32'} FMA-pipe peak = 148 SM x {64 if dbl else 128} lanes x 2 x 1.965 GHz (guide unit counts, max clock); "
+                            f"algorithmic flops = {flops_per_grid_point_zstep(w.log2_n, w.n_fields):.0f}/grid-point z-step "
+                            "(merged half-steps, 5 N log2 N per transform); one launch = one step"}
+    else:
+        # fields stream through L2 / HBM: algorithmic bytes per field-point z-step: large engine 32 B
+        # (row pass R+W, column pass R+W), streaming engine 40 B (linear R+W + table, RK4 R+W)
+        esz = 16 if w.precision == "c128" else 8
+        per_fp = (4 * esz) if eng == P.ENGINE_LARGE else (5 * esz)
+        by = per_fp * w.n_fields * units_per_step
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+        peak = float(peaks.get("hbm_gbs", 6543.1))
+        n_launch = max(1, int(launches) // max(1, args.steps))
+        roofline = {"bound": "hbm", "kernel": "k_large" if eng == P.ENGINE_LARGE else "k_linear+k_rk4", "achieved": by / avg_s / 1e9,
+                    "peak": peak, "unit": "GB/s", "frac": by / avg_s / 1e9 / peak, "traffic": traffic,
+                    "note": f"algorithmic bytes = {per_fp} B per field-point z-step; peak = measured HBM copy bandwidth "
+                            f"({'MEASURED_PEAKS.json' if peaks else 'B200_PROFILING.md fallback'}); {n_launch} launch(es) per step; "
+                            "the state of this workload is L2-resident, so this is L2 service measured against the HBM roofline"}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if w.precision == "c64" else "f64", "data": "synthetic",
-            "config": {"workload": f"{w.name}: BASELINE.json configs[{4 if args.workload == 'C4' else 1}], batch {w.batch} x N=2^{w.log2_n} x "
+            "config": {"workload": f"{w.name}: BASELINE.json configs[{args.workload[1]}], batch {w.batch} x N=2^{w.log2_n} x "
                                    f"{w.n_fields} fields, nz={w.nz_per_pass}, {rt_per_step} round trips per step",
-                       "engine": "resident" if o.engine == P.ENGINE_RESIDENT else "streaming",
+                       "engine": eng_name,
                        "l2": "512 MiB flush write between timed steps", "sharding": "independent instances per rank, no collective"},
             "round_trips_per_s": world * w.batch * rt_per_step * args.steps / t_total,
             "field_point_z_steps_per_s": value * w.n_fields,

@@ -419,6 +419,55 @@ template <class T, int L, int NT> struct core_groups {
     static constexpr bool early_tab = sizeof(T) == 4;
 };
 
+// ---- class-granular cluster synchronisation ("flow") ------------------------------------------------------
+// Pass 1 has stride S1 inside a sub-block; its butterfly t' touches the elements t' + S1 k and the
+// pass-0 butterflies t (fused with RK4 in the resident engine, shared out over the cluster in tiles
+// of 32) touch one element t of every sub-block.  So the tiles of *class* c = (t mod S1) / 32 depend
+// only on the pass-1 butterflies of class c of every field, and vice versa: the two cluster-wide
+// barriers of a z-step become 2 NCLS mbarriers per CTA,
+//     ready[c]: every field's inverse pass 1 of class c is done   (G F arrivals: one warp per group and CTA)
+//     done[c] : every tile of class c is integrated and written    (F NW / NCLS arrivals: the warps owning them)
+// A warp waits only for the classes it touches; a warp that is half a phase late delays nobody.
+template <class T, int L, int NT> struct flow_cfg {
+    using PL = plan<L>;
+    static constexpr int G = (NT >= 128) ? 4 : 1, NTG = NT / G, NWG = NTG / 32, NW = NT / 32;
+    static constexpr int S1 = (PL::P >= 3) ? (1 << PL::sbits(PL::P >= 3 ? 1 : 0)) : 0;
+    static constexpr int NCLS = S1 / 32;
+    static constexpr int NB1 = (PL::P >= 3) ? (((1 << L) / G) >> PL::rbits(1)) : 0;
+    static constexpr int NIT = (NTG > 0 && NB1 > 0) ? NB1 / NTG : 0;
+    // pass 1 exists, is a shared-memory pass of its own, whole warps per class, every warp NIT classes
+    static constexpr bool ok = G == 4 && PL::P >= 4 && NCLS >= 1 && NB1 % NTG == 0 && NIT * NWG == NCLS;
+};
+
+__device__ __forceinline__ void mbar_init(uint32_t addr, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(addr), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t addr, uint32_t parity) {
+    asm volatile(
+        "{\n.reg .pred P1;\nLAB_WAIT:\n"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(addr), "r"(parity)
+        : "memory");
+}
+// lanes 0 .. nf-1 of a converged warp arrive on the barrier at local address `addr` in CTA `lane`;
+// release at cluster scope, after a __syncwarp that orders the other lanes' writes before it
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t addr, int lane, int nf) {
+    __syncwarp();
+    if (lane < nf) {
+        uint32_t remote;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(addr), "r"(lane));
+        asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
+    }
+}
+// runtime description of the synchronisation around one linear core
+struct FlowArgs {
+    uint32_t mb;        // shared address of ready[0]; done[c] = mb + 8 (NCLS + c)
+    int nf;             // CTAs in the cluster
+    int wait_in;        // forward pass 1 waits for done[class] (a fused phase precedes)
+    int arrive_out;     // inverse pass 1 arrives on ready[class] (a fused phase follows)
+    uint32_t par_done;  // parity of the done phase to wait for
+};
+
 template <int G, int NTG> __device__ __forceinline__ void group_bar(int g) {
     if constexpr (G == 1) __syncthreads();
     else asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(NTG) : "memory");
@@ -479,34 +528,52 @@ __device__ __forceinline__ void mid_bf(cplx<T>* __restrict__ sm, const TAB* h, i
 }
 
 // forward passes PASS .. LASTF of one group, a group barrier after each
-template <class T, int L, int NT, int PASS, int LASTF>
-__device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g, int tg) {
+template <class T, int L, int NT, int PASS, int LASTF, bool FLOW>
+__device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g, int tg, const FlowArgs& fa) {
     using CG = core_groups<T, L, NT>;
     if constexpr (PASS <= LASTF) {
         constexpr int NB = ((1 << L) / CG::G) >> plan<L>::rbits(PASS);
+        if constexpr (FLOW && PASS == 1) {
+            using FC = flow_cfg<T, L, NT>;
 #pragma unroll 1
-        for (int ul = tg; ul < NB; ul += CG::NTG) fwd_bf<T, L, PASS>(sm, twl, g * NB + ul);
+            for (int it = 0; it < FC::NIT; ++it) {
+                if (fa.wait_in) mbar_wait(fa.mb + 8 * (FC::NCLS + (tg >> 5) + FC::NWG * it), fa.par_done);
+                fwd_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
+            }
+        } else {
+#pragma unroll 1
+            for (int ul = tg; ul < NB; ul += CG::NTG) fwd_bf<T, L, PASS>(sm, twl, g * NB + ul);
+        }
         group_bar<CG::G, CG::NTG>(g);
-        group_fwd<T, L, NT, PASS + 1, LASTF>(sm, twl, g, tg);
+        group_fwd<T, L, NT, PASS + 1, LASTF, FLOW>(sm, twl, g, tg, fa);
     }
 }
 // inverse passes PASS .. 1 of one group, a group barrier before each
-template <class T, int L, int NT, int PASS>
-__device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g, int tg) {
+template <class T, int L, int NT, int PASS, bool FLOW>
+__device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g, int tg, const FlowArgs& fa) {
     using CG = core_groups<T, L, NT>;
     if constexpr (PASS >= 1) {
         constexpr int NB = ((1 << L) / CG::G) >> plan<L>::rbits(PASS);
         group_bar<CG::G, CG::NTG>(g);
+        if constexpr (FLOW && PASS == 1) {
+            using FC = flow_cfg<T, L, NT>;
 #pragma unroll 1
-        for (int ul = tg; ul < NB; ul += CG::NTG) inv_bf<T, L, PASS>(sm, twl, g * NB + ul);
-        group_inv<T, L, NT, PASS - 1>(sm, twl, g, tg);
+            for (int it = 0; it < FC::NIT; ++it) {
+                inv_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
+                if (fa.arrive_out) mbar_arrive_cluster(fa.mb + 8 * ((tg >> 5) + FC::NWG * it), tg & 31, fa.nf);
+            }
+        } else {
+#pragma unroll 1
+            for (int ul = tg; ul < NB; ul += CG::NTG) inv_bf<T, L, PASS>(sm, twl, g * NB + ul);
+        }
+        group_inv<T, L, NT, PASS - 1, FLOW>(sm, twl, g, tg, fa);
     }
 }
 
 // Caller guarantees the field is visible to all threads on entry (barrier) and must barrier before
 // reading the result.  Not inlined: one copy serves every call site of a kernel.
-template <class T, int L, int NT>
-__device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, int tid) {
+template <class T, int L, int NT, bool FLOW = false>
+__device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, int tid, FlowArgs fa = FlowArgs{}) {
     using PL = plan<L>;
     using CG = core_groups<T, L, NT>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -516,7 +583,7 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
     const int g = (CG::G == 1) ? 0 : tid / CG::NTG, tg = (CG::G == 1) ? tid : tid % CG::NTG;
     constexpr int R = 1 << CG::RBL, NBF = (1 << L) >> CG::RBL;
     if constexpr (CG::chain) {
-        group_fwd<T, L, NT, 1, PL::P - 3>(sm, twl, g, tg);
+        group_fwd<T, L, NT, 1, PL::P - 3, FLOW>(sm, twl, g, tg, fa);
 #pragma unroll 1
         for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
             const int u = g * CG::NBL + ul;
@@ -535,9 +602,9 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
             __syncwarp();
             inv_bf<T, L, PL::P - 2>(sm, twl, u);
         }
-        group_inv<T, L, NT, PL::P - 3>(sm, twl, g, tg);
+        group_inv<T, L, NT, PL::P - 3, FLOW>(sm, twl, g, tg, fa);
     } else {
-        group_fwd<T, L, NT, 1, PL::P - 2>(sm, twl, g, tg);
+        group_fwd<T, L, NT, 1, PL::P - 2, FLOW>(sm, twl, g, tg, fa);
 #pragma unroll 1
         for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
             const int u = g * CG::NBL + ul;
@@ -546,7 +613,7 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
             for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
             mid_bf<T, L>(sm, h, u);
         }
-        group_inv<T, L, NT, PL::P - 2>(sm, twl, g, tg);
+        group_inv<T, L, NT, PL::P - 2, FLOW>(sm, twl, g, tg, fa);
     }
 }
 
