@@ -28,6 +28,7 @@
 // compile-time offsets (elem_addr below).
 #pragma once
 #include <cuda_runtime.h>
+#include <cstdint>
 #include <utility>
 
 namespace opo {

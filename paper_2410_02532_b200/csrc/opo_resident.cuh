@@ -48,7 +48,15 @@ template <class T, int L, int F> struct res_layout {
     static constexpr size_t tw0_offset = (smem_layout<T, L>::total + 15) / 16 * 16;
     static constexpr size_t tw0_bytes = (size_t)MAXT * 3 * NT * sizeof(cplx<T>);
     static constexpr bool tw0_smem = tw0_offset + tw0_bytes <= 232448;    // 227 KB per CTA
-    static constexpr size_t total = tw0_smem ? tw0_offset + tw0_bytes : smem_layout<T, L>::total;
+    static constexpr size_t data_end = tw0_smem ? tw0_offset + tw0_bytes : smem_layout<T, L>::total;
+    // flow synchronisation (opo_fft.cuh): ready[NCLS], done[NCLS] mbarriers
+    using FC = flow_cfg<T, L, NT>;
+    static constexpr bool flow = FC::ok && (F * FC::NW) % (FC::NCLS > 0 ? FC::NCLS : 1) == 0 && NTILES % 1 == 0 && S >= 32 &&
+                                 F * NW <= NTILES;      // every warp owns at least one tile
+    static constexpr size_t mbar_offset = (data_end + 15) / 16 * 16;
+    static constexpr size_t total = flow ? mbar_offset + 16 * (size_t)(FC::NCLS > 0 ? FC::NCLS : 1) : data_end;
+    static constexpr int done_count = flow ? F * FC::NW / FC::NCLS : 0;
+    static constexpr int ready_count = FC::G * F;
 };
 
 // inverse pass 0 -> RK4 -> forward pass 0 on this CTA's share of the radix-4 butterflies.
@@ -59,8 +67,9 @@ template <class T, int L, int F> struct res_layout {
 template <class T, int L, int F, int NT, int RANK>
 __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, const cplx<T>* __restrict__ tw0,
                                                 const cplx<T>* __restrict__ tw0s, cplx<T> e0, cplx<T> e1, cplx<T> e2,
-                                                const T* kap, T h) {
+                                                const T* kap, T h, uint32_t mb, uint32_t parity) {
     static_assert(plan<L>::rbits(0) == 2, "pass 0 must be radix 4");
+    using RL = res_layout<T, L, F>;
     constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
     constexpr int NTILES = (S + 31) / 32, NW = NT / 32;
     constexpr bool TWS = res_layout<T, L, F>::tw0_smem;
@@ -79,6 +88,9 @@ __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, co
         }
     };
     int tile = RANK + F * warp, i = 0;
+    // all tiles of a warp belong to one class (F NW is a multiple of NCLS)
+    const int cls = RL::flow ? tile % (RL::FC::NCLS > 0 ? RL::FC::NCLS : 1) : 0;
+    if constexpr (RL::flow) mbar_wait(mb + 8 * cls, parity);      // ready[cls]: every field's inverse pass 1 of my class
     if (tile < NTILES) prefetch(tile);
 #pragma unroll 1
     for (; tile < NTILES; tile += F * NW, ++i) {
@@ -131,6 +143,7 @@ __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, co
                 for (int k = 0; k < R; ++k) fld[x][p0 + elem_off<T, RB, SB>(k)] = v[x][k];
         }
     }
+    if constexpr (RL::flow) mbar_arrive_cluster(mb + 8 * (RL::FC::NCLS + cls), lane, F);   // done[cls] in every CTA
 }
 
 // stand-alone pass 0 on the CTA's own field (the first and last linear operator of a call)
@@ -175,6 +188,30 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
                 for (int k = 0; k < 3; ++k) d[(i * 3 + k) * NT + tid] = ldg(&tw[k * S + t]);
         }
     }
+    constexpr bool FLOW = RL::flow;
+    using FC = flow_cfg<T, L, NT>;
+    const uint32_t mb = (uint32_t)__cvta_generic_to_shared(smem_raw + RL::mbar_offset);
+    if constexpr (FLOW) {
+        if (tid == 0) {
+            for (int c = 0; c < FC::NCLS; ++c) {
+                mbar_init(mb + 8 * c, RL::ready_count);
+                mbar_init(mb + 8 * (FC::NCLS + c), RL::done_count);
+            }
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        cluster.sync();     // every CTA's barriers exist before anybody arrives on them
+    }
+    uint32_t fz = 0;        // fused phases executed so far by this cluster (mbarrier phase parity)
+    // this warp's classes in pass 1 (as in group_fwd / group_inv)
+    const int wg = (tid % FC::NTG) >> 5, lane = tid & 31;
+    auto flow_wait_done_all = [&](uint32_t parity) {      // the previous fused phase has released all of my field
+        if constexpr (FLOW)
+            for (int it = 0; it < FC::NIT; ++it) mbar_wait(mb + 8 * (FC::NCLS + wg + FC::NWG * it), parity);
+    };
+    auto flow_arrive_ready_all = [&]() {                   // stands in for the arrivals of an inverse pass 1
+        if constexpr (FLOW)
+            for (int it = 0; it < FC::NIT; ++it) mbar_arrive_cluster(mb + 8 * (wg + FC::NWG * it), lane, F);
+    };
     const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
     const cplx<T>* tabH2 = reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
     const bool resonant = a.resonant[x] != 0;
@@ -210,25 +247,40 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
         for (int q = 0; q <= total; ++q) {
             const int s = rt_mode ? q % nz : a.z0 + q;          // index of the RK4 step that follows
             const bool crossing = rt_mode && q > 0 && q < total && s == 0;
+            const bool keep = rt_mode && q == 0 && !resonant && a.steps > 1;   // SH <- first half-stepped input
             if (crossing && !resonant) {
+                if constexpr (FLOW) { flow_wait_done_all((fz - 1) & 1); __syncthreads(); }
                 load(SH);                                        // fresh pump / frozen seed, already half-stepped
+                if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }
             } else {
                 const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
-                linear_core_smem<T, L, NT>(tab, tid);
+                if constexpr (FLOW) {
+                    FlowArgs fa;
+                    fa.mb = mb; fa.nf = F;
+                    fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
+                    fa.arrive_out = (q < total) && !keep;
+                    linear_core_smem<T, L, NT, true>(tab, tid, fa);
+                } else {
+                    linear_core_smem<T, L, NT>(tab, tid);
+                }
             }
-            if (rt_mode && q == 0 && !resonant && a.steps > 1) {   // keep it for the later round trips
+            if (keep) {   // keep it for the later round trips
                 __syncthreads();
                 store(SH);
+                if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }   // only now may the peers write into my field
             }
             if (q == total) break;
-            cluster_arrive();   // my field is ready for its inverse pass 0
+            if constexpr (!FLOW) cluster_arrive();   // my field is ready for its inverse pass 0
             const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
-            cluster_wait();     // ... and so is every other field
-            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0>(fld, tid, tw, tw0s, e0, e1, e2, kap, h);
-            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h);
-            else fused_pass0_rk4<T, L, F, NT, F - 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h);
-            cluster_arrive();
-            cluster_wait();     // every result has landed in its owner's shared memory
+            if constexpr (!FLOW) cluster_wait();     // ... and so is every other field
+            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
+            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
+            else fused_pass0_rk4<T, L, F, NT, F - 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
+            ++fz;
+            if constexpr (!FLOW) {
+                cluster_arrive();
+                cluster_wait();     // every result has landed in its owner's shared memory
+            }
         }
         __syncthreads();
         pass0_local<T, L, NT>(tw, tid, true);
