@@ -427,8 +427,7 @@ template <class T, int L, int NT> struct core_groups {
 // only on the pass-1 butterflies of class c of every field, and vice versa: the two cluster-wide
 // barriers of a z-step become 2 NCLS mbarriers per CTA,
 //     ready[c]: every field's inverse pass 1 of class c is done   (G F arrivals: one warp per group and CTA)
-//     done[c] : every tile of class c is integrated and written    (local warps owning such tiles + 1 waiter, plus the
-//               bytes the other CTAs deliver with st.async)
+//     done[c] : every tile of class c is integrated and written    (F NW / NCLS arrivals: the warps owning them)
 // A warp waits only for the classes it touches; a warp that is half a phase late delays nobody.
 template <class T, int L, int NT> struct flow_cfg {
     using PL = plan<L>;
@@ -451,51 +450,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t addr, uint32_t parity) {
         "@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(addr), "r"(parity)
         : "memory");
 }
-// ready side: lanes 0 .. nf-1 of a converged warp arrive, in CTA `lane`, on the ready barriers of this
-// warp's NIT classes (wgi + NWG it).  ONE cluster-scope release fence (MEMBAR.ALL.GPU on this part,
-// ~900 cycles) covers all of them; the __syncwarp orders the other lanes' shared-memory writes before it.
-template <int NIT, int NWG>
-__device__ __forceinline__ void mbar_arrive_ready(uint32_t mb, int wgi, int lane, int nf) {
+// lanes 0 .. nf-1 of a converged warp arrive on the barrier at local address `addr` in CTA `lane`;
+// release at cluster scope, after a __syncwarp that orders the other lanes' writes before it
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t addr, int lane, int nf) {
     __syncwarp();
     if (lane < nf) {
-        asm volatile("fence.acq_rel.cluster;" ::: "memory");
-#pragma unroll
-        for (int it = 0; it < NIT; ++it) {
-            uint32_t remote;
-            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(mb + 8 * (wgi + NWG * it)), "r"(lane));
-            asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
-        }
+        uint32_t remote;
+        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(addr), "r"(lane));
+        asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
     }
-}
-// done side.  Results for a foreign field travel as st.async (remote store that completes bytes on the
-// owner's done barrier: no fence at all); results for the own field are plain shared-memory stores
-// followed by a CTA-scope arrival.  The designated waiter posts the bytes its CTA expects for the
-// phase (txb[c], next to the barriers) together with its own arrival, then everybody waits.
-__device__ __forceinline__ void mbar_arrive_local(uint32_t addr, int lane) {
-    __syncwarp();
-    if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(addr) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_done(uint32_t addr, uint32_t txb_addr, uint32_t parity, bool designated, int lane) {
-    if (designated && lane == 0) {
-        uint32_t bytes;
-        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(bytes) : "r"(txb_addr));
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(addr), "r"(bytes) : "memory");
-    }
-    mbar_wait(addr, parity);
-}
-__device__ __forceinline__ void st_async(uint32_t addr, cplx<float> v, uint32_t mbar) {
-    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(addr), "f"(v.re),
-                 "f"(v.im), "r"(mbar)
-                 : "memory");
-}
-__device__ __forceinline__ void st_async(uint32_t addr, cplx<double> v, uint32_t mbar) {
-    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(addr), "d"(v.re),
-                 "d"(v.im), "r"(mbar)
-                 : "memory");
 }
 // runtime description of the synchronisation around one linear core
 struct FlowArgs {
-    uint32_t mb;        // shared address of ready[0]; done[c] = mb + 8 (NCLS + c); txb[c] = mb + 16 NCLS + 4 c
+    uint32_t mb;        // shared address of ready[0]; done[c] = mb + 8 (NCLS + c)
     int nf;             // CTAs in the cluster
     int wait_in;        // forward pass 1 waits for done[class] (a fused phase precedes)
     int arrive_out;     // inverse pass 1 arrives on ready[class] (a fused phase follows)
@@ -571,10 +538,7 @@ __device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g
             using FC = flow_cfg<T, L, NT>;
 #pragma unroll 1
             for (int it = 0; it < FC::NIT; ++it) {
-                if (fa.wait_in) {
-                    const int c = (tg >> 5) + FC::NWG * it;
-                    mbar_wait_done(fa.mb + 8 * (FC::NCLS + c), fa.mb + 16 * FC::NCLS + 4 * c, fa.par_done, g == 0, tg & 31);
-                }
+                if (fa.wait_in) mbar_wait(fa.mb + 8 * (FC::NCLS + (tg >> 5) + FC::NWG * it), fa.par_done);
                 fwd_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
             }
         } else {
@@ -597,8 +561,8 @@ __device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g
 #pragma unroll 1
             for (int it = 0; it < FC::NIT; ++it) {
                 inv_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
+                if (fa.arrive_out) mbar_arrive_cluster(fa.mb + 8 * ((tg >> 5) + FC::NWG * it), tg & 31, fa.nf);
             }
-            if (fa.arrive_out) mbar_arrive_ready<FC::NIT, FC::NWG>(fa.mb, tg >> 5, tg & 31, fa.nf);
         } else {
 #pragma unroll 1
             for (int ul = tg; ul < NB; ul += CG::NTG) inv_bf<T, L, PASS>(sm, twl, g * NB + ul);

@@ -54,9 +54,9 @@ template <class T, int L, int F> struct res_layout {
     static constexpr bool flow = FC::ok && (F * FC::NW) % (FC::NCLS > 0 ? FC::NCLS : 1) == 0 && NTILES % 1 == 0 && S >= 32 &&
                                  F * NW <= NTILES;      // every warp owns at least one tile
     static constexpr size_t mbar_offset = (data_end + 15) / 16 * 16;
-    static constexpr size_t total = flow ? mbar_offset + 20 * (size_t)(FC::NCLS > 0 ? FC::NCLS : 1) : data_end;   // + txb[NCLS]
+    static constexpr size_t total = flow ? mbar_offset + 16 * (size_t)(FC::NCLS > 0 ? FC::NCLS : 1) : data_end;
+    static constexpr int done_count = flow ? F * FC::NW / FC::NCLS : 0;
     static constexpr int ready_count = FC::G * F;
-    static constexpr int tile_bytes = 4 * 32 * (int)sizeof(cplx<T>);       // one tile of one field
 };
 
 // inverse pass 0 -> RK4 -> forward pass 0 on this CTA's share of the radix-4 butterflies.
@@ -67,7 +67,7 @@ template <class T, int L, int F> struct res_layout {
 template <class T, int L, int F, int NT, int RANK>
 __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, const cplx<T>* __restrict__ tw0,
                                                 const cplx<T>* __restrict__ tw0s, cplx<T> e0, cplx<T> e1, cplx<T> e2,
-                                                const T* kap, T h, uint32_t mb, uint32_t parity, const uint32_t* rb) {
+                                                const T* kap, T h, uint32_t mb, uint32_t parity) {
     static_assert(plan<L>::rbits(0) == 2, "pass 0 must be radix 4");
     using RL = res_layout<T, L, F>;
     constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
@@ -138,21 +138,12 @@ __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, co
                 for (int k = 1; k < R; ++k) v[x][k] = cmul(v[x][k], w[k - 1]);
             }
 #pragma unroll
-            for (int x = 0; x < F; ++x) {
-                if (RL::flow && x != RANK) {
-                    uint32_t rbar;      // done[cls] of the owner
-                    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rbar) : "r"(mb + 8 * (RL::FC::NCLS + cls)), "r"(x));
+            for (int x = 0; x < F; ++x)
 #pragma unroll
-                    for (int k = 0; k < R; ++k)
-                        st_async(rb[x] + (uint32_t)((p0 + elem_off<T, RB, SB>(k)) * sizeof(cplx<T>)), v[x][k], rbar);
-                } else {
-#pragma unroll
-                    for (int k = 0; k < R; ++k) fld[x][p0 + elem_off<T, RB, SB>(k)] = v[x][k];
-                }
-            }
+                for (int k = 0; k < R; ++k) fld[x][p0 + elem_off<T, RB, SB>(k)] = v[x][k];
         }
     }
-    if constexpr (RL::flow) mbar_arrive_local(mb + 8 * (RL::FC::NCLS + cls), lane);   // my own field's share of done[cls]
+    if constexpr (RL::flow) mbar_arrive_cluster(mb + 8 * (RL::FC::NCLS + cls), lane, F);   // done[cls] in every CTA
 }
 
 // stand-alone pass 0 on the CTA's own field (the first and last linear operator of a call)
@@ -162,24 +153,6 @@ __device__ __noinline__ void pass0_local(const cplx<T>* tw, int tid, bool invers
     cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);
     if (inverse) inv_pass_smem<T, L, 0, NT, false>(sm, tw, tid);
     else fwd_pass_smem<T, L, 0, NT, false>(sm, tw, tid);
-}
-
-// the previous fused phase has released all of my field (every warp waits for its pass-1 classes)
-template <class T, int L, int NT>
-__device__ __forceinline__ void flow_wait_done_all(uint32_t mb, int tid, uint32_t parity) {
-    using FC = flow_cfg<T, L, NT>;
-    const int wg = (tid % FC::NTG) >> 5, lane = tid & 31;
-#pragma unroll 1
-    for (int it = 0; it < FC::NIT; ++it) {
-        const int c = wg + FC::NWG * it;
-        mbar_wait_done(mb + 8 * (FC::NCLS + c), mb + 16 * FC::NCLS + 4 * c, parity, tid < FC::NTG, lane);
-    }
-}
-// stands in for the arrivals of an inverse pass 1
-template <class T, int L, int NT>
-__device__ __forceinline__ void flow_arrive_ready_all(uint32_t mb, int tid, int nf) {
-    using FC = flow_cfg<T, L, NT>;
-    mbar_arrive_ready<(FC::NIT > 0 ? FC::NIT : 1), FC::NWG>(mb, (tid % FC::NTG) >> 5, tid & 31, nf);
 }
 
 template <class T, int L, int F>
@@ -221,23 +194,24 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
     if constexpr (FLOW) {
         if (tid == 0) {
             for (int c = 0; c < FC::NCLS; ++c) {
-                int my_warps = 0, my_tiles = 0;       // warps / tiles of class c that this CTA integrates itself
-                for (int w = 0; w < FC::NW; ++w) my_warps += (x + F * w) % FC::NCLS == c;
-                for (int tile = c; tile < RL::NTILES; tile += FC::NCLS) my_tiles += tile % F == x;
                 mbar_init(mb + 8 * c, RL::ready_count);
-                mbar_init(mb + 8 * (FC::NCLS + c), my_warps + 1);
-                reinterpret_cast<uint32_t*>(smem_raw + RL::mbar_offset + 16 * FC::NCLS)[c] =
-                    (uint32_t)((RL::NTILES / FC::NCLS - my_tiles) * RL::tile_bytes);
+                mbar_init(mb + 8 * (FC::NCLS + c), RL::done_count);
             }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
         cluster.sync();     // every CTA's barriers exist before anybody arrives on them
     }
     uint32_t fz = 0;        // fused phases executed so far by this cluster (mbarrier phase parity)
-    uint32_t rb[F];         // shared::cluster addresses of every CTA's field
-#pragma unroll
-    for (int f = 0; f < F; ++f)
-        asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rb[f]) : "r"((uint32_t)__cvta_generic_to_shared(sm)), "r"(f));
+    // this warp's classes in pass 1 (as in group_fwd / group_inv)
+    const int wg = (tid % FC::NTG) >> 5, lane = tid & 31;
+    auto flow_wait_done_all = [&](uint32_t parity) {      // the previous fused phase has released all of my field
+        if constexpr (FLOW)
+            for (int it = 0; it < FC::NIT; ++it) mbar_wait(mb + 8 * (FC::NCLS + wg + FC::NWG * it), parity);
+    };
+    auto flow_arrive_ready_all = [&]() {                   // stands in for the arrivals of an inverse pass 1
+        if constexpr (FLOW)
+            for (int it = 0; it < FC::NIT; ++it) mbar_arrive_cluster(mb + 8 * (wg + FC::NWG * it), lane, F);
+    };
     const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
     const cplx<T>* tabH2 = reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
     const bool resonant = a.resonant[x] != 0;
@@ -275,9 +249,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
             const bool crossing = rt_mode && q > 0 && q < total && s == 0;
             const bool keep = rt_mode && q == 0 && !resonant && a.steps > 1;   // SH <- first half-stepped input
             if (crossing && !resonant) {
-                if constexpr (FLOW) { flow_wait_done_all<T, L, NT>(mb, tid, (fz - 1) & 1); __syncthreads(); }
+                if constexpr (FLOW) { flow_wait_done_all((fz - 1) & 1); __syncthreads(); }
                 load(SH);                                        // fresh pump / frozen seed, already half-stepped
-                if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all<T, L, NT>(mb, tid, F); }
+                if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }
             } else {
                 const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
                 if constexpr (FLOW) {
@@ -293,15 +267,15 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
             if (keep) {   // keep it for the later round trips
                 __syncthreads();
                 store(SH);
-                if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all<T, L, NT>(mb, tid, F); }   // only now may the peers write into my field
+                if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }   // only now may the peers write into my field
             }
             if (q == total) break;
             if constexpr (!FLOW) cluster_arrive();   // my field is ready for its inverse pass 0
             const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
             if constexpr (!FLOW) cluster_wait();     // ... and so is every other field
-            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1, rb);
-            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1, rb);
-            else fused_pass0_rk4<T, L, F, NT, F - 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1, rb);
+            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
+            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
+            else fused_pass0_rk4<T, L, F, NT, F - 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
             ++fz;
             if constexpr (!FLOW) {
                 cluster_arrive();
