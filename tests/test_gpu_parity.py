@@ -11,6 +11,7 @@ import opo_workloads as W
 pytestmark = pytest.mark.gpu
 
 TOL = {"c128": 1e-10, "c64": 1e-4}
+_ORACLE_CACHE = {}      # oracle results shared by the engine parametrisations of one test
 
 
 def _gpu():
@@ -249,6 +250,73 @@ def test_config4_corners_c64(engine_idx):
     e1 = assert_close(cur, rcur, 1e-4, "C4 current")
     e2 = assert_close(ex, rex, 1e-4, "C4 exit")
     print(f"C4 5 RT engine {engine}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+def test_config4_full_batch_in_bench_launch_configuration():
+    """All 256 instances of C4 in ONE launch -- the configuration bench.py times (45 clusters looping over 5.7 waves of
+    instances) -- compared on sampled instances the oracle can compute one by one: first and last instance of the first
+    wave, first of the second wave, one in the middle, first and last of the ragged last wave."""
+    import os
+    import oracle
+    torch, P = _gpu()
+    w = W.config4().truncated(2)
+    o = P.from_workload(w, engine=P.ENGINE_AUTO)
+    assert o.engine == P.ENGINE_RESIDENT
+    o.roundtrips(w.n_roundtrips)
+    o.sync()
+    sample = [0, 44, 45, 137, 225, 255]
+    cur = np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy()[sample].astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    ex = np.stack([o.get_fields(x, P.WHICH_EXIT).cpu().numpy()[sample].astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    o.check_finite()
+    o.close()
+    ref = oracle.run_workload(w, instances=sample, threads=min(len(sample), os.cpu_count() or 1))
+    e1 = assert_close(cur, ref["current"], 1e-4, "C4 full batch current")
+    e2 = assert_close(ex, ref["exit"], 1e-4, "C4 full batch exit")
+    print(f"C4 full batch, 2 RT, sampled {sample}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+@pytest.mark.parametrize("engine_idx", [0, 1])
+def test_long_noise_seeded_run_power_and_spectrum(engine_idx):
+    """BASELINE.json:north_star, long noise-seeded runs: relative error <= 1e-3 on output signal power and on the power
+    spectrum (not phase; reading R21).  A three-wave singly resonant OPO as C1 but N = 2^12, nz = 50, pumped at 6.25x
+    threshold from a 1e-2 noise seed, 200 round trips: the signal grows by ~5 orders of magnitude in power and
+    saturates (pump depletion 85 %), so 10 000 z-steps of fp32 rounding pass through the gain before they are compared."""
+    engine = engines()[engine_idx]
+    base = W.config1()
+    k = base.kappa()
+    log2_n, nz, nrt = 12, 50, 200
+    w = W.Workload(
+        name="long_sro_2^12", length_m=base.length_m, d_eff_m_per_V=base.d_eff_m_per_V, n_fields=3,
+        lambda_m=list(base.lambda_m), n_index=list(base.n_index), beta1_s_per_m=list(base.beta1_s_per_m),
+        beta2_s2_per_m=list(base.beta2_s2_per_m), alpha_per_m=[0.0, 0.0, 0.0], ref_field=1, resonant=[0, 1, 0],
+        R=[0.0, 0.98, 0.0], delta_rad=[0.0, 0.0, 0.0], delta_T_s=[0.0, 0.0, 0.0], gdd_s2=[0.0, 0.0, 0.0],
+        log2_n=log2_n, window_s=base.window_s * (1 << log2_n) / base.n, nz_per_pass=nz, precision="c64", batch=1,
+        n_roundtrips=nrt, dk_per_m=np.zeros(1))
+    a_th = math.acosh(1.0 / math.sqrt(0.98)) / (math.sqrt(k[1] * k[2]) * w.length_m)     # reading R18 (SRO)
+    a_p = 2.5 * a_th                                                                     # 6.25x threshold in power
+    w.pump = W._round_to_precision(np.full((1, w.n), a_p, dtype=np.complex128), "c64")
+    w.seeds = [None] + [W._round_to_precision(W.complex_gaussian_noise(900 + x, w.n, 1e-2 * a_p)[None, :], "c64") for x in (1, 2)]
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine)
+    if "long" not in _ORACLE_CACHE:
+        _ORACLE_CACHE["long"] = run_oracle(w)
+    rcur, rex = _ORACLE_CACHE["long"]
+    # output signal power (reading R16): (1 - R_s) mean |exit_s|^2 of the last round trip
+    p_gpu = (1.0 - 0.98) * np.mean(np.abs(ex[0, 1]) ** 2)
+    p_ref = (1.0 - 0.98) * np.mean(np.abs(rex[0, 1]) ** 2)
+    assert 1.0 - np.mean(np.abs(rex[0, 0]) ** 2) / a_p ** 2 > 0.5, "the run must have reached saturation, else the test shows nothing"
+    err_p = abs(p_gpu - p_ref) / p_ref
+    s_gpu = np.abs(np.fft.fft(ex[0, 1])) ** 2
+    s_ref = np.abs(np.fft.fft(rex[0, 1])) ** 2
+    err_s = rel_l2(s_gpu, s_ref)
+    # pump depletion as a second scalar
+    d_gpu = 1.0 - np.mean(np.abs(ex[0, 0]) ** 2) / a_p ** 2
+    d_ref = 1.0 - np.mean(np.abs(rex[0, 0]) ** 2) / a_p ** 2
+    print(f"long run engine {engine}: signal power rel err {err_p:.3e}, power spectrum rel L2 {err_s:.3e}, "
+          f"pump depletion {d_gpu:.4f} vs {d_ref:.4f}, field rel L2 {rel_l2(ex[0, 1], rex[0, 1]):.3e}")
+    assert err_p <= 1e-3, err_p
+    assert err_s <= 1e-3, err_s
+    assert abs(d_gpu - d_ref) <= 1e-3
 
 
 # ---------------------------------------------------------------------------------------------------------
