@@ -42,10 +42,10 @@ def flops_per_grid_point_zstep(log2_n: int, n_fields: int) -> float:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu captures
-# of exactly this launch configuration (profiles/r01e_*.md); None where no capture of that configuration exists.
+# of exactly this launch configuration (profiles/r01f_*.md); None where no capture of that configuration exists.
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, engine, round trips per step): bytes
-    ("C4", "resident", 300): 185325824 + 242958080,     # profiles/r01e_dram_c4_default.csv (one 3.16 s launch)
+    ("C4", "resident", 300): 187344896 + 243991040,     # profiles/r01f_dram_c4_default.csv (one 3.1 s launch)
 }
 
 
