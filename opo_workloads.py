@@ -67,6 +67,9 @@ class Workload:
     pump: np.ndarray = None          # [batch or 1][N]
     seeds: List[Optional[np.ndarray]] = None   # per field: None (pump) or [batch][N]
     notes: str = ""
+    # intracavity phase modulator per field: depth [rad] (0 = none) and frequency [Hz]
+    eom_beta_rad: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
+    eom_f_hz: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
 
     @property
     def n(self) -> int:

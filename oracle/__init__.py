@@ -44,6 +44,7 @@ def lib():
                                         ctypes.c_int]
         L.opo_oracle_destroy.argtypes = [ctypes.c_void_p]
         L.opo_oracle_set_field.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, _DP]
+        L.opo_oracle_set_eom.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double]
         L.opo_oracle_propagate.argtypes = [ctypes.c_void_p, ctypes.c_int]
         L.opo_oracle_propagate.restype = ctypes.c_int
         L.opo_oracle_roundtrips.argtypes = [ctypes.c_void_p, ctypes.c_int]
@@ -119,6 +120,10 @@ class OracleOpo:
         code = {"state": 0, "input": 1, "both": 2}[which]
         lib().opo_oracle_set_field(self._h, field, code, d.view(np.float64).ctypes.data_as(_DP))
 
+    def set_eom(self, field: int, beta_rad: float, f_hz: float):
+        """Intracavity phase modulator on a resonant field; beta = 0 switches it off."""
+        lib().opo_oracle_set_eom(self._h, int(field), float(beta_rad), float(f_hz))
+
     def propagate(self, nz: int) -> int:
         return lib().opo_oracle_propagate(self._h, int(nz))
 
@@ -150,6 +155,9 @@ def from_workload(w, b: int = 0, use_float: bool = False) -> OracleOpo:
     o.set_field(0, w.pump_of(b))
     for x in range(1, w.n_fields):
         o.set_field(x, w.seeds[x][b])
+    for x in range(w.n_fields):
+        if w.eom_beta_rad[x] != 0.0:
+            o.set_eom(x, w.eom_beta_rad[x], w.eom_f_hz[x])
     return o
 
 

@@ -22,12 +22,15 @@
 //   boundary (Eq. 6, Listing 3; R11-R15):
 //        exit_x <- A_x
 //        resonant x:     A_x <- sqrt(R_x) e^{i delta_x} IDFT( G_x .* DFT(A_x) )
+//                        A_x[n] <- A_x[n] exp(i beta_x sin(2 pi f_x tau_n))   intracavity EOM, last element
+//                                  (Listing 3; off when beta_x = 0)
 //        non-resonant x: A_x <- S_x   (stored input: fresh pump / frozen seed)
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): P1 naive DFT, P2 Gaussian GVD closed form, P3 GVM
 // integer shift, P4 cosh^2 gain (+dk), P5 degenerate phase-sensitive gain (paper's pi/4, -3pi/4,
 // PAPER.md:L400), P6 Manley-Rowe, P7 depleted SHG closed form, P8 2nd-order convergence, P9 cold
-// cavity, P10 threshold growth.  Parity unpinned: reading R12 (non-resonant fields restart from
+// cavity, P10 threshold growth, P13 EOM sidebands = Bessel J_m(beta) (Jacobi-Anger) and element order.
+// Parity unpinned: reading R12 (non-resonant fields restart from
 // S_x) is a convention with no physical pin; the paper's P_th values (L348) and Figs 3-5.
 // =================================================================================================
 #include <cmath>
@@ -101,6 +104,7 @@ struct Params {
     double lambda_m[3], n_index[3], beta1[3], beta2[3], alpha[3];
     int resonant[3];
     double R[3], delta_rad[3], delta_T[3], gdd[3];
+    double eom_beta[3], eom_f[3];   // intracavity phase modulator: depth [rad], frequency [Hz]
 };
 
 template <class R>
@@ -230,6 +234,16 @@ struct Oracle {
                 double r = std::sqrt(p.R[x]);
                 C m((R)(r * std::cos(p.delta_rad[x])), (R)(r * std::sin(p.delta_rad[x])));
                 for (int n = 0; n < N; ++n) A[x][n] = A[x][n] * m;
+                // intracavity EOM, last element of the boundary (Listing 3, after AddGDD and AddPhase):
+                // A(tau) -> A(tau) exp(i beta sin(2 pi f_pm tau))          PAPER.md:L149-154; tau_n = (n - N/2) dt (R19)
+                if (p.eom_beta[x] != 0.0) {
+                    double dt = p.window_s / (double)N;
+                    for (int n = 0; n < N; ++n) {
+                        double tau = (double)(n - N / 2) * dt;
+                        double ph = p.eom_beta[x] * std::sin(2.0 * kPi * p.eom_f[x] * tau);
+                        A[x][n] = A[x][n] * C((R)std::cos(ph), (R)std::sin(ph));
+                    }
+                }
             } else {
                 A[x] = S[x];
             }
@@ -308,6 +322,13 @@ void opo_oracle_set_field(void* h, int field, int which, const double* reim) {
         if (which != 1) set_vec(hnd->d->A[field], reim);
         if (which != 0) set_vec(hnd->d->S[field], reim);
     }
+}
+
+// intracavity phase modulator on (resonant) field x; beta = 0 switches it off
+void opo_oracle_set_eom(void* h, int field, double beta_rad, double f_hz) {
+    Handle* hnd = (Handle*)h;
+    if (hnd->is_float) { hnd->f->p.eom_beta[field] = beta_rad; hnd->f->p.eom_f[field] = f_hz; }
+    else               { hnd->d->p.eom_beta[field] = beta_rad; hnd->d->p.eom_f[field] = f_hz; }
 }
 
 int opo_oracle_propagate(void* h, int nz) {

@@ -485,3 +485,68 @@ def test_nan_when_dz_too_coarse():
     o.set_field(1, np.full(16, 1.0 + 1j, complex))
     o.propagate(60)
     assert not np.all(np.isfinite(o.get_field(1)))
+
+
+# ---------------------------------------------------------------------------------------------
+# P13  intracavity EOM (Listing 3)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("beta,q", [(0.8, 1), (2.4048, 3), (-1.3, 2)])
+def test_p13_eom_sidebands_are_bessel_functions(beta, q):
+    """A CW field through a cold cavity with only the modulator: exp(i beta sin(theta)) = sum_m J_m(beta)
+    e^{i m theta} (Jacobi-Anger).  With f_pm = q / T_win, theta_n = 2 pi q (n - N/2) / N, so bin m q of the
+    unnormalised forward DFT holds N J_m(beta) (-1)^{m q} and every other bin is empty.  Pins the form of the
+    modulator, the sign of beta, the time origin (R19) and the 2 pi in the argument."""
+    from scipy.special import jv
+    log2n, T = 8, 10 * PS
+    n = 1 << log2n
+    o = make(n_fields=3, log2_n=log2n, window_s=T, nz=4, length=5e-3, resonant=(0, 1, 0), R=(0, 1.0, 0))
+    o.set_eom(1, beta, q / T)
+    o.set_field(0, np.zeros(n, complex))
+    o.set_field(1, np.ones(n, complex))
+    o.set_field(2, np.zeros(n, complex))
+    assert o.roundtrips(1) == 0
+    spec = o.get_field(1, CURRENT, FREQ)
+    expect = np.zeros(n, complex)
+    for m in range(-40, 41):
+        expect[(m * q) % n] += n * jv(m, beta) * (-1.0) ** (m * q)
+    assert np.abs(spec - expect).max() < 1e-10 * n
+    # beta = 2.4048 is the first zero of J_0: the carrier is (almost) extinguished
+    if abs(beta - 2.4048) < 1e-9:
+        assert abs(spec[0]) < 1e-4 * n
+    # a pure phase modulation leaves |A| untouched
+    assert np.abs(np.abs(o.get_field(1)) - 1.0).max() < 1e-13
+
+
+def test_p13_eom_acts_after_gdd_and_mirror_on_resonant_fields_only():
+    """Order of the boundary elements (Listing 3; R15): spectral phase, mirror, then the modulator, which
+    does not commute with the spectral phase.  Checked against the same chain written with the library FFT; the
+    swapped order must differ.  A non-resonant field ignores its modulator (it restarts from S_x)."""
+    log2n, T = 8, 10 * PS
+    n = 1 << log2n
+    dt = T / n
+    R, delta, gdd, dT, beta, f = 0.81, 0.2, -4000 * FS * FS, 25 * FS, 1.1, 3 / T
+    o = make(n_fields=3, log2_n=log2n, window_s=T, nz=4, length=5e-3, resonant=(0, 1, 0), R=(0, R, 0),
+             delta_rad=(0, delta, 0), delta_T=(0, dT, 0), gdd=(0, gdd, 0))
+    o.set_eom(1, beta, f)
+    o.set_eom(2, 0.7, f)            # idler is not resonant: no effect
+    rng = np.random.default_rng(5)
+    a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    s2 = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    o.set_field(0, np.zeros(n, complex))
+    o.set_field(1, a)
+    o.set_field(2, s2)
+    assert o.roundtrips(1) == 0
+    om = 2 * np.pi * np.fft.fftfreq(n, d=1.0 / n) / (n * dt)
+    G = np.exp(1j * (gdd / 2) * om ** 2 - 1j * om * dT)
+    tau = (np.arange(n) - n // 2) * dt
+    E = np.exp(1j * beta * np.sin(2 * np.pi * f * tau))
+    m = math.sqrt(R) * np.exp(1j * delta)
+    right = m * np.fft.ifft(G * np.fft.fft(a)) * E
+    wrong = m * np.fft.ifft(G * np.fft.fft(a * E))
+    got = o.get_field(1)
+    assert rel_l2(got, right) < 1e-12
+    assert rel_l2(got, wrong) > 1e-2
+    assert rel_l2(o.get_field(2), s2) < 1e-15      # pump = 0, so the idler seed passes unchanged and is re-injected
+    # the exit field is taken before the boundary: no modulator on it
+    assert rel_l2(o.get_field(1, EXIT), a) < 1e-12
