@@ -116,6 +116,16 @@ int opo_set_stream(opo_handle* h, void* cuda_stream);
 #define OPO_PARAM_GDD 3
 int opo_set_batch_param(opo_handle* h, int param, int field, const double* host_vals, int count);
 
+/* Intracavity electro-optic phase modulator on a resonant field, the last element of the cavity boundary
+ * ("A(tau) -> A(tau) exp(i beta sin(2 pi f_pm tau))"; Listing 3
+ * PhaseModulatorIntraCavity, after AddGDD and AddPhase): every round trip, after the spectral phase and the
+ * mirror factor, A_x[n] *= exp(i beta sin(2 pi f_pm tau_n)), tau_n = (n - N/2) dt.  beta_rad = 0 removes it.
+ * Same modulator for every instance.  OPO_ERR_INVALID_ARG for a non-resonant field (it restarts from its
+ * stored input every round trip, so a modulator on it would never act).  The table is built in fp64 on the
+ * host.  With a modulator present the boundary is no longer merged into the neighbouring half-steps: the
+ * resident and large-N engines then run one launch per round trip. */
+int opo_set_eom(opo_handle* h, int field, double beta_rad, double f_mod_hz);
+
 /* Pump input S_p (PAPER.md:L268 ReadPump): time-domain complex [N] (per_instance = 0, broadcast to
  * all instances) or [batch][N].  Copied into the handle; re-injected at every round-trip boundary;
  * also becomes the current pump field when z = 0. */

@@ -69,6 +69,7 @@ def lib() -> ctypes.CDLL:
         L.opo_destroy.argtypes = [vp]
         L.opo_set_stream.argtypes = [vp, vp]
         L.opo_set_batch_param.argtypes = [vp, ci, ci, ctypes.POINTER(ctypes.c_double), ci]
+        L.opo_set_eom.argtypes = [vp, ci, ctypes.c_double, ctypes.c_double]
         L.opo_set_pump.argtypes = [vp, vp, ci]
         L.opo_set_pump_host.argtypes = [vp, vp, ci]
         L.opo_set_field.argtypes = [vp, ci, vp]
@@ -91,7 +92,7 @@ def lib() -> ctypes.CDLL:
     return _lib
 
 
-EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_pump",
+EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_eom", "opo_set_pump",
            "opo_set_pump_host", "opo_set_field", "opo_set_field_host", "opo_propagate", "opo_roundtrips",
            "opo_get_fields", "opo_get_fields_host", "opo_sync", "opo_check_finite", "opo_get_z_steps",
            "opo_set_option", "opo_get_info", "opo_last_error"]
@@ -137,6 +138,10 @@ def opo_set_stream(h, cuda_stream: int):
 def opo_set_batch_param(h, param: int, field: int, values):
     v = np.ascontiguousarray(values, dtype=np.float64)
     _check(h, lib().opo_set_batch_param(h, param, field, v.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), v.size))
+
+
+def opo_set_eom(h, field: int, beta_rad: float, f_mod_hz: float):
+    _check(h, lib().opo_set_eom(h, int(field), float(beta_rad), float(f_mod_hz)))
 
 
 def opo_set_pump(h, dev_ptr: int, per_instance: bool):
@@ -246,6 +251,9 @@ class Opo:
     def set_batch_param(self, param, field, values):
         opo_set_batch_param(self._h, param, field, values)
 
+    def set_eom(self, field, beta_rad, f_mod_hz):
+        opo_set_eom(self._h, field, beta_rad, f_mod_hz)
+
     def set_pump(self, pump):
         per = pump.dim() == 2 and pump.shape[0] == self.batch and self.batch > 1
         shape = (self.batch, self.n) if per else tuple(pump.shape)
@@ -312,6 +320,9 @@ def from_workload(w, engine=ENGINE_AUTO, host_inputs=False) -> Opo:
         o.set_batch_param(PARAM_DK, 0, w.dk_per_m)
     if w.delta_T_signal_s is not None:
         o.set_batch_param(PARAM_DELTA_T, 1, w.delta_T_signal_s)
+    for x in range(w.n_fields):
+        if w.eom_beta_rad[x] != 0.0:
+            o.set_eom(x, w.eom_beta_rad[x], w.eom_f_hz[x])
     load_inputs(o, w, host_inputs)
     return o
 

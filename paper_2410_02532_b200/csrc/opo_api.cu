@@ -113,6 +113,8 @@ struct opo_handle {
     void* tabHB[3] = {nullptr, nullptr, nullptr};
     size_t tabB_count[3] = {0, 0, 0};      // instances allocated for GM / HB (1 or B)
     void* mirror[3] = {nullptr, nullptr, nullptr};
+    void* eom[3] = {nullptr, nullptr, nullptr};       // [N] exp(i beta sin(2 pi f tau_n)) or null
+    double eom_beta[3] = {0, 0, 0}, eom_f[3] = {0, 0, 0};
     bool boundary_fft[3] = {false, false, false};
     void* phase = nullptr;
     int* flag = nullptr;
@@ -374,7 +376,7 @@ int ensure_tables(opo_handle* h) {
 
 void free_all(opo_handle* h) {
     for (int x = 0; x < 3; ++x) {
-        void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->mirror[x]};
+        void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->mirror[x], h->eom[x]};
         for (void* p : ptrs) if (p) cudaFree(p);
     }
     void* more[] = {h->scratch, h->tw, h->perm, h->phase, h->flag, h->tw2, h->wlo, h->whi, h->perm2, h->scratch2, h->barrier};
@@ -592,6 +594,20 @@ int stream_boundary(opo_handle* h) {
     return OPO_OK;
 }
 
+// intracavity phase modulator after the boundary (Listing 3), streaming / large engines
+bool any_eom(const opo_handle* h) {
+    for (int x = 0; x < h->F; ++x) if (h->eom[x]) return true;
+    return false;
+}
+int apply_eom(opo_handle* h) {
+    for (int x = 0; x < h->F; ++x) {
+        if (!h->eom[x]) continue;
+        opo::MulTabArgs m{h->cur[x], h->eom[x], h->B, h->N};
+        OPO_LAUNCH(h, h->dbl ? opo::launch_multab_f64(m, h->stream) : opo::launch_multab_f32(m, h->stream));
+    }
+    return OPO_OK;
+}
+
 // ---- resident engine ---------------------------------------------------------------------------------------------
 int resident_run(opo_handle* h, int mode, int z0, int steps) {
     opo::ResidentArgs a{};
@@ -600,6 +616,7 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
         a.tabH[x] = h->tabH[x]; a.tabH2[x] = h->tabH2[x]; a.tabHB[x] = h->tabHB[x]; a.tabGM[x] = h->tabGM[x];
         a.tab_stride[x] = h->per_inst_boundary[x] ? h->N : 0;
         a.mirror[x] = h->mirror[x];
+        a.eom[x] = h->eom[x];
         a.boundary_fft[x] = h->boundary_fft[x] ? 1 : 0;
         a.resonant[x] = h->fields.resonant[x] ? 1 : 0;
         a.kappa[x] = h->kappa[x];
@@ -764,13 +781,52 @@ int opo_roundtrips(opo_handle* h, int n) {
     if (n == 0) return OPO_OK;
     if (int rc = check_async(h)) return rc;
     if (int rc = ensure_tables(h)) return rc;
-    if (h->large) return large_run(h, 1, 0, n);
-    if (engine_in_use(h) == OPO_ENGINE_RESIDENT) return resident_run(h, 1, 0, n);
+    // a phase modulator acts in the time domain between the boundary's spectral phase and the next pass, so the
+    // boundary cannot be merged into the neighbouring half-steps: one launch per round trip then
+    const bool eom = any_eom(h);
+    if (h->large) {
+        if (!eom) return large_run(h, 1, 0, n);
+        for (int m = 0; m < n; ++m) {
+            if (int rc = large_run(h, 1, 0, 1)) return rc;
+            if (int rc = apply_eom(h)) return rc;
+        }
+        return OPO_OK;
+    }
+    if (engine_in_use(h) == OPO_ENGINE_RESIDENT) {
+        if (!eom) return resident_run(h, 1, 0, n);
+        for (int m = 0; m < n; ++m)
+            if (int rc = resident_run(h, 1, 0, 1)) return rc;      // the kernel applies the modulator with its last store
+        return OPO_OK;
+    }
     for (int m = 0; m < n; ++m) {
         if (int rc = stream_steps(h, 0, h->nz, true)) return rc;
         if (int rc = stream_boundary(h)) return rc;
+        if (eom) if (int rc = apply_eom(h)) return rc;
     }
     return OPO_OK;
+}
+
+int opo_set_eom(opo_handle* h, int field, double beta_rad, double f_mod_hz) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    if (field < 0 || field >= h->F) return fail(h, OPO_ERR_INVALID_ARG, "field out of range");
+    if (!h->fields.resonant[field]) return fail(h, OPO_ERR_INVALID_ARG, "a phase modulator acts on resonant fields only");
+    if (!std::isfinite(beta_rad) || !std::isfinite(f_mod_hz)) return fail(h, OPO_ERR_INVALID_ARG, "non-finite modulator parameter");
+    if (int rc = check_async(h)) return rc;
+    h->eom_beta[field] = beta_rad; h->eom_f[field] = f_mod_hz;
+    if (beta_rad == 0.0) {
+        if (h->eom[field]) { OPO_CUDA(h, cudaStreamSynchronize(h->stream)); cudaFree(h->eom[field]); h->eom[field] = nullptr; }
+        return OPO_OK;
+    }
+    if (!h->eom[field] && cudaMalloc(&h->eom[field], (size_t)h->N * h->esz) != cudaSuccess)
+        return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the modulator table failed");
+    std::vector<cd> E(h->N);
+    const double dt = h->grid.window_s / (double)h->N;
+    for (int n = 0; n < h->N; ++n) {
+        const double tau = (double)(n - h->N / 2) * dt;                       // reading R19
+        const double ph = beta_rad * std::sin(2.0 * kPi * f_mod_hz * tau);
+        E[n] = cd(std::cos(ph), std::sin(ph));
+    }
+    return upload_complex(h, h->eom[field], E.data(), (size_t)h->N, true);
 }
 
 int opo_sync(opo_handle* h) {

@@ -37,6 +37,13 @@ struct Rk4Args {
     int step;              // z-step index s: stage phases at 2s, 2s+1, 2s+2
 };
 
+// A[b][n] *= E[n]  (intracavity phase modulator exp(i beta sin(2 pi f tau_n)))
+struct MulTabArgs {
+    void* A;
+    const void* E;         // [N] complex
+    int batch, n;
+};
+
 // A[b][n] *= m[b]  (mirror sqrt(R) e^{i delta}, Eq. 6)
 struct ScaleArgs {
     void* A;
@@ -66,6 +73,8 @@ struct ResidentArgs {
     const void* tabGM[3];  // G m / N, un-merged boundary       (resonant; maybe per instance)
     long long tab_stride[3];   // instance stride of HB / GM (0 = shared)
     const void* mirror[3]; // [B] complex sqrt(R) e^{i delta} (used when the boundary has no G)
+    const void* eom[3];    // [N] complex exp(i beta sin(2 pi f tau_n)) applied after the boundary of the call's last
+                           // round trip, or null
     int boundary_fft[3];   // resonant field needs the transform pair at the boundary
     int resonant[3];
     const void* tw;
@@ -130,6 +139,7 @@ struct LargeInfo {
     cudaError_t launch_linear_##SUFFIX(int log2n, const LinArgs& a, cudaStream_t s);    \
     cudaError_t launch_rk4_##SUFFIX(const Rk4Args& a, cudaStream_t s);                  \
     cudaError_t launch_scale_##SUFFIX(const ScaleArgs& a, cudaStream_t s);              \
+    cudaError_t launch_multab_##SUFFIX(const MulTabArgs& a, cudaStream_t s);            \
     cudaError_t launch_freq_##SUFFIX(int log2n, const FreqArgs& a, cudaStream_t s);     \
     cudaError_t launch_finite_##SUFFIX(const void* A, long long count, int* flag, cudaStream_t s); \
     cudaError_t resident_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);     \

@@ -120,6 +120,16 @@ __global__ void __launch_bounds__(256) k_scale(ScaleArgs a) {
     }
 }
 
+// intracavity phase modulator: A[b][n] *= E[n]
+template <class T>
+__global__ void __launch_bounds__(256) k_multab(MulTabArgs a) {
+    const long long total = (long long)a.batch * a.n;
+    cplx<T>* A = reinterpret_cast<cplx<T>*>(a.A);
+    const cplx<T>* E = reinterpret_cast<const cplx<T>*>(a.E);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
+        A[i] = cmul(A[i], ldg(&E[(int)(i % a.n)]));
+}
+
 template <class T, int L>
 __global__ void __launch_bounds__(cta_threads<T, L>::value) k_freq(FreqArgs a) {
     constexpr int N = 1 << L, NT = cta_threads<T, L>::value;
@@ -185,6 +195,10 @@ template <class T> cudaError_t launch_rk4_T(const Rk4Args& a, cudaStream_t s) {
 }
 template <class T> cudaError_t launch_scale_T(const ScaleArgs& a, cudaStream_t s) {
     k_scale<T><<<grid_for((long long)a.batch * a.n, 256), 256, 0, s>>>(a);
+    return cudaGetLastError();
+}
+template <class T> cudaError_t launch_multab_T(const MulTabArgs& a, cudaStream_t s) {
+    k_multab<T><<<grid_for((long long)a.batch * a.n, 256), 256, 0, s>>>(a);
     return cudaGetLastError();
 }
 template <class T> cudaError_t launch_finite_T(const void* A, long long count, int* flag, cudaStream_t s) {

@@ -1,5 +1,5 @@
 // opo_pointwise.cu -- the size-independent kernels of the streaming engine (RK4, mirror scale,
-// finite check) for both precisions.
+// phase-modulator table, finite check) for both precisions.
 #include "opo_kernels.cuh"
 
 namespace opo {
@@ -8,6 +8,8 @@ cudaError_t launch_rk4_f32(const Rk4Args& a, cudaStream_t s) { return launch_rk4
 cudaError_t launch_rk4_f64(const Rk4Args& a, cudaStream_t s) { return launch_rk4_T<double>(a, s); }
 cudaError_t launch_scale_f32(const ScaleArgs& a, cudaStream_t s) { return launch_scale_T<float>(a, s); }
 cudaError_t launch_scale_f64(const ScaleArgs& a, cudaStream_t s) { return launch_scale_T<double>(a, s); }
+cudaError_t launch_multab_f32(const MulTabArgs& a, cudaStream_t s) { return launch_multab_T<float>(a, s); }
+cudaError_t launch_multab_f64(const MulTabArgs& a, cudaStream_t s) { return launch_multab_T<double>(a, s); }
 cudaError_t launch_finite_f32(const void* A, long long count, int* flag, cudaStream_t s) { return launch_finite_T<float>(A, count, flag, s); }
 cudaError_t launch_finite_f64(const void* A, long long count, int* flag, cudaStream_t s) { return launch_finite_T<double>(A, count, flag, s); }
 

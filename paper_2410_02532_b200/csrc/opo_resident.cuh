@@ -291,6 +291,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
         } else {
             store(reinterpret_cast<cplx<T>*>(a.exitb[x]) + (size_t)b * N);     // fields at z = L of the last pass
             if (resonant) {
+                // intracavity phase modulator, last element of the boundary (Listing 3)
+                const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]);
+                cplx<T> mf = {(T)1, (T)0};
                 if (a.boundary_fft[x]) {
                     const cplx<T>* tabGM = reinterpret_cast<const cplx<T>*>(a.tabGM[x]) + (size_t)b * a.tab_stride[x];
                     __syncthreads();
@@ -300,9 +303,13 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
                     __syncthreads();
                     pass0_local<T, L, NT>(tw, tid, true);
                     __syncthreads();
-                    store(cur);
                 } else {
-                    const cplx<T> mf = ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b);
+                    mf = ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b);
+                }
+                if (E != nullptr) {
+#pragma unroll 4
+                    for (int i = tid; i < N; i += NT) cur[i] = cmul(cmul(sm[phys<T>(i)], mf), ldg(&E[i]));
+                } else {
 #pragma unroll 4
                     for (int i = tid; i < N; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
                 }

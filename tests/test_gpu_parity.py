@@ -394,6 +394,81 @@ def test_config3_one_roundtrip_c64():
 # ---------------------------------------------------------------------------------------------------------
 # boundary behaviour of the ABI itself
 # ---------------------------------------------------------------------------------------------------------
+# ---------------------------------------------------------------------------------------------------------
+# intracavity phase modulator (Listing 3)
+# ---------------------------------------------------------------------------------------------------------
+def _with_eom(w):
+    """Modulator on every resonant field: depth ~1 rad, frequency = a few free spectral ranges of the time window
+    (the paper: 'on the order of the cavity free-spectral range'), not an integer multiple so nothing is periodic."""
+    w.eom_beta_rad = [0.0, 0.0, 0.0]
+    w.eom_f_hz = [0.0, 0.0, 0.0]
+    for x in range(w.n_fields):
+        if w.resonant[x]:
+            w.eom_beta_rad[x] = 0.9 + 0.4 * x
+            w.eom_f_hz[x] = (2.3 + x) / w.window_s
+    return w
+
+
+@pytest.mark.parametrize("engine_idx", [0, 1])
+@pytest.mark.parametrize("precision,log2_n,n_fields,gdd", [("c128", 10, 2, 0.0), ("c64", 12, 3, 0.0), ("c64", 9, 3, 0.7),
+                                                           ("c64", 14, 3, 0.7), ("c128", 8, 3, 0.7)])
+def test_eom_roundtrips_match_oracle(precision, log2_n, n_fields, gdd, engine_idx):
+    """Round trips with the modulator as last boundary element, with and without the spectral-phase transform in the
+    boundary, across a call boundary (3 = 2 + 1 round trips), both engines."""
+    engine = engines()[engine_idx]
+    w = _with_eom(small_workload(log2_n, n_fields, precision, nz=5, batch=2, dk=11.0, gdd_dt2=gdd, drad=0.3))
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine, n_roundtrips=3, calls=2)
+    rcur, rex = run_oracle(w, n_roundtrips=3)
+    e1 = assert_close(cur, rcur, TOL[precision], "EOM current")
+    e2 = assert_close(ex, rex, TOL[precision], "EOM exit")
+    # the modulator must have done something: without it the result differs at O(1)
+    w0 = small_workload(log2_n, n_fields, precision, nz=5, batch=2, dk=11.0, gdd_dt2=gdd, drad=0.3)
+    c0, _ = run_oracle(w0, n_roundtrips=3)
+    assert rel_l2(c0[0, 1], rcur[0, 1]) > 0.1
+    print(f"EOM {precision} 2^{log2_n} F={n_fields} engine {engine}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+def test_eom_large_engine_matches_oracle():
+    w = _with_eom(small_workload(15, 2, "c64", nz=4, batch=1, dk=5.0, gdd_dt2=0.7, drad=0.3))
+    torch, P = _gpu()
+    cur, ex, eng = run_gpu(w, P.ENGINE_AUTO, n_roundtrips=2)
+    assert eng == P.ENGINE_LARGE
+    rcur, rex = run_oracle(w, n_roundtrips=2)
+    e1 = assert_close(cur, rcur, 1e-4, "EOM large current")
+    e2 = assert_close(ex, rex, 1e-4, "EOM large exit")
+    print(f"EOM large engine 2^15: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+def test_eom_config1_20_roundtrips_and_abi_errors():
+    """C1 (N = 2^14, 100 z-steps) with a modulator on the signal at ~3 free spectral ranges, 20 round trips; the call
+    rejects non-resonant fields and beta = 0 removes the modulator again."""
+    torch, P = _gpu()
+    w = W.config1().truncated(20)
+    w.eom_beta_rad = [0.0, 1.2, 0.0]
+    w.eom_f_hz = [0.0, 3.0 / w.window_s, 0.0]
+    cur, ex, eng = run_gpu(w, P.ENGINE_AUTO)
+    assert eng == P.ENGINE_RESIDENT
+    rcur, rex = run_oracle(w)
+    e1 = assert_close(cur, rcur, 1e-4, "C1+EOM current")
+    e2 = assert_close(ex, rex, 1e-4, "C1+EOM exit")
+    print(f"C1 + EOM, 20 RT: rel L2 current {e1:.3e} exit {e2:.3e}")
+    o = P.from_workload(w)
+    with pytest.raises(P.OpoError) as ei:
+        o.set_eom(0, 1.0, 1e11)                # the pump is not resonant
+    assert ei.value.status == P.ERR_INVALID_ARG
+    with pytest.raises(P.OpoError):
+        o.set_eom(5, 1.0, 1e11)
+    o.set_eom(1, 0.0, 0.0)                      # removed again: plain C1
+    o.roundtrips(2)
+    o.sync()
+    got = o.get_fields(1, P.WHICH_CURRENT).cpu().numpy().astype(np.complex128)
+    o.close()
+    w2 = W.config1().truncated(2)
+    rc2, _ = run_oracle(w2)
+    assert rel_l2(got[0], rc2[0, 1]) <= 1e-4
+
+
 def test_abi_errors_and_state():
     torch, P = _gpu()
     w = small_workload(8, 2, "c64", nz=4)
