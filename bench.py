@@ -178,6 +178,9 @@ def main():
     ap.add_argument("--workload", default="C4", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--rt-per-step", type=int, default=0, help="round trips per step (default: the config's full length for C4 and C0, 100 for C1, 20 for C2, 2 for C3)")
     ap.add_argument("--engine", default="auto", choices=["auto", "resident", "streaming"])
+    ap.add_argument("--eom", action="store_true",
+                    help="intracavity phase modulator on the signal (PAPER.md:L149-154; beta = 1 rad, f = 3 / window): the "
+                         "paper's 'EOM' cavity configuration; the boundary is then not merged (one launch per round trip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -207,6 +210,9 @@ def main():
         torch.cuda.synchronize()
 
     w = make_workload(args.workload, rank)
+    if args.eom:
+        w.eom_beta_rad = [0.0, 1.0, 0.0]
+        w.eom_f_hz = [0.0, 3.0 / w.window_s, 0.0]
     rt_per_step = args.rt_per_step or {"C0": w.n_roundtrips, "C1": 100, "C2": 20, "C3": 2, "C4": w.n_roundtrips}[args.workload]
     engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "streaming": P.ENGINE_STREAMING}[args.engine]
     o = P.from_workload(w, engine=engine)
@@ -314,7 +320,7 @@ def main():
             "ms_per_step": t_total / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if w.precision == "c64" else "f64", "data": "synthetic",
             "config": {"workload": f"{w.name}: BASELINE.json configs[{args.workload[1]}], batch {w.batch} x N=2^{w.log2_n} x "
-                                   f"{w.n_fields} fields, nz={w.nz_per_pass}, {rt_per_step} round trips per step",
+                                   f"{w.n_fields} fields, nz={w.nz_per_pass}, {rt_per_step} round trips per step" + (", EOM on the signal" if args.eom else ""),
                        "engine": eng_name,
                        "l2": "512 MiB flush write between timed steps", "sharding": "independent instances per rank, no collective"},
             "round_trips_per_s": world * w.batch * rt_per_step * args.steps / t_total,

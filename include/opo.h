@@ -145,6 +145,16 @@ int opo_propagate(opo_handle* h, int nz);
  * pass (before the mirror). */
 int opo_roundtrips(opo_handle* h, int n);
 
+/* Nanosecond regime (PAPER.md:L228 NS_OPO, L302, L322-335): the pump pulse is much longer than a round trip, so
+ * it is a long vector of n consecutive windows; round trip m is pumped by slice m (ReadPump, L268) and the field
+ * that leaves the crystal in round trip m is appended to a long output vector (SaveRoundTrip, L272).
+ *   dev_pump_train: [n][N] (per_instance = 0, every instance sees the same train) or [n][batch][N], time domain;
+ *   dev_out_train : NULL, or [n][batch][N]: exit field `out_field` (z = L, before the mirror) of every round trip.
+ * Equivalent to n x { opo_set_pump(slice m); opo_roundtrips(1); copy of OPO_WHICH_EXIT } with everything staying
+ * on the device and on the handle's stream.  Afterwards the stored pump input is the last slice.
+ * OPO_ERR_UNSUPPORTED for a resonant pump, OPO_ERR_STATE unless z = 0. */
+int opo_roundtrips_train(opo_handle* h, int n, const void* dev_pump_train, int per_instance, void* dev_out_train, int out_field);
+
 #define OPO_WHICH_CURRENT 0
 #define OPO_WHICH_EXIT 1
 #define OPO_DOMAIN_TIME 0

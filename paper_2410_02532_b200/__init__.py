@@ -76,6 +76,7 @@ def lib() -> ctypes.CDLL:
         L.opo_set_field_host.argtypes = [vp, ci, vp]
         L.opo_propagate.argtypes = [vp, ci]
         L.opo_roundtrips.argtypes = [vp, ci]
+        L.opo_roundtrips_train.argtypes = [vp, ci, vp, ci, vp, ci]
         L.opo_get_fields.argtypes = [vp, ci, ci, ci, vp]
         L.opo_get_fields_host.argtypes = [vp, ci, ci, ci, vp]
         L.opo_sync.argtypes = [vp]
@@ -93,7 +94,7 @@ def lib() -> ctypes.CDLL:
 
 
 EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_eom", "opo_set_pump",
-           "opo_set_pump_host", "opo_set_field", "opo_set_field_host", "opo_propagate", "opo_roundtrips",
+           "opo_set_pump_host", "opo_set_field", "opo_set_field_host", "opo_propagate", "opo_roundtrips", "opo_roundtrips_train",
            "opo_get_fields", "opo_get_fields_host", "opo_sync", "opo_check_finite", "opo_get_z_steps",
            "opo_set_option", "opo_get_info", "opo_last_error"]
 
@@ -166,6 +167,11 @@ def opo_propagate(h, nz: int):
 
 def opo_roundtrips(h, n: int):
     _check(h, lib().opo_roundtrips(h, int(n)))
+
+
+def opo_roundtrips_train(h, n: int, dev_pump_train: int, per_instance: bool, dev_out_train: int, out_field: int):
+    _check(h, lib().opo_roundtrips_train(h, int(n), ctypes.c_void_p(dev_pump_train), int(per_instance),
+                                         ctypes.c_void_p(dev_out_train) if dev_out_train else None, int(out_field)))
 
 
 def opo_get_fields(h, field: int, which: int, domain: int, dev_ptr: int):
@@ -274,6 +280,20 @@ class Opo:
 
     def roundtrips(self, n):
         opo_roundtrips(self._h, n)
+
+    def roundtrips_train(self, pump_train, out_field=None):
+        """pump_train: CUDA tensor [n][N] or [n][batch][N]; returns the exit field `out_field` of every round trip,
+        [n][batch][N], or None (nanosecond regime)."""
+        torch = self._torch
+        assert pump_train.is_cuda and pump_train.dtype == self.dtype
+        n = pump_train.shape[0]
+        per = pump_train.dim() == 3
+        assert tuple(pump_train.shape[1:]) == ((self.batch, self.n) if per else (self.n,))
+        pump_train = pump_train.contiguous()
+        out = torch.empty((n, self.batch, self.n), dtype=self.dtype, device="cuda") if out_field is not None else None
+        opo_roundtrips_train(self._h, n, pump_train.data_ptr(), per, out.data_ptr() if out is not None else 0,
+                             out_field if out_field is not None else 0)
+        return out
 
     def get_fields(self, field, which=WHICH_CURRENT, domain=DOMAIN_TIME, out=None):
         torch = self._torch

@@ -806,6 +806,25 @@ int opo_roundtrips(opo_handle* h, int n) {
     return OPO_OK;
 }
 
+int opo_roundtrips_train(opo_handle* h, int n, const void* dev_pump_train, int per_instance, void* dev_out_train, int out_field) {
+    if (!h || !dev_pump_train) return fail(h, OPO_ERR_INVALID_ARG, "null argument");
+    if (n < 0) return fail(h, OPO_ERR_INVALID_ARG, "n must be >= 0");
+    if (dev_out_train && (out_field < 0 || out_field >= h->F)) return fail(h, OPO_ERR_INVALID_ARG, "out_field out of range");
+    if (h->fields.resonant[0]) return fail(h, OPO_ERR_UNSUPPORTED, "a pump train needs a single-pass (non-resonant) pump");
+    if (h->z_steps != 0) return fail(h, OPO_ERR_STATE, "roundtrips requires z = 0");
+    const size_t slice = (size_t)h->N * h->esz * (per_instance ? (size_t)h->B : 1);
+    for (int m = 0; m < n; ++m) {
+        // ReadPump: the m-th slice of the long pump vector becomes the intracavity pump
+        if (int rc = set_pump_impl(h, (const char*)dev_pump_train + (size_t)m * slice, per_instance, cudaMemcpyDeviceToDevice)) return rc;
+        if (int rc = opo_roundtrips(h, 1)) return rc;
+        // SaveRoundTrip: the field leaving the crystal in this round trip
+        if (dev_out_train)
+            OPO_CUDA(h, cudaMemcpyAsync((char*)dev_out_train + (size_t)m * h->field_bytes(), h->exitb[out_field], h->field_bytes(),
+                                        cudaMemcpyDeviceToDevice, h->stream));
+    }
+    return OPO_OK;
+}
+
 int opo_set_eom(opo_handle* h, int field, double beta_rad, double f_mod_hz) {
     if (!h) return OPO_ERR_INVALID_ARG;
     if (field < 0 || field >= h->F) return fail(h, OPO_ERR_INVALID_ARG, "field out of range");

@@ -469,6 +469,47 @@ def test_eom_config1_20_roundtrips_and_abi_errors():
     assert rel_l2(got[0], rc2[0, 1]) <= 1e-4
 
 
+# ---------------------------------------------------------------------------------------------------------
+# nanosecond regime: pump train in, round-trip train out
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("engine_idx", [0, 1])
+@pytest.mark.parametrize("precision,log2_n,n_fields", [("c64", 12, 2), ("c128", 9, 3)])
+def test_pump_train_matches_oracle_loop(precision, log2_n, n_fields, engine_idx):
+    """A pump pulse 6 windows long (Gaussian envelope sampled across the train, as the paper's ns pulse across many
+    round trips): round trip m is pumped by slice m; the signal leaving the crystal in every round trip is recorded.
+    The oracle side is the definition written out: set the pump slice, one round trip, read the exit field."""
+    import oracle
+    torch, P = _gpu()
+    engine = engines()[engine_idx]
+    w = small_workload(log2_n, n_fields, precision, nz=5, batch=2, dk=9.0, gdd_dt2=0.5, drad=0.2)
+    _engine_or_skip(w, engine)
+    n_rt, n = 6, w.n
+    g = np.arange(n_rt * n) / (n_rt * n) - 0.5
+    env = np.exp(-(g / 0.22) ** 2) * np.exp(1j * 2.0 * g)                       # long pulse with a slow chirp
+    a_p = np.abs(w.pump[0]).max()
+    train = W._round_to_precision((a_p * env).reshape(n_rt, n), precision)        # [n_rt][N], same for both instances
+    o = P.from_workload(w, engine=engine)
+    tt = torch.from_numpy(train).to(o.dtype).cuda()
+    out = o.roundtrips_train(tt, out_field=1)
+    o.sync()
+    got_out = out.cpu().numpy().astype(np.complex128)
+    got_cur = np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    o.close()
+    tol = TOL[precision]
+    for b in range(w.batch):
+        ro = oracle.from_workload(w, b)
+        for m in range(n_rt):
+            ro.set_field(0, train[m])
+            assert ro.roundtrips(1) == 0
+            ref = ro.get_field(1, oracle.EXIT)
+            assert rel_l2(got_out[m, b], ref) <= tol, (m, b, rel_l2(got_out[m, b], ref))
+        for x in range(w.n_fields):
+            ref = ro.get_field(x, oracle.CURRENT)
+            assert rel_l2(got_cur[b, x], ref) <= tol
+    # the pump is re-injected from the last slice
+    assert rel_l2(got_cur[0, 0], train[-1]) == 0.0
+
+
 def test_abi_errors_and_state():
     torch, P = _gpu()
     w = small_workload(8, 2, "c64", nz=4)
