@@ -40,6 +40,28 @@ struct alignas(2 * sizeof(T)) cplx {
 
 template <class T> __device__ __forceinline__ cplx<T> operator+(cplx<T> a, cplx<T> b) { return {a.re + b.re, a.im + b.im}; }
 template <class T> __device__ __forceinline__ cplx<T> operator-(cplx<T> a, cplx<T> b) { return {a.re - b.re, a.im - b.im}; }
+// fp32: complex add / subtract as ONE packed instruction (FADD2 on sm_100: two lanes of the FP32 pipe for two
+// cycles, but a single issue slot -- the kernels are issue-bound, the FP32 pipe is ~55 % busy)
+__device__ __forceinline__ unsigned long long pack2(cplx<float> a) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.re), "f"(a.im));
+    return r;
+}
+__device__ __forceinline__ cplx<float> unpack2(unsigned long long v) {
+    cplx<float> r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.re), "=f"(r.im) : "l"(v));
+    return r;
+}
+template <> __device__ __forceinline__ cplx<float> operator+(cplx<float> a, cplx<float> b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)));
+    return unpack2(r);
+}
+template <> __device__ __forceinline__ cplx<float> operator-(cplx<float> a, cplx<float> b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)));
+    return unpack2(r);
+}
 // a * b
 template <class T> __device__ __forceinline__ cplx<T> cmul(cplx<T> a, cplx<T> b) {
     return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re};
