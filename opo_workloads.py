@@ -70,6 +70,8 @@ class Workload:
     # intracavity phase modulator per field: depth [rad] (0 = none) and frequency [Hz]
     eom_beta_rad: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
     eom_f_hz: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
+    # third-order dispersion per field [s^3/m] (Eq. 5, reading R7); 0 = none
+    beta3_s3_per_m: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
 
     @property
     def n(self) -> int:

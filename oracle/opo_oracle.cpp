@@ -18,6 +18,7 @@
 //        (A_p, A_s[, A_i])[n] <- one classic RK4 step of size h of the coupling terms of
 //                                Eqs 2-4, abscissae z, z+h/2, z+h/2, z+h (R3, R4)
 //        A_x <- IDFT( H_x .* DFT(A_x) );  z += h
+//        (optional third-order dispersion: D_x -= (beta3_x/6) Omega^3, reading R7)
 //   pass    = nz z-steps from z = 0
 //   boundary (Eq. 6, Listing 3; R11-R15):
 //        exit_x <- A_x
@@ -29,7 +30,8 @@
 // Pins (tests/test_oracle_*.py, -m "not gpu"): P1 naive DFT, P2 Gaussian GVD closed form, P3 GVM
 // integer shift, P4 cosh^2 gain (+dk), P5 degenerate phase-sensitive gain (paper's pi/4, -3pi/4,
 // PAPER.md:L400), P6 Manley-Rowe, P7 depleted SHG closed form, P8 2nd-order convergence, P9 cold
-// cavity, P10 threshold growth, P13 EOM sidebands = Bessel J_m(beta) (Jacobi-Anger) and element order.
+// cavity, P10 threshold growth, P13 EOM sidebands = Bessel J_m(beta) (Jacobi-Anger) and element order,
+// P14 third-order dispersion: centroid delay (beta3 z/2)(Omega_0^2 + s^2) of an offset Gaussian.
 // Parity unpinned: reading R12 (non-resonant fields restart from
 // S_x) is a convention with no physical pin; the paper's P_th values (L348) and Figs 3-5.
 // =================================================================================================
@@ -104,6 +106,7 @@ struct Params {
     double lambda_m[3], n_index[3], beta1[3], beta2[3], alpha[3];
     int resonant[3];
     double R[3], delta_rad[3], delta_T[3], gdd[3];
+    double beta3[3];                // third-order dispersion of field x [s^3/m] (Eq. 5; reading R7), 0 unless set
     double eom_beta[3], eom_f[3];   // intracavity phase modulator: depth [rad], frequency [Hz]
 };
 
@@ -151,7 +154,9 @@ struct Oracle {
             for (int k = 0; k < N; ++k) {
                 double om = omega(k);
                 // D_x(Omega) = -Delta beta1_x Omega + (beta2_x / 2) Omega^2          Eq. 5, R7/R8
-                double D = -db1 * om + 0.5 * p.beta2[x] * om * om;
+                //              - (beta3_x / 6) Omega^3      third-order dispersion in its physical form +(beta3/6) d^3/dtau^3
+                //                (R7: the term as printed in Eq. 5 would be a gain, not a phase)
+                double D = -db1 * om + 0.5 * p.beta2[x] * om * om - p.beta3[x] / 6.0 * om * om * om;
                 // H_x = exp( (-alpha_x/2 + i D_x) h/2 )                              half step
                 std::complex<double> e = std::exp(std::complex<double>(-0.5 * p.alpha[x], D) * (0.5 * h));
                 H[x][k] = C((R)e.real(), (R)e.imag());
@@ -322,6 +327,13 @@ void opo_oracle_set_field(void* h, int field, int which, const double* reim) {
         if (which != 1) set_vec(hnd->d->A[field], reim);
         if (which != 0) set_vec(hnd->d->S[field], reim);
     }
+}
+
+// third-order dispersion of field x; rebuilds the multiplier tables
+void opo_oracle_set_beta3(void* h, int field, double beta3_s3_per_m) {
+    Handle* hnd = (Handle*)h;
+    if (hnd->is_float) { hnd->f->p.beta3[field] = beta3_s3_per_m; hnd->f->build_tables(); }
+    else               { hnd->d->p.beta3[field] = beta3_s3_per_m; hnd->d->build_tables(); }
 }
 
 // intracavity phase modulator on (resonant) field x; beta = 0 switches it off

@@ -275,6 +275,29 @@ def test_config4_full_batch_in_bench_launch_configuration():
     print(f"C4 full batch, 2 RT, sampled {sample}: rel L2 current {e1:.3e} exit {e2:.3e}")
 
 
+def test_resident_engine_is_bitwise_reproducible():
+    """The resident kernel synchronises its three CTAs per instance with class-granular mbarriers instead of cluster
+    barriers; a missing dependency would be a data race, and a race shows up as run-to-run differences.  Two runs of the
+    full C4 batch (256 instances, 6 waves over the clusters) must agree bit for bit; a run split into one call per round
+    trip (un-merged boundary, state through HBM) must agree to rounding."""
+    torch, P = _gpu()
+    w = W.config4().truncated(3)
+    outs = []
+    for calls in (1, 1, 3):
+        o = P.from_workload(w, engine=P.ENGINE_RESIDENT)
+        for _ in range(calls):
+            o.roundtrips(w.n_roundtrips // calls)
+        o.sync()
+        outs.append([o.get_fields(x, which).clone() for x in range(w.n_fields) for which in (P.WHICH_CURRENT, P.WHICH_EXIT)])
+        o.close()
+    for a, b in zip(outs[0], outs[1]):
+        assert torch.equal(a.view(torch.float32), b.view(torch.float32)), "two identical launches differ: data race"
+    # one launch per round trip takes the un-merged boundary path: equal to rounding, not bit for bit
+    for a, b in zip(outs[0], outs[2]):
+        d = (a - b).abs().max().item() / a.abs().max().item()
+        assert d < 1e-5, d
+
+
 @pytest.mark.parametrize("engine_idx", [0, 1])
 def test_long_noise_seeded_run_power_and_spectrum(engine_idx):
     """BASELINE.json:north_star, long noise-seeded runs: relative error <= 1e-3 on output signal power and on the power

@@ -550,3 +550,43 @@ def test_p13_eom_acts_after_gdd_and_mirror_on_resonant_fields_only():
     assert rel_l2(o.get_field(2), s2) < 1e-15      # pump = 0, so the idler seed passes unchanged and is re-injected
     # the exit field is taken before the boundary: no modulator on it
     assert rel_l2(o.get_field(1, EXIT), a) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# P14  third-order dispersion (Eq. 5 in the reading R7)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("b3_fs3_per_um,w0", [(40.0, 0.0), (-25.0, 0.12e15), (60.0, -0.05e15)])
+def test_p14_tod_group_delay_of_an_offset_gaussian(b3_fs3_per_um, w0):
+    """Pure third-order dispersion, no coupling.  For dA/dz = +(beta3/6) d^3A/dtau^3 a spectral component at physical
+    offset w (field ~ e^{-i w tau}) acquires the phase -(beta3/6)(-w)^3 ... in the bin convention of R8 the multiplier is
+    exp(-i (beta3/6) Omega_k^3 z).  The centroid of |A|^2 moves by the power-weighted mean group delay, in closed form
+    for a Gaussian spectrum centred on Omega_0 with power-spectrum variance s^2:  <tau> = (beta3 z / 2)(Omega_0^2 + s^2),
+    independent of the sign of Omega_0 (even in Omega) and odd in beta3.  Pins sign, the 1/6 and the Omega^3."""
+    log2n, T, L, nz = 10, 20 * PS, 5e-3, 10
+    n = 1 << log2n
+    dt = T / n
+    b3 = b3_fs3_per_um * FS ** 3 / UM
+    T0 = 150 * FS
+    o = make(n_fields=2, log2_n=log2n, window_s=T, nz=nz, length=L, d_eff=0.0)
+    o.set_beta3(1, b3)
+    tau = (np.arange(n) - n // 2) * dt
+    # carrier offset chosen on the bin grid so that the field is periodic on the window
+    kbin = round(w0 * n * dt / (2 * np.pi))
+    om0 = 2 * np.pi * kbin / (n * dt)
+    a = np.exp(-tau ** 2 / (2 * T0 ** 2)) * np.exp(1j * om0 * tau)     # spectrum centred on bin +kbin (Omega_k = om0)
+    o.set_field(0, np.zeros(n, complex))
+    o.set_field(1, a)
+    assert o.propagate(nz) == 0
+    out = o.get_field(1)
+    p = np.abs(out) ** 2
+    centroid = np.sum(tau * p) / np.sum(p)
+    s2 = 1.0 / (2 * T0 ** 2)                       # variance of |A~|^2 for A = exp(-tau^2 / 2 T0^2)
+    # group delay under R8: multiplier exp(i D z), D = -(beta3/6) Omega^3, delay = -dD/dOmega ... z = (beta3/2) Omega^2 z
+    expect = 0.5 * b3 * L * (om0 ** 2 + s2)
+    assert abs(centroid - expect) < 2e-4 * max(abs(expect), T0), (centroid, expect)
+    assert abs(np.sum(p) / np.sum(np.abs(a) ** 2) - 1.0) < 1e-12     # a pure phase: energy conserved
+    # exact spectral check against the closed-form multiplier with the library FFT
+    om = 2 * np.pi * np.fft.fftfreq(n, d=1.0 / n) / (n * dt)
+    ref = np.fft.ifft(np.fft.fft(a) * np.exp(-1j * (b3 / 6.0) * om ** 3 * L))
+    assert rel_l2(out, ref) < 1e-11
