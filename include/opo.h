@@ -116,6 +116,11 @@ int opo_set_stream(opo_handle* h, void* cuda_stream);
 #define OPO_PARAM_GDD 3
 int opo_set_batch_param(opo_handle* h, int param, int field, const double* host_vals, int count);
 
+/* Third-order dispersion of field `field` [s^3/m] (Eq. 5; reading R7 of DESIGN.md: the physical form
+ * dA/dz = +(beta3/6) d^3A/dtau^3, i.e. D_x(Omega) gains the term -(beta3_x/6) Omega^3; the term as printed would be a
+ * gain).  0 removes it.  Only the fp64 host tables change (rebuilt before the next propagate / roundtrips call). */
+int opo_set_beta3(opo_handle* h, int field, double beta3_s3_per_m);
+
 /* Intracavity electro-optic phase modulator on a resonant field, the last element of the cavity boundary
  * ("A(tau) -> A(tau) exp(i beta sin(2 pi f_pm tau))"; Listing 3
  * PhaseModulatorIntraCavity, after AddGDD and AddPhase): every round trip, after the spectral phase and the

@@ -70,6 +70,7 @@ def lib() -> ctypes.CDLL:
         L.opo_set_stream.argtypes = [vp, vp]
         L.opo_set_batch_param.argtypes = [vp, ci, ci, ctypes.POINTER(ctypes.c_double), ci]
         L.opo_set_eom.argtypes = [vp, ci, ctypes.c_double, ctypes.c_double]
+        L.opo_set_beta3.argtypes = [vp, ci, ctypes.c_double]
         L.opo_set_pump.argtypes = [vp, vp, ci]
         L.opo_set_pump_host.argtypes = [vp, vp, ci]
         L.opo_set_field.argtypes = [vp, ci, vp]
@@ -93,7 +94,7 @@ def lib() -> ctypes.CDLL:
     return _lib
 
 
-EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_eom", "opo_set_pump",
+EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_eom", "opo_set_beta3", "opo_set_pump",
            "opo_set_pump_host", "opo_set_field", "opo_set_field_host", "opo_propagate", "opo_roundtrips", "opo_roundtrips_train",
            "opo_get_fields", "opo_get_fields_host", "opo_sync", "opo_check_finite", "opo_get_z_steps",
            "opo_set_option", "opo_get_info", "opo_last_error"]
@@ -139,6 +140,10 @@ def opo_set_stream(h, cuda_stream: int):
 def opo_set_batch_param(h, param: int, field: int, values):
     v = np.ascontiguousarray(values, dtype=np.float64)
     _check(h, lib().opo_set_batch_param(h, param, field, v.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), v.size))
+
+
+def opo_set_beta3(h, field: int, beta3_s3_per_m: float):
+    _check(h, lib().opo_set_beta3(h, int(field), float(beta3_s3_per_m)))
 
 
 def opo_set_eom(h, field: int, beta_rad: float, f_mod_hz: float):
@@ -257,6 +262,9 @@ class Opo:
     def set_batch_param(self, param, field, values):
         opo_set_batch_param(self._h, param, field, values)
 
+    def set_beta3(self, field, beta3_s3_per_m):
+        opo_set_beta3(self._h, field, beta3_s3_per_m)
+
     def set_eom(self, field, beta_rad, f_mod_hz):
         opo_set_eom(self._h, field, beta_rad, f_mod_hz)
 
@@ -343,6 +351,8 @@ def from_workload(w, engine=ENGINE_AUTO, host_inputs=False) -> Opo:
     for x in range(w.n_fields):
         if w.eom_beta_rad[x] != 0.0:
             o.set_eom(x, w.eom_beta_rad[x], w.eom_f_hz[x])
+        if w.beta3_s3_per_m[x] != 0.0:
+            o.set_beta3(x, w.beta3_s3_per_m[x])
     load_inputs(o, w, host_inputs)
     return o
 

@@ -115,6 +115,7 @@ struct opo_handle {
     void* mirror[3] = {nullptr, nullptr, nullptr};
     void* eom[3] = {nullptr, nullptr, nullptr};       // [N] exp(i beta sin(2 pi f tau_n)) or null
     double eom_beta[3] = {0, 0, 0}, eom_f[3] = {0, 0, 0};
+    double beta3[3] = {0, 0, 0};                      // third-order dispersion [s^3/m] (opo_set_beta3)
     bool boundary_fft[3] = {false, false, false};
     void* phase = nullptr;
     int* flag = nullptr;
@@ -242,9 +243,10 @@ int build_tables(opo_handle* h) {
     for (int x = 0; x < F; ++x) {
         const double db1 = h->fields.beta1_s_per_m[x] - h->fields.beta1_s_per_m[h->fields.ref_field];
         const double b2 = h->fields.beta2_s2_per_m[x], al = h->fields.alpha_per_m[x];
+        const double b3 = h->beta3[x] / 6.0;            // D_x -= (beta3_x/6) Omega^3   (reading R7)
         for (int k = 0; k < N; ++k) {
             const double om = omega_of(h, k);
-            const double D = -db1 * om + 0.5 * b2 * om * om;
+            const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
             Hh[k] = std::exp(cd(-0.5 * al, D) * (0.5 * h->h));
         }
         for (int k = 0; k < N; ++k) M[k] = Hh[k] * invN;
@@ -252,7 +254,7 @@ int build_tables(opo_handle* h) {
         if (int rc = upload_table(h, h->tabH[x], lay.data(), N)) return rc;
         for (int k = 0; k < N; ++k) {
             const double om = omega_of(h, k);
-            const double D = -db1 * om + 0.5 * b2 * om * om;
+            const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
             M[k] = std::exp(cd(-0.5 * al, D) * h->h) * invN;     // H^2 evaluated directly in fp64
         }
         to_engine_layout(h, pl, M.data(), lay.data());
@@ -283,7 +285,7 @@ int build_tables(opo_handle* h) {
                 const double om = omega_of(h, k);
                 const double ph = 0.5 * h->gdd[x][b] * om * om - om * h->dT[x][b];
                 const cd gm = cd(std::cos(ph), std::sin(ph)) * mir[b];
-                const double D = -db1 * om + 0.5 * b2 * om * om;
+                const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
                 M[k] = gm * invN;
                 Hh[k] = std::exp(cd(-0.5 * al, D) * h->h) * gm * invN;
             }
@@ -822,6 +824,15 @@ int opo_roundtrips_train(opo_handle* h, int n, const void* dev_pump_train, int p
             OPO_CUDA(h, cudaMemcpyAsync((char*)dev_out_train + (size_t)m * h->field_bytes(), h->exitb[out_field], h->field_bytes(),
                                         cudaMemcpyDeviceToDevice, h->stream));
     }
+    return OPO_OK;
+}
+
+int opo_set_beta3(opo_handle* h, int field, double beta3_s3_per_m) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    if (field < 0 || field >= h->F) return fail(h, OPO_ERR_INVALID_ARG, "field out of range");
+    if (!std::isfinite(beta3_s3_per_m)) return fail(h, OPO_ERR_INVALID_ARG, "non-finite beta3");
+    h->beta3[field] = beta3_s3_per_m;
+    h->tables_dirty = true;
     return OPO_OK;
 }
 

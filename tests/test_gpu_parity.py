@@ -533,6 +533,40 @@ def test_pump_train_matches_oracle_loop(precision, log2_n, n_fields, engine_idx)
     assert rel_l2(got_cur[0, 0], train[-1]) == 0.0
 
 
+# ---------------------------------------------------------------------------------------------------------
+# third-order dispersion (Eq. 5 in the reading R7): tables only
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("engine_idx", [0, 1])
+@pytest.mark.parametrize("precision,log2_n,n_fields", [("c64", 12, 3), ("c128", 10, 2), ("c64", 14, 3)])
+def test_third_order_dispersion_matches_oracle(precision, log2_n, n_fields, engine_idx):
+    engine = engines()[engine_idx]
+    w = small_workload(log2_n, n_fields, precision, nz=5, batch=2, dk=7.0, gdd_dt2=0.5, drad=0.2)
+    # beta3 L / 6 * Omega_max^3 of a few radians at the band edge: clearly visible, well resolved
+    om_max = math.pi / w.dt
+    w.beta3_s3_per_m = [(1.5 + x) * 6.0 * 3.0 / (om_max ** 3 * w.length_m) for x in range(n_fields)] + [0.0] * (3 - n_fields)
+    _engine_or_skip(w, engine)
+    cur, ex, _ = run_gpu(w, engine, n_roundtrips=2)
+    rcur, rex = run_oracle(w, n_roundtrips=2)
+    e1 = assert_close(cur, rcur, TOL[precision], "TOD current")
+    e2 = assert_close(ex, rex, TOL[precision], "TOD exit")
+    w0 = small_workload(log2_n, n_fields, precision, nz=5, batch=2, dk=7.0, gdd_dt2=0.5, drad=0.2)
+    c0, _ = run_oracle(w0, n_roundtrips=2)
+    assert rel_l2(c0[0, 1], rcur[0, 1]) > 0.05          # the term does something
+    print(f"TOD {precision} 2^{log2_n} engine {engine}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
+def test_third_order_dispersion_large_engine():
+    torch, P = _gpu()
+    w = small_workload(15, 2, "c64", nz=4, batch=1, dk=5.0, gdd_dt2=0.5, drad=0.2)
+    om_max = math.pi / w.dt
+    w.beta3_s3_per_m = [2.0 * 18.0 / (om_max ** 3 * w.length_m), -1.0 * 18.0 / (om_max ** 3 * w.length_m), 0.0]
+    cur, ex, eng = run_gpu(w, P.ENGINE_AUTO, n_roundtrips=2)
+    assert eng == P.ENGINE_LARGE
+    rcur, rex = run_oracle(w, n_roundtrips=2)
+    assert_close(cur, rcur, 1e-4, "TOD large current")
+    assert_close(ex, rex, 1e-4, "TOD large exit")
+
+
 def test_abi_errors_and_state():
     torch, P = _gpu()
     w = small_workload(8, 2, "c64", nz=4)
