@@ -42,11 +42,16 @@ def flops_per_grid_point_zstep(log2_n: int, n_fields: int) -> float:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu captures
-# of exactly this launch configuration (profiles/r01f_*.md); None where no capture of that configuration exists.
+# of exactly this launch configuration (profiles/r01h_*.md); None where no capture of that configuration exists.
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, engine, round trips per step): bytes
-    ("C4", "resident", 300): 187344896 + 243991040,     # profiles/r01f_dram_c4_default.csv (one 3.1 s launch)
+    ("C4", "resident", 300): 237353216 + 317747200,     # profiles/r01h_dram_c4_default.csv (one 3.06 s launch)
 }
+
+
+# sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed of the resident kernel on C4 (profiles/r01h_resident_kernel_final.md,
+# `ncu --set full` capture of a 2-round-trip launch): how busy the FP32 pipe is over all SM cycles of the launch
+NCU_FP32_PIPE_PCT = {("C4", "resident"): 48.8}
 
 
 def ncu_traffic_bytes(workload: str, engine: str, rt_per_step: int):
@@ -299,6 +304,7 @@ def main():
         peak_tflops = 148 * (64 if dbl else 128) * 2 * 1.965e9 / 1e12
         roofline = {"bound": "alu", "kernel": "k_resident", "achieved": fl / avg_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
                     "frac": fl / avg_s / 1e12 / peak_tflops, "traffic": traffic,
+                    "fp32_pipe_busy_pct_ncu": NCU_FP32_PIPE_PCT.get((args.workload, eng_name)),
                     "note": f"{'FP64' if dbl else 'FP32'} FMA-pipe peak = 148 SM x {64 if dbl else 128} lanes x 2 x 1.965 GHz (guide unit counts, max clock); "
                             f"algorithmic flops = {flops_per_grid_point_zstep(w.log2_n, w.n_fields):.0f}/grid-point z-step "
                             "(merged half-steps, 5 N log2 N per transform); one launch = one step"}
