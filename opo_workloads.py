@@ -72,6 +72,8 @@ class Workload:
     eom_f_hz: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
     # third-order dispersion per field [s^3/m] (Eq. 5, reading R7); 0 = none
     beta3_s3_per_m: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
+    # operator splitting: 0 = L/2 - N - L/2 (default), 1 = N/2 - L - N/2 (the paper's Eq. 10-11)
+    splitting: int = 0
 
     @property
     def n(self) -> int:

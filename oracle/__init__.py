@@ -46,6 +46,7 @@ def lib():
         L.opo_oracle_set_field.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, _DP]
         L.opo_oracle_set_eom.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double]
         L.opo_oracle_set_beta3.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double]
+        L.opo_oracle_set_splitting.argtypes = [ctypes.c_void_p, ctypes.c_int]
         L.opo_oracle_propagate.argtypes = [ctypes.c_void_p, ctypes.c_int]
         L.opo_oracle_propagate.restype = ctypes.c_int
         L.opo_oracle_roundtrips.argtypes = [ctypes.c_void_p, ctypes.c_int]
@@ -121,6 +122,10 @@ class OracleOpo:
         code = {"state": 0, "input": 1, "both": 2}[which]
         lib().opo_oracle_set_field(self._h, field, code, d.view(np.float64).ctypes.data_as(_DP))
 
+    def set_splitting(self, splitting: int):
+        """0: L/2 - N - L/2 (default); 1: N/2 - L - N/2, the order of the paper's Eq. 10-11."""
+        lib().opo_oracle_set_splitting(self._h, int(splitting))
+
     def set_beta3(self, field: int, beta3_s3_per_m: float):
         """Third-order dispersion of a field (Eq. 5 in the reading R7)."""
         lib().opo_oracle_set_beta3(self._h, int(field), float(beta3_s3_per_m))
@@ -165,6 +170,8 @@ def from_workload(w, b: int = 0, use_float: bool = False) -> OracleOpo:
             o.set_eom(x, w.eom_beta_rad[x], w.eom_f_hz[x])
         if w.beta3_s3_per_m[x] != 0.0:
             o.set_beta3(x, w.beta3_s3_per_m[x])
+    if w.splitting:
+        o.set_splitting(w.splitting)
     return o
 
 

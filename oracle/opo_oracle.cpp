@@ -18,6 +18,7 @@
 //        (A_p, A_s[, A_i])[n] <- one classic RK4 step of size h of the coupling terms of
 //                                Eqs 2-4, abscissae z, z+h/2, z+h/2, z+h (R3, R4)
 //        A_x <- IDFT( H_x .* DFT(A_x) );  z += h
+//        (optional: the paper's own order N/2 - L - N/2 of Eq. 10-11, two RK4 half-steps around one full linear step)
 //        (optional third-order dispersion: D_x -= (beta3_x/6) Omega^3, reading R7)
 //   pass    = nz z-steps from z = 0
 //   boundary (Eq. 6, Listing 3; R11-R15):
@@ -31,7 +32,8 @@
 // integer shift, P4 cosh^2 gain (+dk), P5 degenerate phase-sensitive gain (paper's pi/4, -3pi/4,
 // PAPER.md:L400), P6 Manley-Rowe, P7 depleted SHG closed form, P8 2nd-order convergence, P9 cold
 // cavity, P10 threshold growth, P13 EOM sidebands = Bessel J_m(beta) (Jacobi-Anger) and element order,
-// P14 third-order dispersion: centroid delay (beta3 z/2)(Omega_0^2 + s^2) of an offset Gaussian.
+// P14 third-order dispersion: centroid delay (beta3 z/2)(Omega_0^2 + s^2) of an offset Gaussian, P15 N/2-L-N/2 ordering:
+// second-order convergence, O(h^2) agreement with L/2-N-L/2, exact agreement when the operators commute.
 // Parity unpinned: reading R12 (non-resonant fields restart from
 // S_x) is a convention with no physical pin; the paper's P_th values (L348) and Figs 3-5.
 // =================================================================================================
@@ -106,6 +108,7 @@ struct Params {
     double lambda_m[3], n_index[3], beta1[3], beta2[3], alpha[3];
     int resonant[3];
     double R[3], delta_rad[3], delta_T[3], gdd[3];
+    int splitting;                  // 0: L/2 - N - L/2 (north_star, default); 1: N/2 - L - N/2 (the paper's Eq. 10-11)
     double beta3[3];                // third-order dispersion of field x [s^3/m] (Eq. 5; reading R7), 0 unless set
     double eom_beta[3], eom_f[3];   // intracavity phase modulator: depth [rad], frequency [Hz]
 };
@@ -119,7 +122,7 @@ struct Oracle {
     double z;       // position inside the crystal, 0 at the entrance (R4, R20)
     double kappa[3];
     Fft<R> fft;
-    std::vector<C> A[3], S[3], EX[3], H[3], G[3];
+    std::vector<C> A[3], S[3], EX[3], H[3], HF[3], G[3];
     bool boundary_needs_transform[3];
 
     // Omega_k = 2 pi k' / (N dt), natural FFT order, Nyquist bin negative (R9)
@@ -149,6 +152,7 @@ struct Oracle {
     void build_tables() {
         for (int x = 0; x < F; ++x) {
             H[x].resize(N);
+            HF[x].resize(N);
             G[x].resize(N);
             double db1 = p.beta1[x] - p.beta1[p.ref_field];       // Delta beta1_x (R7, R10)
             for (int k = 0; k < N; ++k) {
@@ -160,6 +164,9 @@ struct Oracle {
                 // H_x = exp( (-alpha_x/2 + i D_x) h/2 )                              half step
                 std::complex<double> e = std::exp(std::complex<double>(-0.5 * p.alpha[x], D) * (0.5 * h));
                 H[x][k] = C((R)e.real(), (R)e.imag());
+                // full step exp( (-alpha_x/2 + i D_x) h ), used by the N/2 - L - N/2 ordering (Eq. 11)
+                std::complex<double> ef = std::exp(std::complex<double>(-0.5 * p.alpha[x], D) * h);
+                HF[x][k] = C((R)ef.real(), (R)ef.imag());
                 // G_x = exp( i (gamma_x/2) Omega^2 - i Omega DeltaT_x )              L145, R13, R14
                 double ph = 0.5 * p.gdd[x] * om * om - om * p.delta_T[x];
                 G[x][k] = C((R)std::cos(ph), (R)std::sin(ph));
@@ -194,8 +201,18 @@ struct Oracle {
         }
     }
 
-    void nonlinear_step() {
-        const R hh = (R)h;
+    void linear_full_step() {
+        for (int x = 0; x < F; ++x) {
+            fft.transform(A[x].data(), false);
+            for (int k = 0; k < N; ++k) A[x][k] = A[x][k] * HF[x][k];
+            fft.transform(A[x].data(), true);
+        }
+    }
+
+    // one classic RK4 step of size hstep of the coupling terms, from position z0 (R3, R4)
+    void nonlinear_step(double z0, double hstep) {
+        const R hh = (R)hstep;
+        const double z = z0, h = hstep;
         for (int n = 0; n < N; ++n) {
             C y[3], k1[3], k2[3], k3[3], k4[3], t[3];
             for (int x = 0; x < F; ++x) y[x] = A[x][n];
@@ -212,9 +229,15 @@ struct Oracle {
     }
 
     void z_step() {
-        linear_half_step();
-        nonlinear_step();
-        linear_half_step();
+        if (p.splitting == 0) {          // L/2 - N - L/2 ("its counterpart"; north_star; R2)
+            linear_half_step();
+            nonlinear_step(z, h);
+            linear_half_step();
+        } else {                          // N/2 - L - N/2, the order the paper implements (Eq. 10-11)
+            nonlinear_step(z, 0.5 * h);
+            linear_full_step();
+            nonlinear_step(z + 0.5 * h, 0.5 * h);
+        }
         z += h;
     }
 
@@ -327,6 +350,13 @@ void opo_oracle_set_field(void* h, int field, int which, const double* reim) {
         if (which != 1) set_vec(hnd->d->A[field], reim);
         if (which != 0) set_vec(hnd->d->S[field], reim);
     }
+}
+
+// 0: L/2 - N - L/2 (default), 1: N/2 - L - N/2 (Eq. 10-11)
+void opo_oracle_set_splitting(void* h, int splitting) {
+    Handle* hnd = (Handle*)h;
+    if (hnd->is_float) hnd->f->p.splitting = splitting;
+    else               hnd->d->p.splitting = splitting;
 }
 
 // third-order dispersion of field x; rebuilds the multiplier tables

@@ -590,3 +590,51 @@ def test_p14_tod_group_delay_of_an_offset_gaussian(b3_fs3_per_um, w0):
     om = 2 * np.pi * np.fft.fftfreq(n, d=1.0 / n) / (n * dt)
     ref = np.fft.ifft(np.fft.fft(a) * np.exp(-1j * (b3 / 6.0) * om ** 3 * L))
     assert rel_l2(out, ref) < 1e-11
+
+
+# ---------------------------------------------------------------------------------------------
+# P15  the paper's own operator order N/2 - L - N/2 (Eq. 10-11)
+# ---------------------------------------------------------------------------------------------
+
+def _p15_run(nz, splitting, beta=True, d_eff=14e-12):
+    log2n, L = 7, 5e-3
+    n = 1 << log2n
+    tau = (np.arange(n) - n // 2) * (10 * PS / n)
+    o = make(n_fields=3, log2_n=log2n, nz=nz, length=L, dk=40.0, d_eff=d_eff,
+             beta1=(0.3 * FS / UM, 0.0, -0.2 * FS / UM) if beta else (0, 0, 0),
+             beta2=(35 * FS * FS / UM, 12 * FS * FS / UM, 5 * FS * FS / UM) if beta else (0, 0, 0))
+    o.set_splitting(splitting)
+    ks = 2 * np.pi * 14e-12 / (2.16 * 1000 * NM)
+    amp = 1.0 / (ks * L)
+    o.set_field(0, amp * np.exp(-(tau / (0.8 * PS)) ** 2).astype(complex))
+    o.set_field(1, 0.3 * amp * np.exp(-((tau - 0.5 * PS) / (0.6 * PS)) ** 2) * np.exp(2j * np.pi * tau / (3 * PS)))
+    o.set_field(2, 0.2 * amp * np.exp(-((tau + 0.4 * PS) / (0.7 * PS)) ** 2).astype(complex))
+    assert o.propagate(nz) == 0
+    return np.concatenate([o.get_field(x) for x in range(3)])
+
+
+def test_p15_nln_ordering_is_second_order_and_agrees_with_lnl_to_second_order():
+    gv = golden()
+    order = gv["symmetrized_ssfm_local_error_order"] - 1            # printed: local error O(dz^3) (L131)
+    ref = _p15_run(16 * 32, 1)
+    e = [np.linalg.norm(_p15_run(nz, 1) - ref) for nz in (16, 32, 64)]
+    assert abs(e[0] / e[1] - 2 ** order) < 0.1 and abs(e[1] / e[2] - 2 ** order) < 0.1
+    # "equivalent to its counterpart L/2 - N - L/2, since both lead to the same solution" (L133): same limit, and
+    # the two orders differ from each other by O(h^2) -- not bit for bit
+    d = [np.linalg.norm(_p15_run(nz, 1) - _p15_run(nz, 0)) for nz in (16, 32, 64)]
+    assert d[0] > 0 and abs(d[0] / d[1] - 4.0) < 0.2 and abs(d[1] / d[2] - 4.0) < 0.2
+    d512 = np.linalg.norm(ref - _p15_run(16 * 32, 0))
+    assert abs(d512 / (d[2] / 64.0) - 1.0) < 0.05               # still falling as h^2: the limits coincide
+
+
+def test_p15_nln_ordering_special_cases():
+    # no coupling: both orders are the same product of linear multipliers, H.H = exp(D h)
+    a = _p15_run(10, 1, d_eff=0.0)
+    b = _p15_run(10, 0, d_eff=0.0)
+    assert rel_l2(a, b) < 1e-13
+    # no dispersion: N/2 - L - N/2 is plain RK4 with step h/2 (2 nz steps), L/2 - N - L/2 is RK4 with step h:
+    # the N/2-L-N/2 run with nz steps must equal the L/2-N-L/2 run with 2 nz steps
+    a = _p15_run(10, 1, beta=False)
+    b = _p15_run(20, 0, beta=False)
+    assert rel_l2(a, b) < 1e-13
+    assert rel_l2(a, _p15_run(10, 0, beta=False)) > 1e-9          # and not the h-step result
