@@ -25,6 +25,8 @@ WHICH_CURRENT, WHICH_EXIT = 0, 1
 DOMAIN_TIME, DOMAIN_FREQ = 0, 1
 ENGINE_AUTO, ENGINE_RESIDENT, ENGINE_STREAMING, ENGINE_LARGE = 0, 1, 2, 3
 OPT_ENGINE = 0
+OPT_SPLITTING = 1
+SPLITTING_LNL, SPLITTING_NLN = 0, 1
 INFO_ENGINE, INFO_LAUNCHES, INFO_N, INFO_BATCH, INFO_SM_COUNT = 0, 1, 2, 3, 4
 
 _D3 = ctypes.c_double * 3
@@ -353,6 +355,8 @@ def from_workload(w, engine=ENGINE_AUTO, host_inputs=False) -> Opo:
             o.set_eom(x, w.eom_beta_rad[x], w.eom_f_hz[x])
         if w.beta3_s3_per_m[x] != 0.0:
             o.set_beta3(x, w.beta3_s3_per_m[x])
+    if w.splitting:
+        opo_set_option(o._h, OPT_SPLITTING, int(w.splitting))
     load_inputs(o, w, host_inputs)
     return o
 

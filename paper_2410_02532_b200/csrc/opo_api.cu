@@ -116,6 +116,7 @@ struct opo_handle {
     void* eom[3] = {nullptr, nullptr, nullptr};       // [N] exp(i beta sin(2 pi f tau_n)) or null
     double eom_beta[3] = {0, 0, 0}, eom_f[3] = {0, 0, 0};
     double beta3[3] = {0, 0, 0};                      // third-order dispersion [s^3/m] (opo_set_beta3)
+    int splitting = 0;                                // OPO_OPT_SPLITTING
     bool boundary_fft[3] = {false, false, false};
     void* phase = nullptr;
     int* flag = nullptr;
@@ -300,12 +301,16 @@ int build_tables(opo_handle* h) {
 }
 
 // phase[b][j] = exp(i dk_b j h/2), j = 0 .. 2 nz   (R4: z from the crystal entrance)
+int phase_stride(const opo_handle* h) { return (h->splitting ? 4 : 2) * h->nz + 1; }
+
+// N/2 - L - N/2 (OPO_SPLITTING_NLN): the RK4 steps have size h/2, so the table runs in steps of h/4, j = 0 .. 4 nz
 int build_phase(opo_handle* h) {
-    const int stride = 2 * h->nz + 1;
+    const int stride = phase_stride(h);
+    const double dz = h->splitting ? 0.25 * h->h : 0.5 * h->h;
     std::vector<cd> ph((size_t)h->B * stride);
     for (int b = 0; b < h->B; ++b)
         for (int j = 0; j < stride; ++j) {
-            const double a = h->dk[b] * (0.5 * h->h) * (double)j;
+            const double a = h->dk[b] * dz * (double)j;
             ph[(size_t)b * stride + j] = cd(std::cos(a), std::sin(a));
         }
     if (int rc = upload_complex(h, h->phase, ph.data(), ph.size())) return rc;
@@ -447,7 +452,7 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
             cudaMalloc(&h->mirror[x], (size_t)h->B * h->esz) != cudaSuccess)
             return bail(OPO_ERR_ALLOC, "cudaMalloc of tables failed");
     }
-    if (cudaMalloc(&h->scratch, fb) != cudaSuccess || cudaMalloc(&h->phase, (size_t)h->B * (2 * h->nz + 1) * h->esz) != cudaSuccess ||
+    if (cudaMalloc(&h->scratch, fb) != cudaSuccess || cudaMalloc(&h->phase, (size_t)h->B * (4 * h->nz + 1) * h->esz) != cudaSuccess ||
         cudaMalloc((void**)&h->flag, sizeof(int)) != cudaSuccess)
         return bail(OPO_ERR_ALLOC, "cudaMalloc of scratch failed");
     if (int rc = build_fft_tables(h)) { std::string m = h->err; return bail(rc, m); }
@@ -555,11 +560,13 @@ int stream_linear_all(opo_handle* h, TableKind kind, bool to_exit) {
     return OPO_OK;
 }
 
-int stream_rk4(opo_handle* h, int step) {
+// one RK4 step of the coupling terms; phase_index < 0: full step h of z-step `step`; otherwise a half step h/2
+// whose stage phases start at phase_index in the h/4 table (N/2 - L - N/2)
+int stream_rk4(opo_handle* h, int step, int phase_index = -1) {
     opo::Rk4Args a{};
     for (int x = 0; x < h->F; ++x) { a.A[x] = h->cur[x]; a.kappa[x] = h->kappa[x]; }
-    a.n_fields = h->F; a.batch = h->B; a.n = h->N; a.h = h->h;
-    a.phase = h->phase; a.phase_stride = 2 * h->nz + 1; a.step = step;
+    a.n_fields = h->F; a.batch = h->B; a.n = h->N; a.h = phase_index < 0 ? h->h : 0.5 * h->h;
+    a.phase = h->phase; a.phase_stride = phase_stride(h); a.step = step; a.phase_index = phase_index;
     OPO_LAUNCH(h, h->dbl ? opo::launch_rk4_f64(a, h->stream) : opo::launch_rk4_f32(a, h->stream));
     return OPO_OK;
 }
@@ -567,6 +574,17 @@ int stream_rk4(opo_handle* h, int step) {
 // nsteps z-steps from step index z0, half-steps merged:  H, N, H^2, N, ..., N, H
 int stream_steps(opo_handle* h, int z0, int nsteps, bool to_exit) {
     if (nsteps <= 0) return OPO_OK;
+    if (h->splitting) {      // N/2 - L - N/2 (Eq. 10-11), un-merged: two RK4 half-steps around one full linear step
+        for (int s = z0; s < z0 + nsteps; ++s) {
+            if (int rc = stream_rk4(h, s, 4 * s)) return rc;
+            if (int rc = stream_linear_all(h, TAB_H2, false)) return rc;
+            if (int rc = stream_rk4(h, s, 4 * s + 2)) return rc;
+        }
+        if (to_exit)
+            for (int x = 0; x < h->F; ++x)
+                OPO_CUDA(h, cudaMemcpyAsync(h->exitb[x], h->cur[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+        return OPO_OK;
+    }
     if (int rc = stream_linear_all(h, TAB_H, false)) return rc;
     for (int s = 0; s < nsteps; ++s) {
         if (int rc = stream_rk4(h, z0 + s)) return rc;
@@ -623,9 +641,9 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
         a.resonant[x] = h->fields.resonant[x] ? 1 : 0;
         a.kappa[x] = h->kappa[x];
     }
-    a.tw = h->tw; a.phase = h->phase; a.phase_stride = 2 * h->nz + 1;
+    a.tw = h->tw; a.phase = h->phase; a.phase_stride = phase_stride(h);
     a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
-    a.mode = mode; a.z0 = z0; a.steps = steps;
+    a.mode = mode; a.z0 = z0; a.steps = steps; a.nln = h->splitting;
     const int n_clusters = std::min(h->B, h->rinfo.max_clusters);
     OPO_LAUNCH(h, h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream)
                          : opo::launch_resident_f32(h->L, a, n_clusters, h->stream));
@@ -768,6 +786,7 @@ int opo_propagate(opo_handle* h, int nz) {
     if (int rc = check_async(h)) return rc;
     if (int rc = ensure_tables(h)) return rc;
     int rc;
+    if (h->large && h->splitting) return fail(h, OPO_ERR_UNSUPPORTED, "the N/2-L-N/2 ordering is not implemented in the large-N engine");
     if (h->large) rc = large_run(h, 0, h->z_steps, nz);
     else if (engine_in_use(h) == OPO_ENGINE_RESIDENT) rc = resident_run(h, 0, h->z_steps, nz);
     else rc = stream_steps(h, h->z_steps, nz, false);
@@ -786,6 +805,7 @@ int opo_roundtrips(opo_handle* h, int n) {
     // a phase modulator acts in the time domain between the boundary's spectral phase and the next pass, so the
     // boundary cannot be merged into the neighbouring half-steps: one launch per round trip then
     const bool eom = any_eom(h);
+    if (h->large && h->splitting) return fail(h, OPO_ERR_UNSUPPORTED, "the N/2-L-N/2 ordering is not implemented in the large-N engine");
     if (h->large) {
         if (!eom) return large_run(h, 1, 0, n);
         for (int m = 0; m < n; ++m) {
@@ -795,7 +815,7 @@ int opo_roundtrips(opo_handle* h, int n) {
         return OPO_OK;
     }
     if (engine_in_use(h) == OPO_ENGINE_RESIDENT) {
-        if (!eom) return resident_run(h, 1, 0, n);
+        if (!eom && !h->splitting) return resident_run(h, 1, 0, n);
         for (int m = 0; m < n; ++m)
             if (int rc = resident_run(h, 1, 0, 1)) return rc;      // the kernel applies the modulator with its last store
         return OPO_OK;
@@ -888,6 +908,12 @@ int opo_get_z_steps(const opo_handle* h, int* out) {
 
 int opo_set_option(opo_handle* h, int option, int value) {
     if (!h) return OPO_ERR_INVALID_ARG;
+    if (option == OPO_OPT_SPLITTING) {
+        if (value != OPO_SPLITTING_LNL && value != OPO_SPLITTING_NLN) return fail(h, OPO_ERR_INVALID_ARG, "unknown splitting");
+        if (h->z_steps != 0) return fail(h, OPO_ERR_STATE, "the splitting can only change at z = 0");
+        if (value != h->splitting) { h->splitting = value; h->phase_dirty = true; }
+        return OPO_OK;
+    }
     if (option != OPO_OPT_ENGINE) return fail(h, OPO_ERR_INVALID_ARG, "unknown option");
     if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING && value != OPO_ENGINE_LARGE)
         return fail(h, OPO_ERR_INVALID_ARG, "unknown engine");

@@ -34,7 +34,8 @@ struct Rk4Args {
     double h;
     const void* phase;     // [B][2 nz + 1] complex: exp(i dk_b * j * h/2)
     int phase_stride;      // 2 nz + 1
-    int step;              // z-step index s: stage phases at 2s, 2s+1, 2s+2
+    int step;              // z-step index s: stage phases at 2s, 2s+1, 2s+2 (phase_index < 0)
+    int phase_index;       // >= 0: stage phases at phase_index, +1, +2 instead (N/2 - L - N/2: steps of h/4)
 };
 
 // A[b][n] *= E[n]  (intracavity phase modulator exp(i beta sin(2 pi f tau_n)))
@@ -84,6 +85,8 @@ struct ResidentArgs {
     double h;
     int n_fields, batch, nz;   // nz = steps per pass
     int mode;              // 0 = propagate `steps` z-steps from step index z0; 1 = `steps` round trips
+    int nln;               // 1: order N/2 - L - N/2 (Eq. 10-11); phase table then has stride 4 nz + 1 (steps of h/4)
+                           //    and mode 1 takes steps = 1
     int z0;
     int steps;
 };

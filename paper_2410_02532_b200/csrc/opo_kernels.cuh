@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(256) k_rk4(Rk4Args a) {
     for (int x = 0; x < F; ++x) A[x] = reinterpret_cast<cplx<T>*>(a.A[x]);
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
         const int b = (int)(i / n);
-        const cplx<T>* p = ph + (size_t)b * a.phase_stride + 2 * a.step;
+        const cplx<T>* p = ph + (size_t)b * a.phase_stride + (a.phase_index >= 0 ? a.phase_index : 2 * a.step);
         const cplx<T> e0 = ldg(p), e1 = ldg(p + 1), e2 = ldg(p + 2);
         cplx<T> y[F];
 #pragma unroll

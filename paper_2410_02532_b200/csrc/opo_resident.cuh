@@ -25,6 +25,7 @@
 // BASELINE.json configs[4]); instances are independent, there is no inter-cluster communication.
 #pragma once
 #include <cooperative_groups.h>
+#include <type_traits>
 
 #include "opo_kernels.cuh"
 
@@ -64,10 +65,10 @@ template <class T, int L, int F> struct res_layout {
 // foreign fields are issued before the arithmetic of the current one (the link moves ~16 B/clk per
 // SM, so the exchange takes about as long as the arithmetic and has to run under it).  RANK is a
 // template parameter so that "foreign" is a compile-time property of the field index.
-template <class T, int L, int F, int NT, int RANK>
+template <class T, int L, int F, int NT, int RANK, bool NLN>
 __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, const cplx<T>* __restrict__ tw0,
                                                 const cplx<T>* __restrict__ tw0s, cplx<T> e0, cplx<T> e1, cplx<T> e2,
-                                                const T* kap, T h, uint32_t mb, uint32_t parity) {
+                                                cplx<T> e3, cplx<T> e4, int halves, T pre, T post, const T* kap, T h, uint32_t mb, uint32_t parity) {
     static_assert(plan<L>::rbits(0) == 2, "pass 0 must be radix 4");
     using RL = res_layout<T, L, F>;
     constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
@@ -127,7 +128,16 @@ __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, co
                 cplx<T> y[F];
 #pragma unroll
                 for (int x = 0; x < F; ++x) y[x] = v[x][j];
+                if constexpr (NLN) {      // a pass-0 pair with no table between (first / last half-step) carries its own 1/4
+#pragma unroll
+                    for (int x = 0; x < F; ++x) y[x] = {y[x].re * pre, y[x].im * pre};
+                }
                 Rk4<T, F>::step(y, e0, e1, e2, kap, h);
+                if constexpr (NLN) {      // N/2 - L - N/2: two half-steps meet between two linear operators
+                    if (halves == 2) Rk4<T, F>::step(y, e2, e3, e4, kap, h);
+#pragma unroll
+                    for (int x = 0; x < F; ++x) y[x] = {y[x].re * post, y[x].im * post};
+                }
 #pragma unroll
                 for (int x = 0; x < F; ++x) v[x][j] = y[x];
             }
@@ -155,7 +165,8 @@ __device__ __noinline__ void pass0_local(const cplx<T>* tw, int tid, bool invers
     else fwd_pass_smem<T, L, 0, NT, false>(sm, tw, tid);
 }
 
-template <class T, int L, int F>
+// NLN: the N/2 - L - N/2 ordering is a separate instantiation, so that the default kernel carries none of its code
+template <class T, int L, int F, bool NLN = false>
 __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(ResidentArgs a) {
     constexpr int N = 1 << L, NT = cta_threads<T, L>::value;
     using PL = plan<L>;
@@ -241,6 +252,45 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
         pass0_local<T, L, NT>(tw, tid, false);
         __syncthreads();
 
+        if constexpr (NLN) {
+            // inverse pass 0 -> RK4 -> forward pass 0 over the cluster, with the synchronisation around it
+            auto run_fused = [&](cplx<T> e0, cplx<T> e1, cplx<T> e2, cplx<T> e3, cplx<T> e4, int halves, T hstep, T pre, T post) {
+                if constexpr (!FLOW) { cluster_arrive(); cluster_wait(); }      // every field is ready for its inverse pass 0
+                if (x == 0) fused_pass0_rk4<T, L, F, NT, 0, true>(fld, tid, tw, tw0s, e0, e1, e2, e3, e4, halves, pre, post, kap, hstep, mb, fz & 1);
+                else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1, true>(fld, tid, tw, tw0s, e0, e1, e2, e3, e4, halves, pre, post, kap, hstep, mb, fz & 1);
+                else fused_pass0_rk4<T, L, F, NT, F - 1, true>(fld, tid, tw, tw0s, e0, e1, e2, e3, e4, halves, pre, post, kap, hstep, mb, fz & 1);
+                ++fz;
+                if constexpr (!FLOW) { cluster_arrive(); cluster_wait(); }      // every result has landed in its owner's shared memory
+            };
+            // the paper's own order N/2 - L - N/2 (Eq. 10-11), adjacent half-steps NOT merged into one
+            // RK4 step (they are two RK4 steps of h/2): [N/2] (L [N/2 N/2])^(n-1) L [N/2], every L a full step (table H2).
+            // The tables carry the 1/N of one forward + inverse transform; the first and the last half-step sit between a
+            // forward and an inverse pass 0 with no table, hence their own exact factor 1/4.
+            // phase table: exp(i dk j h/4).  One pass per launch (the host loops over round trips).
+            const int zs = rt_mode ? 0 : a.z0, nsteps = rt_mode ? nz : a.steps;
+            const T hh = (T)0.5 * h;
+            if constexpr (FLOW) flow_arrive_ready_all();
+            {
+                const cplx<T>* p = ph + 4 * zs;
+                run_fused(ldg(p), ldg(p + 1), ldg(p + 2), ldg(p + 2), ldg(p + 2), 1, hh, (T)0.25, (T)1);
+            }
+#pragma unroll 1
+            for (int q = 0; q < nsteps; ++q) {
+                if constexpr (FLOW) {
+                    FlowArgs fa;
+                    fa.mb = mb; fa.nf = F;
+                    fa.wait_in = 1; fa.par_done = (fz - 1) & 1;
+                    fa.arrive_out = 1;
+                    linear_core_smem<T, L, NT, true>(tabH2, tid, fa);
+                } else {
+                    linear_core_smem<T, L, NT>(tabH2, tid);
+                }
+                const cplx<T>* p = ph + 4 * (zs + q) + 2;
+                if (q + 1 < nsteps) run_fused(ldg(p), ldg(p + 1), ldg(p + 2), ldg(p + 3), ldg(p + 4), 2, hh, (T)1, (T)1);
+                else run_fused(ldg(p), ldg(p + 1), ldg(p + 2), ldg(p + 2), ldg(p + 2), 1, hh, (T)1, (T)0.25);
+            }
+            if constexpr (FLOW) flow_wait_done_all((fz - 1) & 1);     // the last half-step has landed in my field
+        } else {
         // q counts linear operators: q = 0 first half-step, q = total last half-step, between them the
         // merged full steps; in round-trip mode q = m nz + s and s = 0 (m > 0) crosses the boundary
 #pragma unroll 1
@@ -273,15 +323,16 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(Reside
             if constexpr (!FLOW) cluster_arrive();   // my field is ready for its inverse pass 0
             const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
             if constexpr (!FLOW) cluster_wait();     // ... and so is every other field
-            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
-            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
-            else fused_pass0_rk4<T, L, F, NT, F - 1>(fld, tid, tw, tw0s, e0, e1, e2, kap, h, mb, fz & 1);
+            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0, false>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
+            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1, false>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
+            else fused_pass0_rk4<T, L, F, NT, F - 1, false>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
             ++fz;
             if constexpr (!FLOW) {
                 cluster_arrive();
                 cluster_wait();     // every result has landed in its owner's shared memory
             }
         }
+        }   // L/2 - N - L/2
         __syncthreads();
         pass0_local<T, L, NT>(tw, tid, true);
         __syncthreads();
@@ -331,7 +382,9 @@ template <class T, int L, int F> cudaError_t resident_cfg(cudaLaunchConfig_t* cf
     const size_t smem = res_layout<T, L, F>::total;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_resident<T, L, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_resident<T, L, F, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_resident<T, L, F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -371,7 +424,7 @@ template <class T, int L, int F> cudaError_t launch_resident_LF(const ResidentAr
     cudaLaunchAttribute attr[1];
     cudaError_t e = resident_cfg<T, L, F>(&cfg, attr, n_clusters, s);
     if (e != cudaSuccess) return e;
-    return cudaLaunchKernelEx(&cfg, k_resident<T, L, F>, a);
+    return a.nln ? cudaLaunchKernelEx(&cfg, k_resident<T, L, F, true>, a) : cudaLaunchKernelEx(&cfg, k_resident<T, L, F, false>, a);
 }
 
 template <class T, int L> cudaError_t launch_resident_L(const ResidentArgs& a, int n_clusters, cudaStream_t s) {

@@ -112,6 +112,7 @@ def _engine_or_skip(w, engine):
 
 def assert_close(got, ref, tol, what):
     worst = 0.0
+    assert np.isfinite(got).all(), f"{what}: non-finite values in the CUDA result"
     for b in range(ref.shape[0]):
         for x in range(ref.shape[1]):
             if np.linalg.norm(ref[b, x]) == 0.0:
@@ -565,6 +566,58 @@ def test_third_order_dispersion_large_engine():
     rcur, rex = run_oracle(w, n_roundtrips=2)
     assert_close(cur, rcur, 1e-4, "TOD large current")
     assert_close(ex, rex, 1e-4, "TOD large exit")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the paper's own operator order N/2 - L - N/2 (Eq. 10-11)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("engine_idx", [0, 1])
+@pytest.mark.parametrize("precision,log2_n,n_fields", [("c64", 12, 3), ("c128", 10, 2), ("c64", 14, 3), ("c64", 8, 2), ("c128", 13, 3)])
+def test_nln_ordering_matches_oracle(precision, log2_n, n_fields, engine_idx):
+    """Partial passes (2 + 3 z-steps), then full round trips with the boundary (spectral phase, mirror, modulator),
+    all in the N/2 - L - N/2 order, against the oracle in the same order; the result must differ from the L/2 - N - L/2
+    result by more than the tolerance (else the switch would not be tested)."""
+    engine = engines()[engine_idx]
+    w = _with_eom(small_workload(log2_n, n_fields, precision, nz=5, batch=2, dk=23.0, gdd_dt2=0.6, drad=0.3))
+    w.splitting = 1
+    _engine_or_skip(w, engine)
+    cur, _, _ = run_gpu(w, engine, propagate=[2, 3])
+    rcur, _ = run_oracle(w, propagate=[2, 3])
+    e0 = assert_close(cur, rcur, TOL[precision], "NLN propagate")
+    cur, ex, _ = run_gpu(w, engine, n_roundtrips=3, calls=2)
+    rcur, rex = run_oracle(w, n_roundtrips=3)
+    e1 = assert_close(cur, rcur, TOL[precision], "NLN current")
+    e2 = assert_close(ex, rex, TOL[precision], "NLN exit")
+    w.splitting = 0
+    c0, _ = run_oracle(w, n_roundtrips=3)
+    assert rel_l2(c0[0, 1], rcur[0, 1]) > 20 * TOL[precision]
+    print(f"NLN {precision} 2^{log2_n} F={n_fields} engine {engine}: rel L2 propagate {e0:.3e} current {e1:.3e} exit {e2:.3e}")
+
+
+def test_nln_ordering_config1_and_large_engine_refusal():
+    torch, P = _gpu()
+    w = W.config1().truncated(3)
+    w.splitting = 1
+    cur, ex, eng = run_gpu(w, P.ENGINE_AUTO)
+    assert eng == P.ENGINE_RESIDENT
+    rcur, rex = run_oracle(w)
+    e1 = assert_close(cur, rcur, 1e-4, "C1 NLN current")
+    e2 = assert_close(ex, rex, 1e-4, "C1 NLN exit")
+    print(f"C1 in the N/2-L-N/2 order, 3 RT: rel L2 current {e1:.3e} exit {e2:.3e}")
+    wl = small_workload(15, 2, "c64", nz=4, batch=1)
+    wl.splitting = 1
+    o = P.from_workload(wl)
+    with pytest.raises(P.OpoError) as ei:
+        o.roundtrips(1)
+    assert ei.value.status == P.ERR_UNSUPPORTED
+    o.close()
+    # the splitting can only change at z = 0
+    o = P.from_workload(W.config0())
+    o.propagate(1)
+    with pytest.raises(P.OpoError) as ei:
+        P.opo_set_option(o._h, P.OPT_SPLITTING, P.SPLITTING_NLN)
+    assert ei.value.status == P.ERR_STATE
+    o.close()
 
 
 def test_abi_errors_and_state():
