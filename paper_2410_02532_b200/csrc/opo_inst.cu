@@ -15,11 +15,20 @@ namespace opo {
 #define OPO_CAT3(a, b, c) OPO_CAT3_(a, b, c)
 #define OPO_NAME(base) OPO_CAT3(base, OPO_SUFFIX, OPO_L)
 
+#ifndef OPO_NLN
 cudaError_t OPO_NAME(launch_linear_)(const LinArgs& a, cudaStream_t s) { return launch_linear_L<OPO_T, OPO_L>(a, s); }
 cudaError_t OPO_NAME(launch_freq_)(const FreqArgs& a, cudaStream_t s) { return launch_freq_L<OPO_T, OPO_L>(a, s); }
 cudaError_t OPO_NAME(resident_info_)(int n_fields, ResidentInfo* out) { return resident_info_L<OPO_T, OPO_L>(n_fields, out); }
-cudaError_t OPO_NAME(launch_resident_)(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
-    return launch_resident_L<OPO_T, OPO_L>(a, n_clusters, s);
+#endif
+#ifdef OPO_NLN
+// the N/2 - L - N/2 instantiation of the resident kernel only (build.py compiles this file a second time with -DOPO_NLN)
+cudaError_t OPO_NAME(launch_resident_nln_)(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    return launch_resident_L<OPO_T, OPO_L, true>(a, n_clusters, s);
 }
+#else
+cudaError_t OPO_NAME(launch_resident_)(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    return launch_resident_L<OPO_T, OPO_L, false>(a, n_clusters, s);
+}
+#endif
 
 }  // namespace opo

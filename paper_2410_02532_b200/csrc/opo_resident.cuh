@@ -384,8 +384,6 @@ template <class T, int L, int F> cudaError_t resident_cfg(cudaLaunchConfig_t* cf
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(k_resident<T, L, F, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_resident<T, L, F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
         configured = true;
     }
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -419,16 +417,26 @@ template <class T, int L> cudaError_t resident_info_L(int n_fields, ResidentInfo
     return n_fields == 3 ? resident_info_LF<T, L, 3>(out) : resident_info_LF<T, L, 2>(out);
 }
 
-template <class T, int L, int F> cudaError_t launch_resident_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+// NLN = true is instantiated in its own translation units (opo_inst_nln.cu): the default kernel's object code stays
+// byte for byte what it is without the N/2 - L - N/2 ordering
+template <class T, int L, int F, bool NLN> cudaError_t launch_resident_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
     cudaLaunchConfig_t cfg{};
     cudaLaunchAttribute attr[1];
     cudaError_t e = resident_cfg<T, L, F>(&cfg, attr, n_clusters, s);
     if (e != cudaSuccess) return e;
-    return a.nln ? cudaLaunchKernelEx(&cfg, k_resident<T, L, F, true>, a) : cudaLaunchKernelEx(&cfg, k_resident<T, L, F, false>, a);
+    if constexpr (NLN) {
+        static bool configured = false;
+        if (!configured) {
+            e = cudaFuncSetAttribute(k_resident<T, L, F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.dynamicSmemBytes);
+            if (e != cudaSuccess) return e;
+            configured = true;
+        }
+    }
+    return cudaLaunchKernelEx(&cfg, k_resident<T, L, F, NLN>, a);
 }
 
-template <class T, int L> cudaError_t launch_resident_L(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
-    return a.n_fields == 3 ? launch_resident_LF<T, L, 3>(a, n_clusters, s) : launch_resident_LF<T, L, 2>(a, n_clusters, s);
+template <class T, int L, bool NLN> cudaError_t launch_resident_L(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    return a.n_fields == 3 ? launch_resident_LF<T, L, 3, NLN>(a, n_clusters, s) : launch_resident_LF<T, L, 2, NLN>(a, n_clusters, s);
 }
 
 }  // namespace opo
