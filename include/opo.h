@@ -194,8 +194,8 @@ int opo_get_z_steps(const opo_handle* h, int* out_steps);
 /* Operator splitting of a z-step.  LNL (default, BASELINE.json north_star): linear half-step,
  * one RK4 step h, linear half-step.  NLN: the order the paper implements, Eq. 10-11: one RK4 step of h/2, the full
  * linear step, one RK4 step of h/2 (stage abscissae z, z+h/4, z+h/2 and z+h/2, z+3h/4, z+h).  Both are second
- * order and differ by O(h^2).  Can change at z = 0 only.  Resident and streaming engines; OPO_ERR_UNSUPPORTED at
- * propagate / roundtrips on the large-N engine.  With NLN the resident engine runs one launch per round trip. */
+ * order and differ by O(h^2).  Can change at z = 0 only.  With NLN the resident and large-N engines run one launch
+ * per round trip. */
 #define OPO_OPT_SPLITTING 1
 #define OPO_SPLITTING_LNL 0
 #define OPO_SPLITTING_NLN 1

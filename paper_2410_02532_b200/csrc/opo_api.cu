@@ -660,7 +660,7 @@ void large_common(const opo_handle* h, opo::LargeArgs& a) {
         a.kappa[x] = h->kappa[x];
     }
     a.tw1 = h->tw; a.tw2 = h->tw2; a.wlo = h->wlo; a.whi = h->whi; a.perm1 = h->perm; a.perm2 = h->perm2;
-    a.phase = h->phase; a.phase_stride = 2 * h->nz + 1;
+    a.phase = h->phase; a.phase_stride = phase_stride(h); a.nln = h->splitting;
     a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
     a.field_mask = (1 << h->F) - 1;
     a.barrier = h->barrier; a.barrier_base = 0;
@@ -696,7 +696,7 @@ int large_run(opo_handle* h, int mode, int z0, int steps) {
     if (fft_mask) {
         opo::LargeArgs g{};
         large_common(h, g);
-        g.mode = 0; g.z0 = 0; g.steps = 0; g.field_mask = fft_mask;
+        g.mode = 0; g.z0 = 0; g.steps = 0; g.field_mask = fft_mask; g.nln = 0;     // one linear operator, whatever the splitting
         for (int x = 0; x < h->F; ++x) {
             g.tabH[x] = h->tabGM[x];
             g.tabH_stride[x] = h->per_inst_boundary[x] ? h->N : 0;
@@ -786,7 +786,6 @@ int opo_propagate(opo_handle* h, int nz) {
     if (int rc = check_async(h)) return rc;
     if (int rc = ensure_tables(h)) return rc;
     int rc;
-    if (h->large && h->splitting) return fail(h, OPO_ERR_UNSUPPORTED, "the N/2-L-N/2 ordering is not implemented in the large-N engine");
     if (h->large) rc = large_run(h, 0, h->z_steps, nz);
     else if (engine_in_use(h) == OPO_ENGINE_RESIDENT) rc = resident_run(h, 0, h->z_steps, nz);
     else rc = stream_steps(h, h->z_steps, nz, false);
@@ -805,9 +804,8 @@ int opo_roundtrips(opo_handle* h, int n) {
     // a phase modulator acts in the time domain between the boundary's spectral phase and the next pass, so the
     // boundary cannot be merged into the neighbouring half-steps: one launch per round trip then
     const bool eom = any_eom(h);
-    if (h->large && h->splitting) return fail(h, OPO_ERR_UNSUPPORTED, "the N/2-L-N/2 ordering is not implemented in the large-N engine");
     if (h->large) {
-        if (!eom) return large_run(h, 1, 0, n);
+        if (!eom && !h->splitting) return large_run(h, 1, 0, n);
         for (int m = 0; m < n; ++m) {
             if (int rc = large_run(h, 1, 0, 1)) return rc;
             if (int rc = apply_eom(h)) return rc;

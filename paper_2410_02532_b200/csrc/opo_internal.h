@@ -126,6 +126,7 @@ struct LargeArgs {
                                // 1 = `steps` round trips; 2 = forward DFT read-out
     int z0;
     int steps;
+    int nln;                   // 1: order N/2 - L - N/2; phase table in steps of h/4; mode 1 takes steps = 1
     unsigned long long* barrier;        // zeroed by the host before the launch
     unsigned long long barrier_base;    // counter value at launch (0)
 };

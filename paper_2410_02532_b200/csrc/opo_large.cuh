@@ -81,7 +81,8 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 // inverse pass 0 -> RK4 -> forward pass 0 for butterfly t of all F fields held in local shared memory
 template <class T, int L, int F>
 __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, const cplx<T>* __restrict__ tw0s,
-                                                cplx<T> e0, cplx<T> e1, cplx<T> e2, const T* kap, T h) {
+                                                cplx<T> e0, cplx<T> e1, cplx<T> e2, const T* kap, T h,
+                                                bool two = false, cplx<T> e3 = cplx<T>{}, cplx<T> e4 = cplx<T>{}) {
     constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
     cplx<T> w[R - 1];
 #pragma unroll
@@ -104,6 +105,7 @@ __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, cons
 #pragma unroll
         for (int x = 0; x < F; ++x) y[x] = v[x][j];
         Rk4<T, F>::step(y, e0, e1, e2, kap, h);
+        if (two) Rk4<T, F>::step(y, e2, e3, e4, kap, h);      // N/2 - L - N/2: two half-steps meet here
 #pragma unroll
         for (int x = 0; x < F; ++x) v[x][j] = y[x];
     }
@@ -119,7 +121,9 @@ __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, cons
         for (int k = 0; k < R; ++k) fld[x][p0 + elem_off<T, RB, SB>(k)] = v[x][k];
 }
 
-enum { COL_FWD = 0, COL_RK4 = 1, COL_INV = 2 };
+// COL_NFWD / COL_INVN (N/2 - L - N/2 ordering): an RK4 half-step in the time domain before the forward / after the
+// inverse column transform; COL_RK4 then takes two half-steps
+enum { COL_FWD = 0, COL_RK4 = 1, COL_INV = 2, COL_NFWD = 3, COL_INVN = 4 };
 enum { ROW_LINEAR = 0, ROW_RELOAD = 1, ROW_FREQ = 2 };
 
 template <class T, int L, int F> struct LargeEngine {
@@ -144,7 +148,7 @@ template <class T, int L, int F> struct LargeEngine {
     // src/dst: per-field base pointers ([B][N]); fields outside `mask` are neither read nor written.
     template <int MODE>
     __device__ __forceinline__ void col_pass(cplx<T>* const* src, cplx<T>* const* dst, int mask, int batch,
-                                             const cplx<T>* phase, int phase_stride, int s, const T* kap, T h) {
+                                             const cplx<T>* phase, int phase_stride, int pidx, const T* kap, T h, bool two = false) {
         const int n_tiles = batch * C::TILES_PER_INST;
         const int team = tid / C::TT1, lt = tid % C::TT1;
         cplx<T>* smt = sm + team * C::CSTRIDE;
@@ -161,15 +165,34 @@ template <class T, int L, int F> struct LargeEngine {
                     sm[(x * C::TC + c) * C::CSTRIDE + phys<T>(n1)] = ldcg(g + (size_t)n1 * C::N2 + c);
                 }
             }
-            if constexpr (MODE != COL_FWD) {
+            // pointwise RK4 half-step on the tile in the time domain (Eq. 10-11)
+            auto rk4_tile = [&]() {
+                __syncthreads();
+                const cplx<T>* ph = phase + (size_t)b * phase_stride + pidx;
+                const cplx<T> e0 = ldg(ph), e1 = ldg(ph + 1), e2 = ldg(ph + 2);
+#pragma unroll 1
+                for (int it = tid; it < C::TC * C::N1; it += C::NT) {
+                    const int c = it / C::N1, n1 = it % C::N1;
+                    cplx<T> y[F];
+#pragma unroll
+                    for (int x = 0; x < F; ++x) y[x] = sm[(x * C::TC + c) * C::CSTRIDE + phys<T>(n1)];
+                    Rk4<T, F>::step(y, e0, e1, e2, kap, h);
+#pragma unroll
+                    for (int x = 0; x < F; ++x) sm[(x * C::TC + c) * C::CSTRIDE + phys<T>(n1)] = y[x];
+                }
+            };
+            if constexpr (MODE == COL_NFWD) rk4_tile();
+            if constexpr (MODE != COL_FWD && MODE != COL_NFWD) {
                 __syncthreads();
                 inv_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
-                inv_passes<T, C::L1, C::TT1, true, (MODE == COL_INV ? 0 : 1)>(smt, tw1, lt);
+                inv_passes<T, C::L1, C::TT1, true, ((MODE == COL_INV || MODE == COL_INVN) ? 0 : 1)>(smt, tw1, lt);
             }
+            if constexpr (MODE == COL_INVN) rk4_tile();
             if constexpr (MODE == COL_RK4) {
                 __syncthreads();
-                const cplx<T>* ph = phase + (size_t)b * phase_stride + 2 * s;
+                const cplx<T>* ph = phase + (size_t)b * phase_stride + pidx;
                 const cplx<T> e0 = ldg(ph), e1 = ldg(ph + 1), e2 = ldg(ph + 2);
+                const cplx<T> e3 = two ? ldg(ph + 3) : e2, e4 = two ? ldg(ph + 4) : e2;
                 constexpr int S = C::N1 / 4;
 #pragma unroll 1
                 for (int it = tid; it < C::TC * S; it += C::NT) {
@@ -177,12 +200,12 @@ template <class T, int L, int F> struct LargeEngine {
                     cplx<T>* fld[F];
 #pragma unroll
                     for (int x = 0; x < F; ++x) fld[x] = sm + (x * C::TC + c) * C::CSTRIDE;
-                    pass0_rk4_local<T, C::L1, F>(fld, t, tw1 + P1::tw_offset(0), e0, e1, e2, kap, h);
+                    pass0_rk4_local<T, C::L1, F>(fld, t, tw1 + P1::tw_offset(0), e0, e1, e2, kap, h, two, e3, e4);
                 }
             }
-            if constexpr (MODE != COL_INV) {
+            if constexpr (MODE != COL_INV && MODE != COL_INVN) {
                 __syncthreads();
-                fwd_passes<T, C::L1, C::TT1, true, (MODE == COL_FWD ? 0 : 1)>(smt, tw1, lt);
+                fwd_passes<T, C::L1, C::TT1, true, ((MODE == COL_FWD || MODE == COL_NFWD) ? 0 : 1)>(smt, tw1, lt);
                 fwd_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
             }
             __syncthreads();
@@ -330,6 +353,32 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
     const bool rt_mode = a.mode == 1;
     const int total = rt_mode ? a.steps * nz : a.steps;
 
+    if (a.nln) {
+        // N/2 - L - N/2 (Eq. 10-11): [N/2] (L [N/2 N/2])^(n-1) L [N/2]; every L a full step (table H2),
+        // every RK4 step of size h/2, phase table in steps of h/4; one pass per launch (mode 1: steps = 1)
+        const int zs = rt_mode ? 0 : a.z0, nsteps = rt_mode ? nz : a.steps;
+        const T hh = (T)0.5 * h;
+        e.template col_pass<COL_NFWD>(cur, cur, mask, batch, phase, a.phase_stride, 4 * zs, kap, hh);
+        grid_barrier(a.barrier, target);
+#pragma unroll
+        for (int x = 0; x < F; ++x) {
+            op.sh_store[x] = nullptr; op.aux[x] = nullptr; op.out[x] = nullptr; op.tab_stride[x] = 0;
+            op.kind[x] = ((mask >> x) & 1) ? ROW_LINEAR : -1;
+            op.tab[x] = reinterpret_cast<const TAB*>(a.tabH2[x]);
+        }
+#pragma unroll 1
+        for (int q = 0; q < nsteps; ++q) {
+            e.row_pass(cur, op, batch, a.perm1, a.perm2);
+            grid_barrier(a.barrier, target);
+            if (q + 1 < nsteps) {
+                e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 4 * (zs + q) + 2, kap, hh, true);
+                grid_barrier(a.barrier, target);
+            }
+        }
+        e.template col_pass<COL_INVN>(cur, cur, mask, batch, phase, a.phase_stride, 4 * (zs + nsteps - 1) + 2, kap, hh);
+        return;
+    }
+
     e.template col_pass<COL_FWD>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
     grid_barrier(a.barrier, target);
 #pragma unroll 1
@@ -359,7 +408,7 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
         e.row_pass(cur, op, batch, a.perm1, a.perm2);
         grid_barrier(a.barrier, target);
         if (q == total) break;
-        e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, s, kap, h);
+        e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 2 * s, kap, h);
         grid_barrier(a.barrier, target);
     }
     e.template col_pass<COL_INV>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);

@@ -594,7 +594,7 @@ def test_nln_ordering_matches_oracle(precision, log2_n, n_fields, engine_idx):
     print(f"NLN {precision} 2^{log2_n} F={n_fields} engine {engine}: rel L2 propagate {e0:.3e} current {e1:.3e} exit {e2:.3e}")
 
 
-def test_nln_ordering_config1_and_large_engine_refusal():
+def test_nln_ordering_config1_and_large_engine():
     torch, P = _gpu()
     w = W.config1().truncated(3)
     w.splitting = 1
@@ -604,13 +604,18 @@ def test_nln_ordering_config1_and_large_engine_refusal():
     e1 = assert_close(cur, rcur, 1e-4, "C1 NLN current")
     e2 = assert_close(ex, rex, 1e-4, "C1 NLN exit")
     print(f"C1 in the N/2-L-N/2 order, 3 RT: rel L2 current {e1:.3e} exit {e2:.3e}")
-    wl = small_workload(15, 2, "c64", nz=4, batch=1)
+    # large-N engine in the same order, with the boundary transform and the modulator
+    wl = _with_eom(small_workload(15, 2, "c64", nz=4, batch=1, dk=9.0, gdd_dt2=0.6, drad=0.3))
     wl.splitting = 1
-    o = P.from_workload(wl)
-    with pytest.raises(P.OpoError) as ei:
-        o.roundtrips(1)
-    assert ei.value.status == P.ERR_UNSUPPORTED
-    o.close()
+    cur, _, eng = run_gpu(wl, P.ENGINE_AUTO, propagate=[1, 3])
+    assert eng == P.ENGINE_LARGE
+    rcur, _ = run_oracle(wl, propagate=[1, 3])
+    e0 = assert_close(cur, rcur, 1e-4, "large NLN propagate")
+    cur, ex, _ = run_gpu(wl, P.ENGINE_AUTO, n_roundtrips=2)
+    rcur, rex = run_oracle(wl, n_roundtrips=2)
+    e1 = assert_close(cur, rcur, 1e-4, "large NLN current")
+    e2 = assert_close(ex, rex, 1e-4, "large NLN exit")
+    print(f"large-N engine in the N/2-L-N/2 order: rel L2 propagate {e0:.3e} current {e1:.3e} exit {e2:.3e}")
     # the splitting can only change at z = 0
     o = P.from_workload(W.config0())
     o.propagate(1)
