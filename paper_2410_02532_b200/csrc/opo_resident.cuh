@@ -58,6 +58,9 @@ template <class T, int L, int F> struct res_layout {
     static constexpr size_t total = flow ? mbar_offset + 16 * (size_t)(FC::NCLS > 0 ? FC::NCLS : 1) : data_end;
     static constexpr int done_count = flow ? F * FC::NW / FC::NCLS : 0;
     static constexpr int ready_count = FC::G * F;
+    // two clusters' CTAs share an SM when shared memory (plus 1 KB of system reservation each) and registers allow it:
+    // the exchange of one instance then runs under the arithmetic of another
+    static constexpr int ctas_per_sm = (2 * (total + 1024) <= 233472 && 2 * NT * 128 <= 65536) ? 2 : 1;
 };
 
 // inverse pass 0 -> RK4 -> forward pass 0 on this CTA's share of the radix-4 butterflies.
@@ -167,7 +170,7 @@ __device__ __noinline__ void pass0_local(const cplx<T>* tw, int tid, bool invers
 
 // NLN: the N/2 - L - N/2 ordering is a separate instantiation, so that the default kernel carries none of its code
 template <class T, int L, int F, bool NLN = false>
-__global__ void __launch_bounds__(cta_threads<T, L>::value, 1) k_resident(ResidentArgs a) {
+__global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>::ctas_per_sm) k_resident(ResidentArgs a) {
     constexpr int N = 1 << L, NT = cta_threads<T, L>::value;
     using PL = plan<L>;
     using SL = smem_layout<T, L>;
