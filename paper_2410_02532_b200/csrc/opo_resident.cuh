@@ -13,9 +13,15 @@
 //            needs all F fields at those four grid points.  The butterflies t are dealt to the F
 //            CTAs in tiles of 32; a CTA reads its own field locally and the foreign fields through
 //            distributed shared memory, transforms, integrates, transforms back and writes all F
-//            fields back.  The DSMEM traffic (2/3 of the state in each direction) overlaps the
-//            butterfly and RK4 arithmetic of the same phase.
-//   one cluster barrier before and after the fused phase.
+//            fields back.  The loop over a warp's tiles is software-pipelined: the DSMEM loads of the
+//            next tile are in flight under the arithmetic of the current one (the SM-to-SM link moves
+//            ~16 B/clk per SM, measured; 2/3 of the state crosses it in each direction per z-step).
+//   sync   : N >= 2^12: class-granular mbarriers (flow_cfg in opo_fft.cuh), no cluster-wide barrier;
+//            smaller N: one cluster barrier before and one after the fused phase.
+//
+// Variants: the paper's order N/2 - L - N/2 (Eq. 10-11) is the instantiation NLN = true (two RK4
+// half-steps in the fused phase, one pass per launch); the intracavity phase modulator (L149-154)
+// rides on the last store of a call.
 //
 // Merged tables: H.H = H2 between RK4 steps; H . G m . H = HB across the cavity boundary for a
 // resonant field; a non-resonant field restarts every round trip
@@ -25,7 +31,6 @@
 // BASELINE.json configs[4]); instances are independent, there is no inter-cluster communication.
 #pragma once
 #include <cooperative_groups.h>
-#include <type_traits>
 
 #include "opo_kernels.cuh"
 
