@@ -1,13 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the SSFM/OPO hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4|C1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C0..C4] [--eom]
 
 One "step" = the whole hot path over one batch: `rt_per_step` cavity round trips (each = nz z-steps
 of FFT . dispersion . IFFT + RK4, then the boundary operator) of every instance of the workload.
 Default workload: BASELINE.json configs[4] (256 independent N = 2^14 three-wave OPOs, 100 z-steps,
 300 round trips -- the batched N = 2^14 case the roofline target is quoted on); `--workload C1` runs
-configs[1] (the same OPO, a single instance: latency-bound, 3 of 148 SMs).
+configs[1] (the same OPO, a single instance: latency-bound, 3 of 148 SMs), C0 / C2 / C3 the other configs
+(C3: N = 2^18 on the large-N engine, roofline against the HBM peak).
 
 Prints ONE JSON line (rank 0).  `value` = grid-point z-steps/s with inputs resident in HBM;
 `e2e` = the same through the host-buffer ABI calls (H2D of pump and seeds, D2H of the exit signal
