@@ -183,7 +183,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--rt-per-step", type=int, default=0, help="round trips per step (default: the config's full length for C4 and C0, 100 for C1, 20 for C2, 2 for C3)")
-    ap.add_argument("--engine", default="auto", choices=["auto", "resident", "streaming"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "resident", "streaming", "cufft"],
+                    help="cufft = the internal cuFFT + elementwise-kernel baseline (north_star item (d)), not the product")
     ap.add_argument("--eom", action="store_true",
                     help="intracavity phase modulator on the signal (PAPER.md:L149-154; beta = 1 rad, f = 3 / window): the "
                          "paper's 'EOM' cavity configuration; the boundary is then not merged (one launch per round trip)")
@@ -220,7 +221,7 @@ def main():
         w.eom_beta_rad = [0.0, 1.0, 0.0]
         w.eom_f_hz = [0.0, 3.0 / w.window_s, 0.0]
     rt_per_step = args.rt_per_step or {"C0": w.n_roundtrips, "C1": 100, "C2": 20, "C3": 2, "C4": w.n_roundtrips}[args.workload]
-    engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "streaming": P.ENGINE_STREAMING}[args.engine]
+    engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "streaming": P.ENGINE_STREAMING, "cufft": P.ENGINE_CUFFT}[args.engine]
     o = P.from_workload(w, engine=engine)
     units_per_step = w.batch * w.n * w.nz_per_pass * rt_per_step          # grid-point z-steps, this rank
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
@@ -296,7 +297,7 @@ def main():
     # ---- roofline of the dominant kernel ----------------------------------------------------
     avg_s = statistics.mean(per_step_ms) * 1e-3
     eng = o.engine
-    eng_name = {P.ENGINE_RESIDENT: "resident", P.ENGINE_STREAMING: "streaming", P.ENGINE_LARGE: "large"}.get(eng, str(eng))
+    eng_name = {P.ENGINE_RESIDENT: "resident", P.ENGINE_STREAMING: "streaming", P.ENGINE_LARGE: "large", P.ENGINE_CUFFT: "cufft"}.get(eng, str(eng))
     traffic = ncu_traffic_bytes(args.workload, eng_name, rt_per_step)
     if eng == P.ENGINE_RESIDENT:
         # fields stay in shared memory: bound by FP32 instruction issue
@@ -313,12 +314,13 @@ def main():
         # fields stream through L2 / HBM: algorithmic bytes per field-point z-step: large engine 32 B
         # (row pass R+W, column pass R+W), streaming engine 40 B (linear R+W + table, RK4 R+W)
         esz = 16 if w.precision == "c128" else 8
-        per_fp = (4 * esz) if eng == P.ENGINE_LARGE else (5 * esz)
+        # cuFFT baseline: FFT R+W, multiply R+W + table, inverse FFT R+W, RK4 R+W = 9 complex per field-point z-step
+        per_fp = (4 * esz) if eng == P.ENGINE_LARGE else ((9 * esz) if eng == P.ENGINE_CUFFT else (5 * esz))
         by = per_fp * w.n_fields * units_per_step
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
         peak = float(peaks.get("hbm_gbs", 6543.1))
         n_launch = max(1, int(launches) // max(1, args.steps))
-        roofline = {"bound": "hbm", "kernel": "k_large" if eng == P.ENGINE_LARGE else "k_linear+k_rk4", "achieved": by / avg_s / 1e9,
+        roofline = {"bound": "hbm", "kernel": "k_large" if eng == P.ENGINE_LARGE else ("cufft+k_multab+k_rk4" if eng == P.ENGINE_CUFFT else "k_linear+k_rk4"), "achieved": by / avg_s / 1e9,
                     "peak": peak, "unit": "GB/s", "frac": by / avg_s / 1e9 / peak, "traffic": traffic,
                     "note": f"algorithmic bytes = {per_fp} B per field-point z-step; peak = measured HBM copy bandwidth "
                             f"({'MEASURED_PEAKS.json' if peaks else 'B200_PROFILING.md fallback'}); {n_launch} launch(es) per step; "

@@ -190,6 +190,10 @@ int opo_get_z_steps(const opo_handle* h, int* out_steps);
 #define OPO_ENGINE_RESIDENT 1
 #define OPO_ENGINE_STREAMING 2
 #define OPO_ENGINE_LARGE 3
+/* Internal baseline, not the product (BASELINE.json north_star item (d)): cuFFT C2C over the batch + separate
+ * elementwise kernels (table multiply, RK4, mirror), the structure of the paper's own program (PAPER.md:L248,
+ * L286-287).  Never chosen by AUTO; libcufft is loaded on request.  Sizes of the streaming engine. */
+#define OPO_ENGINE_CUFFT 4
 #define OPO_OPT_ENGINE 0
 /* Operator splitting of a z-step.  LNL (default, BASELINE.json north_star): linear half-step,
  * one RK4 step h, linear half-step.  NLN: the order the paper implements, Eq. 10-11: one RK4 step of h/2, the full

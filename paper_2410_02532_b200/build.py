@@ -81,7 +81,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         objs = list(ex.map(compile_one, _jobs(only)))
-    cmd = [nvcc, "-shared", "-o", LIB, *objs, "-cudart", "static"]
+    cmd = [nvcc, "-shared", "-o", LIB, *objs, "-cudart", "static", "-ldl"]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         raise RuntimeError(f"link failed:\n{res.stdout}\n{res.stderr}")

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include <cuda_runtime.h>
+#include <dlfcn.h>
 
 #include "../../include/opo.h"
 #include "opo_internal.h"
@@ -117,6 +118,12 @@ struct opo_handle {
     double eom_beta[3] = {0, 0, 0}, eom_f[3] = {0, 0, 0};
     double beta3[3] = {0, 0, 0};                      // third-order dispersion [s^3/m] (opo_set_beta3)
     int splitting = 0;                                // OPO_OPT_SPLITTING
+    // cuFFT baseline engine: plan over [B][N] and natural-order tables (H, H^2, G m; all with 1/N folded in)
+    int cufft_plan = -1;
+    void* natH[3] = {nullptr, nullptr, nullptr};
+    void* natH2[3] = {nullptr, nullptr, nullptr};
+    void* natGM[3] = {nullptr, nullptr, nullptr};
+    size_t natGM_count[3] = {0, 0, 0};
     bool boundary_fft[3] = {false, false, false};
     void* phase = nullptr;
     int* flag = nullptr;
@@ -146,6 +153,40 @@ struct opo_handle {
 };
 
 namespace {
+
+
+// ---- cuFFT, for the internal baseline engine only (BASELINE.json north_star item (d): "a cuFFT + separate
+// elementwise-kernel pipeline kept as an internal baseline, not the product").  Loaded with dlopen on first use so
+// that libopo.so itself has no dependency on it.
+typedef int cufftHandle_t;
+struct CufftApi {
+    void* lib = nullptr;
+    int (*PlanMany)(cufftHandle_t*, int, int*, int*, int, int, int*, int, int, int, int) = nullptr;
+    int (*SetStream)(cufftHandle_t, cudaStream_t) = nullptr;
+    int (*ExecC2C)(cufftHandle_t, void*, void*, int) = nullptr;
+    int (*ExecZ2Z)(cufftHandle_t, void*, void*, int) = nullptr;
+    int (*Destroy)(cufftHandle_t) = nullptr;
+    bool ok = false;
+};
+CufftApi& cufft_api() {
+    static CufftApi api;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        const char* names[] = {"libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so.11", "/usr/local/cuda/lib64/libcufft.so"};
+        for (const char* n : names) { api.lib = dlopen(n, RTLD_NOW | RTLD_LOCAL); if (api.lib) break; }
+        if (api.lib) {
+            api.PlanMany = (decltype(api.PlanMany))dlsym(api.lib, "cufftPlanMany");
+            api.SetStream = (decltype(api.SetStream))dlsym(api.lib, "cufftSetStream");
+            api.ExecC2C = (decltype(api.ExecC2C))dlsym(api.lib, "cufftExecC2C");
+            api.ExecZ2Z = (decltype(api.ExecZ2Z))dlsym(api.lib, "cufftExecZ2Z");
+            api.Destroy = (decltype(api.Destroy))dlsym(api.lib, "cufftDestroy");
+            api.ok = api.PlanMany && api.SetStream && api.ExecC2C && api.ExecZ2Z && api.Destroy;
+        }
+    }
+    return api;
+}
+constexpr int kCufftC2C = 0x29, kCufftZ2Z = 0x69, kCufftForward = -1, kCufftInverse = 1;
 
 int fail(opo_handle* h, int code, const std::string& msg) {
     if (h) h->err = msg; else g_create_error = msg;
@@ -253,6 +294,7 @@ int build_tables(opo_handle* h) {
         for (int k = 0; k < N; ++k) M[k] = Hh[k] * invN;
         to_engine_layout(h, pl, M.data(), lay.data());
         if (int rc = upload_table(h, h->tabH[x], lay.data(), N)) return rc;
+        if (h->natH[x]) if (int rc = upload_complex(h, h->natH[x], M.data(), N)) return rc;        // cuFFT baseline: natural order
         for (int k = 0; k < N; ++k) {
             const double om = omega_of(h, k);
             const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
@@ -260,6 +302,7 @@ int build_tables(opo_handle* h) {
         }
         to_engine_layout(h, pl, M.data(), lay.data());
         if (int rc = upload_table(h, h->tabH2[x], lay.data(), N)) return rc;
+        if (h->natH2[x]) if (int rc = upload_complex(h, h->natH2[x], M.data(), N)) return rc;
 
         if (!h->fields.resonant[x]) continue;
         // boundary tables, shared or per instance
@@ -292,6 +335,15 @@ int build_tables(opo_handle* h) {
             }
             to_engine_layout(h, pl, M.data(), lay.data());
             if (int rc = upload_table(h, (char*)h->tabGM[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
+            if (h->natH[x]) {      // cuFFT baseline
+                if (h->natGM_count[x] != need) {
+                    if (h->natGM[x]) cudaFree(h->natGM[x]);
+                    h->natGM[x] = nullptr;
+                    if (cudaMalloc(&h->natGM[x], need * N * h->esz) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc of baseline tables failed");
+                    h->natGM_count[x] = need;
+                }
+                if (int rc = upload_complex(h, (char*)h->natGM[x] + b * N * h->esz, M.data(), N)) return rc;
+            }
             to_engine_layout(h, pl, Hh.data(), lay.data());
             if (int rc = upload_table(h, (char*)h->tabHB[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
         }
@@ -383,9 +435,10 @@ int ensure_tables(opo_handle* h) {
 
 void free_all(opo_handle* h) {
     for (int x = 0; x < 3; ++x) {
-        void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->mirror[x], h->eom[x]};
+        void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->mirror[x], h->eom[x], h->natH[x], h->natH2[x], h->natGM[x]};
         for (void* p : ptrs) if (p) cudaFree(p);
     }
+    if (h->cufft_plan >= 0 && cufft_api().ok) cufft_api().Destroy(h->cufft_plan);
     void* more[] = {h->scratch, h->tw, h->perm, h->phase, h->flag, h->tw2, h->wlo, h->whi, h->perm2, h->scratch2, h->barrier};
     for (void* p : more) if (p) cudaFree(p);
 }
@@ -488,6 +541,7 @@ int opo_destroy(opo_handle* h) {
 int opo_set_stream(opo_handle* h, void* s) {
     if (!h) return OPO_ERR_INVALID_ARG;
     h->stream = (cudaStream_t)s;
+    if (h->cufft_plan >= 0) cufft_api().SetStream(h->cufft_plan, h->stream);
     return OPO_OK;
 }
 
@@ -541,13 +595,34 @@ int check_async(opo_handle* h) {
 int engine_in_use(const opo_handle* h) {
     if (h->large) return OPO_ENGINE_LARGE;
     if (h->engine_opt == OPO_ENGINE_STREAMING) return OPO_ENGINE_STREAMING;
+    if (h->engine_opt == OPO_ENGINE_CUFFT) return OPO_ENGINE_CUFFT;
     return h->resident_ok ? OPO_ENGINE_RESIDENT : OPO_ENGINE_STREAMING;
 }
 
 // ---- streaming engine ------------------------------------------------------------------------------------------
 enum TableKind { TAB_H, TAB_H2 };
 
+// cuFFT baseline: A <- IDFT(tab .* DFT(A)) as three launches per field (forward C2C over the batch, table multiply, inverse C2C)
+int cufft_linear(opo_handle* h, int x, const void* tab, long long tab_stride) {
+    CufftApi& cf = cufft_api();
+    const int rc1 = h->dbl ? cf.ExecZ2Z(h->cufft_plan, h->cur[x], h->cur[x], kCufftForward) : cf.ExecC2C(h->cufft_plan, h->cur[x], h->cur[x], kCufftForward);
+    if (rc1 != 0) return fail(h, OPO_ERR_CUDA, "cufftExec (forward) failed");
+    opo::MulTabArgs m{h->cur[x], tab, h->B, h->N, tab_stride};
+    OPO_LAUNCH(h, h->dbl ? opo::launch_multab_f64(m, h->stream) : opo::launch_multab_f32(m, h->stream));
+    const int rc2 = h->dbl ? cf.ExecZ2Z(h->cufft_plan, h->cur[x], h->cur[x], kCufftInverse) : cf.ExecC2C(h->cufft_plan, h->cur[x], h->cur[x], kCufftInverse);
+    if (rc2 != 0) return fail(h, OPO_ERR_CUDA, "cufftExec (inverse) failed");
+    h->launches += 2;
+    return OPO_OK;
+}
+
 int stream_linear_all(opo_handle* h, TableKind kind, bool to_exit) {
+    if (engine_in_use(h) == OPO_ENGINE_CUFFT) {
+        for (int x = 0; x < h->F; ++x) {
+            if (int rc = cufft_linear(h, x, kind == TAB_H ? h->natH[x] : h->natH2[x], 0)) return rc;
+            if (to_exit) OPO_CUDA(h, cudaMemcpyAsync(h->exitb[x], h->cur[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+        }
+        return OPO_OK;
+    }
     opo::LinArgs a{};
     a.n_slots = h->F; a.batch = h->B; a.tw = h->tw;
     for (int x = 0; x < h->F; ++x) {
@@ -600,6 +675,8 @@ int stream_boundary(opo_handle* h) {
     for (int x = 0; x < h->F; ++x) {
         if (!h->fields.resonant[x]) {
             OPO_CUDA(h, cudaMemcpyAsync(h->cur[x], h->S[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+        } else if (h->boundary_fft[x] && engine_in_use(h) == OPO_ENGINE_CUFFT) {
+            if (int rc = cufft_linear(h, x, h->natGM[x], h->per_inst_boundary[x] ? h->N : 0)) return rc;
         } else if (h->boundary_fft[x]) {
             opo::LinSlot& sl = a.slot[a.n_slots++];
             sl.src = h->cur[x]; sl.dst = h->cur[x]; sl.dst2 = nullptr;
@@ -622,7 +699,7 @@ bool any_eom(const opo_handle* h) {
 int apply_eom(opo_handle* h) {
     for (int x = 0; x < h->F; ++x) {
         if (!h->eom[x]) continue;
-        opo::MulTabArgs m{h->cur[x], h->eom[x], h->B, h->N};
+        opo::MulTabArgs m{h->cur[x], h->eom[x], h->B, h->N, 0};
         OPO_LAUNCH(h, h->dbl ? opo::launch_multab_f64(m, h->stream) : opo::launch_multab_f32(m, h->stream));
     }
     return OPO_OK;
@@ -913,8 +990,26 @@ int opo_set_option(opo_handle* h, int option, int value) {
         return OPO_OK;
     }
     if (option != OPO_OPT_ENGINE) return fail(h, OPO_ERR_INVALID_ARG, "unknown option");
-    if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING && value != OPO_ENGINE_LARGE)
+    if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING && value != OPO_ENGINE_LARGE &&
+        value != OPO_ENGINE_CUFFT)
         return fail(h, OPO_ERR_INVALID_ARG, "unknown engine");
+    if (value == OPO_ENGINE_CUFFT) {
+        if (h->large) return fail(h, OPO_ERR_UNSUPPORTED, "the cuFFT baseline serves the sizes of the streaming engine");
+        CufftApi& cf = cufft_api();
+        if (!cf.ok) return fail(h, OPO_ERR_UNSUPPORTED, "libcufft could not be loaded");
+        if (h->cufft_plan < 0) {
+            int n[1] = {h->N};
+            cufftHandle_t plan;
+            if (cf.PlanMany(&plan, 1, n, nullptr, 1, h->N, nullptr, 1, h->N, h->dbl ? kCufftZ2Z : kCufftC2C, h->B) != 0)
+                return fail(h, OPO_ERR_CUDA, "cufftPlanMany failed");
+            h->cufft_plan = plan;
+            for (int x = 0; x < h->F; ++x)
+                if (cudaMalloc(&h->natH[x], (size_t)h->N * h->esz) != cudaSuccess || cudaMalloc(&h->natH2[x], (size_t)h->N * h->esz) != cudaSuccess)
+                    return fail(h, OPO_ERR_ALLOC, "cudaMalloc of baseline tables failed");
+            h->tables_dirty = true;
+        }
+        cf.SetStream(h->cufft_plan, h->stream);
+    }
     if (h->large && value != OPO_ENGINE_AUTO && value != OPO_ENGINE_LARGE)
         return fail(h, OPO_ERR_UNSUPPORTED, "N > 2^14 (c128: > 2^13) runs on the large-N engine only");
     if (!h->large && value == OPO_ENGINE_LARGE)

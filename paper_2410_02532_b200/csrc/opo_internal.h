@@ -38,11 +38,13 @@ struct Rk4Args {
     int phase_index;       // >= 0: stage phases at phase_index, +1, +2 instead (N/2 - L - N/2: steps of h/4)
 };
 
-// A[b][n] *= E[n]  (intracavity phase modulator exp(i beta sin(2 pi f tau_n)))
+// A[b][n] *= E[n]  (intracavity phase modulator exp(i beta sin(2 pi f tau_n)); also the
+// frequency-domain table multiply of the cuFFT baseline engine)
 struct MulTabArgs {
     void* A;
-    const void* E;         // [N] complex
+    const void* E;         // [N] complex, or [B][N] with tab_stride = N
     int batch, n;
+    long long tab_stride;  // elements between instances (0 = shared)
 };
 
 // A[b][n] *= m[b]  (mirror sqrt(R) e^{i delta}, Eq. 6)

@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(256) k_multab(MulTabArgs a) {
     cplx<T>* A = reinterpret_cast<cplx<T>*>(a.A);
     const cplx<T>* E = reinterpret_cast<const cplx<T>*>(a.E);
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
-        A[i] = cmul(A[i], ldg(&E[(int)(i % a.n)]));
+        A[i] = cmul(A[i], ldg(&E[(i / a.n) * a.tab_stride + (i % a.n)]));
 }
 
 template <class T, int L>

@@ -625,6 +625,23 @@ def test_nln_ordering_config1_and_large_engine():
     o.close()
 
 
+# ---------------------------------------------------------------------------------------------------------
+# internal baseline: cuFFT + separate elementwise kernels (BASELINE.json north_star item (d))
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision,log2_n,n_fields,splitting", [("c64", 12, 3, 0), ("c128", 10, 2, 0), ("c64", 14, 3, 0), ("c64", 9, 3, 1)])
+def test_cufft_baseline_engine_matches_oracle(precision, log2_n, n_fields, splitting):
+    torch, P = _gpu()
+    w = _with_eom(small_workload(log2_n, n_fields, precision, nz=5, batch=3, dk=13.0, gdd_dt2=0.6, drad=0.3))
+    w.delta_T_signal_s = np.array([-2.0, 0.0, 3.0]) * w.dt          # per-instance boundary table
+    w.splitting = splitting
+    cur, ex, eng = run_gpu(w, P.ENGINE_CUFFT, n_roundtrips=3, calls=2)
+    assert eng == P.ENGINE_CUFFT
+    rcur, rex = run_oracle(w, n_roundtrips=3)
+    e1 = assert_close(cur, rcur, TOL[precision], "cuFFT baseline current")
+    e2 = assert_close(ex, rex, TOL[precision], "cuFFT baseline exit")
+    print(f"cuFFT baseline {precision} 2^{log2_n}: rel L2 current {e1:.3e} exit {e2:.3e}")
+
+
 def test_abi_errors_and_state():
     torch, P = _gpu()
     w = small_workload(8, 2, "c64", nz=4)
