@@ -45,6 +45,8 @@ def _jobs(only=None):
         jobs.append(("opo_inst.cu", f"opo_inst_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
         # the N/2 - L - N/2 instantiation of the resident kernel, in an object of its own
         jobs.append(("opo_inst.cu", f"opo_inst_nln_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_NLN"]))
+        # the dk = 0 instantiation (no stage phases in RK4), likewise
+        jobs.append(("opo_inst.cu", f"opo_inst_dk0_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_NLN", "-DOPO_DK0"]))
     for typ, suf, l in LARGE_INSTANCES:
         if only and f"{suf}:{l}" not in only:
             continue

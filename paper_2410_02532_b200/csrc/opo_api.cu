@@ -721,6 +721,8 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     a.tw = h->tw; a.phase = h->phase; a.phase_stride = phase_stride(h);
     a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
     a.mode = mode; a.z0 = z0; a.steps = steps; a.nln = h->splitting;
+    a.dk0 = !h->splitting;
+    for (int b = 0; b < h->B; ++b) if (h->dk[b] != 0.0) a.dk0 = 0;
     const int n_clusters = std::min(h->B, h->rinfo.max_clusters);
     OPO_LAUNCH(h, h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream)
                          : opo::launch_resident_f32(h->L, a, n_clusters, h->stream));

@@ -10,7 +10,8 @@ namespace opo {
     cudaError_t launch_freq_##SUF##_L##LL(const FreqArgs&, cudaStream_t) __attribute__((weak));               \
     cudaError_t resident_info_##SUF##_L##LL(int, ResidentInfo*) __attribute__((weak));                        \
     cudaError_t launch_resident_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));     \
-    cudaError_t launch_resident_nln_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
+    cudaError_t launch_resident_nln_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak)); \
+    cudaError_t launch_resident_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
 
 #define OPO_DECL_ALL(SUF) \
     OPO_DECL(SUF, 6) OPO_DECL(SUF, 7) OPO_DECL(SUF, 8) OPO_DECL(SUF, 9) OPO_DECL(SUF, 10) OPO_DECL(SUF, 11) \
@@ -42,6 +43,7 @@ OPO_DECL_LARGE(f64, 14) OPO_DECL_LARGE(f64, 15) OPO_DECL_LARGE(f64, 16) OPO_DECL
     cudaError_t resident_info_##SUF(int log2n, int n_fields, ResidentInfo* out) { OPO_SWITCH(resident_info_, SUF, log2n, n_fields, out) } \
     cudaError_t launch_resident_##SUF(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s) {        \
         if (a.nln) { OPO_SWITCH(launch_resident_nln_, SUF, log2n, a, n_clusters, s) }                             \
+        if (a.dk0) { OPO_SWITCH(launch_resident_dk0_, SUF, log2n, a, n_clusters, s) }                             \
         OPO_SWITCH(launch_resident_, SUF, log2n, a, n_clusters, s)                                                \
     }
 

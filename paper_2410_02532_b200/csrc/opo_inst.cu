@@ -20,7 +20,12 @@ cudaError_t OPO_NAME(launch_linear_)(const LinArgs& a, cudaStream_t s) { return 
 cudaError_t OPO_NAME(launch_freq_)(const FreqArgs& a, cudaStream_t s) { return launch_freq_L<OPO_T, OPO_L>(a, s); }
 cudaError_t OPO_NAME(resident_info_)(int n_fields, ResidentInfo* out) { return resident_info_L<OPO_T, OPO_L>(n_fields, out); }
 #endif
-#ifdef OPO_NLN
+#if defined(OPO_DK0)
+// the dk = 0 instantiation of the resident kernel only (build.py: -DOPO_NLN -DOPO_DK0 selects this branch)
+cudaError_t OPO_NAME(launch_resident_dk0_)(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    return launch_resident_L<OPO_T, OPO_L, false, true>(a, n_clusters, s);
+}
+#elif defined(OPO_NLN)
 // the N/2 - L - N/2 instantiation of the resident kernel only (build.py compiles this file a second time with -DOPO_NLN)
 cudaError_t OPO_NAME(launch_resident_nln_)(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
     return launch_resident_L<OPO_T, OPO_L, true>(a, n_clusters, s);

@@ -73,7 +73,7 @@ template <class T, int L, int F> struct res_layout {
 // foreign fields are issued before the arithmetic of the current one (the link moves ~16 B/clk per
 // SM, so the exchange takes about as long as the arithmetic and has to run under it).  RANK is a
 // template parameter so that "foreign" is a compile-time property of the field index.
-template <class T, int L, int F, int NT, int RANK, bool NLN>
+template <class T, int L, int F, int NT, int RANK, bool NLN, bool DK0 = false>
 __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, const cplx<T>* __restrict__ tw0,
                                                 const cplx<T>* __restrict__ tw0s, cplx<T> e0, cplx<T> e1, cplx<T> e2,
                                                 cplx<T> e3, cplx<T> e4, int halves, T pre, T post, const T* kap, T h, uint32_t mb, uint32_t parity) {
@@ -140,7 +140,7 @@ __device__ __forceinline__ void fused_pass0_rk4(cplx<T>* const* fld, int tid, co
 #pragma unroll
                     for (int x = 0; x < F; ++x) y[x] = {y[x].re * pre, y[x].im * pre};
                 }
-                Rk4<T, F>::step(y, e0, e1, e2, kap, h);
+                Rk4<T, F>::template step<DK0>(y, e0, e1, e2, kap, h);
                 if constexpr (NLN) {      // N/2 - L - N/2: two half-steps meet between two linear operators
                     if (halves == 2) Rk4<T, F>::step(y, e2, e3, e4, kap, h);
 #pragma unroll
@@ -174,7 +174,8 @@ __device__ __noinline__ void pass0_local(const cplx<T>* tw, int tid, bool invers
 }
 
 // NLN: the N/2 - L - N/2 ordering is a separate instantiation, so that the default kernel carries none of its code
-template <class T, int L, int F, bool NLN = false>
+// DK0: every instance has dk = 0 (BASELINE.json configs[0..3]): the RK4 stage phases are skipped; again its own instantiation
+template <class T, int L, int F, bool NLN = false, bool DK0 = false>
 __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>::ctas_per_sm) k_resident(ResidentArgs a) {
     constexpr int N = 1 << L, NT = cta_threads<T, L>::value;
     using PL = plan<L>;
@@ -331,9 +332,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
             if constexpr (!FLOW) cluster_arrive();   // my field is ready for its inverse pass 0
             const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
             if constexpr (!FLOW) cluster_wait();     // ... and so is every other field
-            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0, false>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
-            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1, false>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
-            else fused_pass0_rk4<T, L, F, NT, F - 1, false>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
+            if (x == 0) fused_pass0_rk4<T, L, F, NT, 0, false, DK0>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
+            else if (F == 2 || x == 1) fused_pass0_rk4<T, L, F, NT, 1, false, DK0>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
+            else fused_pass0_rk4<T, L, F, NT, F - 1, false, DK0>(fld, tid, tw, tw0s, e0, e1, e2, e2, e2, 1, (T)1, (T)1, kap, h, mb, fz & 1);
             ++fz;
             if constexpr (!FLOW) {
                 cluster_arrive();
@@ -427,24 +428,24 @@ template <class T, int L> cudaError_t resident_info_L(int n_fields, ResidentInfo
 
 // NLN = true is instantiated in its own translation units (opo_inst_nln.cu): the default kernel's object code stays
 // byte for byte what it is without the N/2 - L - N/2 ordering
-template <class T, int L, int F, bool NLN> cudaError_t launch_resident_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+template <class T, int L, int F, bool NLN, bool DK0 = false> cudaError_t launch_resident_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
     cudaLaunchConfig_t cfg{};
     cudaLaunchAttribute attr[1];
     cudaError_t e = resident_cfg<T, L, F>(&cfg, attr, n_clusters, s);
     if (e != cudaSuccess) return e;
-    if constexpr (NLN) {
+    if constexpr (NLN || DK0) {
         static bool configured = false;
         if (!configured) {
-            e = cudaFuncSetAttribute(k_resident<T, L, F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.dynamicSmemBytes);
+            e = cudaFuncSetAttribute(k_resident<T, L, F, NLN, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.dynamicSmemBytes);
             if (e != cudaSuccess) return e;
             configured = true;
         }
     }
-    return cudaLaunchKernelEx(&cfg, k_resident<T, L, F, NLN>, a);
+    return cudaLaunchKernelEx(&cfg, k_resident<T, L, F, NLN, DK0>, a);
 }
 
-template <class T, int L, bool NLN> cudaError_t launch_resident_L(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
-    return a.n_fields == 3 ? launch_resident_LF<T, L, 3, NLN>(a, n_clusters, s) : launch_resident_LF<T, L, 2, NLN>(a, n_clusters, s);
+template <class T, int L, bool NLN, bool DK0 = false> cudaError_t launch_resident_L(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    return a.n_fields == 3 ? launch_resident_LF<T, L, 3, NLN, DK0>(a, n_clusters, s) : launch_resident_LF<T, L, 2, NLN, DK0>(a, n_clusters, s);
 }
 
 }  // namespace opo
