@@ -118,6 +118,7 @@ struct opo_handle {
     double eom_beta[3] = {0, 0, 0}, eom_f[3] = {0, 0, 0};
     double beta3[3] = {0, 0, 0};                      // third-order dispersion [s^3/m] (opo_set_beta3)
     int splitting = 0;                                // OPO_OPT_SPLITTING
+    int* rt_flags = nullptr;                          // resident engine, split launches: [B][F] round trips done
     // cuFFT baseline engine: plan over [B][N] and natural-order tables (H, H^2, G m; all with 1/N folded in)
     int cufft_plan = -1;
     void* natH[3] = {nullptr, nullptr, nullptr};
@@ -439,6 +440,7 @@ void free_all(opo_handle* h) {
         for (void* p : ptrs) if (p) cudaFree(p);
     }
     if (h->cufft_plan >= 0 && cufft_api().ok) cufft_api().Destroy(h->cufft_plan);
+    if (h->rt_flags) cudaFree(h->rt_flags);
     void* more[] = {h->scratch, h->tw, h->perm, h->phase, h->flag, h->tw2, h->wlo, h->whi, h->perm2, h->scratch2, h->barrier};
     for (void* p : more) if (p) cudaFree(p);
 }
@@ -724,6 +726,14 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     a.dk0 = !h->splitting;
     for (int b = 0; b < h->B; ++b) if (h->dk[b] != 0.0) a.dk0 = 0;
     const int n_clusters = std::min(h->B, h->rinfo.max_clusters);
+    // more instances than clusters and not a multiple: deal round trips instead of instances (see the kernel)
+    a.split = 0; a.flags = nullptr;
+    if (mode == 1 && !h->splitting && steps > 1 && h->B > n_clusters && h->B % n_clusters != 0) {
+        if (!h->rt_flags && cudaMalloc((void**)&h->rt_flags, (size_t)h->B * 3 * sizeof(int)) != cudaSuccess)
+            return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the round-trip flags failed");
+        OPO_CUDA(h, cudaMemsetAsync(h->rt_flags, 0, (size_t)h->B * 3 * sizeof(int), h->stream));
+        a.split = 1; a.flags = h->rt_flags;
+    }
     OPO_LAUNCH(h, h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream)
                          : opo::launch_resident_f32(h->L, a, n_clusters, h->stream));
     return OPO_OK;

@@ -80,6 +80,15 @@ __device__ __forceinline__ cplx<double> ldg(const cplx<double>* p) {
     double2 v = __ldg(reinterpret_cast<const double2*>(p));
     return {v.x, v.y};
 }
+// L2-coherent load (data another SM wrote earlier in the same launch)
+__device__ __forceinline__ cplx<float> ldcg_c(const cplx<float>* p) {
+    float2 v = __ldcg(reinterpret_cast<const float2*>(p));
+    return {v.x, v.y};
+}
+__device__ __forceinline__ cplx<double> ldcg_c(const cplx<double>* p) {
+    double2 v = __ldcg(reinterpret_cast<const double2*>(p));
+    return {v.x, v.y};
+}
 // twiddle fetch: SMEM = plain load from a shared-memory copy, otherwise read-only global load
 template <bool SMEM, class T> __device__ __forceinline__ cplx<T> ldtw(const cplx<T>* p) {
     if constexpr (SMEM) return *p;

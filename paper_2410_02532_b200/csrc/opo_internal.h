@@ -87,6 +87,8 @@ struct ResidentArgs {
     double h;
     int n_fields, batch, nz;   // nz = steps per pass
     int mode;              // 0 = propagate `steps` z-steps from step index z0; 1 = `steps` round trips
+    int split;             // 1 (mode 1 only): work is dealt to the clusters in round trips, not instances (opo_resident.cuh)
+    int* flags;            // [B][F] round trips completed per (instance, field), zeroed before a split launch
     int dk0;               // 1: dk = 0 for every instance (and nln = 0): the kernel variant without stage phases
     int nln;               // 1: order N/2 - L - N/2 (Eq. 10-11); phase table then has stride 4 nz + 1 (steps of h/4)
                            //    and mode 1 takes steps = 1

@@ -276,6 +276,40 @@ def test_config4_full_batch_in_bench_launch_configuration():
     print(f"C4 full batch, 2 RT, sampled {sample}: rel L2 current {e1:.3e} exit {e2:.3e}")
 
 
+def test_config4_full_batch_with_round_trip_split_schedule():
+    """256 instances on 45 clusters are not a whole number of waves, so the resident kernel deals round trips, not
+    instances, to its clusters: an instance cut by a range boundary runs its first round trips on one cluster and the
+    rest on the next, handed over through HBM and a release / acquire flag.  5 round trips per instance make the cuts fall
+    inside instances (1280 units / 45 clusters = 29 per cluster: instances 5, 11, 17, ... are split).  Sampled instances,
+    split and unsplit, against the oracle; and the result must not depend on the schedule: one launch per round trip
+    (no split possible) gives the same fields to rounding."""
+    import os
+    import oracle
+    torch, P = _gpu()
+    w = W.config4().truncated(5)
+    o = P.from_workload(w, engine=P.ENGINE_AUTO)
+    assert o.engine == P.ENGINE_RESIDENT
+    o.roundtrips(5)
+    o.sync()
+    o.check_finite()
+    sample = [0, 5, 11, 17, 137, 203, 255]
+    cur = np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    ex = np.stack([o.get_fields(x, P.WHICH_EXIT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    o.close()
+    ref = oracle.run_workload(w, instances=sample, threads=min(len(sample), os.cpu_count() or 1))
+    e1 = assert_close(cur[sample], ref["current"], 1e-4, "C4 split schedule current")
+    e2 = assert_close(ex[sample], ref["exit"], 1e-4, "C4 split schedule exit")
+    o = P.from_workload(w, engine=P.ENGINE_AUTO)
+    for _ in range(5):
+        o.roundtrips(1)
+    o.sync()
+    cur1 = np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    o.close()
+    worst = max(rel_l2(cur[b, x], cur1[b, x]) for b in range(w.batch) for x in range(1, w.n_fields))
+    assert worst < 2e-5, worst
+    print(f"C4 full batch, 5 RT, split schedule: rel L2 vs oracle current {e1:.3e} exit {e2:.3e}; vs call-by-call {worst:.3e}")
+
+
 def test_resident_engine_is_bitwise_reproducible():
     """The resident kernel synchronises its three CTAs per instance with class-granular mbarriers instead of cluster
     barriers; a missing dependency would be a data race, and a race shows up as run-to-run differences.  Two runs of the
