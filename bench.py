@@ -43,15 +43,15 @@ def flops_per_grid_point_zstep(log2_n: int, n_fields: int) -> float:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu captures
-# of exactly this launch configuration (profiles/r01h_*.md); None where no capture of that configuration exists.
+# of exactly this launch configuration (profiles/r01l_*.md); None where no capture of that configuration exists.
 NCU_DRAM_BYTES_PER_LAUNCH = {
     # (workload, engine, round trips per step): bytes
-    ("C4", "resident", 300): 237353216 + 317747200,     # profiles/r01h_dram_c4_default.csv (one 3.06 s launch)
+    ("C4", "resident", 300): 233805312 + 294712064,     # profiles/r01l_dram_c4_default.csv (one 2.95 s launch)
 }
 
 
-# sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed of the resident kernel on C4 (profiles/r01h_resident_kernel_final.md,
-# `ncu --set full` capture of a 2-round-trip launch): how busy the FP32 pipe is over all SM cycles of the launch
+# sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed of the resident kernel on C4 (profiles/r01l_resident_kernel_split_schedule.md,
+# `ncu --set full` capture of a 3-round-trip launch): how busy the FP32 pipe is over all SM cycles of the launch
 NCU_FP32_PIPE_PCT = {("C4", "resident"): 48.8}
 
 
