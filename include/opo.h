@@ -127,8 +127,8 @@ int opo_set_beta3(opo_handle* h, int field, double beta3_s3_per_m);
  * mirror factor, A_x[n] *= exp(i beta sin(2 pi f_pm tau_n)), tau_n = (n - N/2) dt.  beta_rad = 0 removes it.
  * Same modulator for every instance.  OPO_ERR_INVALID_ARG for a non-resonant field (it restarts from its
  * stored input every round trip, so a modulator on it would never act).  The table is built in fp64 on the
- * host.  With a modulator present the boundary is no longer merged into the neighbouring half-steps: the
- * resident and large-N engines then run one launch per round trip. */
+ * host.  With a modulator present the boundary is not merged into the next half-step (the resident engine runs
+ * core(H G m), the modulator in the time domain, core(H) at a crossing; the large-N engine one launch per round trip). */
 int opo_set_eom(opo_handle* h, int field, double beta_rad, double f_mod_hz);
 
 /* Pump input S_p (PAPER.md:L268 ReadPump): time-domain complex [N] (per_instance = 0, broadcast to

@@ -112,6 +112,7 @@ struct opo_handle {
     void* tabH2[3] = {nullptr, nullptr, nullptr};
     void* tabGM[3] = {nullptr, nullptr, nullptr};
     void* tabHB[3] = {nullptr, nullptr, nullptr};
+    void* tabHG[3] = {nullptr, nullptr, nullptr};      // H G m / N: last half-step + boundary, when a modulator follows
     size_t tabB_count[3] = {0, 0, 0};      // instances allocated for GM / HB (1 or B)
     void* mirror[3] = {nullptr, nullptr, nullptr};
     void* eom[3] = {nullptr, nullptr, nullptr};       // [N] exp(i beta sin(2 pi f tau_n)) or null
@@ -311,9 +312,11 @@ int build_tables(opo_handle* h) {
         if (h->tabB_count[x] != need) {
             if (h->tabGM[x]) cudaFree(h->tabGM[x]);
             if (h->tabHB[x]) cudaFree(h->tabHB[x]);
-            h->tabGM[x] = h->tabHB[x] = nullptr;
+            if (h->tabHG[x]) cudaFree(h->tabHG[x]);
+            h->tabGM[x] = h->tabHB[x] = h->tabHG[x] = nullptr;
             if (cudaMalloc(&h->tabGM[x], need * N * h->tab_esz) != cudaSuccess ||
-                cudaMalloc(&h->tabHB[x], need * N * h->tab_esz) != cudaSuccess)
+                cudaMalloc(&h->tabHB[x], need * N * h->tab_esz) != cudaSuccess ||
+                cudaMalloc(&h->tabHG[x], need * N * h->tab_esz) != cudaSuccess)
                 return fail(h, OPO_ERR_ALLOC, "cudaMalloc of boundary tables failed");
             h->tabB_count[x] = need;
         }
@@ -347,6 +350,14 @@ int build_tables(opo_handle* h) {
             }
             to_engine_layout(h, pl, Hh.data(), lay.data());
             if (int rc = upload_table(h, (char*)h->tabHB[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
+            // H G m: the last half-step of a pass and the boundary, the modulator and the next half-step follow separately
+            for (int k = 0; k < N; ++k) {
+                const double om = omega_of(h, k);
+                const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
+                Hh[k] = std::exp(cd(-0.5 * al, D) * (0.5 * h->h)) * M[k];
+            }
+            to_engine_layout(h, pl, Hh.data(), lay.data());
+            if (int rc = upload_table(h, (char*)h->tabHG[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
         }
     }
     h->tables_dirty = false;
@@ -436,7 +447,7 @@ int ensure_tables(opo_handle* h) {
 
 void free_all(opo_handle* h) {
     for (int x = 0; x < 3; ++x) {
-        void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->mirror[x], h->eom[x], h->natH[x], h->natH2[x], h->natGM[x]};
+        void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->tabHG[x], h->mirror[x], h->eom[x], h->natH[x], h->natH2[x], h->natGM[x]};
         for (void* p : ptrs) if (p) cudaFree(p);
     }
     if (h->cufft_plan >= 0 && cufft_api().ok) cufft_api().Destroy(h->cufft_plan);
@@ -712,7 +723,7 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     opo::ResidentArgs a{};
     for (int x = 0; x < h->F; ++x) {
         a.cur[x] = h->cur[x]; a.S[x] = h->S[x]; a.exitb[x] = h->exitb[x]; a.SH[x] = h->SH[x];
-        a.tabH[x] = h->tabH[x]; a.tabH2[x] = h->tabH2[x]; a.tabHB[x] = h->tabHB[x]; a.tabGM[x] = h->tabGM[x];
+        a.tabH[x] = h->tabH[x]; a.tabH2[x] = h->tabH2[x]; a.tabHB[x] = h->tabHB[x]; a.tabGM[x] = h->tabGM[x]; a.tabHG[x] = h->tabHG[x];
         a.tab_stride[x] = h->per_inst_boundary[x] ? h->N : 0;
         a.mirror[x] = h->mirror[x];
         a.eom[x] = h->eom[x];
@@ -902,9 +913,11 @@ int opo_roundtrips(opo_handle* h, int n) {
         return OPO_OK;
     }
     if (engine_in_use(h) == OPO_ENGINE_RESIDENT) {
-        if (!eom && !h->splitting) return resident_run(h, 1, 0, n);
+        // a modulator is applied inside the kernel (between two linear cores at a crossing, with the last store at the
+        // end of a call); only the N/2 - L - N/2 ordering runs one pass per launch
+        if (!h->splitting) return resident_run(h, 1, 0, n);
         for (int m = 0; m < n; ++m)
-            if (int rc = resident_run(h, 1, 0, 1)) return rc;      // the kernel applies the modulator with its last store
+            if (int rc = resident_run(h, 1, 0, 1)) return rc;
         return OPO_OK;
     }
     for (int m = 0; m < n; ++m) {

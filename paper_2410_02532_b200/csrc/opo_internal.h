@@ -74,6 +74,7 @@ struct ResidentArgs {
     const void* tabH2[3];  // merged full step     (shared)
     const void* tabHB[3];  // H G m H merged across the boundary (resonant; maybe per instance)
     const void* tabGM[3];  // G m / N, un-merged boundary       (resonant; maybe per instance)
+    const void* tabHG[3];  // H G m / N: last half-step + boundary, used when a modulator (eom) follows
     long long tab_stride[3];   // instance stride of HB / GM (0 = shared)
     const void* mirror[3]; // [B] complex sqrt(R) e^{i delta} (used when the boundary has no G)
     const void* eom[3];    // [N] complex exp(i beta sin(2 pi f tau_n)) applied after the boundary of the call's last

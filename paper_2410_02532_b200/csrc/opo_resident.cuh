@@ -346,6 +346,38 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                 if constexpr (FLOW) { flow_wait_done_all((fz - 1) & 1); __syncthreads(); }
                 load(SH);                                        // fresh pump / frozen seed, already half-stepped
                 if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }
+            } else if (crossing && a.eom[x] != nullptr) {
+                // resonant field with an intracavity modulator: the modulator acts in the time domain
+                // between the boundary's spectral factor and the next pass, so the crossing is
+                //   core(H G m) -> inverse pass 0 -> x E[n] -> forward pass 0 -> core(H)
+                const cplx<T>* tabHG = reinterpret_cast<const cplx<T>*>(a.tabHG[x]) + (size_t)b * a.tab_stride[x];
+                const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]);
+                if constexpr (FLOW) {
+                    FlowArgs fa;
+                    fa.mb = mb; fa.nf = F;
+                    fa.wait_in = 1; fa.par_done = (fz - 1) & 1;
+                    fa.arrive_out = 0;
+                    linear_core_smem<T, L, NT, true>(tabHG, tid, fa);
+                } else {
+                    linear_core_smem<T, L, NT>(tabHG, tid);
+                }
+                __syncthreads();
+                pass0_local<T, L, NT>(tw, tid, true);
+                __syncthreads();
+#pragma unroll 4
+                for (int i = tid; i < N; i += NT) sm[phys<T>(i)] = cmul(sm[phys<T>(i)], ldg(&E[i]));
+                __syncthreads();
+                pass0_local<T, L, NT>(tw, tid, false);
+                __syncthreads();
+                if constexpr (FLOW) {
+                    FlowArgs fa;
+                    fa.mb = mb; fa.nf = F;
+                    fa.wait_in = 0; fa.par_done = 0;
+                    fa.arrive_out = 1;
+                    linear_core_smem<T, L, NT, true>(tabH, tid, fa);
+                } else {
+                    linear_core_smem<T, L, NT>(tabH, tid);
+                }
             } else {
                 const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
                 if constexpr (FLOW) {
