@@ -33,7 +33,10 @@
 // PAPER.md:L400), P6 Manley-Rowe, P7 depleted SHG closed form, P8 2nd-order convergence, P9 cold
 // cavity, P10 threshold growth, P13 EOM sidebands = Bessel J_m(beta) (Jacobi-Anger) and element order,
 // P14 third-order dispersion: centroid delay (beta3 z/2)(Omega_0^2 + s^2) of an offset Gaussian, P15 N/2-L-N/2 ordering:
-// second-order convergence, O(h^2) agreement with L/2-N-L/2, exact agreement when the operators commute.
+// second-order convergence, O(h^2) agreement with L/2-N-L/2, exact agreement when the operators commute,
+// P16 loss: power falls as exp(-alpha_x z), a pure scale (alpha/2 on the amplitude, Eq. 5), P17 pump re-injection: after
+// the boundary the pump is the stored input bit for bit and round trip 2 equals a hand-composed single pass (L268, R11),
+// P18 z restarts at the crystal entrance every pass with dk != 0 (R4): round trips = passes on fresh oracles.
 // Parity unpinned: reading R12 (non-resonant fields restart from
 // S_x) is a convention with no physical pin; the paper's P_th values (L348) and Figs 3-5.
 // =================================================================================================

@@ -638,3 +638,183 @@ def test_p15_nln_ordering_special_cases():
     b = _p15_run(20, 0, beta=False)
     assert rel_l2(a, b) < 1e-13
     assert rel_l2(a, _p15_run(10, 0, beta=False)) > 1e-9          # and not the h-step result
+
+
+# ---------------------------------------------------------------------------------------------
+# P16  loss: Eq. 5 carries -(alpha_x/2) A_x on the AMPLITUDE, so power falls as e^{-alpha_x z}
+# ---------------------------------------------------------------------------------------------
+
+def test_p16_loss_is_alpha_over_two_on_the_amplitude():
+    """Coupling off, dispersion on, alpha_x different per field: sum|A_x(L)|^2 / sum|A_x(0)|^2 = exp(-alpha_x L)
+    (alpha is the POWER attenuation: the amplitude factor is exp(-alpha_x L / 2)), and the loss is a pure scale:
+    the output equals the lossless output times exp(-alpha_x L / 2), spectral phase untouched.  A factor alpha
+    instead of alpha/2 (or a dropped term) fails both."""
+    log2n, T, L, nz = 8, 10 * PS, 5e-3, 20
+    n = 1 << log2n
+    alpha = (37.0, 110.0, 5.5)            # 1/m; alpha L = 0.185, 0.55, 0.0275
+    b1 = (0.3 * FS / UM, 0.0, -0.17 * FS / UM)
+    b2 = (0.35 * FS * FS / UM, 0.12 * FS * FS / UM, 0.05 * FS * FS / UM)
+    rng = np.random.default_rng(16)
+    a = [rng.standard_normal(n) + 1j * rng.standard_normal(n) for _ in range(3)]
+    out = {}
+    for al in (alpha, (0.0, 0.0, 0.0)):
+        o = make(n_fields=3, log2_n=log2n, window_s=T, nz=nz, length=L, d_eff=0.0, beta1=b1, beta2=b2, alpha=al)
+        for x in range(3):
+            o.set_field(x, a[x])
+        assert o.propagate(nz) == 0
+        out[al] = [o.get_field(x) for x in range(3)]
+    for x in range(3):
+        lossy, lossless = out[alpha][x], out[(0.0, 0.0, 0.0)][x]
+        p_ratio = np.sum(np.abs(lossy) ** 2) / np.sum(np.abs(a[x]) ** 2)
+        assert abs(p_ratio / math.exp(-alpha[x] * L) - 1) < 1e-13
+        assert rel_l2(lossy, lossless * math.exp(-0.5 * alpha[x] * L)) < 1e-13
+        assert abs(np.sum(np.abs(lossless) ** 2) / np.sum(np.abs(a[x]) ** 2) - 1) < 1e-13   # dispersion alone is unitary
+    # a partial pass: z = 7 h
+    o = make(n_fields=2, log2_n=log2n, window_s=T, nz=nz, length=L, d_eff=0.0, alpha=(0.0, 64.0))
+    o.set_field(1, a[1])
+    assert o.propagate(7) == 0
+    assert abs(np.sum(np.abs(o.get_field(1)) ** 2) / np.sum(np.abs(a[1]) ** 2) / math.exp(-64.0 * L * 7 / nz) - 1) < 1e-13
+
+
+def test_p16_loss_enters_the_cold_cavity_round_trip_factor():
+    """Cold cavity with loss: per round trip the power falls by R exp(-alpha_s L)."""
+    log2n, L, nz, R, al, m = 6, 5e-3, 10, 0.9, 48.0, 5
+    n = 1 << log2n
+    o = make(n_fields=2, log2_n=log2n, nz=nz, length=L, d_eff=0.0, resonant=(0, 1), R=(0, R), alpha=(0.0, al),
+             beta2=(0.0, 0.2 * FS * FS / UM))
+    rng = np.random.default_rng(17)
+    a = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    o.set_field(0, np.zeros(n, complex))
+    o.set_field(1, a)
+    assert o.roundtrips(m) == 0
+    assert abs(np.sum(np.abs(o.get_field(1)) ** 2) / np.sum(np.abs(a) ** 2) / (R * math.exp(-al * L)) ** m - 1) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# P17  pump re-injection at the boundary (ReadPump, PAPER.md:L268; readings R11, R12): every round trip starts
+#      from the stored pump input S_p, whatever the crystal did to the pump in the pass before
+# ---------------------------------------------------------------------------------------------
+
+def _mirror(a, R, delta=0.0):
+    return math.sqrt(R) * np.exp(1j * delta) * a
+
+
+def test_p17_depleted_pump_is_replaced_by_the_stored_input_every_round_trip():
+    log2n, L, nz, R = 6, 5e-3, 40, 0.7
+    n = 1 << log2n
+    kw = dict(n_fields=3, log2_n=log2n, nz=nz, length=L, dk=60.0, resonant=(0, 1, 0), R=(0, R, 0),
+              beta1=(0.3 * FS / UM, 0.0, -0.17 * FS / UM),
+              beta2=(0.35 * FS * FS / UM, 0.12 * FS * FS / UM, 0.05 * FS * FS / UM))
+    o = make(**kw)
+    ks = o.kappa(1)
+    amp = 1.5 / (ks * L)                              # kappa A L ~ 1.5: heavy depletion in a single pass (as in P6)
+    rng = np.random.default_rng(170)
+    Sp = amp * (0.8 + 0.2 * (rng.standard_normal(n) + 1j * rng.standard_normal(n)))
+    Ss = 0.5 * amp * (0.7 + 0.3 * (rng.standard_normal(n) + 1j * rng.standard_normal(n)))
+    Si = 0.2 * amp * (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    for x, s in enumerate((Sp, Ss, Si)):
+        o.set_field(x, s)
+    assert o.roundtrips(1) == 0
+    # after the boundary the current pump IS the stored input, bit for bit; the pump that left the crystal is not
+    assert np.array_equal(o.get_field(0, CURRENT), Sp)
+    ex_p = o.get_field(0, EXIT)
+    assert abs(np.sum(np.abs(ex_p) ** 2) / np.sum(np.abs(Sp) ** 2) - 1) > 0.05
+    assert rel_l2(ex_p, Sp) > 0.05
+    assert np.array_equal(o.get_field(2, CURRENT), Si)              # R12: the non-resonant idler restarts too
+    ex_s1 = o.get_field(1, EXIT)
+    assert o.roundtrips(1) == 0
+    # round trip 2, composed by hand from single passes only: fresh pump, mirrored signal, fresh idler, z = 0
+    c = make(**kw)
+    c.set_field(0, Sp)
+    c.set_field(1, _mirror(ex_s1, R))
+    c.set_field(2, Si)
+    assert c.propagate(nz) == 0
+    for x in range(3):
+        assert rel_l2(o.get_field(x, EXIT), c.get_field(x)) < 1e-13
+    # ... and NOT what a pass fed with the depleted pump would give
+    d = make(**kw)
+    d.set_field(0, ex_p)
+    d.set_field(1, _mirror(ex_s1, R))
+    d.set_field(2, Si)
+    assert d.propagate(nz) == 0
+    assert rel_l2(o.get_field(1, EXIT), d.get_field(1)) > 1e-2
+
+
+def test_p17_set_field_input_only_changes_the_next_injection():
+    """The stored input can be replaced between round trips (a pump train): the new S_p is what the next
+    boundary injects, the current state is untouched."""
+    log2n, nz = 5, 10
+    n = 1 << log2n
+    o = make(n_fields=2, log2_n=log2n, nz=nz, resonant=(0, 1), R=(0, 0.9))
+    ks = o.kappa(1)
+    amp = 0.7 / (ks * 5e-3)
+    o.set_field(0, np.full(n, amp, complex))
+    o.set_field(1, np.full(n, 0.3 * amp * np.exp(0.4j), complex))
+    new_pump = np.full(n, 0.5 * amp * np.exp(0.2j), complex)
+    o.set_field(0, new_pump, which="input")
+    assert np.array_equal(o.get_field(0, CURRENT), np.full(n, amp, complex))
+    assert o.roundtrips(1) == 0
+    assert np.array_equal(o.get_field(0, CURRENT), new_pump)
+
+
+# ---------------------------------------------------------------------------------------------
+# P18  z is measured from the crystal entrance and starts again at 0 in every pass (reading R4): with dk != 0 the
+#      phase e^{-/+ i dk z} of Eqs 2-4 (PAPER.md:L87-89) must not run on across round trips
+# ---------------------------------------------------------------------------------------------
+
+def test_p18_dk_phase_restarts_at_the_crystal_entrance_every_round_trip():
+    log2n, L, nz, R, delta, trips = 5, 5e-3, 25, 0.8, 0.3, 3
+    n = 1 << log2n
+    dk = 2.0 / L                                       # dk L = 2: a phase error of 2 rad per missed reset
+    kw = dict(n_fields=2, log2_n=log2n, nz=nz, length=L, dk=dk, resonant=(0, 1), R=(0, R), delta_rad=(0, delta),
+              beta1=(0.3 * FS / UM, 0.0), beta2=(0.35 * FS * FS / UM, 0.10 * FS * FS / UM))
+    o = make(**kw)
+    ks = o.kappa(1)
+    amp = 0.9 / (ks * L)                               # degenerate two-wave: the gain depends on the relative phase
+    rng = np.random.default_rng(18)
+    Sp = amp * (0.9 + 0.1 * (rng.standard_normal(n) + 1j * rng.standard_normal(n)))
+    Ss = 0.3 * amp * (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    o.set_field(0, Sp)
+    o.set_field(1, Ss)
+    assert o.roundtrips(trips) == 0
+    assert o.z == 0.0
+    # the same three passes on fresh oracles (each starts at z = 0), boundary applied in numpy
+    sig = Ss
+    for m in range(trips):
+        c = make(**kw)
+        c.set_field(0, Sp)
+        c.set_field(1, sig)
+        assert c.propagate(nz) == 0
+        ex = [c.get_field(0), c.get_field(1)]
+        sig = _mirror(ex[1], R, delta)
+    for x in range(2):
+        assert rel_l2(o.get_field(x, EXIT), ex[x]) < 1e-13
+    assert rel_l2(o.get_field(1, CURRENT), sig) < 1e-13
+    # a crystal three times as long walked in three pieces has z running on: must NOT be what roundtrips() does
+    kw3 = dict(kw, nz=trips * nz, length=trips * L)
+    r = make(**kw3)
+    r.set_field(0, Sp)
+    r.set_field(1, Ss)
+    for m in range(trips):
+        assert r.propagate(nz) == 0
+        exr = [r.get_field(0), r.get_field(1)]
+        r.set_field(0, Sp, which="state")
+        r.set_field(1, _mirror(exr[1], R, delta), which="state")
+    assert rel_l2(exr[1], ex[1]) > 1e-2
+    # three-wave as well (C4 sweeps dk over +-50 1/m for 300 round trips)
+    kw = dict(n_fields=3, log2_n=log2n, nz=nz, length=L, dk=-1.3 / L, resonant=(0, 1, 0), R=(0, R, 0))
+    o = make(**kw)
+    Si = 0.2 * amp * (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    for x, s in enumerate((Sp, Ss, Si)):
+        o.set_field(x, s)
+    assert o.roundtrips(2) == 0
+    sig = Ss
+    for m in range(2):
+        c = make(**kw)
+        for x, s in enumerate((Sp, sig, Si)):
+            c.set_field(x, s)
+        assert c.propagate(nz) == 0
+        ex = [c.get_field(x) for x in range(3)]
+        sig = _mirror(ex[1], R)
+    for x in range(3):
+        assert rel_l2(o.get_field(x, EXIT), ex[x]) < 1e-13
