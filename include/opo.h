@@ -176,7 +176,7 @@ int opo_check_finite(opo_handle* h);
 /* Position inside the crystal in z-steps taken since the entrance (0 .. nz_per_pass). */
 int opo_get_z_steps(const opo_handle* h, int* out_steps);
 
-/* Execution engine.  AUTO picks RESIDENT where one field fits one SM's shared memory (N <= 2^14 c64,
+/* Execution engine.  AUTO picks RESIDENT or SOLO (see below) where one field fits one SM's shared memory (N <= 2^14 c64,
  * N <= 2^13 c128), else LARGE.
  *   RESIDENT : one thread-block cluster per instance, one CTA per field, fields stay in shared
  *              memory across z-steps and round trips; one launch per opo_propagate/opo_roundtrips.
@@ -194,6 +194,12 @@ int opo_get_z_steps(const opo_handle* h, int* out_steps);
  * elementwise kernels (table multiply, RK4, mirror), the structure of the paper's own program (PAPER.md:L248,
  * L286-287).  Never chosen by AUTO; libcufft is loaded on request.  Sizes of the streaming engine. */
 #define OPO_ENGINE_CUFFT 4
+/* SOLO: one CTA (one SM) per instance, same sizes as RESIDENT: one field in shared memory, the other fields in the SM's
+ * tensor memory (TMEM), so the RK4 step of the coupling terms finds all fields of a grid point on
+ * one SM and nothing crosses the SM-to-SM link; one launch per opo_propagate / opo_roundtrips.  AUTO picks it for
+ * batches that keep (nearly) every SM busy (BASELINE.json configs[4]), RESIDENT for few instances (lowest latency per
+ * instance).  The N/2 - L - N/2 ordering runs on RESIDENT. */
+#define OPO_ENGINE_SOLO 5
 #define OPO_OPT_ENGINE 0
 /* Operator splitting of a z-step.  LNL (default, BASELINE.json north_star): linear half-step,
  * one RK4 step h, linear half-step.  NLN: the order the paper implements, Eq. 10-11: one RK4 step of h/2, the full

@@ -8,6 +8,7 @@ travels to the GPU box with the working tree.
 from __future__ import annotations
 
 import os
+import re
 import subprocess
 import sys
 from concurrent.futures import ThreadPoolExecutor
@@ -32,9 +33,28 @@ def _nvcc() -> str:
 
 
 def _newest_source_mtime() -> float:
-    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+    paths = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if os.path.isfile(os.path.join(CSRC, f))]
     paths.append(os.path.join(os.path.dirname(HERE), "include", "opo.h"))
     return max(os.path.getmtime(p) for p in paths)
+
+
+_INCLUDE = re.compile(r'^\s*#\s*include\s*"([^"]+)"', re.M)
+_DEPS = {}
+
+
+def _deps_mtime(path: str) -> float:
+    """Newest modification time of a source and of every file it includes with "..." (recursively)."""
+    path = os.path.normpath(path)
+    if path in _DEPS:
+        return _DEPS[path]
+    _DEPS[path] = m = os.path.getmtime(path)
+    with open(path) as f:
+        for inc in _INCLUDE.findall(f.read()):
+            cand = os.path.normpath(os.path.join(os.path.dirname(path), inc))
+            if os.path.exists(cand):
+                m = max(m, _deps_mtime(cand))
+    _DEPS[path] = m
+    return m
 
 
 def _jobs(only=None):
@@ -47,6 +67,9 @@ def _jobs(only=None):
         jobs.append(("opo_inst.cu", f"opo_inst_nln_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_NLN"]))
         # the dk = 0 instantiation (no stage phases in RK4), likewise
         jobs.append(("opo_inst.cu", f"opo_inst_dk0_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_NLN", "-DOPO_DK0"]))
+        # the solo engine (one CTA per instance, fields in shared + tensor memory): general and dk = 0 instantiations
+        jobs.append(("opo_inst_solo.cu", f"opo_inst_solo_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
+        jobs.append(("opo_inst_solo.cu", f"opo_inst_solo_dk0_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_DK0"]))
     for typ, suf, l in LARGE_INSTANCES:
         if only and f"{suf}:{l}" not in only:
             continue
@@ -64,12 +87,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
-    newest = _newest_source_mtime()
+    _DEPS.clear()
 
     def compile_one(job) -> str:
         src, objname, defs = job
         obj = os.path.join(OBJ, objname)
-        if not force and os.path.exists(obj) and os.path.getmtime(obj) >= newest:
+        # an object is stale when its source or a header it includes is newer
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) >= _deps_mtime(os.path.join(CSRC, src)):
             return obj
         cmd = [nvcc, *NVCC_FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", obj]
         res = subprocess.run(cmd, capture_output=True, text=True)

@@ -147,6 +147,9 @@ struct opo_handle {
     int engine_opt = OPO_ENGINE_AUTO;
     bool resident_ok = false;
     opo::ResidentInfo rinfo{};
+    bool solo_ok = false;                             // solo engine (one CTA per instance, fields in shared + tensor memory)
+    opo::ResidentInfo sinfo{};                        // max_clusters = co-resident CTAs on the device
+    int device = 0;
     long long launches = 0;
     std::string err;
     std::vector<int> host_perm;
@@ -498,6 +501,7 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
     h->tab_esz = h->large ? 16 : h->esz;
     h->h = c->length_m / (double)g->nz_per_pass;
     h->sm_count = prop.multiProcessorCount;
+    h->device = dev;
     for (int x = 0; x < h->F; ++x) h->kappa[x] = 2.0 * kPi * c->d_eff_m_per_V / (f->n[x] * f->lambda_m[x]);
     if (h->F == 2) h->kappa[0] *= 0.5;                                                                         // reading R5
     h->dk.assign(h->B, c->dk_per_m);
@@ -536,6 +540,9 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
         // resident engine availability
         cudaError_t e = h->dbl ? opo::resident_info_f64(h->L, h->F, &h->rinfo) : opo::resident_info_f32(h->L, h->F, &h->rinfo);
         h->resident_ok = (e == cudaSuccess && h->rinfo.max_clusters > 0);
+        if (e != cudaSuccess) cudaGetLastError();
+        e = h->dbl ? opo::solo_info_f64(h->L, h->F, &h->sinfo) : opo::solo_info_f32(h->L, h->F, &h->sinfo);
+        h->solo_ok = (e == cudaSuccess && h->sinfo.max_clusters > 0);
         if (e != cudaSuccess) cudaGetLastError();
     }
     if (cudaDeviceSynchronize() != cudaSuccess) return bail(OPO_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
@@ -605,10 +612,25 @@ int check_async(opo_handle* h) {
     return OPO_OK;
 }
 
+// AUTO between the two on-chip engines: the cluster engine gives an instance F SMs (lowest latency per instance,
+// rinfo.max_clusters instances at a time), the solo engine one SM (no SM-to-SM exchange, every SM busy, sinfo.max_clusters
+// instances at a time).  Per z-step an instance takes ~2.6x longer on one SM than on a cluster of three (measured on C4 /
+// C1), so solo wins once the batch keeps more than ~2.6x as many CTAs busy as there are clusters.
+bool prefer_solo(const opo_handle* h) {
+    if (!h->solo_ok || h->splitting) return false;      // the N/2 - L - N/2 ordering runs on the cluster engine
+    if (!h->resident_ok) return true;
+    const double solo_slots = (double)std::min(h->B, h->sinfo.max_clusters);
+    const double cluster_slots = (double)std::min(h->B, h->rinfo.max_clusters);
+    return solo_slots > 2.6 * cluster_slots;
+}
+
 int engine_in_use(const opo_handle* h) {
     if (h->large) return OPO_ENGINE_LARGE;
     if (h->engine_opt == OPO_ENGINE_STREAMING) return OPO_ENGINE_STREAMING;
     if (h->engine_opt == OPO_ENGINE_CUFFT) return OPO_ENGINE_CUFFT;
+    if (h->engine_opt == OPO_ENGINE_SOLO && h->solo_ok && !h->splitting) return OPO_ENGINE_SOLO;
+    if (h->engine_opt == OPO_ENGINE_RESIDENT && h->resident_ok) return OPO_ENGINE_RESIDENT;
+    if (prefer_solo(h)) return OPO_ENGINE_SOLO;
     return h->resident_ok ? OPO_ENGINE_RESIDENT : OPO_ENGINE_STREAMING;
 }
 
@@ -736,7 +758,8 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     a.mode = mode; a.z0 = z0; a.steps = steps; a.nln = h->splitting;
     a.dk0 = !h->splitting;
     for (int b = 0; b < h->B; ++b) if (h->dk[b] != 0.0) a.dk0 = 0;
-    const int n_clusters = std::min(h->B, h->rinfo.max_clusters);
+    const bool solo = engine_in_use(h) == OPO_ENGINE_SOLO;
+    const int n_clusters = std::min(h->B, solo ? h->sinfo.max_clusters : h->rinfo.max_clusters);
     // more instances than clusters and not a multiple: deal round trips instead of instances (see the kernel)
     a.split = 0; a.flags = nullptr;
     if (mode == 1 && !h->splitting && steps > 1 && h->B > n_clusters && h->B % n_clusters != 0) {
@@ -745,8 +768,11 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
         OPO_CUDA(h, cudaMemsetAsync(h->rt_flags, 0, (size_t)h->B * 3 * sizeof(int), h->stream));
         a.split = 1; a.flags = h->rt_flags;
     }
-    OPO_LAUNCH(h, h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream)
-                         : opo::launch_resident_f32(h->L, a, n_clusters, h->stream));
+    if (solo)
+        OPO_LAUNCH(h, h->dbl ? opo::launch_solo_f64(h->L, a, n_clusters, h->stream) : opo::launch_solo_f32(h->L, a, n_clusters, h->stream));
+    else
+        OPO_LAUNCH(h, h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream)
+                             : opo::launch_resident_f32(h->L, a, n_clusters, h->stream));
     return OPO_OK;
 }
 
@@ -887,7 +913,7 @@ int opo_propagate(opo_handle* h, int nz) {
     if (int rc = ensure_tables(h)) return rc;
     int rc;
     if (h->large) rc = large_run(h, 0, h->z_steps, nz);
-    else if (engine_in_use(h) == OPO_ENGINE_RESIDENT) rc = resident_run(h, 0, h->z_steps, nz);
+    else if (engine_in_use(h) == OPO_ENGINE_RESIDENT || engine_in_use(h) == OPO_ENGINE_SOLO) rc = resident_run(h, 0, h->z_steps, nz);
     else rc = stream_steps(h, h->z_steps, nz, false);
     if (rc) return rc;
     h->z_steps += nz;
@@ -912,7 +938,7 @@ int opo_roundtrips(opo_handle* h, int n) {
         }
         return OPO_OK;
     }
-    if (engine_in_use(h) == OPO_ENGINE_RESIDENT) {
+    if (engine_in_use(h) == OPO_ENGINE_RESIDENT || engine_in_use(h) == OPO_ENGINE_SOLO) {
         // a modulator is applied inside the kernel (between two linear cores at a crossing, with the last store at the
         // end of a call); only the N/2 - L - N/2 ordering runs one pass per launch
         if (!h->splitting) return resident_run(h, 1, 0, n);
@@ -1016,7 +1042,7 @@ int opo_set_option(opo_handle* h, int option, int value) {
     }
     if (option != OPO_OPT_ENGINE) return fail(h, OPO_ERR_INVALID_ARG, "unknown option");
     if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING && value != OPO_ENGINE_LARGE &&
-        value != OPO_ENGINE_CUFFT)
+        value != OPO_ENGINE_CUFFT && value != OPO_ENGINE_SOLO)
         return fail(h, OPO_ERR_INVALID_ARG, "unknown engine");
     if (value == OPO_ENGINE_CUFFT) {
         if (h->large) return fail(h, OPO_ERR_UNSUPPORTED, "the cuFFT baseline serves the sizes of the streaming engine");
@@ -1041,6 +1067,8 @@ int opo_set_option(opo_handle* h, int option, int value) {
         return fail(h, OPO_ERR_UNSUPPORTED, "the large-N engine serves N > 2^14 (c128: > 2^13) only");
     if (value == OPO_ENGINE_RESIDENT && !h->resident_ok)
         return fail(h, OPO_ERR_UNSUPPORTED, "resident engine unavailable for this size/precision on this device");
+    if (value == OPO_ENGINE_SOLO && !h->solo_ok)
+        return fail(h, OPO_ERR_UNSUPPORTED, "solo engine unavailable for this size/precision on this device");
     h->engine_opt = value;
     return OPO_OK;
 }

@@ -11,7 +11,10 @@ namespace opo {
     cudaError_t resident_info_##SUF##_L##LL(int, ResidentInfo*) __attribute__((weak));                        \
     cudaError_t launch_resident_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));     \
     cudaError_t launch_resident_nln_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak)); \
-    cudaError_t launch_resident_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
+    cudaError_t launch_resident_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak)); \
+    cudaError_t solo_info_##SUF##_L##LL(int, ResidentInfo*) __attribute__((weak));                            \
+    cudaError_t launch_solo_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));      \
+    cudaError_t launch_solo_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
 
 #define OPO_DECL_ALL(SUF) \
     OPO_DECL(SUF, 6) OPO_DECL(SUF, 7) OPO_DECL(SUF, 8) OPO_DECL(SUF, 9) OPO_DECL(SUF, 10) OPO_DECL(SUF, 11) \
@@ -45,6 +48,11 @@ OPO_DECL_LARGE(f64, 14) OPO_DECL_LARGE(f64, 15) OPO_DECL_LARGE(f64, 16) OPO_DECL
         if (a.nln) { OPO_SWITCH(launch_resident_nln_, SUF, log2n, a, n_clusters, s) }                             \
         if (a.dk0) { OPO_SWITCH(launch_resident_dk0_, SUF, log2n, a, n_clusters, s) }                             \
         OPO_SWITCH(launch_resident_, SUF, log2n, a, n_clusters, s)                                                \
+    }                                                                                                             \
+    cudaError_t solo_info_##SUF(int log2n, int n_fields, ResidentInfo* out) { OPO_SWITCH(solo_info_, SUF, log2n, n_fields, out) } \
+    cudaError_t launch_solo_##SUF(int log2n, const ResidentArgs& a, int n_ctas, cudaStream_t s) {                 \
+        if (a.dk0) { OPO_SWITCH(launch_solo_dk0_, SUF, log2n, a, n_ctas, s) }                                     \
+        OPO_SWITCH(launch_solo_, SUF, log2n, a, n_ctas, s)                                                        \
     }
 
 OPO_DISPATCHERS(f32)

@@ -1,5 +1,6 @@
 // opo_internal.h -- plain-C++ interface between the host library (opo_api.cu) and the templated
-// kernel launchers (opo_inst_f32.cu / opo_inst_f64.cu).  No CUDA templates leak through here.
+// kernel launchers (opo_inst.cu, opo_inst_solo.cu, opo_inst_large.cu, one object per precision and size,
+// routed by opo_dispatch.cu).  No CUDA templates leak through here.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -63,8 +64,9 @@ struct FreqArgs {
     int batch;
 };
 
-// ---- resident engine ---------------------------------------------------------------------------------
-// One thread-block cluster per instance, CTA rank = field.  See opo_resident.cuh.
+// ---- resident (cluster) engine and solo engine ---------------------------------------------------------
+// Cluster engine: one thread-block cluster per instance, CTA rank = field (opo_resident.cuh).
+// Solo engine: one CTA per instance, one field in shared memory, the others in tensor memory (opo_solo.cuh).
 struct ResidentArgs {
     void* cur[3];          // [B][N] current fields (read at start, written at end)
     const void* S[3];      // stored inputs (non-resonant fields restart from these)
@@ -154,6 +156,8 @@ struct LargeInfo {
     cudaError_t launch_finite_##SUFFIX(const void* A, long long count, int* flag, cudaStream_t s); \
     cudaError_t resident_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);     \
     cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
+    cudaError_t solo_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);         \
+    cudaError_t launch_solo_##SUFFIX(int log2n, const ResidentArgs& a, int n_ctas, cudaStream_t s); \
     cudaError_t large_info_##SUFFIX(int log2n, int n_fields, int batch, int sm_count, LargeInfo* out);       \
     cudaError_t launch_large_##SUFFIX(int log2n, const LargeArgs& a, int grid, cudaStream_t s);
 
