@@ -216,6 +216,7 @@ int opo_set_option(opo_handle* h, int option, int value);
 #define OPO_INFO_N 2
 #define OPO_INFO_BATCH 3
 #define OPO_INFO_SM_COUNT 4
+#define OPO_INFO_SLOTS 5           /* co-resident work slots (clusters / CTAs) the next roundtrips call deals its work to */
 int opo_get_info(const opo_handle* h, int what, long long* out);
 
 /* Last error text of this handle (or of the failed opo_create when h is NULL).  Never NULL. */

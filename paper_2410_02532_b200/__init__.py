@@ -27,7 +27,7 @@ ENGINE_AUTO, ENGINE_RESIDENT, ENGINE_STREAMING, ENGINE_LARGE, ENGINE_CUFFT, ENGI
 OPT_ENGINE = 0
 OPT_SPLITTING = 1
 SPLITTING_LNL, SPLITTING_NLN = 0, 1
-INFO_ENGINE, INFO_LAUNCHES, INFO_N, INFO_BATCH, INFO_SM_COUNT = 0, 1, 2, 3, 4
+INFO_ENGINE, INFO_LAUNCHES, INFO_N, INFO_BATCH, INFO_SM_COUNT, INFO_SLOTS = 0, 1, 2, 3, 4, 5
 
 _D3 = ctypes.c_double * 3
 _I3 = ctypes.c_int * 3

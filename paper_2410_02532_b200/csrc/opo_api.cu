@@ -1081,6 +1081,14 @@ int opo_get_info(const opo_handle* h, int what, long long* out) {
         case OPO_INFO_N: *out = h->N; return OPO_OK;
         case OPO_INFO_BATCH: *out = h->B; return OPO_OK;
         case OPO_INFO_SM_COUNT: *out = h->sm_count; return OPO_OK;
+        case OPO_INFO_SLOTS: {
+            const int e = engine_in_use(h);
+            if (e == OPO_ENGINE_SOLO) *out = std::min(h->B, h->sinfo.max_clusters);
+            else if (e == OPO_ENGINE_RESIDENT) *out = std::min(h->B, h->rinfo.max_clusters);
+            else if (e == OPO_ENGINE_LARGE) *out = h->linfo.grid;
+            else *out = (long long)h->B * h->F;
+            return OPO_OK;
+        }
         default: return OPO_ERR_INVALID_ARG;
     }
 }

@@ -481,6 +481,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t addr, uint32_t parity) {
         "@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(addr), "r"(parity)
         : "memory");
 }
+// the same with acquire at CTA scope: all producers are threads of this CTA (solo engine), no cache invalidation needed
+__device__ __forceinline__ void mbar_wait_cta(uint32_t addr, uint32_t parity) {
+    asm volatile(
+        "{\n.reg .pred P1;\nLAB_WAIT:\n"
+        "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}" ::"r"(addr), "r"(parity)
+        : "memory");
+}
+// arrive on a barrier of this CTA; release at CTA scope after a __syncwarp that orders the other lanes' writes before it
+__device__ __forceinline__ void mbar_arrive_cta(uint32_t addr, int lane) {
+    __syncwarp();
+    if (lane == 0) asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(addr) : "memory");
+}
 // lanes 0 .. nf-1 of a converged warp arrive on the barrier at local address `addr` in CTA `lane`;
 // release at cluster scope, after a __syncwarp that orders the other lanes' writes before it
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t addr, int lane, int nf) {
@@ -560,7 +573,7 @@ __device__ __forceinline__ void mid_bf(cplx<T>* __restrict__ sm, const TAB* h, i
 }
 
 // forward passes PASS .. LASTF of one group, a group barrier after each
-template <class T, int L, int NT, int PASS, int LASTF, bool FLOW>
+template <class T, int L, int NT, int PASS, int LASTF, bool FLOW, bool CTA = false>
 __device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g, int tg, const FlowArgs& fa) {
     using CG = core_groups<T, L, NT>;
     if constexpr (PASS <= LASTF) {
@@ -569,7 +582,10 @@ __device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g
             using FC = flow_cfg<T, L, NT>;
 #pragma unroll 1
             for (int it = 0; it < FC::NIT; ++it) {
-                if (fa.wait_in) mbar_wait(fa.mb + 8 * (FC::NCLS + (tg >> 5) + FC::NWG * it), fa.par_done);
+                if (fa.wait_in) {
+                    if constexpr (CTA) mbar_wait_cta(fa.mb + 8 * (FC::NCLS + (tg >> 5) + FC::NWG * it), fa.par_done);
+                    else mbar_wait(fa.mb + 8 * (FC::NCLS + (tg >> 5) + FC::NWG * it), fa.par_done);
+                }
                 fwd_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
             }
         } else {
@@ -577,11 +593,11 @@ __device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g
             for (int ul = tg; ul < NB; ul += CG::NTG) fwd_bf<T, L, PASS>(sm, twl, g * NB + ul);
         }
         group_bar<CG::G, CG::NTG>(g);
-        group_fwd<T, L, NT, PASS + 1, LASTF, FLOW>(sm, twl, g, tg, fa);
+        group_fwd<T, L, NT, PASS + 1, LASTF, FLOW, CTA>(sm, twl, g, tg, fa);
     }
 }
 // inverse passes PASS .. 1 of one group, a group barrier before each
-template <class T, int L, int NT, int PASS, bool FLOW>
+template <class T, int L, int NT, int PASS, bool FLOW, bool CTA = false>
 __device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g, int tg, const FlowArgs& fa) {
     using CG = core_groups<T, L, NT>;
     if constexpr (PASS >= 1) {
@@ -592,19 +608,23 @@ __device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g
 #pragma unroll 1
             for (int it = 0; it < FC::NIT; ++it) {
                 inv_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
-                if (fa.arrive_out) mbar_arrive_cluster(fa.mb + 8 * ((tg >> 5) + FC::NWG * it), tg & 31, fa.nf);
+                if (fa.arrive_out) {
+                    if constexpr (CTA) mbar_arrive_cta(fa.mb + 8 * ((tg >> 5) + FC::NWG * it), tg & 31);
+                    else mbar_arrive_cluster(fa.mb + 8 * ((tg >> 5) + FC::NWG * it), tg & 31, fa.nf);
+                }
             }
         } else {
 #pragma unroll 1
             for (int ul = tg; ul < NB; ul += CG::NTG) inv_bf<T, L, PASS>(sm, twl, g * NB + ul);
         }
-        group_inv<T, L, NT, PASS - 1, FLOW>(sm, twl, g, tg, fa);
+        group_inv<T, L, NT, PASS - 1, FLOW, CTA>(sm, twl, g, tg, fa);
     }
 }
 
 // Caller guarantees the field is visible to all threads on entry (barrier) and must barrier before
 // reading the result.  Not inlined: one copy serves every call site of a kernel.
-template <class T, int L, int NT, bool FLOW = false>
+// CTA: the flow barriers are used by threads of this CTA only (solo engine): acquire / release at CTA scope
+template <class T, int L, int NT, bool FLOW = false, bool CTA = false>
 __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, int tid, FlowArgs fa = FlowArgs{}) {
     using PL = plan<L>;
     using CG = core_groups<T, L, NT>;
@@ -615,7 +635,7 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
     const int g = (CG::G == 1) ? 0 : tid / CG::NTG, tg = (CG::G == 1) ? tid : tid % CG::NTG;
     constexpr int R = 1 << CG::RBL, NBF = (1 << L) >> CG::RBL;
     if constexpr (CG::chain) {
-        group_fwd<T, L, NT, 1, PL::P - 3, FLOW>(sm, twl, g, tg, fa);
+        group_fwd<T, L, NT, 1, PL::P - 3, FLOW, CTA>(sm, twl, g, tg, fa);
 #pragma unroll 1
         for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
             const int u = g * CG::NBL + ul;
@@ -634,9 +654,9 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
             __syncwarp();
             inv_bf<T, L, PL::P - 2>(sm, twl, u);
         }
-        group_inv<T, L, NT, PL::P - 3, FLOW>(sm, twl, g, tg, fa);
+        group_inv<T, L, NT, PL::P - 3, FLOW, CTA>(sm, twl, g, tg, fa);
     } else {
-        group_fwd<T, L, NT, 1, PL::P - 2, FLOW>(sm, twl, g, tg, fa);
+        group_fwd<T, L, NT, 1, PL::P - 2, FLOW, CTA>(sm, twl, g, tg, fa);
 #pragma unroll 1
         for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
             const int u = g * CG::NBL + ul;
@@ -645,7 +665,7 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
             for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
             mid_bf<T, L>(sm, h, u);
         }
-        group_inv<T, L, NT, PL::P - 2, FLOW>(sm, twl, g, tg, fa);
+        group_inv<T, L, NT, PL::P - 2, FLOW, CTA>(sm, twl, g, tg, fa);
     }
 }
 

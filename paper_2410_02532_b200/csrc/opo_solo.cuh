@@ -82,12 +82,6 @@ __device__ __forceinline__ void tmem_st4(uint32_t addr, const cplx<double>* v) {
                  "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
 }
 
-// arrive on a barrier of this CTA; release at CTA scope after a __syncwarp that orders the other lanes' writes before it
-__device__ __forceinline__ void mbar_arrive_local(uint32_t addr, int lane) {
-    __syncwarp();
-    if (lane == 0) asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(addr) : "memory");
-}
-
 template <class T, int L, int F> struct solo_layout {
     static constexpr int NT = cta_threads<T, L>::value;
     static constexpr int S = 1 << (L - 2), NTILES = (S + 31) / 32, NW = NT / 32;
@@ -142,7 +136,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                 mbar_init(mb + 8 * c, SO::ready_count);
                 mbar_init(mb + 8 * (FC::NCLS + c), SO::done_count);
             }
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");      // (the only scope this fence has)
         }
     }
     // tensor memory: (F - 1) field slots
@@ -161,11 +155,11 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
     const int cls = FLOW ? warp % SO::NCLS1 : 0;       // all tiles of a warp belong to one class (NW is a multiple of NCLS)
     auto flow_wait_done_all = [&](uint32_t parity) {
         if constexpr (FLOW)
-            for (int it = 0; it < FC::NIT; ++it) mbar_wait(mb + 8 * (FC::NCLS + wg + FC::NWG * it), parity);
+            for (int it = 0; it < FC::NIT; ++it) mbar_wait_cta(mb + 8 * (FC::NCLS + wg + FC::NWG * it), parity);
     };
     auto flow_arrive_ready_all = [&]() {
         if constexpr (FLOW)
-            for (int it = 0; it < FC::NIT; ++it) mbar_arrive_local(mb + 8 * (wg + FC::NWG * it), lane);
+            for (int it = 0; it < FC::NIT; ++it) mbar_arrive_cta(mb + 8 * (wg + FC::NWG * it), lane);
     };
     T kap[3] = {(T)a.kappa[0], (T)a.kappa[1], (T)a.kappa[2]};
     const T h = (T)a.h;
@@ -203,7 +197,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
     };
     // swap k: field k (shared memory) <-> field k + 1 (slot k)
     auto swap_fields = [&](int slot) {
-        if constexpr (FLOW) mbar_wait(mb + 8 * cls, fz & 1);         // ready[cls]: inverse pass 1 of my class is done in all groups
+        if constexpr (FLOW) mbar_wait_cta(mb + 8 * cls, fz & 1);         // ready[cls]: inverse pass 1 of my class is done in all groups
         else __syncthreads();
         int i = 0;
 #pragma unroll 1
@@ -223,14 +217,14 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
             tmem_st4(tmem_at(slot, i), out);
         }
         tmem_wait_st();
-        if constexpr (FLOW) mbar_arrive_local(mb + 8 * (FC::NCLS + cls), lane);    // done[cls]
+        if constexpr (FLOW) mbar_arrive_cta(mb + 8 * (FC::NCLS + cls), lane);    // done[cls]
         else __syncthreads();
         ++fz;
     };
     // fused: inverse pass 0 -> RK4 -> forward pass 0; field F-1 in shared memory, field x < F-1 in slot x;
     // afterwards field 0 in shared memory, field x >= 1 in slot x - 1
     auto fused = [&](cplx<T> e0, cplx<T> e1, cplx<T> e2) {
-        if constexpr (FLOW) mbar_wait(mb + 8 * cls, fz & 1);
+        if constexpr (FLOW) mbar_wait_cta(mb + 8 * cls, fz & 1);
         else __syncthreads();
         cplx<T> wn[R - 1];
         auto load_tw = [&](int tile) {
@@ -284,7 +278,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
             for (int x = 1; x < F; ++x) tmem_st4(tmem_at(x - 1, i), v[x]);
         }
         tmem_wait_st();
-        if constexpr (FLOW) mbar_arrive_local(mb + 8 * (FC::NCLS + cls), lane);
+        if constexpr (FLOW) mbar_arrive_cta(mb + 8 * (FC::NCLS + cls), lane);
         else __syncthreads();
         ++fz;
     };
@@ -294,7 +288,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
             fa.mb = mb; fa.nf = 1;
             fa.wait_in = wait_in; fa.par_done = (fz - 1) & 1;
             fa.arrive_out = arrive_out;
-            linear_core_smem<T, L, NT, true>(tab, tid, fa);
+            linear_core_smem<T, L, NT, true, true>(tab, tid, fa);
         } else {
             linear_core_smem<T, L, NT>(tab, tid);
         }
