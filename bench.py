@@ -12,7 +12,7 @@ configs[1] (the same OPO, a single instance: latency-bound, 3 of 148 SMs), C0 / 
 
 Prints ONE JSON line (rank 0).  `value` = grid-point z-steps/s with inputs resident in HBM;
 `e2e` = the same through the host-buffer ABI calls (H2D of pump and seeds, D2H of the exit signal
-inside the timed region); `roofline` = the resident kernel against the FP32-pipe peak (DESIGN.md);
+inside the timed region); `roofline` = the dominant kernel against the FP32 FMA peak measured in the same run (DESIGN.md);
 `cpu_baseline` = the fp64 oracle on this host's cores on a bounded sample.
 `--impl reference` times the oracle instead (rank 0 only).
 """
@@ -42,21 +42,23 @@ def flops_per_grid_point_zstep(log2_n: int, n_fields: int) -> float:
     return n_fields * (2 * 5 * log2_n + 6 + 76)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the committed ncu captures
-# of exactly this launch configuration (profiles/r01l_*.md); None where no capture of that configuration exists.
-NCU_DRAM_BYTES_PER_LAUNCH = {
-    # (workload, engine, round trips per step): bytes
-    ("C4", "resident", 300): 233805312 + 294712064,     # profiles/r01l_dram_c4_default.csv (one 2.95 s launch)
-}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per launch come from ncu captures, which bench.py
+# cannot take itself (a number printed under a profiler is never a bench value): profiles/ncu_traffic.json lists, per
+# (workload, engine, round trips per step), the bytes, the capture file and the commit it was taken at.  No entry -> null.
+def ncu_traffic(workload: str, engine: str, rt_per_step: int):
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    for e in json.load(open(path)).get("captures", []):
+        if e.get("workload") == workload and e.get("engine") == engine and e.get("rt_per_step") == rt_per_step:
+            return e.get("dram_bytes_per_launch"), f"{e.get('source')} @ {e.get('commit')}"
+    return None, None
 
 
-# sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed of the resident kernel on C4 (profiles/r01l_resident_kernel_split_schedule.md,
-# `ncu --set full` capture of a 3-round-trip launch): how busy the FP32 pipe is over all SM cycles of the launch
-NCU_FP32_PIPE_PCT = {("C4", "resident"): 48.8}
-
-
-def ncu_traffic_bytes(workload: str, engine: str, rt_per_step: int):
-    return NCU_DRAM_BYTES_PER_LAUNCH.get((workload, engine, rt_per_step))
+# shared-memory bytes per field-point z-step of the on-chip engines: six passes over the field
+# (pass 0 + RK4, forward pass 1, the three-pass chain, inverse pass 1), each a read and a write of one complex value
+def smem_bytes_per_field_point_zstep(precision: str) -> float:
+    return 6 * 2 * (16 if precision == "c128" else 8)
 
 
 def make_workload(name: str, rank: int):
@@ -298,16 +300,27 @@ def main():
     avg_s = statistics.mean(per_step_ms) * 1e-3
     eng = o.engine
     eng_name = {P.ENGINE_RESIDENT: "resident", P.ENGINE_SOLO: "solo", P.ENGINE_STREAMING: "streaming", P.ENGINE_LARGE: "large", P.ENGINE_CUFFT: "cufft"}.get(eng, str(eng))
-    traffic = ncu_traffic_bytes(args.workload, eng_name, rt_per_step)
+    traffic, traffic_source = ncu_traffic(args.workload, eng_name, rt_per_step)
     if eng in (P.ENGINE_RESIDENT, P.ENGINE_SOLO):
-        # fields stay in shared memory: bound by FP32 instruction issue
+        # fields stay on chip (shared memory / tensor memory): bound by the FP32 (FP64) FMA pipe, shared memory second.
+        # Both peaks are MEASURED here, on this device, by the library's own micro-benchmark kernels (opo_selftest_peak).
         fl = flops_per_grid_point_zstep(w.log2_n, w.n_fields) * units_per_step          # per launch (= per step)
         dbl = w.precision == "c128"
-        peak_tflops = 148 * (64 if dbl else 128) * 2 * 1.965e9 / 1e12
-        roofline = {"bound": "alu", "kernel": "k_solo" if eng == P.ENGINE_SOLO else "k_resident", "achieved": fl / avg_s / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
-                    "frac": fl / avg_s / 1e12 / peak_tflops, "traffic": traffic,
-                    "fp32_pipe_busy_pct_ncu": NCU_FP32_PIPE_PCT.get((args.workload, eng_name)),
-                    "note": f"{'FP64' if dbl else 'FP32'} FMA-pipe peak = 148 SM x {64 if dbl else 128} lanes x 2 x 1.965 GHz (guide unit counts, max clock); "
+        sms = int(P.opo_get_info(o._h, P.INFO_SM_COUNT))
+        sm_max_ghz = (clocks.get("sm_max_mhz") or 1965.0) / 1e3
+        peak_nominal = sms * (64 if dbl else 128) * 2 * sm_max_ghz * 1e9 / 1e12
+        peak_meas = P.opo_selftest_peak(P.PEAK_FP64_FMA if dbl else P.PEAK_FP32_FMA)
+        smem_peak = P.opo_selftest_peak(P.PEAK_SMEM)
+        smem_by = smem_bytes_per_field_point_zstep(w.precision) * w.n_fields * units_per_step
+        roofline = {"bound": "alu", "kernel": "k_solo" if eng == P.ENGINE_SOLO else "k_resident", "achieved": fl / avg_s / 1e12,
+                    "peak": peak_meas, "unit": "TFLOP/s", "frac": fl / avg_s / 1e12 / peak_meas,
+                    "peak_nominal": peak_nominal, "frac_of_nominal": fl / avg_s / 1e12 / peak_nominal,
+                    "traffic": traffic, "traffic_source": traffic_source,
+                    "smem": {"achieved": smem_by / avg_s / 1e9, "peak": smem_peak, "unit": "GB/s", "frac": smem_by / avg_s / 1e9 / smem_peak,
+                             "note": f"algorithmic shared-memory bytes = {smem_bytes_per_field_point_zstep(w.precision):.0f} B per field-point z-step "
+                                     "(6 passes x read + write); peak = conflict-free 16 B loads + stores on every SM, measured in this run"},
+                    "note": f"peak = {'FP64' if dbl else 'FP32'} FMA throughput measured in this run by opo_selftest_peak (independent FMA chains on every SM); "
+                            f"peak_nominal = {sms} SM x {64 if dbl else 128} lanes x 2 x {sm_max_ghz:.3f} GHz; "
                             f"algorithmic flops = {flops_per_grid_point_zstep(w.log2_n, w.n_fields):.0f}/grid-point z-step "
                             "(merged half-steps, 5 N log2 N per transform); one launch = one step"}
     else:
@@ -321,7 +334,7 @@ def main():
         peak = float(peaks.get("hbm_gbs", 6543.1))
         n_launch = max(1, int(launches) // max(1, args.steps))
         roofline = {"bound": "hbm", "kernel": "k_large" if eng == P.ENGINE_LARGE else ("cufft+k_multab+k_rk4" if eng == P.ENGINE_CUFFT else "k_linear+k_rk4"), "achieved": by / avg_s / 1e9,
-                    "peak": peak, "unit": "GB/s", "frac": by / avg_s / 1e9 / peak, "traffic": traffic,
+                    "peak": peak, "unit": "GB/s", "frac": by / avg_s / 1e9 / peak, "traffic": traffic, "traffic_source": traffic_source,
                     "note": f"algorithmic bytes = {per_fp} B per field-point z-step; peak = measured HBM copy bandwidth "
                             f"({'MEASURED_PEAKS.json' if peaks else 'B200_PROFILING.md fallback'}); {n_launch} launch(es) per step; "
                             "the state of this workload is L2-resident, so this is L2 service measured against the HBM roofline"}

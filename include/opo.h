@@ -219,6 +219,17 @@ int opo_set_option(opo_handle* h, int option, int value);
 #define OPO_INFO_SLOTS 5           /* co-resident work slots (clusters / CTAs) the next roundtrips call deals its work to */
 int opo_get_info(const opo_handle* h, int what, long long* out);
 
+/* Device peaks measured on the spot with the library's own micro-benchmark kernels, the roofline denominators bench.py
+ * reports against; independent of any handle, runs on the default stream of the current device
+ * and takes ~0.1 s.  FP32 / FP64: independent FMA chains on every SM [TFLOP/s]; SMEM: conflict-free 16-byte shared-memory
+ * loads + stores on every SM [GB/s]; TMEM_LD / TMEM_ST: tcgen05.ld / tcgen05.st of a thread's own columns [GB/s]. */
+#define OPO_PEAK_FP32_FMA 0
+#define OPO_PEAK_FP64_FMA 1
+#define OPO_PEAK_SMEM 2
+#define OPO_PEAK_TMEM_LD 3
+#define OPO_PEAK_TMEM_ST 4
+int opo_selftest_peak(int what, double* out_value);
+
 /* Last error text of this handle (or of the failed opo_create when h is NULL).  Never NULL. */
 const char* opo_last_error(const opo_handle* h);
 

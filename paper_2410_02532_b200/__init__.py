@@ -87,6 +87,7 @@ def lib() -> ctypes.CDLL:
         L.opo_get_z_steps.argtypes = [vp, ctypes.POINTER(ci)]
         L.opo_set_option.argtypes = [vp, ci, ci]
         L.opo_get_info.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_longlong)]
+        L.opo_selftest_peak.argtypes = [ci, ctypes.POINTER(ctypes.c_double)]
         L.opo_last_error.argtypes = [vp]
         L.opo_last_error.restype = ctypes.c_char_p
         for name in EXPORTS:
@@ -99,7 +100,7 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_eom", "opo_set_beta3", "opo_set_pump",
            "opo_set_pump_host", "opo_set_field", "opo_set_field_host", "opo_propagate", "opo_roundtrips", "opo_roundtrips_train",
            "opo_get_fields", "opo_get_fields_host", "opo_sync", "opo_check_finite", "opo_get_z_steps",
-           "opo_set_option", "opo_get_info", "opo_last_error"]
+           "opo_set_option", "opo_get_info", "opo_selftest_peak", "opo_last_error"]
 
 
 def _check(handle, status: int):
@@ -205,6 +206,16 @@ def opo_get_z_steps(h) -> int:
 
 def opo_set_option(h, option: int, value: int):
     _check(h, lib().opo_set_option(h, option, value))
+
+
+PEAK_FP32_FMA, PEAK_FP64_FMA, PEAK_SMEM, PEAK_TMEM_LD, PEAK_TMEM_ST = 0, 1, 2, 3, 4
+
+
+def opo_selftest_peak(what: int) -> float:
+    """Device peak measured by the library's own micro-benchmark kernels (TFLOP/s or GB/s, see include/opo.h)."""
+    out = ctypes.c_double()
+    _check(None, lib().opo_selftest_peak(what, ctypes.byref(out)))
+    return out.value
 
 
 def opo_get_info(h, what: int) -> int:

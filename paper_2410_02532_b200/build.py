@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libopo.so")
-PLAIN_SOURCES = ["opo_api.cu", "opo_dispatch.cu", "opo_pointwise.cu"]
+PLAIN_SOURCES = ["opo_api.cu", "opo_dispatch.cu", "opo_pointwise.cu", "opo_selftest.cu"]
 # (type, suffix, log2 N): one object per size-specialised instance of opo_inst.cu
 INSTANCES = [("float", "f32", l) for l in range(6, 15)] + [("double", "f64", l) for l in range(6, 14)]
 LARGE_INSTANCES = [("float", "f32", l) for l in range(15, 19)] + [("double", "f64", l) for l in range(14, 19)]

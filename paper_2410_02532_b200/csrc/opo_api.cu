@@ -320,7 +320,7 @@ int build_tables(opo_handle* h) {
             if (cudaMalloc(&h->tabGM[x], need * N * h->tab_esz) != cudaSuccess ||
                 cudaMalloc(&h->tabHB[x], need * N * h->tab_esz) != cudaSuccess ||
                 cudaMalloc(&h->tabHG[x], need * N * h->tab_esz) != cudaSuccess)
-                return fail(h, OPO_ERR_ALLOC, "cudaMalloc of boundary tables failed");
+            { cudaGetLastError(); return fail(h, OPO_ERR_ALLOC, "cudaMalloc of boundary tables failed"); }
             h->tabB_count[x] = need;
         }
         bool any_fft = false;
@@ -605,9 +605,11 @@ namespace {
         ++(h)->launches;                                                                   \
     } while (0)
 
-// surface a sticky asynchronous fault from earlier work without synchronising
+// Surface an error left by earlier asynchronous work without synchronising.  The CUDA "last error" is per host thread, not
+// per handle: it is reported once and cleared (cudaGetLastError), so a non-sticky error -- somebody's failed allocation or
+// launch -- does not fail every later call on every handle; a sticky one (a device fault) keeps coming back by itself.
 int check_async(opo_handle* h) {
-    cudaError_t e = cudaPeekAtLastError();
+    cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, OPO_ERR_CUDA, std::string("earlier asynchronous fault: ") + cudaGetErrorString(e));
     return OPO_OK;
 }
@@ -763,16 +765,27 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     // more instances than clusters and not a multiple: deal round trips instead of instances (see the kernel)
     a.split = 0; a.flags = nullptr;
     if (mode == 1 && !h->splitting && steps > 1 && h->B > n_clusters && h->B % n_clusters != 0) {
-        if (!h->rt_flags && cudaMalloc((void**)&h->rt_flags, (size_t)h->B * 3 * sizeof(int)) != cudaSuccess)
+        if (!h->rt_flags && cudaMalloc((void**)&h->rt_flags, (size_t)h->B * 3 * sizeof(int)) != cudaSuccess) {
+            cudaGetLastError();
             return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the round-trip flags failed");
+        }
         OPO_CUDA(h, cudaMemsetAsync(h->rt_flags, 0, (size_t)h->B * 3 * sizeof(int), h->stream));
         a.split = 1; a.flags = h->rt_flags;
     }
-    if (solo)
-        OPO_LAUNCH(h, h->dbl ? opo::launch_solo_f64(h->L, a, n_clusters, h->stream) : opo::launch_solo_f32(h->L, a, n_clusters, h->stream));
-    else
-        OPO_LAUNCH(h, h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream)
-                             : opo::launch_resident_f32(h->L, a, n_clusters, h->stream));
+    auto launch = [&]() {
+        if (solo) return h->dbl ? opo::launch_solo_f64(h->L, a, n_clusters, h->stream) : opo::launch_solo_f32(h->L, a, n_clusters, h->stream);
+        return h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream) : opo::launch_resident_f32(h->L, a, n_clusters, h->stream);
+    };
+    cudaError_t e = launch();
+    if (e != cudaSuccess && a.split) {
+        // the split schedule needs every cluster / CTA of the grid resident (cooperative launch); if the device cannot
+        // promise that right now, deal whole instances instead -- slower by the ragged last wave, never a hang
+        cudaGetLastError();
+        a.split = 0; a.flags = nullptr;
+        e = launch();
+    }
+    if (e != cudaSuccess) return fail(h, OPO_ERR_CUDA, std::string("launch of the on-chip kernel: ") + cudaGetErrorString(e));
+    ++h->launches;
     return OPO_OK;
 }
 
@@ -846,9 +859,10 @@ int copy_in(opo_handle* h, void* dst_field, const void* src, bool per_instance, 
     if (per_instance) {
         OPO_CUDA(h, cudaMemcpyAsync(dst_field, src, one * h->B, kind, h->stream));
     } else {
+        // one slice in, one kernel replicates it to every instance
         OPO_CUDA(h, cudaMemcpyAsync(dst_field, src, one, kind, h->stream));
-        for (int b = 1; b < h->B; ++b)
-            OPO_CUDA(h, cudaMemcpyAsync((char*)dst_field + b * one, dst_field, one, cudaMemcpyDeviceToDevice, h->stream));
+        if (h->B > 1)
+            OPO_LAUNCH(h, h->dbl ? opo::launch_broadcast_f64(dst_field, h->B, h->N, h->stream) : opo::launch_broadcast_f32(dst_field, h->B, h->N, h->stream));
     }
     return OPO_OK;
 }
@@ -993,8 +1007,10 @@ int opo_set_eom(opo_handle* h, int field, double beta_rad, double f_mod_hz) {
         if (h->eom[field]) { OPO_CUDA(h, cudaStreamSynchronize(h->stream)); cudaFree(h->eom[field]); h->eom[field] = nullptr; }
         return OPO_OK;
     }
-    if (!h->eom[field] && cudaMalloc(&h->eom[field], (size_t)h->N * h->esz) != cudaSuccess)
+    if (!h->eom[field] && cudaMalloc(&h->eom[field], (size_t)h->N * h->esz) != cudaSuccess) {
+        cudaGetLastError();
         return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the modulator table failed");
+    }
     std::vector<cd> E(h->N);
     const double dt = h->grid.window_s / (double)h->N;
     for (int n = 0; n < h->N; ++n) {

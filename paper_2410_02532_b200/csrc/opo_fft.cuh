@@ -676,6 +676,21 @@ __device__ __forceinline__ void forward_only_smem(cplx<T>* sm, const cplx<T>* tw
     fwd_pass_smem<T, L, plan<L>::P - 1, NT, false>(sm, tw, tid);
 }
 
+// cudaFuncSetAttribute is per device: remember per (function, device) that it has been done
+struct device_once {
+    bool done[64] = {};
+    // true if `set` still has to run for the current device (and marks it done when `set` succeeds)
+    template <class F> cudaError_t run(F&& set) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64 && done[dev]) return cudaSuccess;
+        e = set();
+        if (e == cudaSuccess && dev >= 0 && dev < 64) done[dev] = true;
+        return e;
+    }
+};
+
 // threads per CTA for a 2^L-point field: 32 points per thread for large fields (keeps the register
 // budget at 128+/thread for the radix-16 butterflies), 16 for small ones
 template <class T, int L> struct cta_threads {

@@ -154,6 +154,7 @@ struct LargeInfo {
     cudaError_t launch_multab_##SUFFIX(const MulTabArgs& a, cudaStream_t s);            \
     cudaError_t launch_freq_##SUFFIX(int log2n, const FreqArgs& a, cudaStream_t s);     \
     cudaError_t launch_finite_##SUFFIX(const void* A, long long count, int* flag, cudaStream_t s); \
+    cudaError_t launch_broadcast_##SUFFIX(void* dst, int batch, int n, cudaStream_t s); \
     cudaError_t resident_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);     \
     cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
     cudaError_t solo_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);         \

@@ -157,6 +157,14 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value) k_freq(FreqArgs a) {
     for (int i = tid; i < N; i += NT) dst[__ldg(&a.perm[i])] = sm[phys<T>(i)];
 }
 
+// dst[b][i] = dst[0][i], b = 1 .. batch-1 (one input broadcast to every instance: opo_set_pump with per_instance = 0)
+template <class T>
+__global__ void __launch_bounds__(256) k_broadcast(cplx<T>* dst, int batch, int n) {
+    const long long total = (long long)(batch - 1) * n;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x)
+        dst[n + i] = dst[i % n];
+}
+
 template <class T>
 __global__ void __launch_bounds__(256) k_finite(const T* A, long long count, int* flag) {
     int bad = 0;
@@ -171,31 +179,31 @@ __global__ void __launch_bounds__(256) k_finite(const T* A, long long count, int
 template <class T, int L> cudaError_t launch_linear_L(const LinArgs& a, cudaStream_t s) {
     constexpr int NT = cta_threads<T, L>::value;
     const size_t smem = (size_t)padded_len<T>(1 << L) * sizeof(cplx<T>);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_linear<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static device_once once;
+    cudaError_t e = once.run([&] { return cudaFuncSetAttribute(k_linear<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); });
+    if (e != cudaSuccess) return e;
     k_linear<T, L><<<a.n_slots * a.batch, NT, smem, s>>>(a);
     return cudaGetLastError();
 }
 template <class T, int L> cudaError_t launch_freq_L(const FreqArgs& a, cudaStream_t s) {
     constexpr int NT = cta_threads<T, L>::value;
     const size_t smem = (size_t)padded_len<T>(1 << L) * sizeof(cplx<T>);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_freq<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static device_once once;
+    cudaError_t e = once.run([&] { return cudaFuncSetAttribute(k_freq<T, L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); });
+    if (e != cudaSuccess) return e;
     k_freq<T, L><<<a.batch, NT, smem, s>>>(a);
     return cudaGetLastError();
 }
 
+// grid of a grid-stride pointwise kernel: enough CTAs for 16 per SM of the current device
 inline int grid_for(long long total, int block) {
+    static int sms[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) dev = 0;
+    if (sms[dev] == 0 && cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms[dev] = 148;
     long long g = (total + block - 1) / block;
-    const long long cap = 148LL * 16;
+    const long long cap = (long long)sms[dev] * 16;
     return (int)(g < 1 ? 1 : (g > cap ? cap : g));
 }
 
@@ -211,6 +219,11 @@ template <class T> cudaError_t launch_scale_T(const ScaleArgs& a, cudaStream_t s
 }
 template <class T> cudaError_t launch_multab_T(const MulTabArgs& a, cudaStream_t s) {
     k_multab<T><<<grid_for((long long)a.batch * a.n, 256), 256, 0, s>>>(a);
+    return cudaGetLastError();
+}
+template <class T> cudaError_t launch_broadcast_T(void* dst, int batch, int n, cudaStream_t s) {
+    if (batch <= 1) return cudaSuccess;
+    k_broadcast<T><<<grid_for((long long)(batch - 1) * n, 256), 256, 0, s>>>(reinterpret_cast<cplx<T>*>(dst), batch, n);
     return cudaGetLastError();
 }
 template <class T> cudaError_t launch_finite_T(const void* A, long long count, int* flag, cudaStream_t s) {

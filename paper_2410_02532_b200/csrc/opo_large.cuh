@@ -415,14 +415,9 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
 }
 
 template <class T, int L, int F> cudaError_t large_setup() {
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_large<T, L, F>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)large_cfg<T, L, F>::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    return cudaSuccess;
+    static device_once once;
+    return once.run([&] { return cudaFuncSetAttribute(k_large<T, L, F>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                      (int)large_cfg<T, L, F>::SMEM_BYTES); });
 }
 
 template <class T, int L, int F> cudaError_t large_info_LF(int batch, int sm_count, LargeInfo* out) {

@@ -464,12 +464,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
 template <class T, int L, int F> cudaError_t resident_cfg(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, int n_clusters, cudaStream_t s) {
     constexpr int NT = cta_threads<T, L>::value;
     const size_t smem = res_layout<T, L, F>::total;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_resident<T, L, F, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    static device_once once;
+    cudaError_t e0 = once.run([&] { return cudaFuncSetAttribute(k_resident<T, L, F, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); });
+    if (e0 != cudaSuccess) return e0;
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = F;
     attr[0].val.clusterDim.y = 1;
@@ -485,7 +482,7 @@ template <class T, int L, int F> cudaError_t resident_cfg(cudaLaunchConfig_t* cf
 
 template <class T, int L, int F> cudaError_t resident_info_LF(ResidentInfo* out) {
     cudaLaunchConfig_t cfg{};
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     cudaError_t e = resident_cfg<T, L, F>(&cfg, attr, 1, nullptr);
     if (e != cudaSuccess) return e;
     int n = 0;
@@ -501,20 +498,25 @@ template <class T, int L> cudaError_t resident_info_L(int n_fields, ResidentInfo
     return n_fields == 3 ? resident_info_LF<T, L, 3>(out) : resident_info_LF<T, L, 2>(out);
 }
 
-// NLN = true is instantiated in its own translation units (opo_inst_nln.cu): the default kernel's object code stays
-// byte for byte what it is without the N/2 - L - N/2 ordering
+// NLN = true and DK0 = true are instantiated in their own objects (opo_inst.cu with -DOPO_NLN / -DOPO_DK0): the default
+// kernel's object code stays byte for byte what it is without the N/2 - L - N/2 ordering.
+// With a.split the launch is cooperative: the round-trip split schedule spins on a flag another cluster sets, which is
+// safe only if every cluster of the grid is resident; a cooperative launch fails (cudaErrorCooperativeLaunchTooLarge)
+// instead of hanging when that cannot be guaranteed, and the host then launches without the split.
 template <class T, int L, int F, bool NLN, bool DK0 = false> cudaError_t launch_resident_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
     cudaLaunchConfig_t cfg{};
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     cudaError_t e = resident_cfg<T, L, F>(&cfg, attr, n_clusters, s);
     if (e != cudaSuccess) return e;
     if constexpr (NLN || DK0) {
-        static bool configured = false;
-        if (!configured) {
-            e = cudaFuncSetAttribute(k_resident<T, L, F, NLN, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.dynamicSmemBytes);
-            if (e != cudaSuccess) return e;
-            configured = true;
-        }
+        static device_once once;
+        e = once.run([&] { return cudaFuncSetAttribute(k_resident<T, L, F, NLN, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.dynamicSmemBytes); });
+        if (e != cudaSuccess) return e;
+    }
+    if (a.split) {
+        attr[1].id = cudaLaunchAttributeCooperative;
+        attr[1].val.cooperative = 1;
+        cfg.numAttrs = 2;
     }
     return cudaLaunchKernelEx(&cfg, k_resident<T, L, F, NLN, DK0>, a);
 }

@@ -466,9 +466,8 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
 }
 
 template <class T, int L, int F, bool DK0> cudaError_t solo_setup() {
-    cudaError_t e = cudaFuncSetAttribute(k_solo<T, L, F, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)solo_layout<T, L, F>::total);
-    if (e != cudaSuccess) return e;
-    return cudaSuccess;
+    static device_once once;
+    return once.run([&] { return cudaFuncSetAttribute(k_solo<T, L, F, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)solo_layout<T, L, F>::total); });
 }
 
 template <class T, int L, int F> cudaError_t solo_info_LF(ResidentInfo* out) {

@@ -1,0 +1,145 @@
+"""Parity at the lengths BASELINE.json:north_star states, on all five configurations:
+
+  * every config truncated to 20 round trips: complex64 rel. L2 field error <= 1e-4 (C0: complex128, <= 1e-10, its full length)
+      C1 and C0 are in test_gpu_parity.py; here C2 with all 11 detunings, C3 (N = 2^18) and a 16-instance subset of C4
+      including the four sweep corners;
+  * the full-length noise-seeded runs: relative error <= 1e-3 on the output signal power and on the power spectrum
+      (not phase, reading R21): C1 x 1000, C2 x 500 (11 detunings), C4 x 300 (16-instance subset).
+
+Short oracle runs are computed in the test (all host cores); the long ones (minutes to tens of minutes of oracle) are
+read from tests/golden/*.npz, written by tests/golden/make_long_run_goldens.py, which calls only oracle/.  The file
+names carry a hash of the inputs: if the input recipe changes, the golden is not found and the test fails loudly.
+"""
+import glob
+import os
+import sys
+
+import numpy as np
+import pytest
+
+import opo_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+sys.path.insert(0, GOLDEN)
+
+
+def _gpu():
+    import torch
+    import paper_2410_02532_b200 as P
+    return torch, P
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def golden(stem, w):
+    from make_long_run_goldens import workload_hash
+    path = os.path.join(GOLDEN, f"{stem}_{workload_hash(w)}.npz")
+    assert os.path.exists(path), (f"{path} not found: the inputs of {w.name} changed (stale: {glob.glob(os.path.join(GOLDEN, stem + '_*.npz'))}); "
+                                  "re-run tests/golden/make_long_run_goldens.py")
+    return np.load(path)
+
+
+def run_gpu_exit(w, engine=None):
+    torch, P = _gpu()
+    o = P.from_workload(w, engine=P.ENGINE_AUTO if engine is None else engine)
+    o.roundtrips(w.n_roundtrips)
+    o.sync()
+    o.check_finite()
+    ex = np.stack([o.get_fields(x, P.WHICH_EXIT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1)
+    eng = o.engine
+    o.close()
+    return ex, eng
+
+
+# ---- 20 round trips, field error ------------------------------------------------------------------------------------
+
+def test_config2_all_detunings_20rt():
+    import oracle
+    w = W.config2().truncated(20)
+    ex, eng = run_gpu_exit(w)
+    ref = oracle.run_workload(w, threads=min(w.batch, os.cpu_count() or 1))["exit"]
+    worst = max(rel_l2(ex[b, x], ref[b, x]) for b in range(w.batch) for x in range(w.n_fields))
+    print(f"C2, 11 detunings x 20 RT (4000 z-steps), engine {eng}: worst rel L2 {worst:.3e}")
+    assert worst <= 1e-4
+
+
+def test_config4_subset16_20rt_both_onchip_engines():
+    import oracle
+    from make_long_run_goldens import C4_SUBSET
+    torch, P = _gpu()
+    w = W.config4().truncated(20).subset(C4_SUBSET)
+    ref = oracle.run_workload(w, threads=min(w.batch, os.cpu_count() or 1))["exit"]
+    for engine in (P.ENGINE_SOLO, P.ENGINE_RESIDENT):
+        ex, eng = run_gpu_exit(w, engine)
+        assert eng == engine
+        worst = max(rel_l2(ex[b, x], ref[b, x]) for b in range(w.batch) for x in range(w.n_fields))
+        print(f"C4, 16 instances incl. the 4 corners x 20 RT, engine {eng}: worst rel L2 {worst:.3e}")
+        assert worst <= 1e-4
+
+
+def test_config3_golden_20rt():
+    """C3 (N = 2^18, nz = 500): 10 000 z-steps on the large-N engine against the cached oracle result."""
+    torch, P = _gpu()
+    w = W.config3().truncated(20)
+    g = golden("c3_20rt", w)
+    ex, eng = run_gpu_exit(w)
+    assert eng == P.ENGINE_LARGE
+    e_p = rel_l2(ex[0, 0], g["exit_pump"].astype(np.complex128))
+    e_s = rel_l2(ex[0, 1], g["exit_signal"].astype(np.complex128))
+    print(f"C3 x 20 RT (10 000 z-steps): rel L2 pump {e_p:.3e} signal {e_s:.3e}")
+    assert e_p <= 1e-4 and e_s <= 1e-4
+
+
+# ---- full-length noise-seeded runs: output signal power and power spectrum -----------------------------------------------
+
+def _long_run(stem, w, engines):
+    torch, P = _gpu()
+    g = golden(stem, w)
+    assert int(g["n_roundtrips"]) == w.n_roundtrips
+    R_s = w.R[1]
+    out = {}
+    for engine in engines:
+        ex, eng = run_gpu_exit(w, engine)
+        p_out = (1.0 - R_s) * np.mean(np.abs(ex[:, 1]) ** 2, axis=1)
+        p_in = np.array([np.mean(np.abs(w.pump_of(b)) ** 2) for b in range(w.batch)])
+        depl = 1.0 - np.mean(np.abs(ex[:, 0]) ** 2, axis=1) / p_in
+        spec = np.abs(np.fft.fft(ex[:, 1], axis=1)) ** 2
+        e_p = np.abs(p_out - g["p_out"]) / g["p_out"]
+        e_s = np.array([rel_l2(spec[b], g["spectrum"][b].astype(np.float64)) for b in range(w.batch)])
+        e_d = np.abs(depl - g["depletion"])
+        f_p = np.abs(g["float_p_out"] - g["p_out"]) / g["p_out"] if "float_p_out" in g else np.zeros(1)
+        f_s = g["float_spectrum_rel_l2"] if "float_spectrum_rel_l2" in g else np.zeros(1)
+        print(f"{w.name} x {w.n_roundtrips} RT, engine {eng}: signal power rel err max {e_p.max():.3e}, power spectrum rel L2 max {e_s.max():.3e}, "
+              f"pump depletion abs err max {e_d.max():.3e} (depletion {g['depletion'].min():.3f}..{g['depletion'].max():.3f}); "
+              f"float oracle vs fp64 oracle (P12): power {f_p.max():.3e}, spectrum {f_s.max():.3e}")
+        out[eng] = (e_p, e_s, e_d)
+    return out
+
+
+def test_config1_full_length_power_and_spectrum():
+    torch, P = _gpu()
+    w = W.config1()
+    res = _long_run("c1_1000rt", w, [P.ENGINE_RESIDENT, P.ENGINE_SOLO])
+    for e_p, e_s, e_d in res.values():
+        assert e_p.max() <= 1e-3 and e_s.max() <= 1e-3
+
+
+def test_config2_full_length_power_and_spectrum():
+    torch, P = _gpu()
+    w = W.config2()
+    res = _long_run("c2_500rt", w, [P.ENGINE_AUTO])
+    for e_p, e_s, e_d in res.values():
+        assert e_p.max() <= 1e-3 and e_s.max() <= 1e-3
+
+
+def test_config4_subset16_full_length_power_and_spectrum():
+    from make_long_run_goldens import C4_SUBSET
+    torch, P = _gpu()
+    w = W.config4().subset(C4_SUBSET)
+    res = _long_run("c4_300rt_sub16", w, [P.ENGINE_SOLO, P.ENGINE_RESIDENT])
+    for e_p, e_s, e_d in res.values():
+        assert e_p.max() <= 1e-3 and e_s.max() <= 1e-3

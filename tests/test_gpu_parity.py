@@ -538,7 +538,8 @@ def test_large_boundary_without_transform_and_nonresonant_restart():
 
 def test_config3_one_roundtrip_c64():
     """BASELINE.json configs[3] at its full grid (N = 2^18, nz = 500), one round trip (the oracle needs
-    ~20 s for it; 20 round trips are covered by sampled golden values, test_config3_golden_20rt)."""
+    ~20 s for it; 20 round trips are compared against the cached oracle result in
+    tests/test_gpu_config_length.py::test_config3_golden_20rt)."""
     torch, P = _gpu()
     w = W.config3().truncated(1)
     cur, ex, eng = run_gpu(w, P.ENGINE_AUTO)
