@@ -74,6 +74,9 @@ class Workload:
     beta3_s3_per_m: List[float] = field(default_factory=lambda: [0.0, 0.0, 0.0])
     # operator splitting: 0 = L/2 - N - L/2 (default), 1 = N/2 - L - N/2 (the paper's Eq. 10-11)
     splitting: int = 0
+    # several crystals in series (reading R25): list of (length_m, dk_per_m, d_eff_m_per_V, nz) or None for
+    # the single crystal (length_m, dk_per_m, d_eff_m_per_V, nz_per_pass); nz_per_pass must then be the sum of the nz
+    segments: Optional[list] = None
 
     @property
     def n(self) -> int:

@@ -47,6 +47,8 @@ def lib():
         L.opo_oracle_set_eom.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double]
         L.opo_oracle_set_beta3.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double]
         L.opo_oracle_set_splitting.argtypes = [ctypes.c_void_p, ctypes.c_int]
+        L.opo_oracle_set_segments.argtypes = [ctypes.c_void_p, ctypes.c_int, _DP, _DP, _DP, _IP]
+        L.opo_oracle_set_segments.restype = ctypes.c_int
         L.opo_oracle_propagate.argtypes = [ctypes.c_void_p, ctypes.c_int]
         L.opo_oracle_propagate.restype = ctypes.c_int
         L.opo_oracle_roundtrips.argtypes = [ctypes.c_void_p, ctypes.c_int]
@@ -130,6 +132,13 @@ class OracleOpo:
         """Third-order dispersion of a field (Eq. 5 in the reading R7)."""
         lib().opo_oracle_set_beta3(self._h, int(field), float(beta3_s3_per_m))
 
+    def set_segments(self, segments) -> int:
+        """Crystal segments in series (PAPER.md:L447; reading R25): a list of (length_m, dk_per_m, d_eff_m_per_V, nz);
+        an empty list restores the single crystal of the constructor.  Only at the start of a pass."""
+        n = len(segments)
+        return lib().opo_oracle_set_segments(self._h, n, _darr([s[0] for s in segments], max(n, 1)), _darr([s[1] for s in segments], max(n, 1)),
+                                             _darr([s[2] for s in segments], max(n, 1)), _iarr([s[3] for s in segments], max(n, 1)))
+
     def set_eom(self, field: int, beta_rad: float, f_hz: float):
         """Intracavity phase modulator on a resonant field; beta = 0 switches it off."""
         lib().opo_oracle_set_eom(self._h, int(field), float(beta_rad), float(f_hz))
@@ -172,6 +181,12 @@ def from_workload(w, b: int = 0, use_float: bool = False) -> OracleOpo:
             o.set_beta3(x, w.beta3_s3_per_m[x])
     if w.splitting:
         o.set_splitting(w.splitting)
+    if getattr(w, "segments", None):
+        # per-instance dk sweeps apply to the first segment (include/opo.h, OPO_PARAM_DK)
+        segs = [tuple(sg) for sg in w.segments]
+        if len(w.dk_per_m) > 1:
+            segs[0] = (segs[0][0], w.dk_of(b), segs[0][2], segs[0][3])
+        assert o.set_segments(segs) == 0
     return o
 
 

@@ -27,6 +27,11 @@
 //                        A_x[n] <- A_x[n] exp(i beta_x sin(2 pi f_x tau_n))   intracavity EOM, last element
 //                                  (Listing 3; off when beta_x = 0)
 //        non-resonant x: A_x <- S_x   (stored input: fresh pump / frozen seed)
+//        resonant pump (x = 0, reading R24): the input coupler adds the external pump,
+//                        A_p <- [boundary of a resonant field] + sqrt(1 - R_p) S_p     (R_p = 0 is the single-pass rule above)
+//   several crystals in series ("one or more nonlinear media", reading R25): a pass is a
+//        sequence of segments (length L_j, dk_j, d_eff_j, nz_j); each is walked with its own h_j = L_j / nz_j,
+//        kappa_x = 2 pi d_eff_j / (n_x lambda_x) and dk_j, z measured from the segment's own entrance
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): P1 naive DFT, P2 Gaussian GVD closed form, P3 GVM
 // integer shift, P4 cosh^2 gain (+dk), P5 degenerate phase-sensitive gain (paper's pi/4, -3pi/4,
@@ -36,7 +41,11 @@
 // second-order convergence, O(h^2) agreement with L/2-N-L/2, exact agreement when the operators commute,
 // P16 loss: power falls as exp(-alpha_x z), a pure scale (alpha/2 on the amplitude, Eq. 5), P17 pump re-injection: after
 // the boundary the pump is the stored input bit for bit and round trip 2 equals a hand-composed single pass (L268, R11),
-// P18 z restarts at the crystal entrance every pass with dk != 0 (R4): round trips = passes on fresh oracles.
+// P18 z restarts at the crystal entrance every pass with dk != 0 (R4): round trips = passes on fresh oracles,
+// P19 resonant pump: cold-cavity build-up to the closed-form Airy steady state sqrt(1-R) S / (1 - sqrt(R) e^{i delta} G e^{i D L})
+// per bin, geometric partial sums on the way, R_p = 0 equals the single-pass rule,
+// P20 crystal segments: a crystal cut in two equal-parameter segments with dk = 0 equals the uncut crystal; with dk != 0 it
+// equals two single passes chained by hand; a second segment with d_eff -> -d_eff undoes the first one (dispersion off).
 // Parity unpinned: reading R12 (non-resonant fields restart from
 // S_x) is a convention with no physical pin; the paper's P_th values (L348) and Figs 3-5.
 // =================================================================================================
@@ -114,6 +123,10 @@ struct Params {
     int splitting;                  // 0: L/2 - N - L/2 (north_star, default); 1: N/2 - L - N/2 (the paper's Eq. 10-11)
     double beta3[3];                // third-order dispersion of field x [s^3/m] (Eq. 5; reading R7), 0 unless set
     double eom_beta[3], eom_f[3];   // intracavity phase modulator: depth [rad], frequency [Hz]
+    // crystal segments in series (reading R25); n_seg = 0 means the single crystal (length_m, dk_per_m, d_eff, nz)
+    int n_seg;
+    double seg_len[8], seg_dk[8], seg_deff[8];
+    int seg_nz[8];
 };
 
 template <class R>
@@ -121,12 +134,26 @@ struct Oracle {
     using C = std::complex<R>;
     Params p;
     int N, F;
-    double h;       // dz = L / nz
-    double z;       // position inside the crystal, 0 at the entrance (R4, R20)
-    double kappa[3];
+    double h;       // dz = L / nz of the current segment
+    double z;       // position inside the current crystal segment, 0 at its entrance (R4, R20, R25)
+    double kappa[3];            // of the current segment
+    int K;                      // number of segments
+    int seg, seg_step;          // current segment and z-steps taken inside it
+    double seg_h[8], seg_kappa[8][3];
     Fft<R> fft;
-    std::vector<C> A[3], S[3], EX[3], H[3], HF[3], G[3];
+    std::vector<C> A[3], S[3], EX[3], G[3];
+    std::vector<C> Hs[8][3], HFs[8][3];     // half-step / full-step multipliers per segment
     bool boundary_needs_transform[3];
+
+    double seg_len(int j) const { return p.n_seg ? p.seg_len[j] : p.length_m; }
+    double seg_dk(int j) const { return p.n_seg ? p.seg_dk[j] : p.dk_per_m; }
+    double seg_deff(int j) const { return p.n_seg ? p.seg_deff[j] : p.d_eff; }
+    int seg_nz(int j) const { return p.n_seg ? p.seg_nz[j] : p.nz; }
+    int steps_per_pass() const { int t = 0; for (int j = 0; j < K; ++j) t += seg_nz(j); return t; }
+    void enter_segment(int j) {
+        seg = j; seg_step = 0; z = 0.0; h = seg_h[j];
+        for (int x = 0; x < F; ++x) kappa[x] = seg_kappa[j][x];
+    }
 
     // Omega_k = 2 pi k' / (N dt), natural FFT order, Nyquist bin negative (R9)
     double omega(int k) const {
@@ -139,12 +166,9 @@ struct Oracle {
         p = pp;
         F = p.n_fields;
         N = 1 << p.log2n;
-        h = p.length_m / (double)p.nz;
-        z = 0.0;
+        seg = 0; seg_step = 0; z = 0.0;
         fft.init(p.log2n);
         for (int x = 0; x < F; ++x) {
-            // kappa_x = 2 pi d_eff / (n_x lambda_x)                               PAPER.md:L97
-            kappa[x] = 2.0 * kPi * p.d_eff / (p.n_index[x] * p.lambda_m[x]);
             A[x].assign(N, C(0, 0));
             S[x].assign(N, C(0, 0));
             EX[x].assign(N, C(0, 0));
@@ -153,9 +177,19 @@ struct Oracle {
     }
 
     void build_tables() {
+        K = p.n_seg ? p.n_seg : 1;
+        for (int j = 0; j < K; ++j) {
+            seg_h[j] = seg_len(j) / (double)seg_nz(j);             // dz = L_j / nz_j
+            // kappa_x = 2 pi d_eff / (n_x lambda_x)                                          PAPER.md:L97
+            for (int x = 0; x < F; ++x) seg_kappa[j][x] = 2.0 * kPi * seg_deff(j) / (p.n_index[x] * p.lambda_m[x]);
+        }
+        for (int j = 0; j < K; ++j)
         for (int x = 0; x < F; ++x) {
-            H[x].resize(N);
-            HF[x].resize(N);
+            std::vector<C>& H = Hs[j][x];
+            std::vector<C>& HF = HFs[j][x];
+            const double h = seg_h[j];
+            H.resize(N);
+            HF.resize(N);
             G[x].resize(N);
             double db1 = p.beta1[x] - p.beta1[p.ref_field];       // Delta beta1_x (R7, R10)
             for (int k = 0; k < N; ++k) {
@@ -166,29 +200,32 @@ struct Oracle {
                 double D = -db1 * om + 0.5 * p.beta2[x] * om * om - p.beta3[x] / 6.0 * om * om * om;
                 // H_x = exp( (-alpha_x/2 + i D_x) h/2 )                              half step
                 std::complex<double> e = std::exp(std::complex<double>(-0.5 * p.alpha[x], D) * (0.5 * h));
-                H[x][k] = C((R)e.real(), (R)e.imag());
+                H[k] = C((R)e.real(), (R)e.imag());
                 // full step exp( (-alpha_x/2 + i D_x) h ), used by the N/2 - L - N/2 ordering (Eq. 11)
                 std::complex<double> ef = std::exp(std::complex<double>(-0.5 * p.alpha[x], D) * h);
-                HF[x][k] = C((R)ef.real(), (R)ef.imag());
+                HF[k] = C((R)ef.real(), (R)ef.imag());
                 // G_x = exp( i (gamma_x/2) Omega^2 - i Omega DeltaT_x )              L145, R13, R14
                 double ph = 0.5 * p.gdd[x] * om * om - om * p.delta_T[x];
                 G[x][k] = C((R)std::cos(ph), (R)std::sin(ph));
             }
             boundary_needs_transform[x] = (p.gdd[x] != 0.0) || (p.delta_T[x] != 0.0);   // L284
         }
+        // the position inside the pass is kept; step size and couplings are those of the current segment
+        h = seg_h[seg];
+        for (int x = 0; x < F; ++x) kappa[x] = seg_kappa[seg][x];
     }
 
     void linear_half_step() {
         for (int x = 0; x < F; ++x) {
             fft.transform(A[x].data(), false);
-            for (int k = 0; k < N; ++k) A[x][k] = A[x][k] * H[x][k];
+            for (int k = 0; k < N; ++k) A[x][k] = A[x][k] * Hs[seg][x][k];
             fft.transform(A[x].data(), true);
         }
     }
 
     // right-hand side of Eqs 2-4 without L, at position zz
     void rhs(double zz, const C* y, C* f) const {
-        double ph = p.dk_per_m * zz;
+        double ph = seg_dk(seg) * zz;                  // dk of the current crystal segment, z from its entrance
         C em((R)std::cos(ph), (R)(-std::sin(ph)));    // e^{-i dk z}
         C ep((R)std::cos(ph), (R)(std::sin(ph)));     // e^{+i dk z}
         const C I(0, 1);
@@ -207,7 +244,7 @@ struct Oracle {
     void linear_full_step() {
         for (int x = 0; x < F; ++x) {
             fft.transform(A[x].data(), false);
-            for (int k = 0; k < N; ++k) A[x][k] = A[x][k] * HF[x][k];
+            for (int k = 0; k < N; ++k) A[x][k] = A[x][k] * HFs[seg][x][k];
             fft.transform(A[x].data(), true);
         }
     }
@@ -242,14 +279,32 @@ struct Oracle {
             nonlinear_step(z + 0.5 * h, 0.5 * h);
         }
         z += h;
+        ++seg_step;
+    }
+
+    bool at_pass_start() const { return seg == 0 && seg_step == 0; }
+    // one z-step of the pass; moves on to the next crystal segment when the current one is finished.
+    // false if the pass is already complete
+    bool pass_step() {
+        while (seg_step >= seg_nz(seg)) {
+            if (seg + 1 >= K) return false;
+            enter_segment(seg + 1);
+        }
+        z_step();
+        return true;
+    }
+
+    int steps_done() const {
+        int t = seg_step;
+        for (int j = 0; j < seg; ++j) t += seg_nz(j);
+        return t;
     }
 
     int propagate(int nsteps) {
         if (nsteps < 0) return 1;
-        // error if it would pass z = L
-        double zend = z + nsteps * h;
-        if (zend > p.length_m * (1.0 + 1e-9)) return 5;
-        for (int s = 0; s < nsteps; ++s) z_step();
+        // error if it would pass the end of the last crystal
+        if (steps_done() + nsteps > steps_per_pass()) return 5;
+        for (int s = 0; s < nsteps; ++s) pass_step();
         return 0;
     }
 
@@ -275,19 +330,26 @@ struct Oracle {
                         A[x][n] = A[x][n] * C((R)std::cos(ph), (R)std::sin(ph));
                     }
                 }
+                // resonant pump (reading R24): the input coupler of power reflectivity R_p transmits the external pump S_p
+                if (x == 0) {
+                    R t = (R)std::sqrt(1.0 - p.R[x]);
+                    for (int n = 0; n < N; ++n) A[x][n] = A[x][n] + t * S[x][n];
+                }
             } else {
                 A[x] = S[x];
             }
         }
+        enter_segment(0);
         z = 0.0;
     }
 
     int roundtrips(int n) {
         if (n < 0) return 1;
-        if (z != 0.0) return 5;
+        if (!at_pass_start()) return 5;
         for (int m = 0; m < n; ++m) {
+            enter_segment(0);
             z = 0.0;
-            for (int s = 0; s < p.nz; ++s) z_step();
+            while (pass_step()) {}
             boundary();
         }
         return 0;
@@ -367,6 +429,20 @@ void opo_oracle_set_beta3(void* h, int field, double beta3_s3_per_m) {
     Handle* hnd = (Handle*)h;
     if (hnd->is_float) { hnd->f->p.beta3[field] = beta3_s3_per_m; hnd->f->build_tables(); }
     else               { hnd->d->p.beta3[field] = beta3_s3_per_m; hnd->d->build_tables(); }
+}
+
+// crystal segments in series (reading R25); n = 0 restores the single crystal of opo_oracle_create.  Only at the start of a pass.
+int opo_oracle_set_segments(void* h, int n, const double* len, const double* dk, const double* deff, const int* nz) {
+    Handle* hnd = (Handle*)h;
+    if (n < 0 || n > 8) return 1;
+    for (int j = 0; j < n; ++j) if (!(len[j] > 0.0) || nz[j] <= 0) return 1;
+    auto apply = [&](Params& p) {
+        p.n_seg = n;
+        for (int j = 0; j < n; ++j) { p.seg_len[j] = len[j]; p.seg_dk[j] = dk[j]; p.seg_deff[j] = deff[j]; p.seg_nz[j] = nz[j]; }
+    };
+    if (hnd->is_float) { if (!hnd->f->at_pass_start()) return 5; apply(hnd->f->p); hnd->f->build_tables(); }
+    else               { if (!hnd->d->at_pass_start()) return 5; apply(hnd->d->p); hnd->d->build_tables(); }
+    return 0;
 }
 
 // intracavity phase modulator on (resonant) field x; beta = 0 switches it off

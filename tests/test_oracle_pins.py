@@ -818,3 +818,192 @@ def test_p18_dk_phase_restarts_at_the_crystal_entrance_every_round_trip():
         sig = _mirror(ex[1], R)
     for x in range(3):
         assert rel_l2(o.get_field(x, EXIT), ex[x]) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# P19  resonant pump (reading R24: the paper names triply resonant oscillators, without an
+#      injection rule): A_p <- sqrt(R_p) e^{i delta_p} IDFT(G_p DFT(A_p(L))) + sqrt(1 - R_p) S_p at every boundary
+# ---------------------------------------------------------------------------------------------
+
+def test_p19_cold_cavity_pump_builds_up_to_the_airy_steady_state():
+    """Coupling off (d_eff = 0): the intracavity pump after m boundaries, started from the transmitted input t S_p, is
+    the geometric partial sum  t S~[k] (1 - rho_k^{m+1}) / (1 - rho_k),  rho_k = sqrt(R) e^{i delta} G[k] e^{i D(Omega_k) L},
+    and converges to the Airy steady state  t S~[k] / (1 - rho_k)  per bin.  On resonance (delta = 0, bin 0) the
+    intracavity power is enhanced by (1 - R) / (1 - sqrt(R))^2."""
+    log2n, T, L, nz = 7, 10 * PS, 5e-3, 8
+    n = 1 << log2n
+    dt = T / n
+    Rp, delta, gdd, dT = 0.6, 0.4, 300 * FS * FS, -7 * FS
+    b1p, b2p = 0.05 * FS / UM, 0.35 * FS * FS / UM
+    o = make(n_fields=2, log2_n=log2n, window_s=T, nz=nz, length=L, d_eff=0.0, resonant=(1, 0), R=(Rp, 0),
+             delta_rad=(delta, 0), delta_T=(dT, 0), gdd=(gdd, 0), beta1=(b1p, 0.0), beta2=(b2p, 0.0), ref_field=1)
+    rng = np.random.default_rng(19)
+    S = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    t = math.sqrt(1 - Rp)
+    o.set_field(0, S, which="input")
+    o.set_field(0, t * S, which="state")
+    om = 2 * np.pi * np.fft.fftfreq(n, d=1.0 / n) / (n * dt)
+    rho = math.sqrt(Rp) * np.exp(1j * delta) * np.exp(1j * (gdd / 2) * om ** 2 - 1j * om * dT) * np.exp(1j * (-b1p * om + b2p / 2 * om ** 2) * L)
+    Sf = np.fft.fft(S)
+    done = 0
+    for m in (1, 2, 5, 40):
+        assert o.roundtrips(m - done) == 0
+        done = m
+        expect = np.fft.ifft(t * Sf * (1 - rho ** (m + 1)) / (1 - rho))
+        assert rel_l2(o.get_field(0), expect) < 1e-12
+    assert o.roundtrips(200) == 0                       # 0.6^120 ~ 1e-27: converged
+    airy = np.fft.ifft(t * Sf / (1 - rho))
+    assert rel_l2(o.get_field(0), airy) < 1e-12
+    # on resonance, CW input: power enhancement (1 - R) / (1 - sqrt(R))^2
+    o = make(n_fields=2, log2_n=4, nz=4, d_eff=0.0, resonant=(1, 0), R=(Rp, 0))
+    o.set_field(0, np.ones(16, complex), which="input")
+    o.set_field(0, t * np.ones(16, complex), which="state")
+    assert o.roundtrips(300) == 0
+    assert abs(abs(o.get_field(0)[0]) ** 2 / ((1 - Rp) / (1 - math.sqrt(Rp)) ** 2) - 1) < 1e-12
+
+
+def test_p19_single_pass_pump_is_the_r_equals_zero_case_and_signal_gets_no_injection():
+    """R_p = 0 with the pump flagged resonant gives exactly the single-pass rule A_p <- S_p (R11); the injection acts on
+    the pump only: a resonant signal is not topped up from its seed."""
+    log2n, nz = 5, 10
+    n = 1 << log2n
+    kw = dict(n_fields=3, log2_n=log2n, nz=nz, dk=30.0, beta2=(0.35 * FS * FS / UM, 0.12 * FS * FS / UM, 0.05 * FS * FS / UM))
+    a = make(resonant=(1, 1, 0), R=(0.0, 0.9, 0), **kw)
+    b = make(resonant=(0, 1, 0), R=(0.0, 0.9, 0), **kw)
+    ks = a.kappa(1)
+    amp = 0.8 / (ks * 5e-3)
+    rng = np.random.default_rng(191)
+    f = [amp * (0.7 + 0.3 * (rng.standard_normal(n) + 1j * rng.standard_normal(n))) for _ in range(3)]
+    for o in (a, b):
+        for x in range(3):
+            o.set_field(x, f[x] * (1.0, 0.2, 0.1)[x])
+        assert o.roundtrips(3) == 0
+    for x in range(3):
+        assert rel_l2(a.get_field(x), b.get_field(x)) < 1e-14
+        assert rel_l2(a.get_field(x, EXIT), b.get_field(x, EXIT)) < 1e-14
+    # cold cavity, signal resonant: pure decay, no source term
+    c = make(n_fields=2, log2_n=4, nz=4, d_eff=0.0, resonant=(0, 1), R=(0, 0.5))
+    c.set_field(0, np.zeros(16, complex))
+    c.set_field(1, np.ones(16, complex))
+    assert c.roundtrips(4) == 0
+    assert abs(abs(c.get_field(1)[0]) ** 2 - 0.5 ** 4) < 1e-14
+
+
+def test_p19_resonant_pump_with_coupling_composes_from_single_passes():
+    """Round trip 2 of a doubly resonant pump + signal equals a single pass fed by hand with
+    sqrt(R_p) e^{i delta_p} exit_p + sqrt(1 - R_p) S_p and sqrt(R_s) exit_s."""
+    log2n, nz, L = 5, 30, 5e-3
+    n = 1 << log2n
+    Rp, Rs, dp = 0.5, 0.8, 0.6
+    kw = dict(n_fields=2, log2_n=log2n, nz=nz, length=L, dk=40.0, resonant=(1, 1), R=(Rp, Rs), delta_rad=(dp, 0.0),
+              beta1=(0.3 * FS / UM, 0.0), beta2=(0.35 * FS * FS / UM, 0.10 * FS * FS / UM))
+    o = make(**kw)
+    ks = o.kappa(1)
+    amp = 1.0 / (ks * L)
+    rng = np.random.default_rng(192)
+    Sp = amp * (0.9 + 0.1 * (rng.standard_normal(n) + 1j * rng.standard_normal(n)))
+    Ss = 0.3 * amp * (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    o.set_field(0, Sp, which="input")
+    o.set_field(0, math.sqrt(1 - Rp) * Sp, which="state")
+    o.set_field(1, Ss)
+    assert o.roundtrips(1) == 0
+    ex = [o.get_field(x, EXIT) for x in range(2)]
+    nxt_p = _mirror(ex[0], Rp, dp) + math.sqrt(1 - Rp) * Sp
+    assert rel_l2(o.get_field(0), nxt_p) < 1e-14
+    assert o.roundtrips(1) == 0
+    c = make(**kw)
+    c.set_field(0, nxt_p)
+    c.set_field(1, _mirror(ex[1], Rs))
+    assert c.propagate(nz) == 0
+    for x in range(2):
+        assert rel_l2(o.get_field(x, EXIT), c.get_field(x)) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# P20  several crystals in series (PAPER.md:L447 "one or more nonlinear media"; SURVEY 8(f) N4; reading R25)
+# ---------------------------------------------------------------------------------------------
+
+def _p20_fields(n, amp, seed=20):
+    rng = np.random.default_rng(seed)
+    return [amp * s * (0.7 + 0.3 * (rng.standard_normal(n) + 1j * rng.standard_normal(n))) for s in (1.0, 0.4, 0.2)]
+
+
+def test_p20_a_crystal_cut_in_two_is_the_same_crystal_when_dk_is_zero():
+    """Two segments with the parameters of the whole crystal and dk = 0 are the uncut crystal step for step."""
+    log2n, L, nz = 6, 5e-3, 24
+    n = 1 << log2n
+    kw = dict(n_fields=3, log2_n=log2n, nz=nz, length=L, dk=0.0, beta1=(0.3 * FS / UM, 0.0, -0.17 * FS / UM),
+              beta2=(0.35 * FS * FS / UM, 0.12 * FS * FS / UM, 0.05 * FS * FS / UM), resonant=(0, 1, 0), R=(0, 0.9, 0))
+    a, b = make(**kw), make(**kw)
+    assert b.set_segments([(L * 10 / 24, 0.0, 14e-12, 10), (L * 14 / 24, 0.0, 14e-12, 14)]) == 0
+    amp = 1.2 / (a.kappa(1) * L)
+    for o in (a, b):
+        for x, f in enumerate(_p20_fields(n, amp)):
+            o.set_field(x, f)
+        assert o.roundtrips(2) == 0
+    for x in range(3):
+        assert rel_l2(b.get_field(x, EXIT), a.get_field(x, EXIT)) < 1e-13
+        assert rel_l2(b.get_field(x), a.get_field(x)) < 1e-13
+
+
+def test_p20_segments_equal_single_passes_chained_by_hand():
+    """Different length, step size, dk and d_eff per segment: the pass equals one single-crystal oracle per segment,
+    each started at z = 0 of its own crystal, fed with the previous one's output; z does NOT run on across segments."""
+    log2n = 6
+    n = 1 << log2n
+    segs = [(3e-3, 150.0, 14e-12, 12), (1e-3, -400.0, 9e-12, 7), (2e-3, 60.0, -14e-12, 10)]
+    kw = dict(n_fields=3, log2_n=log2n, beta1=(0.3 * FS / UM, 0.0, -0.17 * FS / UM),
+              beta2=(0.35 * FS * FS / UM, 0.12 * FS * FS / UM, 0.05 * FS * FS / UM), alpha=(2.0, 5.0, 1.0))
+    o = make(nz=29, length=6e-3, **kw)
+    assert o.set_segments(segs) == 0
+    amp = 1.0 / (2 * np.pi * 14e-12 / (2.16 * 1000 * NM) * 6e-3)
+    f = _p20_fields(n, amp, seed=21)
+    for x in range(3):
+        o.set_field(x, f[x])
+    assert o.propagate(12 + 3) == 0                # stops inside the second crystal
+    assert abs(o.z - 3 * 1e-3 / 7) < 1e-18          # z counts from that crystal's entrance
+    assert o.propagate(29 - 15) == 0
+    assert o.propagate(1) == 5                      # the pass is complete
+    cur = f
+    for (ln, dk, deff, nz) in segs:
+        c = make(nz=nz, length=ln, dk=dk, d_eff=deff, **kw)
+        for x in range(3):
+            c.set_field(x, cur[x])
+        assert c.propagate(nz) == 0
+        cur = [c.get_field(x) for x in range(3)]
+    for x in range(3):
+        assert rel_l2(o.get_field(x), cur[x]) < 1e-13
+    # one crystal of the total length with the first segment's parameters is something else
+    w = make(nz=29, length=6e-3, dk=150.0, **kw)
+    for x in range(3):
+        w.set_field(x, f[x])
+    w.propagate(29)
+    assert rel_l2(w.get_field(1), cur[1]) > 1e-2
+
+
+def test_p20_a_reversed_second_crystal_undoes_the_first():
+    """Dispersion off, dk = 0: the coupled-wave equations with d_eff -> -d_eff are the same equations
+    run backwards in z, so crystal + its reversed copy returns the input up to the RK4 truncation error, which falls as
+    h^4; and round trips restart from segment 0."""
+    log2n, L = 4, 5e-3
+    n = 1 << log2n
+    errs = []
+    for nz in (20, 40):
+        o = make(n_fields=3, log2_n=log2n, nz=2 * nz, length=2 * L, resonant=(0, 1, 0), R=(0, 1.0, 0))
+        assert o.set_segments([(L, 0.0, 14e-12, nz), (L, 0.0, -14e-12, nz)]) == 0
+        amp = 1.3 / (o.kappa(1) * L)
+        f = _p20_fields(n, amp, seed=22)
+        for x in range(3):
+            o.set_field(x, f[x])
+        assert o.propagate(nz) == 0
+        assert abs(np.sum(np.abs(o.get_field(0)) ** 2) / np.sum(np.abs(f[0]) ** 2) - 1) > 0.05      # the first crystal did something
+        assert o.propagate(nz) == 0
+        errs.append(max(rel_l2(o.get_field(x), f[x]) for x in range(3)))
+    assert errs[0] < 1e-6 and 8 < errs[0] / errs[1] < 32
+    o = make(n_fields=3, log2_n=log2n, nz=40, length=2 * L, resonant=(0, 1, 0), R=(0, 1.0, 0))
+    o.set_segments([(L, 0.0, 14e-12, 20), (L, 0.0, -14e-12, 20)])
+    for x in range(3):
+        o.set_field(x, f[x])
+    assert o.roundtrips(3) == 0                      # R = 1, everything undone each pass: still the input
+    assert rel_l2(o.get_field(1), f[1]) < 1e-5
+    assert o.kappa(1) > 0                            # back in segment 0 after the boundary
