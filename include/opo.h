@@ -22,6 +22,10 @@
  *       resonant x:      A_x <- sqrt(R_x) e^{i delta_x} IDFT( G_x .* DFT(A_x) ),
  *                        G_x[k] = exp(i (gdd_x/2) Omega_k^2 - i Omega_k delta_T_x)  (R13-R15)
  *       non-resonant x:  A_x <- S_x   (stored input: fresh pump / frozen seed)      (R11, R12)
+ *       resonant pump (x = 0; PAPER.md:L311 names doubly / triply resonant oscillators without an injection rule; reading
+ *                        R24): the input coupler of power reflectivity R_p adds the external pump,
+ *                        A_p <- sqrt(R_p) e^{i delta_p} IDFT( G_p .* DFT(A_p) ) [x modulator] + sqrt(1 - R_p) S_p;
+ *                        R_p = 0 is the single-pass rule above.  Not on the large-N engine.
  *
  * Grid (L175-178; R8, R9, R19): N = 2^log2_n points, dt = window/N, tau_n = (n - N/2) dt,
  * Omega_k = 2 pi k'/(N dt), k' = k (k < N/2) or k - N.  DFT: X[k] = sum_n x[n] e^{-2 pi i k n/N},
@@ -56,7 +60,7 @@ typedef struct opo_handle opo_handle;
 typedef enum {
     OPO_OK = 0,
     OPO_ERR_INVALID_ARG = 1, /* null pointer, N not a supported power of two, n_fields not 2|3, R outside [0,1], nz <= 0 ... */
-    OPO_ERR_UNSUPPORTED = 2, /* e.g. resonant pump (the paper gives no injection rule), precision/size combination */
+    OPO_ERR_UNSUPPORTED = 2, /* precision/size/engine combination (e.g. a resonant pump or several crystals at N > 2^14) */
     OPO_ERR_ALLOC = 3,
     OPO_ERR_CUDA = 4,        /* message from the CUDA runtime in opo_last_error */
     OPO_ERR_STATE = 5,       /* propagate past z = L, roundtrips at z != 0 */
@@ -80,7 +84,7 @@ typedef struct {
     double beta2_s2_per_m[3];  /* k''_x */
     double alpha_per_m[3];     /* power attenuation alpha_x */
     int ref_field;             /* co-moving frame (paper: the signal, L101) */
-    int resonant[3];           /* pump must be 0 */
+    int resonant[3];           /* a resonant pump (reading R24) re-enters through an input coupler, see below */
     double R[3];               /* power reflectivity 1 - theta_x, resonant fields */
     double delta_rad[3];       /* carrier detuning phase delta_x of Eq. 6 */
     double delta_T_s[3];       /* group-delay detuning: A(tau) -> A(tau - delta_T), circular (R13) */
@@ -116,6 +120,21 @@ int opo_set_stream(opo_handle* h, void* cuda_stream);
 #define OPO_PARAM_GDD 3
 int opo_set_batch_param(opo_handle* h, int param, int field, const double* host_vals, int count);
 
+/* Several crystals in series inside one pass ("incorporation of one or more nonlinear media"; SURVEY 8(f) N4;
+ * reading R25): segment j is walked in nz fixed steps h_j = length_m / nz with its own kappa_x = 2 pi d_eff / (n_x lambda_x)
+ * and its own dk, z counted from that crystal's entrance; the fields' dispersion and loss are those of opo_fields for
+ * every segment.  Replaces the crystal of opo_create (n = 0 restores it); afterwards a pass has sum(nz) z-steps, which
+ * is what opo_propagate counts.  Per-instance OPO_PARAM_DK values act on the first segment and are reset by this call.
+ * Only at z = 0 (OPO_ERR_STATE otherwise).  With n > 1 the host-sequenced STREAMING engine runs the pass (AUTO picks it);
+ * OPO_ERR_UNSUPPORTED on the large-N engine and the cuFFT baseline. */
+typedef struct {
+    double length_m;
+    double dk_per_m;
+    double d_eff_m_per_V;
+    int nz;
+} opo_segment;
+int opo_set_segments(opo_handle* h, int n, const opo_segment* segs);
+
 /* Third-order dispersion of field `field` [s^3/m] (Eq. 5; reading R7 of DESIGN.md: the physical form
  * dA/dz = +(beta3/6) d^3A/dtau^3, i.e. D_x(Omega) gains the term -(beta3_x/6) Omega^3; the term as printed would be a
  * gain).  0 removes it.  Only the fp64 host tables change (rebuilt before the next propagate / roundtrips call). */
@@ -132,8 +151,9 @@ int opo_set_beta3(opo_handle* h, int field, double beta3_s3_per_m);
 int opo_set_eom(opo_handle* h, int field, double beta_rad, double f_mod_hz);
 
 /* Pump input S_p (PAPER.md:L268 ReadPump): time-domain complex [N] (per_instance = 0, broadcast to
- * all instances) or [batch][N].  Copied into the handle; re-injected at every round-trip boundary;
- * also becomes the current pump field when z = 0. */
+ * all instances) or [batch][N].  Copied into the handle; re-injected at every round-trip boundary; when z = 0 the
+ * current pump field becomes what the boundary injects into an empty cavity: S_p (single-pass pump) or
+ * sqrt(1 - R_p) S_p (resonant pump, reading R24). */
 int opo_set_pump(opo_handle* h, const void* dev_pump, int per_instance);
 int opo_set_pump_host(opo_handle* h, const void* host_pump, int per_instance);
 

@@ -7,6 +7,7 @@ the CUDA package (paper_2410_02532_b200) and shares no code with it.
 from __future__ import annotations
 
 import ctypes
+import math
 import os
 import subprocess
 from concurrent.futures import ThreadPoolExecutor
@@ -172,6 +173,9 @@ def from_workload(w, b: int = 0, use_float: bool = False) -> OracleOpo:
                   resonant=w.resonant, R=w.R, delta_rad=w.delta_rad, delta_T_s=dT, gdd_s2=w.gdd_s2,
                   use_float=use_float)
     o.set_field(0, w.pump_of(b))
+    if w.resonant[0]:
+        # resonant pump (reading R24): at m = 0 the cavity holds what the input coupler transmits, sqrt(1 - R_p) S_p
+        o.set_field(0, math.sqrt(1.0 - w.R[0]) * w.pump_of(b), which="state")
     for x in range(1, w.n_fields):
         o.set_field(x, w.seeds[x][b])
     for x in range(w.n_fields):

@@ -48,6 +48,10 @@ class opo_grid(ctypes.Structure):
                 ("precision", ctypes.c_int), ("batch", ctypes.c_int)]
 
 
+class opo_segment(ctypes.Structure):
+    _fields_ = [("length_m", ctypes.c_double), ("dk_per_m", ctypes.c_double), ("d_eff_m_per_V", ctypes.c_double), ("nz", ctypes.c_int)]
+
+
 class OpoError(RuntimeError):
     def __init__(self, status: int, message: str):
         super().__init__(f"libopo status {status}: {message}")
@@ -87,6 +91,7 @@ def lib() -> ctypes.CDLL:
         L.opo_get_z_steps.argtypes = [vp, ctypes.POINTER(ci)]
         L.opo_set_option.argtypes = [vp, ci, ci]
         L.opo_get_info.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_longlong)]
+        L.opo_set_segments.argtypes = [vp, ci, ctypes.POINTER(opo_segment)]
         L.opo_selftest_peak.argtypes = [ci, ctypes.POINTER(ctypes.c_double)]
         L.opo_last_error.argtypes = [vp]
         L.opo_last_error.restype = ctypes.c_char_p
@@ -100,7 +105,7 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_eom", "opo_set_beta3", "opo_set_pump",
            "opo_set_pump_host", "opo_set_field", "opo_set_field_host", "opo_propagate", "opo_roundtrips", "opo_roundtrips_train",
            "opo_get_fields", "opo_get_fields_host", "opo_sync", "opo_check_finite", "opo_get_z_steps",
-           "opo_set_option", "opo_get_info", "opo_selftest_peak", "opo_last_error"]
+           "opo_set_option", "opo_get_info", "opo_selftest_peak", "opo_set_segments", "opo_last_error"]
 
 
 def _check(handle, status: int):
@@ -143,6 +148,15 @@ def opo_set_stream(h, cuda_stream: int):
 def opo_set_batch_param(h, param: int, field: int, values):
     v = np.ascontiguousarray(values, dtype=np.float64)
     _check(h, lib().opo_set_batch_param(h, param, field, v.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), v.size))
+
+
+def opo_set_segments(h, segments):
+    """segments: sequence of (length_m, dk_per_m, d_eff_m_per_V, nz); empty restores the crystal of opo_create."""
+    n = len(segments)
+    arr = (opo_segment * max(n, 1))()
+    for j, sg in enumerate(segments):
+        arr[j].length_m, arr[j].dk_per_m, arr[j].d_eff_m_per_V, arr[j].nz = float(sg[0]), float(sg[1]), float(sg[2]), int(sg[3])
+    _check(h, lib().opo_set_segments(h, n, arr))
 
 
 def opo_set_beta3(h, field: int, beta3_s3_per_m: float):
@@ -275,6 +289,9 @@ class Opo:
     def set_batch_param(self, param, field, values):
         opo_set_batch_param(self._h, param, field, values)
 
+    def set_segments(self, segments):
+        opo_set_segments(self._h, segments)
+
     def set_beta3(self, field, beta3_s3_per_m):
         opo_set_beta3(self._h, field, beta3_s3_per_m)
 
@@ -357,6 +374,8 @@ def from_workload(w, engine=ENGINE_AUTO, host_inputs=False) -> Opo:
             beta2_s2_per_m=w.beta2_s2_per_m, alpha_per_m=w.alpha_per_m, ref_field=w.ref_field,
             resonant=w.resonant, R=w.R, delta_rad=w.delta_rad, delta_T_s=w.delta_T_s, gdd_s2=w.gdd_s2,
             precision=w.precision, batch=w.batch, engine=engine)
+    if getattr(w, "segments", None):
+        o.set_segments(w.segments)          # before the per-instance dk sweep, which acts on the first segment
     if len(w.dk_per_m) > 1:
         o.set_batch_param(PARAM_DK, 0, w.dk_per_m)
     if w.delta_T_signal_s is not None:

@@ -147,6 +147,14 @@ struct opo_handle {
     int engine_opt = OPO_ENGINE_AUTO;
     bool resident_ok = false;
     opo::ResidentInfo rinfo{};
+    // crystal segments in series (opo_set_segments, reading R25).  n_seg = 1: the crystal of opo_create.
+    // nz is the number of z-steps of a whole pass; h and kappa above are those of segment 0.
+    struct Segment { double len = 0, dk = 0, deff = 0, hstep = 0, kappa[3] = {0, 0, 0}; int nz = 0; };
+    int n_seg = 1;
+    Segment seg[8];
+    void* segH[8][3] = {};                            // per-segment tables, allocated when n_seg > 1 (streaming engine):
+    void* segH2[8][3] = {};                           //   half step H_j / N, full step H_j^2 / N,
+    void* segHX[8][3] = {};                           //   H_j H_{j+1} / N across the junction of two crystals
     bool solo_ok = false;                             // solo engine (one CTA per instance, fields in shared + tensor memory)
     opo::ResidentInfo sinfo{};                        // max_clusters = co-resident CTAs on the device
     int device = 0;
@@ -283,31 +291,43 @@ namespace {
 // Device tables carry the 1/N of the inverse transform and are stored in mid-pass layout:
 //   tabH = H/N, tabH2 = H^2/N, tabGM = G m/N, tabHB = H^2 G m/N (half-steps merged across the boundary).
 int build_tables(opo_handle* h) {
-    const int N = h->N, F = h->F, B = h->B;
+    const int N = h->N, F = h->F, B = h->B, K = h->n_seg;
     HostPlan pl(h->large ? h->L2 : h->L);
     const double invN = 1.0 / (double)N;
-    std::vector<cd> Hh(N), M(N), lay(N);
+    const double h0 = h->seg[0].hstep, hl = h->seg[K - 1].hstep;      // first and last step size of a pass
+    std::vector<cd> Hh(N), M(N), lay(N), Dx(N);
     for (int x = 0; x < F; ++x) {
         const double db1 = h->fields.beta1_s_per_m[x] - h->fields.beta1_s_per_m[h->fields.ref_field];
         const double b2 = h->fields.beta2_s2_per_m[x], al = h->fields.alpha_per_m[x];
         const double b3 = h->beta3[x] / 6.0;            // D_x -= (beta3_x/6) Omega^3   (reading R7)
         for (int k = 0; k < N; ++k) {
             const double om = omega_of(h, k);
-            const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
-            Hh[k] = std::exp(cd(-0.5 * al, D) * (0.5 * h->h));
+            Dx[k] = cd(-0.5 * al, -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om);      // -alpha_x/2 + i D_x(Omega_k)
         }
-        for (int k = 0; k < N; ++k) M[k] = Hh[k] * invN;
+        // first linear operator of a pass / of a call: half step of segment 0
+        for (int k = 0; k < N; ++k) M[k] = std::exp(Dx[k] * (0.5 * h0)) * invN;
         to_engine_layout(h, pl, M.data(), lay.data());
         if (int rc = upload_table(h, h->tabH[x], lay.data(), N)) return rc;
         if (h->natH[x]) if (int rc = upload_complex(h, h->natH[x], M.data(), N)) return rc;        // cuFFT baseline: natural order
-        for (int k = 0; k < N; ++k) {
-            const double om = omega_of(h, k);
-            const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
-            M[k] = std::exp(cd(-0.5 * al, D) * h->h) * invN;     // H^2 evaluated directly in fp64
-        }
+        for (int k = 0; k < N; ++k) M[k] = std::exp(Dx[k] * h0) * invN;                            // H^2 evaluated directly in fp64
         to_engine_layout(h, pl, M.data(), lay.data());
         if (int rc = upload_table(h, h->tabH2[x], lay.data(), N)) return rc;
         if (h->natH2[x]) if (int rc = upload_complex(h, h->natH2[x], M.data(), N)) return rc;
+        if (K > 1) {
+            // several crystals: per segment the half step, the full step and the junction H_j H_{j+1}
+            for (int j = 0; j < K; ++j) {
+                const double hj = h->seg[j].hstep;
+                for (int v = 0; v < 3; ++v) {
+                    if (v == 2 && j == K - 1) continue;
+                    const double len = v == 0 ? 0.5 * hj : (v == 1 ? hj : 0.5 * (hj + h->seg[j + 1].hstep));
+                    void** dst = v == 0 ? &h->segH[j][x] : (v == 1 ? &h->segH2[j][x] : &h->segHX[j][x]);
+                    if (!*dst && cudaMalloc(dst, (size_t)N * h->tab_esz) != cudaSuccess) { cudaGetLastError(); return fail(h, OPO_ERR_ALLOC, "cudaMalloc of segment tables failed"); }
+                    for (int k = 0; k < N; ++k) M[k] = std::exp(Dx[k] * len) * invN;
+                    to_engine_layout(h, pl, M.data(), lay.data());
+                    if (int rc = upload_table(h, *dst, lay.data(), N)) return rc;
+                }
+            }
+        }
 
         if (!h->fields.resonant[x]) continue;
         // boundary tables, shared or per instance
@@ -336,9 +356,9 @@ int build_tables(opo_handle* h) {
                 const double om = omega_of(h, k);
                 const double ph = 0.5 * h->gdd[x][b] * om * om - om * h->dT[x][b];
                 const cd gm = cd(std::cos(ph), std::sin(ph)) * mir[b];
-                const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
                 M[k] = gm * invN;
-                Hh[k] = std::exp(cd(-0.5 * al, D) * h->h) * gm * invN;
+                // last half-step of the pass, boundary, first half-step of the next pass
+                Hh[k] = std::exp(Dx[k] * (0.5 * (hl + h0))) * gm * invN;
             }
             to_engine_layout(h, pl, M.data(), lay.data());
             if (int rc = upload_table(h, (char*)h->tabGM[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
@@ -346,7 +366,7 @@ int build_tables(opo_handle* h) {
                 if (h->natGM_count[x] != need) {
                     if (h->natGM[x]) cudaFree(h->natGM[x]);
                     h->natGM[x] = nullptr;
-                    if (cudaMalloc(&h->natGM[x], need * N * h->esz) != cudaSuccess) return fail(h, OPO_ERR_ALLOC, "cudaMalloc of baseline tables failed");
+                    if (cudaMalloc(&h->natGM[x], need * N * h->esz) != cudaSuccess) { cudaGetLastError(); return fail(h, OPO_ERR_ALLOC, "cudaMalloc of baseline tables failed"); }
                     h->natGM_count[x] = need;
                 }
                 if (int rc = upload_complex(h, (char*)h->natGM[x] + b * N * h->esz, M.data(), N)) return rc;
@@ -354,11 +374,7 @@ int build_tables(opo_handle* h) {
             to_engine_layout(h, pl, Hh.data(), lay.data());
             if (int rc = upload_table(h, (char*)h->tabHB[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
             // H G m: the last half-step of a pass and the boundary, the modulator and the next half-step follow separately
-            for (int k = 0; k < N; ++k) {
-                const double om = omega_of(h, k);
-                const double D = -db1 * om + 0.5 * b2 * om * om - b3 * om * om * om;
-                Hh[k] = std::exp(cd(-0.5 * al, D) * (0.5 * h->h)) * M[k];
-            }
+            for (int k = 0; k < N; ++k) Hh[k] = std::exp(Dx[k] * (0.5 * hl)) * M[k];
             to_engine_layout(h, pl, Hh.data(), lay.data());
             if (int rc = upload_table(h, (char*)h->tabHG[x] + b * N * h->tab_esz, lay.data(), N)) return rc;
         }
@@ -367,19 +383,33 @@ int build_tables(opo_handle* h) {
     return OPO_OK;
 }
 
+// index of the first phase-table entry of z-step s (counted from the start of the pass): the table of an instance is the
+// concatenation of one table per crystal segment, [q nz_j + 1] entries exp(i dk_j i h_j / q), q = 2 (4: N/2 - L - N/2),
+// because z restarts at every crystal entrance (readings R4, R25)
+int segment_of_step(const opo_handle* h, int s) {
+    int j = 0, first = 0;
+    while (j + 1 < h->n_seg && s >= first + h->seg[j].nz) { first += h->seg[j].nz; ++j; }
+    return j;
+}
+
 // phase[b][j] = exp(i dk_b j h/2), j = 0 .. 2 nz   (R4: z from the crystal entrance)
-int phase_stride(const opo_handle* h) { return (h->splitting ? 4 : 2) * h->nz + 1; }
+int phase_stride(const opo_handle* h) { return (h->splitting ? 4 : 2) * h->nz + h->n_seg; }
 
 // N/2 - L - N/2 (OPO_SPLITTING_NLN): the RK4 steps have size h/2, so the table runs in steps of h/4, j = 0 .. 4 nz
 int build_phase(opo_handle* h) {
-    const int stride = phase_stride(h);
-    const double dz = h->splitting ? 0.25 * h->h : 0.5 * h->h;
+    const int stride = phase_stride(h), q = h->splitting ? 4 : 2;
     std::vector<cd> ph((size_t)h->B * stride);
-    for (int b = 0; b < h->B; ++b)
-        for (int j = 0; j < stride; ++j) {
-            const double a = h->dk[b] * dz * (double)j;
-            ph[(size_t)b * stride + j] = cd(std::cos(a), std::sin(a));
+    for (int b = 0; b < h->B; ++b) {
+        size_t at = (size_t)b * stride;
+        for (int j = 0; j < h->n_seg; ++j) {
+            const double dk = j == 0 ? h->dk[b] : h->seg[j].dk;        // per-instance sweeps act on the first crystal
+            const double dz = h->seg[j].hstep / (double)q;
+            for (int i = 0; i <= q * h->seg[j].nz; ++i) {
+                const double a = dk * dz * (double)i;
+                ph[at++] = cd(std::cos(a), std::sin(a));
+            }
         }
+    }
     if (int rc = upload_complex(h, h->phase, ph.data(), ph.size())) return rc;
     h->phase_dirty = false;
     return OPO_OK;
@@ -453,6 +483,11 @@ void free_all(opo_handle* h) {
         void* ptrs[] = {h->cur[x], h->S[x], h->exitb[x], h->SH[x], h->tabH[x], h->tabH2[x], h->tabGM[x], h->tabHB[x], h->tabHG[x], h->mirror[x], h->eom[x], h->natH[x], h->natH2[x], h->natGM[x]};
         for (void* p : ptrs) if (p) cudaFree(p);
     }
+    for (int j = 0; j < 8; ++j)
+        for (int x = 0; x < 3; ++x) {
+            void* ptrs[] = {h->segH[j][x], h->segH2[j][x], h->segHX[j][x]};
+            for (void* p : ptrs) if (p) cudaFree(p);
+        }
     if (h->cufft_plan >= 0 && cufft_api().ok) cufft_api().Destroy(h->cufft_plan);
     if (h->rt_flags) cudaFree(h->rt_flags);
     void* more[] = {h->scratch, h->tw, h->perm, h->phase, h->flag, h->tw2, h->wlo, h->whi, h->perm2, h->scratch2, h->barrier};
@@ -478,10 +513,11 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
         if (!(f->lambda_m[x] > 0.0) || !(f->n[x] > 0.0)) return fail(nullptr, OPO_ERR_INVALID_ARG, "lambda and n must be positive");
         if (f->resonant[x] && !(f->R[x] >= 0.0 && f->R[x] <= 1.0)) return fail(nullptr, OPO_ERR_INVALID_ARG, "R outside [0, 1]");
     }
-    if (f->resonant[0]) return fail(nullptr, OPO_ERR_UNSUPPORTED, "resonant pump: the paper gives no input-coupling rule");
     const int maxL = (g->precision == OPO_PRECISION_C64) ? opo::kMaxLog2Smem : opo::kMaxLog2Smem - 1;
     if (g->log2_n < opo::kMinLog2 || g->log2_n > opo::kMaxLog2)
         return fail(nullptr, OPO_ERR_UNSUPPORTED, "grid size not supported (2^6 .. 2^18)");
+    if (f->resonant[0] && g->log2_n > maxL)
+        return fail(nullptr, OPO_ERR_UNSUPPORTED, "resonant pump: not on the large-N engine (N > 2^14, c128: > 2^13)");
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -504,6 +540,9 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
     h->device = dev;
     for (int x = 0; x < h->F; ++x) h->kappa[x] = 2.0 * kPi * c->d_eff_m_per_V / (f->n[x] * f->lambda_m[x]);
     if (h->F == 2) h->kappa[0] *= 0.5;                                                                         // reading R5
+    h->n_seg = 1;
+    h->seg[0].len = c->length_m; h->seg[0].dk = c->dk_per_m; h->seg[0].deff = c->d_eff_m_per_V; h->seg[0].nz = h->nz; h->seg[0].hstep = h->h;
+    for (int x = 0; x < 3; ++x) h->seg[0].kappa[x] = h->kappa[x];
     h->dk.assign(h->B, c->dk_per_m);
     for (int x = 0; x < 3; ++x) {
         h->dT[x].assign(h->B, x < h->F ? f->delta_T_s[x] : 0.0);
@@ -522,7 +561,7 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
             cudaMalloc(&h->mirror[x], (size_t)h->B * h->esz) != cudaSuccess)
             return bail(OPO_ERR_ALLOC, "cudaMalloc of tables failed");
     }
-    if (cudaMalloc(&h->scratch, fb) != cudaSuccess || cudaMalloc(&h->phase, (size_t)h->B * (4 * h->nz + 1) * h->esz) != cudaSuccess ||
+    if (cudaMalloc(&h->scratch, fb) != cudaSuccess || cudaMalloc(&h->phase, (size_t)h->B * (4 * h->nz + 8) * h->esz) != cudaSuccess ||
         cudaMalloc((void**)&h->flag, sizeof(int)) != cudaSuccess)
         return bail(OPO_ERR_ALLOC, "cudaMalloc of scratch failed");
     if (int rc = build_fft_tables(h)) { std::string m = h->err; return bail(rc, m); }
@@ -628,6 +667,7 @@ bool prefer_solo(const opo_handle* h) {
 
 int engine_in_use(const opo_handle* h) {
     if (h->large) return OPO_ENGINE_LARGE;
+    if (h->n_seg > 1) return OPO_ENGINE_STREAMING;       // several crystals in series: host-sequenced engine only
     if (h->engine_opt == OPO_ENGINE_STREAMING) return OPO_ENGINE_STREAMING;
     if (h->engine_opt == OPO_ENGINE_CUFFT) return OPO_ENGINE_CUFFT;
     if (h->engine_opt == OPO_ENGINE_SOLO && h->solo_ok && !h->splitting) return OPO_ENGINE_SOLO;
@@ -637,7 +677,8 @@ int engine_in_use(const opo_handle* h) {
 }
 
 // ---- streaming engine ------------------------------------------------------------------------------------------
-enum TableKind { TAB_H, TAB_H2 };
+// which linear operator: half step of crystal segment j, its full step, or the junction H_j H_{j+1} of two crystals
+enum TableKind { TAB_H, TAB_H2, TAB_HX };
 
 // cuFFT baseline: A <- IDFT(tab .* DFT(A)) as three launches per field (forward C2C over the batch, table multiply, inverse C2C)
 int cufft_linear(opo_handle* h, int x, const void* tab, long long tab_stride) {
@@ -652,8 +693,8 @@ int cufft_linear(opo_handle* h, int x, const void* tab, long long tab_stride) {
     return OPO_OK;
 }
 
-int stream_linear_all(opo_handle* h, TableKind kind, bool to_exit) {
-    if (engine_in_use(h) == OPO_ENGINE_CUFFT) {
+int stream_linear_all(opo_handle* h, TableKind kind, int j, bool to_exit) {
+    if (engine_in_use(h) == OPO_ENGINE_CUFFT) {          // single crystal only (engine_in_use)
         for (int x = 0; x < h->F; ++x) {
             if (int rc = cufft_linear(h, x, kind == TAB_H ? h->natH[x] : h->natH2[x], 0)) return rc;
             if (to_exit) OPO_CUDA(h, cudaMemcpyAsync(h->exitb[x], h->cur[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
@@ -665,45 +706,63 @@ int stream_linear_all(opo_handle* h, TableKind kind, bool to_exit) {
     for (int x = 0; x < h->F; ++x) {
         a.slot[x].src = h->cur[x]; a.slot[x].dst = h->cur[x];
         a.slot[x].dst2 = to_exit ? h->exitb[x] : nullptr;
-        a.slot[x].tab = (kind == TAB_H) ? h->tabH[x] : h->tabH2[x];
+        if (h->n_seg == 1) a.slot[x].tab = (kind == TAB_H) ? h->tabH[x] : h->tabH2[x];
+        else a.slot[x].tab = kind == TAB_H ? h->segH[j][x] : (kind == TAB_H2 ? h->segH2[j][x] : h->segHX[j][x]);
         a.slot[x].tab_stride = 0;
     }
     OPO_LAUNCH(h, h->dbl ? opo::launch_linear_f64(h->L, a, h->stream) : opo::launch_linear_f32(h->L, a, h->stream));
     return OPO_OK;
 }
 
-// one RK4 step of the coupling terms; phase_index < 0: full step h of z-step `step`; otherwise a half step h/2
-// whose stage phases start at phase_index in the h/4 table (N/2 - L - N/2)
-int stream_rk4(opo_handle* h, int step, int phase_index = -1) {
+// one RK4 step of the coupling terms of z-step `step` (counted from the start of the pass), with the couplings, step size
+// and dk of the crystal segment it lies in; half = -1: the full step h; half = 0 | 1: first / second half step h/2 of the
+// N/2 - L - N/2 ordering (phase table in steps of h/4)
+int stream_rk4(opo_handle* h, int step, int half = -1) {
+    const int j = segment_of_step(h, step);
+    const opo_handle::Segment& sg = h->seg[j];
     opo::Rk4Args a{};
-    for (int x = 0; x < h->F; ++x) { a.A[x] = h->cur[x]; a.kappa[x] = h->kappa[x]; }
-    a.n_fields = h->F; a.batch = h->B; a.n = h->N; a.h = phase_index < 0 ? h->h : 0.5 * h->h;
-    a.phase = h->phase; a.phase_stride = phase_stride(h); a.step = step; a.phase_index = phase_index;
+    for (int x = 0; x < h->F; ++x) { a.A[x] = h->cur[x]; a.kappa[x] = sg.kappa[x]; }
+    a.n_fields = h->F; a.batch = h->B; a.n = h->N; a.h = half < 0 ? sg.hstep : 0.5 * sg.hstep;
+    a.phase = h->phase; a.phase_stride = phase_stride(h); a.step = step;
+    // entry of the concatenated per-segment tables (segment_of_step): q s + j, q = 2 | 4
+    a.phase_index = half < 0 ? 2 * step + j : 4 * step + j + 2 * half;
     OPO_LAUNCH(h, h->dbl ? opo::launch_rk4_f64(a, h->stream) : opo::launch_rk4_f32(a, h->stream));
     return OPO_OK;
 }
 
-// nsteps z-steps from step index z0, half-steps merged:  H, N, H^2, N, ..., N, H
+// nsteps z-steps from step index z0, half-steps merged:  H, N, H^2, N, ..., N, H; at the junction of two crystals the
+// merged operator is H_j H_{j+1}
 int stream_steps(opo_handle* h, int z0, int nsteps, bool to_exit) {
     if (nsteps <= 0) return OPO_OK;
     if (h->splitting) {      // N/2 - L - N/2 (Eq. 10-11), un-merged: two RK4 half-steps around one full linear step
         for (int s = z0; s < z0 + nsteps; ++s) {
-            if (int rc = stream_rk4(h, s, 4 * s)) return rc;
-            if (int rc = stream_linear_all(h, TAB_H2, false)) return rc;
-            if (int rc = stream_rk4(h, s, 4 * s + 2)) return rc;
+            if (int rc = stream_rk4(h, s, 0)) return rc;
+            if (int rc = stream_linear_all(h, TAB_H2, segment_of_step(h, s), false)) return rc;
+            if (int rc = stream_rk4(h, s, 1)) return rc;
         }
         if (to_exit)
             for (int x = 0; x < h->F; ++x)
                 OPO_CUDA(h, cudaMemcpyAsync(h->exitb[x], h->cur[x], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
         return OPO_OK;
     }
-    if (int rc = stream_linear_all(h, TAB_H, false)) return rc;
+    if (int rc = stream_linear_all(h, TAB_H, segment_of_step(h, z0), false)) return rc;
     for (int s = 0; s < nsteps; ++s) {
         if (int rc = stream_rk4(h, z0 + s)) return rc;
-        if (s + 1 < nsteps) if (int rc = stream_linear_all(h, TAB_H2, false)) return rc;
+        if (s + 1 < nsteps) {
+            const int j = segment_of_step(h, z0 + s), jn = segment_of_step(h, z0 + s + 1);
+            if (int rc = stream_linear_all(h, j == jn ? TAB_H2 : TAB_HX, j, false)) return rc;
+        }
     }
-    return stream_linear_all(h, TAB_H, to_exit);
+    return stream_linear_all(h, TAB_H, segment_of_step(h, z0 + nsteps - 1), to_exit);
 }
+
+// A <- (accumulate ? A : 0) + c S  (input coupler of a resonant pump, reading R24)
+int stream_axpy(opo_handle* h, void* A, const void* S, double c, bool accumulate) {
+    OPO_LAUNCH(h, h->dbl ? opo::launch_axpy_f64(A, S, c, accumulate ? 1 : 0, (long long)h->B * h->N, h->stream)
+                         : opo::launch_axpy_f32(A, S, c, accumulate ? 1 : 0, (long long)h->B * h->N, h->stream));
+    return OPO_OK;
+}
+double pump_inject(const opo_handle* h) { return h->fields.resonant[0] ? std::sqrt(1.0 - h->fields.R[0]) : 0.0; }
 
 // cavity boundary on the fields at z = L (readings R11-R15)
 int stream_boundary(opo_handle* h) {
@@ -725,6 +784,9 @@ int stream_boundary(opo_handle* h) {
     }
     if (a.n_slots > 0)
         OPO_LAUNCH(h, h->dbl ? opo::launch_linear_f64(h->L, a, h->stream) : opo::launch_linear_f32(h->L, a, h->stream));
+    // resonant pump: the input coupler adds sqrt(1 - R_p) S_p (reading R24; with a modulator on the pump it acts before the
+    // injection, as in the oracle)
+    if (h->fields.resonant[0] && !h->eom[0]) return stream_axpy(h, h->cur[0], h->S[0], pump_inject(h), true);
     return OPO_OK;
 }
 
@@ -738,6 +800,8 @@ int apply_eom(opo_handle* h) {
         if (!h->eom[x]) continue;
         opo::MulTabArgs m{h->cur[x], h->eom[x], h->B, h->N, 0};
         OPO_LAUNCH(h, h->dbl ? opo::launch_multab_f64(m, h->stream) : opo::launch_multab_f32(m, h->stream));
+        if (x == 0 && h->fields.resonant[0])        // the input coupler comes after the pump's own modulator (stream_boundary)
+            if (int rc = stream_axpy(h, h->cur[0], h->S[0], pump_inject(h), true)) return rc;
     }
     return OPO_OK;
 }
@@ -755,6 +819,7 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
         a.resonant[x] = h->fields.resonant[x] ? 1 : 0;
         a.kappa[x] = h->kappa[x];
     }
+    a.inject = pump_inject(h);
     a.tw = h->tw; a.phase = h->phase; a.phase_stride = phase_stride(h);
     a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
     a.mode = mode; a.z0 = z0; a.steps = steps; a.nln = h->splitting;
@@ -871,8 +936,12 @@ int set_pump_impl(opo_handle* h, const void* p, int per_instance, cudaMemcpyKind
     if (!h || !p) return fail(h, OPO_ERR_INVALID_ARG, "null argument");
     if (int rc = check_async(h)) return rc;
     if (int rc = copy_in(h, h->S[0], p, per_instance != 0, kind)) return rc;
-    if (h->z_steps == 0)
+    if (h->z_steps == 0) {
+        // what the boundary injects into an empty cavity: S_p for a single-pass pump, sqrt(1 - R_p) S_p through the
+        // input coupler of a resonant one (reading R24)
+        if (h->fields.resonant[0]) return stream_axpy(h, h->cur[0], h->S[0], pump_inject(h), false);
         OPO_CUDA(h, cudaMemcpyAsync(h->cur[0], h->S[0], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
+    }
     return OPO_OK;
 }
 
@@ -984,6 +1053,48 @@ int opo_roundtrips_train(opo_handle* h, int n, const void* dev_pump_train, int p
             OPO_CUDA(h, cudaMemcpyAsync((char*)dev_out_train + (size_t)m * h->field_bytes(), h->exitb[out_field], h->field_bytes(),
                                         cudaMemcpyDeviceToDevice, h->stream));
     }
+    return OPO_OK;
+}
+
+int opo_set_segments(opo_handle* h, int n, const opo_segment* segs) {
+    if (!h) return OPO_ERR_INVALID_ARG;
+    if (n < 0 || n > 8 || (n > 0 && !segs)) return fail(h, OPO_ERR_INVALID_ARG, "0 .. 8 segments");
+    if (h->z_steps != 0) return fail(h, OPO_ERR_STATE, "the crystal segments can only change at z = 0");
+    if (h->large && n > 1) return fail(h, OPO_ERR_UNSUPPORTED, "several crystals: not on the large-N engine (N > 2^14, c128: > 2^13)");
+    if (n > 1 && h->engine_opt == OPO_ENGINE_CUFFT) return fail(h, OPO_ERR_UNSUPPORTED, "several crystals: not on the cuFFT baseline engine");
+    long long total = 0;
+    for (int j = 0; j < n; ++j) {
+        if (!(segs[j].length_m > 0.0) || segs[j].nz <= 0 || !std::isfinite(segs[j].dk_per_m) || !std::isfinite(segs[j].d_eff_m_per_V))
+            return fail(h, OPO_ERR_INVALID_ARG, "segment length and nz must be positive, dk and d_eff finite");
+        total += segs[j].nz;
+    }
+    if (int rc = check_async(h)) return rc;
+    if (n == 0) {       // back to the crystal of opo_create
+        h->n_seg = 1;
+        h->seg[0].len = h->crystal.length_m; h->seg[0].dk = h->crystal.dk_per_m; h->seg[0].deff = h->crystal.d_eff_m_per_V;
+        h->seg[0].nz = h->grid.nz_per_pass;
+    } else {
+        h->n_seg = n;
+        for (int j = 0; j < n; ++j) { h->seg[j].len = segs[j].length_m; h->seg[j].dk = segs[j].dk_per_m; h->seg[j].deff = segs[j].d_eff_m_per_V; h->seg[j].nz = segs[j].nz; }
+    }
+    h->nz = 0;
+    for (int j = 0; j < h->n_seg; ++j) {
+        opo_handle::Segment& sg = h->seg[j];
+        sg.hstep = sg.len / (double)sg.nz;
+        for (int x = 0; x < h->F; ++x) sg.kappa[x] = 2.0 * kPi * sg.deff / (h->fields.n[x] * h->fields.lambda_m[x]);
+        if (h->F == 2) sg.kappa[0] *= 0.5;                                                                               // reading R5
+        h->nz += sg.nz;
+    }
+    h->h = h->seg[0].hstep;
+    for (int x = 0; x < 3; ++x) h->kappa[x] = h->seg[0].kappa[x];
+    // per-instance dk sweeps act on the first crystal; a new segment list resets them to its dk
+    h->dk.assign(h->B, h->seg[0].dk);
+    OPO_CUDA(h, cudaStreamSynchronize(h->stream));
+    cudaFree(h->phase);
+    h->phase = nullptr;
+    if (cudaMalloc(&h->phase, (size_t)h->B * (4 * (size_t)h->nz + 8) * h->esz) != cudaSuccess) { cudaGetLastError(); return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the phase table failed"); }
+    h->tables_dirty = true;
+    h->phase_dirty = true;
     return OPO_OK;
 }
 

@@ -83,6 +83,7 @@ struct ResidentArgs {
                            // round trip, or null
     int boundary_fft[3];   // resonant field needs the transform pair at the boundary
     int resonant[3];
+    double inject;         // resonant pump (field 0): sqrt(1 - R_p), the input coupler adds inject * S_p at every boundary (R24); else 0
     const void* tw;
     const void* phase;     // as Rk4Args
     int phase_stride;
@@ -155,6 +156,7 @@ struct LargeInfo {
     cudaError_t launch_freq_##SUFFIX(int log2n, const FreqArgs& a, cudaStream_t s);     \
     cudaError_t launch_finite_##SUFFIX(const void* A, long long count, int* flag, cudaStream_t s); \
     cudaError_t launch_broadcast_##SUFFIX(void* dst, int batch, int n, cudaStream_t s); \
+    cudaError_t launch_axpy_##SUFFIX(void* A, const void* S, double c, int accumulate, long long count, cudaStream_t s); \
     cudaError_t resident_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);     \
     cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
     cudaError_t solo_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);         \

@@ -165,6 +165,16 @@ __global__ void __launch_bounds__(256) k_broadcast(cplx<T>* dst, int batch, int 
         dst[n + i] = dst[i % n];
 }
 
+// A[i] = (accumulate ? A[i] : 0) + c S[i]   (input coupler of a resonant pump, reading R24 of DESIGN.md)
+template <class T>
+__global__ void __launch_bounds__(256) k_axpy(cplx<T>* A, const cplx<T>* __restrict__ S, T c, int accumulate, long long count) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        const cplx<T> s = S[i];
+        cplx<T> a = accumulate ? A[i] : cplx<T>{(T)0, (T)0};
+        A[i] = {a.re + c * s.re, a.im + c * s.im};
+    }
+}
+
 template <class T>
 __global__ void __launch_bounds__(256) k_finite(const T* A, long long count, int* flag) {
     int bad = 0;
@@ -224,6 +234,10 @@ template <class T> cudaError_t launch_multab_T(const MulTabArgs& a, cudaStream_t
 template <class T> cudaError_t launch_broadcast_T(void* dst, int batch, int n, cudaStream_t s) {
     if (batch <= 1) return cudaSuccess;
     k_broadcast<T><<<grid_for((long long)(batch - 1) * n, 256), 256, 0, s>>>(reinterpret_cast<cplx<T>*>(dst), batch, n);
+    return cudaGetLastError();
+}
+template <class T> cudaError_t launch_axpy_T(void* A, const void* S, double c, int accumulate, long long count, cudaStream_t s) {
+    k_axpy<T><<<grid_for(count, 256), 256, 0, s>>>(reinterpret_cast<cplx<T>*>(A), reinterpret_cast<const cplx<T>*>(S), (T)c, accumulate, count);
     return cudaGetLastError();
 }
 template <class T> cudaError_t launch_finite_T(const void* A, long long count, int* flag, cudaStream_t s) {

@@ -281,6 +281,21 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
             for (int i = tid; i < N; i += NT) g[i] = sm[phys<T>(i)];
         };
 
+        // resonant pump (reading R24): the input coupler adds t S_p at every boundary, and the first half-step of the next
+        // pass acts on the sum: SH_p <- IDFT(H DFT(S_p)) (up to its inverse pass 0) once per piece of work, t SH_p is added
+        // after the merged boundary operator at every crossing
+        const T tinj = (T)a.inject;
+        const bool inj_any = x == 0 && tinj != (T)0 && resonant;
+        if (inj_any && rt_mode && steps_l > 1 && !NLN) {
+            load(reinterpret_cast<const cplx<T>*>(a.S[x]) + (size_t)b * N);
+            __syncthreads();
+            pass0_local<T, L, NT>(tw, tid, false);
+            __syncthreads();
+            linear_core_smem<T, L, NT>(tabH, tid);
+            __syncthreads();
+            store(SH);
+            __syncthreads();
+        }
         if (a.split && rt0 > 0) {       // the earlier round trips of this instance ran on another cluster
             if (tid == 0) {
                 int v;
@@ -342,6 +357,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
             const int s = rt_mode ? q % nz : a.z0 + q;          // index of the RK4 step that follows
             const bool crossing = rt_mode && q > 0 && q < total && s == 0;
             const bool keep = rt_mode && q == 0 && !resonant && steps_l > 1;   // SH <- first half-stepped input
+            const bool inj = crossing && inj_any;                               // input coupler of a resonant pump
             if (crossing && !resonant) {
                 if constexpr (FLOW) { flow_wait_done_all((fz - 1) & 1); __syncthreads(); }
                 load(SH);                                        // fresh pump / frozen seed, already half-stepped
@@ -373,7 +389,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                     FlowArgs fa;
                     fa.mb = mb; fa.nf = F;
                     fa.wait_in = 0; fa.par_done = 0;
-                    fa.arrive_out = 1;
+                    fa.arrive_out = !inj;
                     linear_core_smem<T, L, NT, true>(tabH, tid, fa);
                 } else {
                     linear_core_smem<T, L, NT>(tabH, tid);
@@ -384,11 +400,21 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                     FlowArgs fa;
                     fa.mb = mb; fa.nf = F;
                     fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
-                    fa.arrive_out = (q < total) && !keep;
+                    fa.arrive_out = (q < total) && !keep && !inj;
                     linear_core_smem<T, L, NT, true>(tab, tid, fa);
                 } else {
                     linear_core_smem<T, L, NT>(tab, tid);
                 }
+            }
+            if (inj) {
+                __syncthreads();
+                const cplx<T>* __restrict__ g = SH;
+#pragma unroll 4
+                for (int i = tid; i < N; i += NT) {
+                    const cplx<T> v = sm[phys<T>(i)], sv = g[i];
+                    sm[phys<T>(i)] = {v.re + tinj * sv.re, v.im + tinj * sv.im};
+                }
+                if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }
             }
             if (keep) {   // keep it for the later round trips
                 __syncthreads();
@@ -439,6 +465,11 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                 } else {
 #pragma unroll 4
                     for (int i = tid; i < N; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
+                }
+                if (inj_any) {     // input coupler (reading R24)
+                    const cplx<T>* __restrict__ Sp = reinterpret_cast<const cplx<T>*>(a.S[x]) + (size_t)b * N;
+#pragma unroll 4
+                    for (int i = tid; i < N; i += NT) { const cplx<T> v = cur[i], sv = Sp[i]; cur[i] = {v.re + tinj * sv.re, v.im + tinj * sv.im}; }
                 }
             } else {
                 const cplx<T>* __restrict__ S = reinterpret_cast<const cplx<T>*>(a.S[x]) + (size_t)b * N;

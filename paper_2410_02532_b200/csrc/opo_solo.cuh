@@ -326,6 +326,22 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
             for (int i = tid; i < N; i += NT) g[i] = sm[phys<T>(i)];
         };
 
+        // resonant pump (reading R24): the input coupler adds t S_p at every boundary, and the first half-step of the next
+        // pass acts on the sum: SH_p <- IDFT(H DFT(S_p)) (up to its inverse pass 0) once per piece of work, t SH_p is added
+        // after the merged boundary operator at every crossing
+        const T tinj = (T)a.inject;
+        const bool inj_any = tinj != (T)0 && a.resonant[0] != 0;
+        if (inj_any && rt_mode && steps_l > 1) {
+            load(reinterpret_cast<const cplx<T>*>(a.S[0]) + (size_t)b * N);
+            __syncthreads();
+            pass0_local<T, L, NT>(tw, tid, false);
+            __syncthreads();
+            linear_core_smem<T, L, NT>(reinterpret_cast<const cplx<T>*>(a.tabH[0]), tid);
+            __syncthreads();
+            store(reinterpret_cast<cplx<T>*>(a.SH[0]) + (size_t)b * N);
+            __syncthreads();
+        }
+
         // ---- bring the instance on chip: every field through shared memory and forward pass 0; fields 1.. park in TMEM
         if (a.split && rt0 > 0) {       // the earlier round trips of this instance ran on another CTA
             if (tid == 0) {
@@ -365,6 +381,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                 const bool keep = rt_mode && q == 0 && !resonant && steps_l > 1;     // SH <- first half-stepped input
                 const bool first_core = q == 0 && x == 0;                             // no transition precedes
                 const bool last_core = q == total && x == F - 1;                      // no transition follows
+                const bool inj = x == 0 && crossing && inj_any;                       // input coupler of a resonant pump
                 const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
                 cplx<T>* SH = reinterpret_cast<cplx<T>*>(a.SH[x]) + (size_t)b * N;
                 if (crossing && !resonant) {
@@ -385,13 +402,23 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                     __syncthreads();
                     pass0_local<T, L, NT>(tw, tid, false);
                     __syncthreads();
-                    core(tabH, false, true);
+                    core(tabH, false, !inj);
                 } else {
                     const cplx<T>* tab = tabH;
                     if (q != 0 && q != total)
                         tab = crossing ? reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x]
                                        : reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
-                    core(tab, !first_core, !last_core && !keep);
+                    core(tab, !first_core, !last_core && !keep && !inj);
+                }
+                if (inj) {
+                    __syncthreads();
+                    const cplx<T>* __restrict__ g = SH;
+#pragma unroll 4
+                    for (int i = tid; i < N; i += NT) {
+                        const cplx<T> v = sm[phys<T>(i)], sv = g[i];
+                        sm[phys<T>(i)] = {v.re + tinj * sv.re, v.im + tinj * sv.im};
+                    }
+                    if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }
                 }
                 if (keep) {   // keep it for the later round trips
                     __syncthreads();
@@ -442,6 +469,11 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                     } else {
 #pragma unroll 4
                         for (int i = tid; i < N; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
+                    }
+                    if (x == 0 && inj_any) {     // input coupler (reading R24)
+                        const cplx<T>* __restrict__ Sp = reinterpret_cast<const cplx<T>*>(a.S[0]) + (size_t)b * N;
+#pragma unroll 4
+                        for (int i = tid; i < N; i += NT) { const cplx<T> v = cur[i], sv = Sp[i]; cur[i] = {v.re + tinj * sv.re, v.im + tinj * sv.im}; }
                     }
                 } else {
                     const cplx<T>* __restrict__ Sx = reinterpret_cast<const cplx<T>*>(a.S[x]) + (size_t)b * N;

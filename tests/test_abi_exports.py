@@ -51,7 +51,7 @@ def test_invalid_arguments_are_rejected_before_touching_the_device():
               resonant=[0, 1], R=[0, 0.98])
     for bad, status in ((dict(n_fields=4), P.ERR_INVALID_ARG), (dict(log2_n=30), P.ERR_INVALID_ARG),
                         (dict(nz_per_pass=0), P.ERR_INVALID_ARG), (dict(R=[0, 1.5]), P.ERR_INVALID_ARG),
-                        (dict(resonant=[1, 1]), P.ERR_UNSUPPORTED)):
+                        (dict(resonant=[1, 1], log2_n=16), P.ERR_UNSUPPORTED)):      # resonant pump: not on the large-N engine
         with pytest.raises(P.OpoError) as e:
             P.Opo(**{**kw, **bad})
         assert e.value.status == status, bad

@@ -210,6 +210,82 @@ def test_boundary_without_transform_and_nonresonant_restart(engine_idx):
 
 
 # ---------------------------------------------------------------------------------------------------------
+# resonant pump (input coupler, reading R24) and several crystals in series (reading R25)
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("engine_idx", ENGINE_IDX)
+@pytest.mark.parametrize("precision,log2_n,n_fields,calls,eom", [
+    ("c128", 9, 3, 1, False), ("c128", 10, 2, 2, True), ("c64", 12, 3, 1, False), ("c64", 14, 3, 2, False), ("c64", 8, 2, 1, True)])
+def test_resonant_pump_matches_oracle(precision, log2_n, n_fields, calls, eom, engine_idx):
+    """Doubly / triply resonant cavity: the pump is mirrored like the other resonant fields (own R_p, carrier phase, GDD)
+    and the input coupler adds sqrt(1 - R_p) S_p at every boundary; inside the on-chip kernels that is t SH_p added after
+    the merged boundary operator.  4 round trips in one call and split over two calls (the un-merged boundary of the
+    call's last round trip), per-instance detuning of the pump, a modulator on the pump before the coupler."""
+    engine = engines()[engine_idx]
+    w = small_workload(log2_n, n_fields, precision, nz=4, batch=3, dk=-20.0, gdd_dt2=-1.3, drad=0.4, strong=False)
+    w.resonant = [1, 1, 1][:n_fields]
+    w.R = [0.6, 0.9, 0.7][:n_fields]
+    w.delta_rad = [0.35, 0.4, -0.2][:n_fields]
+    w.gdd_s2 = [0.8 * w.dt ** 2] + list(w.gdd_s2[1:])
+    if eom:
+        w.eom_beta_rad = [0.5, 0.0, 0.0]
+        w.eom_f_hz = [2.0 / w.window_s, 0.0, 0.0]
+    _engine_or_skip(w, engine)
+    cur, ex, eng = run_gpu(w, engine, n_roundtrips=4, calls=calls)
+    assert eng == engine
+    rcur, rex = run_oracle(w, n_roundtrips=4)
+    tol = TOL[precision] if precision == "c128" else 3e-5
+    assert_close(cur, rcur, tol, "current")
+    assert_close(ex, rex, tol, "exit")
+    # the cavity really stored pump light: the intracavity pump differs from what a single-pass pump would be
+    assert rel_l2(cur[0, 0], np.sqrt(1 - 0.6) * w.pump[0]) > 0.05
+
+
+def test_resonant_pump_builds_up_in_a_cold_cavity():
+    """Airy build-up measured on the CUDA path alone (no oracle): coupling off, CW pump on resonance, after many round
+    trips the intracavity pump power is (1 - R) / (1 - sqrt(R))^2 times the input."""
+    torch, P = _gpu()
+    w = small_workload(10, 2, "c128", nz=2, batch=1, strong=False)
+    w.d_eff_m_per_V = 0.0
+    w.resonant, w.R, w.delta_rad, w.gdd_s2 = [1, 0], [0.5, 0.0], [0.0, 0.0], [0.0, 0.0]
+    w.beta1_s_per_m, w.beta2_s2_per_m = [0.0, 0.0], [0.0, 0.0]
+    w.pump = np.ones((1, w.n), dtype=np.complex128)
+    for engine in (P.ENGINE_RESIDENT, P.ENGINE_SOLO, P.ENGINE_STREAMING):
+        cur, _, _ = run_gpu(w, engine, n_roundtrips=120)
+        assert abs(np.mean(np.abs(cur[0, 0]) ** 2) / ((1 - 0.5) / (1 - np.sqrt(0.5)) ** 2) - 1) < 1e-10
+
+
+@pytest.mark.parametrize("precision,log2_n,n_fields,splitting", [("c128", 9, 3, 0), ("c64", 12, 3, 0), ("c64", 14, 2, 0), ("c128", 8, 2, 1), ("c64", 11, 3, 1)])
+def test_crystal_segments_match_oracle(precision, log2_n, n_fields, splitting):
+    """Three crystals in series with different length, step size, dk and d_eff (the last one reversed): partial passes
+    that stop inside the second crystal, then round trips with the boundary merged across the last and first crystal's
+    half-steps; per-instance dk on the first crystal.  Runs on the host-sequenced streaming engine (AUTO picks it)."""
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=9, batch=2, dk=30.0, gdd_dt2=-0.9, drad=0.3, strong=False)
+    L = w.length_m
+    w.segments = [(0.5 * L, 30.0, w.d_eff_m_per_V, 4), (0.2 * L, -90.0, 0.6 * w.d_eff_m_per_V, 2), (0.3 * L, 10.0, -w.d_eff_m_per_V, 3)]
+    w.splitting = splitting
+    cur, _, eng = run_gpu(w, P.ENGINE_AUTO, propagate=[5, 1, 3])
+    assert eng == P.ENGINE_STREAMING
+    ref, _ = run_oracle(w, propagate=[9])
+    tol = TOL[precision] if precision == "c128" else 3e-5
+    assert_close(cur, ref, tol, "single pass through three crystals")
+    cur, ex, _ = run_gpu(w, P.ENGINE_AUTO, n_roundtrips=3)
+    rcur, rex = run_oracle(w, n_roundtrips=3)
+    assert_close(cur, rcur, tol, "current")
+    assert_close(ex, rex, tol, "exit")
+    # and the ABI's own rules
+    o = P.from_workload(w)
+    o.propagate(2)
+    with pytest.raises(P.OpoError) as e:
+        o.set_segments([(L, 0.0, 1e-12, 5)])
+    assert e.value.status == P.ERR_STATE
+    with pytest.raises(P.OpoError) as e:
+        o.propagate(8)                      # 2 + 8 > 9 steps per pass
+    assert e.value.status == P.ERR_STATE
+    o.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
 # the five configurations of BASELINE.json (truncated to <= 20 round trips where they are longer)
 # ---------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("engine_idx", ENGINE_IDX)
@@ -795,8 +871,8 @@ def test_abi_errors_and_state():
     o.check_finite()
     o.close()
     with pytest.raises(P.OpoError) as e:
-        bad = small_workload(8, 2, "c64")
-        bad.resonant = [1, 1]
+        bad = small_workload(16, 2, "c64")
+        bad.resonant = [1, 1]               # a resonant pump is not available on the large-N engine
         P.from_workload(bad)
     assert e.value.status == P.ERR_UNSUPPORTED
     with pytest.raises(P.OpoError) as e:
