@@ -29,13 +29,17 @@
 
 namespace opo {
 
+#ifndef OPO_LARGE_TC
+#define OPO_LARGE_TC 4
+#endif
+
 template <class T> struct large_tab { using type = cplx<T>; };
 template <> struct large_tab<float> { using type = tabx<float>; };
 
 template <class T, int L, int F> struct large_cfg {
     static constexpr int L1 = L / 2, L2 = L - L1;
     static constexpr int N1 = 1 << L1, N2 = 1 << L2, N = 1 << L;
-    static constexpr int TC = 4;                       // columns per tile
+    static constexpr int TC = OPO_LARGE_TC;            // columns per tile
     static constexpr int TT1 = N1 / 16, TT2 = N2 / 16; // threads per column / row transform
     static constexpr int NT = F * TC * TT1;            // one team per (field, column)
     static constexpr int ROWS = NT / TT2;              // rows per chunk in the row pass
@@ -67,13 +71,14 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
     target += gridDim.x;
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(ctr, 1ULL);
+        // arrive: the release orders this CTA's global stores (made visible to this thread by the __syncthreads) before
+        // the increment; wait: relaxed polls (no cache invalidation per poll), one acquire fence at the end
+        asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
         unsigned long long v;
         do {
-            asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+            asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
         } while (v < target);
-        __threadfence();
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
     }
     __syncthreads();
 }
@@ -155,14 +160,27 @@ template <class T, int L, int F> struct LargeEngine {
 #pragma unroll 1
         for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             const int b = tile / C::TILES_PER_INST, c0 = (tile % C::TILES_PER_INST) * C::TC;
+            {   // all loads of the tile are in flight before the first one is consumed (the pass is latency-bound)
+                constexpr int CNT = (C::N1 * C::TC + C::NT - 1) / C::NT;
+                cplx<T> r[F][CNT];
 #pragma unroll
-            for (int x = 0; x < F; ++x) {
-                if (!((mask >> x) & 1)) continue;
-                const cplx<T>* g = src[x] + (size_t)b * C::N + c0;
-#pragma unroll 4
-                for (int i = tid; i < C::N1 * C::TC; i += C::NT) {
-                    const int n1 = i / C::TC, c = i % C::TC;
-                    sm[(x * C::TC + c) * C::CSTRIDE + phys<T>(n1)] = ldcg(g + (size_t)n1 * C::N2 + c);
+                for (int x = 0; x < F; ++x) {
+                    if (!((mask >> x) & 1)) continue;
+                    const cplx<T>* g = src[x] + (size_t)b * C::N + c0;
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) {
+                        const int i = tid + j * C::NT;
+                        if (i < C::N1 * C::TC) r[x][j] = ldcg(g + (size_t)(i / C::TC) * C::N2 + (i % C::TC));
+                    }
+                }
+#pragma unroll
+                for (int x = 0; x < F; ++x) {
+                    if (!((mask >> x) & 1)) continue;
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) {
+                        const int i = tid + j * C::NT;
+                        if (i < C::N1 * C::TC) sm[(x * C::TC + i % C::TC) * C::CSTRIDE + phys<T>(i / C::TC)] = r[x][j];
+                    }
                 }
             }
             // pointwise RK4 half-step on the tile in the time domain (Eq. 10-11)
@@ -258,9 +276,13 @@ template <class T, int L, int F> struct LargeEngine {
                 continue;
             }
             const int k1 = __ldg(&perm1[active ? r : 0]);
-            if (active) {
-#pragma unroll 4
-                for (int i = lt; i < C::N2; i += C::TT2) smt[phys<T>(i)] = cmul(ldcg(g + i), big_twiddle(k1, i));
+            if (active) {       // all loads of the row in flight before the first one is consumed
+                constexpr int CNT = C::N2 / C::TT2;
+                cplx<T> r[CNT];
+#pragma unroll
+                for (int j = 0; j < CNT; ++j) r[j] = ldcg(g + lt + j * C::TT2);
+#pragma unroll
+                for (int j = 0; j < CNT; ++j) smt[phys<T>(lt + j * C::TT2)] = cmul(r[j], big_twiddle(k1, lt + j * C::TT2));
             }
             __syncthreads();
             if (kind == ROW_FREQ) {
