@@ -185,7 +185,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--rt-per-step", type=int, default=0, help="round trips per step (default: the config's full length for C4 and C0, 100 for C1, 20 for C2, 2 for C3)")
-    ap.add_argument("--engine", default="auto", choices=["auto", "resident", "solo", "streaming", "cufft"],
+    ap.add_argument("--engine", default="auto", choices=["auto", "resident", "solo", "wide", "streaming", "cufft"],
                     help="cufft = the internal cuFFT + elementwise-kernel baseline (north_star item (d)), not the product")
     ap.add_argument("--eom", action="store_true",
                     help="intracavity phase modulator on the signal (PAPER.md:L149-154; beta = 1 rad, f = 3 / window): the "
@@ -223,7 +223,7 @@ def main():
         w.eom_beta_rad = [0.0, 1.0, 0.0]
         w.eom_f_hz = [0.0, 3.0 / w.window_s, 0.0]
     rt_per_step = args.rt_per_step or {"C0": w.n_roundtrips, "C1": 100, "C2": 20, "C3": 2, "C4": w.n_roundtrips}[args.workload]
-    engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "solo": P.ENGINE_SOLO, "streaming": P.ENGINE_STREAMING, "cufft": P.ENGINE_CUFFT}[args.engine]
+    engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "solo": P.ENGINE_SOLO, "wide": P.ENGINE_WIDE, "streaming": P.ENGINE_STREAMING, "cufft": P.ENGINE_CUFFT}[args.engine]
     o = P.from_workload(w, engine=engine)
     units_per_step = w.batch * w.n * w.nz_per_pass * rt_per_step          # grid-point z-steps, this rank
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
@@ -299,9 +299,9 @@ def main():
     # ---- roofline of the dominant kernel ----------------------------------------------------
     avg_s = statistics.mean(per_step_ms) * 1e-3
     eng = o.engine
-    eng_name = {P.ENGINE_RESIDENT: "resident", P.ENGINE_SOLO: "solo", P.ENGINE_STREAMING: "streaming", P.ENGINE_LARGE: "large", P.ENGINE_CUFFT: "cufft"}.get(eng, str(eng))
+    eng_name = {P.ENGINE_RESIDENT: "resident", P.ENGINE_SOLO: "solo", P.ENGINE_WIDE: "wide", P.ENGINE_STREAMING: "streaming", P.ENGINE_LARGE: "large", P.ENGINE_CUFFT: "cufft"}.get(eng, str(eng))
     traffic, traffic_source = ncu_traffic(args.workload, eng_name, rt_per_step)
-    if eng in (P.ENGINE_RESIDENT, P.ENGINE_SOLO):
+    if eng in (P.ENGINE_RESIDENT, P.ENGINE_SOLO, P.ENGINE_WIDE):
         # fields stay on chip (shared memory / tensor memory): bound by the FP32 (FP64) FMA pipe, shared memory second.
         # Both peaks are MEASURED here, on this device, by the library's own micro-benchmark kernels (opo_selftest_peak).
         fl = flops_per_grid_point_zstep(w.log2_n, w.n_fields) * units_per_step          # per launch (= per step)
@@ -312,7 +312,7 @@ def main():
         peak_meas = P.opo_selftest_peak(P.PEAK_FP64_FMA if dbl else P.PEAK_FP32_FMA)
         smem_peak = P.opo_selftest_peak(P.PEAK_SMEM)
         smem_by = smem_bytes_per_field_point_zstep(w.precision) * w.n_fields * units_per_step
-        roofline = {"bound": "alu", "kernel": "k_solo" if eng == P.ENGINE_SOLO else "k_resident", "achieved": fl / avg_s / 1e12,
+        roofline = {"bound": "alu", "kernel": {P.ENGINE_SOLO: "k_solo", P.ENGINE_WIDE: "k_wide"}.get(eng, "k_resident"), "achieved": fl / avg_s / 1e12,
                     "peak": peak_meas, "unit": "TFLOP/s", "frac": fl / avg_s / 1e12 / peak_meas,
                     "peak_nominal": peak_nominal, "frac_of_nominal": fl / avg_s / 1e12 / peak_nominal,
                     "traffic": traffic, "traffic_source": traffic_source,

@@ -220,6 +220,14 @@ int opo_get_z_steps(const opo_handle* h, int* out_steps);
  * batches that keep (nearly) every SM busy (BASELINE.json configs[4]), RESIDENT for few instances (lowest latency per
  * instance).  The N/2 - L - N/2 ordering runs on RESIDENT. */
 #define OPO_ENGINE_SOLO 5
+/* WIDE: one thread-block cluster of 4 F CTAs per instance (N = 2^12 .. 2^14; c128: 2^12, 2^13): every field is split
+ * over four SMs along the radix-4 first pass of the transform, the pass that crosses the split (fused with the RK4
+ * step) exchanges its operands over distributed shared memory; one launch per opo_propagate /
+ * opo_roundtrips.  The lowest latency per z-step: AUTO picks it when the whole batch fits the co-resident clusters in
+ * one wave (the paper's own workload, one OPO followed for thousands of round trips; BASELINE.json
+ * configs[1], [2]).  Not with the N/2 - L - N/2 ordering, a phase modulator or a resonant pump: those run on RESIDENT
+ * (a request for WIDE is then served by RESIDENT / SOLO as AUTO would). */
+#define OPO_ENGINE_WIDE 6
 #define OPO_OPT_ENGINE 0
 /* Operator splitting of a z-step.  LNL (default, BASELINE.json north_star): linear half-step,
  * one RK4 step h, linear half-step.  NLN: the order the paper implements, Eq. 10-11: one RK4 step of h/2, the full

@@ -23,7 +23,7 @@ PRECISION_C64, PRECISION_C128 = 0, 1
 PARAM_DK, PARAM_DELTA_T, PARAM_DELTA_RAD, PARAM_GDD = 0, 1, 2, 3
 WHICH_CURRENT, WHICH_EXIT = 0, 1
 DOMAIN_TIME, DOMAIN_FREQ = 0, 1
-ENGINE_AUTO, ENGINE_RESIDENT, ENGINE_STREAMING, ENGINE_LARGE, ENGINE_CUFFT, ENGINE_SOLO = 0, 1, 2, 3, 4, 5
+ENGINE_AUTO, ENGINE_RESIDENT, ENGINE_STREAMING, ENGINE_LARGE, ENGINE_CUFFT, ENGINE_SOLO, ENGINE_WIDE = 0, 1, 2, 3, 4, 5, 6
 OPT_ENGINE = 0
 OPT_SPLITTING = 1
 SPLITTING_LNL, SPLITTING_NLN = 0, 1

@@ -20,6 +20,8 @@ LIB = os.path.join(HERE, "libopo.so")
 PLAIN_SOURCES = ["opo_api.cu", "opo_dispatch.cu", "opo_pointwise.cu", "opo_selftest.cu"]
 # (type, suffix, log2 N): one object per size-specialised instance of opo_inst.cu
 INSTANCES = [("float", "f32", l) for l in range(6, 15)] + [("double", "f64", l) for l in range(6, 14)]
+# wide engine (a cluster of 4 F CTAs per instance): the sizes whose plan is 4 . 16 . r . r'
+WIDE_INSTANCES = [("float", "f32", l) for l in range(12, 15)] + [("double", "f64", l) for l in range(12, 14)]
 LARGE_INSTANCES = [("float", "f32", l) for l in range(15, 19)] + [("double", "f64", l) for l in range(14, 19)]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
@@ -70,6 +72,11 @@ def _jobs(only=None):
         # the solo engine (one CTA per instance, fields in shared + tensor memory): general and dk = 0 instantiations
         jobs.append(("opo_inst_solo.cu", f"opo_inst_solo_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
         jobs.append(("opo_inst_solo.cu", f"opo_inst_solo_dk0_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_DK0"]))
+    for typ, suf, l in WIDE_INSTANCES:
+        if only and f"{suf}:{l}" not in only:
+            continue
+        jobs.append(("opo_inst_wide.cu", f"opo_inst_wide_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
+        jobs.append(("opo_inst_wide.cu", f"opo_inst_wide_dk0_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_DK0"]))
     for typ, suf, l in LARGE_INSTANCES:
         if only and f"{suf}:{l}" not in only:
             continue

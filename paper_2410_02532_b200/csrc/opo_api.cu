@@ -157,6 +157,8 @@ struct opo_handle {
     void* segHX[8][3] = {};                           //   H_j H_{j+1} / N across the junction of two crystals
     bool solo_ok = false;                             // solo engine (one CTA per instance, fields in shared + tensor memory)
     opo::ResidentInfo sinfo{};                        // max_clusters = co-resident CTAs on the device
+    bool wide_ok = false;                             // wide engine (a cluster of 4 F CTAs per instance)
+    opo::ResidentInfo winfo{};                        // max_clusters = co-resident clusters of 4 F CTAs
     int device = 0;
     long long launches = 0;
     std::string err;
@@ -583,6 +585,9 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
         e = h->dbl ? opo::solo_info_f64(h->L, h->F, &h->sinfo) : opo::solo_info_f32(h->L, h->F, &h->sinfo);
         h->solo_ok = (e == cudaSuccess && h->sinfo.max_clusters > 0);
         if (e != cudaSuccess) cudaGetLastError();
+        e = h->dbl ? opo::wide_info_f64(h->L, h->F, &h->winfo) : opo::wide_info_f32(h->L, h->F, &h->winfo);
+        h->wide_ok = (e == cudaSuccess && h->winfo.max_clusters > 0);
+        if (e != cudaSuccess) cudaGetLastError();
     }
     if (cudaDeviceSynchronize() != cudaSuccess) return bail(OPO_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
     *out = h;
@@ -665,15 +670,36 @@ bool prefer_solo(const opo_handle* h) {
     return solo_slots > 2.6 * cluster_slots;
 }
 
+// The wide engine serves the default ordering without a modulator and without a resonant pump (opo_wide.cuh).
+bool wide_serves(const opo_handle* h) {
+    if (!h->wide_ok || h->splitting || h->n_seg > 1 || h->fields.resonant[0]) return false;
+    for (int x = 0; x < h->F; ++x)
+        if (h->eom[x]) return false;
+    return true;
+}
+
+// AUTO takes the wide engine (4 F SMs per instance, the lowest latency per z-step) when the whole batch fits the
+// co-resident clusters of 4 F CTAs in one wave and would leave most of the GPU idle on the cluster engine.
+bool prefer_wide(const opo_handle* h) {
+    return wide_serves(h) && h->B <= h->winfo.max_clusters;
+}
+
 int engine_in_use(const opo_handle* h) {
     if (h->large) return OPO_ENGINE_LARGE;
     if (h->n_seg > 1) return OPO_ENGINE_STREAMING;       // several crystals in series: host-sequenced engine only
     if (h->engine_opt == OPO_ENGINE_STREAMING) return OPO_ENGINE_STREAMING;
     if (h->engine_opt == OPO_ENGINE_CUFFT) return OPO_ENGINE_CUFFT;
+    if (h->engine_opt == OPO_ENGINE_WIDE && wide_serves(h)) return OPO_ENGINE_WIDE;
     if (h->engine_opt == OPO_ENGINE_SOLO && h->solo_ok && !h->splitting) return OPO_ENGINE_SOLO;
     if (h->engine_opt == OPO_ENGINE_RESIDENT && h->resident_ok) return OPO_ENGINE_RESIDENT;
+    if (h->engine_opt == OPO_ENGINE_AUTO && prefer_wide(h)) return OPO_ENGINE_WIDE;
     if (prefer_solo(h)) return OPO_ENGINE_SOLO;
     return h->resident_ok ? OPO_ENGINE_RESIDENT : OPO_ENGINE_STREAMING;
+}
+
+bool on_chip_engine(const opo_handle* h) {
+    const int e = engine_in_use(h);
+    return e == OPO_ENGINE_RESIDENT || e == OPO_ENGINE_SOLO || e == OPO_ENGINE_WIDE;
 }
 
 // ---- streaming engine ------------------------------------------------------------------------------------------
@@ -825,11 +851,11 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     a.mode = mode; a.z0 = z0; a.steps = steps; a.nln = h->splitting;
     a.dk0 = !h->splitting;
     for (int b = 0; b < h->B; ++b) if (h->dk[b] != 0.0) a.dk0 = 0;
-    const bool solo = engine_in_use(h) == OPO_ENGINE_SOLO;
-    const int n_clusters = std::min(h->B, solo ? h->sinfo.max_clusters : h->rinfo.max_clusters);
+    const bool solo = engine_in_use(h) == OPO_ENGINE_SOLO, wide = engine_in_use(h) == OPO_ENGINE_WIDE;
+    const int n_clusters = std::min(h->B, wide ? h->winfo.max_clusters : solo ? h->sinfo.max_clusters : h->rinfo.max_clusters);
     // more instances than clusters and not a multiple: deal round trips instead of instances (see the kernel)
     a.split = 0; a.flags = nullptr;
-    if (mode == 1 && !h->splitting && steps > 1 && h->B > n_clusters && h->B % n_clusters != 0) {
+    if (mode == 1 && !wide && !h->splitting && steps > 1 && h->B > n_clusters && h->B % n_clusters != 0) {
         if (!h->rt_flags && cudaMalloc((void**)&h->rt_flags, (size_t)h->B * 3 * sizeof(int)) != cudaSuccess) {
             cudaGetLastError();
             return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the round-trip flags failed");
@@ -838,6 +864,7 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
         a.split = 1; a.flags = h->rt_flags;
     }
     auto launch = [&]() {
+        if (wide) return h->dbl ? opo::launch_wide_f64(h->L, a, n_clusters, h->stream) : opo::launch_wide_f32(h->L, a, n_clusters, h->stream);
         if (solo) return h->dbl ? opo::launch_solo_f64(h->L, a, n_clusters, h->stream) : opo::launch_solo_f32(h->L, a, n_clusters, h->stream);
         return h->dbl ? opo::launch_resident_f64(h->L, a, n_clusters, h->stream) : opo::launch_resident_f32(h->L, a, n_clusters, h->stream);
     };
@@ -996,7 +1023,7 @@ int opo_propagate(opo_handle* h, int nz) {
     if (int rc = ensure_tables(h)) return rc;
     int rc;
     if (h->large) rc = large_run(h, 0, h->z_steps, nz);
-    else if (engine_in_use(h) == OPO_ENGINE_RESIDENT || engine_in_use(h) == OPO_ENGINE_SOLO) rc = resident_run(h, 0, h->z_steps, nz);
+    else if (on_chip_engine(h)) rc = resident_run(h, 0, h->z_steps, nz);
     else rc = stream_steps(h, h->z_steps, nz, false);
     if (rc) return rc;
     h->z_steps += nz;
@@ -1021,7 +1048,7 @@ int opo_roundtrips(opo_handle* h, int n) {
         }
         return OPO_OK;
     }
-    if (engine_in_use(h) == OPO_ENGINE_RESIDENT || engine_in_use(h) == OPO_ENGINE_SOLO) {
+    if (on_chip_engine(h)) {
         // a modulator is applied inside the kernel (between two linear cores at a crossing, with the last store at the
         // end of a call); only the N/2 - L - N/2 ordering runs one pass per launch
         if (!h->splitting) return resident_run(h, 1, 0, n);
@@ -1169,7 +1196,7 @@ int opo_set_option(opo_handle* h, int option, int value) {
     }
     if (option != OPO_OPT_ENGINE) return fail(h, OPO_ERR_INVALID_ARG, "unknown option");
     if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING && value != OPO_ENGINE_LARGE &&
-        value != OPO_ENGINE_CUFFT && value != OPO_ENGINE_SOLO)
+        value != OPO_ENGINE_CUFFT && value != OPO_ENGINE_SOLO && value != OPO_ENGINE_WIDE)
         return fail(h, OPO_ERR_INVALID_ARG, "unknown engine");
     if (value == OPO_ENGINE_CUFFT) {
         if (h->large) return fail(h, OPO_ERR_UNSUPPORTED, "the cuFFT baseline serves the sizes of the streaming engine");
@@ -1196,6 +1223,8 @@ int opo_set_option(opo_handle* h, int option, int value) {
         return fail(h, OPO_ERR_UNSUPPORTED, "resident engine unavailable for this size/precision on this device");
     if (value == OPO_ENGINE_SOLO && !h->solo_ok)
         return fail(h, OPO_ERR_UNSUPPORTED, "solo engine unavailable for this size/precision on this device");
+    if (value == OPO_ENGINE_WIDE && !h->wide_ok)
+        return fail(h, OPO_ERR_UNSUPPORTED, "wide engine unavailable for this size/precision on this device (N = 2^12 .. 2^14; c128: 2^12, 2^13)");
     h->engine_opt = value;
     return OPO_OK;
 }
@@ -1211,6 +1240,7 @@ int opo_get_info(const opo_handle* h, int what, long long* out) {
         case OPO_INFO_SLOTS: {
             const int e = engine_in_use(h);
             if (e == OPO_ENGINE_SOLO) *out = std::min(h->B, h->sinfo.max_clusters);
+            else if (e == OPO_ENGINE_WIDE) *out = std::min(h->B, h->winfo.max_clusters);
             else if (e == OPO_ENGINE_RESIDENT) *out = std::min(h->B, h->rinfo.max_clusters);
             else if (e == OPO_ENGINE_LARGE) *out = h->linfo.grid;
             else *out = (long long)h->B * h->F;

@@ -71,6 +71,34 @@ template <class T> __device__ __forceinline__ cplx<T> cmulc(cplx<T> a, cplx<T> b
     return {a.re * b.re + a.im * b.im, a.im * b.re - a.re * b.im};
 }
 
+// a * conj(b) / |b|^2 to first order, for a rounded unit-modulus b.  A forward pass multiplies by the rounded twiddle w and
+// the inverse pass by conj(w), so the pair scales its butterfly leg by |w|^2 = 1 + d, d ~ 3e-8 rms in fp32 -- the same d at
+// every z-step.  Twiddle *phase* rounding is a similarity transform of the step and does not accumulate; this magnitude
+// defect does, linearly in the number of z-steps, while the data rounding errors add up as a random walk (measured on
+// IDFT(DFT(A)) alone: 3.5e-8 per z-step, 3.5e-4 after the 10^4 z-steps of C3 x 20 round trips; with the defect taken out
+// the same loop grows as sqrt(n)).  No choice of float pair near the unit circle helps (for small angles the granularity
+// of cos alone is 1.2e-7 in |w|^2).  d is evaluated without cancellation error -- the larger component has a^2 >= 1/2, so
+// a^2 - 1 is exact, and an FMA recovers the rounding of a^2 -- and the correction -d a conj(b), which is smaller than
+// half an ulp of the result, enters the sum BEFORE its single rounding (applied after the rounding it would be rounded
+// away again, every time).  fp64: d ~ 1e-16, nothing to do.
+__device__ __forceinline__ float unit_defect(cplx<float> w) {
+    const float ar = fabsf(w.re), ai = fabsf(w.im);
+    const float a = fmaxf(ar, ai), b = fminf(ar, ai);
+    const float p = a * a;
+    const float e = __fmaf_rn(a, a, -p);
+    return __fmaf_rn(b, b, p - 1.0f) + e;
+}
+// d = |b|^2 - 1 supplied by the caller
+__device__ __forceinline__ cplx<float> cmulc_unit(cplx<float> a, cplx<float> b, float d) {
+    const float re0 = __fmaf_rn(a.re, b.re, a.im * b.im), im0 = __fmaf_rn(a.im, b.re, -(a.re * b.im));
+    const float sr = -d * re0, si = -d * im0;
+    return {__fmaf_rn(a.re, b.re, __fmaf_rn(a.im, b.im, sr)), __fmaf_rn(a.im, b.re, __fmaf_rn(-a.re, b.im, si))};
+}
+template <class T> __device__ __forceinline__ cplx<T> cmulc_unit(cplx<T> a, cplx<T> b) {
+    if constexpr (sizeof(T) == 4) return cmulc_unit(a, b, unit_defect(b));
+    else return cmulc(a, b);
+}
+
 // read-only (non-coherent) global load of one complex value
 __device__ __forceinline__ cplx<float> ldg(const cplx<float>* p) {
     float2 v = __ldg(reinterpret_cast<const float2*>(p));
@@ -312,7 +340,8 @@ __device__ __forceinline__ void fwd_pass_smem(cplx<T>* __restrict__ sm, const cp
 }
 
 // ---- one inverse (DIT) pass over shared memory ---------------------------------------------------------
-template <class T, int L, int PASS, int NT, bool TWS>
+// UF: the twiddle multiply takes the twiddle's magnitude defect out (cmulc_unit)
+template <class T, int L, int PASS, int NT, bool TWS, bool UF = false>
 __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid) {
     using PL = plan<L>;
     constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
@@ -327,7 +356,10 @@ __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cp
         for (int k = 0; k < R; ++k) v[k] = p[elem_off<T, RB, SB>(k)];
         if constexpr (SB > 0) {
 #pragma unroll
-            for (int k = 1; k < R; ++k) v[k] = cmulc(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
+            for (int k = 1; k < R; ++k) {
+                if constexpr (UF) v[k] = cmulc_unit(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
+                else v[k] = cmulc(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
+            }
         }
         dit_inv<T, R>::run(v);
 #pragma unroll
@@ -388,22 +420,27 @@ __device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const TA
     }
 }
 
+// barrier between two shared-memory passes: the whole CTA, or (WS) the warp when a transform's team never spans warps
+template <bool WS> __device__ __forceinline__ void pass_sync() {
+    if constexpr (WS) __syncwarp();
+    else __syncthreads();
+}
 // forward passes FIRST .. P-2 (everything before the fused middle), with the barriers between them
-template <class T, int L, int NT, bool TWS, int PASS>
+template <class T, int L, int NT, bool TWS, int PASS, bool WS = false>
 __device__ __forceinline__ void fwd_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
     if constexpr (PASS < plan<L>::P - 1) {
         fwd_pass_smem<T, L, PASS, NT, TWS>(sm, tw, tid);
-        __syncthreads();
-        fwd_passes<T, L, NT, TWS, PASS + 1>(sm, tw, tid);
+        pass_sync<WS>();
+        fwd_passes<T, L, NT, TWS, PASS + 1, WS>(sm, tw, tid);
     }
 }
 // inverse passes P-2 .. LAST
-template <class T, int L, int NT, bool TWS, int LAST, int PASS = plan<L>::P - 2>
+template <class T, int L, int NT, bool TWS, int LAST, bool WS = false, bool UF = false, int PASS = plan<L>::P - 2>
 __device__ __forceinline__ void inv_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
     if constexpr (PASS >= LAST) {
-        __syncthreads();
-        inv_pass_smem<T, L, PASS, NT, TWS>(sm, tw, tid);
-        inv_passes<T, L, NT, TWS, LAST, PASS - 1>(sm, tw, tid);
+        pass_sync<WS>();
+        inv_pass_smem<T, L, PASS, NT, TWS, UF>(sm, tw, tid);
+        inv_passes<T, L, NT, TWS, LAST, WS, UF, PASS - 1>(sm, tw, tid);
     }
 }
 

@@ -1,5 +1,5 @@
 // opo_internal.h -- plain-C++ interface between the host library (opo_api.cu) and the templated
-// kernel launchers (opo_inst.cu, opo_inst_solo.cu, opo_inst_large.cu, one object per precision and size,
+// kernel launchers (opo_inst.cu, opo_inst_solo.cu, opo_inst_wide.cu, opo_inst_large.cu, one object per precision and size,
 // routed by opo_dispatch.cu).  No CUDA templates leak through here.
 #pragma once
 #include <cuda_runtime.h>
@@ -67,6 +67,7 @@ struct FreqArgs {
 // ---- resident (cluster) engine and solo engine ---------------------------------------------------------
 // Cluster engine: one thread-block cluster per instance, CTA rank = field (opo_resident.cuh).
 // Solo engine: one CTA per instance, one field in shared memory, the others in tensor memory (opo_solo.cuh).
+// Wide engine: one cluster of 4 F CTAs per instance, every field split over four CTAs (opo_wide.cuh).
 struct ResidentArgs {
     void* cur[3];          // [B][N] current fields (read at start, written at end)
     const void* S[3];      // stored inputs (non-resonant fields restart from these)
@@ -161,6 +162,8 @@ struct LargeInfo {
     cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
     cudaError_t solo_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);         \
     cudaError_t launch_solo_##SUFFIX(int log2n, const ResidentArgs& a, int n_ctas, cudaStream_t s); \
+    cudaError_t wide_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);         \
+    cudaError_t launch_wide_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
     cudaError_t large_info_##SUFFIX(int log2n, int n_fields, int batch, int sm_count, LargeInfo* out);       \
     cudaError_t launch_large_##SUFFIX(int log2n, const LargeArgs& a, int grid, cudaStream_t s);
 

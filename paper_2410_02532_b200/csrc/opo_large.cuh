@@ -101,7 +101,7 @@ __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, cons
 #pragma unroll
     for (int x = 0; x < F; ++x) {
 #pragma unroll
-        for (int k = 1; k < R; ++k) v[x][k] = cmulc(v[x][k], w[k - 1]);
+        for (int k = 1; k < R; ++k) v[x][k] = cmulc_unit(v[x][k], w[k - 1]);
         dit_inv<T, R>::run(v[x]);
     }
 #pragma unroll
@@ -148,6 +148,9 @@ template <class T, int L, int F> struct LargeEngine {
         const int p = k1 * n2;
         return cmul(whi[p >> C::L1], wlo[p & (C::N1 - 1)]);
     }
+    // The row pass multiplies by w = big_twiddle on the way in and by conj(w) on the way out; in fp32 the rounded product has
+    // |w|^2 = 1 + d, d ~ 1e-7, the same at every z-step: cmulc_unit takes it out (opo_fft.cuh).
+    __device__ __forceinline__ cplx<T> mul_conj_unit(cplx<T> v, cplx<T> w) const { return cmulc_unit(v, w); }
 
     // ---- column pass over this CTA's tiles ----------------------------------------------------------
     // src/dst: per-field base pointers ([B][N]); fields outside `mask` are neither read nor written.
@@ -203,7 +206,7 @@ template <class T, int L, int F> struct LargeEngine {
             if constexpr (MODE != COL_FWD && MODE != COL_NFWD) {
                 __syncthreads();
                 inv_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
-                inv_passes<T, C::L1, C::TT1, true, ((MODE == COL_INV || MODE == COL_INVN) ? 0 : 1)>(smt, tw1, lt);
+                inv_passes<T, C::L1, C::TT1, true, ((MODE == COL_INV || MODE == COL_INVN) ? 0 : 1), true, true>(smt, tw1, lt);
             }
             if constexpr (MODE == COL_INVN) rk4_tile();
             if constexpr (MODE == COL_RK4) {
@@ -223,7 +226,7 @@ template <class T, int L, int F> struct LargeEngine {
             }
             if constexpr (MODE != COL_INV && MODE != COL_INVN) {
                 __syncthreads();
-                fwd_passes<T, C::L1, C::TT1, true, ((MODE == COL_FWD || MODE == COL_NFWD) ? 0 : 1)>(smt, tw1, lt);
+                fwd_passes<T, C::L1, C::TT1, true, ((MODE == COL_FWD || MODE == COL_NFWD) ? 0 : 1), true>(smt, tw1, lt);
                 fwd_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
             }
             __syncthreads();
@@ -276,19 +279,27 @@ template <class T, int L, int F> struct LargeEngine {
                 continue;
             }
             const int k1 = __ldg(&perm1[active ? r : 0]);
-            if (active) {       // all loads of the row in flight before the first one is consumed
-                constexpr int CNT = C::N2 / C::TT2;
-                cplx<T> r[CNT];
+            // A row is one team's business from its first load to its last store, and a team (N2 / 16 <= 32 threads) never
+            // spans warps: every barrier of the row pass is a __syncwarp, the warps of a CTA drift apart and one row's
+            // loads run under another row's arithmetic.  All loads of the row -- data and multiplier table -- are in flight
+            // before the first one is consumed (the pass is bound by latency, not by bandwidth).
+            constexpr int CNT = C::N2 / C::TT2;
+            constexpr int RM = 1 << P2::rbits(P2::P - 1), NBM = C::N2 / RM, NIT = NBM / C::TT2;
+            static_assert(NBM % C::TT2 == 0, "whole iterations of the middle pass per team");
+            cplx<T> rv[CNT];
+            if (active) {
 #pragma unroll
-                for (int j = 0; j < CNT; ++j) r[j] = ldcg(g + lt + j * C::TT2);
-#pragma unroll
-                for (int j = 0; j < CNT; ++j) smt[phys<T>(lt + j * C::TT2)] = cmul(r[j], big_twiddle(k1, lt + j * C::TT2));
+                for (int j = 0; j < CNT; ++j) rv[j] = ldcg(g + lt + j * C::TT2);
             }
-            __syncthreads();
             if (kind == ROW_FREQ) {
-                fwd_passes<T, C::L2, C::TT2, true, 0>(smt, tw2, lt);
+                if (active) {
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) smt[phys<T>(lt + j * C::TT2)] = cmul(rv[j], big_twiddle(k1, lt + j * C::TT2));
+                }
+                __syncwarp();
+                fwd_passes<T, C::L2, C::TT2, true, 0, true>(smt, tw2, lt);
                 fwd_pass_smem<T, C::L2, P2::P - 1, C::TT2, true>(smt, tw2, lt);
-                __syncthreads();
+                __syncwarp();
                 if (active) {
                     cplx<T>* o = op.out[x] + (size_t)b * C::N + k1;
 #pragma unroll 4
@@ -296,21 +307,36 @@ template <class T, int L, int F> struct LargeEngine {
                 }
             } else {
                 const TAB* tab = op.tab[x] + (size_t)b * op.tab_stride[x] + (size_t)(active ? r : 0) * C::N2;
-                fwd_passes<T, C::L2, C::TT2, true, 0>(smt, tw2, lt);
-                mid_pass_smem<T, C::L2, C::TT2, TAB>(smt, tab, lt);
-                inv_passes<T, C::L2, C::TT2, true, 0>(smt, tw2, lt);
-                __syncthreads();
+                TAB hh[NIT][RM];
+#pragma unroll
+                for (int it = 0; it < NIT; ++it)
+#pragma unroll
+                    for (int k = 0; k < RM; ++k) hh[it][k] = ldg(&tab[k * NBM + lt + it * C::TT2]);
+                cplx<T> w[CNT];
+#pragma unroll
+                for (int j = 0; j < CNT; ++j) w[j] = big_twiddle(k1, lt + j * C::TT2);
+                if (active) {
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) smt[phys<T>(lt + j * C::TT2)] = cmul(rv[j], w[j]);
+                }
+                __syncwarp();
+                fwd_passes<T, C::L2, C::TT2, true, 0, true>(smt, tw2, lt);
+#pragma unroll
+                for (int it = 0; it < NIT; ++it) mid_bf<T, C::L2, TAB>(smt, hh[it], lt + it * C::TT2);
+                inv_passes<T, C::L2, C::TT2, true, 0, true, true>(smt, tw2, lt);
+                __syncwarp();
                 if (active) {
                     cplx<T>* sh = op.sh_store[x] ? op.sh_store[x] + off : nullptr;
-#pragma unroll 4
-                    for (int i = lt; i < C::N2; i += C::TT2) {
-                        const cplx<T> v = cmulc(smt[phys<T>(i)], big_twiddle(k1, i));
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) {
+                        const int i = lt + j * C::TT2;
+                        const cplx<T> v = mul_conj_unit(smt[phys<T>(i)], w[j]);
                         g[i] = v;
                         if (sh) sh[i] = v;
                     }
                 }
             }
-            __syncthreads();
+            __syncwarp();
         }
     }
 };

@@ -1,0 +1,429 @@
+// opo_wide.cuh -- wide engine: ONE OPO instance on a thread-block cluster of 4 F CTAs, every field split over four SMs,
+// the FFT stages that cross the split exchanged over distributed shared memory (BASELINE.json north_star item (a)).
+//
+// Why.  The paper's own workload is a single OPO followed for 10^3 .. 10^4 round trips ("massive and
+// sequential simulations", L252), i.e. BASELINE.json configs[1] and [2]: nothing to batch, and z-steps are strictly
+// sequential.  The cluster engine (opo_resident.cuh) gives such an instance F SMs, and each of them has to issue the
+// whole 2^14-point transform pair of its field: ~16 us per z-step on 3 of 148 SMs.  Here the instance gets 4 F SMs.
+//
+// Decomposition.  The radix-4 pass 0 (decimation in frequency, butterflies over x[t + j N/4], j = 0..3) leaves four
+// independent sub-transforms of S = N/4 points.  CTA rank 4 x + j of the cluster holds sub-block j of field x -- logical
+// indices [j S, (j + 1) S), the same index range before and after pass 0 -- in (padded) shared memory for the whole call.
+//
+//   core  : CTA-local.  Forward passes 1..P-1, table multiply, inverse passes P-1..1 of the sub-block (opo_fft.cuh), one
+//           radix-16 butterfly per thread and pass (N = 2^14: 256 threads).
+//   fused : inverse pass 0 -> RK4 of the coupling terms -> forward pass 0, on registers.  The
+//           butterfly t needs element t of all four sub-blocks of all F fields: 4 F CTAs.  The S butterflies are dealt
+//           to the warps of the cluster in tiles of 32; a thread reads its 4 F values through distributed shared memory
+//           (one of them is local), integrates, and writes them back to their owners.
+//   sync  : no cluster-wide barrier inside the z-step loop.  The pass-1 butterfly t' touches the elements t' + (S/16) k,
+//           so the tiles of class c = (tile mod S/512) depend exactly on the pass-1 butterflies of warp c of every CTA, and
+//           vice versa: warp c of each of the 4 F CTAs forms a ring of its own, synchronised by two mbarriers per CTA
+//           and class (ready[c], done[c]: 4 F remote arrivals each).  The 16 tiles of a class are dealt to the 4 F warps of
+//           its ring (rotated by the class so that every CTA gets the same number of tiles).
+//
+// Everything else (merged tables H, H2, HB = H2 G m across the cavity boundary; stored
+// inputs SH of non-resonant fields re-injected every round trip, L268; mirror / spectral phase / modulator of the
+// call's last round trip) is the cluster engine's logic on sub-blocks.  Not served here (the host keeps those on the
+// cluster engine): the N/2 - L - N/2 ordering, a modulator at an inner crossing, a resonant pump.
+#pragma once
+#include "opo_resident.cuh"
+
+namespace opo {
+
+template <class T, int L, int F> struct wide_layout {
+    using PL = plan<L>;
+    static constexpr int C = 4;                              // CTAs per field = sub-blocks left by the radix-4 pass 0
+    static constexpr int NCTA = C * F;                       // cluster size: 8 (two-wave) or 12 (three-wave: a non-portable size)
+    static constexpr int S = 1 << (L - 2);                   // points of a sub-block = number of pass-0 butterflies
+    static constexpr int NT = S / 16;                        // one radix-16 pass-1 butterfly per thread
+    static constexpr int NW = NT / 32;                       // warps per CTA = classes
+    static constexpr int TPC = 16;                           // tiles (of 32 pass-0 butterflies) per class: S / 32 / NW
+    static constexpr int MAXT = (TPC + NCTA - 1) / NCTA;     // tiles per warp
+    static constexpr bool ok = PL::P == 4 && PL::rbits(0) == 2 && PL::rbits(1) == 4 && NT >= 32;
+    static constexpr size_t field_bytes = (size_t)padded_len<T>(S) * sizeof(cplx<T>);
+    static constexpr size_t tw_bytes = (size_t)PL::tw_local_count * sizeof(cplx<T>);
+    static constexpr size_t mbar_offset = (field_bytes + tw_bytes + 15) / 16 * 16;
+    static constexpr size_t total = mbar_offset + 16 * (size_t)(NW > 0 ? NW : 1);
+};
+
+// distributed shared memory through 32-bit shared::cluster addresses (half the address registers of generic pointers)
+__device__ __forceinline__ uint32_t dsmem_addr(uint32_t local_addr, int rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ cplx<float> dsmem_ld(uint32_t addr, cplx<float>) {
+    cplx<float> v;
+    asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.re), "=f"(v.im) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ cplx<double> dsmem_ld(uint32_t addr, cplx<double>) {
+    cplx<double> v;
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.re), "=d"(v.im) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void dsmem_st(uint32_t addr, cplx<float> v) {
+    asm volatile("st.shared::cluster.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.re), "f"(v.im) : "memory");
+}
+__device__ __forceinline__ void dsmem_st(uint32_t addr, cplx<double> v) {
+    asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.re), "d"(v.im) : "memory");
+}
+
+struct WideFlow {
+    uint32_t mb;         // shared address of ready[0]; done[c] = mb + 8 (NW + c)
+    int ncta;            // CTAs in the cluster
+    int wait_in;         // forward pass 1 waits for done[warp] (a fused phase precedes)
+    int arrive_out;      // inverse pass 1 arrives on ready[warp] of every CTA (a fused phase follows)
+    uint32_t par_done;
+};
+
+// The linear core of one sub-block.  smv is the "virtual" base of the field: logical index i lives at smv[phys(i)], and
+// this CTA holds i in [j S, (j + 1) S) only; the butterfly and table indices are the global ones of plan<L>.
+template <class T, int L, int NT>
+__device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const cplx<T>* __restrict__ tab, int j, int tid, WideFlow fa) {
+    using PL = plan<L>;
+    constexpr int NW = NT / 32, S = 1 << (L - 2);
+    constexpr int RBL = PL::rbits(3), R = 1 << RBL, NBF = (1 << L) >> RBL, NBL = S >> RBL;
+    constexpr int NB2 = S >> PL::rbits(2);
+    constexpr bool chain = PL::rbits(2) == RBL && NBL % NT == 0;     // N = 2^14: passes 2, 3, 2 stay inside a warp's blocks
+    const int warp = tid >> 5, lane = tid & 31;
+    if (fa.wait_in) mbar_wait(fa.mb + 8 * (NW + warp), fa.par_done);
+    fwd_bf<T, L, 1>(smv, twl, j * NT + tid);
+    __syncthreads();
+    if constexpr (chain) {
+#pragma unroll 1
+        for (int ul = tid; ul < NBL; ul += NT) {
+            const int u = j * NBL + ul;
+            cplx<T> h[R];
+#pragma unroll
+            for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
+            fwd_bf<T, L, 2>(smv, twl, u);
+            __syncwarp();
+            mid_bf<T, L>(smv, h, u);
+            __syncwarp();
+            inv_bf<T, L, 2>(smv, twl, u);
+        }
+    } else {
+#pragma unroll 1
+        for (int ul = tid; ul < NB2; ul += NT) fwd_bf<T, L, 2>(smv, twl, j * NB2 + ul);
+        __syncthreads();
+#pragma unroll 1
+        for (int ul = tid; ul < NBL; ul += NT) {
+            const int u = j * NBL + ul;
+            cplx<T> h[R];
+#pragma unroll
+            for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
+            mid_bf<T, L>(smv, h, u);
+        }
+        __syncthreads();
+#pragma unroll 1
+        for (int ul = tid; ul < NB2; ul += NT) inv_bf<T, L, 2>(smv, twl, j * NB2 + ul);
+    }
+    __syncthreads();
+    inv_bf<T, L, 1>(smv, twl, j * NT + tid);
+    if (fa.arrive_out) mbar_arrive_cluster(fa.mb + 8 * warp, lane, fa.ncta);
+}
+
+enum { WIDE_RK4 = 0, WIDE_FWD0 = 1, WIDE_INV0 = 2 };
+
+template <class T, int L, int F, bool DK0 = false>
+__global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentArgs a) {
+    using WL = wide_layout<T, L, F>;
+    using PL = plan<L>;
+    static_assert(WL::ok, "wide engine: N = 4 . 16 . r . r'");
+    constexpr int N = 1 << L, S = WL::S, NT = WL::NT, NW = WL::NW, NCTA = WL::NCTA, R = 4;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);          // my sub-block: local index i at sm[phys(i)]
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
+    const int x = rank / WL::C, j = rank % WL::C;               // my field, my sub-block
+    const int cid = blockIdx.x / NCTA, n_clusters = gridDim.x / NCTA;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+
+    uint32_t fld[F][R];                                          // sub-block k of field f, wherever it lives in the cluster
+#pragma unroll
+    for (int f = 0; f < F; ++f)
+#pragma unroll
+        for (int k = 0; k < R; ++k) fld[f][k] = dsmem_addr((uint32_t)__cvta_generic_to_shared(sm), f * WL::C + k);
+    cplx<T>* const smv = sm - phys<T>(j * S);                    // phys(j S + i) = phys(j S) + phys(i): S is a multiple of the pad period
+
+    const cplx<T>* tw = reinterpret_cast<const cplx<T>*>(a.tw);
+    {   // shared-memory copy of the twiddles of the local passes, addressed as the global table is
+        cplx<T>* d = reinterpret_cast<cplx<T>*>(smem_raw + WL::field_bytes);
+        for (int i = tid; i < PL::tw_local_count; i += NT) d[i] = ldg(&tw[PL::tw_local_begin + i]);
+    }
+    const cplx<T>* twl = reinterpret_cast<const cplx<T>*>(smem_raw + WL::field_bytes) - PL::tw_local_begin;
+    const uint32_t mb = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::mbar_offset);
+    if (tid == 0) {
+        for (int c = 0; c < NW; ++c) {
+            mbar_init(mb + 8 * c, NCTA);              // ready[c]: warp c of every CTA after its inverse pass 1
+            mbar_init(mb + 8 * (NW + c), NCTA);       // done[c] : warp c of every CTA after its tiles
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    cluster.sync();       // every CTA's barriers exist (and its twiddle copy is complete) before anybody arrives on them
+
+    // this thread's pass-0 butterflies -- the same at every z-step -- and their twiddles
+    int nt_own = 0;
+    int p_own[WL::MAXT];
+    cplx<T> w0[WL::MAXT][R - 1];
+    {
+        int m = ((rank - 4 * warp) % NCTA + NCTA) % NCTA;        // tile m of class c goes to CTA (m + 4 c) mod NCTA
+#pragma unroll
+        for (int i = 0; i < WL::MAXT; ++i, m += NCTA) {
+            p_own[i] = 0;
+#pragma unroll
+            for (int k = 0; k < R - 1; ++k) w0[i][k] = cplx<T>{(T)1, (T)0};
+            if (m < WL::TPC) {
+                const int t = (warp + NW * m) * 32 + lane;
+                p_own[i] = phys<T>(t) * (int)sizeof(cplx<T>);       // byte offset inside a sub-block
+#pragma unroll
+                for (int k = 0; k < R - 1; ++k) w0[i][k] = ldg(&tw[k * S + t]);
+                nt_own = i + 1;
+            }
+        }
+    }
+
+    T kap[3] = {(T)a.kappa[0], (T)a.kappa[1], (T)a.kappa[2]};
+    const T h = (T)a.h;
+    const int nz = a.nz;
+    const bool rt_mode = a.mode != 0;
+    const bool resonant = a.resonant[x] != 0;
+    const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
+    const cplx<T>* tabH2 = reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
+    uint32_t fz = 0;          // fused phases executed so far (mbarrier phase parity)
+
+    // pass-0 butterflies of this thread's tiles: MODE = WIDE_RK4: inverse pass 0 -> RK4 -> forward pass 0 (all fields);
+    // WIDE_FWD0 / WIDE_INV0: the pass alone, on the fields of `mask`
+    auto tiles = [&](auto mode_tag, int mask, cplx<T> e0, cplx<T> e1, cplx<T> e2) {
+        constexpr int MODE = decltype(mode_tag)::value;
+        cplx<T> v[WL::MAXT][F][R];
+#pragma unroll
+        for (int i = 0; i < WL::MAXT; ++i) {        // all loads of all tiles in flight before the first is consumed
+            if (i < nt_own) {
+#pragma unroll
+                for (int f = 0; f < F; ++f) {
+                    if (MODE != WIDE_RK4 && !((mask >> f) & 1)) continue;
+#pragma unroll
+                    for (int k = 0; k < R; ++k) v[i][f][k] = dsmem_ld(fld[f][k] + p_own[i], cplx<T>{});
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < WL::MAXT; ++i) {
+            if (i < nt_own) {
+#pragma unroll
+                for (int f = 0; f < F; ++f) {
+                    if (MODE != WIDE_RK4 && !((mask >> f) & 1)) continue;
+                    if constexpr (MODE != WIDE_FWD0) {
+#pragma unroll
+                        for (int k = 1; k < R; ++k) v[i][f][k] = cmulc(v[i][f][k], w0[i][k - 1]);
+                        dit_inv<T, R>::run(v[i][f]);
+                    }
+                }
+                if constexpr (MODE == WIDE_RK4) {
+#pragma unroll
+                    for (int q = 0; q < R; ++q) {
+                        cplx<T> y[F];
+#pragma unroll
+                        for (int f = 0; f < F; ++f) y[f] = v[i][f][q];
+                        Rk4<T, F>::template step<DK0>(y, e0, e1, e2, kap, h);
+#pragma unroll
+                        for (int f = 0; f < F; ++f) v[i][f][q] = y[f];
+                    }
+                }
+#pragma unroll
+                for (int f = 0; f < F; ++f) {
+                    if (MODE != WIDE_RK4 && !((mask >> f) & 1)) continue;
+                    if constexpr (MODE != WIDE_INV0) {
+                        dif<T, R>::run(v[i][f]);
+#pragma unroll
+                        for (int k = 1; k < R; ++k) v[i][f][k] = cmul(v[i][f][k], w0[i][k - 1]);
+                    }
+#pragma unroll
+                    for (int k = 0; k < R; ++k) dsmem_st(fld[f][k] + p_own[i], v[i][f][k]);
+                }
+            }
+        }
+    };
+    using tag_rk4 = std::integral_constant<int, WIDE_RK4>;
+    using tag_fwd0 = std::integral_constant<int, WIDE_FWD0>;
+    using tag_inv0 = std::integral_constant<int, WIDE_INV0>;
+    const cplx<T> one = {(T)1, (T)0};
+    auto cluster_bar = [&]() { cluster_arrive(); cluster_wait(); };
+
+    // a cluster loops over instances b = cid, cid + n_clusters, ...
+#pragma unroll 1
+    for (int b = cid; b < a.batch; b += n_clusters) {
+        const int steps_l = a.steps;
+        const int total = rt_mode ? steps_l * nz : steps_l;     // RK4 steps of this call
+        const size_t off = (size_t)b * N + (size_t)j * S;       // my sub-block inside [B][N]
+        cplx<T>* cur = reinterpret_cast<cplx<T>*>(a.cur[x]) + off;
+        const cplx<T>* ph = reinterpret_cast<const cplx<T>*>(a.phase) + (size_t)b * a.phase_stride;
+        const cplx<T>* tabHB = reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x];
+        cplx<T>* SH = reinterpret_cast<cplx<T>*>(a.SH[x]) + off;
+
+        {
+            const cplx<T>* __restrict__ g = cur;
+#pragma unroll 4
+            for (int i = tid; i < S; i += NT) sm[phys<T>(i)] = g[i];
+        }
+        cluster_bar();                                    // every sub-block of the instance is on chip
+        tiles(tag_fwd0{}, (1 << F) - 1, one, one, one);
+        cluster_bar();
+
+        // q counts linear operators: q = 0 first half-step, q = total last half-step, between them the merged full steps;
+        // in round-trip mode q = m nz + s and s = 0 (m > 0) crosses the cavity boundary
+#pragma unroll 1
+        for (int q = 0; q <= total; ++q) {
+            const int s = rt_mode ? q % nz : a.z0 + q;          // index of the RK4 step that follows
+            const bool crossing = rt_mode && q > 0 && q < total && s == 0;
+            const bool keep = rt_mode && q == 0 && !resonant && steps_l > 1;      // SH <- first half-stepped input
+            cplx<T> e0 = one, e1 = one, e2 = one;
+            if constexpr (!DK0) {
+                if (q < total) { e0 = ldg(ph + 2 * s); e1 = ldg(ph + 2 * s + 1); e2 = ldg(ph + 2 * s + 2); }
+            }
+            if (crossing && !resonant) {
+                // fresh pump / frozen seed, already half-stepped: a thread reloads the elements of its own
+                // pass-1 butterfly, i.e. of its class, as soon as the tiles of that class have let go of them
+                mbar_wait(mb + 8 * (NW + warp), (fz - 1) & 1);
+                const cplx<T>* __restrict__ g = SH;
+#pragma unroll
+                for (int k = 0; k < 16; ++k) sm[phys<T>(tid + NT * k)] = g[tid + NT * k];
+                mbar_arrive_cluster(mb + 8 * warp, lane, NCTA);
+            } else {
+                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
+                WideFlow fa;
+                fa.mb = mb; fa.ncta = NCTA;
+                fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
+                fa.arrive_out = (q < total) && !keep;
+                wide_core<T, L, NT>(smv, twl, tab, j, tid, fa);
+                if (keep) {       // the elements of my own inverse pass-1 butterfly: no barrier needed
+                    cplx<T>* __restrict__ g = SH;
+#pragma unroll
+                    for (int k = 0; k < 16; ++k) g[tid + NT * k] = sm[phys<T>(tid + NT * k)];
+                    mbar_arrive_cluster(mb + 8 * warp, lane, NCTA);
+                }
+            }
+            if (q == total) break;
+            mbar_wait(mb + 8 * warp, fz & 1);                 // ready[warp]: inverse pass 1 of my class is done in every CTA
+            tiles(tag_rk4{}, (1 << F) - 1, e0, e1, e2);
+            mbar_arrive_cluster(mb + 8 * (NW + warp), lane, NCTA);      // done[warp] in every CTA
+            ++fz;
+        }
+        cluster_bar();                                    // every field is ready for its inverse pass 0
+        tiles(tag_inv0{}, (1 << F) - 1, one, one, one);
+        cluster_bar();
+
+        if (!rt_mode) {
+            cplx<T>* __restrict__ g = cur;
+#pragma unroll 4
+            for (int i = tid; i < S; i += NT) g[i] = sm[phys<T>(i)];
+        } else {
+            {   // fields at z = L of the last pass
+                cplx<T>* __restrict__ g = reinterpret_cast<cplx<T>*>(a.exitb[x]) + off;
+#pragma unroll 4
+                for (int i = tid; i < S; i += NT) g[i] = sm[phys<T>(i)];
+            }
+            // mirror, spectral phase and phase modulator of the call's last round trip
+            int maskb = 0;
+#pragma unroll
+            for (int f = 0; f < F; ++f)
+                if (a.resonant[f] && a.boundary_fft[f]) maskb |= 1 << f;
+            if (maskb) {        // uniform over the cluster
+                tiles(tag_fwd0{}, maskb, one, one, one);
+                cluster_bar();
+                if ((maskb >> x) & 1) {
+                    const cplx<T>* tabGM = reinterpret_cast<const cplx<T>*>(a.tabGM[x]) + (size_t)b * a.tab_stride[x];
+                    WideFlow fa{};
+                    wide_core<T, L, NT>(smv, twl, tabGM, j, tid, fa);
+                }
+                cluster_bar();
+                tiles(tag_inv0{}, maskb, one, one, one);
+                cluster_bar();
+            }
+            if (resonant) {
+                const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]);
+                cplx<T> mf = one;
+                if (!a.boundary_fft[x]) mf = ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b);
+                if (E != nullptr) {
+#pragma unroll 4
+                    for (int i = tid; i < S; i += NT) cur[i] = cmul(cmul(sm[phys<T>(i)], mf), ldg(&E[j * S + i]));
+                } else {
+#pragma unroll 4
+                    for (int i = tid; i < S; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
+                }
+            } else {
+                const cplx<T>* __restrict__ Sx = reinterpret_cast<const cplx<T>*>(a.S[x]) + off;
+#pragma unroll 4
+                for (int i = tid; i < S; i += NT) cur[i] = Sx[i];
+            }
+        }
+        // the next instance's load overwrites shared memory that only this CTA reads from here on: all foreign
+        // accesses of this instance ended at the last cluster barrier
+        __syncthreads();
+    }
+    cluster.sync();     // keep shared memory alive until every peer has left its last tile phase
+}
+
+template <class T, int L, int F, bool DK0> cudaError_t wide_cfg(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, int n_clusters, cudaStream_t s) {
+    using WL = wide_layout<T, L, F>;
+    static device_once once;
+    cudaError_t e0 = once.run([&] {
+        cudaError_t e = cudaFuncSetAttribute(k_wide<T, L, F, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WL::total);
+        if (e != cudaSuccess) return e;
+        if (WL::NCTA > 8) e = cudaFuncSetAttribute(k_wide<T, L, F, DK0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        return e;
+    });
+    if (e0 != cudaSuccess) return e0;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = WL::NCTA;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg->gridDim = dim3((unsigned)(n_clusters * WL::NCTA), 1, 1);
+    cfg->blockDim = dim3(WL::NT, 1, 1);
+    cfg->dynamicSmemBytes = WL::total;
+    cfg->stream = s;
+    cfg->attrs = attr;
+    cfg->numAttrs = 1;
+    return cudaSuccess;
+}
+
+template <class T, int L, int F> cudaError_t wide_info_LF(ResidentInfo* out) {
+    if constexpr (!wide_layout<T, L, F>::ok) {
+        return cudaErrorNotSupported;
+    } else {
+        cudaLaunchConfig_t cfg{};
+        cudaLaunchAttribute attr[1];
+        cudaError_t e = wide_cfg<T, L, F, false>(&cfg, attr, 1, nullptr);
+        if (e != cudaSuccess) return e;
+        int n = 0;
+        e = cudaOccupancyMaxActiveClusters(&n, k_wide<T, L, F, false>, &cfg);
+        if (e != cudaSuccess) return e;
+        out->threads = wide_layout<T, L, F>::NT;
+        out->smem_bytes = cfg.dynamicSmemBytes;
+        out->max_clusters = n;
+        return cudaSuccess;
+    }
+}
+template <class T, int L> cudaError_t wide_info_L(int n_fields, ResidentInfo* out) {
+    return n_fields == 3 ? wide_info_LF<T, L, 3>(out) : wide_info_LF<T, L, 2>(out);
+}
+
+template <class T, int L, int F, bool DK0> cudaError_t launch_wide_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    if constexpr (!wide_layout<T, L, F>::ok) {
+        return cudaErrorNotSupported;
+    } else {
+        cudaLaunchConfig_t cfg{};
+        cudaLaunchAttribute attr[1];
+        cudaError_t e = wide_cfg<T, L, F, DK0>(&cfg, attr, n_clusters, s);
+        if (e != cudaSuccess) return e;
+        return cudaLaunchKernelEx(&cfg, k_wide<T, L, F, DK0>, a);
+    }
+}
+template <class T, int L, bool DK0> cudaError_t launch_wide_L(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    return a.n_fields == 3 ? launch_wide_LF<T, L, 3, DK0>(a, n_clusters, s) : launch_wide_LF<T, L, 2, DK0>(a, n_clusters, s);
+}
+
+}  // namespace opo

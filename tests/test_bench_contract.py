@@ -36,10 +36,10 @@ def test_our_arm_line():
     for k in COMMON + ("clocks", "roofline", "round_trips_per_s"):
         assert k in d, k
     assert d["value"] > 1e9 and d["n_gpus"] == 1 and d["dtype"] == "f32" and d["scaling"] == "weak" and d["data"] == "synthetic"
-    assert d["config"]["engine"] == "resident" and "C4" in d["config"]["workload"]
+    assert d["config"]["engine"] == "solo" and "C4" in d["config"]["workload"]      # what AUTO picks for a batch >= SM count
     r = d["roofline"]
     assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9 and 0.05 < r["frac"] < 1.0
-    assert d["gpu_launches"] == d["steps"]                      # one launch of the resident kernel per step
+    assert d["gpu_launches"] == d["steps"]                      # one launch of the on-chip kernel per step
     assert d["e2e"]["h2d_bytes_per_step"] == 256 * 16384 * 8 * 3 and d["e2e"]["d2h_bytes_per_step"] == 256 * 16384 * 8
     assert d["e2e"]["value"] > 0 and d["e2e"]["value"] != d["value"]
     assert d["clocks"]["sm_mhz"] is None or d["clocks"]["sm_mhz"] > 0

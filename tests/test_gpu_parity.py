@@ -96,17 +96,18 @@ def run_oracle(w, n_roundtrips=None, propagate=None):
 
 
 def engines():
-    """streaming (unfused internal baseline), resident (cluster per instance), solo (one CTA per instance, TMEM)"""
+    """streaming (unfused internal baseline), resident (cluster per instance), solo (one CTA per instance, TMEM),
+    wide (a cluster of 4 F CTAs per instance, fields split over four SMs; N = 2^12 .. 2^14 only)"""
     import paper_2410_02532_b200 as P
-    return [P.ENGINE_STREAMING, P.ENGINE_RESIDENT, P.ENGINE_SOLO]
+    return [P.ENGINE_STREAMING, P.ENGINE_RESIDENT, P.ENGINE_SOLO, P.ENGINE_WIDE]
 
 
-ENGINE_IDX = [0, 1, 2]
+ENGINE_IDX = [0, 1, 2, 3]
 
 
 def _engine_or_skip(w, engine):
     torch, P = _gpu()
-    if engine in (P.ENGINE_RESIDENT, P.ENGINE_SOLO):
+    if engine in (P.ENGINE_RESIDENT, P.ENGINE_SOLO, P.ENGINE_WIDE):
         o = P.from_workload(w, engine=P.ENGINE_AUTO)
         try:
             o.set_engine(engine)
@@ -282,6 +283,52 @@ def test_crystal_segments_match_oracle(precision, log2_n, n_fields, splitting):
     with pytest.raises(P.OpoError) as e:
         o.propagate(8)                      # 2 + 8 > 9 steps per pass
     assert e.value.status == P.ERR_STATE
+    o.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# wide engine (a cluster of 4 F CTAs per instance): every size it serves, full boundary operator with per-instance
+# sweeps, non-resonant restart, several calls, more instances than co-resident clusters
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision,log2_n,n_fields,calls,batch", [
+    ("c64", 12, 3, 1, 3), ("c64", 12, 2, 2, 3), ("c64", 13, 2, 1, 3), ("c64", 13, 3, 3, 2), ("c64", 14, 3, 1, 3), ("c64", 14, 2, 2, 2),
+    ("c128", 12, 2, 1, 3), ("c128", 12, 3, 3, 2), ("c128", 13, 3, 1, 2), ("c128", 13, 2, 2, 3), ("c64", 12, 3, 1, 37)])
+def test_wide_engine_roundtrips_with_boundary(precision, log2_n, n_fields, calls, batch):
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=4, batch=batch, dk=-20.0, gdd_dt2=-1.7, drad=0.4, strong=False)
+    w.delta_T_signal_s = (np.arange(batch) % 5 - 2.0) * 1.25 * w.dt
+    if n_fields == 3:
+        w.resonant = [0, 1, 0]      # the idler restarts from its seed every round trip (R12)
+    _engine_or_skip(w, P.ENGINE_WIDE)
+    cur, ex, eng = run_gpu(w, P.ENGINE_WIDE, n_roundtrips=3, calls=calls)
+    assert eng == P.ENGINE_WIDE
+    rcur, rex = run_oracle(w, n_roundtrips=3)
+    tol = TOL[precision] if precision == "c128" else 3e-5
+    assert_close(cur, rcur, tol, "current")
+    assert_close(ex, rex, tol, "exit")
+    # the same workload on the cluster engine: both follow the same factorisation, so they agree to rounding
+    cur2, ex2, eng2 = run_gpu(w, P.ENGINE_RESIDENT, n_roundtrips=3, calls=calls)
+    assert eng2 == P.ENGINE_RESIDENT
+    assert_close(ex, ex2, 1e-12 if precision == "c128" else 1e-5, "wide vs cluster engine")
+
+
+def test_wide_engine_is_what_auto_picks_for_a_single_instance_and_falls_back():
+    torch, P = _gpu()
+    w = W.config1().truncated(1)
+    o = P.from_workload(w)
+    assert o.engine == P.ENGINE_WIDE and int(P.opo_get_info(o._h, P.INFO_SLOTS)) == 1
+    o.close()
+    w4 = W.config4().truncated(1)
+    o = P.from_workload(w4)
+    assert o.engine == P.ENGINE_SOLO        # a batch that fills the GPU stays on the solo engine
+    o.set_engine(P.ENGINE_WIDE)
+    assert o.engine == P.ENGINE_WIDE        # ... unless the caller insists
+    o.close()
+    ws = small_workload(9, 3, "c64")
+    o = P.from_workload(ws)
+    with pytest.raises(P.OpoError):
+        o.set_engine(P.ENGINE_WIDE)         # N = 2^9: not a size of the wide engine
+    assert o.engine != P.ENGINE_WIDE
     o.close()
 
 
