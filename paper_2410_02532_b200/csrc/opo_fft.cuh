@@ -94,6 +94,7 @@ __device__ __forceinline__ cplx<float> cmulc_unit(cplx<float> a, cplx<float> b, 
     const float sr = -d * re0, si = -d * im0;
     return {__fmaf_rn(a.re, b.re, __fmaf_rn(a.im, b.im, sr)), __fmaf_rn(a.im, b.re, __fmaf_rn(-a.re, b.im, si))};
 }
+__device__ __forceinline__ cplx<double> cmulc_unit(cplx<double> a, cplx<double> b, float) { return cmulc(a, b); }
 template <class T> __device__ __forceinline__ cplx<T> cmulc_unit(cplx<T> a, cplx<T> b) {
     if constexpr (sizeof(T) == 4) return cmulc_unit(a, b, unit_defect(b));
     else return cmulc(a, b);
@@ -340,9 +341,10 @@ __device__ __forceinline__ void fwd_pass_smem(cplx<T>* __restrict__ sm, const cp
 }
 
 // ---- one inverse (DIT) pass over shared memory ---------------------------------------------------------
-// UF: the twiddle multiply takes the twiddle's magnitude defect out (cmulc_unit)
+// UF: the twiddle multiply takes the twiddle's magnitude defect out (cmulc_unit); dtw (fp32): the defects |w|^2 - 1,
+// tabulated with the index of the twiddle table (null: evaluated on the fly)
 template <class T, int L, int PASS, int NT, bool TWS, bool UF = false>
-__device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid) {
+__device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid, const float* __restrict__ dtw = nullptr) {
     using PL = plan<L>;
     constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
     constexpr int NBF = (1 << L) / R;
@@ -357,8 +359,12 @@ __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cp
         if constexpr (SB > 0) {
 #pragma unroll
             for (int k = 1; k < R; ++k) {
-                if constexpr (UF) v[k] = cmulc_unit(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
-                else v[k] = cmulc(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
+                if constexpr (UF && sizeof(T) == 4) {
+                    const cplx<T> wk = ldtw<TWS>(&w[((k - 1) << SB) + t]);
+                    v[k] = cmulc_unit(v[k], wk, dtw != nullptr ? dtw[PL::tw_offset(PASS) + ((k - 1) << SB) + t] : unit_defect(wk));
+                } else {
+                    v[k] = cmulc(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
+                }
             }
         }
         dit_inv<T, R>::run(v);
@@ -420,27 +426,29 @@ __device__ __forceinline__ void mid_pass_smem(cplx<T>* __restrict__ sm, const TA
     }
 }
 
-// barrier between two shared-memory passes: the whole CTA, or (WS) the warp when a transform's team never spans warps
-template <bool WS> __device__ __forceinline__ void pass_sync() {
-    if constexpr (WS) __syncwarp();
-    else __syncthreads();
+// barrier between two shared-memory passes of a transform run by a team of threads.  SY = 0: the team is the CTA; 1..32: the
+// team never spans warps, a __syncwarp will do; > 32: a named barrier of SY threads, id `bar` (1..15)
+template <int SY> __device__ __forceinline__ void pass_sync(int bar = 0) {
+    if constexpr (SY == 0) __syncthreads();
+    else if constexpr (SY <= 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(SY) : "memory");
 }
 // forward passes FIRST .. P-2 (everything before the fused middle), with the barriers between them
-template <class T, int L, int NT, bool TWS, int PASS, bool WS = false>
-__device__ __forceinline__ void fwd_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
+template <class T, int L, int NT, bool TWS, int PASS, int SY = 0>
+__device__ __forceinline__ void fwd_passes(cplx<T>* sm, const cplx<T>* tw, int tid, int bar = 0) {
     if constexpr (PASS < plan<L>::P - 1) {
         fwd_pass_smem<T, L, PASS, NT, TWS>(sm, tw, tid);
-        pass_sync<WS>();
-        fwd_passes<T, L, NT, TWS, PASS + 1, WS>(sm, tw, tid);
+        pass_sync<SY>(bar);
+        fwd_passes<T, L, NT, TWS, PASS + 1, SY>(sm, tw, tid, bar);
     }
 }
 // inverse passes P-2 .. LAST
-template <class T, int L, int NT, bool TWS, int LAST, bool WS = false, bool UF = false, int PASS = plan<L>::P - 2>
-__device__ __forceinline__ void inv_passes(cplx<T>* sm, const cplx<T>* tw, int tid) {
+template <class T, int L, int NT, bool TWS, int LAST, int SY = 0, bool UF = false, int PASS = plan<L>::P - 2>
+__device__ __forceinline__ void inv_passes(cplx<T>* sm, const cplx<T>* tw, int tid, int bar = 0, const float* dtw = nullptr) {
     if constexpr (PASS >= LAST) {
-        pass_sync<WS>();
-        inv_pass_smem<T, L, PASS, NT, TWS, UF>(sm, tw, tid);
-        inv_passes<T, L, NT, TWS, LAST, WS, UF, PASS - 1>(sm, tw, tid);
+        pass_sync<SY>(bar);
+        inv_pass_smem<T, L, PASS, NT, TWS, UF>(sm, tw, tid, dtw);
+        inv_passes<T, L, NT, TWS, LAST, SY, UF, PASS - 1>(sm, tw, tid, bar, dtw);
     }
 }
 

@@ -40,7 +40,17 @@ template <class T, int L, int F> struct large_cfg {
     static constexpr int L1 = L / 2, L2 = L - L1;
     static constexpr int N1 = 1 << L1, N2 = 1 << L2, N = 1 << L;
     static constexpr int TC = OPO_LARGE_TC;            // columns per tile
-    static constexpr int TT1 = N1 / 16, TT2 = N2 / 16; // threads per column / row transform
+    // Points per thread of a transform.  8 points per thread (twice the warps, teams of two warps with named barriers) was
+    // measured SLOWER on C3 (17.0 vs 14.8 us per z-step): the compute phases are ~54 % issue-bound already, the radix-16
+    // pass then runs on half a team and every thread repeats the index arithmetic.
+#ifdef OPO_LARGE_PT
+    static constexpr int PT = OPO_LARGE_PT;
+#else
+    static constexpr int PT = 16;
+#endif
+    static constexpr int TT1 = N1 / PT, TT2 = N2 / PT; // threads per column / row transform (a "team")
+    // barrier of a team between passes: teams of <= 32 threads never span warps (pass_sync in opo_fft.cuh)
+    static constexpr int SY1 = TT1 <= 32 ? 1 : TT1, SY2 = TT2 <= 32 ? 1 : TT2;
     static constexpr int NT = F * TC * TT1;            // one team per (field, column)
     static constexpr int ROWS = NT / TT2;              // rows per chunk in the row pass
     static constexpr int SKEW = (128 / (int)sizeof(cplx<T>)) / TC;   // makes the transposing tile load conflict-free
@@ -49,10 +59,21 @@ template <class T, int L, int F> struct large_cfg {
     static constexpr int FIELD_ELEMS = (F * TC * CSTRIDE > ROWS * RSTRIDE) ? F * TC * CSTRIDE : ROWS * RSTRIDE;
     static constexpr int TW1 = plan<L1>::tw_total, TW2 = plan<L2>::tw_total;
     static constexpr int SMEM_ELEMS = FIELD_ELEMS + TW1 + TW2 + N1 + N2;
-    static constexpr size_t SMEM_BYTES = (size_t)SMEM_ELEMS * sizeof(cplx<T>);
+    static constexpr size_t BASE_BYTES = (size_t)SMEM_ELEMS * sizeof(cplx<T>);
+    // Per-CTA caches of what a row team needs at EVERY z-step when the CTA keeps the same rows for the whole launch (one
+    // chunk per CTA: C3): the rows' slice of the merged full-step table H2 (fp32: hi + lo, 16 B per entry -- 8 MB per
+    // z-step out of L2 otherwise, which is what the row pass was waiting for), and (fp32) the rows' four-step twiddles
+    // W_N^{n2 k1} with their magnitude defects; plus (fp32) the defects of the pass twiddles.
+    static constexpr size_t TABC_BYTES = (size_t)ROWS * N2 * sizeof(typename large_tab<T>::type);
+    static constexpr size_t WC_BYTES = sizeof(T) == 4 ? (size_t)ROWS * N2 * (sizeof(cplx<T>) + sizeof(float)) : 0;
+    static constexpr size_t DTW_BYTES = sizeof(T) == 4 ? (size_t)(TW1 + TW2) * sizeof(float) : 0;
+    static constexpr size_t CACHE_OFFSET = (BASE_BYTES + 15) / 16 * 16;
+    static constexpr bool CACHE = CACHE_OFFSET + TABC_BYTES + WC_BYTES + DTW_BYTES <= 232448;
+    static constexpr size_t SMEM_BYTES = CACHE ? CACHE_OFFSET + TABC_BYTES + WC_BYTES + DTW_BYTES : CACHE_OFFSET + DTW_BYTES;
     static constexpr int TILES_PER_INST = N2 / TC;
     static constexpr int CHUNKS_PER_FIELD = (N1 + ROWS - 1) / ROWS;
     static_assert(ROWS >= 1, "a CTA must hold at least one row");
+    static_assert((TT1 <= 32 || F * TC <= 15) && (TT2 <= 32 || ROWS <= 15), "one named barrier per team");
 };
 
 // coherent (L2) load of field data written by other SMs earlier in the same launch
@@ -87,11 +108,17 @@ __device__ __forceinline__ void grid_barrier(unsigned long long* ctr, unsigned l
 template <class T, int L, int F>
 __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, const cplx<T>* __restrict__ tw0s,
                                                 cplx<T> e0, cplx<T> e1, cplx<T> e2, const T* kap, T h,
-                                                bool two = false, cplx<T> e3 = cplx<T>{}, cplx<T> e4 = cplx<T>{}) {
+                                                bool two = false, cplx<T> e3 = cplx<T>{}, cplx<T> e4 = cplx<T>{},
+                                                const float* __restrict__ dtw0 = nullptr) {
     constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
     cplx<T> w[R - 1];
+    float wd[R - 1];        // magnitude defects of the twiddles (fp32, cmulc_unit)
 #pragma unroll
-    for (int k = 0; k < R - 1; ++k) w[k] = tw0s[k * S + t];
+    for (int k = 0; k < R - 1; ++k) {
+        w[k] = tw0s[k * S + t];
+        if constexpr (sizeof(T) == 4) wd[k] = dtw0 != nullptr ? dtw0[k * S + t] : unit_defect(w[k]);
+        else wd[k] = 0.0f;
+    }
     const int p0 = elem_base<T, RB, SB>(0, t);
     cplx<T> v[F][R];
 #pragma unroll
@@ -101,7 +128,7 @@ __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, cons
 #pragma unroll
     for (int x = 0; x < F; ++x) {
 #pragma unroll
-        for (int k = 1; k < R; ++k) v[x][k] = cmulc_unit(v[x][k], w[k - 1]);
+        for (int k = 1; k < R; ++k) v[x][k] = cmulc_unit(v[x][k], w[k - 1], wd[k - 1]);
         dit_inv<T, R>::run(v[x]);
     }
 #pragma unroll
@@ -143,14 +170,20 @@ template <class T, int L, int F> struct LargeEngine {
     const cplx<T>* wlo;     // W_N^j, j < N1
     const cplx<T>* whi;     // W_N^{j N1}, j < N2
     int tid;
+    const float* dtw1 = nullptr;    // |w|^2 - 1 of the pass twiddles (fp32; opo_fft.cuh), indexed as tw1 / tw2
+    const float* dtw2 = nullptr;
+    // row caches (large_cfg::CACHE): valid for rows of `cache_tab` handled by this CTA's teams
+    const void* cache_src = nullptr;        // the global table the cached slice was copied from (null: no cache)
+    const TAB* cache_tab = nullptr;         // [ROWS][N2] in mid-pass layout
+    const cplx<T>* cache_w = nullptr;       // [ROWS][N2] four-step twiddles of the rows
+    const float* cache_wd = nullptr;        // [ROWS][N2] their defects
 
     __device__ __forceinline__ cplx<T> big_twiddle(int k1, int n2) const {
         const int p = k1 * n2;
         return cmul(whi[p >> C::L1], wlo[p & (C::N1 - 1)]);
     }
-    // The row pass multiplies by w = big_twiddle on the way in and by conj(w) on the way out; in fp32 the rounded product has
-    // |w|^2 = 1 + d, d ~ 1e-7, the same at every z-step: cmulc_unit takes it out (opo_fft.cuh).
-    __device__ __forceinline__ cplx<T> mul_conj_unit(cplx<T> v, cplx<T> w) const { return cmulc_unit(v, w); }
+    // (the row pass multiplies by w = big_twiddle on the way in and by conj(w) on the way out; in fp32 the rounded product has
+    // |w|^2 = 1 + d, d ~ 1e-7, the same at every z-step: cmulc_unit takes it out, opo_fft.cuh)
 
     // ---- column pass over this CTA's tiles ----------------------------------------------------------
     // src/dst: per-field base pointers ([B][N]); fields outside `mask` are neither read nor written.
@@ -206,7 +239,7 @@ template <class T, int L, int F> struct LargeEngine {
             if constexpr (MODE != COL_FWD && MODE != COL_NFWD) {
                 __syncthreads();
                 inv_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
-                inv_passes<T, C::L1, C::TT1, true, ((MODE == COL_INV || MODE == COL_INVN) ? 0 : 1), true, true>(smt, tw1, lt);
+                inv_passes<T, C::L1, C::TT1, true, ((MODE == COL_INV || MODE == COL_INVN) ? 0 : 1), C::SY1, true>(smt, tw1, lt, 1 + team, dtw1);
             }
             if constexpr (MODE == COL_INVN) rk4_tile();
             if constexpr (MODE == COL_RK4) {
@@ -221,12 +254,13 @@ template <class T, int L, int F> struct LargeEngine {
                     cplx<T>* fld[F];
 #pragma unroll
                     for (int x = 0; x < F; ++x) fld[x] = sm + (x * C::TC + c) * C::CSTRIDE;
-                    pass0_rk4_local<T, C::L1, F>(fld, t, tw1 + P1::tw_offset(0), e0, e1, e2, kap, h, two, e3, e4);
+                    pass0_rk4_local<T, C::L1, F>(fld, t, tw1 + P1::tw_offset(0), e0, e1, e2, kap, h, two, e3, e4,
+                                                 dtw1 != nullptr ? dtw1 + P1::tw_offset(0) : nullptr);
                 }
             }
             if constexpr (MODE != COL_INV && MODE != COL_INVN) {
                 __syncthreads();
-                fwd_passes<T, C::L1, C::TT1, true, ((MODE == COL_FWD || MODE == COL_NFWD) ? 0 : 1), true>(smt, tw1, lt);
+                fwd_passes<T, C::L1, C::TT1, true, ((MODE == COL_FWD || MODE == COL_NFWD) ? 0 : 1), C::SY1>(smt, tw1, lt, 1 + team);
                 fwd_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
             }
             __syncthreads();
@@ -254,11 +288,18 @@ template <class T, int L, int F> struct LargeEngine {
         cplx<T>* out[3];          // ROW_FREQ: natural-order destination
     };
 
+    // The row pass begins with the grid barrier that separates it from the column pass before it: everything that does not
+    // depend on the fields (multiplier table entries from L2, the row's twiddles) is requested BEFORE that barrier, so its
+    // latency is spent while the CTA waits for the slowest column tile anyway.
     __device__ __forceinline__ void row_pass(cplx<T>* const* data, const RowOp& op, int batch, const int* __restrict__ perm1,
-                                             const int* __restrict__ perm2) {
+                                             const int* __restrict__ perm2, unsigned long long* bar_ctr, unsigned long long& bar_target) {
         const int n_chunks = batch * F * C::CHUNKS_PER_FIELD;
         const int team = tid / C::TT2, lt = tid % C::TT2;
         cplx<T>* smt = sm + team * C::RSTRIDE;
+        bool synced = false;        // uniform over the CTA
+        auto sync_once = [&]() {
+            if (!synced) { grid_barrier(bar_ctr, bar_target); synced = true; }
+        };
 #pragma unroll 1
         for (int chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
             const int b = chunk / (F * C::CHUNKS_PER_FIELD);
@@ -271,6 +312,7 @@ template <class T, int L, int F> struct LargeEngine {
             const size_t off = (size_t)b * C::N + (size_t)(active ? r : 0) * C::N2;
             cplx<T>* g = data[x] + off;
             if (kind == ROW_RELOAD) {
+                sync_once();
                 if (active) {
                     const cplx<T>* __restrict__ a = op.aux[x] + off;
 #pragma unroll 4
@@ -278,28 +320,31 @@ template <class T, int L, int F> struct LargeEngine {
                 }
                 continue;
             }
-            const int k1 = __ldg(&perm1[active ? r : 0]);
-            // A row is one team's business from its first load to its last store, and a team (N2 / 16 <= 32 threads) never
-            // spans warps: every barrier of the row pass is a __syncwarp, the warps of a CTA drift apart and one row's
-            // loads run under another row's arithmetic.  All loads of the row -- data and multiplier table -- are in flight
+            // this CTA's rows of this table are in shared memory (merged full step H2: every z-step but the ends of a pass)
+            const bool cached = kind == ROW_LINEAR && cache_src != nullptr && cache_src == (const void*)op.tab[x] && op.tab_stride[x] == 0;
+            const int k1 = (cached && sizeof(T) == 4) ? 0 : __ldg(&perm1[active ? r : 0]);      // (the cached twiddles need no k1)
+            // A row is one team's business from its first load to its last store: every barrier of the row pass is the
+            // team's own (a __syncwarp, or a named barrier when the team has two warps), the teams of a CTA drift apart and
+            // one row's loads run under another row's arithmetic.  All loads of the row -- data and multiplier table -- are in flight
             // before the first one is consumed (the pass is bound by latency, not by bandwidth).
             constexpr int CNT = C::N2 / C::TT2;
             constexpr int RM = 1 << P2::rbits(P2::P - 1), NBM = C::N2 / RM, NIT = NBM / C::TT2;
             static_assert(NBM % C::TT2 == 0, "whole iterations of the middle pass per team");
             cplx<T> rv[CNT];
-            if (active) {
-#pragma unroll
-                for (int j = 0; j < CNT; ++j) rv[j] = ldcg(g + lt + j * C::TT2);
-            }
             if (kind == ROW_FREQ) {
+                sync_once();
+                if (active) {
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) rv[j] = ldcg(g + lt + j * C::TT2);
+                }
                 if (active) {
 #pragma unroll
                     for (int j = 0; j < CNT; ++j) smt[phys<T>(lt + j * C::TT2)] = cmul(rv[j], big_twiddle(k1, lt + j * C::TT2));
                 }
-                __syncwarp();
-                fwd_passes<T, C::L2, C::TT2, true, 0, true>(smt, tw2, lt);
+                pass_sync<C::SY2>(1 + team);
+                fwd_passes<T, C::L2, C::TT2, true, 0, C::SY2>(smt, tw2, lt, 1 + team);
                 fwd_pass_smem<T, C::L2, P2::P - 1, C::TT2, true>(smt, tw2, lt);
-                __syncwarp();
+                pass_sync<C::SY2>(1 + team);
                 if (active) {
                     cplx<T>* o = op.out[x] + (size_t)b * C::N + k1;
 #pragma unroll 4
@@ -308,36 +353,68 @@ template <class T, int L, int F> struct LargeEngine {
             } else {
                 const TAB* tab = op.tab[x] + (size_t)b * op.tab_stride[x] + (size_t)(active ? r : 0) * C::N2;
                 TAB hh[NIT][RM];
-#pragma unroll
-                for (int it = 0; it < NIT; ++it)
-#pragma unroll
-                    for (int k = 0; k < RM; ++k) hh[it][k] = ldg(&tab[k * NBM + lt + it * C::TT2]);
                 cplx<T> w[CNT];
+                float wd[CNT];
+                if (!cached) {
 #pragma unroll
-                for (int j = 0; j < CNT; ++j) w[j] = big_twiddle(k1, lt + j * C::TT2);
+                    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+                        for (int k = 0; k < RM; ++k) hh[it][k] = ldg(&tab[k * NBM + lt + it * C::TT2]);
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) {
+                        w[j] = big_twiddle(k1, lt + j * C::TT2);
+                        if constexpr (sizeof(T) == 4) wd[j] = unit_defect(w[j]);
+                        else wd[j] = 0.0f;
+                    }
+                }
+                sync_once();
+                if (active) {
+#pragma unroll
+                    for (int j = 0; j < CNT; ++j) rv[j] = ldcg(g + lt + j * C::TT2);
+                }
+                if (cached) {
+                    if constexpr (sizeof(T) == 4) {
+#pragma unroll
+                        for (int j = 0; j < CNT; ++j) {
+                            w[j] = cache_w[team * C::N2 + lt + j * C::TT2];
+                            wd[j] = cache_wd[team * C::N2 + lt + j * C::TT2];
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < CNT; ++j) { w[j] = big_twiddle(k1, lt + j * C::TT2); wd[j] = 0.0f; }
+                    }
+                }
                 if (active) {
 #pragma unroll
                     for (int j = 0; j < CNT; ++j) smt[phys<T>(lt + j * C::TT2)] = cmul(rv[j], w[j]);
                 }
-                __syncwarp();
-                fwd_passes<T, C::L2, C::TT2, true, 0, true>(smt, tw2, lt);
+                pass_sync<C::SY2>(1 + team);
+                fwd_passes<T, C::L2, C::TT2, true, 0, C::SY2>(smt, tw2, lt, 1 + team);
+                if (cached) {
+                    const TAB* ct = cache_tab + team * C::N2;
+#pragma unroll
+                    for (int it = 0; it < NIT; ++it)
+#pragma unroll
+                        for (int k = 0; k < RM; ++k) hh[it][k] = ct[k * NBM + lt + it * C::TT2];
+                }
 #pragma unroll
                 for (int it = 0; it < NIT; ++it) mid_bf<T, C::L2, TAB>(smt, hh[it], lt + it * C::TT2);
-                inv_passes<T, C::L2, C::TT2, true, 0, true, true>(smt, tw2, lt);
-                __syncwarp();
+                inv_passes<T, C::L2, C::TT2, true, 0, C::SY2, true>(smt, tw2, lt, 1 + team, dtw2);
+                pass_sync<C::SY2>(1 + team);
                 if (active) {
                     cplx<T>* sh = op.sh_store[x] ? op.sh_store[x] + off : nullptr;
 #pragma unroll
                     for (int j = 0; j < CNT; ++j) {
                         const int i = lt + j * C::TT2;
-                        const cplx<T> v = mul_conj_unit(smt[phys<T>(i)], w[j]);
+                        const cplx<T> v = cmulc_unit(smt[phys<T>(i)], w[j], wd[j]);
                         g[i] = v;
                         if (sh) sh[i] = v;
                     }
                 }
             }
-            __syncwarp();
+            pass_sync<C::SY2>(1 + team);
         }
+        sync_once();        // a CTA without a row of its own still takes part in the barrier
     }
 };
 
@@ -368,6 +445,46 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
         e.whi = copy(a.whi, C::N2);
     }
     __syncthreads();
+    if constexpr (sizeof(T) == 4) {     // magnitude defects of the pass twiddles
+        float* d = reinterpret_cast<float*>(smem_raw + C::CACHE_OFFSET + (C::CACHE ? C::TABC_BYTES + C::WC_BYTES : 0));
+        for (int i = tid; i < C::TW1; i += C::NT) d[i] = unit_defect(e.tw1[i]);
+        for (int i = tid; i < C::TW2; i += C::NT) d[C::TW1 + i] = unit_defect(e.tw2[i]);
+        e.dtw1 = d;
+        e.dtw2 = d + C::TW1;
+    }
+    if constexpr (C::CACHE) {
+        // one chunk of rows per CTA for the whole launch: keep the rows' slice of H2 and their four-step twiddles on chip
+        const int n_chunks = a.batch * F * C::CHUNKS_PER_FIELD;
+        if (a.mode != 2 && n_chunks <= (int)gridDim.x && (int)blockIdx.x < n_chunks) {
+            const int rem = blockIdx.x % (F * C::CHUNKS_PER_FIELD);
+            const int x = rem / C::CHUNKS_PER_FIELD, r0 = (rem % C::CHUNKS_PER_FIELD) * C::ROWS;
+            if ((a.field_mask >> x) & 1) {
+                const TAB* src = reinterpret_cast<const TAB*>(a.tabH2[x]);
+                TAB* ct = reinterpret_cast<TAB*>(smem_raw + C::CACHE_OFFSET);
+                for (int i = tid; i < C::ROWS * C::N2; i += C::NT) {
+                    const int rr = r0 + i / C::N2;
+                    if (rr < C::N1) ct[i] = ldg(&src[(size_t)rr * C::N2 + i % C::N2]);
+                }
+                e.cache_src = src;
+                e.cache_tab = ct;
+                if constexpr (sizeof(T) == 4) {
+                    cplx<T>* cw = reinterpret_cast<cplx<T>*>(smem_raw + C::CACHE_OFFSET + C::TABC_BYTES);
+                    float* cd = reinterpret_cast<float*>(smem_raw + C::CACHE_OFFSET + C::TABC_BYTES + (size_t)C::ROWS * C::N2 * sizeof(cplx<T>));
+                    for (int i = tid; i < C::ROWS * C::N2; i += C::NT) {
+                        const int rr = r0 + i / C::N2;
+                        if (rr < C::N1) {
+                            const cplx<T> w = e.big_twiddle(__ldg(&a.perm1[rr]), i % C::N2);
+                            cw[i] = w;
+                            cd[i] = unit_defect(w);
+                        }
+                    }
+                    e.cache_w = cw;
+                    e.cache_wd = cd;
+                }
+            }
+        }
+    }
+    __syncthreads();
 
     cplx<T>* cur[F];
     cplx<T>* srcp[F];
@@ -388,13 +505,12 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
     if (a.mode == 2) {
         // frequency read-out: column transforms src -> cur slot (scratch), rows -> natural order
         e.template col_pass<COL_FWD>(srcp, dstp, mask, batch, phase, a.phase_stride, 0, kap, h);
-        grid_barrier(a.barrier, target);
 #pragma unroll
         for (int x = 0; x < F; ++x) {
             op.kind[x] = ((mask >> x) & 1) ? ROW_FREQ : -1;
             op.out[x] = reinterpret_cast<cplx<T>*>(a.out[x]);
         }
-        e.row_pass(cur, op, batch, a.perm1, a.perm2);
+        e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);
         return;
     }
 
@@ -407,7 +523,6 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
         const int zs = rt_mode ? 0 : a.z0, nsteps = rt_mode ? nz : a.steps;
         const T hh = (T)0.5 * h;
         e.template col_pass<COL_NFWD>(cur, cur, mask, batch, phase, a.phase_stride, 4 * zs, kap, hh);
-        grid_barrier(a.barrier, target);
 #pragma unroll
         for (int x = 0; x < F; ++x) {
             op.sh_store[x] = nullptr; op.aux[x] = nullptr; op.out[x] = nullptr; op.tab_stride[x] = 0;
@@ -416,19 +531,15 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
         }
 #pragma unroll 1
         for (int q = 0; q < nsteps; ++q) {
-            e.row_pass(cur, op, batch, a.perm1, a.perm2);
+            e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);      // (begins with the grid barrier)
             grid_barrier(a.barrier, target);
-            if (q + 1 < nsteps) {
-                e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 4 * (zs + q) + 2, kap, hh, true);
-                grid_barrier(a.barrier, target);
-            }
+            if (q + 1 < nsteps) e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 4 * (zs + q) + 2, kap, hh, true);
         }
         e.template col_pass<COL_INVN>(cur, cur, mask, batch, phase, a.phase_stride, 4 * (zs + nsteps - 1) + 2, kap, hh);
         return;
     }
 
     e.template col_pass<COL_FWD>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
-    grid_barrier(a.barrier, target);
 #pragma unroll 1
     for (int q = 0; q <= total; ++q) {
         const int s = rt_mode ? q % nz : a.z0 + q;
@@ -453,11 +564,10 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
                 if (rt_mode && q == 0 && !res && a.steps > 1) op.sh_store[x] = reinterpret_cast<cplx<T>*>(a.SH[x]);
             }
         }
-        e.row_pass(cur, op, batch, a.perm1, a.perm2);
+        e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);          // (begins with the grid barrier)
         grid_barrier(a.barrier, target);
         if (q == total) break;
         e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 2 * s, kap, h);
-        grid_barrier(a.barrier, target);
     }
     e.template col_pass<COL_INV>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
 }
