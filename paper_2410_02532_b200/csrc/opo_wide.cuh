@@ -18,9 +18,15 @@
 //           (one of them is local), integrates, and writes them back to their owners.
 //   sync  : no cluster-wide barrier inside the z-step loop.  The pass-1 butterfly t' touches the elements t' + (S/16) k,
 //           so the tiles of class c = (tile mod S/512) depend exactly on the pass-1 butterflies of warp c of every CTA, and
-//           vice versa: warp c of each of the 4 F CTAs forms a ring of its own, synchronised by two mbarriers per CTA
-//           and class (ready[c], done[c]: 4 F remote arrivals each).  The 16 tiles of a class are dealt to the 4 F warps of
-//           its ring (rotated by the class so that every CTA gets the same number of tiles).
+//           vice versa: warp c of each of the 4 F CTAs forms a ring of its own.  The 16 tiles of a class are dealt to the 4 F
+//           warps of its ring (rotated by the class so that every CTA gets the same number of tiles).
+//   push  : all traffic between the SMs is asynchronous stores (st.async ... mbarrier::complete_tx::bytes).  The inverse
+//           pass 1 does not write its 16 results back in place: it sends each one to the staging buffer of the warp that
+//           owns its tile; that warp waits on a local mbarrier (ready[c], armed with the bytes it expects), reads its 4 F
+//           operands per butterfly from LOCAL shared memory, integrates, and sends every result to its owner's field, where
+//           the forward pass 1 waits on done[c] the same way.  No remote load, no release fence and no arrival message is
+//           ever waited for: a z-step was 7.2 us with remote loads + release/acquire arrivals (the top stalls were the
+//           long scoreboard of the remote loads and the membar of the releases).
 //
 // Everything else (merged tables H, H2, HB = H2 G m across the cavity boundary; stored
 // inputs SH of non-resonant fields re-injected every round trip, L268; mirror / spectral phase / modulator of the
@@ -43,8 +49,13 @@ template <class T, int L, int F> struct wide_layout {
     static constexpr bool ok = PL::P == 4 && PL::rbits(0) == 2 && PL::rbits(1) == 4 && NT >= 32;
     static constexpr size_t field_bytes = (size_t)padded_len<T>(S) * sizeof(cplx<T>);
     static constexpr size_t tw_bytes = (size_t)PL::tw_local_count * sizeof(cplx<T>);
-    static constexpr size_t mbar_offset = (field_bytes + tw_bytes + 15) / 16 * 16;
+    static constexpr int NQ = C * F;                         // operands of a pass-0 butterfly over all fields
+    // staging buffer of the fused phase: [warp][tile of the warp][field, sub-block][lane]
+    static constexpr size_t stage_offset = (field_bytes + tw_bytes + 15) / 16 * 16;
+    static constexpr size_t stage_bytes = (size_t)(NW > 0 ? NW : 1) * MAXT * NQ * 32 * sizeof(cplx<T>);
+    static constexpr size_t mbar_offset = stage_offset + stage_bytes;
     static constexpr size_t total = mbar_offset + 16 * (size_t)(NW > 0 ? NW : 1);
+    static constexpr uint32_t done_bytes = TPC * 32 * (uint32_t)sizeof(cplx<T>);      // results per class and phase arriving in a CTA
 };
 
 // distributed shared memory through 32-bit shared::cluster addresses (half the address registers of generic pointers)
@@ -70,25 +81,58 @@ __device__ __forceinline__ void dsmem_st(uint32_t addr, cplx<double> v) {
     asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.re), "d"(v.im) : "memory");
 }
 
+// asynchronous store into a CTA of the cluster; its bytes are counted on the mbarrier `mbar` OF THAT CTA (complete_tx),
+// which is what orders the data before the waiter's reads: no fence, no arrival message
+__device__ __forceinline__ void st_async(uint32_t addr, cplx<float> v, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(addr), "f"(v.re), "f"(v.im), "r"(mbar) : "memory");
+}
+__device__ __forceinline__ void st_async(uint32_t addr, cplx<double> v, uint32_t mbar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(addr), "d"(v.re), "d"(v.im), "r"(mbar) : "memory");
+}
+// one thread arms a barrier of its own CTA for the next phase: its single arrival plus the bytes that phase will bring
+__device__ __forceinline__ void mbar_arm(uint32_t addr, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.release.cta.shared::cta.b64 _, [%0], %1;" ::"r"(addr), "r"(bytes) : "memory");
+}
+
 struct WideFlow {
     uint32_t mb;         // shared address of ready[0]; done[c] = mb + 8 (NW + c)
-    int ncta;            // CTAs in the cluster
+    uint32_t stage;      // shared address of the staging buffer
+    int q_me;            // my operand slot 4 x + j in a staged butterfly
     int wait_in;         // forward pass 1 waits for done[warp] (a fused phase precedes)
-    int arrive_out;      // inverse pass 1 arrives on ready[warp] of every CTA (a fused phase follows)
+    int push_out;        // inverse pass 1 sends its results to the owners of their tiles (a fused phase follows); else in place
     uint32_t par_done;
 };
 
+// The 16 values v[m] = elements t' + (S/16) m of this thread's pass-1 butterfly t' (class c = warp) go to the warps that own
+// the tiles c + NW m: CTA (m + 4 c) mod NCTA, that warp's tile m / NCTA, operand slot q_me, lane t' mod 32.
+template <class T, int NW, int NCTA, int MAXT, int NQ>
+__device__ __forceinline__ void wide_push16(const cplx<T>* v, const WideFlow& fa, int warp, int lane) {
+    const uint32_t slot = fa.stage + (uint32_t)(((warp * MAXT) * NQ + fa.q_me) * 32 + lane) * (uint32_t)sizeof(cplx<T>);
+    const uint32_t bar = fa.mb + 8 * warp;
+#pragma unroll
+    for (int m = 0; m < 16; ++m) {
+        const int owner = (m + 4 * warp) % NCTA;
+        st_async(dsmem_addr(slot + (uint32_t)((m / NCTA) * NQ * 32) * (uint32_t)sizeof(cplx<T>), owner), v[m], dsmem_addr(bar, owner));
+    }
+}
+
 // The linear core of one sub-block.  smv is the "virtual" base of the field: logical index i lives at smv[phys(i)], and
 // this CTA holds i in [j S, (j + 1) S) only; the butterfly and table indices are the global ones of plan<L>.
-template <class T, int L, int NT>
-__device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const cplx<T>* __restrict__ tab, int j, int tid, WideFlow fa) {
+// sh_keep (may be null): the results of the inverse pass 1 are also stored there (the half-stepped input of a non-resonant
+// field, kept for the later round trips).
+template <class T, int L, int NT, int NCTA, int MAXT, int NQ>
+__device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const cplx<T>* __restrict__ tab, int j, int tid, WideFlow fa,
+                                       cplx<T>* __restrict__ sh_keep) {
     using PL = plan<L>;
     constexpr int NW = NT / 32, S = 1 << (L - 2);
     constexpr int RBL = PL::rbits(3), R = 1 << RBL, NBF = (1 << L) >> RBL, NBL = S >> RBL;
     constexpr int NB2 = S >> PL::rbits(2);
     constexpr bool chain = PL::rbits(2) == RBL && NBL % NT == 0;     // N = 2^14: passes 2, 3, 2 stay inside a warp's blocks
     const int warp = tid >> 5, lane = tid & 31;
-    if (fa.wait_in) mbar_wait(fa.mb + 8 * (NW + warp), fa.par_done);
+    if (fa.wait_in) {
+        mbar_wait(fa.mb + 8 * (NW + warp), fa.par_done);
+        if (lane == 0) mbar_arm(fa.mb + 8 * (NW + warp), 16u * 32u * (uint32_t)sizeof(cplx<T>));       // the results of the next fused phase
+    }
     fwd_bf<T, L, 1>(smv, twl, j * NT + tid);
     __syncthreads();
     if constexpr (chain) {
@@ -121,8 +165,26 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
         for (int ul = tid; ul < NB2; ul += NT) inv_bf<T, L, 2>(smv, twl, j * NB2 + ul);
     }
     __syncthreads();
-    inv_bf<T, L, 1>(smv, twl, j * NT + tid);
-    if (fa.arrive_out) mbar_arrive_cluster(fa.mb + 8 * warp, lane, fa.ncta);
+    if (!fa.push_out) {
+        inv_bf<T, L, 1>(smv, twl, j * NT + tid);
+    } else {
+        // inverse pass 1 with its results sent to the owners of their tiles
+        constexpr int RB = PL::rbits(1), R1 = 1 << RB, SB = PL::sbits(1);
+        static_assert(R1 == 16 && (1 << SB) == NT, "one radix-16 pass-1 butterfly per thread");
+        const cplx<T>* __restrict__ w = twl + PL::tw_offset(1);
+        const cplx<T>* __restrict__ p = smv + elem_base<T, RB, SB>(j, tid);
+        cplx<T> v[R1];
+#pragma unroll
+        for (int k = 0; k < R1; ++k) v[k] = p[elem_off<T, RB, SB>(k)];
+#pragma unroll
+        for (int k = 1; k < R1; ++k) v[k] = cmulc(v[k], w[((k - 1) << SB) + tid]);
+        dit_inv<T, R1>::run(v);
+        wide_push16<T, NW, NCTA, MAXT, NQ>(v, fa, warp, lane);
+        if (sh_keep != nullptr) {
+#pragma unroll
+            for (int m = 0; m < R1; ++m) sh_keep[tid + NT * m] = v[m];
+        }
+    }
 }
 
 enum { WIDE_RK4 = 0, WIDE_FWD0 = 1, WIDE_INV0 = 2 };
@@ -157,12 +219,12 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
     const uint32_t mb = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::mbar_offset);
     if (tid == 0) {
         for (int c = 0; c < NW; ++c) {
-            mbar_init(mb + 8 * c, NCTA);              // ready[c]: warp c of every CTA after its inverse pass 1
-            mbar_init(mb + 8 * (NW + c), NCTA);       // done[c] : warp c of every CTA after its tiles
+            mbar_init(mb + 8 * c, 1);                 // ready[c]: the operands of warp c's tiles have arrived in its staging buffer
+            mbar_init(mb + 8 * (NW + c), 1);          // done[c] : the results of all tiles of class c have arrived in my field
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    cluster.sync();       // every CTA's barriers exist (and its twiddle copy is complete) before anybody arrives on them
+    cluster.sync();       // every CTA's barriers exist (and its twiddle copy is complete) before anybody sends to them
 
     // this thread's pass-0 butterflies -- the same at every z-step -- and their twiddles
     int nt_own = 0;
@@ -185,6 +247,21 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
         }
     }
 
+    // Every phase of a barrier has ONE arrival -- its own warp's, which also announces the bytes the phase will bring
+    // (mbar_arm) -- and completes when those bytes have landed.  A warp arms the next phase right after its wait; bytes that
+    // arrive before the arming leave the count negative for a moment, which the barrier allows.
+    const uint32_t ready_bytes = (uint32_t)nt_own * WL::NQ * 32 * (uint32_t)sizeof(cplx<T>);
+    if (lane == 0) {
+        mbar_arm(mb + 8 * warp, ready_bytes);
+        mbar_arm(mb + 8 * (NW + warp), WL::done_bytes);
+    }
+    WideFlow fb;
+    fb.mb = mb;
+    fb.stage = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::stage_offset);
+    fb.q_me = rank;
+    fb.wait_in = 0; fb.push_out = 0; fb.par_done = 0;
+    const cplx<T>* stg = reinterpret_cast<const cplx<T>*>(smem_raw + WL::stage_offset) + (size_t)(warp * WL::MAXT) * WL::NQ * 32 + lane;
+
     T kap[3] = {(T)a.kappa[0], (T)a.kappa[1], (T)a.kappa[2]};
     const T h = (T)a.h;
     const int nz = a.nz;
@@ -199,20 +276,28 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
     auto tiles = [&](auto mode_tag, int mask, cplx<T> e0, cplx<T> e1, cplx<T> e2) {
         constexpr int MODE = decltype(mode_tag)::value;
         cplx<T> v[WL::MAXT][F][R];
+        if constexpr (MODE != WIDE_RK4) {
 #pragma unroll
-        for (int i = 0; i < WL::MAXT; ++i) {        // all loads of all tiles in flight before the first is consumed
-            if (i < nt_own) {
+            for (int i = 0; i < WL::MAXT; ++i) {        // remote loads: all of them in flight before the first is consumed
+                if (i < nt_own) {
 #pragma unroll
-                for (int f = 0; f < F; ++f) {
-                    if (MODE != WIDE_RK4 && !((mask >> f) & 1)) continue;
+                    for (int f = 0; f < F; ++f) {
+                        if (!((mask >> f) & 1)) continue;
 #pragma unroll
-                    for (int k = 0; k < R; ++k) v[i][f][k] = dsmem_ld(fld[f][k] + p_own[i], cplx<T>{});
+                        for (int k = 0; k < R; ++k) v[i][f][k] = dsmem_ld(fld[f][k] + p_own[i], cplx<T>{});
+                    }
                 }
             }
         }
 #pragma unroll
         for (int i = 0; i < WL::MAXT; ++i) {
             if (i < nt_own) {
+                if constexpr (MODE == WIDE_RK4) {       // operands staged in local shared memory by the owners' inverse pass 1
+#pragma unroll
+                    for (int f = 0; f < F; ++f)
+#pragma unroll
+                        for (int k = 0; k < R; ++k) v[i][f][k] = stg[(i * WL::NQ + f * WL::C + k) * 32];
+                }
 #pragma unroll
                 for (int f = 0; f < F; ++f) {
                     if (MODE != WIDE_RK4 && !((mask >> f) & 1)) continue;
@@ -242,7 +327,11 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
                         for (int k = 1; k < R; ++k) v[i][f][k] = cmul(v[i][f][k], w0[i][k - 1]);
                     }
 #pragma unroll
-                    for (int k = 0; k < R; ++k) dsmem_st(fld[f][k] + p_own[i], v[i][f][k]);
+                    for (int k = 0; k < R; ++k) {
+                        if constexpr (MODE == WIDE_RK4)
+                            st_async(fld[f][k] + p_own[i], v[i][f][k], fld[f][k] + (uint32_t)(WL::mbar_offset + 8 * (NW + warp)));    // counted on done[warp] of the owner
+                        else dsmem_st(fld[f][k] + p_own[i], v[i][f][k]);
+                    }
                 }
             }
         }
@@ -285,31 +374,26 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
                 if (q < total) { e0 = ldg(ph + 2 * s); e1 = ldg(ph + 2 * s + 1); e2 = ldg(ph + 2 * s + 2); }
             }
             if (crossing && !resonant) {
-                // fresh pump / frozen seed, already half-stepped: a thread reloads the elements of its own
-                // pass-1 butterfly, i.e. of its class, as soon as the tiles of that class have let go of them
+                // fresh pump / frozen seed, already half-stepped: a thread sends the elements of its own pass-1
+                // butterfly, i.e. of its class, to the tiles' owners as an inverse pass 1 would
                 mbar_wait(mb + 8 * (NW + warp), (fz - 1) & 1);
+                if (lane == 0) mbar_arm(mb + 8 * (NW + warp), WL::done_bytes);
                 const cplx<T>* __restrict__ g = SH;
+                cplx<T> v[16];
 #pragma unroll
-                for (int k = 0; k < 16; ++k) sm[phys<T>(tid + NT * k)] = g[tid + NT * k];
-                mbar_arrive_cluster(mb + 8 * warp, lane, NCTA);
+                for (int k = 0; k < 16; ++k) v[k] = g[tid + NT * k];
+                wide_push16<T, NW, NCTA, WL::MAXT, WL::NQ>(v, fb, warp, lane);
             } else {
                 const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
-                WideFlow fa;
-                fa.mb = mb; fa.ncta = NCTA;
+                WideFlow fa = fb;
                 fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
-                fa.arrive_out = (q < total) && !keep;
-                wide_core<T, L, NT>(smv, twl, tab, j, tid, fa);
-                if (keep) {       // the elements of my own inverse pass-1 butterfly: no barrier needed
-                    cplx<T>* __restrict__ g = SH;
-#pragma unroll
-                    for (int k = 0; k < 16; ++k) g[tid + NT * k] = sm[phys<T>(tid + NT * k)];
-                    mbar_arrive_cluster(mb + 8 * warp, lane, NCTA);
-                }
+                fa.push_out = q < total;
+                wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
             }
             if (q == total) break;
-            mbar_wait(mb + 8 * warp, fz & 1);                 // ready[warp]: inverse pass 1 of my class is done in every CTA
+            mbar_wait(mb + 8 * warp, fz & 1);                 // ready[warp]: the operands of my tiles are in my staging buffer
+            if (lane == 0) mbar_arm(mb + 8 * warp, ready_bytes);
             tiles(tag_rk4{}, (1 << F) - 1, e0, e1, e2);
-            mbar_arrive_cluster(mb + 8 * (NW + warp), lane, NCTA);      // done[warp] in every CTA
             ++fz;
         }
         cluster_bar();                                    // every field is ready for its inverse pass 0
@@ -336,8 +420,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
                 cluster_bar();
                 if ((maskb >> x) & 1) {
                     const cplx<T>* tabGM = reinterpret_cast<const cplx<T>*>(a.tabGM[x]) + (size_t)b * a.tab_stride[x];
-                    WideFlow fa{};
-                    wide_core<T, L, NT>(smv, twl, tabGM, j, tid, fa);
+                    wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tabGM, j, tid, fb, nullptr);
                 }
                 cluster_bar();
                 tiles(tag_inv0{}, maskb, one, one, one);
