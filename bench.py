@@ -190,6 +190,9 @@ def main():
     ap.add_argument("--eom", action="store_true",
                     help="intracavity phase modulator on the signal (PAPER.md:L149-154; beta = 1 rad, f = 3 / window): the "
                          "paper's 'EOM' cavity configuration; the boundary is then not merged (one launch per round trip)")
+    ap.add_argument("--train", action="store_true",
+                    help="nanosecond regime (PAPER.md:L322-335): opo_roundtrips_train -- a pump slice per round trip in, the exit "
+                         "signal of every round trip out, one launch per round trip; default 20 round trips per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -222,7 +225,7 @@ def main():
     if args.eom:
         w.eom_beta_rad = [0.0, 1.0, 0.0]
         w.eom_f_hz = [0.0, 3.0 / w.window_s, 0.0]
-    rt_per_step = args.rt_per_step or {"C0": w.n_roundtrips, "C1": 100, "C2": 20, "C3": 2, "C4": w.n_roundtrips}[args.workload]
+    rt_per_step = args.rt_per_step or (20 if args.train else {"C0": w.n_roundtrips, "C1": 100, "C2": 20, "C3": 2, "C4": w.n_roundtrips}[args.workload])
     engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "solo": P.ENGINE_SOLO, "wide": P.ENGINE_WIDE, "streaming": P.ENGINE_STREAMING, "cufft": P.ENGINE_CUFFT}[args.engine]
     o = P.from_workload(w, engine=engine)
     units_per_step = w.batch * w.n * w.nz_per_pass * rt_per_step          # grid-point z-steps, this rank
@@ -241,8 +244,15 @@ def main():
         for x in range(1, w.n_fields):
             o.set_field(x, d_seeds[x])
 
+    d_train = None
+    if args.train:      # the same pump slice every round trip: the work of the default step, driven slice by slice
+        d_train = (d_pump if d_pump.shape[0] > 1 else d_pump[0]).unsqueeze(0).expand(rt_per_step, *((-1,) * (d_pump.dim() if d_pump.shape[0] > 1 else 1))).contiguous()
+
     def step_resident_inputs():
-        o.roundtrips(rt_per_step)
+        if args.train:
+            o.roundtrips_train(d_train, out_field=1)
+        else:
+            o.roundtrips(rt_per_step)
 
     def step_e2e():
         o.set_pump(h_pump if h_pump.shape[0] > 1 else h_pump[0])
@@ -343,7 +353,7 @@ def main():
             "dtype": "f32" if w.precision == "c64" else "f64", "data": "synthetic",
             "config": {"workload": f"{w.name}: BASELINE.json configs[{args.workload[1]}], batch {w.batch} x N=2^{w.log2_n} x "
                                    f"{w.n_fields} fields, nz={w.nz_per_pass}, {rt_per_step} round trips per step" + (", EOM on the signal" if args.eom else ""),
-                       "engine": eng_name,
+                       "engine": eng_name, **({"mode": "pump train: one pump slice in and one exit slice out per round trip (opo_roundtrips_train)"} if args.train else {}),
                        "l2": "512 MiB flush write between timed steps", "sharding": "independent instances per rank, no collective"},
             "round_trips_per_s": world * w.batch * rt_per_step * args.steps / t_total,
             "field_point_z_steps_per_s": value * w.n_fields,

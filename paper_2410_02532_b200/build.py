@@ -87,7 +87,8 @@ def _jobs(only=None):
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile every CUDA source for sm_100a and link libopo.so.  OPO_BUILD_ONLY="f32:14,f64:10"
     (development only) restricts the size-specialised instances; sizes left out report
-    OPO_ERR_UNSUPPORTED at opo_create."""
+    OPO_ERR_UNSUPPORTED at opo_create.  OPO_EXTRA_NVCC_FLAGS (diagnostic builds, e.g. -DOPO_LARGE_TIMING) is
+    appended to every compile; use it with --force and rebuild without it afterwards."""
     only = os.environ.get("OPO_BUILD_ONLY")
     only = set(only.split(",")) if only else None
     if not force and not only and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source_mtime():
@@ -102,7 +103,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         # an object is stale when its source or a header it includes is newer
         if not force and os.path.exists(obj) and os.path.getmtime(obj) >= _deps_mtime(os.path.join(CSRC, src)):
             return obj
-        cmd = [nvcc, *NVCC_FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("OPO_EXTRA_NVCC_FLAGS", "").split(), *defs, "-c", os.path.join(CSRC, src), "-o", obj]
         res = subprocess.run(cmd, capture_output=True, text=True)
         with open(obj + ".log", "w") as f:
             f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
@@ -112,8 +113,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
             print(res.stderr)
         return obj
 
+    jobs = _jobs(only)
+    for src in sorted({j[0] for j in jobs}):        # fill the dependency cache before the threads start: _deps_mtime is not
+        _deps_mtime(os.path.join(CSRC, src))        # re-entrant (a half-computed entry would hide a changed header)
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
-        objs = list(ex.map(compile_one, _jobs(only)))
+        objs = list(ex.map(compile_one, jobs))
     cmd = [nvcc, "-shared", "-o", LIB, *objs, "-cudart", "static", "-ldl"]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:

@@ -661,7 +661,7 @@ int check_async(opo_handle* h) {
 // AUTO between the two on-chip engines: the cluster engine gives an instance F SMs (lowest latency per instance,
 // rinfo.max_clusters instances at a time), the solo engine one SM (no SM-to-SM exchange, every SM busy, sinfo.max_clusters
 // instances at a time).  Per z-step an instance takes ~2.6x longer on one SM than on a cluster of three (measured on C4 /
-// C1, DESIGN.md section 5.5), so solo wins once the batch keeps more than ~2.6x as many CTAs busy as there are clusters.
+// C1, DESIGN.md section 5.3), so solo wins once the batch keeps more than ~2.6x as many CTAs busy as there are clusters.
 bool prefer_solo(const opo_handle* h) {
     if (!h->solo_ok || h->splitting) return false;      // the N/2 - L - N/2 ordering runs on the cluster engine
     if (!h->resident_ok) return true;
@@ -679,14 +679,14 @@ bool wide_serves(const opo_handle* h) {
 }
 
 // AUTO takes the wide engine (4 F SMs per instance, the lowest latency per z-step) when it finishes the batch sooner than
-// the cluster engine: an instance takes 2.2x less time per z-step on 4 F SMs than on F (measured on C1: 7.2 vs 15.9 us),
+// the cluster engine: an instance takes 2.8x less time per z-step on 4 F SMs than on F (measured on C1: 5.7 vs 15.9 us),
 // but only winfo.max_clusters clusters of 4 F CTAs are co-resident (7 of 12 CTAs on a B200), so the batch runs in waves.
 bool prefer_wide(const opo_handle* h) {
     if (!wide_serves(h)) return false;
     if (!h->resident_ok) return true;
     const int waves_w = (h->B + h->winfo.max_clusters - 1) / h->winfo.max_clusters;
     const int waves_r = (h->B + h->rinfo.max_clusters - 1) / h->rinfo.max_clusters;
-    return (double)waves_w < 2.2 * (double)waves_r;
+    return (double)waves_w < 2.8 * (double)waves_r;
 }
 
 int engine_in_use(const opo_handle* h) {

@@ -158,7 +158,19 @@ __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, cons
 enum { COL_FWD = 0, COL_RK4 = 1, COL_INV = 2, COL_NFWD = 3, COL_INVN = 4 };
 enum { ROW_LINEAR = 0, ROW_RELOAD = 1, ROW_FREQ = 2 };
 
+// Diagnostic build (-DOPO_LARGE_TIMING; OPO_EXTRA_NVCC_FLAGS of build.py): thread 0 of a CTA accumulates clock64 stamps per
+// phase of a z-step, two CTAs print their per-z-step averages when the launch ends (profiles/r02f_large_kernel.md).
+#ifdef OPO_LARGE_TIMING
+#define OPO_TSTAMP(eng, i) do { if (threadIdx.x == 0) { const long long t_ = clock64(); (eng).t_acc[i] += t_ - (eng).t_last; (eng).t_last = t_; } } while (0)
+#else
+#define OPO_TSTAMP(eng, i) do {} while (0)
+#endif
+
 template <class T, int L, int F> struct LargeEngine {
+#ifdef OPO_LARGE_TIMING
+    long long t_acc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    long long t_last = 0;
+#endif
     using C = large_cfg<T, L, F>;
     using TAB = typename large_tab<T>::type;
     using P1 = plan<C::L1>;
@@ -235,6 +247,10 @@ template <class T, int L, int F> struct LargeEngine {
                     for (int x = 0; x < F; ++x) sm[(x * C::TC + c) * C::CSTRIDE + phys<T>(n1)] = y[x];
                 }
             };
+#ifdef OPO_LARGE_TIMING
+            __syncthreads();
+            OPO_TSTAMP(*this, 0);                           // column tile loaded
+#endif
             if constexpr (MODE == COL_NFWD) rk4_tile();
             if constexpr (MODE != COL_FWD && MODE != COL_NFWD) {
                 __syncthreads();
@@ -264,6 +280,7 @@ template <class T, int L, int F> struct LargeEngine {
                 fwd_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
             }
             __syncthreads();
+            OPO_TSTAMP(*this, 1);                           // column transforms + RK4
 #pragma unroll
             for (int x = 0; x < F; ++x) {
                 if (!((mask >> x) & 1)) continue;
@@ -275,6 +292,7 @@ template <class T, int L, int F> struct LargeEngine {
                 }
             }
             __syncthreads();
+            OPO_TSTAMP(*this, 2);                           // column tile stored
         }
     }
 
@@ -367,7 +385,9 @@ template <class T, int L, int F> struct LargeEngine {
                         else wd[j] = 0.0f;
                     }
                 }
+                OPO_TSTAMP(*this, 3);                       // row prologue
                 sync_once();
+                OPO_TSTAMP(*this, 4);                       // grid barrier after the column pass
                 if (active) {
 #pragma unroll
                     for (int j = 0; j < CNT; ++j) rv[j] = ldcg(g + lt + j * C::TT2);
@@ -389,6 +409,7 @@ template <class T, int L, int F> struct LargeEngine {
                     for (int j = 0; j < CNT; ++j) smt[phys<T>(lt + j * C::TT2)] = cmul(rv[j], w[j]);
                 }
                 pass_sync<C::SY2>(1 + team);
+                OPO_TSTAMP(*this, 5);                       // row loaded (team 0)
                 fwd_passes<T, C::L2, C::TT2, true, 0, C::SY2>(smt, tw2, lt, 1 + team);
                 if (cached) {
                     const TAB* ct = cache_tab + team * C::N2;
@@ -401,6 +422,7 @@ template <class T, int L, int F> struct LargeEngine {
                 for (int it = 0; it < NIT; ++it) mid_bf<T, C::L2, TAB>(smt, hh[it], lt + it * C::TT2);
                 inv_passes<T, C::L2, C::TT2, true, 0, C::SY2, true>(smt, tw2, lt, 1 + team, dtw2);
                 pass_sync<C::SY2>(1 + team);
+                OPO_TSTAMP(*this, 6);                       // row transforms (team 0)
                 if (active) {
                     cplx<T>* sh = op.sh_store[x] ? op.sh_store[x] + off : nullptr;
 #pragma unroll
@@ -565,11 +587,20 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
             }
         }
         e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);          // (begins with the grid barrier)
+        OPO_TSTAMP(e, 7);                                   // row stored
         grid_barrier(a.barrier, target);
+        OPO_TSTAMP(e, 8);                                   // grid barrier after the row pass
         if (q == total) break;
         e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 2 * s, kap, h);
     }
     e.template col_pass<COL_INV>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
+#ifdef OPO_LARGE_TIMING
+    // (the first column-load interval of a launch starts at t = 0 and is left out: divide the rest by the z-steps timed)
+    if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == gridDim.x / 2) && total >= 100)
+        printf("k_large cta %d, cycles per z-step (%d z-steps): col compute %lld store %lld | row prologue %lld barrier %lld load %lld "
+               "compute %lld store %lld barrier %lld | next col load = z-step time minus these\n", (int)blockIdx.x, total, e.t_acc[1] / total,
+               e.t_acc[2] / total, e.t_acc[3] / total, e.t_acc[4] / total, e.t_acc[5] / total, e.t_acc[6] / total, e.t_acc[7] / total, e.t_acc[8] / total);
+#endif
 }
 
 template <class T, int L, int F> cudaError_t large_setup() {

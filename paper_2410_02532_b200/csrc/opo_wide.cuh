@@ -19,7 +19,9 @@
 //   sync  : no cluster-wide barrier inside the z-step loop.  The pass-1 butterfly t' touches the elements t' + (S/16) k,
 //           so the tiles of class c = (tile mod S/512) depend exactly on the pass-1 butterflies of warp c of every CTA, and
 //           vice versa: warp c of each of the 4 F CTAs forms a ring of its own.  The 16 tiles of a class are dealt to the 4 F
-//           warps of its ring (rotated by the class so that every CTA gets the same number of tiles).
+//           warps of its ring (rotated by the class so that every CTA gets the same number of tiles): two tiles per warp
+//           with two fields; with three fields 12 warps would share 16 tiles, so the four left over per class go to
+//           HELPER warps -- up to three extra warps per CTA that take no part in the core and integrate one tile each.
 //   push  : all traffic between the SMs is asynchronous stores (st.async ... mbarrier::complete_tx::bytes).  The inverse
 //           pass 1 does not write its 16 results back in place: it sends each one to the staging buffer of the warp that
 //           owns its tile; that warp waits on a local mbarrier (ready[c], armed with the bytes it expects), reads its 4 F
@@ -45,16 +47,21 @@ template <class T, int L, int F> struct wide_layout {
     static constexpr int NT = S / 16;                        // one radix-16 pass-1 butterfly per thread
     static constexpr int NW = NT / 32;                       // warps per CTA = classes
     static constexpr int TPC = 16;                           // tiles (of 32 pass-0 butterflies) per class: S / 32 / NW
-    static constexpr int MAXT = (TPC + NCTA - 1) / NCTA;     // tiles per warp
+    // core warps own TPC / NCTA tiles each (rounded down); the EX tiles left over go to NH helper warps per CTA, one each
+    static constexpr int MAXT = TPC / NCTA;                  // tiles per core warp: 2 (two fields), 1 (three fields)
+    static constexpr int EX = (TPC - MAXT * NCTA) * NW;      // tiles of the cluster no core warp owns: 0 / 4 NW
+    static constexpr int NH = (EX + NCTA - 1) / NCTA;        // helper warps per CTA
+    static constexpr int NTH = NT + 32 * NH;                 // threads per CTA
+    static constexpr int NSLOT = NW * MAXT + NH;             // staging slots (one per owned tile)
     static constexpr bool ok = PL::P == 4 && PL::rbits(0) == 2 && PL::rbits(1) == 4 && NT >= 32;
     static constexpr size_t field_bytes = (size_t)padded_len<T>(S) * sizeof(cplx<T>);
     static constexpr size_t tw_bytes = (size_t)PL::tw_local_count * sizeof(cplx<T>);
     static constexpr int NQ = C * F;                         // operands of a pass-0 butterfly over all fields
-    // staging buffer of the fused phase: [warp][tile of the warp][field, sub-block][lane]
+    // staging buffer of the fused phase: [slot][field, sub-block][lane]; slot = warp MAXT + tile (core warps), NW MAXT + h (helpers)
     static constexpr size_t stage_offset = (field_bytes + tw_bytes + 15) / 16 * 16;
-    static constexpr size_t stage_bytes = (size_t)(NW > 0 ? NW : 1) * MAXT * NQ * 32 * sizeof(cplx<T>);
-    static constexpr size_t mbar_offset = stage_offset + stage_bytes;
-    static constexpr size_t total = mbar_offset + 16 * (size_t)(NW > 0 ? NW : 1);
+    static constexpr size_t stage_bytes = (size_t)(NSLOT > 0 ? NSLOT : 1) * NQ * 32 * sizeof(cplx<T>);
+    static constexpr size_t mbar_offset = stage_offset + stage_bytes;           // ready[NW], done[NW], helper_ready[NH]
+    static constexpr size_t total = mbar_offset + 8 * (size_t)(2 * NW + NH) + 8;
     static constexpr uint32_t done_bytes = TPC * 32 * (uint32_t)sizeof(cplx<T>);      // results per class and phase arriving in a CTA
 };
 
@@ -104,15 +111,21 @@ struct WideFlow {
 };
 
 // The 16 values v[m] = elements t' + (S/16) m of this thread's pass-1 butterfly t' (class c = warp) go to the warps that own
-// the tiles c + NW m: CTA (m + 4 c) mod NCTA, that warp's tile m / NCTA, operand slot q_me, lane t' mod 32.
+// the tiles c + NW m.  m < MAXT NCTA: core warp c of CTA (m + 4 c) mod NCTA, its tile m / NCTA; the others: tile number
+// e = (m - MAXT NCTA) NW + c of the left-over tiles, helper e / NCTA of CTA e mod NCTA.  Operand slot q_me, lane t' mod 32.
 template <class T, int NW, int NCTA, int MAXT, int NQ>
 __device__ __forceinline__ void wide_push16(const cplx<T>* v, const WideFlow& fa, int warp, int lane) {
-    const uint32_t slot = fa.stage + (uint32_t)(((warp * MAXT) * NQ + fa.q_me) * 32 + lane) * (uint32_t)sizeof(cplx<T>);
-    const uint32_t bar = fa.mb + 8 * warp;
+    constexpr uint32_t SLOT = (uint32_t)(NQ * 32 * sizeof(cplx<T>));
+    const uint32_t base = fa.stage + (uint32_t)(fa.q_me * 32 + lane) * (uint32_t)sizeof(cplx<T>);
 #pragma unroll
     for (int m = 0; m < 16; ++m) {
-        const int owner = (m + 4 * warp) % NCTA;
-        st_async(dsmem_addr(slot + (uint32_t)((m / NCTA) * NQ * 32) * (uint32_t)sizeof(cplx<T>), owner), v[m], dsmem_addr(bar, owner));
+        if (m < MAXT * NCTA) {
+            const int owner = (m + 4 * warp) % NCTA;
+            st_async(dsmem_addr(base + (uint32_t)(warp * MAXT + m / NCTA) * SLOT, owner), v[m], dsmem_addr(fa.mb + 8 * warp, owner));
+        } else {
+            const int e = (m - MAXT * NCTA) * NW + warp, owner = e % NCTA, hlp = e / NCTA;
+            st_async(dsmem_addr(base + (uint32_t)(NW * MAXT + hlp) * SLOT, owner), v[m], dsmem_addr(fa.mb + 8 * (2 * NW + hlp), owner));
+        }
     }
 }
 
@@ -129,12 +142,13 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
     constexpr int NB2 = S >> PL::rbits(2);
     constexpr bool chain = PL::rbits(2) == RBL && NBL % NT == 0;     // N = 2^14: passes 2, 3, 2 stay inside a warp's blocks
     const int warp = tid >> 5, lane = tid & 31;
+    auto core_bar = [] { asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); };      // the core threads only (helper warps do not come here)
     if (fa.wait_in) {
         mbar_wait(fa.mb + 8 * (NW + warp), fa.par_done);
         if (lane == 0) mbar_arm(fa.mb + 8 * (NW + warp), 16u * 32u * (uint32_t)sizeof(cplx<T>));       // the results of the next fused phase
     }
     fwd_bf<T, L, 1>(smv, twl, j * NT + tid);
-    __syncthreads();
+    core_bar();
     if constexpr (chain) {
 #pragma unroll 1
         for (int ul = tid; ul < NBL; ul += NT) {
@@ -151,7 +165,7 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
     } else {
 #pragma unroll 1
         for (int ul = tid; ul < NB2; ul += NT) fwd_bf<T, L, 2>(smv, twl, j * NB2 + ul);
-        __syncthreads();
+        core_bar();
 #pragma unroll 1
         for (int ul = tid; ul < NBL; ul += NT) {
             const int u = j * NBL + ul;
@@ -160,11 +174,11 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
             for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
             mid_bf<T, L>(smv, h, u);
         }
-        __syncthreads();
+        core_bar();
 #pragma unroll 1
         for (int ul = tid; ul < NB2; ul += NT) inv_bf<T, L, 2>(smv, twl, j * NB2 + ul);
     }
-    __syncthreads();
+    core_bar();
     if (!fa.push_out) {
         inv_bf<T, L, 1>(smv, twl, j * NT + tid);
     } else {
@@ -190,7 +204,7 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
 enum { WIDE_RK4 = 0, WIDE_FWD0 = 1, WIDE_INV0 = 2 };
 
 template <class T, int L, int F, bool DK0 = false>
-__global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentArgs a) {
+__global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentArgs a) {
     using WL = wide_layout<T, L, F>;
     using PL = plan<L>;
     static_assert(WL::ok, "wide engine: N = 4 . 16 . r . r'");
@@ -213,7 +227,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
     const cplx<T>* tw = reinterpret_cast<const cplx<T>*>(a.tw);
     {   // shared-memory copy of the twiddles of the local passes, addressed as the global table is
         cplx<T>* d = reinterpret_cast<cplx<T>*>(smem_raw + WL::field_bytes);
-        for (int i = tid; i < PL::tw_local_count; i += NT) d[i] = ldg(&tw[PL::tw_local_begin + i]);
+        for (int i = tid; i < PL::tw_local_count; i += WL::NTH) d[i] = ldg(&tw[PL::tw_local_begin + i]);
     }
     const cplx<T>* twl = reinterpret_cast<const cplx<T>*>(smem_raw + WL::field_bytes) - PL::tw_local_begin;
     const uint32_t mb = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::mbar_offset);
@@ -222,23 +236,33 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
             mbar_init(mb + 8 * c, 1);                 // ready[c]: the operands of warp c's tiles have arrived in its staging buffer
             mbar_init(mb + 8 * (NW + c), 1);          // done[c] : the results of all tiles of class c have arrived in my field
         }
+        for (int hh = 0; hh < WL::NH; ++hh) mbar_init(mb + 8 * (2 * NW + hh), 1);      // the operands of helper hh's tile have arrived
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     cluster.sync();       // every CTA's barriers exist (and its twiddle copy is complete) before anybody sends to them
 
     // this thread's pass-0 butterflies -- the same at every z-step -- and their twiddles
+    const bool core = warp < NW;                  // a core warp: one pass-1 butterfly per thread, MAXT tiles; else a helper: one tile
     int nt_own = 0;
+    int cls = warp;                               // class of my tiles
     int p_own[WL::MAXT];
     cplx<T> w0[WL::MAXT][R - 1];
     {
-        int m = ((rank - 4 * warp) % NCTA + NCTA) % NCTA;        // tile m of class c goes to CTA (m + 4 c) mod NCTA
+        int m = ((rank - 4 * warp) % NCTA + NCTA) % NCTA;        // tile m < MAXT NCTA of class c goes to CTA (m + 4 c) mod NCTA
+        int n_mine = WL::MAXT;
+        if (!core) {                                             // left-over tile e = hlp NCTA + rank: class e mod NW
+            const int e = (warp - NW) * NCTA + rank;
+            cls = e % NW;
+            m = WL::MAXT * NCTA + e / NW;
+            n_mine = e < WL::EX ? 1 : 0;
+        }
 #pragma unroll
         for (int i = 0; i < WL::MAXT; ++i, m += NCTA) {
             p_own[i] = 0;
 #pragma unroll
             for (int k = 0; k < R - 1; ++k) w0[i][k] = cplx<T>{(T)1, (T)0};
-            if (m < WL::TPC) {
-                const int t = (warp + NW * m) * 32 + lane;
+            if (i < n_mine) {
+                const int t = (cls + NW * m) * 32 + lane;
                 p_own[i] = phys<T>(t) * (int)sizeof(cplx<T>);       // byte offset inside a sub-block
 #pragma unroll
                 for (int k = 0; k < R - 1; ++k) w0[i][k] = ldg(&tw[k * S + t]);
@@ -251,16 +275,18 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
     // (mbar_arm) -- and completes when those bytes have landed.  A warp arms the next phase right after its wait; bytes that
     // arrive before the arming leave the count negative for a moment, which the barrier allows.
     const uint32_t ready_bytes = (uint32_t)nt_own * WL::NQ * 32 * (uint32_t)sizeof(cplx<T>);
+    const uint32_t my_ready = mb + 8 * (core ? warp : 2 * NW + (warp - NW));
     if (lane == 0) {
-        mbar_arm(mb + 8 * warp, ready_bytes);
-        mbar_arm(mb + 8 * (NW + warp), WL::done_bytes);
+        if (nt_own > 0) mbar_arm(my_ready, ready_bytes);
+        if (core) mbar_arm(mb + 8 * (NW + warp), WL::done_bytes);
     }
     WideFlow fb;
     fb.mb = mb;
     fb.stage = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::stage_offset);
     fb.q_me = rank;
     fb.wait_in = 0; fb.push_out = 0; fb.par_done = 0;
-    const cplx<T>* stg = reinterpret_cast<const cplx<T>*>(smem_raw + WL::stage_offset) + (size_t)(warp * WL::MAXT) * WL::NQ * 32 + lane;
+    const cplx<T>* stg = reinterpret_cast<const cplx<T>*>(smem_raw + WL::stage_offset) +
+                         (size_t)(core ? warp * WL::MAXT : NW * WL::MAXT + (warp - NW)) * WL::NQ * 32 + lane;       // my staging slot(s)
 
     T kap[3] = {(T)a.kappa[0], (T)a.kappa[1], (T)a.kappa[2]};
     const T h = (T)a.h;
@@ -329,7 +355,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
 #pragma unroll
                     for (int k = 0; k < R; ++k) {
                         if constexpr (MODE == WIDE_RK4)
-                            st_async(fld[f][k] + p_own[i], v[i][f][k], fld[f][k] + (uint32_t)(WL::mbar_offset + 8 * (NW + warp)));    // counted on done[warp] of the owner
+                            st_async(fld[f][k] + p_own[i], v[i][f][k], fld[f][k] + (uint32_t)(WL::mbar_offset + 8 * (NW + cls)));    // counted on done[class] of the owner
                         else dsmem_st(fld[f][k] + p_own[i], v[i][f][k]);
                     }
                 }
@@ -353,7 +379,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
         const cplx<T>* tabHB = reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x];
         cplx<T>* SH = reinterpret_cast<cplx<T>*>(a.SH[x]) + off;
 
-        {
+        if (core) {
             const cplx<T>* __restrict__ g = cur;
 #pragma unroll 4
             for (int i = tid; i < S; i += NT) sm[phys<T>(i)] = g[i];
@@ -373,7 +399,9 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
             if constexpr (!DK0) {
                 if (q < total) { e0 = ldg(ph + 2 * s); e1 = ldg(ph + 2 * s + 1); e2 = ldg(ph + 2 * s + 2); }
             }
-            if (crossing && !resonant) {
+            if (!core) {
+                // a helper warp has no part in the linear core
+            } else if (crossing && !resonant) {
                 // fresh pump / frozen seed, already half-stepped: a thread sends the elements of its own pass-1
                 // butterfly, i.e. of its class, to the tiles' owners as an inverse pass 1 would
                 mbar_wait(mb + 8 * (NW + warp), (fz - 1) & 1);
@@ -391,9 +419,11 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
                 wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
             }
             if (q == total) break;
-            mbar_wait(mb + 8 * warp, fz & 1);                 // ready[warp]: the operands of my tiles are in my staging buffer
-            if (lane == 0) mbar_arm(mb + 8 * warp, ready_bytes);
-            tiles(tag_rk4{}, (1 << F) - 1, e0, e1, e2);
+            if (nt_own > 0) {
+                mbar_wait(my_ready, fz & 1);                  // the operands of my tiles are in my staging buffer
+                if (lane == 0) mbar_arm(my_ready, ready_bytes);
+                tiles(tag_rk4{}, (1 << F) - 1, e0, e1, e2);
+            }
             ++fz;
         }
         cluster_bar();                                    // every field is ready for its inverse pass 0
@@ -401,11 +431,13 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
         cluster_bar();
 
         if (!rt_mode) {
-            cplx<T>* __restrict__ g = cur;
+            if (core) {
+                cplx<T>* __restrict__ g = cur;
 #pragma unroll 4
-            for (int i = tid; i < S; i += NT) g[i] = sm[phys<T>(i)];
+                for (int i = tid; i < S; i += NT) g[i] = sm[phys<T>(i)];
+            }
         } else {
-            {   // fields at z = L of the last pass
+            if (core) {   // fields at z = L of the last pass
                 cplx<T>* __restrict__ g = reinterpret_cast<cplx<T>*>(a.exitb[x]) + off;
 #pragma unroll 4
                 for (int i = tid; i < S; i += NT) g[i] = sm[phys<T>(i)];
@@ -416,9 +448,10 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
             for (int f = 0; f < F; ++f)
                 if (a.resonant[f] && a.boundary_fft[f]) maskb |= 1 << f;
             if (maskb) {        // uniform over the cluster
+                cluster_bar();                            // nobody writes into a field whose owner still stores its exit copy
                 tiles(tag_fwd0{}, maskb, one, one, one);
                 cluster_bar();
-                if ((maskb >> x) & 1) {
+                if (core && ((maskb >> x) & 1)) {
                     const cplx<T>* tabGM = reinterpret_cast<const cplx<T>*>(a.tabGM[x]) + (size_t)b * a.tab_stride[x];
                     wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tabGM, j, tid, fb, nullptr);
                 }
@@ -426,7 +459,9 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NT, 1) k_wide(ResidentAr
                 tiles(tag_inv0{}, maskb, one, one, one);
                 cluster_bar();
             }
-            if (resonant) {
+            if (!core) {
+                // (helpers hold no field)
+            } else if (resonant) {
                 const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]);
                 cplx<T> mf = one;
                 if (!a.boundary_fft[x]) mf = ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b);
@@ -465,7 +500,7 @@ template <class T, int L, int F, bool DK0> cudaError_t wide_cfg(cudaLaunchConfig
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg->gridDim = dim3((unsigned)(n_clusters * WL::NCTA), 1, 1);
-    cfg->blockDim = dim3(WL::NT, 1, 1);
+    cfg->blockDim = dim3(WL::NTH, 1, 1);
     cfg->dynamicSmemBytes = WL::total;
     cfg->stream = s;
     cfg->attrs = attr;
@@ -484,7 +519,7 @@ template <class T, int L, int F> cudaError_t wide_info_LF(ResidentInfo* out) {
         int n = 0;
         e = cudaOccupancyMaxActiveClusters(&n, k_wide<T, L, F, false>, &cfg);
         if (e != cudaSuccess) return e;
-        out->threads = wide_layout<T, L, F>::NT;
+        out->threads = wide_layout<T, L, F>::NTH;
         out->smem_bytes = cfg.dynamicSmemBytes;
         out->max_clusters = n;
         return cudaSuccess;
