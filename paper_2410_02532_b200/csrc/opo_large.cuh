@@ -309,6 +309,15 @@ template <class T, int L, int F> struct LargeEngine {
     // The row pass begins with the grid barrier that separates it from the column pass before it: everything that does not
     // depend on the fields (multiplier table entries from L2, the row's twiddles) is requested BEFORE that barrier, so its
     // latency is spent while the CTA waits for the slowest column tile anyway.
+    // element x of a per-field array by a chain of selects: the arrays of RowOp stay in registers (indexed with a runtime x
+    // they went to local memory, and every row pass began with a chain of dependent local loads: 1.5 k cycles)
+    template <class A> static __device__ __forceinline__ A pick(const A* arr, int x) {
+        A v = arr[0];
+#pragma unroll
+        for (int f = 1; f < F; ++f) v = (x == f) ? arr[f] : v;
+        return v;
+    }
+
     __device__ __forceinline__ void row_pass(cplx<T>* const* data, const RowOp& op, int batch, const int* __restrict__ perm1,
                                              const int* __restrict__ perm2, unsigned long long* bar_ctr, unsigned long long& bar_target) {
         const int n_chunks = batch * F * C::CHUNKS_PER_FIELD;
@@ -324,22 +333,22 @@ template <class T, int L, int F> struct LargeEngine {
             const int rem = chunk % (F * C::CHUNKS_PER_FIELD);
             const int x = rem / C::CHUNKS_PER_FIELD;
             const int r = (rem % C::CHUNKS_PER_FIELD) * C::ROWS + team;
-            const int kind = op.kind[x];
+            const int kind = pick(op.kind, x);
             if (kind < 0) continue;                                 // uniform over the CTA
             const bool active = r < C::N1;
             const size_t off = (size_t)b * C::N + (size_t)(active ? r : 0) * C::N2;
-            cplx<T>* g = data[x] + off;
+            cplx<T>* g = pick(data, x) + off;
             if (kind == ROW_RELOAD) {
                 sync_once();
                 if (active) {
-                    const cplx<T>* __restrict__ a = op.aux[x] + off;
+                    const cplx<T>* __restrict__ a = pick(op.aux, x) + off;
 #pragma unroll 4
                     for (int i = lt; i < C::N2; i += C::TT2) g[i] = ldcg(a + i);
                 }
                 continue;
             }
             // this CTA's rows of this table are in shared memory (merged full step H2: every z-step but the ends of a pass)
-            const bool cached = kind == ROW_LINEAR && cache_src != nullptr && cache_src == (const void*)op.tab[x] && op.tab_stride[x] == 0;
+            const bool cached = kind == ROW_LINEAR && cache_src != nullptr && cache_src == (const void*)pick(op.tab, x) && pick(op.tab_stride, x) == 0;
             const int k1 = (cached && sizeof(T) == 4) ? 0 : __ldg(&perm1[active ? r : 0]);      // (the cached twiddles need no k1)
             // A row is one team's business from its first load to its last store: every barrier of the row pass is the
             // team's own (a __syncwarp, or a named barrier when the team has two warps), the teams of a CTA drift apart and
@@ -364,12 +373,12 @@ template <class T, int L, int F> struct LargeEngine {
                 fwd_pass_smem<T, C::L2, P2::P - 1, C::TT2, true>(smt, tw2, lt);
                 pass_sync<C::SY2>(1 + team);
                 if (active) {
-                    cplx<T>* o = op.out[x] + (size_t)b * C::N + k1;
+                    cplx<T>* o = pick(op.out, x) + (size_t)b * C::N + k1;
 #pragma unroll 4
                     for (int i = lt; i < C::N2; i += C::TT2) o[(size_t)__ldg(&perm2[i]) * C::N1] = smt[phys<T>(i)];
                 }
             } else {
-                const TAB* tab = op.tab[x] + (size_t)b * op.tab_stride[x] + (size_t)(active ? r : 0) * C::N2;
+                const TAB* tab = pick(op.tab, x) + (size_t)b * pick(op.tab_stride, x) + (size_t)(active ? r : 0) * C::N2;
                 TAB hh[NIT][RM];
                 cplx<T> w[CNT];
                 float wd[CNT];
@@ -424,7 +433,7 @@ template <class T, int L, int F> struct LargeEngine {
                 pass_sync<C::SY2>(1 + team);
                 OPO_TSTAMP(*this, 6);                       // row transforms (team 0)
                 if (active) {
-                    cplx<T>* sh = op.sh_store[x] ? op.sh_store[x] + off : nullptr;
+                    cplx<T>* sh = pick(op.sh_store, x) ? pick(op.sh_store, x) + off : nullptr;
 #pragma unroll
                     for (int j = 0; j < CNT; ++j) {
                         const int i = lt + j * C::TT2;
@@ -562,9 +571,9 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
     }
 
     e.template col_pass<COL_FWD>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
+    int s = rt_mode ? 0 : a.z0;        // index of the RK4 step that follows the operator q: q mod nz / z0 + q
 #pragma unroll 1
-    for (int q = 0; q <= total; ++q) {
-        const int s = rt_mode ? q % nz : a.z0 + q;
+    for (int q = 0; q <= total; ++q, s = (rt_mode && s + 1 == nz) ? 0 : s + 1) {
         const bool crossing = rt_mode && q > 0 && q < total && s == 0;
 #pragma unroll
         for (int x = 0; x < F; ++x) {

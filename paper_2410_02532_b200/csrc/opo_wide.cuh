@@ -144,7 +144,7 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
     const int warp = tid >> 5, lane = tid & 31;
     auto core_bar = [] { asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); };      // the core threads only (helper warps do not come here)
     if (fa.wait_in) {
-        mbar_wait(fa.mb + 8 * (NW + warp), fa.par_done);
+        mbar_wait_cta(fa.mb + 8 * (NW + warp), fa.par_done);      // (acquire at CTA scope: the bytes counted on the barrier are visible, and L1 is left alone)
         if (lane == 0) mbar_arm(fa.mb + 8 * (NW + warp), 16u * 32u * (uint32_t)sizeof(cplx<T>));       // the results of the next fused phase
     }
     fwd_bf<T, L, 1>(smv, twl, j * NT + tid);
@@ -404,7 +404,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
             } else if (crossing && !resonant) {
                 // fresh pump / frozen seed, already half-stepped: a thread sends the elements of its own pass-1
                 // butterfly, i.e. of its class, to the tiles' owners as an inverse pass 1 would
-                mbar_wait(mb + 8 * (NW + warp), (fz - 1) & 1);
+                mbar_wait_cta(mb + 8 * (NW + warp), (fz - 1) & 1);
                 if (lane == 0) mbar_arm(mb + 8 * (NW + warp), WL::done_bytes);
                 const cplx<T>* __restrict__ g = SH;
                 cplx<T> v[16];
@@ -420,7 +420,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
             }
             if (q == total) break;
             if (nt_own > 0) {
-                mbar_wait(my_ready, fz & 1);                  // the operands of my tiles are in my staging buffer
+                mbar_wait_cta(my_ready, fz & 1);                // the operands of my tiles are in my staging buffer
                 if (lane == 0) mbar_arm(my_ready, ready_bytes);
                 tiles(tag_rk4{}, (1 << F) - 1, e0, e1, e2);
             }
