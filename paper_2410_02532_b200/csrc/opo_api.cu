@@ -157,6 +157,7 @@ struct opo_handle {
     void* segHX[8][3] = {};                           //   H_j H_{j+1} / N across the junction of two crystals
     bool solo_ok = false;                             // solo engine (one CTA per instance, fields in shared + tensor memory)
     opo::ResidentInfo sinfo{};                        // max_clusters = co-resident CTAs on the device
+    int tab_cycle = 1;                                // roundings of H^2 cycled through by the on-chip engines (fp32: 16; build_tables)
     bool wide_ok = false;                             // wide engine (a cluster of 4 F CTAs per instance)
     opo::ResidentInfo winfo{};                        // max_clusters = co-resident clusters of 4 F CTAs
     int device = 0;
@@ -314,6 +315,24 @@ int build_tables(opo_handle* h) {
         for (int k = 0; k < N; ++k) M[k] = std::exp(Dx[k] * h0) * invN;                            // H^2 evaluated directly in fp64
         to_engine_layout(h, pl, M.data(), lay.data());
         if (int rc = upload_table(h, h->tabH2[x], lay.data(), N)) return rc;
+        if (h->tab_cycle > 1) {
+            // fp32, on-chip engines: a cycle of roundings of H^2 with error feedback.  One rounded table T = fl(M) puts the same
+            // 3e-8 of error per bin into every z-step (coherent: 3e4 z-steps of C4 turn it into ~5e-4).  Here table j of the
+            // cycle is T_j = fl(M / r_{j-1}), r_j = r_{j-1} T_j / M the relative error of the product applied so far, so after
+            // any number of z-steps the product of the tables is M^n to ONE rounding, and the drift per z-step falls by the
+            // cycle length.  Copy 0 is fl(M) itself (the host-sequenced baseline engines, which do not cycle, use it).
+            std::vector<cd> ratio(N, cd(1.0, 0.0));
+            for (int j = 0; j < h->tab_cycle; ++j) {
+                for (int k = 0; k < N; ++k) {
+                    const cd want = M[k] / ratio[k];
+                    const cd t((double)(float)want.real(), (double)(float)want.imag());
+                    Hh[k] = t;
+                    if (M[k] != cd(0.0, 0.0)) ratio[k] *= t / M[k];
+                }
+                to_engine_layout(h, pl, Hh.data(), lay.data());
+                if (int rc = upload_table(h, (char*)h->tabH2[x] + (size_t)j * N * h->tab_esz, lay.data(), N)) return rc;
+            }
+        }
         if (h->natH2[x]) if (int rc = upload_complex(h, h->natH2[x], M.data(), N)) return rc;
         if (K > 1) {
             // several crystals: per segment the half step, the full step and the junction H_j H_{j+1}
@@ -537,6 +556,7 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
     h->L1 = h->L / 2;
     h->L2 = h->L - h->L1;
     h->tab_esz = h->large ? 16 : h->esz;
+    h->tab_cycle = (!h->large && !h->dbl) ? 16 : 1;       // (a power of two: the kernels index with a mask)
     h->h = c->length_m / (double)g->nz_per_pass;
     h->sm_count = prop.multiProcessorCount;
     h->device = dev;
@@ -559,7 +579,8 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
             if (cudaMalloc(p, fb) != cudaSuccess) return bail(OPO_ERR_ALLOC, "cudaMalloc of field state failed");
             cudaMemset(*p, 0, fb);
         }
-        if (cudaMalloc(&h->tabH[x], (size_t)h->N * h->tab_esz) != cudaSuccess || cudaMalloc(&h->tabH2[x], (size_t)h->N * h->tab_esz) != cudaSuccess ||
+        if (cudaMalloc(&h->tabH[x], (size_t)h->N * h->tab_esz) != cudaSuccess ||
+            cudaMalloc(&h->tabH2[x], (size_t)h->tab_cycle * h->N * h->tab_esz) != cudaSuccess ||
             cudaMalloc(&h->mirror[x], (size_t)h->B * h->esz) != cudaSuccess)
             return bail(OPO_ERR_ALLOC, "cudaMalloc of tables failed");
     }
@@ -854,6 +875,7 @@ int resident_run(opo_handle* h, int mode, int z0, int steps) {
     a.tw = h->tw; a.phase = h->phase; a.phase_stride = phase_stride(h);
     a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
     a.mode = mode; a.z0 = z0; a.steps = steps; a.nln = h->splitting;
+    a.tab_cycle_mask = h->tab_cycle - 1;
     a.dk0 = !h->splitting;
     for (int b = 0; b < h->B; ++b) if (h->dk[b] != 0.0) a.dk0 = 0;
     const bool solo = engine_in_use(h) == OPO_ENGINE_SOLO, wide = engine_in_use(h) == OPO_ENGINE_WIDE;

@@ -74,7 +74,8 @@ struct ResidentArgs {
     void* exitb[3];        // exit fields (z = L of the last pass), written when write_exit
     void* SH[3];           // scratch [B][N]: IDFT(H DFT(S_x)) of non-resonant fields
     const void* tabH[3];   // half step            (shared)
-    const void* tabH2[3];  // merged full step     (shared)
+    const void* tabH2[3];  // merged full step     (shared): [tab_cycle_mask + 1][N], a cycle of roundings with error feedback
+                           //   (opo_api.cu build_tables); operator q of a call uses copy q & tab_cycle_mask
     const void* tabHB[3];  // H G m H merged across the boundary (resonant; maybe per instance)
     const void* tabGM[3];  // G m / N, un-merged boundary       (resonant; maybe per instance)
     const void* tabHG[3];  // H G m / N: last half-step + boundary, used when a modulator (eom) follows
@@ -91,6 +92,7 @@ struct ResidentArgs {
     double kappa[3];
     double h;
     int n_fields, batch, nz;   // nz = steps per pass
+    int tab_cycle_mask;    // see tabH2
     int mode;              // 0 = propagate `steps` z-steps from step index z0; 1 = `steps` round trips
     int split;             // 1 (mode 1 only): work is dealt to the clusters in round trips, not instances (opo_resident.cuh)
     int* flags;            // [B][F] round trips completed per (instance, field), zeroed before a split launch

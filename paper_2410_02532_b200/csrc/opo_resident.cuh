@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                     linear_core_smem<T, L, NT>(tabH, tid);
                 }
             } else {
-                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
+                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2 + (size_t)(q & a.tab_cycle_mask) * N);
                 if constexpr (FLOW) {
                     FlowArgs fa;
                     fa.mb = mb; fa.nf = F;

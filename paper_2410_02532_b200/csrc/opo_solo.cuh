@@ -407,7 +407,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                     const cplx<T>* tab = tabH;
                     if (q != 0 && q != total)
                         tab = crossing ? reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x]
-                                       : reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
+                                       : reinterpret_cast<const cplx<T>*>(a.tabH2[x]) + (size_t)(q & a.tab_cycle_mask) * N;
                     core(tab, !first_core, !last_core && !keep && !inj);
                 }
                 if (inj) {

@@ -412,7 +412,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 for (int k = 0; k < 16; ++k) v[k] = g[tid + NT * k];
                 wide_push16<T, NW, NCTA, WL::MAXT, WL::NQ>(v, fb, warp, lane);
             } else {
-                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2);
+                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2 + (size_t)(q & a.tab_cycle_mask) * N);
                 WideFlow fa = fb;
                 fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
                 fa.push_out = q < total;
