@@ -123,7 +123,7 @@ def _long_run(stem, w, engines):
 def test_config1_full_length_power_and_spectrum():
     torch, P = _gpu()
     w = W.config1()
-    res = _long_run("c1_1000rt", w, [P.ENGINE_RESIDENT, P.ENGINE_SOLO])
+    res = _long_run("c1_1000rt", w, [P.ENGINE_WIDE, P.ENGINE_RESIDENT, P.ENGINE_SOLO])      # wide is what AUTO picks for C1
     for e_p, e_s, e_d in res.values():
         assert e_p.max() <= 1e-3 and e_s.max() <= 1e-3
 
