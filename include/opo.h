@@ -96,7 +96,7 @@ typedef struct {
 
 /* grid: PAPER.md:L175-178 (dt = t_rt/n), L162 (nz), L193 (precision) */
 typedef struct {
-    int log2_n;        /* 6 .. 18 */
+    int log2_n;        /* 4 .. 18 */
     double window_s;   /* N dt, the round-trip window t_rt */
     int nz_per_pass;   /* z-steps per crystal pass; h = length_m / nz_per_pass */
     int precision;     /* OPO_PRECISION_C64 | OPO_PRECISION_C128 */

@@ -19,7 +19,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libopo.so")
 PLAIN_SOURCES = ["opo_api.cu", "opo_dispatch.cu", "opo_pointwise.cu", "opo_selftest.cu"]
 # (type, suffix, log2 N): one object per size-specialised instance of opo_inst.cu
-INSTANCES = [("float", "f32", l) for l in range(6, 15)] + [("double", "f64", l) for l in range(6, 14)]
+INSTANCES = [("float", "f32", l) for l in range(4, 15)] + [("double", "f64", l) for l in range(4, 14)]
 # wide engine (a cluster of 4 F CTAs per instance): the sizes whose plan is 4 . 16 . r . r'
 WIDE_INSTANCES = [("float", "f32", l) for l in range(12, 15)] + [("double", "f64", l) for l in range(12, 14)]
 LARGE_INSTANCES = [("float", "f32", l) for l in range(15, 19)] + [("double", "f64", l) for l in range(14, 19)]

@@ -536,7 +536,7 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
     }
     const int maxL = (g->precision == OPO_PRECISION_C64) ? opo::kMaxLog2Smem : opo::kMaxLog2Smem - 1;
     if (g->log2_n < opo::kMinLog2 || g->log2_n > opo::kMaxLog2)
-        return fail(nullptr, OPO_ERR_UNSUPPORTED, "grid size not supported (2^6 .. 2^18)");
+        return fail(nullptr, OPO_ERR_UNSUPPORTED, "grid size not supported (2^4 .. 2^18)");
     if (f->resonant[0] && g->log2_n > maxL)
         return fail(nullptr, OPO_ERR_UNSUPPORTED, "resonant pump: not on the large-N engine (N > 2^14, c128: > 2^13)");
 

@@ -20,7 +20,7 @@ namespace opo {
     cudaError_t launch_wide_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
 
 #define OPO_DECL_ALL(SUF) \
-    OPO_DECL(SUF, 6) OPO_DECL(SUF, 7) OPO_DECL(SUF, 8) OPO_DECL(SUF, 9) OPO_DECL(SUF, 10) OPO_DECL(SUF, 11) \
+    OPO_DECL(SUF, 4) OPO_DECL(SUF, 5) OPO_DECL(SUF, 6) OPO_DECL(SUF, 7) OPO_DECL(SUF, 8) OPO_DECL(SUF, 9) OPO_DECL(SUF, 10) OPO_DECL(SUF, 11) \
     OPO_DECL(SUF, 12) OPO_DECL(SUF, 13) OPO_DECL(SUF, 14)
 
 OPO_DECL_ALL(f32)
@@ -37,6 +37,7 @@ OPO_DECL_LARGE(f64, 14) OPO_DECL_LARGE(f64, 15) OPO_DECL_LARGE(f64, 16) OPO_DECL
 
 #define OPO_SWITCH(FN, SUF, log2n, ...)                                                            \
     switch (log2n) {                                                                               \
+        OPO_CASE(FN, SUF, 4, __VA_ARGS__) OPO_CASE(FN, SUF, 5, __VA_ARGS__)                                      \
         OPO_CASE(FN, SUF, 6, __VA_ARGS__) OPO_CASE(FN, SUF, 7, __VA_ARGS__) OPO_CASE(FN, SUF, 8, __VA_ARGS__)    \
         OPO_CASE(FN, SUF, 9, __VA_ARGS__) OPO_CASE(FN, SUF, 10, __VA_ARGS__) OPO_CASE(FN, SUF, 11, __VA_ARGS__)  \
         OPO_CASE(FN, SUF, 12, __VA_ARGS__) OPO_CASE(FN, SUF, 13, __VA_ARGS__) OPO_CASE(FN, SUF, 14, __VA_ARGS__) \

@@ -265,7 +265,7 @@ template <class T> struct dit_inv<T, 1> { static __device__ __forceinline__ void
 // radix-16 passes (as many as possible) then 8 / 4, never radix 2:
 //   (L-2)%4 == 0: 16..16 | 1: 16..16,8,4 | 2: 16..16,4 | 3: 16..16,8
 template <int L> struct plan {
-    static_assert(L >= 6 && L <= 14, "shared-memory FFT supports 2^6 .. 2^14");
+    static_assert(L >= 4 && L <= 14, "shared-memory FFT supports 2^4 .. 2^14");
     static constexpr int L1 = L - 2;
     static constexpr int rem = L1 % 4;
     static constexpr int n16 = (rem == 1) ? (L1 / 4 - 1) : (L1 / 4);

@@ -6,7 +6,7 @@
 
 namespace opo {
 
-constexpr int kMinLog2 = 6;
+constexpr int kMinLog2 = 4;
 constexpr int kMaxLog2Smem = 14;   // one field in one SM's shared memory (fp32); fp64: 13
 constexpr int kMaxLog2 = 18;       // large-N engine above kMaxLog2Smem
 

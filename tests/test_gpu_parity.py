@@ -135,7 +135,7 @@ def assert_close(got, ref, tol, what):
 # ---------------------------------------------------------------------------------------------------------
 # FFT read-out: opo_get_fields(FREQ) against the oracle's own transform, every supported size
 # ---------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("precision,log2_n", [("c64", l) for l in range(6, 15)] + [("c128", l) for l in range(6, 14)])
+@pytest.mark.parametrize("precision,log2_n", [("c64", l) for l in range(4, 15)] + [("c128", l) for l in range(4, 14)])
 def test_frequency_readout_matches_oracle_fft(precision, log2_n):
     import oracle
     torch, P = _gpu()
@@ -153,6 +153,7 @@ def test_frequency_readout_matches_oracle_fft(precision, log2_n):
 # ---------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("engine_idx", ENGINE_IDX)
 @pytest.mark.parametrize("precision,log2_n,n_fields", [
+    ("c128", 4, 3), ("c128", 5, 2), ("c64", 4, 2), ("c64", 5, 3),          # the smallest grids of the ABI: N = 16, 32
     ("c128", 6, 2), ("c128", 7, 3), ("c128", 9, 3), ("c128", 10, 2), ("c128", 11, 3), ("c128", 13, 3),
     ("c64", 6, 3), ("c64", 8, 2), ("c64", 9, 3), ("c64", 10, 3), ("c64", 11, 2), ("c64", 12, 3), ("c64", 13, 3),
     ("c64", 14, 3), ("c64", 14, 2)])
@@ -182,7 +183,7 @@ def test_partial_passes_continue_dk_phase(engine_idx):
 # ---------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("engine_idx", ENGINE_IDX)
 @pytest.mark.parametrize("precision,log2_n,n_fields,calls", [
-    ("c128", 8, 3, 1), ("c128", 8, 3, 3), ("c128", 10, 2, 1), ("c64", 11, 3, 1), ("c64", 12, 2, 3)])
+    ("c128", 4, 3, 1), ("c64", 5, 2, 3), ("c128", 8, 3, 1), ("c128", 8, 3, 3), ("c128", 10, 2, 1), ("c64", 11, 3, 1), ("c64", 12, 2, 3)])
 def test_roundtrips_with_boundary(precision, log2_n, n_fields, calls, engine_idx):
     engine = engines()[engine_idx]
     torch, P = _gpu()
@@ -922,6 +923,13 @@ def test_abi_errors_and_state():
         bad.resonant = [1, 1]               # a resonant pump is not available on the large-N engine
         P.from_workload(bad)
     assert e.value.status == P.ERR_UNSUPPORTED
+    for bad_log2 in (3, 19):                 # N outside [2^4, 2^18]
+        with pytest.raises(P.OpoError) as e:
+            P.Opo(n_fields=2, log2_n=bad_log2, window_s=1e-11, nz_per_pass=4, length_m=5e-3, dk_per_m=0.0, d_eff_m_per_V=14e-12,
+                  lambda_m=[532e-9, 1064e-9], n_index=[2.23, 2.16], beta1_s_per_m=[0.0, 0.0], beta2_s2_per_m=[0.0, 0.0],
+                  alpha_per_m=[0.0, 0.0], ref_field=1, resonant=[0, 1], R=[0.0, 0.9], delta_rad=[0.0, 0.0], delta_T_s=[0.0, 0.0],
+                  gdd_s2=[0.0, 0.0])
+        assert e.value.status == P.ERR_INVALID_ARG
     with pytest.raises(P.OpoError) as e:
         bad = small_workload(8, 2, "c64")
         bad.R = [0.0, 1.5]
