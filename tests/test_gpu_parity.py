@@ -313,6 +313,26 @@ def test_wide_engine_roundtrips_with_boundary(precision, log2_n, n_fields, calls
     assert_close(ex, ex2, 1e-12 if precision == "c128" else 1e-5, "wide vs cluster engine")
 
 
+@pytest.mark.parametrize("precision,log2_n,n_fields,batch", [("c64", 12, 3, 61), ("c64", 13, 2, 45), ("c64", 14, 3, 15), ("c128", 12, 3, 23)])
+def test_wide_engine_many_instances_bitwise_repeatable(precision, log2_n, n_fields, batch):
+    """Several instances per cluster, several round trips per instance, every cluster of the GPU busy: two runs must agree bit
+    for bit (every value crosses the SM-to-SM network asynchronously: a missing wait would show as a difference between runs),
+    and with the cluster engine to rounding."""
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=5, batch=batch, dk=15.0, gdd_dt2=-0.9, drad=0.2, strong=False)
+    w.delta_T_signal_s = (np.arange(batch) % 7 - 3.0) * 0.75 * w.dt
+    if n_fields == 3:
+        w.resonant = [0, 1, 0]
+    _engine_or_skip(w, P.ENGINE_WIDE)
+    runs = [run_gpu(w, P.ENGINE_WIDE, n_roundtrips=6, calls=2) for _ in range(3)]
+    for cur, ex, eng in runs[1:]:
+        assert eng == P.ENGINE_WIDE
+        assert np.array_equal(cur, runs[0][0]) and np.array_equal(ex, runs[0][1])
+    cur2, ex2, _ = run_gpu(w, P.ENGINE_RESIDENT, n_roundtrips=6, calls=2)
+    assert_close(runs[0][1], ex2, 1e-12 if precision == "c128" else 1e-5, "wide vs cluster engine, exit")
+    assert_close(runs[0][0], cur2, 1e-12 if precision == "c128" else 1e-5, "wide vs cluster engine, current")
+
+
 def test_wide_engine_is_what_auto_picks_for_a_single_instance_and_falls_back():
     torch, P = _gpu()
     w = W.config1().truncated(1)
