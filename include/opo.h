@@ -176,7 +176,8 @@ int opo_roundtrips(opo_handle* h, int n);
  *   dev_pump_train: [n][N] (per_instance = 0, every instance sees the same train) or [n][batch][N], time domain;
  *   dev_out_train : NULL, or [n][batch][N]: exit field `out_field` (z = L, before the mirror) of every round trip.
  * Equivalent to n x { opo_set_pump(slice m); opo_roundtrips(1); copy of OPO_WHICH_EXIT } with everything staying
- * on the device and on the handle's stream.  Afterwards the stored pump input is the last slice.
+ * on the device and on the handle's stream (the SOLO engine does the whole train in one launch, reading the slices and
+ * writing the exit fields at the round-trip crossings inside the kernel).  Afterwards the stored pump input is the last slice.
  * OPO_ERR_UNSUPPORTED for a resonant pump, OPO_ERR_STATE unless z = 0. */
 int opo_roundtrips_train(opo_handle* h, int n, const void* dev_pump_train, int per_instance, void* dev_out_train, int out_field);
 

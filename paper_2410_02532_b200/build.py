@@ -72,6 +72,8 @@ def _jobs(only=None):
         # the solo engine (one CTA per instance, fields in shared + tensor memory): general and dk = 0 instantiations
         jobs.append(("opo_inst_solo.cu", f"opo_inst_solo_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}"]))
         jobs.append(("opo_inst_solo.cu", f"opo_inst_solo_dk0_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_DK0"]))
+        # ... and its pump-train instantiation (slices in, exit fields out at the round-trip crossings inside the launch)
+        jobs.append(("opo_inst_solo.cu", f"opo_inst_solo_train_{suf}_L{l}.o", [f"-DOPO_T={typ}", f"-DOPO_SUFFIX={suf}", f"-DOPO_L={l}", "-DOPO_TRAIN"]))
     for typ, suf, l in WIDE_INSTANCES:
         if only and f"{suf}:{l}" not in only:
             continue

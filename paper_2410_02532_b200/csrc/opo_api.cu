@@ -859,8 +859,23 @@ int apply_eom(opo_handle* h) {
 }
 
 // ---- resident engine ---------------------------------------------------------------------------------------------
-int resident_run(opo_handle* h, int mode, int z0, int steps) {
+// pump train handled inside the launch (solo engine): slices in, exit fields of `out_field` out
+struct TrainArgs {
+    const void* pump = nullptr;
+    bool per_instance = false;
+    void* out = nullptr;
+    int out_field = 0;
+};
+
+int resident_run(opo_handle* h, int mode, int z0, int steps, const TrainArgs* train = nullptr) {
     opo::ResidentArgs a{};
+    if (train) {
+        a.train = train->pump;
+        a.train_stride = (long long)h->N * (train->per_instance ? h->B : 1);
+        a.train_inst_stride = train->per_instance ? h->N : 0;
+        a.out_train = train->out;
+        a.out_field = train->out_field;
+    }
     for (int x = 0; x < h->F; ++x) {
         a.cur[x] = h->cur[x]; a.S[x] = h->S[x]; a.exitb[x] = h->exitb[x]; a.SH[x] = h->SH[x];
         a.tabH[x] = h->tabH[x]; a.tabH2[x] = h->tabH2[x]; a.tabHB[x] = h->tabHB[x]; a.tabGM[x] = h->tabGM[x]; a.tabHG[x] = h->tabHG[x];
@@ -1098,6 +1113,15 @@ int opo_roundtrips_train(opo_handle* h, int n, const void* dev_pump_train, int p
     if (h->fields.resonant[0]) return fail(h, OPO_ERR_UNSUPPORTED, "a pump train needs a single-pass (non-resonant) pump");
     if (h->z_steps != 0) return fail(h, OPO_ERR_STATE, "roundtrips requires z = 0");
     const size_t slice = (size_t)h->N * h->esz * (per_instance ? (size_t)h->B : 1);
+    if (n > 0 && engine_in_use(h) == OPO_ENGINE_SOLO && !h->splitting && !any_eom(h)) {
+        // one launch for the whole train: the kernel reads slice m at the crossing into round trip m and writes the exit field
+        // of every round trip (opo_solo.cuh, TRAIN); the stored pump input ends up as the last slice, as in the loop below
+        if (int rc = set_pump_impl(h, (const char*)dev_pump_train + (size_t)(n - 1) * slice, per_instance, cudaMemcpyDeviceToDevice)) return rc;
+        if (int rc = ensure_tables(h)) return rc;
+        TrainArgs t;
+        t.pump = dev_pump_train; t.per_instance = per_instance != 0; t.out = dev_out_train; t.out_field = dev_out_train ? out_field : 0;
+        return resident_run(h, 1, 0, n, &t);
+    }
     for (int m = 0; m < n; ++m) {
         // ReadPump: the m-th slice of the long pump vector becomes the intracavity pump
         if (int rc = set_pump_impl(h, (const char*)dev_pump_train + (size_t)m * slice, per_instance, cudaMemcpyDeviceToDevice)) return rc;

@@ -15,6 +15,7 @@ namespace opo {
     cudaError_t solo_info_##SUF##_L##LL(int, ResidentInfo*) __attribute__((weak));                            \
     cudaError_t launch_solo_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));      \
     cudaError_t launch_solo_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak)); \
+    cudaError_t launch_solo_train_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak)); \
     cudaError_t wide_info_##SUF##_L##LL(int, ResidentInfo*) __attribute__((weak));                            \
     cudaError_t launch_wide_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));      \
     cudaError_t launch_wide_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
@@ -55,6 +56,7 @@ OPO_DECL_LARGE(f64, 14) OPO_DECL_LARGE(f64, 15) OPO_DECL_LARGE(f64, 16) OPO_DECL
     }                                                                                                             \
     cudaError_t solo_info_##SUF(int log2n, int n_fields, ResidentInfo* out) { OPO_SWITCH(solo_info_, SUF, log2n, n_fields, out) } \
     cudaError_t launch_solo_##SUF(int log2n, const ResidentArgs& a, int n_ctas, cudaStream_t s) {                 \
+        if (a.train) { OPO_SWITCH(launch_solo_train_, SUF, log2n, a, n_ctas, s) }                                 \
         if (a.dk0) { OPO_SWITCH(launch_solo_dk0_, SUF, log2n, a, n_ctas, s) }                                     \
         OPO_SWITCH(launch_solo_, SUF, log2n, a, n_ctas, s)                                                        \
     }                                                                                                             \

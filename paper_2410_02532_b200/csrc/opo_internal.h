@@ -96,6 +96,13 @@ struct ResidentArgs {
     int mode;              // 0 = propagate `steps` z-steps from step index z0; 1 = `steps` round trips
     int split;             // 1 (mode 1 only): work is dealt to the clusters in round trips, not instances (opo_resident.cuh)
     int* flags;            // [B][F] round trips completed per (instance, field), zeroed before a split launch
+    // pump train inside the launch (solo engine, mode 1): round trip r of the call is pumped by
+    // slice r, and the exit field `out_field` of round trip r goes to out_train[r]
+    const void* train;     // [steps][N] (train_inst_stride = 0) or [steps][B][N] (train_inst_stride = N); null: no train
+    long long train_stride;        // elements between slices
+    long long train_inst_stride;
+    void* out_train;       // [steps][B][N] or null
+    int out_field;
     int dk0;               // 1: dk = 0 for every instance (and nln = 0): the kernel variant without stage phases
     int nln;               // 1: order N/2 - L - N/2 (Eq. 10-11); phase table then has stride 4 nz + 1 (steps of h/4)
                            //    and mode 1 takes steps = 1

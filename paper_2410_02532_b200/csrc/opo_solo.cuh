@@ -108,7 +108,11 @@ template <class T, int L, int F> struct solo_layout {
     static constexpr int ctas_per_sm = ctas_per_sm_raw < 1 ? 1 : (ctas_per_sm_raw > 4 ? 4 : ctas_per_sm_raw);
 };
 
-template <class T, int L, int F, bool DK0 = false>
+// TRAIN: the pump-train instantiation (nanosecond regime; objects of its own so that the default
+// kernel's code is untouched): at every round-trip crossing the pump is the next slice of a long pump vector (loaded in the
+// time domain, forward pass 0 and its first half-step follow), and the field `out_field` is taken out at z = L -- last
+// half-step, inverse pass 0, store, then the boundary and the next half-step as one operator -- instead of crossing merged.
+template <class T, int L, int F, bool DK0 = false, bool TRAIN = false>
 __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>::ctas_per_sm) k_solo(ResidentArgs a) {
     constexpr int N = 1 << L, NT = cta_threads<T, L>::value;
     using PL = plan<L>;
@@ -357,7 +361,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
         for (int xi = 0; xi < F; ++xi) {
             const int x = (xi + 1) % F;         // 1, 2, .., F-1, 0: field 0 stays in shared memory
             const cplx<T>* cur = reinterpret_cast<const cplx<T>*>(a.cur[x]) + (size_t)b * N;
-            if (a.split && rt0 > 0) {
+            if (TRAIN && x == 0) {              // ReadPump: the slice of this piece's first round trip
+                load(reinterpret_cast<const cplx<T>*>(a.train) + (size_t)rt0 * a.train_stride + (size_t)b * a.train_inst_stride);
+            } else if (a.split && rt0 > 0) {
 #pragma unroll 4
                 for (int i = tid; i < N; i += NT) sm[phys<T>(i)] = ldcg_c(cur + i);
             } else {
@@ -378,13 +384,41 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
 #pragma unroll
             for (int x = 0; x < F; ++x) {
                 const bool resonant = a.resonant[x] != 0;
-                const bool keep = rt_mode && q == 0 && !resonant && steps_l > 1;     // SH <- first half-stepped input
+                const bool keep = rt_mode && q == 0 && !resonant && steps_l > 1 && !(TRAIN && x == 0);     // SH <- first half-stepped input
                 const bool first_core = q == 0 && x == 0;                             // no transition precedes
                 const bool last_core = q == total && x == F - 1;                      // no transition follows
                 const bool inj = x == 0 && crossing && inj_any;                       // input coupler of a resonant pump
                 const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
                 cplx<T>* SH = reinterpret_cast<cplx<T>*>(a.SH[x]) + (size_t)b * N;
-                if (crossing && !resonant) {
+                const int rt_done = rt0 + q / (nz > 0 ? nz : 1);      // round trips of the instance completed at a crossing
+                if (TRAIN && crossing && (x == 0 || (x == a.out_field && a.out_train != nullptr))) {
+                    if (x == a.out_field && a.out_train != nullptr) {
+                        // SaveRoundTrip: the field at z = L of the round trip just finished, before the mirror
+                        core(tabH, true, false);
+                        __syncthreads();
+                        pass0_local<T, L, NT>(tw, tid, true);
+                        __syncthreads();
+                        cplx<T>* __restrict__ o = reinterpret_cast<cplx<T>*>(a.out_train) + ((size_t)(rt_done - 1) * a.batch + b) * N;
+                        const cplx<T> mf = (resonant && !a.boundary_fft[x]) ? ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b) : cplx<T>{(T)1, (T)0};
+#pragma unroll 4
+                        for (int i = tid; i < N; i += NT) { const cplx<T> v = sm[phys<T>(i)]; o[i] = v; sm[phys<T>(i)] = cmul(v, mf); }
+                        __syncthreads();
+                    } else {
+                        if constexpr (FLOW) { flow_wait_done_all((fz - 1) & 1); }
+                        __syncthreads();
+                    }
+                    if (x == 0) {                    // ReadPump: the slice of the round trip that begins (the pump is single-pass)
+                        load(reinterpret_cast<const cplx<T>*>(a.train) + (size_t)rt_done * a.train_stride + (size_t)b * a.train_inst_stride);
+                        __syncthreads();
+                    } else if (!resonant) {          // a non-resonant field restarts from its stored input (R12)
+                        load(reinterpret_cast<const cplx<T>*>(a.S[x]) + (size_t)b * N);
+                        __syncthreads();
+                    }
+                    pass0_local<T, L, NT>(tw, tid, false);
+                    __syncthreads();
+                    // the boundary (spectral phase and mirror: G m, or the mirror alone, applied above) and the first half-step
+                    core((resonant && a.boundary_fft[x]) ? reinterpret_cast<const cplx<T>*>(a.tabHG[x]) + (size_t)b * a.tab_stride[x] : tabH, false, true);
+                } else if (crossing && !resonant) {
                     if constexpr (FLOW) { flow_wait_done_all((fz - 1) & 1); __syncthreads(); }
                     load(SH);                                        // fresh pump / frozen seed, already half-stepped
                     if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }
@@ -447,6 +481,8 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                 store(cur);
             } else {
                 store(reinterpret_cast<cplx<T>*>(a.exitb[x]) + (size_t)b * N);     // fields at z = L of the last pass
+                if (TRAIN && x == a.out_field && a.out_train != nullptr)
+                    store(reinterpret_cast<cplx<T>*>(a.out_train) + ((size_t)(rt0 + steps_l - 1) * a.batch + b) * N);
                 if (a.resonant[x]) {
                     // mirror, spectral phase and phase modulator of the last round trip of the call
                     const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]);
@@ -497,9 +533,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
     if (warp == 0) tmem_dealloc(tmem_base, SO::cols_alloc);
 }
 
-template <class T, int L, int F, bool DK0> cudaError_t solo_setup() {
+template <class T, int L, int F, bool DK0, bool TRAIN = false> cudaError_t solo_setup() {
     static device_once once;
-    return once.run([&] { return cudaFuncSetAttribute(k_solo<T, L, F, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)solo_layout<T, L, F>::total); });
+    return once.run([&] { return cudaFuncSetAttribute(k_solo<T, L, F, DK0, TRAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)solo_layout<T, L, F>::total); });
 }
 
 template <class T, int L, int F> cudaError_t solo_info_LF(ResidentInfo* out) {
@@ -527,12 +563,12 @@ template <class T, int L> cudaError_t solo_info_L(int n_fields, ResidentInfo* ou
     return n_fields == 3 ? solo_info_LF<T, L, 3>(out) : solo_info_LF<T, L, 2>(out);
 }
 
-template <class T, int L, int F, bool DK0> cudaError_t launch_solo_LF(const ResidentArgs& a, int n_ctas, cudaStream_t s) {
+template <class T, int L, int F, bool DK0, bool TRAIN = false> cudaError_t launch_solo_LF(const ResidentArgs& a, int n_ctas, cudaStream_t s) {
     using SO = solo_layout<T, L, F>;
     if constexpr (!SO::fits) {
         return cudaErrorNotSupported;
     } else {
-        cudaError_t e = solo_setup<T, L, F, DK0>();
+        cudaError_t e = solo_setup<T, L, F, DK0, TRAIN>();
         if (e != cudaSuccess) return e;
         cudaLaunchConfig_t cfg{};
         cudaLaunchAttribute attr[1];
@@ -544,11 +580,11 @@ template <class T, int L, int F, bool DK0> cudaError_t launch_solo_LF(const Resi
         cfg.stream = s;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, k_solo<T, L, F, DK0>, a);
+        return cudaLaunchKernelEx(&cfg, k_solo<T, L, F, DK0, TRAIN>, a);
     }
 }
-template <class T, int L, bool DK0> cudaError_t launch_solo_L(const ResidentArgs& a, int n_ctas, cudaStream_t s) {
-    return a.n_fields == 3 ? launch_solo_LF<T, L, 3, DK0>(a, n_ctas, s) : launch_solo_LF<T, L, 2, DK0>(a, n_ctas, s);
+template <class T, int L, bool DK0, bool TRAIN = false> cudaError_t launch_solo_L(const ResidentArgs& a, int n_ctas, cudaStream_t s) {
+    return a.n_fields == 3 ? launch_solo_LF<T, L, 3, DK0, TRAIN>(a, n_ctas, s) : launch_solo_LF<T, L, 2, DK0, TRAIN>(a, n_ctas, s);
 }
 
 }  // namespace opo

@@ -813,6 +813,55 @@ def test_pump_train_matches_oracle_loop(precision, log2_n, n_fields, engine_idx)
     assert rel_l2(got_cur[0, 0], train[-1]) == 0.0
 
 
+@pytest.mark.parametrize("precision,log2_n,n_fields,batch,out_field,idler_resonant,gdd", [
+    ("c64", 10, 3, 331, 1, False, 0.5),       # more instances than CTAs and not a multiple: round trips dealt to the CTAs, slices by absolute index
+    ("c64", 11, 3, 5, 2, False, 0.0),         # the recorded field is the non-resonant idler; mirror without a transform
+    ("c128", 10, 2, 3, 0, False, 0.5),        # the recorded field is the pump itself
+    ("c64", 12, 3, 4, 1, True, 0.0)])
+def test_pump_train_inside_the_solo_launch(precision, log2_n, n_fields, batch, out_field, idler_resonant, gdd):
+    """The solo engine takes the whole train in ONE launch (slices read and exit fields written at the round-trip crossings
+    inside the kernel), with a per-instance train.  Reference: the host-sequenced streaming engine driven slice by slice
+    (itself checked against the oracle loop above), and the oracle loop on sampled instances."""
+    import oracle
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=4, batch=batch, dk=9.0, gdd_dt2=gdd, drad=0.2, strong=False)
+    if n_fields == 3:
+        w.resonant = [0, 1, 1 if idler_resonant else 0]
+    _engine_or_skip(w, P.ENGINE_SOLO)
+    n_rt, n = 5, w.n
+    g = np.arange(n_rt * n) / (n_rt * n) - 0.5
+    env = np.exp(-(g / 0.22) ** 2) * np.exp(1j * 2.0 * g)
+    a_p = np.abs(w.pump[0]).max()
+    base = (a_p * env).reshape(n_rt, 1, n)
+    train = W._round_to_precision(base * (1.0 + 0.05 * (np.arange(batch) % 9))[None, :, None], precision)      # [n_rt][B][N]
+    res = {}
+    for engine in (P.ENGINE_SOLO, P.ENGINE_STREAMING):
+        o = P.from_workload(w, engine=engine)
+        l0 = o.launches
+        out = o.roundtrips_train(torch.from_numpy(train).to(o.dtype).cuda(), out_field=out_field)
+        o.sync()
+        res[engine] = (out.cpu().numpy().astype(np.complex128),
+                       np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1),
+                       np.stack([o.get_fields(x, P.WHICH_EXIT).cpu().numpy().astype(np.complex128) for x in range(w.n_fields)], axis=1),
+                       o.launches - l0)
+        o.close()
+    assert res[P.ENGINE_SOLO][3] <= 3, "the solo engine runs the train in one kernel launch (plus the pump broadcast)"
+    tol = 1e-12 if precision == "c128" else 2e-5
+    for k, what in ((0, "train of exit fields"), (1, "current"), (2, "exit")):
+        a, bb = res[P.ENGINE_SOLO][k], res[P.ENGINE_STREAMING][k]
+        assert np.isfinite(a).all()
+        flat_a, flat_b = a.reshape(-1, n), bb.reshape(-1, n)
+        worst = max(rel_l2(flat_a[i], flat_b[i]) for i in range(flat_a.shape[0]) if np.linalg.norm(flat_b[i]) > 0)
+        assert worst <= tol, (what, worst)
+    for b in sorted({0, batch // 2, batch - 1}):
+        ro = oracle.from_workload(w, b)
+        for m in range(n_rt):
+            ro.set_field(0, train[m, b])
+            assert ro.roundtrips(1) == 0
+            assert rel_l2(res[P.ENGINE_SOLO][0][m, b], ro.get_field(out_field, oracle.EXIT)) <= TOL[precision]
+    assert np.array_equal(res[P.ENGINE_SOLO][1][:, 0], train[-1].astype(np.complex128))      # the pump is re-injected from the last slice
+
+
 # ---------------------------------------------------------------------------------------------------------
 # third-order dispersion (PAPER.md:L99 Eq. 5 in the reading R7; SURVEY 8(f) N2): tables only
 # ---------------------------------------------------------------------------------------------------------
