@@ -10,6 +10,8 @@ changed input recipe cannot silently be compared against stale values.
 Files (numpy .npz, under tests/golden/):
   c3_20rt_<hash>.npz          C3 (N = 2^18, nz = 500), exit pump and signal after 20 round trips, complex64
                               (the rounding of the stored value, 6e-8, is far below the 1e-4 tolerance)
+  c3s_20rt_<hash>.npz         C3 on N = 2^15 (the smallest grid of the large-N engine), 20 round trips = 10^4 z-steps: exit
+                              fields of the fp64 oracle and (pin P12) the field error of the oracle run in `float`
   c1_1000rt_<hash>.npz        long noise-seeded runs (BASELINE.json north_star: <= 1e-3 on output signal power and on
   c2_500rt_<hash>.npz         the power spectrum, not phase; reading R21): per instance the output signal power
   c4_300rt_sub16_<hash>.npz   (1 - R_s) mean|exit_s|^2 (R16), the pump depletion 1 - mean|exit_p|^2 / mean|S_p|^2, the
@@ -76,7 +78,7 @@ def summarise(w, ex):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--only", default="C3,C4,C1,C2")
+    ap.add_argument("--only", default="C3,C3s,C4,C1,C2")
     ap.add_argument("--threads", type=int, default=os.cpu_count() or 1)
     ap.add_argument("--no-float", action="store_true", help="skip the float instantiation of the oracle (pin P12)")
     args = ap.parse_args()
@@ -91,6 +93,19 @@ def main():
         np.savez_compressed(os.path.join(HERE, name), exit_pump=res["exit"][0, 0].astype(np.complex64),
                             exit_signal=res["exit"][0, 1].astype(np.complex64), n_roundtrips=20)
         print(f"{name}: {time.time() - t0:.0f} s", flush=True)
+    if "C3s" in only:
+        w = W.config3(20, 15)
+        name = f"c3s_20rt_{workload_hash(w)}.npz"
+        t0 = time.time()
+        res = oracle.run_workload(w, threads=1)
+        out = {"exit_pump": res["exit"][0, 0].astype(np.complex64), "exit_signal": res["exit"][0, 1].astype(np.complex64), "n_roundtrips": 20}
+        if not args.no_float:
+            resf = oracle.run_workload(w, threads=1, use_float=True)
+            fe = [float(np.linalg.norm(resf["exit"][0, x] - res["exit"][0, x]) / np.linalg.norm(res["exit"][0, x])) for x in range(2)]
+            out["float_field_rel_l2"] = np.array(fe)
+            report["C3s"] = {"p12_float_vs_fp64_field_rel_l2_pump": fe[0], "p12_float_vs_fp64_field_rel_l2_signal": fe[1]}
+        np.savez_compressed(os.path.join(HERE, name), **out)
+        print(f"{name}: {time.time() - t0:.0f} s {json.dumps(report.get('C3s', {}))}", flush=True)
     for key, (stem, w) in long_run_workloads().items():
         if key not in only:
             continue
