@@ -14,8 +14,8 @@
 //           radix-16 butterfly per thread and pass (N = 2^14: 256 threads).
 //   fused : inverse pass 0 -> RK4 of the coupling terms -> forward pass 0, on registers.  The
 //           butterfly t needs element t of all four sub-blocks of all F fields: 4 F CTAs.  The S butterflies are dealt
-//           to the warps of the cluster in tiles of 32; a thread reads its 4 F values through distributed shared memory
-//           (one of them is local), integrates, and writes them back to their owners.
+//           to the warps of the cluster in tiles of 32; a thread finds the 4 F operands of its butterfly in its warp's
+//           staging buffer (see "push"), integrates, and sends the 4 F results to the CTAs that own them.
 //   sync  : no cluster-wide barrier inside the z-step loop.  The pass-1 butterfly t' touches the elements t' + (S/16) k,
 //           so the tiles of class c = (tile mod S/512) depend exactly on the pass-1 butterflies of warp c of every CTA, and
 //           vice versa: warp c of each of the 4 F CTAs forms a ring of its own.  The 16 tiles of a class are dealt to the 4 F
@@ -28,7 +28,10 @@
 //           operands per butterfly from LOCAL shared memory, integrates, and sends every result to its owner's field, where
 //           the forward pass 1 waits on done[c] the same way.  No remote load, no release fence and no arrival message is
 //           ever waited for: a z-step was 7.2 us with remote loads + release/acquire arrivals (the top stalls were the
-//           long scoreboard of the remote loads and the membar of the releases).
+//           long scoreboard of the remote loads and the membar of the releases), 5.5 us this way.  The waits acquire at CTA
+//           scope: the bytes counted on a barrier are visible to its waiter, and a cluster-scope acquire would make
+//           ptxas invalidate L1 (CCTL.IVALL) at every wait.  The pass-0 phases at the two ends of a call (no RK4) read
+//           and write the fields in place through ld / st.shared::cluster between cluster barriers.
 //
 // Everything else (merged tables H, H2, HB = H2 G m across the cavity boundary; stored
 // inputs SH of non-resonant fields re-injected every round trip, L268; mirror / spectral phase / modulator of the
