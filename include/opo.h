@@ -226,8 +226,8 @@ int opo_get_z_steps(const opo_handle* h, int* out_steps);
  * step) exchanges its operands over distributed shared memory; one launch per opo_propagate /
  * opo_roundtrips.  The lowest latency per z-step: AUTO picks it when the whole batch fits the co-resident clusters in
  * one wave (the paper's own workload, one OPO followed for thousands of round trips; BASELINE.json
- * configs[1], [2]).  Not with the N/2 - L - N/2 ordering, a phase modulator or a resonant pump: those run on RESIDENT
- * (a request for WIDE is then served by RESIDENT / SOLO as AUTO would). */
+ * configs[1], [2]).  Not with the N/2 - L - N/2 ordering or a resonant pump: those run on RESIDENT (a request for WIDE is
+ * then served by RESIDENT / SOLO as AUTO would). */
 #define OPO_ENGINE_WIDE 6
 #define OPO_OPT_ENGINE 0
 /* Operator splitting of a z-step.  LNL (default, BASELINE.json north_star): linear half-step,

@@ -691,12 +691,9 @@ bool prefer_solo(const opo_handle* h) {
     return solo_slots > 2.6 * cluster_slots;
 }
 
-// The wide engine serves the default ordering without a modulator and without a resonant pump (opo_wide.cuh).
+// The wide engine serves the default ordering without a resonant pump (opo_wide.cuh).
 bool wide_serves(const opo_handle* h) {
-    if (!h->wide_ok || h->splitting || h->n_seg > 1 || h->fields.resonant[0]) return false;
-    for (int x = 0; x < h->F; ++x)
-        if (h->eom[x]) return false;
-    return true;
+    return h->wide_ok && !h->splitting && h->n_seg == 1 && !h->fields.resonant[0];
 }
 
 // AUTO takes the wide engine (4 F SMs per instance, the lowest latency per z-step) when it finishes the batch sooner than

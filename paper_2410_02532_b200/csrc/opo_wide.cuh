@@ -36,7 +36,8 @@
 // Everything else (merged tables H, H2, HB = H2 G m across the cavity boundary; stored
 // inputs SH of non-resonant fields re-injected every round trip, L268; mirror / spectral phase / modulator of the
 // call's last round trip) is the cluster engine's logic on sub-blocks.  Not served here (the host keeps those on the
-// cluster engine): the N/2 - L - N/2 ordering, a modulator at an inner crossing, a resonant pump.
+// cluster engine): the N/2 - L - N/2 ordering and a resonant pump.  A phase modulator acts at a crossing
+// between two in-place pass-0 phases of the modulated field, as in the cluster engine.
 #pragma once
 #include "opo_resident.cuh"
 
@@ -299,6 +300,11 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
     const cplx<T>* tabH = reinterpret_cast<const cplx<T>*>(a.tabH[x]);
     const cplx<T>* tabH2 = reinterpret_cast<const cplx<T>*>(a.tabH2[x]);
     uint32_t fz = 0;          // fused phases executed so far (mbarrier phase parity)
+    int mask_eom = 0;         // resonant fields with an intracavity phase modulator
+#pragma unroll
+    for (int f = 0; f < F; ++f)
+        if (a.eom[f] != nullptr && a.resonant[f]) mask_eom |= 1 << f;
+    const bool my_eom = (mask_eom >> x) & 1;
 
     // pass-0 butterflies of this thread's tiles: MODE = WIDE_RK4: inverse pass 0 -> RK4 -> forward pass 0 (all fields);
     // WIDE_FWD0 / WIDE_INV0: the pass alone, on the fields of `mask`
@@ -404,6 +410,13 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
             }
             if (!core) {
                 // a helper warp has no part in the linear core
+            } else if (crossing && my_eom) {
+                // the modulator acts in the time domain between the boundary's spectral factor and the next pass: last
+                // half-step and boundary in place (table H G m), the rest below
+                WideFlow fa = fb;
+                fa.wait_in = 1; fa.par_done = (fz - 1) & 1;
+                fa.push_out = 0;
+                wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, reinterpret_cast<const cplx<T>*>(a.tabHG[x]) + (size_t)b * a.tab_stride[x], j, tid, fa, nullptr);
             } else if (crossing && !resonant) {
                 // fresh pump / frozen seed, already half-stepped: a thread sends the elements of its own pass-1
                 // butterfly, i.e. of its class, to the tiles' owners as an inverse pass 1 would
@@ -420,6 +433,26 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
                 fa.push_out = q < total;
                 wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
+            }
+            if (crossing && mask_eom) {         // uniform over the cluster
+                // inverse pass 0 -> x E[n] -> forward pass 0 -> first half-step of the next pass, for the modulated fields; the
+                // other fields have sent their operands already and their owners' tiles simply wait for these
+                cluster_bar();
+                tiles(tag_inv0{}, mask_eom, one, one, one);
+                cluster_bar();
+                if (core && my_eom) {
+                    const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]) + (size_t)j * S;
+#pragma unroll 4
+                    for (int i = tid; i < S; i += NT) sm[phys<T>(i)] = cmul(sm[phys<T>(i)], ldg(&E[i]));
+                }
+                cluster_bar();
+                tiles(tag_fwd0{}, mask_eom, one, one, one);
+                cluster_bar();
+                if (core && my_eom) {
+                    WideFlow fa = fb;
+                    fa.wait_in = 0; fa.push_out = 1;
+                    wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tabH, j, tid, fa, nullptr);
+                }
             }
             if (q == total) break;
             if (nt_own > 0) {

@@ -750,12 +750,13 @@ def test_eom_config1_20_roundtrips_and_abi_errors():
     w = W.config1().truncated(20)
     w.eom_beta_rad = [0.0, 1.2, 0.0]
     w.eom_f_hz = [0.0, 3.0 / w.window_s, 0.0]
-    cur, ex, eng = run_gpu(w, P.ENGINE_AUTO)
-    assert eng == P.ENGINE_RESIDENT
     rcur, rex = run_oracle(w)
-    e1 = assert_close(cur, rcur, 1e-4, "C1+EOM current")
-    e2 = assert_close(ex, rex, 1e-4, "C1+EOM exit")
-    print(f"C1 + EOM, 20 RT: rel L2 current {e1:.3e} exit {e2:.3e}")
+    for engine, expect in ((P.ENGINE_AUTO, P.ENGINE_WIDE), (P.ENGINE_RESIDENT, P.ENGINE_RESIDENT), (P.ENGINE_SOLO, P.ENGINE_SOLO)):
+        cur, ex, eng = run_gpu(w, engine)
+        assert eng == expect               # AUTO: one instance goes to the wide engine, modulator or not
+        e1 = assert_close(cur, rcur, 1e-4, "C1+EOM current")
+        e2 = assert_close(ex, rex, 1e-4, "C1+EOM exit")
+        print(f"C1 + EOM, 20 RT, engine {eng}: rel L2 current {e1:.3e} exit {e2:.3e}")
     o = P.from_workload(w)
     with pytest.raises(P.OpoError) as ei:
         o.set_eom(0, 1.0, 1e11)                # the pump is not resonant
