@@ -341,8 +341,10 @@ __device__ __forceinline__ void fwd_pass_smem(cplx<T>* __restrict__ sm, const cp
 }
 
 // ---- one inverse (DIT) pass over shared memory ---------------------------------------------------------
-// UF: the twiddle multiply takes the twiddle's magnitude defect out (cmulc_unit); dtw (fp32): the defects |w|^2 - 1,
-// tabulated with the index of the twiddle table (null: evaluated on the fly)
+// UF: the twiddle multiply can take the twiddles' magnitude defect out (cmulc_unit).  dtw (fp32): the defects to remove,
+// tabulated with the index of the twiddle table -- a multiple K (|w|^2 - 1) when the caller corrects only every K-th
+// application (the defect is ~3e-8: K uncorrected pairs make (1 + d)^K = 1 + K d to 1e-13, and one corrected multiply
+// takes all of it out); null: this application is a plain multiply
 template <class T, int L, int PASS, int NT, bool TWS, bool UF = false>
 __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int tid, const float* __restrict__ dtw = nullptr) {
     using PL = plan<L>;
@@ -357,14 +359,18 @@ __device__ __forceinline__ void inv_pass_smem(cplx<T>* __restrict__ sm, const cp
 #pragma unroll
         for (int k = 0; k < R; ++k) v[k] = p[elem_off<T, RB, SB>(k)];
         if constexpr (SB > 0) {
+            bool plain = true;
+            if constexpr (UF && sizeof(T) == 4) {
+                if (dtw != nullptr) {       // uniform over the launch at this point of the program
+                    plain = false;
 #pragma unroll
-            for (int k = 1; k < R; ++k) {
-                if constexpr (UF && sizeof(T) == 4) {
-                    const cplx<T> wk = ldtw<TWS>(&w[((k - 1) << SB) + t]);
-                    v[k] = cmulc_unit(v[k], wk, dtw != nullptr ? dtw[PL::tw_offset(PASS) + ((k - 1) << SB) + t] : unit_defect(wk));
-                } else {
-                    v[k] = cmulc(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
+                    for (int k = 1; k < R; ++k)
+                        v[k] = cmulc_unit(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]), dtw[PL::tw_offset(PASS) + ((k - 1) << SB) + t]);
                 }
+            }
+            if (plain) {
+#pragma unroll
+                for (int k = 1; k < R; ++k) v[k] = cmulc(v[k], ldtw<TWS>(&w[((k - 1) << SB) + t]));
             }
         }
         dit_inv<T, R>::run(v);

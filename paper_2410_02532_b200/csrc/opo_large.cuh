@@ -112,25 +112,31 @@ __device__ __forceinline__ void pass0_rk4_local(cplx<T>* const* fld, int t, cons
                                                 const float* __restrict__ dtw0 = nullptr) {
     constexpr int RB = 2, R = 4, SB = L - 2, S = 1 << SB;
     cplx<T> w[R - 1];
-    float wd[R - 1];        // magnitude defects of the twiddles (fp32, cmulc_unit)
 #pragma unroll
-    for (int k = 0; k < R - 1; ++k) {
-        w[k] = tw0s[k * S + t];
-        if constexpr (sizeof(T) == 4) wd[k] = dtw0 != nullptr ? dtw0[k * S + t] : unit_defect(w[k]);
-        else wd[k] = 0.0f;
-    }
+    for (int k = 0; k < R - 1; ++k) w[k] = tw0s[k * S + t];
     const int p0 = elem_base<T, RB, SB>(0, t);
     cplx<T> v[F][R];
 #pragma unroll
     for (int x = 0; x < F; ++x)
 #pragma unroll
         for (int k = 0; k < R; ++k) v[x][k] = fld[x][p0 + elem_off<T, RB, SB>(k)];
+    // dtw0 (fp32): the magnitude defects to take out of the twiddles in this application (cmulc_unit); null: plain multiply
+    if (sizeof(T) == 4 && dtw0 != nullptr) {
+        float wd[R - 1];
 #pragma unroll
-    for (int x = 0; x < F; ++x) {
+        for (int k = 0; k < R - 1; ++k) wd[k] = dtw0[k * S + t];
 #pragma unroll
-        for (int k = 1; k < R; ++k) v[x][k] = cmulc_unit(v[x][k], w[k - 1], wd[k - 1]);
-        dit_inv<T, R>::run(v[x]);
+        for (int x = 0; x < F; ++x)
+#pragma unroll
+            for (int k = 1; k < R; ++k) v[x][k] = cmulc_unit(v[x][k], w[k - 1], wd[k - 1]);
+    } else {
+#pragma unroll
+        for (int x = 0; x < F; ++x)
+#pragma unroll
+            for (int k = 1; k < R; ++k) v[x][k] = cmulc(v[x][k], w[k - 1]);
     }
+#pragma unroll
+    for (int x = 0; x < F; ++x) dit_inv<T, R>::run(v[x]);
 #pragma unroll
     for (int j = 0; j < R; ++j) {
         cplx<T> y[F];
@@ -182,8 +188,16 @@ template <class T, int L, int F> struct LargeEngine {
     const cplx<T>* wlo;     // W_N^j, j < N1
     const cplx<T>* whi;     // W_N^{j N1}, j < N2
     int tid;
-    const float* dtw1 = nullptr;    // |w|^2 - 1 of the pass twiddles (fp32; opo_fft.cuh), indexed as tw1 / tw2
+    // Magnitude defects of the pass twiddles (fp32; cmulc_unit in opo_fft.cuh), indexed as tw1 / tw2.  The correction is
+    // applied at every FIX_EVERY-th z-step only, FIX_EVERY times as large: the tables hold FIX_EVERY (|w|^2 - 1) and the
+    // kernel sets `fix` for those z-steps (13 instructions per inverse twiddle were 19 % of the instructions of a z-step).
+    // The defect operator does not commute with the dispersion step U, so bunching K corrections leaves K/2 |U - 1| of the
+    // defect behind: with 8 that is a third at the band edge of C3 (0.085 rad per z-step) and a few per cent where the
+    // signal lives; measured on C3 x 20 RT: 6.8e-5 with K = 1, 8 and 16 alike.
+    static constexpr int FIX_EVERY = 8;
+    const float* dtw1 = nullptr;
     const float* dtw2 = nullptr;
+    bool fix = false;               // this z-step takes the accumulated defects out
     // row caches (large_cfg::CACHE): valid for rows of `cache_tab` handled by this CTA's teams
     const void* cache_src = nullptr;        // the global table the cached slice was copied from (null: no cache)
     const TAB* cache_tab = nullptr;         // [ROWS][N2] in mid-pass layout
@@ -255,7 +269,7 @@ template <class T, int L, int F> struct LargeEngine {
             if constexpr (MODE != COL_FWD && MODE != COL_NFWD) {
                 __syncthreads();
                 inv_pass_smem<T, C::L1, P1::P - 1, C::TT1, true>(smt, tw1, lt);
-                inv_passes<T, C::L1, C::TT1, true, ((MODE == COL_INV || MODE == COL_INVN) ? 0 : 1), C::SY1, true>(smt, tw1, lt, 1 + team, dtw1);
+                inv_passes<T, C::L1, C::TT1, true, ((MODE == COL_INV || MODE == COL_INVN) ? 0 : 1), C::SY1, true>(smt, tw1, lt, 1 + team, fix ? dtw1 : nullptr);
             }
             if constexpr (MODE == COL_INVN) rk4_tile();
             if constexpr (MODE == COL_RK4) {
@@ -271,7 +285,7 @@ template <class T, int L, int F> struct LargeEngine {
 #pragma unroll
                     for (int x = 0; x < F; ++x) fld[x] = sm + (x * C::TC + c) * C::CSTRIDE;
                     pass0_rk4_local<T, C::L1, F>(fld, t, tw1 + P1::tw_offset(0), e0, e1, e2, kap, h, two, e3, e4,
-                                                 dtw1 != nullptr ? dtw1 + P1::tw_offset(0) : nullptr);
+                                                 (fix && dtw1 != nullptr) ? dtw1 + P1::tw_offset(0) : nullptr);
                 }
             }
             if constexpr (MODE != COL_INV && MODE != COL_INVN) {
@@ -390,7 +404,7 @@ template <class T, int L, int F> struct LargeEngine {
 #pragma unroll
                     for (int j = 0; j < CNT; ++j) {
                         w[j] = big_twiddle(k1, lt + j * C::TT2);
-                        if constexpr (sizeof(T) == 4) wd[j] = unit_defect(w[j]);
+                        if constexpr (sizeof(T) == 4) wd[j] = fix ? (float)FIX_EVERY * unit_defect(w[j]) : 0.0f;
                         else wd[j] = 0.0f;
                     }
                 }
@@ -406,7 +420,7 @@ template <class T, int L, int F> struct LargeEngine {
 #pragma unroll
                         for (int j = 0; j < CNT; ++j) {
                             w[j] = cache_w[team * C::N2 + lt + j * C::TT2];
-                            wd[j] = cache_wd[team * C::N2 + lt + j * C::TT2];
+                            wd[j] = fix ? cache_wd[team * C::N2 + lt + j * C::TT2] : 0.0f;
                         }
                     } else {
 #pragma unroll
@@ -429,17 +443,27 @@ template <class T, int L, int F> struct LargeEngine {
                 }
 #pragma unroll
                 for (int it = 0; it < NIT; ++it) mid_bf<T, C::L2, TAB>(smt, hh[it], lt + it * C::TT2);
-                inv_passes<T, C::L2, C::TT2, true, 0, C::SY2, true>(smt, tw2, lt, 1 + team, dtw2);
+                inv_passes<T, C::L2, C::TT2, true, 0, C::SY2, true>(smt, tw2, lt, 1 + team, fix ? dtw2 : nullptr);
                 pass_sync<C::SY2>(1 + team);
                 OPO_TSTAMP(*this, 6);                       // row transforms (team 0)
                 if (active) {
                     cplx<T>* sh = pick(op.sh_store, x) ? pick(op.sh_store, x) + off : nullptr;
+                    if (sizeof(T) == 4 && fix) {
 #pragma unroll
-                    for (int j = 0; j < CNT; ++j) {
-                        const int i = lt + j * C::TT2;
-                        const cplx<T> v = cmulc_unit(smt[phys<T>(i)], w[j], wd[j]);
-                        g[i] = v;
-                        if (sh) sh[i] = v;
+                        for (int j = 0; j < CNT; ++j) {
+                            const int i = lt + j * C::TT2;
+                            const cplx<T> v = cmulc_unit(smt[phys<T>(i)], w[j], wd[j]);
+                            g[i] = v;
+                            if (sh) sh[i] = v;
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < CNT; ++j) {
+                            const int i = lt + j * C::TT2;
+                            const cplx<T> v = cmulc(smt[phys<T>(i)], w[j]);
+                            g[i] = v;
+                            if (sh) sh[i] = v;
+                        }
                     }
                 }
             }
@@ -478,8 +502,8 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
     __syncthreads();
     if constexpr (sizeof(T) == 4) {     // magnitude defects of the pass twiddles
         float* d = reinterpret_cast<float*>(smem_raw + C::CACHE_OFFSET + (C::CACHE ? C::TABC_BYTES + C::WC_BYTES : 0));
-        for (int i = tid; i < C::TW1; i += C::NT) d[i] = unit_defect(e.tw1[i]);
-        for (int i = tid; i < C::TW2; i += C::NT) d[C::TW1 + i] = unit_defect(e.tw2[i]);
+        for (int i = tid; i < C::TW1; i += C::NT) d[i] = (float)E::FIX_EVERY * unit_defect(e.tw1[i]);
+        for (int i = tid; i < C::TW2; i += C::NT) d[C::TW1 + i] = (float)E::FIX_EVERY * unit_defect(e.tw2[i]);
         e.dtw1 = d;
         e.dtw2 = d + C::TW1;
     }
@@ -506,7 +530,7 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
                         if (rr < C::N1) {
                             const cplx<T> w = e.big_twiddle(__ldg(&a.perm1[rr]), i % C::N2);
                             cw[i] = w;
-                            cd[i] = unit_defect(w);
+                            cd[i] = (float)E::FIX_EVERY * unit_defect(w);
                         }
                     }
                     e.cache_w = cw;
@@ -562,6 +586,7 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
         }
 #pragma unroll 1
         for (int q = 0; q < nsteps; ++q) {
+            e.fix = (q % E::FIX_EVERY) == 0;
             e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);      // (begins with the grid barrier)
             grid_barrier(a.barrier, target);
             if (q + 1 < nsteps) e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 4 * (zs + q) + 2, kap, hh, true);
@@ -595,6 +620,7 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
                 if (rt_mode && q == 0 && !res && a.steps > 1) op.sh_store[x] = reinterpret_cast<cplx<T>*>(a.SH[x]);
             }
         }
+        e.fix = (q % E::FIX_EVERY) == 0;        // (row pass and the column pass that follows)
         e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);          // (begins with the grid barrier)
         OPO_TSTAMP(e, 7);                                   // row stored
         grid_barrier(a.barrier, target);
@@ -602,6 +628,7 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
         if (q == total) break;
         e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 2 * s, kap, h);
     }
+    e.fix = false;
     e.template col_pass<COL_INV>(cur, cur, mask, batch, phase, a.phase_stride, 0, kap, h);
 #ifdef OPO_LARGE_TIMING
     // (the first column-load interval of a launch starts at t = 0 and is left out: divide the rest by the z-steps timed)
