@@ -155,27 +155,42 @@ template <int R, int J> struct root {
 // x * c for a compile-time constant c.  fp32: c is carried as hi + lo so that the product has no
 // systematic (constant-rounding) bias -- a biased |w| != 1 inside every butterfly would change the
 // field amplitude by ~1e-8 per transform, coherently, and thousands of z-steps add up.
+// KM (fp32 only), the "constant mode": 0 = hi + lo at every application (exact to 1e-15);  1 = hi alone (one instruction
+// instead of two);  2 = hi + kConstBunch lo.  A caller that applies the same butterflies at every z-step may use mode 1 at
+// kConstBunch - 1 of every kConstBunch z-steps and mode 2 at the remaining one: the rounding of hi is a defect of ~3e-8, so
+// the uncorrected steps deviate by (1 + d)^(K-1) = 1 + (K - 1) d to 1e-13 and the corrected one takes exactly that out
+// (solo engine; the lo terms are 8 % of the FP32-pipe work of a z-step).
+constexpr int kConstBunch = 8;
 template <class T> struct kconst;
 template <> struct kconst<double> {
-    template <class C> static __device__ __forceinline__ double mul(double x, C) { return x * C::value; }
+    template <int KM, class C> static __device__ __forceinline__ double mul(double x, C) { return x * C::value; }
     // x * C1 + y * C2
-    template <class C1, class C2> static __device__ __forceinline__ double dot(double x, C1, double y, C2) {
+    template <int KM, class C1, class C2> static __device__ __forceinline__ double dot(double x, C1, double y, C2) {
         return x * C1::value + y * C2::value;
     }
 };
 template <> struct kconst<float> {
-    template <class C> static __device__ __forceinline__ float mul(float x, C) {
+    template <int KM, class C> static __device__ __forceinline__ float mul(float x, C) {
         constexpr float hi = (float)C::value;
-        constexpr float lo = (float)(C::value - (double)hi);
-        return __fmaf_rn(x, hi, x * lo);
+        if constexpr (KM == 1) {
+            return x * hi;
+        } else {
+            constexpr float lo = (float)((KM == 2 ? (double)kConstBunch : 1.0) * (C::value - (double)hi));
+            return __fmaf_rn(x, hi, x * lo);
+        }
     }
-    template <class C1, class C2> static __device__ __forceinline__ float dot(float x, C1, float y, C2) {
-        constexpr float h1 = (float)C1::value, l1 = (float)(C1::value - (double)h1);
-        constexpr float h2 = (float)C2::value, l2 = (float)(C2::value - (double)h2);
-        float t = x * l1;
-        t = __fmaf_rn(y, l2, t);
-        t = __fmaf_rn(x, h1, t);
-        return __fmaf_rn(y, h2, t);
+    template <int KM, class C1, class C2> static __device__ __forceinline__ float dot(float x, C1, float y, C2) {
+        constexpr float h1 = (float)C1::value, h2 = (float)C2::value;
+        if constexpr (KM == 1) {
+            return __fmaf_rn(y, h2, x * h1);
+        } else {
+            constexpr double k = KM == 2 ? (double)kConstBunch : 1.0;
+            constexpr float l1 = (float)(k * (C1::value - (double)h1)), l2 = (float)(k * (C2::value - (double)h2));
+            float t = x * l1;
+            t = __fmaf_rn(y, l2, t);
+            t = __fmaf_rn(x, h1, t);
+            return __fmaf_rn(y, h2, t);
+        }
     }
 };
 struct c_sqrt_half { static constexpr double value = 0.70710678118654752440084436210485; };
@@ -183,7 +198,7 @@ template <int R, int J, bool NEG> struct c_cos { static constexpr double value =
 template <int R, int J, bool NEG> struct c_sin { static constexpr double value = NEG ? -root<R, J>::s : root<R, J>::s; };
 
 // a * w_R^J (forward) or a * conj(w_R^J) (INV)
-template <class T, int R, int J, bool INV>
+template <class T, int R, int J, bool INV, int KM = 0>
 __device__ __forceinline__ cplx<T> mul_root(cplx<T> a) {
     using K = kconst<T>;
     if constexpr (J == 0) {
@@ -192,30 +207,30 @@ __device__ __forceinline__ cplx<T> mul_root(cplx<T> a) {
         if constexpr (INV) return {-a.im, a.re};
         else return {a.im, -a.re};
     } else if constexpr (8 * J == R) {            // w = (1 - i)/sqrt2
-        if constexpr (INV) return {K::mul(a.re - a.im, c_sqrt_half{}), K::mul(a.re + a.im, c_sqrt_half{})};
-        else return {K::mul(a.re + a.im, c_sqrt_half{}), K::mul(a.im - a.re, c_sqrt_half{})};
+        if constexpr (INV) return {K::template mul<KM>(a.re - a.im, c_sqrt_half{}), K::template mul<KM>(a.re + a.im, c_sqrt_half{})};
+        else return {K::template mul<KM>(a.re + a.im, c_sqrt_half{}), K::template mul<KM>(a.im - a.re, c_sqrt_half{})};
     } else if constexpr (8 * J == 3 * R) {        // w = (-1 - i)/sqrt2
-        if constexpr (INV) return {K::mul(-a.re - a.im, c_sqrt_half{}), K::mul(a.re - a.im, c_sqrt_half{})};
-        else return {K::mul(a.im - a.re, c_sqrt_half{}), K::mul(-a.re - a.im, c_sqrt_half{})};
+        if constexpr (INV) return {K::template mul<KM>(-a.re - a.im, c_sqrt_half{}), K::template mul<KM>(a.re - a.im, c_sqrt_half{})};
+        else return {K::template mul<KM>(a.im - a.re, c_sqrt_half{}), K::template mul<KM>(-a.re - a.im, c_sqrt_half{})};
     } else {
         // forward: w = c - i s ; inverse: conj(w) = c + i s
         if constexpr (INV)
-            return {K::dot(a.re, c_cos<R, J, false>{}, a.im, c_sin<R, J, true>{}),
-                    K::dot(a.im, c_cos<R, J, false>{}, a.re, c_sin<R, J, false>{})};
+            return {K::template dot<KM>(a.re, c_cos<R, J, false>{}, a.im, c_sin<R, J, true>{}),
+                    K::template dot<KM>(a.im, c_cos<R, J, false>{}, a.re, c_sin<R, J, false>{})};
         else
-            return {K::dot(a.re, c_cos<R, J, false>{}, a.im, c_sin<R, J, false>{}),
-                    K::dot(a.im, c_cos<R, J, false>{}, a.re, c_sin<R, J, true>{})};
+            return {K::template dot<KM>(a.re, c_cos<R, J, false>{}, a.im, c_sin<R, J, false>{}),
+                    K::template dot<KM>(a.im, c_cos<R, J, false>{}, a.re, c_sin<R, J, true>{})};
     }
 }
 
 // ---- register DFT of size R, natural order in and out ---------------------------------------------
 // Forward: decimation in frequency.  v[j] -> sum_j v[j] w_R^{jk}.
-template <class T, int R> struct dif {
+template <class T, int R, int KM = 0> struct dif {
     template <int J>
     static __device__ __forceinline__ void bf(cplx<T>* v) {
         cplx<T> a = v[J], b = v[J + R / 2];
         v[J] = a + b;
-        v[J + R / 2] = mul_root<T, R, J, false>(a - b);
+        v[J + R / 2] = mul_root<T, R, J, false, KM>(a - b);
     }
     template <int... J>
     static __device__ __forceinline__ void stage(cplx<T>* v, std::integer_sequence<int, J...>) {
@@ -223,8 +238,8 @@ template <class T, int R> struct dif {
     }
     static __device__ __forceinline__ void run(cplx<T>* v) {
         stage(v, std::make_integer_sequence<int, R / 2>{});
-        dif<T, R / 2>::run(v);
-        dif<T, R / 2>::run(v + R / 2);
+        dif<T, R / 2, KM>::run(v);
+        dif<T, R / 2, KM>::run(v + R / 2);
         // X[2m] = first half [m], X[2m+1] = second half [m]
         cplx<T> t[R];
 #pragma unroll
@@ -233,13 +248,13 @@ template <class T, int R> struct dif {
         for (int m = 0; m < R; ++m) v[m] = t[m];
     }
 };
-template <class T> struct dif<T, 1> { static __device__ __forceinline__ void run(cplx<T>*) {} };
+template <class T, int KM> struct dif<T, 1, KM> { static __device__ __forceinline__ void run(cplx<T>*) {} };
 
 // Inverse (unnormalised): decimation in time with conjugate roots -- the adjoint of dif<T,R>.
-template <class T, int R> struct dit_inv {
+template <class T, int R, int KM = 0> struct dit_inv {
     template <int J>
     static __device__ __forceinline__ void bf(cplx<T>* v) {
-        cplx<T> a = v[J], b = mul_root<T, R, J, true>(v[J + R / 2]);
+        cplx<T> a = v[J], b = mul_root<T, R, J, true, KM>(v[J + R / 2]);
         v[J] = a + b;
         v[J + R / 2] = a - b;
     }
@@ -253,12 +268,12 @@ template <class T, int R> struct dit_inv {
         for (int m = 0; m < R / 2; ++m) { t[m] = v[2 * m]; t[m + R / 2] = v[2 * m + 1]; }
 #pragma unroll
         for (int m = 0; m < R; ++m) v[m] = t[m];
-        dit_inv<T, R / 2>::run(v);
-        dit_inv<T, R / 2>::run(v + R / 2);
+        dit_inv<T, R / 2, KM>::run(v);
+        dit_inv<T, R / 2, KM>::run(v + R / 2);
         stage(v, std::make_integer_sequence<int, R / 2>{});
     }
 };
-template <class T> struct dit_inv<T, 1> { static __device__ __forceinline__ void run(cplx<T>*) {} };
+template <class T, int KM> struct dit_inv<T, 1, KM> { static __device__ __forceinline__ void run(cplx<T>*) {} };
 
 // ---- radix plan ------------------------------------------------------------------------------------
 // N = 2^L: pass 0 has radix 4 (the RK4-fused exchange pass); the remaining L - 2 bits are split into
@@ -570,7 +585,7 @@ template <int G, int NTG> __device__ __forceinline__ void group_bar(int g) {
 }
 
 // one forward butterfly u of pass PASS (twiddles from shared memory)
-template <class T, int L, int PASS>
+template <class T, int L, int PASS, int KM = 0>
 __device__ __forceinline__ void fwd_bf(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int u) {
     using PL = plan<L>;
     constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
@@ -580,7 +595,7 @@ __device__ __forceinline__ void fwd_bf(cplx<T>* __restrict__ sm, const cplx<T>* 
     cplx<T> v[R];
 #pragma unroll
     for (int j = 0; j < R; ++j) v[j] = p[elem_off<T, RB, SB>(j)];
-    dif<T, R>::run(v);
+    dif<T, R, KM>::run(v);
     if constexpr (SB > 0) {
 #pragma unroll
         for (int k = 1; k < R; ++k) v[k] = cmul(v[k], w[((k - 1) << SB) + t]);
@@ -588,7 +603,7 @@ __device__ __forceinline__ void fwd_bf(cplx<T>* __restrict__ sm, const cplx<T>* 
 #pragma unroll
     for (int k = 0; k < R; ++k) p[elem_off<T, RB, SB>(k)] = v[k];
 }
-template <class T, int L, int PASS>
+template <class T, int L, int PASS, int KM = 0>
 __device__ __forceinline__ void inv_bf(cplx<T>* __restrict__ sm, const cplx<T>* __restrict__ tw, int u) {
     using PL = plan<L>;
     constexpr int RB = PL::rbits(PASS), R = 1 << RB, SB = PL::sbits(PASS), S = 1 << SB;
@@ -602,12 +617,12 @@ __device__ __forceinline__ void inv_bf(cplx<T>* __restrict__ sm, const cplx<T>* 
 #pragma unroll
         for (int k = 1; k < R; ++k) v[k] = cmulc(v[k], w[((k - 1) << SB) + t]);
     }
-    dit_inv<T, R>::run(v);
+    dit_inv<T, R, KM>::run(v);
 #pragma unroll
     for (int j = 0; j < R; ++j) p[elem_off<T, RB, SB>(j)] = v[j];
 }
 // the fused middle on butterfly u with its table entries already in registers
-template <class T, int L, class TAB>
+template <class T, int L, class TAB, int KM = 0>
 __device__ __forceinline__ void mid_bf(cplx<T>* __restrict__ sm, const TAB* h, int u) {
     using PL = plan<L>;
     constexpr int RB = PL::rbits(PL::P - 1), R = 1 << RB;
@@ -615,16 +630,16 @@ __device__ __forceinline__ void mid_bf(cplx<T>* __restrict__ sm, const TAB* h, i
     cplx<T> v[R];
 #pragma unroll
     for (int j = 0; j < R; ++j) v[j] = p[elem_off<T, RB, 0>(j)];
-    dif<T, R>::run(v);
+    dif<T, R, KM>::run(v);
 #pragma unroll
     for (int k = 0; k < R; ++k) v[k] = tab_mul(v[k], h[k]);
-    dit_inv<T, R>::run(v);
+    dit_inv<T, R, KM>::run(v);
 #pragma unroll
     for (int j = 0; j < R; ++j) p[elem_off<T, RB, 0>(j)] = v[j];
 }
 
 // forward passes PASS .. LASTF of one group, a group barrier after each
-template <class T, int L, int NT, int PASS, int LASTF, bool FLOW, bool CTA = false>
+template <class T, int L, int NT, int PASS, int LASTF, bool FLOW, bool CTA = false, int KM = 0>
 __device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g, int tg, const FlowArgs& fa) {
     using CG = core_groups<T, L, NT>;
     if constexpr (PASS <= LASTF) {
@@ -637,18 +652,18 @@ __device__ __forceinline__ void group_fwd(cplx<T>* sm, const cplx<T>* twl, int g
                     if constexpr (CTA) mbar_wait_cta(fa.mb + 8 * (FC::NCLS + (tg >> 5) + FC::NWG * it), fa.par_done);
                     else mbar_wait(fa.mb + 8 * (FC::NCLS + (tg >> 5) + FC::NWG * it), fa.par_done);
                 }
-                fwd_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
+                fwd_bf<T, L, PASS, KM>(sm, twl, g * NB + tg + CG::NTG * it);
             }
         } else {
 #pragma unroll 1
-            for (int ul = tg; ul < NB; ul += CG::NTG) fwd_bf<T, L, PASS>(sm, twl, g * NB + ul);
+            for (int ul = tg; ul < NB; ul += CG::NTG) fwd_bf<T, L, PASS, KM>(sm, twl, g * NB + ul);
         }
         group_bar<CG::G, CG::NTG>(g);
-        group_fwd<T, L, NT, PASS + 1, LASTF, FLOW, CTA>(sm, twl, g, tg, fa);
+        group_fwd<T, L, NT, PASS + 1, LASTF, FLOW, CTA, KM>(sm, twl, g, tg, fa);
     }
 }
 // inverse passes PASS .. 1 of one group, a group barrier before each
-template <class T, int L, int NT, int PASS, bool FLOW, bool CTA = false>
+template <class T, int L, int NT, int PASS, bool FLOW, bool CTA = false, int KM = 0>
 __device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g, int tg, const FlowArgs& fa) {
     using CG = core_groups<T, L, NT>;
     if constexpr (PASS >= 1) {
@@ -658,7 +673,7 @@ __device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g
             using FC = flow_cfg<T, L, NT>;
 #pragma unroll 1
             for (int it = 0; it < FC::NIT; ++it) {
-                inv_bf<T, L, PASS>(sm, twl, g * NB + tg + CG::NTG * it);
+                inv_bf<T, L, PASS, KM>(sm, twl, g * NB + tg + CG::NTG * it);
                 if (fa.arrive_out) {
                     if constexpr (CTA) mbar_arrive_cta(fa.mb + 8 * ((tg >> 5) + FC::NWG * it), tg & 31);
                     else mbar_arrive_cluster(fa.mb + 8 * ((tg >> 5) + FC::NWG * it), tg & 31, fa.nf);
@@ -666,16 +681,17 @@ __device__ __forceinline__ void group_inv(cplx<T>* sm, const cplx<T>* twl, int g
             }
         } else {
 #pragma unroll 1
-            for (int ul = tg; ul < NB; ul += CG::NTG) inv_bf<T, L, PASS>(sm, twl, g * NB + ul);
+            for (int ul = tg; ul < NB; ul += CG::NTG) inv_bf<T, L, PASS, KM>(sm, twl, g * NB + ul);
         }
-        group_inv<T, L, NT, PASS - 1, FLOW, CTA>(sm, twl, g, tg, fa);
+        group_inv<T, L, NT, PASS - 1, FLOW, CTA, KM>(sm, twl, g, tg, fa);
     }
 }
 
 // Caller guarantees the field is visible to all threads on entry (barrier) and must barrier before
 // reading the result.  Not inlined: one copy serves every call site of a kernel.
 // CTA: the flow barriers are used by threads of this CTA only (solo engine): acquire / release at CTA scope
-template <class T, int L, int NT, bool FLOW = false, bool CTA = false>
+// KM: constant mode of the butterflies (kconst)
+template <class T, int L, int NT, bool FLOW = false, bool CTA = false, int KM = 0>
 __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, int tid, FlowArgs fa = FlowArgs{}) {
     using PL = plan<L>;
     using CG = core_groups<T, L, NT>;
@@ -686,7 +702,7 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
     const int g = (CG::G == 1) ? 0 : tid / CG::NTG, tg = (CG::G == 1) ? tid : tid % CG::NTG;
     constexpr int R = 1 << CG::RBL, NBF = (1 << L) >> CG::RBL;
     if constexpr (CG::chain) {
-        group_fwd<T, L, NT, 1, PL::P - 3, FLOW, CTA>(sm, twl, g, tg, fa);
+        group_fwd<T, L, NT, 1, PL::P - 3, FLOW, CTA, KM>(sm, twl, g, tg, fa);
 #pragma unroll 1
         for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
             const int u = g * CG::NBL + ul;
@@ -695,28 +711,28 @@ __device__ __noinline__ void linear_core_smem(const cplx<T>* __restrict__ tab, i
 #pragma unroll
                 for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
             }
-            fwd_bf<T, L, PL::P - 2>(sm, twl, u);
+            fwd_bf<T, L, PL::P - 2, KM>(sm, twl, u);
             __syncwarp();
             if constexpr (!CG::early_tab) {
 #pragma unroll
                 for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
             }
-            mid_bf<T, L>(sm, h, u);
+            mid_bf<T, L, cplx<T>, KM>(sm, h, u);
             __syncwarp();
-            inv_bf<T, L, PL::P - 2>(sm, twl, u);
+            inv_bf<T, L, PL::P - 2, KM>(sm, twl, u);
         }
-        group_inv<T, L, NT, PL::P - 3, FLOW, CTA>(sm, twl, g, tg, fa);
+        group_inv<T, L, NT, PL::P - 3, FLOW, CTA, KM>(sm, twl, g, tg, fa);
     } else {
-        group_fwd<T, L, NT, 1, PL::P - 2, FLOW, CTA>(sm, twl, g, tg, fa);
+        group_fwd<T, L, NT, 1, PL::P - 2, FLOW, CTA, KM>(sm, twl, g, tg, fa);
 #pragma unroll 1
         for (int ul = tg; ul < CG::NBL; ul += CG::NTG) {
             const int u = g * CG::NBL + ul;
             cplx<T> h[R];
 #pragma unroll
             for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
-            mid_bf<T, L>(sm, h, u);
+            mid_bf<T, L, cplx<T>, KM>(sm, h, u);
         }
-        group_inv<T, L, NT, PL::P - 2, FLOW, CTA>(sm, twl, g, tg, fa);
+        group_inv<T, L, NT, PL::P - 2, FLOW, CTA, KM>(sm, twl, g, tg, fa);
     }
 }
 

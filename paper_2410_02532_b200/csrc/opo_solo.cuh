@@ -286,13 +286,21 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
         else __syncthreads();
         ++fz;
     };
-    auto core = [&](const cplx<T>* tab, bool wait_in, bool arrive_out) {
+    // bunch: this application carries the low parts of the butterflies' compile-time constants for kConstBunch applications
+    // (kconst in opo_fft.cuh; fp32 with the flow synchronisation, i.e. N >= 2^12): the other kConstBunch - 1 use the high
+    // parts alone, one instruction per constant product instead of two
+    auto core = [&](const cplx<T>* tab, bool wait_in, bool arrive_out, bool bunch = false) {
         if constexpr (FLOW) {
             FlowArgs fa;
             fa.mb = mb; fa.nf = 1;
             fa.wait_in = wait_in; fa.par_done = (fz - 1) & 1;
             fa.arrive_out = arrive_out;
-            linear_core_smem<T, L, NT, true, true>(tab, tid, fa);
+            if constexpr (sizeof(T) == 4) {
+                if (bunch) linear_core_smem<T, L, NT, true, true, 2>(tab, tid, fa);
+                else linear_core_smem<T, L, NT, true, true, 1>(tab, tid, fa);
+            } else {
+                linear_core_smem<T, L, NT, true, true>(tab, tid, fa);
+            }
         } else {
             linear_core_smem<T, L, NT>(tab, tid);
         }
@@ -442,7 +450,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                     if (q != 0 && q != total)
                         tab = crossing ? reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x]
                                        : reinterpret_cast<const cplx<T>*>(a.tabH2[x]) + (size_t)(q & a.tab_cycle_mask) * N;
-                    core(tab, !first_core, !last_core && !keep && !inj);
+                    core(tab, !first_core, !last_core && !keep && !inj, (q & (kConstBunch - 1)) == 0);
                 }
                 if (inj) {
                     __syncthreads();

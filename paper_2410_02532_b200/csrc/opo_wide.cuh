@@ -137,7 +137,9 @@ __device__ __forceinline__ void wide_push16(const cplx<T>* v, const WideFlow& fa
 // this CTA holds i in [j S, (j + 1) S) only; the butterfly and table indices are the global ones of plan<L>.
 // sh_keep (may be null): the results of the inverse pass 1 are also stored there (the half-stepped input of a non-resonant
 // field, kept for the later round trips).
-template <class T, int L, int NT, int NCTA, int MAXT, int NQ>
+// KM: constant mode of the butterflies (kconst in opo_fft.cuh; fp32: the z-step loop runs kConstBunch - 1 applications with
+// the high parts of the compile-time roots alone and one that carries kConstBunch low parts)
+template <class T, int L, int NT, int NCTA, int MAXT, int NQ, int KM = 0>
 __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const cplx<T>* __restrict__ tab, int j, int tid, WideFlow fa,
                                        cplx<T>* __restrict__ sh_keep) {
     using PL = plan<L>;
@@ -151,7 +153,7 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
         mbar_wait_cta(fa.mb + 8 * (NW + warp), fa.par_done);      // (acquire at CTA scope: the bytes counted on the barrier are visible, and L1 is left alone)
         if (lane == 0) mbar_arm(fa.mb + 8 * (NW + warp), 16u * 32u * (uint32_t)sizeof(cplx<T>));       // the results of the next fused phase
     }
-    fwd_bf<T, L, 1>(smv, twl, j * NT + tid);
+    fwd_bf<T, L, 1, KM>(smv, twl, j * NT + tid);
     core_bar();
     if constexpr (chain) {
 #pragma unroll 1
@@ -160,15 +162,15 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
             cplx<T> h[R];
 #pragma unroll
             for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
-            fwd_bf<T, L, 2>(smv, twl, u);
+            fwd_bf<T, L, 2, KM>(smv, twl, u);
             __syncwarp();
-            mid_bf<T, L>(smv, h, u);
+            mid_bf<T, L, cplx<T>, KM>(smv, h, u);
             __syncwarp();
-            inv_bf<T, L, 2>(smv, twl, u);
+            inv_bf<T, L, 2, KM>(smv, twl, u);
         }
     } else {
 #pragma unroll 1
-        for (int ul = tid; ul < NB2; ul += NT) fwd_bf<T, L, 2>(smv, twl, j * NB2 + ul);
+        for (int ul = tid; ul < NB2; ul += NT) fwd_bf<T, L, 2, KM>(smv, twl, j * NB2 + ul);
         core_bar();
 #pragma unroll 1
         for (int ul = tid; ul < NBL; ul += NT) {
@@ -176,15 +178,15 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
             cplx<T> h[R];
 #pragma unroll
             for (int k = 0; k < R; ++k) h[k] = ldg(&tab[k * NBF + u]);
-            mid_bf<T, L>(smv, h, u);
+            mid_bf<T, L, cplx<T>, KM>(smv, h, u);
         }
         core_bar();
 #pragma unroll 1
-        for (int ul = tid; ul < NB2; ul += NT) inv_bf<T, L, 2>(smv, twl, j * NB2 + ul);
+        for (int ul = tid; ul < NB2; ul += NT) inv_bf<T, L, 2, KM>(smv, twl, j * NB2 + ul);
     }
     core_bar();
     if (!fa.push_out) {
-        inv_bf<T, L, 1>(smv, twl, j * NT + tid);
+        inv_bf<T, L, 1, KM>(smv, twl, j * NT + tid);
     } else {
         // inverse pass 1 with its results sent to the owners of their tiles
         constexpr int RB = PL::rbits(1), R1 = 1 << RB, SB = PL::sbits(1);
@@ -196,7 +198,7 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
         for (int k = 0; k < R1; ++k) v[k] = p[elem_off<T, RB, SB>(k)];
 #pragma unroll
         for (int k = 1; k < R1; ++k) v[k] = cmulc(v[k], w[((k - 1) << SB) + tid]);
-        dit_inv<T, R1>::run(v);
+        dit_inv<T, R1, KM>::run(v);
         wide_push16<T, NW, NCTA, MAXT, NQ>(v, fa, warp, lane);
         if (sh_keep != nullptr) {
 #pragma unroll
@@ -432,7 +434,12 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 WideFlow fa = fb;
                 fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
                 fa.push_out = q < total;
-                wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
+                if constexpr (sizeof(T) == 4) {
+                    if ((q & (kConstBunch - 1)) == 0) wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ, 2>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
+                    else wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ, 1>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
+                } else {
+                    wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
+                }
             }
             if (crossing && mask_eom) {         // uniform over the cluster
                 // inverse pass 0 -> x E[n] -> forward pass 0 -> first half-step of the next pass, for the modulated fields; the
