@@ -190,6 +190,8 @@ def main():
     ap.add_argument("--eom", action="store_true",
                     help="intracavity phase modulator on the signal (PAPER.md:L149-154; beta = 1 rad, f = 3 / window): the "
                          "paper's 'EOM' cavity configuration; the boundary is then not merged (one launch per round trip)")
+    ap.add_argument("--wide-subblocks", type=int, default=0, choices=[0, 1, 2],
+                    help="wide engine: sub-blocks per CTA (OPO_OPT_WIDE_SUBBLOCKS); 0 = the library's choice")
     ap.add_argument("--train", action="store_true",
                     help="nanosecond regime (PAPER.md:L322-335): opo_roundtrips_train -- a pump slice per round trip in, the exit "
                          "signal of every round trip out, one launch per round trip; default 20 round trips per step")
@@ -228,6 +230,8 @@ def main():
     rt_per_step = args.rt_per_step or (20 if args.train else {"C0": w.n_roundtrips, "C1": 100, "C2": 20, "C3": 2, "C4": w.n_roundtrips}[args.workload])
     engine = {"auto": P.ENGINE_AUTO, "resident": P.ENGINE_RESIDENT, "solo": P.ENGINE_SOLO, "wide": P.ENGINE_WIDE, "streaming": P.ENGINE_STREAMING, "cufft": P.ENGINE_CUFFT}[args.engine]
     o = P.from_workload(w, engine=engine)
+    if args.wide_subblocks:
+        P.opo_set_option(o._h, P.OPT_WIDE_SUBBLOCKS, args.wide_subblocks)
     units_per_step = w.batch * w.n * w.nz_per_pass * rt_per_step          # grid-point z-steps, this rank
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
 

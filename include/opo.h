@@ -236,6 +236,10 @@ int opo_get_z_steps(const opo_handle* h, int* out_steps);
  * order and differ by O(h^2).  Can change at z = 0 only.  With NLN the resident and large-N engines run one launch
  * per round trip. */
 #define OPO_OPT_SPLITTING 1
+/* WIDE engine only: sub-blocks of a field per CTA.  1: clusters of 4 F CTAs (lowest latency per instance, 7 clusters of 12 CTAs
+ * co-resident on a B200); 2: clusters of 2 F CTAs (22 co-resident, each ~1.4x slower per z-step); 0 (default): whichever
+ * finishes the batch sooner. */
+#define OPO_OPT_WIDE_SUBBLOCKS 2
 #define OPO_SPLITTING_LNL 0
 #define OPO_SPLITTING_NLN 1
 int opo_set_option(opo_handle* h, int option, int value);

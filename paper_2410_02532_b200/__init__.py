@@ -25,6 +25,7 @@ WHICH_CURRENT, WHICH_EXIT = 0, 1
 DOMAIN_TIME, DOMAIN_FREQ = 0, 1
 ENGINE_AUTO, ENGINE_RESIDENT, ENGINE_STREAMING, ENGINE_LARGE, ENGINE_CUFFT, ENGINE_SOLO, ENGINE_WIDE = 0, 1, 2, 3, 4, 5, 6
 OPT_ENGINE = 0
+OPT_WIDE_SUBBLOCKS = 2
 OPT_SPLITTING = 1
 SPLITTING_LNL, SPLITTING_NLN = 0, 1
 INFO_ENGINE, INFO_LAUNCHES, INFO_N, INFO_BATCH, INFO_SM_COUNT, INFO_SLOTS = 0, 1, 2, 3, 4, 5

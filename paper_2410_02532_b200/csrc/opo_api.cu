@@ -160,6 +160,8 @@ struct opo_handle {
     int tab_cycle = 1;                                // roundings of H^2 cycled through by the on-chip engines (fp32: 16; build_tables)
     bool wide_ok = false;                             // wide engine (a cluster of 4 F CTAs per instance)
     opo::ResidentInfo winfo{};                        // max_clusters = co-resident clusters of 4 F CTAs
+    int wide_g_opt = 0;                               // OPO_OPT_WIDE_SUBBLOCKS: 0 = AUTO, 1 | 2 = sub-blocks per CTA
+    opo::ResidentInfo winfo2{};                       // ... of 2 F CTAs holding two sub-blocks each (0: that variant is unavailable)
     int device = 0;
     long long launches = 0;
     std::string err;
@@ -606,9 +608,11 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
         e = h->dbl ? opo::solo_info_f64(h->L, h->F, &h->sinfo) : opo::solo_info_f32(h->L, h->F, &h->sinfo);
         h->solo_ok = (e == cudaSuccess && h->sinfo.max_clusters > 0);
         if (e != cudaSuccess) cudaGetLastError();
-        e = h->dbl ? opo::wide_info_f64(h->L, h->F, &h->winfo) : opo::wide_info_f32(h->L, h->F, &h->winfo);
+        e = h->dbl ? opo::wide_info_f64(h->L, h->F, 1, &h->winfo) : opo::wide_info_f32(h->L, h->F, 1, &h->winfo);
         h->wide_ok = (e == cudaSuccess && h->winfo.max_clusters > 0);
         if (e != cudaSuccess) cudaGetLastError();
+        e = h->dbl ? opo::wide_info_f64(h->L, h->F, 2, &h->winfo2) : opo::wide_info_f32(h->L, h->F, 2, &h->winfo2);
+        if (e != cudaSuccess) { cudaGetLastError(); h->winfo2.max_clusters = 0; }
     }
     if (cudaDeviceSynchronize() != cudaSuccess) return bail(OPO_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
     *out = h;
@@ -696,15 +700,29 @@ bool wide_serves(const opo_handle* h) {
     return h->wide_ok && !h->splitting && h->n_seg == 1 && !h->fields.resonant[0];
 }
 
-// AUTO takes the wide engine (4 F SMs per instance, the lowest latency per z-step) when it finishes the batch sooner than
-// the cluster engine: an instance takes 2.8x less time per z-step on 4 F SMs than on F (measured on C1: 5.7 vs 15.9 us),
-// but only winfo.max_clusters clusters of 4 F CTAs are co-resident (7 of 12 CTAs on a B200), so the batch runs in waves.
+// Time of the batch on the wide engine in units of the cluster engine's time per instance: clusters of 4 F CTAs take 1 / 2.9
+// of it per instance (measured on C1: 5.4 vs 15.9 us per z-step) but only winfo.max_clusters of them are co-resident (7 of 12
+// CTAs on a B200); clusters of 2 F CTAs with two sub-blocks per CTA take 1 / 1.4 of it (11.3 us: every SM then moves twice the
+// bytes over the SM-to-SM link, which is what bounds this engine) and 22 are co-resident: they win for 15 .. 22 instances.
+constexpr double kWide1 = 2.9, kWide2 = 1.4;
+int wide_group(const opo_handle* h, double* cost = nullptr) {
+    const int w1 = (h->B + h->winfo.max_clusters - 1) / h->winfo.max_clusters;
+    double c1 = (double)w1 / kWide1, c2 = 1e300;
+    if (h->winfo2.max_clusters > 0) c2 = (double)((h->B + h->winfo2.max_clusters - 1) / h->winfo2.max_clusters) / kWide2;
+    if (h->wide_g_opt == 1) c2 = 1e300;
+    if (h->wide_g_opt == 2 && c2 < 1e300) c1 = 1e300;
+    if (cost) *cost = std::min(c1, c2);
+    return c2 < c1 ? 2 : 1;
+}
+
+// AUTO takes the wide engine when it finishes the batch sooner than the cluster engine.
 bool prefer_wide(const opo_handle* h) {
     if (!wide_serves(h)) return false;
     if (!h->resident_ok) return true;
-    const int waves_w = (h->B + h->winfo.max_clusters - 1) / h->winfo.max_clusters;
+    double cost = 0.0;
+    wide_group(h, &cost);
     const int waves_r = (h->B + h->rinfo.max_clusters - 1) / h->rinfo.max_clusters;
-    return (double)waves_w < 2.8 * (double)waves_r;
+    return cost < (double)waves_r;
 }
 
 int engine_in_use(const opo_handle* h) {
@@ -891,7 +909,8 @@ int resident_run(opo_handle* h, int mode, int z0, int steps, const TrainArgs* tr
     a.dk0 = !h->splitting;
     for (int b = 0; b < h->B; ++b) if (h->dk[b] != 0.0) a.dk0 = 0;
     const bool solo = engine_in_use(h) == OPO_ENGINE_SOLO, wide = engine_in_use(h) == OPO_ENGINE_WIDE;
-    const int n_clusters = std::min(h->B, wide ? h->winfo.max_clusters : solo ? h->sinfo.max_clusters : h->rinfo.max_clusters);
+    a.wide_g = wide ? wide_group(h) : 1;
+    const int n_clusters = std::min(h->B, wide ? (a.wide_g == 2 ? h->winfo2.max_clusters : h->winfo.max_clusters) : solo ? h->sinfo.max_clusters : h->rinfo.max_clusters);
     // more instances than clusters and not a multiple: deal round trips instead of instances (see the kernel)
     a.split = 0; a.flags = nullptr;
     if (mode == 1 && !wide && !h->splitting && steps > 1 && h->B > n_clusters && h->B % n_clusters != 0) {
@@ -1242,6 +1261,12 @@ int opo_set_option(opo_handle* h, int option, int value) {
         if (value != h->splitting) { h->splitting = value; h->phase_dirty = true; }
         return OPO_OK;
     }
+    if (option == OPO_OPT_WIDE_SUBBLOCKS) {
+        if (value < 0 || value > 2) return fail(h, OPO_ERR_INVALID_ARG, "sub-blocks per CTA: 0 (AUTO), 1 or 2");
+        if (value == 2 && h->winfo2.max_clusters <= 0) return fail(h, OPO_ERR_UNSUPPORTED, "two sub-blocks per CTA: unavailable for this size/precision");
+        h->wide_g_opt = value;
+        return OPO_OK;
+    }
     if (option != OPO_OPT_ENGINE) return fail(h, OPO_ERR_INVALID_ARG, "unknown option");
     if (value != OPO_ENGINE_AUTO && value != OPO_ENGINE_RESIDENT && value != OPO_ENGINE_STREAMING && value != OPO_ENGINE_LARGE &&
         value != OPO_ENGINE_CUFFT && value != OPO_ENGINE_SOLO && value != OPO_ENGINE_WIDE)
@@ -1288,7 +1313,7 @@ int opo_get_info(const opo_handle* h, int what, long long* out) {
         case OPO_INFO_SLOTS: {
             const int e = engine_in_use(h);
             if (e == OPO_ENGINE_SOLO) *out = std::min(h->B, h->sinfo.max_clusters);
-            else if (e == OPO_ENGINE_WIDE) *out = std::min(h->B, h->winfo.max_clusters);
+            else if (e == OPO_ENGINE_WIDE) *out = std::min(h->B, wide_group(h) == 2 ? h->winfo2.max_clusters : h->winfo.max_clusters);
             else if (e == OPO_ENGINE_RESIDENT) *out = std::min(h->B, h->rinfo.max_clusters);
             else if (e == OPO_ENGINE_LARGE) *out = h->linfo.grid;
             else *out = (long long)h->B * h->F;

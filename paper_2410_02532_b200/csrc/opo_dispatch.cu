@@ -16,7 +16,7 @@ namespace opo {
     cudaError_t launch_solo_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));      \
     cudaError_t launch_solo_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak)); \
     cudaError_t launch_solo_train_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak)); \
-    cudaError_t wide_info_##SUF##_L##LL(int, ResidentInfo*) __attribute__((weak));                            \
+    cudaError_t wide_info_##SUF##_L##LL(int, int, ResidentInfo*) __attribute__((weak));                       \
     cudaError_t launch_wide_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));      \
     cudaError_t launch_wide_dk0_##SUF##_L##LL(const ResidentArgs&, int, cudaStream_t) __attribute__((weak));
 
@@ -60,7 +60,7 @@ OPO_DECL_LARGE(f64, 14) OPO_DECL_LARGE(f64, 15) OPO_DECL_LARGE(f64, 16) OPO_DECL
         if (a.dk0) { OPO_SWITCH(launch_solo_dk0_, SUF, log2n, a, n_ctas, s) }                                     \
         OPO_SWITCH(launch_solo_, SUF, log2n, a, n_ctas, s)                                                        \
     }                                                                                                             \
-    cudaError_t wide_info_##SUF(int log2n, int n_fields, ResidentInfo* out) { OPO_SWITCH(wide_info_, SUF, log2n, n_fields, out) } \
+    cudaError_t wide_info_##SUF(int log2n, int n_fields, int g, ResidentInfo* out) { OPO_SWITCH(wide_info_, SUF, log2n, n_fields, g, out) } \
     cudaError_t launch_wide_##SUF(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s) {             \
         if (a.dk0) { OPO_SWITCH(launch_wide_dk0_, SUF, log2n, a, n_clusters, s) }                                 \
         OPO_SWITCH(launch_wide_, SUF, log2n, a, n_clusters, s)                                                    \

@@ -15,7 +15,7 @@ namespace opo {
 #if defined(OPO_DK0)
 cudaError_t OPO_NAME(launch_wide_dk0_)(const ResidentArgs& a, int n_clusters, cudaStream_t s) { return launch_wide_L<OPO_T, OPO_L, true>(a, n_clusters, s); }
 #else
-cudaError_t OPO_NAME(wide_info_)(int n_fields, ResidentInfo* out) { return wide_info_L<OPO_T, OPO_L>(n_fields, out); }
+cudaError_t OPO_NAME(wide_info_)(int n_fields, int g, ResidentInfo* out) { return wide_info_L<OPO_T, OPO_L>(n_fields, g, out); }
 cudaError_t OPO_NAME(launch_wide_)(const ResidentArgs& a, int n_clusters, cudaStream_t s) { return launch_wide_L<OPO_T, OPO_L, false>(a, n_clusters, s); }
 #endif
 

@@ -93,6 +93,7 @@ struct ResidentArgs {
     double h;
     int n_fields, batch, nz;   // nz = steps per pass
     int tab_cycle_mask;    // see tabH2
+    int wide_g;            // wide engine: sub-blocks per CTA (1: clusters of 4 F CTAs, 2: clusters of 2 F CTAs)
     int mode;              // 0 = propagate `steps` z-steps from step index z0; 1 = `steps` round trips
     int split;             // 1 (mode 1 only): work is dealt to the clusters in round trips, not instances (opo_resident.cuh)
     int* flags;            // [B][F] round trips completed per (instance, field), zeroed before a split launch
@@ -171,7 +172,7 @@ struct LargeInfo {
     cudaError_t launch_resident_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
     cudaError_t solo_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);         \
     cudaError_t launch_solo_##SUFFIX(int log2n, const ResidentArgs& a, int n_ctas, cudaStream_t s); \
-    cudaError_t wide_info_##SUFFIX(int log2n, int n_fields, ResidentInfo* out);         \
+    cudaError_t wide_info_##SUFFIX(int log2n, int n_fields, int g, ResidentInfo* out);  \
     cudaError_t launch_wide_##SUFFIX(int log2n, const ResidentArgs& a, int n_clusters, cudaStream_t s); \
     cudaError_t large_info_##SUFFIX(int log2n, int n_fields, int batch, int sm_count, LargeInfo* out);       \
     cudaError_t launch_large_##SUFFIX(int log2n, const LargeArgs& a, int grid, cudaStream_t s);

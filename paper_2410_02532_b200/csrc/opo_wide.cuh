@@ -43,30 +43,41 @@
 
 namespace opo {
 
-template <class T, int L, int F> struct wide_layout {
+// G: sub-blocks ("virtual ranks") per CTA.  G = 1: a cluster of 4 F CTAs, the lowest latency for one instance (7 such
+// clusters of 12 are co-resident on a B200).  G = 2: a cluster of 2 F CTAs with two groups of threads, each group the
+// complete machinery of one virtual rank -- its own sub-block, staging slots, barriers and named CTA barrier -- so three
+// times as many instances run at once (22 clusters of 6, a portable cluster size), each a little slower: the engine of
+// sweeps of a dozen instances (BASELINE.json configs[2]).
+template <class T, int L, int F, int G = 1> struct wide_layout {
     using PL = plan<L>;
-    static constexpr int C = 4;                              // CTAs per field = sub-blocks left by the radix-4 pass 0
-    static constexpr int NCTA = C * F;                       // cluster size: 8 (two-wave) or 12 (three-wave: a non-portable size)
+    static constexpr int C = 4;                              // sub-blocks left by the radix-4 pass 0 = virtual ranks per field
+    static constexpr int NV = C * F;                         // virtual ranks of an instance
+    static constexpr int NCTA = NV / G;                      // cluster size: 8 / 12 (G = 1; 12 is a non-portable size), 4 / 6 (G = 2)
     static constexpr int S = 1 << (L - 2);                   // points of a sub-block = number of pass-0 butterflies
-    static constexpr int NT = S / 16;                        // one radix-16 pass-1 butterfly per thread
-    static constexpr int NW = NT / 32;                       // warps per CTA = classes
+    static constexpr int NT = S / 16;                        // threads of a group: one radix-16 pass-1 butterfly per thread
+    static constexpr int NW = NT / 32;                       // warps of a group = classes
     static constexpr int TPC = 16;                           // tiles (of 32 pass-0 butterflies) per class: S / 32 / NW
-    // core warps own TPC / NCTA tiles each (rounded down); the EX tiles left over go to NH helper warps per CTA, one each
-    static constexpr int MAXT = TPC / NCTA;                  // tiles per core warp: 2 (two fields), 1 (three fields)
-    static constexpr int EX = (TPC - MAXT * NCTA) * NW;      // tiles of the cluster no core warp owns: 0 / 4 NW
+    // G = 1: core warps own TPC / NV tiles each (rounded down); the EX tiles left over go to NH helper warps per CTA, one each.
+    // G = 2: no helpers (the registers of 512 core threads are all there is); a warp owns up to ceil(TPC / NV) tiles.
+    static constexpr bool HELP = G == 1;
+    static constexpr int MAXT = HELP ? TPC / NV : (TPC + NV - 1) / NV;      // tiles per core warp
+    static constexpr int EX = HELP ? (TPC - MAXT * NV) * NW : 0;            // tiles of the cluster no core warp owns
     static constexpr int NH = (EX + NCTA - 1) / NCTA;        // helper warps per CTA
-    static constexpr int NTH = NT + 32 * NH;                 // threads per CTA
-    static constexpr int NSLOT = NW * MAXT + NH;             // staging slots (one per owned tile)
-    static constexpr bool ok = PL::P == 4 && PL::rbits(0) == 2 && PL::rbits(1) == 4 && NT >= 32;
-    static constexpr size_t field_bytes = (size_t)padded_len<T>(S) * sizeof(cplx<T>);
+    static constexpr int NCORE = G * NT;                     // core threads per CTA
+    static constexpr int NTH = NCORE + 32 * NH;              // threads per CTA
+    static constexpr int NSLOT = G * NW * MAXT + NH;         // staging slots (one per owned tile)
+    static constexpr bool ok = PL::P == 4 && PL::rbits(0) == 2 && PL::rbits(1) == 4 && NT >= 32 && NV % G == 0 && C % G == 0;
+    static constexpr size_t field_bytes = (size_t)padded_len<T>(S) * sizeof(cplx<T>);       // one sub-block
+    static constexpr size_t tw_offset_bytes = (size_t)G * field_bytes;
     static constexpr size_t tw_bytes = (size_t)PL::tw_local_count * sizeof(cplx<T>);
-    static constexpr int NQ = C * F;                         // operands of a pass-0 butterfly over all fields
-    // staging buffer of the fused phase: [slot][field, sub-block][lane]; slot = warp MAXT + tile (core warps), NW MAXT + h (helpers)
-    static constexpr size_t stage_offset = (field_bytes + tw_bytes + 15) / 16 * 16;
+    static constexpr int NQ = NV;                            // operands of a pass-0 butterfly over all fields
+    // staging buffer of the fused phase: [slot][field, sub-block][lane]; slot = (group NW + warp) MAXT + tile (core warps),
+    // G NW MAXT + h (helpers)
+    static constexpr size_t stage_offset = (tw_offset_bytes + tw_bytes + 15) / 16 * 16;
     static constexpr size_t stage_bytes = (size_t)(NSLOT > 0 ? NSLOT : 1) * NQ * 32 * sizeof(cplx<T>);
-    static constexpr size_t mbar_offset = stage_offset + stage_bytes;           // ready[NW], done[NW], helper_ready[NH]
-    static constexpr size_t total = mbar_offset + 8 * (size_t)(2 * NW + NH) + 8;
-    static constexpr uint32_t done_bytes = TPC * 32 * (uint32_t)sizeof(cplx<T>);      // results per class and phase arriving in a CTA
+    static constexpr size_t mbar_offset = stage_offset + stage_bytes;           // per group ready[NW], done[NW]; then helper_ready[NH]
+    static constexpr size_t total = mbar_offset + 8 * (size_t)(G * 2 * NW + NH) + 8;
+    static constexpr uint32_t done_bytes = TPC * 32 * (uint32_t)sizeof(cplx<T>);      // results per class and phase arriving in a sub-block
 };
 
 // distributed shared memory through 32-bit shared::cluster addresses (half the address registers of generic pointers)
@@ -106,29 +117,31 @@ __device__ __forceinline__ void mbar_arm(uint32_t addr, uint32_t bytes) {
 }
 
 struct WideFlow {
-    uint32_t mb;         // shared address of ready[0]; done[c] = mb + 8 (NW + c)
-    uint32_t stage;      // shared address of the staging buffer
-    int q_me;            // my operand slot 4 x + j in a staged butterfly
+    uint32_t mb;         // shared address of my group's ready[0]; done[c] = mb + 8 (NW + c)
+    uint32_t mb0;        // shared address of the CTA's first barrier (group 0)
+    uint32_t stage;      // shared address of the CTA's staging buffer
+    int q_me;            // my virtual rank 4 x + j = my operand slot in a staged butterfly
     int wait_in;         // forward pass 1 waits for done[warp] (a fused phase precedes)
     int push_out;        // inverse pass 1 sends its results to the owners of their tiles (a fused phase follows); else in place
     uint32_t par_done;
 };
 
-// The 16 values v[m] = elements t' + (S/16) m of this thread's pass-1 butterfly t' (class c = warp) go to the warps that own
-// the tiles c + NW m.  m < MAXT NCTA: core warp c of CTA (m + 4 c) mod NCTA, its tile m / NCTA; the others: tile number
-// e = (m - MAXT NCTA) NW + c of the left-over tiles, helper e / NCTA of CTA e mod NCTA.  Operand slot q_me, lane t' mod 32.
-template <class T, int NW, int NCTA, int MAXT, int NQ>
-__device__ __forceinline__ void wide_push16(const cplx<T>* v, const WideFlow& fa, int warp, int lane) {
+// The 16 values v[m] = elements t' + (S/16) m of this thread's pass-1 butterfly t' (class c = its warp inside the group) go to
+// the warps that own the tiles c + NW m.  m < MAXT NV: warp c of virtual rank (m + 4 c) mod NV -- CTA vr / G, group vr mod G --
+// its tile m / NV; the others (G = 1): tile number e = (m - MAXT NV) NW + c of the left-over tiles, helper e / NV of CTA
+// e mod NV.  Operand slot q_me, lane t' mod 32.
+template <class T, int NW, int NV, int G, int MAXT, int NQ>
+__device__ __forceinline__ void wide_push16(const cplx<T>* v, const WideFlow& fa, int c, int lane) {
     constexpr uint32_t SLOT = (uint32_t)(NQ * 32 * sizeof(cplx<T>));
     const uint32_t base = fa.stage + (uint32_t)(fa.q_me * 32 + lane) * (uint32_t)sizeof(cplx<T>);
 #pragma unroll
     for (int m = 0; m < 16; ++m) {
-        if (m < MAXT * NCTA) {
-            const int owner = (m + 4 * warp) % NCTA;
-            st_async(dsmem_addr(base + (uint32_t)(warp * MAXT + m / NCTA) * SLOT, owner), v[m], dsmem_addr(fa.mb + 8 * warp, owner));
+        if (m < MAXT * NV) {
+            const int vo = (m + 4 * c) % NV, cta = vo / G, go = vo % G;
+            st_async(dsmem_addr(base + (uint32_t)((go * NW + c) * MAXT + m / NV) * SLOT, cta), v[m], dsmem_addr(fa.mb0 + 8 * (go * 2 * NW + c), cta));
         } else {
-            const int e = (m - MAXT * NCTA) * NW + warp, owner = e % NCTA, hlp = e / NCTA;
-            st_async(dsmem_addr(base + (uint32_t)(NW * MAXT + hlp) * SLOT, owner), v[m], dsmem_addr(fa.mb + 8 * (2 * NW + hlp), owner));
+            const int e = (m - MAXT * NV) * NW + c, owner = e % NV, hlp = e / NV;
+            st_async(dsmem_addr(base + (uint32_t)(NW * MAXT + hlp) * SLOT, owner), v[m], dsmem_addr(fa.mb0 + 8 * (2 * NW + hlp), owner));
         }
     }
 }
@@ -139,16 +152,17 @@ __device__ __forceinline__ void wide_push16(const cplx<T>* v, const WideFlow& fa
 // field, kept for the later round trips).
 // KM: constant mode of the butterflies (kconst in opo_fft.cuh; fp32: the z-step loop runs kConstBunch - 1 applications with
 // the high parts of the compile-time roots alone and one that carries kConstBunch low parts)
-template <class T, int L, int NT, int NCTA, int MAXT, int NQ, int KM = 0>
+// tid: index inside the group; bar_id: the group's named CTA barrier
+template <class T, int L, int NT, int NV, int G, int MAXT, int NQ, int KM = 0>
 __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const cplx<T>* __restrict__ tab, int j, int tid, WideFlow fa,
-                                       cplx<T>* __restrict__ sh_keep) {
+                                       cplx<T>* __restrict__ sh_keep, int bar_id) {
     using PL = plan<L>;
     constexpr int NW = NT / 32, S = 1 << (L - 2);
     constexpr int RBL = PL::rbits(3), R = 1 << RBL, NBF = (1 << L) >> RBL, NBL = S >> RBL;
     constexpr int NB2 = S >> PL::rbits(2);
     constexpr bool chain = PL::rbits(2) == RBL && NBL % NT == 0;     // N = 2^14: passes 2, 3, 2 stay inside a warp's blocks
     const int warp = tid >> 5, lane = tid & 31;
-    auto core_bar = [] { asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); };      // the core threads only (helper warps do not come here)
+    auto core_bar = [bar_id] { asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(NT) : "memory"); };      // the threads of this group only
     if (fa.wait_in) {
         mbar_wait_cta(fa.mb + 8 * (NW + warp), fa.par_done);      // (acquire at CTA scope: the bytes counted on the barrier are visible, and L1 is left alone)
         if (lane == 0) mbar_arm(fa.mb + 8 * (NW + warp), 16u * 32u * (uint32_t)sizeof(cplx<T>));       // the results of the next fused phase
@@ -199,7 +213,7 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
 #pragma unroll
         for (int k = 1; k < R1; ++k) v[k] = cmulc(v[k], w[((k - 1) << SB) + tid]);
         dit_inv<T, R1, KM>::run(v);
-        wide_push16<T, NW, NCTA, MAXT, NQ>(v, fa, warp, lane);
+        wide_push16<T, NW, NV, G, MAXT, NQ>(v, fa, warp, lane);
         if (sh_keep != nullptr) {
 #pragma unroll
             for (int m = 0; m < R1; ++m) sh_keep[tid + NT * m] = v[m];
@@ -209,65 +223,70 @@ __device__ __noinline__ void wide_core(cplx<T>* smv, const cplx<T>* twl, const c
 
 enum { WIDE_RK4 = 0, WIDE_FWD0 = 1, WIDE_INV0 = 2 };
 
-template <class T, int L, int F, bool DK0 = false>
-__global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentArgs a) {
-    using WL = wide_layout<T, L, F>;
+template <class T, int L, int F, bool DK0 = false, int G = 1>
+__global__ void __launch_bounds__(wide_layout<T, L, F, G>::NTH, 1) k_wide(ResidentArgs a) {
+    using WL = wide_layout<T, L, F, G>;
     using PL = plan<L>;
     static_assert(WL::ok, "wide engine: N = 4 . 16 . r . r'");
-    constexpr int N = 1 << L, S = WL::S, NT = WL::NT, NW = WL::NW, NCTA = WL::NCTA, R = 4;
+    constexpr int N = 1 << L, S = WL::S, NT = WL::NT, NW = WL::NW, NCTA = WL::NCTA, NV = WL::NV, R = 4;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw);          // my sub-block: local index i at sm[phys(i)]
     cg::cluster_group cluster = cg::this_cluster();
     const int rank = (int)cluster.block_rank();
-    const int x = rank / WL::C, j = rank % WL::C;               // my field, my sub-block
     const int cid = blockIdx.x / NCTA, n_clusters = gridDim.x / NCTA;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // a core warp belongs to group grp = one virtual rank: one pass-1 butterfly per thread, up to MAXT tiles; the warps behind
+    // the groups are helpers (G = 1): one tile each, no part in the core
+    const bool core = warp < G * NW;
+    const int grp = (G > 1 && core) ? warp / NW : 0, wc = core ? warp - grp * NW : 0, tid_g = tid - grp * NT;
+    const int vr = rank * G + grp;                               // my virtual rank
+    const int x = vr / WL::C, j = vr % WL::C;                    // my field (the same for every group of a CTA), my sub-block
+    cplx<T>* sm = reinterpret_cast<cplx<T>*>(smem_raw + (size_t)grp * WL::field_bytes);       // my sub-block: local index i at sm[phys(i)]
 
-    uint32_t fld[F][R];                                          // sub-block k of field f, wherever it lives in the cluster
-#pragma unroll
-    for (int f = 0; f < F; ++f)
-#pragma unroll
-        for (int k = 0; k < R; ++k) fld[f][k] = dsmem_addr((uint32_t)__cvta_generic_to_shared(sm), f * WL::C + k);
+    // sub-block k of field f, wherever it lives in the cluster: CTA (4 f + k) / G, group (4 f + k) mod G (one mapa where it is
+    // used: twelve addresses kept in registers cost the two-group variant, which has 128 registers per thread, more in spills)
+    const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+    auto fld = [smem0](int f, int k) -> uint32_t {
+        return dsmem_addr(smem0 + (uint32_t)(((f * WL::C + k) % G) * WL::field_bytes), (f * WL::C + k) / G);
+    };
     cplx<T>* const smv = sm - phys<T>(j * S);                    // phys(j S + i) = phys(j S) + phys(i): S is a multiple of the pad period
 
     const cplx<T>* tw = reinterpret_cast<const cplx<T>*>(a.tw);
     {   // shared-memory copy of the twiddles of the local passes, addressed as the global table is
-        cplx<T>* d = reinterpret_cast<cplx<T>*>(smem_raw + WL::field_bytes);
+        cplx<T>* d = reinterpret_cast<cplx<T>*>(smem_raw + WL::tw_offset_bytes);
         for (int i = tid; i < PL::tw_local_count; i += WL::NTH) d[i] = ldg(&tw[PL::tw_local_begin + i]);
     }
-    const cplx<T>* twl = reinterpret_cast<const cplx<T>*>(smem_raw + WL::field_bytes) - PL::tw_local_begin;
-    const uint32_t mb = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::mbar_offset);
+    const cplx<T>* twl = reinterpret_cast<const cplx<T>*>(smem_raw + WL::tw_offset_bytes) - PL::tw_local_begin;
+    const uint32_t mb0 = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::mbar_offset);
+    const uint32_t mb = mb0 + 8 * (grp * 2 * NW);                // my group's ready[0]
     if (tid == 0) {
-        for (int c = 0; c < NW; ++c) {
-            mbar_init(mb + 8 * c, 1);                 // ready[c]: the operands of warp c's tiles have arrived in its staging buffer
-            mbar_init(mb + 8 * (NW + c), 1);          // done[c] : the results of all tiles of class c have arrived in my field
-        }
-        for (int hh = 0; hh < WL::NH; ++hh) mbar_init(mb + 8 * (2 * NW + hh), 1);      // the operands of helper hh's tile have arrived
+        for (int c = 0; c < G * 2 * NW; ++c) mbar_init(mb0 + 8 * c, 1);
+        // per group ready[c]: the operands of warp c's tiles have arrived in its staging slots; done[c]: the results of all tiles
+        // of class c have arrived in the group's sub-block
+        for (int hh = 0; hh < WL::NH; ++hh) mbar_init(mb0 + 8 * (G * 2 * NW + hh), 1);      // the operands of helper hh's tile have arrived
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     cluster.sync();       // every CTA's barriers exist (and its twiddle copy is complete) before anybody sends to them
 
     // this thread's pass-0 butterflies -- the same at every z-step -- and their twiddles
-    const bool core = warp < NW;                  // a core warp: one pass-1 butterfly per thread, MAXT tiles; else a helper: one tile
     int nt_own = 0;
-    int cls = warp;                               // class of my tiles
+    int cls = wc;                                 // class of my tiles
     int p_own[WL::MAXT];
     cplx<T> w0[WL::MAXT][R - 1];
     {
-        int m = ((rank - 4 * warp) % NCTA + NCTA) % NCTA;        // tile m < MAXT NCTA of class c goes to CTA (m + 4 c) mod NCTA
+        int m = ((vr - 4 * wc) % NV + NV) % NV;                  // tile m < MAXT NV of class c goes to virtual rank (m + 4 c) mod NV
         int n_mine = WL::MAXT;
-        if (!core) {                                             // left-over tile e = hlp NCTA + rank: class e mod NW
-            const int e = (warp - NW) * NCTA + rank;
+        if (!core) {                                             // (G = 1) left-over tile e = hlp NV + rank: class e mod NW
+            const int e = (warp - NW) * NV + rank;
             cls = e % NW;
-            m = WL::MAXT * NCTA + e / NW;
+            m = WL::MAXT * NV + e / NW;
             n_mine = e < WL::EX ? 1 : 0;
         }
 #pragma unroll
-        for (int i = 0; i < WL::MAXT; ++i, m += NCTA) {
+        for (int i = 0; i < WL::MAXT; ++i, m += NV) {
             p_own[i] = 0;
 #pragma unroll
             for (int k = 0; k < R - 1; ++k) w0[i][k] = cplx<T>{(T)1, (T)0};
-            if (i < n_mine) {
+            if (i < n_mine && m < WL::TPC) {
                 const int t = (cls + NW * m) * 32 + lane;
                 p_own[i] = phys<T>(t) * (int)sizeof(cplx<T>);       // byte offset inside a sub-block
 #pragma unroll
@@ -281,18 +300,19 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
     // (mbar_arm) -- and completes when those bytes have landed.  A warp arms the next phase right after its wait; bytes that
     // arrive before the arming leave the count negative for a moment, which the barrier allows.
     const uint32_t ready_bytes = (uint32_t)nt_own * WL::NQ * 32 * (uint32_t)sizeof(cplx<T>);
-    const uint32_t my_ready = mb + 8 * (core ? warp : 2 * NW + (warp - NW));
+    const uint32_t my_ready = core ? mb + 8 * wc : mb0 + 8 * (G * 2 * NW + (warp - G * NW));
     if (lane == 0) {
         if (nt_own > 0) mbar_arm(my_ready, ready_bytes);
-        if (core) mbar_arm(mb + 8 * (NW + warp), WL::done_bytes);
+        if (core) mbar_arm(mb + 8 * (NW + wc), WL::done_bytes);
     }
     WideFlow fb;
     fb.mb = mb;
+    fb.mb0 = mb0;
     fb.stage = (uint32_t)__cvta_generic_to_shared(smem_raw + WL::stage_offset);
-    fb.q_me = rank;
+    fb.q_me = vr;
     fb.wait_in = 0; fb.push_out = 0; fb.par_done = 0;
     const cplx<T>* stg = reinterpret_cast<const cplx<T>*>(smem_raw + WL::stage_offset) +
-                         (size_t)(core ? warp * WL::MAXT : NW * WL::MAXT + (warp - NW)) * WL::NQ * 32 + lane;       // my staging slot(s)
+                         (size_t)(core ? (grp * NW + wc) * WL::MAXT : G * NW * WL::MAXT + (warp - G * NW)) * WL::NQ * 32 + lane;       // my staging slot(s)
 
     T kap[3] = {(T)a.kappa[0], (T)a.kappa[1], (T)a.kappa[2]};
     const T h = (T)a.h;
@@ -321,7 +341,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                     for (int f = 0; f < F; ++f) {
                         if (!((mask >> f) & 1)) continue;
 #pragma unroll
-                        for (int k = 0; k < R; ++k) v[i][f][k] = dsmem_ld(fld[f][k] + p_own[i], cplx<T>{});
+                        for (int k = 0; k < R; ++k) v[i][f][k] = dsmem_ld(fld(f, k) + p_own[i], cplx<T>{});
                     }
                 }
             }
@@ -365,9 +385,14 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                     }
 #pragma unroll
                     for (int k = 0; k < R; ++k) {
-                        if constexpr (MODE == WIDE_RK4)
-                            st_async(fld[f][k] + p_own[i], v[i][f][k], fld[f][k] + (uint32_t)(WL::mbar_offset + 8 * (NW + cls)));    // counted on done[class] of the owner
-                        else dsmem_st(fld[f][k] + p_own[i], v[i][f][k]);
+                        if constexpr (MODE == WIDE_RK4) {
+                            // counted on done[class] of the owner: its group go = (4 f + k) mod G of its CTA
+                            const uint32_t dst = fld(f, k);
+                            st_async(dst + p_own[i], v[i][f][k],
+                                     dst + (uint32_t)(WL::mbar_offset - ((f * WL::C + k) % G) * WL::field_bytes + 8 * (((f * WL::C + k) % G) * 2 * NW + NW + cls)));
+                        } else {
+                            dsmem_st(fld(f, k) + p_own[i], v[i][f][k]);
+                        }
                     }
                 }
             }
@@ -393,7 +418,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
         if (core) {
             const cplx<T>* __restrict__ g = cur;
 #pragma unroll 4
-            for (int i = tid; i < S; i += NT) sm[phys<T>(i)] = g[i];
+            for (int i = tid_g; i < S; i += NT) sm[phys<T>(i)] = g[i];
         }
         cluster_bar();                                    // every sub-block of the instance is on chip
         tiles(tag_fwd0{}, (1 << F) - 1, one, one, one);
@@ -418,27 +443,27 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 WideFlow fa = fb;
                 fa.wait_in = 1; fa.par_done = (fz - 1) & 1;
                 fa.push_out = 0;
-                wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, reinterpret_cast<const cplx<T>*>(a.tabHG[x]) + (size_t)b * a.tab_stride[x], j, tid, fa, nullptr);
+                wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ>(smv, twl, reinterpret_cast<const cplx<T>*>(a.tabHG[x]) + (size_t)b * a.tab_stride[x], j, tid_g, fa, nullptr, 1 + grp);
             } else if (crossing && !resonant) {
                 // fresh pump / frozen seed, already half-stepped: a thread sends the elements of its own pass-1
                 // butterfly, i.e. of its class, to the tiles' owners as an inverse pass 1 would
-                mbar_wait_cta(mb + 8 * (NW + warp), (fz - 1) & 1);
-                if (lane == 0) mbar_arm(mb + 8 * (NW + warp), WL::done_bytes);
+                mbar_wait_cta(mb + 8 * (NW + wc), (fz - 1) & 1);
+                if (lane == 0) mbar_arm(mb + 8 * (NW + wc), WL::done_bytes);
                 const cplx<T>* __restrict__ g = SH;
                 cplx<T> v[16];
 #pragma unroll
-                for (int k = 0; k < 16; ++k) v[k] = g[tid + NT * k];
-                wide_push16<T, NW, NCTA, WL::MAXT, WL::NQ>(v, fb, warp, lane);
+                for (int k = 0; k < 16; ++k) v[k] = g[tid_g + NT * k];
+                wide_push16<T, NW, NV, G, WL::MAXT, WL::NQ>(v, fb, wc, lane);
             } else {
                 const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2 + (size_t)(q & a.tab_cycle_mask) * N);
                 WideFlow fa = fb;
                 fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
                 fa.push_out = q < total;
                 if constexpr (sizeof(T) == 4) {
-                    if ((q & (kConstBunch - 1)) == 0) wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ, 2>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
-                    else wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ, 1>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
+                    if ((q & (kConstBunch - 1)) == 0) wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ, 2>(smv, twl, tab, j, tid_g, fa, keep ? SH : nullptr, 1 + grp);
+                    else wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ, 1>(smv, twl, tab, j, tid_g, fa, keep ? SH : nullptr, 1 + grp);
                 } else {
-                    wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid, fa, keep ? SH : nullptr);
+                    wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid_g, fa, keep ? SH : nullptr, 1 + grp);
                 }
             }
             if (crossing && mask_eom) {         // uniform over the cluster
@@ -450,7 +475,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 if (core && my_eom) {
                     const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]) + (size_t)j * S;
 #pragma unroll 4
-                    for (int i = tid; i < S; i += NT) sm[phys<T>(i)] = cmul(sm[phys<T>(i)], ldg(&E[i]));
+                    for (int i = tid_g; i < S; i += NT) sm[phys<T>(i)] = cmul(sm[phys<T>(i)], ldg(&E[i]));
                 }
                 cluster_bar();
                 tiles(tag_fwd0{}, mask_eom, one, one, one);
@@ -458,7 +483,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 if (core && my_eom) {
                     WideFlow fa = fb;
                     fa.wait_in = 0; fa.push_out = 1;
-                    wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tabH, j, tid, fa, nullptr);
+                    wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ>(smv, twl, tabH, j, tid_g, fa, nullptr, 1 + grp);
                 }
             }
             if (q == total) break;
@@ -477,13 +502,13 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
             if (core) {
                 cplx<T>* __restrict__ g = cur;
 #pragma unroll 4
-                for (int i = tid; i < S; i += NT) g[i] = sm[phys<T>(i)];
+                for (int i = tid_g; i < S; i += NT) g[i] = sm[phys<T>(i)];
             }
         } else {
             if (core) {   // fields at z = L of the last pass
                 cplx<T>* __restrict__ g = reinterpret_cast<cplx<T>*>(a.exitb[x]) + off;
 #pragma unroll 4
-                for (int i = tid; i < S; i += NT) g[i] = sm[phys<T>(i)];
+                for (int i = tid_g; i < S; i += NT) g[i] = sm[phys<T>(i)];
             }
             // mirror, spectral phase and phase modulator of the call's last round trip
             int maskb = 0;
@@ -496,7 +521,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 cluster_bar();
                 if (core && ((maskb >> x) & 1)) {
                     const cplx<T>* tabGM = reinterpret_cast<const cplx<T>*>(a.tabGM[x]) + (size_t)b * a.tab_stride[x];
-                    wide_core<T, L, NT, NCTA, WL::MAXT, WL::NQ>(smv, twl, tabGM, j, tid, fb, nullptr);
+                    wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ>(smv, twl, tabGM, j, tid_g, fb, nullptr, 1 + grp);
                 }
                 cluster_bar();
                 tiles(tag_inv0{}, maskb, one, one, one);
@@ -510,15 +535,15 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
                 if (!a.boundary_fft[x]) mf = ldg(reinterpret_cast<const cplx<T>*>(a.mirror[x]) + b);
                 if (E != nullptr) {
 #pragma unroll 4
-                    for (int i = tid; i < S; i += NT) cur[i] = cmul(cmul(sm[phys<T>(i)], mf), ldg(&E[j * S + i]));
+                    for (int i = tid_g; i < S; i += NT) cur[i] = cmul(cmul(sm[phys<T>(i)], mf), ldg(&E[j * S + i]));
                 } else {
 #pragma unroll 4
-                    for (int i = tid; i < S; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
+                    for (int i = tid_g; i < S; i += NT) cur[i] = cmul(sm[phys<T>(i)], mf);
                 }
             } else {
                 const cplx<T>* __restrict__ Sx = reinterpret_cast<const cplx<T>*>(a.S[x]) + off;
 #pragma unroll 4
-                for (int i = tid; i < S; i += NT) cur[i] = Sx[i];
+                for (int i = tid_g; i < S; i += NT) cur[i] = Sx[i];
             }
         }
         // the next instance's load overwrites shared memory that only this CTA reads from here on: all foreign
@@ -528,13 +553,13 @@ __global__ void __launch_bounds__(wide_layout<T, L, F>::NTH, 1) k_wide(ResidentA
     cluster.sync();     // keep shared memory alive until every peer has left its last tile phase
 }
 
-template <class T, int L, int F, bool DK0> cudaError_t wide_cfg(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, int n_clusters, cudaStream_t s) {
-    using WL = wide_layout<T, L, F>;
+template <class T, int L, int F, bool DK0, int G> cudaError_t wide_cfg(cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr, int n_clusters, cudaStream_t s) {
+    using WL = wide_layout<T, L, F, G>;
     static device_once once;
     cudaError_t e0 = once.run([&] {
-        cudaError_t e = cudaFuncSetAttribute(k_wide<T, L, F, DK0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WL::total);
+        cudaError_t e = cudaFuncSetAttribute(k_wide<T, L, F, DK0, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WL::total);
         if (e != cudaSuccess) return e;
-        if (WL::NCTA > 8) e = cudaFuncSetAttribute(k_wide<T, L, F, DK0>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (WL::NCTA > 8) e = cudaFuncSetAttribute(k_wide<T, L, F, DK0, G>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
         return e;
     });
     if (e0 != cudaSuccess) return e0;
@@ -551,40 +576,43 @@ template <class T, int L, int F, bool DK0> cudaError_t wide_cfg(cudaLaunchConfig
     return cudaSuccess;
 }
 
-template <class T, int L, int F> cudaError_t wide_info_LF(ResidentInfo* out) {
-    if constexpr (!wide_layout<T, L, F>::ok) {
+template <class T, int L, int F, int G> cudaError_t wide_info_LF(ResidentInfo* out) {
+    if constexpr (!wide_layout<T, L, F, G>::ok || wide_layout<T, L, F, G>::total > 232448) {
         return cudaErrorNotSupported;
     } else {
         cudaLaunchConfig_t cfg{};
         cudaLaunchAttribute attr[1];
-        cudaError_t e = wide_cfg<T, L, F, false>(&cfg, attr, 1, nullptr);
+        cudaError_t e = wide_cfg<T, L, F, false, G>(&cfg, attr, 1, nullptr);
         if (e != cudaSuccess) return e;
         int n = 0;
-        e = cudaOccupancyMaxActiveClusters(&n, k_wide<T, L, F, false>, &cfg);
+        e = cudaOccupancyMaxActiveClusters(&n, k_wide<T, L, F, false, G>, &cfg);
         if (e != cudaSuccess) return e;
-        out->threads = wide_layout<T, L, F>::NTH;
+        out->threads = wide_layout<T, L, F, G>::NTH;
         out->smem_bytes = cfg.dynamicSmemBytes;
         out->max_clusters = n;
         return cudaSuccess;
     }
 }
-template <class T, int L> cudaError_t wide_info_L(int n_fields, ResidentInfo* out) {
-    return n_fields == 3 ? wide_info_LF<T, L, 3>(out) : wide_info_LF<T, L, 2>(out);
+// g: sub-blocks per CTA (1: clusters of 4 F CTAs, 2: clusters of 2 F CTAs)
+template <class T, int L> cudaError_t wide_info_L(int n_fields, int g, ResidentInfo* out) {
+    if (g == 2) return n_fields == 3 ? wide_info_LF<T, L, 3, 2>(out) : wide_info_LF<T, L, 2, 2>(out);
+    return n_fields == 3 ? wide_info_LF<T, L, 3, 1>(out) : wide_info_LF<T, L, 2, 1>(out);
 }
 
-template <class T, int L, int F, bool DK0> cudaError_t launch_wide_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
-    if constexpr (!wide_layout<T, L, F>::ok) {
+template <class T, int L, int F, bool DK0, int G> cudaError_t launch_wide_LF(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
+    if constexpr (!wide_layout<T, L, F, G>::ok || wide_layout<T, L, F, G>::total > 232448) {
         return cudaErrorNotSupported;
     } else {
         cudaLaunchConfig_t cfg{};
         cudaLaunchAttribute attr[1];
-        cudaError_t e = wide_cfg<T, L, F, DK0>(&cfg, attr, n_clusters, s);
+        cudaError_t e = wide_cfg<T, L, F, DK0, G>(&cfg, attr, n_clusters, s);
         if (e != cudaSuccess) return e;
-        return cudaLaunchKernelEx(&cfg, k_wide<T, L, F, DK0>, a);
+        return cudaLaunchKernelEx(&cfg, k_wide<T, L, F, DK0, G>, a);
     }
 }
 template <class T, int L, bool DK0> cudaError_t launch_wide_L(const ResidentArgs& a, int n_clusters, cudaStream_t s) {
-    return a.n_fields == 3 ? launch_wide_LF<T, L, 3, DK0>(a, n_clusters, s) : launch_wide_LF<T, L, 2, DK0>(a, n_clusters, s);
+    if (a.wide_g == 2) return a.n_fields == 3 ? launch_wide_LF<T, L, 3, DK0, 2>(a, n_clusters, s) : launch_wide_LF<T, L, 2, DK0, 2>(a, n_clusters, s);
+    return a.n_fields == 3 ? launch_wide_LF<T, L, 3, DK0, 1>(a, n_clusters, s) : launch_wide_LF<T, L, 2, DK0, 1>(a, n_clusters, s);
 }
 
 }  // namespace opo

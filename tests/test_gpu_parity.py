@@ -333,6 +333,32 @@ def test_wide_engine_many_instances_bitwise_repeatable(precision, log2_n, n_fiel
     assert_close(runs[0][0], cur2, 1e-12 if precision == "c128" else 1e-5, "wide vs cluster engine, current")
 
 
+@pytest.mark.parametrize("precision,log2_n,n_fields,batch", [("c64", 12, 3, 5), ("c64", 13, 2, 4), ("c64", 14, 3, 3), ("c128", 13, 3, 2), ("c64", 12, 3, 61)])
+def test_wide_engine_two_subblocks_per_cta_is_bitwise_the_same(precision, log2_n, n_fields, batch):
+    """OPO_OPT_WIDE_SUBBLOCKS = 2 (clusters of 2 F CTAs, two virtual ranks per CTA) performs exactly the arithmetic of the
+    clusters of 4 F CTAs, thread for thread: the results agree bit for bit; and AUTO picks it where it finishes sooner."""
+    torch, P = _gpu()
+    w = small_workload(log2_n, n_fields, precision, nz=4, batch=batch, dk=-20.0, gdd_dt2=-1.7, drad=0.4, strong=False)
+    w.delta_T_signal_s = (np.arange(batch) % 5 - 2.0) * 1.25 * w.dt
+    if n_fields == 3:
+        w.resonant = [0, 1, 0]
+    _engine_or_skip(w, P.ENGINE_WIDE)
+    res = {}
+    for g in (1, 2):
+        o = P.from_workload(w, engine=P.ENGINE_WIDE)
+        P.opo_set_option(o._h, P.OPT_WIDE_SUBBLOCKS, g)
+        slots = int(P.opo_get_info(o._h, P.INFO_SLOTS))
+        o.roundtrips(3)
+        o.sync()
+        res[g] = (np.stack([o.get_fields(x, P.WHICH_EXIT).cpu().numpy() for x in range(n_fields)]),
+                  np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy() for x in range(n_fields)]), slots)
+        o.close()
+    assert np.array_equal(res[1][0], res[2][0]) and np.array_equal(res[1][1], res[2][1])
+    assert res[2][2] >= res[1][2]               # more instances at once
+    if batch == 61:
+        assert res[2][2] >= 2 * res[1][2]
+
+
 def test_wide_engine_is_what_auto_picks_for_a_single_instance_and_falls_back():
     torch, P = _gpu()
     w = W.config1().truncated(1)
