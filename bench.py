@@ -61,6 +61,24 @@ def smem_bytes_per_field_point_zstep(precision: str) -> float:
     return 6 * 2 * (16 if precision == "c128" else 8)
 
 
+# The wide engine (one instance on a cluster of 4 F CTAs) is bound by the SM-to-SM link: every field value leaves its SM as an
+# operand of the pass-0 / RK4 phase and comes back as a result at every z-step.  Bytes through one
+# SM's port per z-step, sent and received: 2 directions x 2 crossings x esz x N F (NV - 1) / NV / n_ctas.  Peak: 16 B/clk per
+# SM, reads and writes together, measured in round 1 (profiles/r01d_dsmem_microbench.md) -- not re-measured in this run.
+def wide_link_roofline(w, o, P, units_per_step, avg_s, sm_ghz):
+    esz = 16 if w.precision == "c128" else 8
+    nv = 4 * w.n_fields
+    slots = int(P.opo_get_info(o._h, P.INFO_SLOTS))
+    waves = -(-w.batch // max(1, slots))
+    per_sm_per_zstep = 2 * 2 * esz * w.n * w.n_fields * (nv - 1) / nv / nv          # clusters of 4 F CTAs (one sub-block per CTA)
+    zsteps_per_sm = units_per_step / (w.batch * w.n) * waves                        # z-steps an SM works through, wave after wave
+    achieved = per_sm_per_zstep * zsteps_per_sm / avg_s / 1e9
+    peak = 16.0 * sm_ghz
+    return {"achieved": achieved, "peak": peak, "unit": "GB/s per SM", "frac": achieved / peak,
+            "note": "SM-to-SM link traffic of one SM (operands out, results back, both directions); peak = 16 B/clk per SM at the max SM "
+                    "clock, measured in round 1 (profiles/r01d_dsmem_microbench.md); assumes one sub-block per CTA"}
+
+
 def make_workload(name: str, rank: int):
     makers = {"C0": W.config0, "C1": W.config1, "C2": W.config2, "C3": W.config3, "C4": W.config4}
     if name not in makers:
@@ -333,6 +351,7 @@ def main():
                     "smem": {"achieved": smem_by / avg_s / 1e9, "peak": smem_peak, "unit": "GB/s", "frac": smem_by / avg_s / 1e9 / smem_peak,
                              "note": f"algorithmic shared-memory bytes = {smem_bytes_per_field_point_zstep(w.precision):.0f} B per field-point z-step "
                                      "(6 passes x read + write); peak = conflict-free 16 B loads + stores on every SM, measured in this run"},
+                    **({"link": wide_link_roofline(w, o, P, units_per_step, avg_s, sm_max_ghz)} if eng == P.ENGINE_WIDE else {}),
                     "note": f"peak = {'FP64' if dbl else 'FP32'} FMA throughput measured in this run by opo_selftest_peak (independent FMA chains on every SM); "
                             f"peak_nominal = {sms} SM x {64 if dbl else 128} lanes x 2 x {sm_max_ghz:.3f} GHz; "
                             f"algorithmic flops = {flops_per_grid_point_zstep(w.log2_n, w.n_fields):.0f}/grid-point z-step "
