@@ -342,6 +342,9 @@ def test_wide_engine_two_subblocks_per_cta_is_bitwise_the_same(precision, log2_n
     w.delta_T_signal_s = (np.arange(batch) % 5 - 2.0) * 1.25 * w.dt
     if n_fields == 3:
         w.resonant = [0, 1, 0]
+    if log2_n == 13:        # with a phase modulator on the signal: the crossing runs the in-place pass-0 phases
+        w.eom_beta_rad = [0.0, 0.8, 0.0][:n_fields]
+        w.eom_f_hz = [0.0, 2.0 / w.window_s, 0.0][:n_fields]
     _engine_or_skip(w, P.ENGINE_WIDE)
     res = {}
     for g in (1, 2):
