@@ -263,6 +263,36 @@ int opo_get_info(const opo_handle* h, int what, long long* out);
 #define OPO_PEAK_TMEM_ST 4
 int opo_selftest_peak(int what, double* out_value);
 
+/* Forward DFT of caller-owned rows WITHOUT a handle and without any device-memory allocation: the frequency read-out
+ * of opo_get_fields(.., OPO_DOMAIN_FREQ, ..) (same kernel, same tables, bit-identical result) for callers that cannot
+ * afford, or are not allowed, to call cudaMalloc.  Who that is: (1) a process whose framework allocator (PyTorch's caching
+ * allocator, an RMM pool, a lab control program's arena) has already taken the whole of HBM, so that a cudaMalloc of the
+ * library's own would fail although the caller has plenty of room inside its pool; (2) a measurement or feedback loop
+ * that looks at the spectrum every few round trips (PAPER.md:L449 writes spectra out; Listing 3 L279-297 is such a loop)
+ * and cannot take the device-wide synchronisation that cudaMalloc / cudaFree imply; (3) code that must prove, for a
+ * long unattended run, that its device footprint does not grow.  opo_create, by contrast, allocates state and tables.
+ *     dev_in, dev_out : device pointers on the current device, [batch][N] interleaved (re, im), float2 (precision 0) or
+ *                       double2 (precision 1), 16-byte aligned, N = 2^log2_n; both stay the caller's; they may be the
+ *                       same buffer (each row is read completely before it is written).
+ *     result          : dev_out[b][k] = sum_n dev_in[b][n] exp(-2 pi i k n / N), unnormalised, natural order (see "Grid").
+ *     cuda_stream     : a cudaStream_t cast to void* (NULL = default stream); the launch is enqueued there.
+ * Limit: log2_n in 4 .. 14 for complex64, 4 .. 13 for complex128; anything longer returns OPO_ERR_UNSUPPORTED with a
+ * message naming the limit (use a handle for those).  batch is any positive int.
+ * Where the tables live instead: in a 192 KiB array that is part of the library image (a file-scope __device__ array
+ * in opo_api.cu).  Every GPU on which a CUDA context loads libopo.so carries these 192 KiB until the process exits,
+ * whether or not this function is ever called.
+ * First call on each device: looks up that device's address of the array and writes the tables (two host-to-device
+ * copies on cuda_stream followed by a wait for that stream).  Make this first call during start-up, before any stream
+ * capture is begun.  The same copy + wait happens again whenever (log2_n, precision) differ from the previous call on
+ * that device, because the array holds the tables of one size at a time and keeps them between calls.
+ * Concurrency: all calls on a device share the one array.  Calls with the same (log2_n, precision) only read it and
+ * may overlap freely.  A call with a different size rewrites it in the order of ITS stream only: if work from an
+ * earlier call with another size is still running on a different stream, the two race and that earlier result is
+ * garbage.  Keep such calls on one stream or put an event between them.  Host threads may call concurrently (the
+ * bookkeeping is under a mutex); the rule above is about what overlaps on the GPU.
+ * Calls no cudaMalloc / cudaFree / cuFFT.  Errors: status code, text via opo_last_error(NULL) of the calling thread. */
+int opo_spectrum_noalloc(const void* dev_in, void* dev_out, int log2_n, int batch, int precision, void* cuda_stream);
+
 /* Last error text of this handle (or of the failed opo_create when h is NULL).  Never NULL. */
 const char* opo_last_error(const opo_handle* h);
 

@@ -94,6 +94,7 @@ def lib() -> ctypes.CDLL:
         L.opo_get_info.argtypes = [vp, ci, ctypes.POINTER(ctypes.c_longlong)]
         L.opo_set_segments.argtypes = [vp, ci, ctypes.POINTER(opo_segment)]
         L.opo_selftest_peak.argtypes = [ci, ctypes.POINTER(ctypes.c_double)]
+        L.opo_spectrum_noalloc.argtypes = [vp, vp, ci, ci, ci, vp]
         L.opo_last_error.argtypes = [vp]
         L.opo_last_error.restype = ctypes.c_char_p
         for name in EXPORTS:
@@ -106,7 +107,7 @@ def lib() -> ctypes.CDLL:
 EXPORTS = ["opo_create", "opo_destroy", "opo_set_stream", "opo_set_batch_param", "opo_set_eom", "opo_set_beta3", "opo_set_pump",
            "opo_set_pump_host", "opo_set_field", "opo_set_field_host", "opo_propagate", "opo_roundtrips", "opo_roundtrips_train",
            "opo_get_fields", "opo_get_fields_host", "opo_sync", "opo_check_finite", "opo_get_z_steps",
-           "opo_set_option", "opo_get_info", "opo_selftest_peak", "opo_set_segments", "opo_last_error"]
+           "opo_set_option", "opo_get_info", "opo_selftest_peak", "opo_set_segments", "opo_spectrum_noalloc", "opo_last_error"]
 
 
 def _check(handle, status: int):
@@ -231,6 +232,15 @@ def opo_selftest_peak(what: int) -> float:
     out = ctypes.c_double()
     _check(None, lib().opo_selftest_peak(what, ctypes.byref(out)))
     return out.value
+
+
+def opo_spectrum_noalloc(dev_in: int, dev_out: int, log2_n: int, batch: int, precision: int, cuda_stream: int = 0):
+    """Forward DFT of [batch][2^log2_n] rows the caller owns, with no handle and no device allocation inside the library
+    (include/opo.h: for callers whose memory pool owns all of HBM, or whose loop cannot take cudaMalloc's device-wide
+    synchronisation).  Pointers are raw device addresses (tensor.data_ptr()); the tables live in a fixed 192 KiB array
+    inside libopo.so, so rows are limited to 2^14 points (complex64) / 2^13 (complex128)."""
+    _check(None, lib().opo_spectrum_noalloc(ctypes.c_void_p(dev_in), ctypes.c_void_p(dev_out), int(log2_n), int(batch), int(precision),
+                                            ctypes.c_void_p(cuda_stream) if cuda_stream else None))
 
 
 def opo_get_info(h, what: int) -> int:

@@ -8,6 +8,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1324,3 +1325,95 @@ int opo_get_info(const opo_handle* h, int what, long long* out) {
 }
 
 }  // extern "C"
+
+// ---- opo_spectrum_noalloc: the frequency read-out for callers that must not allocate device memory -------------------
+// The read-out kernel (k_freq, opo_kernels.cuh) needs two tables next to its input and output: the pass twiddles of the
+// transform and the map from the transform's digit-reversed positions to frequency indices.  A handle keeps them in
+// cudaMalloc'ed memory.  This entry point keeps them in the fixed array below instead, which is part of the library image:
+// the driver places it when the library is loaded on a GPU and takes it back at process exit, so no call here ever asks
+// the allocator for anything.
+//
+//   bytes [0, 128 KiB)         : pass twiddles, N - 1 entries of float2 (N <= 2^14) or double2 (N <= 2^13)
+//   bytes [128 KiB, 192 KiB)   : int32 position -> frequency index, N entries
+namespace {
+
+constexpr int kNoAllocMaxLog2C64 = 14, kNoAllocMaxLog2C128 = 13;
+constexpr size_t kNoAllocTwBytes = (size_t)8 << kNoAllocMaxLog2C64;       // = 16 << kNoAllocMaxLog2C128
+constexpr size_t kNoAllocPermBytes = (size_t)4 << kNoAllocMaxLog2C64;
+constexpr size_t kNoAllocBytes = kNoAllocTwBytes + kNoAllocPermBytes;     // 192 KiB on every GPU that loads libopo.so
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+// Host view of the array, one entry per device.  `base` is what cudaGetSymbolAddress returned with that device current: the
+// name g_noalloc_scratch itself means nothing to a kernel when it is written in host code.
+struct NoAllocDevice {
+    unsigned char* base = nullptr;
+    int log2_n = -1, precision = -1;      // which tables the array holds now (-1: none yet)
+};
+constexpr int kNoAllocMaxDevices = 64;
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mutex;               // host bookkeeping only; it orders nothing on the GPU
+
+}  // namespace
+
+extern "C" int opo_spectrum_noalloc(const void* dev_in, void* dev_out, int log2_n, int batch, int precision, void* cuda_stream) {
+    if (!dev_in || !dev_out) return fail(nullptr, OPO_ERR_INVALID_ARG, "opo_spectrum_noalloc: null buffer");
+    if (precision != OPO_PRECISION_C64 && precision != OPO_PRECISION_C128)
+        return fail(nullptr, OPO_ERR_INVALID_ARG, "opo_spectrum_noalloc: precision must be 0 (c64) or 1 (c128)");
+    if (batch <= 0) return fail(nullptr, OPO_ERR_INVALID_ARG, "opo_spectrum_noalloc: batch must be positive");
+    if (log2_n < opo::kMinLog2) return fail(nullptr, OPO_ERR_INVALID_ARG, "opo_spectrum_noalloc: log2_n below 4");
+    const bool dbl = precision == OPO_PRECISION_C128;
+    const int max_log2 = dbl ? kNoAllocMaxLog2C128 : kNoAllocMaxLog2C64;
+    if (log2_n > max_log2)
+        return fail(nullptr, OPO_ERR_UNSUPPORTED, "opo_spectrum_noalloc: N = 2^" + std::to_string(log2_n) + " does not fit the built-in table space (limit 2^" +
+                                                      std::to_string(max_log2) + " points per row at this precision); use a handle and opo_get_fields for longer rows");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(nullptr, OPO_ERR_CUDA, std::string("opo_spectrum_noalloc: no usable CUDA device: ") + cudaGetErrorString(cudaGetLastError()));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(nullptr, OPO_ERR_UNSUPPORTED, "opo_spectrum_noalloc: device ordinal above 63");
+
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoAllocDevice& d = g_noalloc_dev[dev];
+    if (!d.base) {
+        // set-up, once per device, with that device current: ask the runtime where this GPU's copy of the array lives
+        int major = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10)
+            return fail(nullptr, OPO_ERR_CUDA, "opo_spectrum_noalloc: libopo is built for sm_100a only");
+        unsigned char* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(nullptr, OPO_ERR_CUDA, std::string("opo_spectrum_noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        }
+        d.base = p;
+    }
+    const int N = 1 << log2_n;
+    if (d.log2_n != log2_n || d.precision != precision) {
+        // The array still holds the tables of the last call on this device; they serve only that size and precision.
+        // Overwrite them in stream order (earlier launches on `stream` finish reading first); launches on OTHER streams
+        // that are still reading them are not waited for -- see the header.
+        d.log2_n = d.precision = -1;
+        const HostPlan pl(log2_n);
+        const std::vector<cd> tw = pass_twiddles(pl);
+        std::vector<int> perm((size_t)N);
+        for (int pos = 0; pos < N; ++pos) perm[pos] = pl.freq_of_pos(pos);
+        cudaError_t e;
+        if (dbl) {
+            e = cudaMemcpyAsync(d.base, tw.data(), tw.size() * sizeof(cd), cudaMemcpyHostToDevice, stream);
+        } else {
+            std::vector<float> tmp(2 * tw.size());
+            for (size_t i = 0; i < tw.size(); ++i) round_unit(tw[i].real(), tw[i].imag(), &tmp[2 * i], &tmp[2 * i + 1]);
+            e = cudaMemcpyAsync(d.base, tmp.data(), tmp.size() * sizeof(float), cudaMemcpyHostToDevice, stream);
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d.base + kNoAllocTwBytes, perm.data(), perm.size() * sizeof(int), cudaMemcpyHostToDevice, stream);
+        // the sources are pageable temporaries: wait until the copies have left them
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        if (e != cudaSuccess) return fail(nullptr, OPO_ERR_CUDA, std::string("opo_spectrum_noalloc: table upload: ") + cudaGetErrorString(e));
+        d.log2_n = log2_n;
+        d.precision = precision;
+    }
+    const opo::FreqArgs a{dev_in, dev_out, reinterpret_cast<const int*>(d.base + kNoAllocTwBytes), d.base, batch};
+    const cudaError_t e = dbl ? opo::launch_freq_f64(log2_n, a, stream) : opo::launch_freq_f32(log2_n, a, stream);
+    if (e != cudaSuccess) return fail(nullptr, e == cudaErrorNotSupported ? OPO_ERR_UNSUPPORTED : OPO_ERR_CUDA, std::string("opo_spectrum_noalloc: launch: ") + cudaGetErrorString(e));
+    return OPO_OK;
+}
