@@ -44,6 +44,11 @@
  *     stream and never frees or keeps it.  The handle owns its state and tables.
  *   - Every call returns an opo_status.  No exceptions, no global state.  Handles are independent;
  *     one handle must not be used from two threads at once.
+ *   - A run may be cut into opo_propagate / opo_roundtrips calls in any way (z-step by z-step as in the paper's own loop,
+ *     PAPER.md:L266-297): the result is the same to rounding.  In complex64 the kernels cycle through several roundings of
+ *     the dispersion tables and apply constant corrections at every 8th operator; both follow the handle's running count
+ *     of operators since opo_create, which no call resets.  Hence two handles driven by the same sequence of calls agree
+ *     bit for bit, while a second run on a REUSED handle differs from the first at rounding level (1e-7 relative).
  *   - Calls enqueue work on the handle's stream and return; asynchronous faults surface at
  *     opo_sync or at the next call (OPO_ERR_CUDA).  There is no CPU fallback of any kind: without
  *     a usable sm_100 device opo_create fails with OPO_ERR_CUDA.

@@ -158,7 +158,13 @@ struct opo_handle {
     void* segHX[8][3] = {};                           //   H_j H_{j+1} / N across the junction of two crystals
     bool solo_ok = false;                             // solo engine (one CTA per instance, fields in shared + tensor memory)
     opo::ResidentInfo sinfo{};                        // max_clusters = co-resident CTAs on the device
-    int tab_cycle = 1;                                // roundings of H^2 cycled through by the on-chip engines (fp32: 16; build_tables)
+    int tab_cycle = 1;                                // roundings of H and of H^2 cycled through by the on-chip engines (fp32: 16; build_tables)
+    // Linear operators / half-step tables / full-step tables applied by this handle since opo_create (kept modulo 2^20, a
+    // multiple of every cycle length).  They go into every launch (ResidentArgs::op0, hq0, fq0; LargeArgs::op0) so that the
+    // table cycles and the bunched constant corrections continue across calls instead of restarting at each call's first
+    // operator: accuracy then does not depend on how a run is cut into opo_propagate / opo_roundtrips calls.  Never reset;
+    // two handles driven by the same sequence of calls give bitwise the same fields.
+    int op_count = 0, hq_count = 0, fq_count = 0;
     bool wide_ok = false;                             // wide engine (a cluster of 4 F CTAs per instance)
     opo::ResidentInfo winfo{};                        // max_clusters = co-resident clusters of 4 F CTAs
     int wide_g_opt = 0;                               // OPO_OPT_WIDE_SUBBLOCKS: 0 = AUTO, 1 | 2 = sub-blocks per CTA
@@ -302,6 +308,27 @@ int build_tables(opo_handle* h) {
     const double invN = 1.0 / (double)N;
     const double h0 = h->seg[0].hstep, hl = h->seg[K - 1].hstep;      // first and last step size of a pass
     std::vector<cd> Hh(N), M(N), lay(N), Dx(N);
+    // fp32, on-chip engines: a cycle of roundings of a table M (H^2, and likewise H) with error feedback.  One rounded table
+    // T = fl(M) puts the same 3e-8 of error per bin into every application (coherent: 3e4 z-steps of C4 turn it into ~5e-4).
+    // Here table j of the cycle is T_j = fl(M / r_{j-1}), r_j = r_{j-1} T_j / M the relative error of the product applied so
+    // far, so after any number of applications the product of the tables is M^n to ONE rounding, and the drift per
+    // application falls by the cycle length.  Copy 0 is fl(M) itself (the host-sequenced baseline engines, which do not
+    // cycle, use it).  The kernels pick the copy by the handle's running count of uses (op_count / hq_count / fq_count).
+    auto upload_cycle = [&](void* dst, const std::vector<cd>& Mt) -> int {
+        if (h->tab_cycle <= 1) return OPO_OK;
+        std::vector<cd> ratio(N, cd(1.0, 0.0));
+        for (int j = 0; j < h->tab_cycle; ++j) {
+            for (int k = 0; k < N; ++k) {
+                const cd want = Mt[k] / ratio[k];
+                const cd t((double)(float)want.real(), (double)(float)want.imag());
+                Hh[k] = t;
+                if (Mt[k] != cd(0.0, 0.0)) ratio[k] *= t / Mt[k];
+            }
+            to_engine_layout(h, pl, Hh.data(), lay.data());
+            if (int rc = upload_table(h, (char*)dst + (size_t)j * N * h->tab_esz, lay.data(), N)) return rc;
+        }
+        return OPO_OK;
+    };
     for (int x = 0; x < F; ++x) {
         const double db1 = h->fields.beta1_s_per_m[x] - h->fields.beta1_s_per_m[h->fields.ref_field];
         const double b2 = h->fields.beta2_s2_per_m[x], al = h->fields.alpha_per_m[x];
@@ -314,28 +341,13 @@ int build_tables(opo_handle* h) {
         for (int k = 0; k < N; ++k) M[k] = std::exp(Dx[k] * (0.5 * h0)) * invN;
         to_engine_layout(h, pl, M.data(), lay.data());
         if (int rc = upload_table(h, h->tabH[x], lay.data(), N)) return rc;
+        if (int rc = upload_cycle(h->tabH[x], M)) return rc;       // (the half-steps at the ends of every call: z-step-by-z-step
+                                                                   //  driving applies nothing else)
         if (h->natH[x]) if (int rc = upload_complex(h, h->natH[x], M.data(), N)) return rc;        // cuFFT baseline: natural order
         for (int k = 0; k < N; ++k) M[k] = std::exp(Dx[k] * h0) * invN;                            // H^2 evaluated directly in fp64
         to_engine_layout(h, pl, M.data(), lay.data());
         if (int rc = upload_table(h, h->tabH2[x], lay.data(), N)) return rc;
-        if (h->tab_cycle > 1) {
-            // fp32, on-chip engines: a cycle of roundings of H^2 with error feedback.  One rounded table T = fl(M) puts the same
-            // 3e-8 of error per bin into every z-step (coherent: 3e4 z-steps of C4 turn it into ~5e-4).  Here table j of the
-            // cycle is T_j = fl(M / r_{j-1}), r_j = r_{j-1} T_j / M the relative error of the product applied so far, so after
-            // any number of z-steps the product of the tables is M^n to ONE rounding, and the drift per z-step falls by the
-            // cycle length.  Copy 0 is fl(M) itself (the host-sequenced baseline engines, which do not cycle, use it).
-            std::vector<cd> ratio(N, cd(1.0, 0.0));
-            for (int j = 0; j < h->tab_cycle; ++j) {
-                for (int k = 0; k < N; ++k) {
-                    const cd want = M[k] / ratio[k];
-                    const cd t((double)(float)want.real(), (double)(float)want.imag());
-                    Hh[k] = t;
-                    if (M[k] != cd(0.0, 0.0)) ratio[k] *= t / M[k];
-                }
-                to_engine_layout(h, pl, Hh.data(), lay.data());
-                if (int rc = upload_table(h, (char*)h->tabH2[x] + (size_t)j * N * h->tab_esz, lay.data(), N)) return rc;
-            }
-        }
+        if (int rc = upload_cycle(h->tabH2[x], M)) return rc;
         if (h->natH2[x]) if (int rc = upload_complex(h, h->natH2[x], M.data(), N)) return rc;
         if (K > 1) {
             // several crystals: per segment the half step, the full step and the junction H_j H_{j+1}
@@ -582,7 +594,7 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
             if (cudaMalloc(p, fb) != cudaSuccess) return bail(OPO_ERR_ALLOC, "cudaMalloc of field state failed");
             cudaMemset(*p, 0, fb);
         }
-        if (cudaMalloc(&h->tabH[x], (size_t)h->N * h->tab_esz) != cudaSuccess ||
+        if (cudaMalloc(&h->tabH[x], (size_t)h->tab_cycle * h->N * h->tab_esz) != cudaSuccess ||
             cudaMalloc(&h->tabH2[x], (size_t)h->tab_cycle * h->N * h->tab_esz) != cudaSuccess ||
             cudaMalloc(&h->mirror[x], (size_t)h->B * h->esz) != cudaSuccess)
             return bail(OPO_ERR_ALLOC, "cudaMalloc of tables failed");
@@ -883,6 +895,13 @@ struct TrainArgs {
     int out_field = 0;
 };
 
+void advance_counts(opo_handle* h, long long ops, long long half_uses, long long full_uses) {
+    constexpr long long kWrap = 1 << 20;
+    h->op_count = (int)((h->op_count + ops) % kWrap);
+    h->hq_count = (int)((h->hq_count + half_uses) % kWrap);
+    h->fq_count = (int)((h->fq_count + full_uses) % kWrap);
+}
+
 int resident_run(opo_handle* h, int mode, int z0, int steps, const TrainArgs* train = nullptr) {
     opo::ResidentArgs a{};
     if (train) {
@@ -907,6 +926,7 @@ int resident_run(opo_handle* h, int mode, int z0, int steps, const TrainArgs* tr
     a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
     a.mode = mode; a.z0 = z0; a.steps = steps; a.nln = h->splitting;
     a.tab_cycle_mask = h->tab_cycle - 1;
+    a.op0 = h->op_count; a.hq0 = h->hq_count; a.fq0 = h->fq_count;
     a.dk0 = !h->splitting;
     for (int b = 0; b < h->B; ++b) if (h->dk[b] != 0.0) a.dk0 = 0;
     const bool solo = engine_in_use(h) == OPO_ENGINE_SOLO, wide = engine_in_use(h) == OPO_ENGINE_WIDE;
@@ -937,6 +957,11 @@ int resident_run(opo_handle* h, int mode, int z0, int steps, const TrainArgs* tr
     }
     if (e != cudaSuccess) return fail(h, OPO_ERR_CUDA, std::string("launch of the on-chip kernel: ") + cudaGetErrorString(e));
     ++h->launches;
+    // what an (uncut) instance has applied in this launch: the operators q = 0 .. total, of which the first and the last are
+    // half-steps and the boundary crossings use tables of their own; N/2 - L - N/2: full steps only
+    const long long passes = mode == 1 ? steps : 1, per_pass = mode == 1 ? h->nz : steps;
+    advance_counts(h, h->splitting ? passes * per_pass : passes * per_pass + 1, h->splitting ? 0 : 2,
+                   h->splitting ? passes * per_pass : passes * (per_pass - 1));
     return OPO_OK;
 }
 
@@ -954,12 +979,17 @@ void large_common(const opo_handle* h, opo::LargeArgs& a) {
     a.h = h->h; a.n_fields = h->F; a.batch = h->B; a.nz = h->nz;
     a.field_mask = (1 << h->F) - 1;
     a.barrier = h->barrier; a.barrier_base = 0;
+    a.op0 = h->op_count;
 }
 
 int large_launch(opo_handle* h, const opo::LargeArgs& a) {
     OPO_CUDA(h, cudaMemsetAsync(h->barrier, 0, sizeof(unsigned long long), h->stream));
     OPO_LAUNCH(h, h->dbl ? opo::launch_large_f64(h->L, a, h->linfo.grid, h->stream)
                          : opo::launch_large_f32(h->L, a, h->linfo.grid, h->stream));
+    if (a.mode != 2) {      // linear operators of this launch (the read-out applies none)
+        const long long total = a.mode == 1 ? (long long)a.steps * a.nz : a.steps;
+        advance_counts(h, a.nln ? total : total + 1, 0, 0);
+    }
     return OPO_OK;
 }
 

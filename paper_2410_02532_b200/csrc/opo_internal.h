@@ -73,9 +73,9 @@ struct ResidentArgs {
     const void* S[3];      // stored inputs (non-resonant fields restart from these)
     void* exitb[3];        // exit fields (z = L of the last pass), written when write_exit
     void* SH[3];           // scratch [B][N]: IDFT(H DFT(S_x)) of non-resonant fields
-    const void* tabH[3];   // half step            (shared)
+    const void* tabH[3];   // half step            (shared): [tab_cycle_mask + 1][N], cycled like tabH2 (copy 0 = the plain rounding)
     const void* tabH2[3];  // merged full step     (shared): [tab_cycle_mask + 1][N], a cycle of roundings with error feedback
-                           //   (opo_api.cu build_tables); operator q of a call uses copy q & tab_cycle_mask
+                           //   (opo_api.cu build_tables); the k-th full step the handle applies uses copy k & tab_cycle_mask
     const void* tabHB[3];  // H G m H merged across the boundary (resonant; maybe per instance)
     const void* tabGM[3];  // G m / N, un-merged boundary       (resonant; maybe per instance)
     const void* tabHG[3];  // H G m / N: last half-step + boundary, used when a modulator (eom) follows
@@ -93,6 +93,12 @@ struct ResidentArgs {
     double h;
     int n_fields, batch, nz;   // nz = steps per pass
     int tab_cycle_mask;    // see tabH2
+    // What the handle has applied before this call (opo_api.cu advances them after every launch), so that neither cycle of
+    // roundings nor the bunched constant correction restarts with the call: z-step-by-z-step driving (PAPER.md:L266-297,
+    // Listing 3 is such a loop) then sees the same sequence of tables and corrections as one long call.
+    int op0;               //   linear-operator applications (selects the applications that carry kConstBunch low parts)
+    int hq0;               //   uses of the half-step table (copy (hq0 + k) & tab_cycle_mask of tabH is used next)
+    int fq0;               //   uses of the full-step table (likewise for tabH2)
     int wide_g;            // wide engine: sub-blocks per CTA (1: clusters of 4 F CTAs, 2: clusters of 2 F CTAs)
     int mode;              // 0 = propagate `steps` z-steps from step index z0; 1 = `steps` round trips
     int split;             // 1 (mode 1 only): work is dealt to the clusters in round trips, not instances (opo_resident.cuh)
@@ -147,6 +153,8 @@ struct LargeArgs {
     int z0;
     int steps;
     int nln;                   // 1: order N/2 - L - N/2; phase table in steps of h/4; mode 1 takes steps = 1
+    int op0;                   // linear operators the handle has applied before this launch (the every-FIX_EVERY-th twiddle defect
+                               // correction is keyed on op0 + q, not on the call's own q)
     unsigned long long* barrier;        // zeroed by the host before the launch
     unsigned long long barrier_base;    // counter value at launch (0)
 };

@@ -586,7 +586,7 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
         }
 #pragma unroll 1
         for (int q = 0; q < nsteps; ++q) {
-            e.fix = (q % E::FIX_EVERY) == 0;
+            e.fix = ((a.op0 + q) % E::FIX_EVERY) == 0;
             e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);      // (begins with the grid barrier)
             grid_barrier(a.barrier, target);
             if (q + 1 < nsteps) e.template col_pass<COL_RK4>(cur, cur, mask, batch, phase, a.phase_stride, 4 * (zs + q) + 2, kap, hh, true);
@@ -620,7 +620,7 @@ __global__ void __launch_bounds__(large_cfg<T, L, F>::NT, 1) k_large(LargeArgs a
                 if (rt_mode && q == 0 && !res && a.steps > 1) op.sh_store[x] = reinterpret_cast<cplx<T>*>(a.SH[x]);
             }
         }
-        e.fix = (q % E::FIX_EVERY) == 0;        // (row pass and the column pass that follows)
+        e.fix = ((a.op0 + q) % E::FIX_EVERY) == 0;        // (row pass and the column pass that follows)
         e.row_pass(cur, op, batch, a.perm1, a.perm2, a.barrier, target);          // (begins with the grid barrier)
         OPO_TSTAMP(e, 7);                                   // row stored
         grid_barrier(a.barrier, target);

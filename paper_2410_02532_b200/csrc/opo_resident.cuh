@@ -266,6 +266,11 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
             break;
         }
         const int total = rt_mode ? steps_l * nz : steps_l;     // RK4 steps of this piece of work
+        // where this piece stands in the handle's count of table uses (ResidentArgs::hq0, fq0): an instance cut into pieces
+        // by the split schedule applies two half-steps more per cut
+        const int cuts = (a.split && rt0 > 0) ? (int)(((long long)b * a.steps + rt0) / quota - ((long long)b * a.steps) / quota) : 0;
+        const int hq_base = a.hq0 + 2 * cuts;
+        const int fq_base = a.fq0 + (rt_mode ? rt0 * (nz - 1) : 0);
         int* const flag = a.flags ? a.flags + (size_t)b * F + x : nullptr;
         cplx<T>* cur = reinterpret_cast<cplx<T>*>(a.cur[x]) + (size_t)b * N;
         const cplx<T>* ph = reinterpret_cast<const cplx<T>*>(a.phase) + (size_t)b * a.phase_stride;
@@ -340,9 +345,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                     fa.mb = mb; fa.nf = F;
                     fa.wait_in = 1; fa.par_done = (fz - 1) & 1;
                     fa.arrive_out = 1;
-                    linear_core_smem<T, L, NT, true>(tabH2, tid, fa);
+                    linear_core_smem<T, L, NT, true>(tabH2 + (size_t)((a.fq0 + q) & a.tab_cycle_mask) * N, tid, fa);
                 } else {
-                    linear_core_smem<T, L, NT>(tabH2, tid);
+                    linear_core_smem<T, L, NT>(tabH2 + (size_t)((a.fq0 + q) & a.tab_cycle_mask) * N, tid);
                 }
                 const cplx<T>* p = ph + 4 * (zs + q) + 2;
                 if (q + 1 < nsteps) run_fused(ldg(p), ldg(p + 1), ldg(p + 2), ldg(p + 3), ldg(p + 4), 2, hh, (T)1, (T)1);
@@ -395,7 +400,9 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                     linear_core_smem<T, L, NT>(tabH, tid);
                 }
             } else {
-                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2 + (size_t)(q & a.tab_cycle_mask) * N);
+                const int fq = fq_base + q - 1 - ((rt_mode && q > 0) ? (q - 1) / nz : 0);      // full steps applied before this one
+                const cplx<T>* tab = (q == 0 || q == total) ? tabH + (size_t)((hq_base + (q == 0 ? 0 : 1)) & a.tab_cycle_mask) * N
+                                                            : (crossing ? tabHB : tabH2 + (size_t)(fq & a.tab_cycle_mask) * N);
                 if constexpr (FLOW) {
                     FlowArgs fa;
                     fa.mb = mb; fa.nf = F;

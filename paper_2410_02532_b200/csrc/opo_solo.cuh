@@ -328,6 +328,12 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
         }
         const int total = rt_mode ? steps_l * nz : steps_l;
         const cplx<T>* ph = reinterpret_cast<const cplx<T>*>(a.phase) + (size_t)b * a.phase_stride;
+        // where this piece stands in the handle's count of operators / table uses (ResidentArgs::op0, hq0, fq0): an instance
+        // cut into pieces by the split schedule applies two half-steps more per cut
+        const int cuts = (a.split && rt0 > 0) ? (int)(((long long)b * a.steps + rt0) / quota - ((long long)b * a.steps) / quota) : 0;
+        const int op_base = a.op0 + (rt_mode ? rt0 * nz : 0) + cuts;
+        const int hq_base = a.hq0 + 2 * cuts;
+        const int fq_base = a.fq0 + (rt_mode ? rt0 * (nz - 1) : 0);
 
         auto load = [&](const cplx<T>* __restrict__ g) {
 #pragma unroll 4
@@ -389,6 +395,8 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
         for (int q = 0; q <= total; ++q) {
             const int s = rt_mode ? q % nz : a.z0 + q;
             const bool crossing = rt_mode && q > 0 && q < total && s == 0;
+            const int fq = fq_base + q - 1 - ((rt_mode && q > 0) ? (q - 1) / nz : 0);      // full steps applied before this one
+            const bool bunch = ((op_base + q) & (kConstBunch - 1)) == 0;
 #pragma unroll
             for (int x = 0; x < F; ++x) {
                 const bool resonant = a.resonant[x] != 0;
@@ -402,7 +410,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                 if (TRAIN && crossing && (x == 0 || (x == a.out_field && a.out_train != nullptr))) {
                     if (x == a.out_field && a.out_train != nullptr) {
                         // SaveRoundTrip: the field at z = L of the round trip just finished, before the mirror
-                        core(tabH, true, false);
+                        core(tabH, true, false, bunch);
                         __syncthreads();
                         pass0_local<T, L, NT>(tw, tid, true);
                         __syncthreads();
@@ -435,7 +443,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                     //   core(H G m) -> inverse pass 0 -> x E[n] -> forward pass 0 -> core(H)
                     const cplx<T>* tabHG = reinterpret_cast<const cplx<T>*>(a.tabHG[x]) + (size_t)b * a.tab_stride[x];
                     const cplx<T>* __restrict__ E = reinterpret_cast<const cplx<T>*>(a.eom[x]);
-                    core(tabHG, true, false);
+                    core(tabHG, true, false, bunch);
                     __syncthreads();
                     pass0_local<T, L, NT>(tw, tid, true);
                     __syncthreads();
@@ -446,11 +454,11 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                     __syncthreads();
                     core(tabH, false, !inj);
                 } else {
-                    const cplx<T>* tab = tabH;
+                    const cplx<T>* tab = tabH + (size_t)((hq_base + (q == 0 ? 0 : 1)) & a.tab_cycle_mask) * N;
                     if (q != 0 && q != total)
                         tab = crossing ? reinterpret_cast<const cplx<T>*>(a.tabHB[x]) + (size_t)b * a.tab_stride[x]
-                                       : reinterpret_cast<const cplx<T>*>(a.tabH2[x]) + (size_t)(q & a.tab_cycle_mask) * N;
-                    core(tab, !first_core, !last_core && !keep && !inj, (q & (kConstBunch - 1)) == 0);
+                                       : reinterpret_cast<const cplx<T>*>(a.tabH2[x]) + (size_t)(fq & a.tab_cycle_mask) * N;
+                    core(tab, !first_core, !last_core && !keep && !inj, bunch);
                 }
                 if (inj) {
                     __syncthreads();

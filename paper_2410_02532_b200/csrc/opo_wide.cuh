@@ -455,12 +455,14 @@ __global__ void __launch_bounds__(wide_layout<T, L, F, G>::NTH, 1) k_wide(Reside
                 for (int k = 0; k < 16; ++k) v[k] = g[tid_g + NT * k];
                 wide_push16<T, NW, NV, G, WL::MAXT, WL::NQ>(v, fb, wc, lane);
             } else {
-                const cplx<T>* tab = (q == 0 || q == total) ? tabH : (crossing ? tabHB : tabH2 + (size_t)(q & a.tab_cycle_mask) * N);
+                const int fq = a.fq0 + q - 1 - ((rt_mode && q > 0) ? (q - 1) / nz : 0);        // full steps applied before this one
+                const cplx<T>* tab = (q == 0 || q == total) ? tabH + (size_t)((a.hq0 + (q == 0 ? 0 : 1)) & a.tab_cycle_mask) * N
+                                                            : (crossing ? tabHB : tabH2 + (size_t)(fq & a.tab_cycle_mask) * N);
                 WideFlow fa = fb;
                 fa.wait_in = q > 0; fa.par_done = (fz - 1) & 1;
                 fa.push_out = q < total;
                 if constexpr (sizeof(T) == 4) {
-                    if ((q & (kConstBunch - 1)) == 0) wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ, 2>(smv, twl, tab, j, tid_g, fa, keep ? SH : nullptr, 1 + grp);
+                    if (((a.op0 + q) & (kConstBunch - 1)) == 0) wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ, 2>(smv, twl, tab, j, tid_g, fa, keep ? SH : nullptr, 1 + grp);
                     else wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ, 1>(smv, twl, tab, j, tid_g, fa, keep ? SH : nullptr, 1 + grp);
                 } else {
                     wide_core<T, L, NT, NV, G, WL::MAXT, WL::NQ>(smv, twl, tab, j, tid_g, fa, keep ? SH : nullptr, 1 + grp);

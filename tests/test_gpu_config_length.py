@@ -159,3 +159,120 @@ def test_config4_subset16_full_length_power_and_spectrum():
     res = _long_run("c4_300rt_sub16", w, [P.ENGINE_SOLO, P.ENGINE_RESIDENT])
     for e_p, e_s, e_d in res.values():
         assert e_p.max() <= 1e-3 and e_s.max() <= 1e-3
+
+
+# ---- call granularity: the same run cut into many calls ----------------------------------------------------------------
+# The paper's own loop is one call per step (Listing 3), and the ABI allows any cut of a run into
+# opo_propagate / opo_roundtrips calls.  The fp32 engines keep 1e4 .. 1e5 z-steps inside tolerance with two devices that are
+# indexed by the operator count: a cycle of 16 roundings of the dispersion tables and constant corrections applied at every
+# 8th operator.  Both are keyed on the handle's running count (ResidentArgs::op0 / hq0 / fq0), not on the call's own, so the
+# accuracy must not depend on the cut.  Tolerances: north_star's 1e-4 against the oracle; 2e-5 between two cuts.
+
+ON_CHIP = ["solo", "wide", "resident"]
+_GRANULARITY_ORACLE = {}
+
+
+def _engine(P, name):
+    return {"solo": P.ENGINE_SOLO, "wide": P.ENGINE_WIDE, "resident": P.ENGINE_RESIDENT}[name]
+
+
+def _fields(o, P, which):
+    return np.stack([o.get_fields(x, which).cpu().numpy().astype(np.complex128) for x in range(o.n_fields)])
+
+
+def _long_single_pass_workload():
+    """C1's grid, crystal data and step (h = 200 um) with a pass of 2000 z-steps (20 x C1's length) and seeds at 1e-3 of the
+    pump, so that signal and idler end at a sizeable fraction of the pump and every field is populated."""
+    w = W.config1(1)
+    w.name = "C1-shaped single pass x 2000"
+    w.length_m = w.length_m * 20
+    w.nz_per_pass = 2000
+    w.seeds = [None] + [W._round_to_precision(s * 1e3, w.precision) for s in w.seeds[1:]]
+    return w
+
+
+@pytest.mark.parametrize("engine_name", ON_CHIP)
+def test_single_pass_2000_steps_call_by_call(engine_name):
+    import oracle
+    torch, P = _gpu()
+    w = _long_single_pass_workload()
+    if "pass" not in _GRANULARITY_ORACLE:
+        r = oracle.from_workload(w)
+        assert r.propagate(w.nz_per_pass) == 0
+        _GRANULARITY_ORACLE["pass"] = np.stack([r.get_field(x) for x in range(w.n_fields)])
+    ref = _GRANULARITY_ORACLE["pass"]
+    got = {}
+    for cut in ("one call", "z-step by z-step", "chunks of 3, 5, 8, ..."):
+        o = P.from_workload(w, engine=_engine(P, engine_name))
+        assert o.engine == _engine(P, engine_name)
+        if cut == "one call":
+            o.propagate(w.nz_per_pass)
+        elif cut == "z-step by z-step":
+            for _ in range(w.nz_per_pass):
+                o.propagate(1)
+        else:
+            left, k = w.nz_per_pass, 0
+            while left:
+                n = min(left, (3, 5, 8, 13, 1, 21)[k % 6])
+                o.propagate(n)
+                left, k = left - n, k + 1
+        o.sync()
+        o.check_finite()
+        got[cut] = _fields(o, P, P.WHICH_CURRENT)
+        o.close()
+    energy = [float(np.mean(np.abs(ref[x]) ** 2)) for x in range(w.n_fields)]
+    for cut, g in got.items():
+        e_ref = [rel_l2(g[x], ref[x]) for x in range(w.n_fields)]
+        e_one = [rel_l2(g[x], got["one call"][x]) for x in range(w.n_fields)]
+        print(f"{w.name}, {engine_name}, {cut}: vs oracle {max(e_ref):.3e}, vs one call {max(e_one):.3e} (mean |A|^2 p/s/i: "
+              f"{energy[0]:.3e} {energy[1]:.3e} {energy[2]:.3e})")
+        assert max(e_ref) <= 1e-4, (cut, e_ref)
+        assert max(e_one) <= 2e-5, (cut, e_one)
+
+
+@pytest.mark.parametrize("engine_name", ON_CHIP)
+def test_config1_20rt_one_call_per_roundtrip(engine_name):
+    import oracle
+    torch, P = _gpu()
+    w = W.config1(20)
+    if "c1x20" not in _GRANULARITY_ORACLE:
+        _GRANULARITY_ORACLE["c1x20"] = oracle.run_workload(w)["exit"][0]
+    ref = _GRANULARITY_ORACLE["c1x20"]
+    got = {}
+    for calls in (1, 20):
+        o = P.from_workload(w, engine=_engine(P, engine_name))
+        for _ in range(calls):
+            o.roundtrips(w.n_roundtrips // calls)
+        o.sync()
+        got[calls] = _fields(o, P, P.WHICH_EXIT)
+        o.close()
+    for calls, g in got.items():
+        e_ref = max(rel_l2(g[x], ref[x]) for x in range(w.n_fields))
+        e_one = max(rel_l2(g[x], got[1][x]) for x in range(w.n_fields))
+        print(f"C1 x 20 RT, {engine_name}, {calls} call(s): vs oracle {e_ref:.3e}, vs one call {e_one:.3e}")
+        assert e_ref <= 1e-4 and e_one <= 2e-5
+
+
+def test_config1_full_length_as_a_pump_train():
+    """C1 x 1000 round trips through opo_roundtrips_train with a constant train (the same physics as opo_roundtrips, so the
+    c1_1000rt golden applies): on the engine AUTO picks for one OPO (wide) that is one launch per round trip, 1000 calls'
+    worth of restarts if the cycles were keyed on the call."""
+    torch, P = _gpu()
+    w = W.config1()
+    g = golden("c1_1000rt", w)
+    o = P.from_workload(w)
+    assert o.engine == P.ENGINE_WIDE
+    pump = torch.from_numpy(np.ascontiguousarray(w.pump[0])).to(torch.complex64).cuda()
+    train = pump[None, :].repeat(w.n_roundtrips, 1).contiguous()
+    out = o.roundtrips_train(train, out_field=1)
+    o.sync()
+    launches = o.launches
+    ex = _fields(o, P, P.WHICH_EXIT)
+    assert torch.equal(out[-1, 0], o.get_fields(1, P.WHICH_EXIT)[0])
+    o.close()
+    p_out = (1.0 - w.R[1]) * np.mean(np.abs(ex[1]) ** 2)
+    spec = np.abs(np.fft.fft(ex[1])) ** 2
+    e_p = abs(p_out - g["p_out"][0]) / g["p_out"][0]
+    e_s = rel_l2(spec, g["spectrum"][0].astype(np.float64))
+    print(f"C1 x 1000 RT as a pump train ({launches} launches): signal power rel err {e_p:.3e}, power spectrum rel L2 {e_s:.3e}")
+    assert e_p <= 1e-3 and e_s <= 1e-3
