@@ -63,20 +63,23 @@ def smem_bytes_per_field_point_zstep(precision: str) -> float:
 
 # The wide engine (one instance on a cluster of 4 F CTAs) is bound by the SM-to-SM link: every field value leaves its SM as an
 # operand of the pass-0 / RK4 phase and comes back as a result at every z-step.  Bytes through one
-# SM's port per z-step, sent and received: 2 directions x 2 crossings x esz x N F (NV - 1) / NV / n_ctas.  Peak: 16 B/clk per
-# SM, reads and writes together, measured in round 1 (profiles/r01d_dsmem_microbench.md) -- not re-measured in this run.
+# SM's port per z-step, sent and received, with G sub-blocks of a field per CTA (OPO_INFO_WIDE_SUBBLOCKS; NV = 4 F sub-blocks
+# on NV / G CTAs, and what stays inside a CTA does not cross the link): 2 directions x 2 crossings x esz x (N F G / NV) x
+# (NV - G) / NV.  Peak: 16 B/clk per SM, reads and writes together, measured in round 1
+# (profiles/r01d_dsmem_microbench.md) -- not re-measured in this run.
 def wide_link_roofline(w, o, P, units_per_step, avg_s, sm_ghz):
     esz = 16 if w.precision == "c128" else 8
     nv = 4 * w.n_fields
     slots = int(P.opo_get_info(o._h, P.INFO_SLOTS))
     waves = -(-w.batch // max(1, slots))
-    per_sm_per_zstep = 2 * 2 * esz * w.n * w.n_fields * (nv - 1) / nv / nv          # clusters of 4 F CTAs (one sub-block per CTA)
+    g = max(1, int(P.opo_get_info(o._h, P.INFO_WIDE_SUBBLOCKS)))
+    per_sm_per_zstep = 2 * 2 * esz * (w.n * w.n_fields * g / nv) * (nv - g) / nv
     zsteps_per_sm = units_per_step / (w.batch * w.n) * waves                        # z-steps an SM works through, wave after wave
     achieved = per_sm_per_zstep * zsteps_per_sm / avg_s / 1e9
     peak = 16.0 * sm_ghz
     return {"achieved": achieved, "peak": peak, "unit": "GB/s per SM", "frac": achieved / peak,
             "note": "SM-to-SM link traffic of one SM (operands out, results back, both directions); peak = 16 B/clk per SM at the max SM "
-                    "clock, measured in round 1 (profiles/r01d_dsmem_microbench.md); assumes one sub-block per CTA"}
+                    "clock, measured in round 1 (profiles/r01d_dsmem_microbench.md); " + f"{g} sub-block(s) per CTA"}
 
 
 def make_workload(name: str, rank: int):
@@ -207,12 +210,12 @@ def main():
                     help="cufft = the internal cuFFT + elementwise-kernel baseline (north_star item (d)), not the product")
     ap.add_argument("--eom", action="store_true",
                     help="intracavity phase modulator on the signal (PAPER.md:L149-154; beta = 1 rad, f = 3 / window): the "
-                         "paper's 'EOM' cavity configuration; the boundary is then not merged (one launch per round trip)")
+                         "paper's 'EOM' cavity configuration; one launch per step on the on-chip engines (table H G m, modulator in the time domain, H at every crossing)")
     ap.add_argument("--wide-subblocks", type=int, default=0, choices=[0, 1, 2],
                     help="wide engine: sub-blocks per CTA (OPO_OPT_WIDE_SUBBLOCKS); 0 = the library's choice")
     ap.add_argument("--train", action="store_true",
                     help="nanosecond regime (PAPER.md:L322-335): opo_roundtrips_train -- a pump slice per round trip in, the exit "
-                         "signal of every round trip out, one launch per round trip; default 20 round trips per step")
+                         "signal of every round trip out; one launch per step on the solo engine (slices read and exit fields written at the crossings inside the kernel), one per round trip elsewhere; default 20 round trips per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

@@ -50,7 +50,9 @@
  *     of operators since opo_create, which no call resets.  Hence two handles driven by the same sequence of calls agree
  *     bit for bit, while a second run on a REUSED handle differs from the first at rounding level (1e-7 relative).
  *   - Calls enqueue work on the handle's stream and return; asynchronous faults surface at
- *     opo_sync or at the next call (OPO_ERR_CUDA).  There is no CPU fallback of any kind: without
+ *     opo_sync or at the next call (OPO_ERR_CUDA).  The CUDA error state of the calling thread is shared with the rest
+ *     of the process: the library looks at it (cudaPeekAtLastError) and clears it only after a failed call of its own,
+ *     so an error that PyTorch or another library raised makes opo calls fail until its owner has dealt with it.  There is no CPU fallback of any kind: without
  *     a usable sm_100 device opo_create fails with OPO_ERR_CUDA.
  */
 #ifndef OPO_H_
@@ -151,14 +153,19 @@ int opo_set_beta3(opo_handle* h, int field, double beta3_s3_per_m);
  * mirror factor, A_x[n] *= exp(i beta sin(2 pi f_pm tau_n)), tau_n = (n - N/2) dt.  beta_rad = 0 removes it.
  * Same modulator for every instance.  OPO_ERR_INVALID_ARG for a non-resonant field (it restarts from its
  * stored input every round trip, so a modulator on it would never act).  The table is built in fp64 on the
- * host.  With a modulator present the boundary is not merged into the next half-step (the resident engine runs
- * core(H G m), the modulator in the time domain, core(H) at a crossing; the large-N engine one launch per round trip). */
+ * host.  The on-chip engines (solo, wide, cluster) keep a whole opo_roundtrips call in one launch with a modulator
+ * present: at a crossing they apply the table H G m, go to the time domain for the modulator and come back for the first
+ * half-step H of the next pass (the boundary is then not merged into that half-step).  The large-N and streaming engines
+ * run one launch sequence per round trip. */
 int opo_set_eom(opo_handle* h, int field, double beta_rad, double f_mod_hz);
 
 /* Pump input S_p (PAPER.md:L268 ReadPump): time-domain complex [N] (per_instance = 0, broadcast to
- * all instances) or [batch][N].  Copied into the handle; re-injected at every round-trip boundary; when z = 0 the
- * current pump field becomes what the boundary injects into an empty cavity: S_p (single-pass pump) or
- * sqrt(1 - R_p) S_p (resonant pump, reading R24). */
+ * all instances) or [batch][N].  Copied into the handle; re-injected at every round-trip boundary.  Single-pass pump: when
+ * z = 0 the current pump field becomes S_p as well, so the new input drives the next pass.  Resonant pump (reading R24):
+ * before the handle has taken its first z-step the current pump field becomes sqrt(1 - R_p) S_p, what the input coupler
+ * lets into an empty cavity; once the run is under way only S_p changes -- the light stored in the cavity stays, and the
+ * boundary of the next round trip injects the new input (a pump ramp between opo_roundtrips calls).  To start over on
+ * the same handle, set the intracavity pump yourself with opo_set_field(h, 0, ..) and then the input with this call. */
 int opo_set_pump(opo_handle* h, const void* dev_pump, int per_instance);
 int opo_set_pump_host(opo_handle* h, const void* host_pump, int per_instance);
 
@@ -255,6 +262,7 @@ int opo_set_option(opo_handle* h, int option, int value);
 #define OPO_INFO_BATCH 3
 #define OPO_INFO_SM_COUNT 4
 #define OPO_INFO_SLOTS 5           /* co-resident work slots (clusters / CTAs) the next roundtrips call deals its work to */
+#define OPO_INFO_WIDE_SUBBLOCKS 6  /* sub-blocks of a field per CTA the WIDE engine will use (1 | 2; see OPO_OPT_WIDE_SUBBLOCKS), 0 on other engines */
 int opo_get_info(const opo_handle* h, int what, long long* out);
 
 /* Device peaks measured on the spot with the library's own micro-benchmark kernels, the roofline denominators bench.py

@@ -28,7 +28,7 @@ OPT_ENGINE = 0
 OPT_WIDE_SUBBLOCKS = 2
 OPT_SPLITTING = 1
 SPLITTING_LNL, SPLITTING_NLN = 0, 1
-INFO_ENGINE, INFO_LAUNCHES, INFO_N, INFO_BATCH, INFO_SM_COUNT, INFO_SLOTS = 0, 1, 2, 3, 4, 5
+INFO_ENGINE, INFO_LAUNCHES, INFO_N, INFO_BATCH, INFO_SM_COUNT, INFO_SLOTS, INFO_WIDE_SUBBLOCKS = 0, 1, 2, 3, 4, 5, 6
 
 _D3 = ctypes.c_double * 3
 _I3 = ctypes.c_int * 3

@@ -145,6 +145,8 @@ struct opo_handle {
     size_t tab_esz = 8;        // bytes per table entry (large engine, c64: hi + lo = 16)
 
     int z_steps = 0;
+    bool run_started = false;       // a z-step has been taken since opo_create (opo_set_pump: empty-cavity start of a resonant pump)
+    size_t phase_bytes = 0;         // capacity of `phase`
     int engine_opt = OPO_ENGINE_AUTO;
     bool resident_ok = false;
     opo::ResidentInfo rinfo{};
@@ -599,7 +601,8 @@ int opo_create(const opo_crystal* c, const opo_fields* f, const opo_grid* g, opo
             cudaMalloc(&h->mirror[x], (size_t)h->B * h->esz) != cudaSuccess)
             return bail(OPO_ERR_ALLOC, "cudaMalloc of tables failed");
     }
-    if (cudaMalloc(&h->scratch, fb) != cudaSuccess || cudaMalloc(&h->phase, (size_t)h->B * (4 * h->nz + 8) * h->esz) != cudaSuccess ||
+    h->phase_bytes = (size_t)h->B * (4 * (size_t)h->nz + 8) * h->esz;
+    if (cudaMalloc(&h->scratch, fb) != cudaSuccess || cudaMalloc(&h->phase, h->phase_bytes) != cudaSuccess ||
         cudaMalloc((void**)&h->flag, sizeof(int)) != cudaSuccess)
         return bail(OPO_ERR_ALLOC, "cudaMalloc of scratch failed");
     if (int rc = build_fft_tables(h)) { std::string m = h->err; return bail(rc, m); }
@@ -687,11 +690,12 @@ namespace {
         ++(h)->launches;                                                                   \
     } while (0)
 
-// Surface an error left by earlier asynchronous work without synchronising.  The CUDA "last error" is per host thread, not
-// per handle: it is reported once and cleared (cudaGetLastError), so a non-sticky error -- somebody's failed allocation or
-// launch -- does not fail every later call on every handle; a sticky one (a device fault) keeps coming back by itself.
+// Surface an error left by earlier asynchronous work without synchronising.  The CUDA "last error" is per host thread and
+// shared with everything else in the process (PyTorch, other handles): it is only looked at here (cudaPeekAtLastError), never
+// cleared, so that whoever raised it still finds it.  The library clears the error state only right after a call of its own
+// has failed (the cudaGetLastError() next to those calls).  A sticky error (a device fault) keeps coming back by itself.
 int check_async(opo_handle* h) {
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = cudaPeekAtLastError();
     if (e != cudaSuccess) return fail(h, OPO_ERR_CUDA, std::string("earlier asynchronous fault: ") + cudaGetErrorString(e));
     return OPO_OK;
 }
@@ -1054,8 +1058,10 @@ int set_pump_impl(opo_handle* h, const void* p, int per_instance, cudaMemcpyKind
     if (int rc = copy_in(h, h->S[0], p, per_instance != 0, kind)) return rc;
     if (h->z_steps == 0) {
         // what the boundary injects into an empty cavity: S_p for a single-pass pump, sqrt(1 - R_p) S_p through the
-        // input coupler of a resonant one (reading R24)
-        if (h->fields.resonant[0]) return stream_axpy(h, h->cur[0], h->S[0], pump_inject(h), false);
+        // input coupler of a resonant one (reading R24).  A resonant pump that has been running holds stored light, which a
+        // new input must not wipe out (a power ramp between opo_roundtrips calls): then only S_p changes and the boundary of
+        // the next round trip injects it, as in the oracle, where the input and the state of a field are set separately.
+        if (h->fields.resonant[0]) return h->run_started ? OPO_OK : stream_axpy(h, h->cur[0], h->S[0], pump_inject(h), false);
         OPO_CUDA(h, cudaMemcpyAsync(h->cur[0], h->S[0], h->field_bytes(), cudaMemcpyDeviceToDevice, h->stream));
     }
     return OPO_OK;
@@ -1116,6 +1122,7 @@ int opo_propagate(opo_handle* h, int nz) {
     else rc = stream_steps(h, h->z_steps, nz, false);
     if (rc) return rc;
     h->z_steps += nz;
+    h->run_started = true;
     return OPO_OK;
 }
 
@@ -1126,6 +1133,7 @@ int opo_roundtrips(opo_handle* h, int n) {
     if (n == 0) return OPO_OK;
     if (int rc = check_async(h)) return rc;
     if (int rc = ensure_tables(h)) return rc;
+    h->run_started = true;
     // a phase modulator acts in the time domain between the boundary's spectral phase and the next pass, so the
     // boundary cannot be merged into the neighbouring half-steps: one launch per round trip then
     const bool eom = any_eom(h);
@@ -1194,6 +1202,23 @@ int opo_set_segments(opo_handle* h, int n, const opo_segment* segs) {
         total += segs[j].nz;
     }
     if (int rc = check_async(h)) return rc;
+    // everything that can fail comes first, so that a failure leaves the handle as it was: a larger phase table (the old
+    // one is kept when it is large enough) and the wait for work that still reads the old one
+    const long long new_nz = n == 0 ? h->grid.nz_per_pass : total;
+    const size_t need = (size_t)h->B * (4 * (size_t)new_nz + 8) * h->esz;
+    void* new_phase = nullptr;
+    if (need > h->phase_bytes && cudaMalloc(&new_phase, need) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the phase table failed");
+    }
+    {
+        const cudaError_t e = cudaStreamSynchronize(h->stream);
+        if (e != cudaSuccess) {
+            if (new_phase) cudaFree(new_phase);
+            return fail(h, OPO_ERR_CUDA, std::string("cudaStreamSynchronize: ") + cudaGetErrorString(e));
+        }
+    }
+    if (new_phase) { cudaFree(h->phase); h->phase = new_phase; h->phase_bytes = need; }
     if (n == 0) {       // back to the crystal of opo_create
         h->n_seg = 1;
         h->seg[0].len = h->crystal.length_m; h->seg[0].dk = h->crystal.dk_per_m; h->seg[0].deff = h->crystal.d_eff_m_per_V;
@@ -1214,10 +1239,12 @@ int opo_set_segments(opo_handle* h, int n, const opo_segment* segs) {
     for (int x = 0; x < 3; ++x) h->kappa[x] = h->seg[0].kappa[x];
     // per-instance dk sweeps act on the first crystal; a new segment list resets them to its dk
     h->dk.assign(h->B, h->seg[0].dk);
-    OPO_CUDA(h, cudaStreamSynchronize(h->stream));
-    cudaFree(h->phase);
-    h->phase = nullptr;
-    if (cudaMalloc(&h->phase, (size_t)h->B * (4 * (size_t)h->nz + 8) * h->esz) != cudaSuccess) { cudaGetLastError(); return fail(h, OPO_ERR_ALLOC, "cudaMalloc of the phase table failed"); }
+    if (h->n_seg == 1)      // a single crystal uses tabH / tabH2: give the per-segment tables back (the stream is idle)
+        for (int j = 0; j < 8; ++j)
+            for (int x = 0; x < 3; ++x) {
+                void** ptrs[] = {&h->segH[j][x], &h->segH2[j][x], &h->segHX[j][x]};
+                for (void** p : ptrs) if (*p) { cudaFree(*p); *p = nullptr; }
+            }
     h->tables_dirty = true;
     h->phase_dirty = true;
     return OPO_OK;
@@ -1350,6 +1377,7 @@ int opo_get_info(const opo_handle* h, int what, long long* out) {
             else *out = (long long)h->B * h->F;
             return OPO_OK;
         }
+        case OPO_INFO_WIDE_SUBBLOCKS: *out = engine_in_use(h) == OPO_ENGINE_WIDE ? wide_group(h) : 0; return OPO_OK;
         default: return OPO_ERR_INVALID_ARG;
     }
 }

@@ -242,6 +242,34 @@ def test_resonant_pump_matches_oracle(precision, log2_n, n_fields, calls, eom, e
     assert rel_l2(cur[0, 0], np.sqrt(1 - 0.6) * w.pump[0]) > 0.05
 
 
+@pytest.mark.parametrize("engine_idx", ENGINE_IDX[:3])
+def test_resonant_pump_input_changed_between_calls_keeps_the_stored_light(engine_idx):
+    """A pump ramp on a triply resonant cavity: two round trips, opo_set_pump with 1.5 x the input, two more.  The second
+    opo_set_pump finds the handle at z = 0 with light stored in the cavity and must change the input only (oracle pin
+    P19, pump input changed mid-run); before round 3 it re-initialised the intracavity pump to sqrt(1 - R_p) S_p."""
+    import oracle
+    torch, P = _gpu()
+    engine = engines()[engine_idx]
+    w = small_workload(10, 3, "c128", nz=4, batch=2, dk=-20.0, gdd_dt2=-1.3, drad=0.4, strong=False)
+    w.resonant, w.R, w.delta_rad = [1, 1, 1], [0.6, 0.9, 0.7], [0.35, 0.4, -0.2]
+    _engine_or_skip(w, engine)
+    o = P.from_workload(w, engine=engine)
+    o.roundtrips(2)
+    o.set_pump(torch.from_numpy(1.5 * w.pump).to(o.dtype).cuda().contiguous())
+    o.roundtrips(2)
+    o.sync()
+    cur = np.stack([o.get_fields(x, P.WHICH_CURRENT).cpu().numpy() for x in range(3)], axis=1)
+    o.close()
+    ref = []
+    for b in range(w.batch):
+        r = oracle.from_workload(w, b)
+        assert r.roundtrips(2) == 0
+        r.set_field(0, 1.5 * w.pump_of(b), which="input")
+        assert r.roundtrips(2) == 0
+        ref.append(np.stack([r.get_field(x) for x in range(3)]))
+    assert_close(cur, np.stack(ref), 1e-10, "pump input changed between calls")
+
+
 def test_resonant_pump_builds_up_in_a_cold_cavity():
     """Airy build-up measured on the CUDA path alone (no oracle): coupling off, CW pump on resonance, after many round
     trips the intracavity pump power is (1 - R) / (1 - sqrt(R))^2 times the input."""

@@ -862,6 +862,37 @@ def test_p19_cold_cavity_pump_builds_up_to_the_airy_steady_state():
     assert abs(abs(o.get_field(0)[0]) ** 2 / ((1 - Rp) / (1 - math.sqrt(Rp)) ** 2) - 1) < 1e-12
 
 
+def test_p19_pump_input_changed_mid_run_leaves_the_stored_light_alone():
+    """Cold cavity again: m1 round trips with input S1, then the input (not the state) becomes S2 for m2 more.  Per bin
+    A = rho^m2 [t S1~ (1 - rho^(m1+1)) / (1 - rho)] + t S2~ (1 - rho^m2) / (1 - rho): the light built up from S1 decays
+    geometrically while S2 is injected from the next boundary on.  (What opo_set_pump does on a running resonant pump.)"""
+    log2n, T, L, nz = 6, 10 * PS, 5e-3, 4
+    n = 1 << log2n
+    dt = T / n
+    Rp, delta, gdd = 0.7, -0.3, 200 * FS * FS
+    b2p = 0.35 * FS * FS / UM
+    o = make(n_fields=2, log2_n=log2n, window_s=T, nz=nz, length=L, d_eff=0.0, resonant=(1, 0), R=(Rp, 0),
+             delta_rad=(delta, 0), gdd=(gdd, 0), beta2=(b2p, 0.0), ref_field=1)
+    rng = np.random.default_rng(193)
+    S1 = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    S2 = 1.5 * (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    t = math.sqrt(1 - Rp)
+    o.set_field(0, S1, which="input")
+    o.set_field(0, t * S1, which="state")
+    om = 2 * np.pi * np.fft.fftfreq(n, d=1.0 / n) / (n * dt)
+    rho = math.sqrt(Rp) * np.exp(1j * delta) * np.exp(1j * (gdd / 2) * om ** 2) * np.exp(1j * (b2p / 2 * om ** 2) * L)
+    m1, m2 = 3, 4
+    assert o.roundtrips(m1) == 0
+    o.set_field(0, S2, which="input")
+    assert o.roundtrips(m2) == 0
+    a1 = t * np.fft.fft(S1) * (1 - rho ** (m1 + 1)) / (1 - rho)
+    expect = np.fft.ifft(rho ** m2 * a1 + t * np.fft.fft(S2) * (1 - rho ** m2) / (1 - rho))
+    assert rel_l2(o.get_field(0), expect) < 1e-12
+    # had the change reset the cavity to t S2 (an empty-cavity start), the result would differ at O(1)
+    wrong = np.fft.ifft(t * np.fft.fft(S2) * (1 - rho ** (m2 + 1)) / (1 - rho))
+    assert rel_l2(wrong, expect) > 0.1
+
+
 def test_p19_single_pass_pump_is_the_r_equals_zero_case_and_signal_gets_no_injection():
     """R_p = 0 with the pump flagged resonant gives exactly the single-pass rule A_p <- S_p (R11); the injection acts on
     the pump only: a resonant signal is not topped up from its seed."""
