@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """Writes the stored expected values of the config-length parity tests (tests/test_gpu_config_length.py).
 
-    python tests/golden/make_long_run_goldens.py [--only C1,C2,C3,C4] [--threads 8] [--no-float]
+    python tests/golden/make_long_run_goldens.py [--only C1,C2,C3,C3s,C3full,C4] [--threads 8] [--no-float]
 
 Calls ONLY oracle/ (the plain fp64 CPU implementation written from the paper) and opo_workloads (seeded inputs);
 nothing here touches the CUDA path.  Each file name carries a hash of the workload's inputs and parameters, so a
@@ -17,7 +17,9 @@ Files (numpy .npz, under tests/golden/):
   c4_300rt_sub16_<hash>.npz   (1 - R_s) mean|exit_s|^2 (R16), the pump depletion 1 - mean|exit_p|^2 / mean|S_p|^2, the
                               power spectrum |DFT(exit_s)|^2 (float32) -- from the fp64 oracle, and (pin P12, reported,
                               not asserted) the same three numbers' deviation when the oracle runs in `float`.
-Oracle cost (8 cores): C3 ~ 6 min, C1 ~ 10 + 10 min, C2 ~ 20 + 20 min, C4 ~ 6 + 6 min.
+  c3_200rt_<hash>.npz         C3 at its full length (200 round trips = 10^5 z-steps on N = 2^18), same three numbers + P12
+Oracle cost (8 cores): C3 ~ 6 min, C1 ~ 10 + 10 min, C2 ~ 20 + 20 min, C4 ~ 6 + 6 min; C3full ~ 70 min (one instance: the fp64
+and the float run take one core each, side by side).
 """
 from __future__ import annotations
 
@@ -27,6 +29,7 @@ import json
 import os
 import sys
 import time
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
@@ -78,7 +81,7 @@ def summarise(w, ex):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--only", default="C3,C3s,C4,C1,C2")
+    ap.add_argument("--only", default="C3,C3s,C4,C1,C2,C3full")
     ap.add_argument("--threads", type=int, default=os.cpu_count() or 1)
     ap.add_argument("--no-float", action="store_true", help="skip the float instantiation of the oracle (pin P12)")
     args = ap.parse_args()
@@ -106,6 +109,29 @@ def main():
             report["C3s"] = {"p12_float_vs_fp64_field_rel_l2_pump": fe[0], "p12_float_vs_fp64_field_rel_l2_signal": fe[1]}
         np.savez_compressed(os.path.join(HERE, name), **out)
         print(f"{name}: {time.time() - t0:.0f} s {json.dumps(report.get('C3s', {}))}", flush=True)
+    if "C3full" in only:
+        # BASELINE.json configs[3] at its own length: one instance, so the fp64 and the float run go side by side
+        w = W.config3()
+        name = f"c3_200rt_{workload_hash(w)}.npz"
+        t0 = time.time()
+        with ThreadPoolExecutor(max_workers=2) as pool:      # ctypes releases the GIL during the C call
+            f64 = pool.submit(oracle.run_workload, w, threads=1)
+            f32 = None if args.no_float else pool.submit(oracle.run_workload, w, threads=1, use_float=True)
+            res = f64.result()
+            resf = f32.result() if f32 else None
+        p_out, depl, spec = summarise(w, res["exit"])
+        out = {"p_out": p_out, "depletion": depl, "spectrum": spec.astype(np.float32), "n_roundtrips": w.n_roundtrips}
+        if resf is not None:
+            pf, df, sf = summarise(w, resf["exit"])
+            out["float_p_out"] = pf
+            out["float_depletion"] = df
+            out["float_spectrum_rel_l2"] = np.array([np.linalg.norm(sf[0] - spec[0]) / np.linalg.norm(spec[0])])
+            out["float_field_rel_l2"] = np.array([np.linalg.norm(resf["exit"][0, 1] - res["exit"][0, 1]) / np.linalg.norm(res["exit"][0, 1])])
+            report["C3"] = {"p12_float_vs_fp64_power_rel_err_max": float(np.max(np.abs(pf - p_out) / p_out)),
+                            "p12_float_vs_fp64_spectrum_rel_l2_max": float(out["float_spectrum_rel_l2"][0]),
+                            "p12_float_vs_fp64_field_rel_l2_max": float(out["float_field_rel_l2"][0])}
+        np.savez_compressed(os.path.join(HERE, name), **out)
+        print(f"{name}: {time.time() - t0:.0f} s; depletion {np.round(depl, 4).tolist()} {json.dumps(report.get('C3', {}))}", flush=True)
     for key, (stem, w) in long_run_workloads().items():
         if key not in only:
             continue

@@ -112,14 +112,18 @@ def test_config3_small_grid_20rt_against_the_float_oracle():
 
 # ---- full-length noise-seeded runs: output signal power and power spectrum -----------------------------------------------
 
-def _long_run(stem, w, engines):
+def _long_run(stem, w, engines, run_w=None, pick=None):
+    """w: the workload the golden was written for; run_w / pick: run a larger batch on the GPU and compare its instances
+    `pick` (seeds and sweep parameters are per instance, so instance pick[i] of run_w is instance i of w)."""
     torch, P = _gpu()
     g = golden(stem, w)
     assert int(g["n_roundtrips"]) == w.n_roundtrips
     R_s = w.R[1]
     out = {}
     for engine in engines:
-        ex, eng = run_gpu_exit(w, engine)
+        ex, eng = run_gpu_exit(w if run_w is None else run_w, engine)
+        if pick is not None:
+            ex = ex[np.asarray(pick)]
         p_out = (1.0 - R_s) * np.mean(np.abs(ex[:, 1]) ** 2, axis=1)
         p_in = np.array([np.mean(np.abs(w.pump_of(b)) ** 2) for b in range(w.batch)])
         depl = 1.0 - np.mean(np.abs(ex[:, 0]) ** 2, axis=1) / p_in
@@ -159,6 +163,33 @@ def test_config4_subset16_full_length_power_and_spectrum():
     res = _long_run("c4_300rt_sub16", w, [P.ENGINE_SOLO, P.ENGINE_RESIDENT])
     for e_p, e_s, e_d in res.values():
         assert e_p.max() <= 1e-3 and e_s.max() <= 1e-3
+
+
+def test_config4_bench_launch_full_length_against_the_subset_golden():
+    """The launch bench.py times -- all 256 instances x 300 round trips in one call: AUTO = the solo engine with the
+    (instance, round-trip) split schedule over 148 CTAs, and the cluster engine -- compared at the 16 golden instances (the 4
+    sweep corners + the diagonal)."""
+    from make_long_run_goldens import C4_SUBSET
+    torch, P = _gpu()
+    full = W.config4()
+    res = _long_run("c4_300rt_sub16", full.subset(C4_SUBSET), [P.ENGINE_AUTO, P.ENGINE_RESIDENT], run_w=full, pick=C4_SUBSET)
+    assert P.ENGINE_SOLO in res and P.ENGINE_RESIDENT in res
+    for e_p, e_s, e_d in res.values():
+        assert e_p.max() <= 1e-3 and e_s.max() <= 1e-3
+
+
+def test_config4_all_256_instances_20rt():
+    """every instance of the sweep for 20 round trips, field error <= 1e-4, in the launch configuration of the
+    bench (AUTO: solo engine, split schedule).  The oracle takes ~2 min on 16 host cores."""
+    import oracle
+    torch, P = _gpu()
+    w = W.config4().truncated(20)
+    ex, eng = run_gpu_exit(w)
+    assert eng == P.ENGINE_SOLO
+    ref = oracle.run_workload(w, threads=os.cpu_count() or 1)["exit"]
+    err = np.array([[rel_l2(ex[b, x], ref[b, x]) for x in range(w.n_fields)] for b in range(w.batch)])
+    print(f"C4, all 256 instances x 20 RT, engine {eng}: worst rel L2 {err.max():.3e} (instance {int(err.max(axis=1).argmax())}), median {np.median(err):.3e}")
+    assert err.max() <= 1e-4
 
 
 # ---- call granularity: the same run cut into many calls ----------------------------------------------------------------
