@@ -19,6 +19,7 @@ inside the timed region); `roofline` = the dominant kernel against the FP32 FMA 
 from __future__ import annotations
 
 import argparse
+import copy
 import json
 import os
 import statistics
@@ -94,6 +95,20 @@ def make_workload(name: str, rank: int):
     return w
 
 
+def replicate(w, batch: int, rank: int):
+    """A single-instance workload (C0, C1, C3) as a batch of `batch` independent OPOs: same pump, crystal and cavity, every
+    instance with its own seeded noise at the rms of the original seed (input scaling only, as in opo_workloads)."""
+    if w.batch != 1:
+        raise SystemExit(f"--batch replicates single-instance workloads; {w.name} already has {w.batch} instances")
+    w = copy.copy(w)
+    w.seeds = [None] + [W._round_to_precision(np.stack([W.complex_gaussian_noise(W.splitmix64(7000 + 10 * x + rank, b) % (1 << 31), w.n,
+                                                                                      float(np.sqrt(np.mean(np.abs(w.seeds[x][0]) ** 2))))
+                                                                  for b in range(batch)]), w.precision) for x in range(1, w.n_fields)]
+    w.batch = batch
+    w.name = f"{w.name} x {batch} instances"
+    return w
+
+
 def max_over_ranks(t_local: float, world: int, device="cuda") -> float:
     """Job time = the slowest rank's device time (no other collective exists on this path)."""
     import torch
@@ -154,6 +169,8 @@ def run_reference(args, rank, world):
     import oracle
     oracle.build()
     w = make_workload(args.workload, 0)
+    if args.batch:
+        w = replicate(w, args.batch, 0)
     cores = os.cpu_count() or 1
     inst = list(range(min(w.batch, cores)))
     # ~0.6 s per round trip per core at N = 2^14, nz = 100: one round trip per instance per step
@@ -216,6 +233,9 @@ def main():
     ap.add_argument("--train", action="store_true",
                     help="nanosecond regime (PAPER.md:L322-335): opo_roundtrips_train -- a pump slice per round trip in, the exit "
                          "signal of every round trip out; one launch per step on the solo engine (slices read and exit fields written at the crossings inside the kernel), one per round trip elsewhere; default 20 round trips per step")
+    ap.add_argument("--batch", type=int, default=0,
+                    help="run a single-instance workload (C0, C1, C3) as a batch of this many independent instances with their own noise "
+                         "seeds, e.g. --workload C0 --batch 2048: complex128 on every SM, roofline against the FP64 FMA pipe (SURVEY 8(d))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -245,6 +265,8 @@ def main():
         torch.cuda.synchronize()
 
     w = make_workload(args.workload, rank)
+    if args.batch:
+        w = replicate(w, args.batch, rank)
     if args.eom:
         w.eom_beta_rad = [0.0, 1.0, 0.0]
         w.eom_f_hz = [0.0, 3.0 / w.window_s, 0.0]

@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
         // by the split schedule applies two half-steps more per cut
         const int cuts = (a.split && rt0 > 0) ? (int)(((long long)b * a.steps + rt0) / quota - ((long long)b * a.steps) / quota) : 0;
         const int hq_base = a.hq0 + 2 * cuts;
-        const int fq_base = a.fq0 + (rt_mode ? rt0 * (nz - 1) : 0);
+        int fq = a.fq0 + (rt_mode ? rt0 * (nz - 1) : 0);       // full steps applied before the next one
         int* const flag = a.flags ? a.flags + (size_t)b * F + x : nullptr;
         cplx<T>* cur = reinterpret_cast<cplx<T>*>(a.cur[x]) + (size_t)b * N;
         const cplx<T>* ph = reinterpret_cast<const cplx<T>*>(a.phase) + (size_t)b * a.phase_stride;
@@ -400,7 +400,6 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                     linear_core_smem<T, L, NT>(tabH, tid);
                 }
             } else {
-                const int fq = fq_base + q - 1 - ((rt_mode && q > 0) ? (q - 1) / nz : 0);      // full steps applied before this one
                 const cplx<T>* tab = (q == 0 || q == total) ? tabH + (size_t)((hq_base + (q == 0 ? 0 : 1)) & a.tab_cycle_mask) * N
                                                             : (crossing ? tabHB : tabH2 + (size_t)(fq & a.tab_cycle_mask) * N);
                 if constexpr (FLOW) {
@@ -429,6 +428,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, res_layout<T, L, F>:
                 if constexpr (FLOW) { __syncthreads(); flow_arrive_ready_all(); }   // only now may the peers write into my field
             }
             if (q == total) break;
+            if (q > 0 && !crossing) ++fq;
             if constexpr (!FLOW) cluster_arrive();   // my field is ready for its inverse pass 0
             const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
             if constexpr (!FLOW) cluster_wait();     // ... and so is every other field

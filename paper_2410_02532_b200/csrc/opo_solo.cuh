@@ -333,7 +333,8 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
         const int cuts = (a.split && rt0 > 0) ? (int)(((long long)b * a.steps + rt0) / quota - ((long long)b * a.steps) / quota) : 0;
         const int op_base = a.op0 + (rt_mode ? rt0 * nz : 0) + cuts;
         const int hq_base = a.hq0 + 2 * cuts;
-        const int fq_base = a.fq0 + (rt_mode ? rt0 * (nz - 1) : 0);
+        int fq = a.fq0 + (rt_mode ? rt0 * (nz - 1) : 0);       // full steps applied before the next one (counted, not divided out:
+                                                               // the table address is on the critical path of every z-step)
 
         auto load = [&](const cplx<T>* __restrict__ g) {
 #pragma unroll 4
@@ -395,7 +396,6 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
         for (int q = 0; q <= total; ++q) {
             const int s = rt_mode ? q % nz : a.z0 + q;
             const bool crossing = rt_mode && q > 0 && q < total && s == 0;
-            const int fq = fq_base + q - 1 - ((rt_mode && q > 0) ? (q - 1) / nz : 0);      // full steps applied before this one
             const bool bunch = ((op_base + q) & (kConstBunch - 1)) == 0;
 #pragma unroll
             for (int x = 0; x < F; ++x) {
@@ -478,6 +478,7 @@ __global__ void __launch_bounds__(cta_threads<T, L>::value, solo_layout<T, L, F>
                 if (x < F - 1) {
                     swap_fields(x);
                 } else if (q < total) {
+                    if (q > 0 && !crossing) ++fq;
                     const cplx<T> e0 = ldg(ph + 2 * s), e1 = ldg(ph + 2 * s + 1), e2 = ldg(ph + 2 * s + 2);
                     fused(e0, e1, e2);
                 }

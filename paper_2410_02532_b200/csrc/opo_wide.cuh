@@ -426,6 +426,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F, G>::NTH, 1) k_wide(Reside
 
         // q counts linear operators: q = 0 first half-step, q = total last half-step, between them the merged full steps;
         // in round-trip mode q = m nz + s and s = 0 (m > 0) crosses the cavity boundary
+        int fq = a.fq0;                                         // full steps applied before the next one (ResidentArgs::fq0)
 #pragma unroll 1
         for (int q = 0; q <= total; ++q) {
             const int s = rt_mode ? q % nz : a.z0 + q;          // index of the RK4 step that follows
@@ -455,7 +456,6 @@ __global__ void __launch_bounds__(wide_layout<T, L, F, G>::NTH, 1) k_wide(Reside
                 for (int k = 0; k < 16; ++k) v[k] = g[tid_g + NT * k];
                 wide_push16<T, NW, NV, G, WL::MAXT, WL::NQ>(v, fb, wc, lane);
             } else {
-                const int fq = a.fq0 + q - 1 - ((rt_mode && q > 0) ? (q - 1) / nz : 0);        // full steps applied before this one
                 const cplx<T>* tab = (q == 0 || q == total) ? tabH + (size_t)((a.hq0 + (q == 0 ? 0 : 1)) & a.tab_cycle_mask) * N
                                                             : (crossing ? tabHB : tabH2 + (size_t)(fq & a.tab_cycle_mask) * N);
                 WideFlow fa = fb;
@@ -489,6 +489,7 @@ __global__ void __launch_bounds__(wide_layout<T, L, F, G>::NTH, 1) k_wide(Reside
                 }
             }
             if (q == total) break;
+            if (q > 0 && !crossing) ++fq;
             if (nt_own > 0) {
                 mbar_wait_cta(my_ready, fz & 1);                // the operands of my tiles are in my staging buffer
                 if (lane == 0) mbar_arm(my_ready, ready_bytes);
