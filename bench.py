@@ -62,25 +62,25 @@ def smem_bytes_per_field_point_zstep(precision: str) -> float:
     return 6 * 2 * (16 if precision == "c128" else 8)
 
 
-# The wide engine (one instance on a cluster of 4 F CTAs) is bound by the SM-to-SM link: every field value leaves its SM as an
-# operand of the pass-0 / RK4 phase and comes back as a result at every z-step.  Bytes through one
-# SM's port per z-step, sent and received, with G sub-blocks of a field per CTA (OPO_INFO_WIDE_SUBBLOCKS; NV = 4 F sub-blocks
-# on NV / G CTAs, and what stays inside a CTA does not cross the link): 2 directions x 2 crossings x esz x (N F G / NV) x
-# (NV - G) / NV.  Peak: 16 B/clk per SM, reads and writes together, measured in round 1
-# (profiles/r01d_dsmem_microbench.md) -- not re-measured in this run.
-def wide_link_roofline(w, o, P, units_per_step, avg_s, sm_ghz):
+# The wide engine (one instance on a cluster of 4 F CTAs) exchanges every field value over the SM-to-SM link twice per z-step: it
+# leaves its SM as an operand of the pass-0 / RK4 phase and comes back as a result.  Bytes one SM SENDS
+# per z-step with G sub-blocks of a field per CTA (OPO_INFO_WIDE_SUBBLOCKS; NV = 4 F sub-blocks on NV / G CTAs, and what stays
+# inside a CTA does not cross the link): 2 crossings x esz x (N F G / NV) x (NV - G) / NV; it receives as much.  Peak: bytes sent
+# per SM with every SM sending and receiving at once, measured in this run (opo_selftest_peak(OPO_PEAK_DSMEM)).  Until round 2
+# this line counted sent + received bytes against a round-1 constant of 16 B/clk.
+def wide_link_roofline(w, o, P, units_per_step, avg_s):
     esz = 16 if w.precision == "c128" else 8
     nv = 4 * w.n_fields
     slots = int(P.opo_get_info(o._h, P.INFO_SLOTS))
     waves = -(-w.batch // max(1, slots))
     g = max(1, int(P.opo_get_info(o._h, P.INFO_WIDE_SUBBLOCKS)))
-    per_sm_per_zstep = 2 * 2 * esz * (w.n * w.n_fields * g / nv) * (nv - g) / nv
+    sent_per_sm_per_zstep = 2 * esz * (w.n * w.n_fields * g / nv) * (nv - g) / nv
     zsteps_per_sm = units_per_step / (w.batch * w.n) * waves                        # z-steps an SM works through, wave after wave
-    achieved = per_sm_per_zstep * zsteps_per_sm / avg_s / 1e9
-    peak = 16.0 * sm_ghz
-    return {"achieved": achieved, "peak": peak, "unit": "GB/s per SM", "frac": achieved / peak,
-            "note": "SM-to-SM link traffic of one SM (operands out, results back, both directions); peak = 16 B/clk per SM at the max SM "
-                    "clock, measured in round 1 (profiles/r01d_dsmem_microbench.md); " + f"{g} sub-block(s) per CTA"}
+    achieved = sent_per_sm_per_zstep * zsteps_per_sm / avg_s / 1e9
+    peak = P.opo_selftest_peak(P.PEAK_DSMEM)
+    return {"achieved": achieved, "peak": peak, "unit": "GB/s sent per SM", "frac": achieved / peak,
+            "note": "SM-to-SM link: bytes one SM sends (operands out, results back; it receives as much); peak = 16-byte remote stores on "
+                    f"every co-resident cluster of 4, every SM sending and receiving at once, measured in this run; {g} sub-block(s) per CTA"}
 
 
 def make_workload(name: str, rank: int):
@@ -376,7 +376,7 @@ def main():
                     "smem": {"achieved": smem_by / avg_s / 1e9, "peak": smem_peak, "unit": "GB/s", "frac": smem_by / avg_s / 1e9 / smem_peak,
                              "note": f"algorithmic shared-memory bytes = {smem_bytes_per_field_point_zstep(w.precision):.0f} B per field-point z-step "
                                      "(6 passes x read + write); peak = conflict-free 16 B loads + stores on every SM, measured in this run"},
-                    **({"link": wide_link_roofline(w, o, P, units_per_step, avg_s, sm_max_ghz)} if eng == P.ENGINE_WIDE else {}),
+                    **({"link": wide_link_roofline(w, o, P, units_per_step, avg_s)} if eng == P.ENGINE_WIDE else {}),
                     "note": f"peak = {'FP64' if dbl else 'FP32'} FMA throughput measured in this run by opo_selftest_peak (independent FMA chains on every SM); "
                             f"peak_nominal = {sms} SM x {64 if dbl else 128} lanes x 2 x {sm_max_ghz:.3f} GHz; "
                             f"algorithmic flops = {flops_per_grid_point_zstep(w.log2_n, w.n_fields):.0f}/grid-point z-step "

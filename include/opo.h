@@ -268,12 +268,15 @@ int opo_get_info(const opo_handle* h, int what, long long* out);
 /* Device peaks measured on the spot with the library's own micro-benchmark kernels, the roofline denominators bench.py
  * reports against; independent of any handle, runs on the default stream of the current device
  * and takes ~0.1 s.  FP32 / FP64: independent FMA chains on every SM [TFLOP/s]; SMEM: conflict-free 16-byte shared-memory
- * loads + stores on every SM [GB/s]; TMEM_LD / TMEM_ST: tcgen05.ld / tcgen05.st of a thread's own columns [GB/s]. */
+ * loads + stores on every SM [GB/s]; TMEM_LD / TMEM_ST: tcgen05.ld / tcgen05.st of a thread's own columns [GB/s];
+ * DSMEM: 16-byte stores into the shared memory of the next CTA of a cluster of 4, all co-resident clusters at once:
+ * bytes SENT per SM [GB/s per SM]; every SM receives the same amount at the same time. */
 #define OPO_PEAK_FP32_FMA 0
 #define OPO_PEAK_FP64_FMA 1
 #define OPO_PEAK_SMEM 2
 #define OPO_PEAK_TMEM_LD 3
 #define OPO_PEAK_TMEM_ST 4
+#define OPO_PEAK_DSMEM 5
 int opo_selftest_peak(int what, double* out_value);
 
 /* Forward DFT of caller-owned rows WITHOUT a handle and without any device-memory allocation: the frequency read-out

@@ -224,7 +224,7 @@ def opo_set_option(h, option: int, value: int):
     _check(h, lib().opo_set_option(h, option, value))
 
 
-PEAK_FP32_FMA, PEAK_FP64_FMA, PEAK_SMEM, PEAK_TMEM_LD, PEAK_TMEM_ST = 0, 1, 2, 3, 4
+PEAK_FP32_FMA, PEAK_FP64_FMA, PEAK_SMEM, PEAK_TMEM_LD, PEAK_TMEM_ST, PEAK_DSMEM = 0, 1, 2, 3, 4, 5
 
 
 def opo_selftest_peak(what: int) -> float:

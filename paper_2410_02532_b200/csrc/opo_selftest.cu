@@ -5,7 +5,11 @@
 //   OPO_PEAK_FP64_FMA   : the same with DFMA                                                               -> TFLOP/s
 //   OPO_PEAK_SMEM       : conflict-free 16-byte shared-memory loads + stores, every SM                     -> GB/s
 //   OPO_PEAK_TMEM_LD/ST : tcgen05.ld / tcgen05.st 32x32b.x8 of a thread's own columns, every SM            -> GB/s
+//   OPO_PEAK_DSMEM      : 16-byte stores into the shared memory of the next CTA of a cluster of 4, on as many clusters as
+//                         are co-resident: bytes SENT per SM (every SM receives as much at the same time)   -> GB/s per SM
 #include <cstdint>
+#include <cstdio>
+#include <cstdlib>
 #include <cuda_runtime.h>
 
 #include "../../include/opo.h"
@@ -92,6 +96,30 @@ __global__ void __launch_bounds__(512, 1) k_peak_tmem(int iters, int store, floa
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base_s) : "memory");
 }
 
+// every CTA of a cluster streams into the shared memory of its successor (the traffic pattern of the wide engine's pushes,
+// opo_wide.cuh: every SM sends and receives at once)
+__global__ void __cluster_dims__(4, 1, 1) __launch_bounds__(512, 1) k_peak_dsmem(int iters, float* sink) {
+    extern __shared__ float4 sm4[];
+    const int tid = threadIdx.x;
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    for (int i = tid; i < 4096; i += 512) sm4[i] = make_float4((float)i, 1.f, 2.f, 3.f);
+    const uint32_t local = (uint32_t)__cvta_generic_to_shared(sm4) + 16u * tid;
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"((rank + 1u) & 3u));
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");   // every peer is resident
+    float4 v = make_float4((float)tid, 1.f, 2.f, 3.f);
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+            asm volatile("st.shared::cluster.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(remote + 8192u * r), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+        v.x += 1.f;
+    }
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");   // nobody exits while a peer still writes into it
+    if (sm4[tid].x == 123456.789f) sink[0] = sm4[tid].y;
+}
+
 template <class F> int timed(F&& launch, double* ms_out) {
     cudaEvent_t e0, e1;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return OPO_ERR_CUDA;
@@ -140,6 +168,22 @@ extern "C" int opo_selftest_peak(int what, double* out_value) {
         rc = timed([&] { k_peak_tmem<<<sms, 512>>>(iters, store, sink); }, &ms);
         const double bytes = 16.0 * 32.0 * 512.0 * (double)iters * (double)sms;        // 16 x (8 columns x 4 B) per thread and iteration
         *out_value = bytes / (ms * 1e-3) / 1e9;
+    } else if (what == OPO_PEAK_DSMEM) {
+        const int iters = 20000;
+        constexpr int kSmem = 120 * 1024;       // more than half of an SM's shared memory: one CTA per SM, so "per CTA" is "per SM"
+        if (cudaFuncSetAttribute(k_peak_dsmem, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem) != cudaSuccess) { cudaFree(sink); cudaGetLastError(); return OPO_ERR_CUDA; }
+        // as many clusters as run at once: a second wave would be timed as if it were part of the first
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(4 * (unsigned)sms, 1, 1);
+        cfg.blockDim = dim3(512, 1, 1);
+        cfg.dynamicSmemBytes = kSmem;
+        int clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&clusters, k_peak_dsmem, &cfg) != cudaSuccess || clusters <= 0) { cudaFree(sink); cudaGetLastError(); return OPO_ERR_CUDA; }
+        if (4 * clusters > sms) clusters = sms / 4;
+        rc = timed([&] { k_peak_dsmem<<<4 * clusters, 512, kSmem>>>(iters, sink); }, &ms);
+        if (getenv("OPO_SELFTEST_VERBOSE")) fprintf(stderr, "k_peak_dsmem: %d clusters of 4 on %d SMs, %.3f ms\n", clusters, sms, ms);
+        const double bytes_per_sm = 8.0 * 16.0 * 512.0 * (double)iters;                 // 8 stores of 16 B per thread and iteration
+        *out_value = bytes_per_sm / (ms * 1e-3) / 1e9;
     } else {
         rc = OPO_ERR_INVALID_ARG;
     }
