@@ -36,14 +36,15 @@
 // Pins (tests/test_oracle_*.py, -m "not gpu"): P1 naive DFT, P2 Gaussian GVD closed form, P3 GVM
 // integer shift, P4 cosh^2 gain (+dk), P5 degenerate phase-sensitive gain (paper's pi/4, -3pi/4,
 // PAPER.md:L400), P6 Manley-Rowe, P7 depleted SHG closed form, P8 2nd-order convergence, P9 cold
-// cavity, P10 threshold growth, P13 EOM sidebands = Bessel J_m(beta) (Jacobi-Anger) and element order,
+// cavity, P10 threshold growth, P11 steady-state pump depletion 4 (sqrt(N) - 1) / N, largest at the printed N = 4,
+// P13 EOM sidebands = Bessel J_m(beta) (Jacobi-Anger) and element order,
 // P14 third-order dispersion: centroid delay (beta3 z/2)(Omega_0^2 + s^2) of an offset Gaussian, P15 N/2-L-N/2 ordering:
 // second-order convergence, O(h^2) agreement with L/2-N-L/2, exact agreement when the operators commute,
 // P16 loss: power falls as exp(-alpha_x z), a pure scale (alpha/2 on the amplitude, Eq. 5), P17 pump re-injection: after
 // the boundary the pump is the stored input bit for bit and round trip 2 equals a hand-composed single pass (L268, R11),
 // P18 z restarts at the crystal entrance every pass with dk != 0 (R4): round trips = passes on fresh oracles,
 // P19 resonant pump: cold-cavity build-up to the closed-form Airy steady state sqrt(1-R) S / (1 - sqrt(R) e^{i delta} G e^{i D L})
-// per bin, geometric partial sums on the way, R_p = 0 equals the single-pass rule,
+// per bin, geometric partial sums on the way, R_p = 0 equals the single-pass rule, the input changed mid-run leaves the stored light alone,
 // P20 crystal segments: a crystal cut in two equal-parameter segments with dk = 0 equals the uncut crystal; with dk != 0 it
 // equals two single passes chained by hand; a second segment with d_eff -> -d_eff undoes the first one (dispersion off).
 // Parity unpinned: reading R12 (non-resonant fields restart from

@@ -207,6 +207,39 @@ def test_p5_degenerate_phase_sensitive_gain_matches_printed_phases():
 
 
 # ---------------------------------------------------------------------------------------------
+# P11 pump depletion against the pumping level N = P_p / P_th ("maximum pump depletion is
+#     achieved at N = 4").  A plane-wave degenerate CW oscillator, signal resonant with R_s = 0.98 (the value the
+#     paper prints), run to its steady state; in the low-loss limit the steady-state depletion of a single-pass
+#     pump is 4 (sqrt(N) - 1) / N, which is 1 at N = 4 and smaller on either side.  Pins the whole loop at once:
+#     coupling constants (R5's factor 1/2: with kappa_p not halved the maximum moves to another N), the mirror,
+#     the re-injection of the pump (R11) and the threshold scaling of the input generator.
+# ---------------------------------------------------------------------------------------------
+
+def test_p11_pump_depletion_is_largest_at_the_printed_pumping_level():
+    import opo_workloads as W
+    gv = golden()
+    L, nz, R = 5e-3, 10, gv["mirror_reflectivity_signal"]
+    ks = make(n_fields=2, log2_n=4, nz=nz, length=L, resonant=(0, 1), R=(0, R)).kappa(1)
+    a_th = W.threshold_amplitude_degenerate(ks, L, R)
+    levels = [3.0, 3.5, 4.0, 4.5, 5.0, 6.25]
+    depletion = []
+    for N in levels:
+        o = make(n_fields=2, log2_n=4, nz=nz, length=L, resonant=(0, 1), R=(0, R))
+        a_p = math.sqrt(N) * a_th
+        o.set_field(0, np.full(16, a_p, complex))
+        o.set_field(1, np.full(16, 1e-3 * a_p * np.exp(1j * np.pi * gv["degenerate_signal_phase_a_over_pi"]), complex))
+        assert o.roundtrips(2000) == 0
+        d1 = 1 - np.mean(np.abs(o.get_field(0, EXIT)) ** 2) / a_p ** 2
+        assert o.roundtrips(200) == 0
+        d2 = 1 - np.mean(np.abs(o.get_field(0, EXIT)) ** 2) / a_p ** 2
+        assert abs(d2 - d1) < 1e-5                       # steady state
+        assert abs(d2 - 4 * (math.sqrt(N) - 1) / N) < 2e-3
+        depletion.append(d2)
+    assert levels[int(np.argmax(depletion))] == gv["pump_depletion_max_at_pumping_level"]
+    assert max(depletion) > 0.9999
+
+
+# ---------------------------------------------------------------------------------------------
 # P6  Manley-Rowe and total energy through a lossless crystal (omega_p = omega_s + omega_i,
 #     PAPER.md:L80).  The linear half-steps are unitary, so the drift is RK4's: ~h^4.
 # ---------------------------------------------------------------------------------------------
